@@ -1,0 +1,854 @@
+// =====================================================================================
+// qmc_oracle.cpp -- CPU ORACLE.  TEST INFRASTRUCTURE ONLY.
+//
+// Plain, slow, obviously-correct FP64 implementation of the hot path of arXiv:1508.02512
+// ("Efficient Numerical Evaluation of Feynman Integrals", Li/Wang/Yan/Zhao): randomly
+// shifted rank-1 lattice QMC over sector-decomposed, eps-expanded Feynman-parameter
+// integrands, with contour deformation in the physical region.
+//
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+// may call this file.  It shares NO code with the CUDA product
+// (paper_1508_02512_b200/csrc): own graph polynomials, own decomposer, own evaluator.
+//
+// "P:<n>" = /root/reference/PAPER.md line n.  "R:<id>" = reading listed in DESIGN.md
+// (section "Readings of the paper").
+//
+// Steps:
+//   O1  U, F from spanning trees / 2-forests                  P:54   (R:C1,C3 sign of F)
+//   O2  primary sectors                                       P:58-78, Eqs. 3-6
+//   O3  iterated decomposition, deterministic rule            P:80-99, Eqs. 7-9 (R:C7)
+//   O4  lattice, shift, wrap, periodising transform           P:149,158,172-181, Eqs.17,18,21
+//   O5  contour deformation + Jacobian at each corner         P:127, Eq. 14 (R:C11,C12)
+//   O6  U^, F^ at the corner, G_Z, Lambda_Z                    P:94-97, Eq. 9
+//   O7  eps-coefficient c_k by the EXPLICIT double sum over   P:105-114, Eqs. 10-12
+//       S (pole variables) and R (subtracted variables)
+//   O8  S[sector][k][shift] = (1/N) sum_i w c_k  (Neumaier)   P:158, Eq. 18
+//   O9  mean, standard error over shifts                      P:161-170, Eqs. 19-20 (R:C15)
+//
+// Pins (tests/test_oracle_*.py, -m "not gpu"): closed forms (bubble, triangle, massless
+// box, double-box poles), the paper's Table 1, brute-force quadrature,
+// Kirchhoff matrix-tree counts, lattice exactness, tiling identity, invariants.
+// No function here is "parity unpinned" except the final VALUE of config 5 (no closed form
+// in the container; pinned by invariants only -- see DESIGN.md).
+// =====================================================================================
+#include <algorithm>
+#include <cmath>
+#include <complex>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <numeric>
+#include <string>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+typedef std::complex<double> cplx;
+typedef std::vector<int> Expo;
+typedef std::map<Expo, double> Poly;  // exponent vector -> coefficient (canonical order)
+
+const double kPi = 3.14159265358979323846264338327950288;
+
+// ------------------------------------------------------------------------------------
+// O1: graph polynomials ("constructed from the topology of the ... graph").
+//   U = sum over spanning trees T of prod_{e not in T} x_e
+//   F = - sum over spanning 2-forests (T1,T2) of (sum_{legs on T1} p)^2 prod_{e not in forest} x_e
+//       + U * sum_e m_e^2 x_e                         (then F -> F - i0; R:C3)
+// Sign fixed by BASELINE.json config 1: F = -p^2 x1 x2 + m^2 (x1+x2)^2.
+// ------------------------------------------------------------------------------------
+struct Graph {
+  int V = 0, P = 0, nlegs = 0;
+  std::vector<int> eu, ev, legv;
+  std::vector<double> m2, gram;  // gram[i*nlegs+j] = p_i . p_j, all legs incoming
+};
+
+int uf_find(std::vector<int>& par, int a) {
+  while (par[a] != a) a = par[a] = par[par[a]];
+  return a;
+}
+
+// true if the edge set `mask` is acyclic; comp[v] = component representative
+bool forest_components(const Graph& g, unsigned mask, std::vector<int>& comp, int& ncomp) {
+  std::vector<int> par(g.V);
+  std::iota(par.begin(), par.end(), 0);
+  for (int e = 0; e < g.P; ++e)
+    if (mask >> e & 1u) {
+      int a = uf_find(par, g.eu[e]), b = uf_find(par, g.ev[e]);
+      if (a == b) return false;  // cycle (also catches self-loops)
+      par[a] = b;
+    }
+  comp.resize(g.V);
+  ncomp = 0;
+  for (int v = 0; v < g.V; ++v) {
+    comp[v] = uf_find(par, v);
+    if (comp[v] == v) ++ncomp;
+  }
+  return true;
+}
+
+void poly_add(Poly& p, const Expo& e, double c) {
+  if (c == 0.0) return;
+  double& r = p[e];
+  r += c;
+  if (r == 0.0) p.erase(e);
+}
+
+Poly poly_mul(const Poly& a, const Poly& b) {
+  Poly r;
+  for (auto& x : a)
+    for (auto& y : b) {
+      Expo e(x.first.size());
+      for (size_t j = 0; j < e.size(); ++j) e[j] = x.first[j] + y.first[j];
+      poly_add(r, e, x.second * y.second);
+    }
+  return r;
+}
+
+int popcount(unsigned m) { return __builtin_popcount(m); }
+
+bool symanzik(const Graph& g, Poly& U, Poly& F, int& L) {
+  L = g.P - g.V + 1;
+  if (L < 1 || g.P > 16) return false;
+  U.clear();
+  F.clear();
+  std::vector<int> comp;
+  int ncomp;
+  Poly F0;
+  for (unsigned mask = 0; mask < (1u << g.P); ++mask) {
+    int k = popcount(mask);
+    if (k != g.V - 1 && k != g.V - 2) continue;
+    if (!forest_components(g, mask, comp, ncomp)) continue;
+    Expo e(g.P);
+    for (int j = 0; j < g.P; ++j) e[j] = (mask >> j & 1u) ? 0 : 1;
+    if (k == g.V - 1 && ncomp == 1) poly_add(U, e, 1.0);
+    if (k == g.V - 2 && ncomp == 2) {
+      // T1 := component containing vertex 0's complement choice is irrelevant by momentum
+      // conservation; take the component that does NOT contain vertex 0.
+      int c0 = comp[0];
+      double s = 0.0;
+      for (int a = 0; a < g.nlegs; ++a)
+        for (int b = 0; b < g.nlegs; ++b)
+          if (comp[g.legv[a]] != c0 && comp[g.legv[b]] != c0) s += g.gram[a * g.nlegs + b];
+      poly_add(F0, e, -s);
+    }
+  }
+  if (U.empty()) return false;  // disconnected
+  Poly M;
+  for (int j = 0; j < g.P; ++j) {
+    Expo e(g.P, 0);
+    e[j] = 1;
+    poly_add(M, e, g.m2[j]);
+  }
+  F = poly_mul(U, M);
+  for (auto& t : F0) poly_add(F, t.first, t.second);
+  return true;
+}
+
+// ------------------------------------------------------------------------------------
+// O2/O3: sectors.
+// ------------------------------------------------------------------------------------
+struct Sector {
+  int primary = 0;
+  std::vector<int> alpha, beta;  // t_j^{alpha_j + beta_j eps}
+  Poly U, F;                     // both with a non-zero constant term (Eqs. 7-8, constants kept inside; R:C6)
+  std::vector<int> sing, reg;    // sing: alpha == -1 ; reg: alpha >= 0
+  std::vector<int> jac;          // exponents of the accumulated Jacobian monomial alone (tiling pin)
+};
+
+struct Problem {
+  Graph g;
+  int L = 0, n = 0;
+  Poly U, F;
+  int aU0 = 0, aU1 = 0, aF0 = 0, aF1 = 0;  // U^{aU0+aU1 eps} F^{aF0+aF1 eps}, D = 4-2eps (Eq. 6)
+  double lambda = 0.0;
+  int kmax = 0, kmin = 0;
+  int max_depth = 64;
+  std::vector<Sector> sectors;
+  int status = 0;  // 0 ok, -2 depth, -3 unsupported
+};
+
+bool has_const(const Poly& p) {
+  if (p.empty()) return false;
+  const Expo& e = p.begin()->first;  // lexicographically smallest = all zeros if present
+  for (int x : e)
+    if (x) return false;
+  return true;
+}
+
+// step 1 of rule A.3: pull the common monomial out of Q, add its exponents to (alpha,beta)
+void factor_out(Poly& Q, int a0, int a1, std::vector<int>& alpha, std::vector<int>& beta) {
+  int n = (int)alpha.size();
+  for (int j = 0; j < n; ++j) {
+    int mn = 1 << 30;
+    for (auto& t : Q) mn = std::min(mn, t.first[j]);
+    if (mn <= 0) continue;
+    Poly R;
+    for (auto& t : Q) {
+      Expo e = t.first;
+      e[j] -= mn;
+      R[e] = t.second;
+    }
+    Q.swap(R);
+    alpha[j] += mn * a0;
+    beta[j] += mn * a1;
+  }
+}
+
+// step 3 of rule A.3: minimum-cardinality hitting set, lexicographically smallest tuple
+std::vector<int> hitting_set(const Poly& target, int n) {
+  for (int r = 1; r <= n; ++r) {
+    std::vector<int> idx(r);
+    std::iota(idx.begin(), idx.end(), 0);
+    while (true) {
+      bool ok = true;
+      for (auto& t : target) {
+        bool hit = false;
+        for (int j : idx)
+          if (t.first[j] > 0) {
+            hit = true;
+            break;
+          }
+        if (!hit) {
+          ok = false;
+          break;
+        }
+      }
+      if (ok) return idx;
+      int p = r - 1;  // next combination in lexicographic order
+      while (p >= 0 && idx[p] == n - r + p) --p;
+      if (p < 0) break;
+      ++idx[p];
+      for (int q = p + 1; q < r; ++q) idx[q] = idx[q - 1] + 1;
+    }
+  }
+  return {};
+}
+
+void decompose(Problem& pb, int primary, Poly U, Poly F, std::vector<int> alpha, std::vector<int> beta,
+               std::vector<int> jac, int depth) {
+  if (pb.status) return;
+  factor_out(U, pb.aU0, pb.aU1, alpha, beta);
+  factor_out(F, pb.aF0, pb.aF1, alpha, beta);
+  const Poly* target = nullptr;
+  if (!has_const(U))
+    target = &U;
+  else if (!has_const(F))
+    target = &F;
+  if (!target) {
+    Sector s;
+    s.primary = primary;
+    s.alpha = alpha;
+    s.beta = beta;
+    s.U = U;
+    s.F = F;
+    s.jac = jac;
+    for (int j = 0; j < pb.n; ++j) {
+      if (alpha[j] == -1) {
+        if (beta[j] == 0) pb.status = -3;
+        s.sing.push_back(j);
+      } else if (alpha[j] >= 0)
+        s.reg.push_back(j);
+      else
+        pb.status = -3;  // alpha <= -2 needs the p>=1 Taylor terms of Eq. 11 (R:C9)
+    }
+    pb.sectors.push_back(s);
+    return;
+  }
+  if (depth >= pb.max_depth) {
+    pb.status = -2;
+    return;
+  }
+  std::vector<int> S = hitting_set(*target, pb.n);
+  if (S.empty()) {
+    pb.status = -2;
+    return;
+  }
+  for (int k : S) {  // child k: t_j -> t_k t_j for j in S \ {k}
+    Poly U2, F2;
+    for (int which = 0; which < 2; ++which) {
+      const Poly& Q = which ? F : U;
+      Poly& R = which ? F2 : U2;
+      for (auto& t : Q) {
+        Expo e = t.first;
+        for (int j : S)
+          if (j != k) e[k] += t.first[j];
+        poly_add(R, e, t.second);
+      }
+    }
+    std::vector<int> a2 = alpha, b2 = beta, j2 = jac;
+    for (int j : S)
+      if (j != k) {
+        a2[k] += alpha[j];
+        b2[k] += beta[j];
+        j2[k] += jac[j];
+      }
+    a2[k] += (int)S.size() - 1;  // Jacobian t_k^{|S|-1}: a monomial, as P:90 requires
+    j2[k] += (int)S.size() - 1;
+    decompose(pb, primary, U2, F2, a2, b2, j2, depth + 1);
+  }
+}
+
+void build_sectors(Problem& pb) {
+  int P = pb.g.P;
+  pb.n = P - 1;
+  // exponents for nu_j = 1: a_U = P-(L+1)D/2, a_F = -(P-LD/2), D = 4-2eps
+  pb.aU0 = P - 2 * (pb.L + 1);
+  pb.aU1 = pb.L + 1;
+  pb.aF0 = -(P - 2 * pb.L);
+  pb.aF1 = -pb.L;
+  pb.sectors.clear();
+  for (int l = 0; l < P; ++l) {
+    // Eq. 4: x_l = 1 (after the delta integration), others renamed t_1..t_{P-1} in order
+    Poly Ul, Fl;
+    for (int which = 0; which < 2; ++which) {
+      const Poly& Q = which ? pb.F : pb.U;
+      Poly& R = which ? Fl : Ul;
+      for (auto& t : Q) {
+        Expo e;
+        for (int j = 0; j < P; ++j)
+          if (j != l) e.push_back(t.first[j]);
+        poly_add(R, e, t.second);
+      }
+    }
+    std::vector<int> zero(pb.n, 0);
+    decompose(pb, l, Ul, Fl, zero, zero, zero, 0);
+  }
+  int smax = 0;
+  for (auto& s : pb.sectors) smax = std::max(smax, (int)s.sing.size());
+  pb.kmin = -smax;
+}
+
+// ------------------------------------------------------------------------------------
+// O4: lattice point, shift, wrap, periodising transform (Eqs. 17, 18, 21).
+// ------------------------------------------------------------------------------------
+// returns false if some y_j == 0 or t_j == 0 (boundary point: contributes exactly 0; R:C18)
+bool lattice_point(uint64_t N, const uint64_t* z, int n, uint64_t i, const double* shift, int transform,
+                   double* y, double* t, double& w) {
+  bool inside = true;
+  w = 1.0;
+  for (int j = 0; j < n; ++j) {
+    // Eq. 17: u = {i z / N}; i*z_j < 2^64 is required (checked by the caller), remainder in integers
+    uint64_t r = (uint64_t)(((unsigned __int128)i * z[j]) % N);
+    double u = (double)r / (double)N;
+    double v = u + shift[j];  // Eq. 18
+    if (v >= 1.0) v -= 1.0;   // fractional part
+    y[j] = v;
+    if (transform == 0) {
+      t[j] = v * v * (3.0 - 2.0 * v);  // Eq. 21: x = 3y^2 - 2y^3
+      w *= 6.0 * v * (1.0 - v);
+    } else {
+      t[j] = 1.0 - std::fabs(2.0 * v - 1.0);  // tent / baker (R:C20), weight 1
+    }
+    if (!(v > 0.0) || !(t[j] > 0.0)) inside = false;
+  }
+  return inside;
+}
+
+// ------------------------------------------------------------------------------------
+// O5/O6: one corner.
+// ------------------------------------------------------------------------------------
+template <class T>
+T ipow(T x, int e) {  // e >= 0; x^0 = 1 also for x == 0
+  T r = T(1.0);
+  for (int k = 0; k < e; ++k) r *= x;
+  return r;
+}
+
+template <class T>
+T eval_poly(const Poly& Q, const std::vector<T>& x) {
+  T s = T(0.0);
+  for (auto& term : Q) {
+    T m = T(term.second);
+    for (size_t j = 0; j < x.size(); ++j) m *= ipow(x[j], term.first[j]);
+    s += m;
+  }
+  return s;
+}
+
+// d/dt_i and d2/dt_i dt_k of a real polynomial at a real point
+double eval_d1(const Poly& Q, const std::vector<double>& x, int i) {
+  double s = 0.0;
+  for (auto& term : Q) {
+    int ei = term.first[i];
+    if (ei == 0) continue;
+    double m = term.second * ei * ipow(x[i], ei - 1);
+    for (size_t j = 0; j < x.size(); ++j)
+      if ((int)j != i) m *= ipow(x[j], term.first[j]);
+    s += m;
+  }
+  return s;
+}
+double eval_d2(const Poly& Q, const std::vector<double>& x, int i, int k) {
+  double s = 0.0;
+  for (auto& term : Q) {
+    int ei = term.first[i], ek = term.first[k];
+    double m = term.second;
+    if (i == k) {
+      if (ei < 2) continue;
+      m *= ei * (ei - 1) * ipow(x[i], ei - 2);
+    } else {
+      if (ei < 1 || ek < 1) continue;
+      m *= ei * ipow(x[i], ei - 1) * ek * ipow(x[k], ek - 1);
+    }
+    for (size_t j = 0; j < x.size(); ++j)
+      if ((int)j != i && (int)j != k) m *= ipow(x[j], term.first[j]);
+    s += m;
+  }
+  return s;
+}
+
+// principal log; a negative real argument carries the -i0 of F -> F - i0 (R:C11): arg = -pi
+cplx log_m(cplx v) {
+  if (v.imag() == 0.0 && v.real() < 0.0) return cplx(std::log(-v.real()), -kPi);
+  return std::log(v);
+}
+double log_m(double v) { return std::log(v); }
+
+cplx det_gauss(std::vector<cplx> a, int n) {  // partial pivoting on |.|
+  cplx det = 1.0;
+  for (int c = 0; c < n; ++c) {
+    int p = c;
+    for (int r = c + 1; r < n; ++r)
+      if (std::abs(a[r * n + c]) > std::abs(a[p * n + c])) p = r;
+    if (a[p * n + c] == cplx(0.0)) return 0.0;
+    if (p != c) {
+      for (int k = 0; k < n; ++k) std::swap(a[p * n + k], a[c * n + k]);
+      det = -det;
+    }
+    det *= a[c * n + c];
+    for (int r = c + 1; r < n; ++r) {
+      cplx f = a[r * n + c] / a[c * n + c];
+      for (int k = c; k < n; ++k) a[r * n + k] -= f * a[c * n + k];
+    }
+  }
+  return det;
+}
+
+struct Counters {
+  int64_t imF_pos = 0, reU_nonpos = 0, nonfinite = 0, boundary = 0;
+};
+
+// real path (lambda == 0): G_Z, Lambda_Z of SURVEY App. A.4 (Eq. 9 integrand at the corner)
+void corner(const Problem& pb, const Sector& s, const std::vector<double>& tau, const double* t, const double* lnt,
+            double& G, double& Lam, Counters&) {
+  double Uv = eval_poly<double>(s.U, tau), Fv = eval_poly<double>(s.F, tau);
+  G = 1.0;
+  Lam = pb.aU1 * log_m(Uv) + pb.aF1 * log_m(Fv);
+  for (int j : s.reg) {
+    G *= ipow(t[j], s.alpha[j]);
+    Lam += s.beta[j] * lnt[j];
+  }
+  double pu = ipow(Uv, std::abs(pb.aU0)), pf = ipow(Fv, std::abs(pb.aF0));
+  G *= (pb.aU0 >= 0 ? pu : 1.0 / pu);
+  G *= (pb.aF0 >= 0 ? pf : 1.0 / pf);
+}
+
+// complex path (lambda > 0): Eq. 14 and its Jacobian (R:C12)
+void corner(const Problem& pb, const Sector& s, const std::vector<double>& tau, const double* t, const double* lnt,
+            cplx& G, cplx& Lam, Counters& cnt) {
+  int n = pb.n;
+  const cplx I(0.0, 1.0);
+  std::vector<double> F1(n);
+  std::vector<cplx> rho(n), zz(n), J(n * n);
+  for (int i = 0; i < n; ++i) F1[i] = eval_d1(s.F, tau, i);
+  for (int i = 0; i < n; ++i) {
+    rho[i] = 1.0 - I * pb.lambda * (1.0 - tau[i]) * F1[i];
+    zz[i] = tau[i] * rho[i];  // z_i = t_i - i lambda t_i (1-t_i) dF/dt_i
+    for (int k = 0; k < n; ++k) {
+      double F2 = eval_d2(s.F, tau, i, k);
+      cplx v = -I * pb.lambda * tau[i] * (1.0 - tau[i]) * F2;
+      if (i == k) v += 1.0 - I * pb.lambda * (1.0 - 2.0 * tau[i]) * F1[i];
+      J[i * n + k] = v;
+    }
+  }
+  cplx Uv = eval_poly<cplx>(s.U, zz), Fv = eval_poly<cplx>(s.F, zz);
+  if (Fv.imag() > 0.0) ++cnt.imF_pos;
+  if (!(Uv.real() > 0.0)) ++cnt.reU_nonpos;
+  G = det_gauss(J, n);
+  Lam = double(pb.aU1) * log_m(Uv) + double(pb.aF1) * log_m(Fv);
+  for (int j = 0; j < n; ++j) {
+    int a = s.alpha[j];
+    cplx p = ipow(rho[j], std::abs(a));
+    G *= (a >= 0 ? p : 1.0 / p);
+    Lam += double(s.beta[j]) * log_m(rho[j]);
+  }
+  for (int j : s.reg) {
+    G *= ipow(t[j], s.alpha[j]);
+    Lam += s.beta[j] * lnt[j];
+  }
+  cplx pu = ipow(Uv, std::abs(pb.aU0)), pf = ipow(Fv, std::abs(pb.aF0));
+  G *= (pb.aU0 >= 0 ? pu : 1.0 / pu);
+  G *= (pb.aF0 >= 0 ? pf : 1.0 / pf);
+}
+
+inline double re_of(double v) { return v; }
+inline double im_of(double) { return 0.0; }
+inline double re_of(cplx v) { return v.real(); }
+inline double im_of(cplx v) { return v.imag(); }
+inline double abs_of(double v) { return std::fabs(v); }
+inline double abs_of(cplx v) { return std::abs(v); }
+
+struct Neumaier {  // compensated sum (O8)
+  double s = 0.0, c = 0.0;
+  void add(double x) {
+    double t = s + x;
+    if (std::fabs(s) >= std::fabs(x))
+      c += (s - t) + x;
+    else
+      c += (x - t) + s;
+    s = t;
+  }
+  double value() const { return s + c; }
+};
+
+// O7: c_k(t) for k = -|sing| .. kmax by the explicit double sum (Eqs. 10-12):
+//  c_k = sum_{S subset sing} sum_{R subset sing\S} (-1)^|R| prod_{j in S} 1/beta_j prod_{j in sing\S} 1/t_j
+//        G_{S u R} (Lambda_{S u R} + sum_{j in sing\S} beta_j ln t_j)^{k+|S|} / (k+|S|)!
+// out[k - kmin_sector], absout = sum of |terms| (the un-cancelled magnitude of R:C19).
+template <class T>
+void sector_point(const Problem& pb, const Sector& s, const double* t, const double* lnt, std::vector<T>& out,
+                  std::vector<double>& absout, Counters& cnt) {
+  int ns = (int)s.sing.size(), nk = pb.kmax + ns + 1;
+  out.assign(nk, T(0.0));
+  absout.assign(nk, 0.0);
+  int nz = 1 << ns;
+  std::vector<T> G(nz), Lam(nz);
+  std::vector<double> tau(pb.n);
+  for (int Z = 0; Z < nz; ++Z) {
+    for (int j = 0; j < pb.n; ++j) tau[j] = t[j];
+    for (int b = 0; b < ns; ++b)
+      if (Z >> b & 1) tau[s.sing[b]] = 0.0;
+    corner(pb, s, tau, t, lnt, G[Z], Lam[Z], cnt);
+  }
+  for (int S = 0; S < nz; ++S) {
+    int cS = popcount((unsigned)S);
+    double pref = 1.0, lsum = 0.0;
+    for (int b = 0; b < ns; ++b) {
+      int j = s.sing[b];
+      if (S >> b & 1)
+        pref *= 1.0 / s.beta[j];
+      else {
+        pref *= 1.0 / t[j];
+        lsum += s.beta[j] * lnt[j];
+      }
+    }
+    int rest = (nz - 1) & ~S;
+    for (int R = rest;; R = (R - 1) & rest) {  // all subsets of sing \ S
+      double sign = (popcount((unsigned)R) & 1) ? -1.0 : 1.0;
+      int Z = S | R;
+      T base = Lam[Z] + lsum;
+      for (int k = -ns; k <= pb.kmax; ++k) {
+        int p = k + cS;
+        if (p < 0) continue;
+        T pw = ipow(base, p);
+        double fact = 1.0;
+        for (int q = 2; q <= p; ++q) fact *= q;
+        T term = sign * pref * G[Z] * pw / fact;
+        out[k + ns] += term;
+        absout[k + ns] += abs_of(term);
+      }
+      if (R == 0) break;
+    }
+  }
+}
+
+}  // namespace
+
+// =====================================================================================
+// C interface (ctypes).  All arrays caller-allocated.
+// =====================================================================================
+extern "C" {
+
+struct orc_problem {
+  Problem pb;
+};
+
+// graph + kinematics -> U, F, sectors.  Returns NULL on invalid graph.
+orc_problem* orc_build(int V, int P, int nlegs, const int* eu, const int* ev, const double* m2, const int* legv,
+                       const double* gram, double lambda, int kmax, int max_depth) {
+  orc_problem* h = new orc_problem;
+  Graph& g = h->pb.g;
+  g.V = V;
+  g.P = P;
+  g.nlegs = nlegs;
+  g.eu.assign(eu, eu + P);
+  g.ev.assign(ev, ev + P);
+  g.m2.assign(m2, m2 + P);
+  g.legv.assign(legv, legv + nlegs);
+  g.gram.assign(gram, gram + nlegs * nlegs);
+  h->pb.lambda = lambda;
+  h->pb.kmax = kmax;
+  h->pb.max_depth = max_depth > 0 ? max_depth : 64;
+  if (!symanzik(g, h->pb.U, h->pb.F, h->pb.L)) {
+    delete h;
+    return nullptr;
+  }
+  build_sectors(h->pb);
+  return h;
+}
+
+// A problem defined by explicit sector tables (used to evaluate tables exported by the product
+// library: DATA crosses, code does not).  Flat layout documented in include/qmc_feynman.h.
+orc_problem* orc_from_tables(const int64_t* w, size_t nwords) {
+  if (nwords < 12) return nullptr;
+  const double* d = reinterpret_cast<const double*>(w);
+  if (w[0] != 0x514D4346 /* 'QMCF' */) return nullptr;
+  orc_problem* h = new orc_problem;
+  Problem& pb = h->pb;
+  int nsec = (int)w[2];
+  pb.n = (int)w[3];
+  pb.kmin = (int)w[4];
+  pb.kmax = (int)w[5];
+  pb.aU0 = (int)w[7];
+  pb.aU1 = (int)w[8];
+  pb.aF0 = (int)w[9];
+  pb.aF1 = (int)w[10];
+  pb.lambda = d[11];
+  size_t p = 12;
+  for (int s = 0; s < nsec; ++s) {
+    Sector sc;
+    sc.primary = (int)w[p++];
+    for (int j = 0; j < pb.n; ++j) sc.alpha.push_back((int)w[p++]);
+    for (int j = 0; j < pb.n; ++j) sc.beta.push_back((int)w[p++]);
+    int nU = (int)w[p++], nF = (int)w[p++];
+    for (int which = 0; which < 2; ++which)
+      for (int m = 0; m < (which ? nF : nU); ++m) {
+        double c = d[p++];
+        Expo e;
+        for (int j = 0; j < pb.n; ++j) e.push_back((int)w[p++]);
+        poly_add(which ? sc.F : sc.U, e, c);
+      }
+    sc.jac.assign(pb.n, 0);
+    for (int j = 0; j < pb.n; ++j) {
+      if (sc.alpha[j] == -1)
+        sc.sing.push_back(j);
+      else
+        sc.reg.push_back(j);
+    }
+    pb.sectors.push_back(sc);
+    if (p > nwords) {
+      delete h;
+      return nullptr;
+    }
+  }
+  return h;
+}
+
+void orc_free(orc_problem* h) { delete h; }
+
+// info[0..10] = status, L, n, n_sectors, kmin, kmax, aU0, aU1, aF0, aF1, n_terms_U ; info[11] = n_terms_F
+void orc_info(const orc_problem* h, int* info) {
+  const Problem& pb = h->pb;
+  int v[12] = {pb.status, pb.L,  pb.n,   (int)pb.sectors.size(), pb.kmin,        pb.kmax,
+               pb.aU0,    pb.aU1, pb.aF0, pb.aF1,                 (int)pb.U.size(), (int)pb.F.size()};
+  std::memcpy(info, v, sizeof v);
+}
+
+// which: 0 = U, 1 = F of the graph (P variables); coeff[nterms], expo[nterms*P]
+void orc_graph_poly(const orc_problem* h, int which, double* coeff, int* expo) {
+  const Poly& Q = which ? h->pb.F : h->pb.U;
+  size_t k = 0;
+  for (auto& t : Q) {
+    coeff[k] = t.second;
+    for (int j = 0; j < h->pb.g.P; ++j) expo[k * h->pb.g.P + j] = t.first[j];
+    ++k;
+  }
+}
+
+// sector data: meta[0..3] = primary, nU, nF, n_sing ; alpha[n], beta[n], jac[n]
+void orc_sector_meta(const orc_problem* h, int s, int* meta, int* alpha, int* beta, int* jac) {
+  const Sector& sc = h->pb.sectors[s];
+  meta[0] = sc.primary;
+  meta[1] = (int)sc.U.size();
+  meta[2] = (int)sc.F.size();
+  meta[3] = (int)sc.sing.size();
+  for (int j = 0; j < h->pb.n; ++j) {
+    alpha[j] = sc.alpha[j];
+    beta[j] = sc.beta[j];
+    jac[j] = sc.jac[j];
+  }
+}
+void orc_sector_poly(const orc_problem* h, int s, int which, double* coeff, int* expo) {
+  const Poly& Q = which ? h->pb.sectors[s].F : h->pb.sectors[s].U;
+  size_t k = 0;
+  for (auto& t : Q) {
+    coeff[k] = t.second;
+    for (int j = 0; j < h->pb.n; ++j) expo[k * h->pb.n + j] = t.first[j];
+    ++k;
+  }
+}
+
+// O4 exposed for the lattice/transform pins: count points starting at index i0 (step 1)
+// y,t: [count][n], w: [count], inside: [count]
+void orc_lattice(uint64_t N, const uint64_t* z, int n, uint64_t i0, uint64_t count, const double* shift,
+                 int transform, double* y, double* t, double* w, int* inside) {
+  for (uint64_t c = 0; c < count; ++c)
+    inside[c] = lattice_point(N, z, n, i0 + c, shift, transform, y + c * n, t + c * n, w[c]) ? 1 : 0;
+}
+
+// O5 exposed for the deformation pins: z(t), det J at a real point of sector s (lambda from the problem)
+void orc_deform(const orc_problem* h, int s, const double* tpt, double* z_re_im, double* det_re_im) {
+  const Problem& pb = h->pb;
+  const Sector& sc = pb.sectors[s];
+  int n = pb.n;
+  const cplx I(0.0, 1.0);
+  std::vector<double> tau(tpt, tpt + n), F1(n);
+  std::vector<cplx> J(n * n);
+  for (int i = 0; i < n; ++i) F1[i] = eval_d1(sc.F, tau, i);
+  for (int i = 0; i < n; ++i) {
+    cplx zi = tau[i] - I * pb.lambda * tau[i] * (1.0 - tau[i]) * F1[i];
+    z_re_im[2 * i] = zi.real();
+    z_re_im[2 * i + 1] = zi.imag();
+    for (int k = 0; k < n; ++k) {
+      cplx v = -I * pb.lambda * tau[i] * (1.0 - tau[i]) * eval_d2(sc.F, tau, i, k);
+      if (i == k) v += 1.0 - I * pb.lambda * (1.0 - 2.0 * tau[i]) * F1[i];
+      J[i * n + k] = v;
+    }
+  }
+  cplx d = det_gauss(J, n);
+  det_re_im[0] = d.real();
+  det_re_im[1] = d.imag();
+}
+
+// the eps-coefficients c_k(t) of sector s at ONE real point t in (0,1)^n  (no lattice, no weight):
+// used by the brute-force quadrature pins.  out[(kmax-kmin_s+1)*2] (Re,Im), orders -n_sing..kmax
+void orc_sector_integrand(const orc_problem* h, int s, const double* tpt, double* out) {
+  const Problem& pb = h->pb;
+  const Sector& sc = pb.sectors[s];
+  std::vector<double> lnt(pb.n), absout;
+  for (int j = 0; j < pb.n; ++j) lnt[j] = std::log(tpt[j]);
+  Counters cnt;
+  if (pb.lambda > 0.0) {
+    std::vector<cplx> o;
+    sector_point<cplx>(pb, sc, tpt, lnt.data(), o, absout, cnt);
+    for (size_t k = 0; k < o.size(); ++k) {
+      out[2 * k] = o[k].real();
+      out[2 * k + 1] = o[k].imag();
+    }
+  } else {
+    std::vector<double> o;
+    sector_point<double>(pb, sc, tpt, lnt.data(), o, absout, cnt);
+    for (size_t k = 0; k < o.size(); ++k) {
+      out[2 * k] = o[k];
+      out[2 * k + 1] = 0.0;
+    }
+  }
+}
+
+// O8: S[sector][k-kmin][shift][2] and A[sector][k-kmin][shift] over the lattice indices
+// i = i_begin + c*i_step, c < i_count (full rule: 0,1,N); always normalised by 1/N (Eq. 18).
+// Sectors [sec_begin, sec_end).  Deterministic for any thread count: each (sector, shift) pair is
+// one serial Neumaier sum over i in increasing order.
+// counters[4] = #corner evaluations with Im F(z) > 0, Re U(z) <= 0, #non-finite points, #boundary points
+int orc_integrate(const orc_problem* h, uint64_t N, const uint64_t* z, int m, const double* shifts, int transform,
+                  uint64_t i_begin, uint64_t i_step, uint64_t i_count, int sec_begin, int sec_end, int nthreads,
+                  double* S, double* A, int64_t* counters) {
+  const Problem& pb = h->pb;
+  if (pb.status) return pb.status;
+  int n = pb.n, K = pb.kmax - pb.kmin + 1;
+  for (int j = 0; j < n; ++j) {
+    if (z[j] == 0 || z[j] >= N || std::gcd(z[j], N) != 1) return -1;  // coprime to n
+  }
+  if (N >= (1ull << 32)) return -1;
+  int nsec = sec_end - sec_begin;
+  std::fill(S, S + (size_t)nsec * K * m * 2, 0.0);
+  if (A) std::fill(A, A + (size_t)nsec * K * m, 0.0);
+  Counters total;
+  bool cx = pb.lambda > 0.0;
+#ifdef _OPENMP
+  if (nthreads > 0) omp_set_num_threads(nthreads);
+#endif
+#pragma omp parallel
+  {
+    Counters cnt;
+    std::vector<double> y(n), t(n), lnt(n), absout;
+    std::vector<cplx> oc;
+    std::vector<double> od;
+#pragma omp for collapse(2) schedule(dynamic, 1)
+    for (int si = 0; si < nsec; ++si)
+      for (int kap = 0; kap < m; ++kap) {
+        const Sector& sc = pb.sectors[sec_begin + si];
+        int ns = (int)sc.sing.size(), off = -ns - pb.kmin;  // order k sits at index k - kmin
+        std::vector<Neumaier> accRe(K), accIm(K), accA(K);
+        for (uint64_t c = 0; c < i_count; ++c) {
+          uint64_t i = i_begin + c * i_step;
+          double w;
+          if (!lattice_point(N, z, n, i, shifts + (size_t)kap * n, transform, y.data(), t.data(), w)) {
+            if (si == 0) ++cnt.boundary;
+            continue;
+          }
+          for (int j = 0; j < n; ++j) lnt[j] = std::log(t[j]);
+          bool finite = true;
+          if (cx) {
+            sector_point<cplx>(pb, sc, t.data(), lnt.data(), oc, absout, cnt);
+            for (auto& v : oc) finite = finite && std::isfinite(v.real()) && std::isfinite(v.imag());
+            if (finite)
+              for (size_t k = 0; k < oc.size(); ++k) {
+                accRe[off + k].add(w * oc[k].real());
+                accIm[off + k].add(w * oc[k].imag());
+                accA[off + k].add(w * absout[k]);
+              }
+          } else {
+            sector_point<double>(pb, sc, t.data(), lnt.data(), od, absout, cnt);
+            for (auto& v : od) finite = finite && std::isfinite(v);
+            if (finite)
+              for (size_t k = 0; k < od.size(); ++k) {
+                accRe[off + k].add(w * od[k]);
+                accA[off + k].add(w * absout[k]);
+              }
+          }
+          if (!finite) ++cnt.nonfinite;
+        }
+        for (int k = 0; k < K; ++k) {
+          size_t o = ((size_t)si * K + k) * m + kap;
+          S[2 * o] = accRe[k].value() / (double)N;
+          S[2 * o + 1] = accIm[k].value() / (double)N;
+          if (A) A[o] = accA[k].value() / (double)N;
+        }
+      }
+#pragma omp critical
+    {
+      total.imF_pos += cnt.imF_pos;
+      total.reU_nonpos += cnt.reU_nonpos;
+      total.nonfinite += cnt.nonfinite;
+      total.boundary += cnt.boundary;
+    }
+  }
+  if (counters) {
+    counters[0] = total.imF_pos;
+    counters[1] = total.reU_nonpos;
+    counters[2] = total.nonfinite;
+    counters[3] = total.boundary;
+  }
+  return 0;
+}
+
+// O9: Eqs. 19-20 on per-shift values.  T[K][m][2] -> mean[K][2], err[K][2] (sqrt of Eq. 20; Re, Im separately)
+void orc_statistics(const double* T, int K, int m, double* mean, double* err) {
+  for (int k = 0; k < K; ++k)
+    for (int c = 0; c < 2; ++c) {
+      double s = 0.0;
+      for (int kap = 0; kap < m; ++kap) s += T[((size_t)k * m + kap) * 2 + c];
+      double q = s / m, v = 0.0;
+      for (int kap = 0; kap < m; ++kap) {
+        double d = T[((size_t)k * m + kap) * 2 + c] - q;
+        v += d * d;
+      }
+      mean[2 * k + c] = q;
+      err[2 * k + c] = std::sqrt(v / ((double)m * (m - 1)));
+    }
+}
+
+int orc_max_threads() {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+}  // extern "C"
