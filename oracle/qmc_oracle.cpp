@@ -126,13 +126,21 @@ bool symanzik(const Graph& g, Poly& U, Poly& F, int& L) {
     for (int j = 0; j < g.P; ++j) e[j] = (mask >> j & 1u) ? 0 : 1;
     if (k == g.V - 1 && ncomp == 1) poly_add(U, e, 1.0);
     if (k == g.V - 2 && ncomp == 2) {
-      // T1 := component containing vertex 0's complement choice is irrelevant by momentum
-      // conservation; take the component that does NOT contain vertex 0.
-      int c0 = comp[0];
-      double s = 0.0;
+      // (sum_{legs on T1} p)^2 = (sum_{legs on T2} p)^2 by momentum conservation; evaluate it on the side
+      // with FEWER legs (tie: the side without leg 0) so that on-shell zeros stay exact, and snap
+      // rounding residues of the Gram matrix to an exact 0 (R:C24) -- a spurious 1e-16 coefficient
+      // would fake a constant term in F^ and stop the decomposition too early.
+      int c0 = comp[g.legv.empty() ? 0 : g.legv[0]], n0 = 0;
+      for (int a = 0; a < g.nlegs; ++a) n0 += (comp[g.legv[a]] == c0);
+      bool use_other = (2 * n0 >= g.nlegs);  // side without leg 0 unless it has more legs
+      double s = 0.0, scale = 0.0;
       for (int a = 0; a < g.nlegs; ++a)
-        for (int b = 0; b < g.nlegs; ++b)
-          if (comp[g.legv[a]] != c0 && comp[g.legv[b]] != c0) s += g.gram[a * g.nlegs + b];
+        for (int b = 0; b < g.nlegs; ++b) {
+          scale = std::max(scale, std::fabs(g.gram[a * g.nlegs + b]));
+          bool ina = (comp[g.legv[a]] == c0) != use_other, inb = (comp[g.legv[b]] == c0) != use_other;
+          if (ina && inb) s += g.gram[a * g.nlegs + b];
+        }
+      if (std::fabs(s) <= 1e-12 * scale) s = 0.0;
       poly_add(F0, e, -s);
     }
   }
