@@ -1,0 +1,151 @@
+/* =======================================================================================
+ * qmc_feynman.h -- C ABI of the B200-native hot path of arXiv:1508.02512
+ * ("Efficient Numerical Evaluation of Feynman Integrals", Li, Wang, Yan, Zhao):
+ * randomly shifted rank-1 lattice quasi-Monte Carlo integration of sector-decomposed,
+ * eps-expanded Feynman-parameter integrands, with contour deformation in the physical region.
+ *
+ * "P:<n>" cites /root/reference/PAPER.md line n; "R:Cxx" cites a reading listed in DESIGN.md.
+ *
+ * Two calls carry the path (BASELINE.json north_star):
+ *   qmc_prepare  (graph, kinematics, eps_order) -> sector tables          [host only]
+ *   qmc_integrate(sector tables, N, m, seed)    -> Laurent coefficients +- errors   [CUDA, sm_100a]
+ *
+ * Conventions
+ *  - Every function returns 0 (QMC_OK) or a negative qmc_status; nothing throws, aborts or prints.
+ *  - All pointers are HOST pointers unless the name says `dev_`.  Inputs are borrowed for the duration
+ *    of the call.  `qmc_tables` is created by qmc_prepare and destroyed by qmc_tables_free.  Outputs go
+ *    to caller-allocated buffers (NULL = not wanted).
+ *  - Device memory is owned by the caller: `dev_workspace` is any device allocation of at least
+ *    qmc_workspace_bytes() bytes (e.g. a torch tensor's data_ptr()), `cuda_stream` is a cudaStream_t
+ *    (e.g. torch.cuda.current_stream().cuda_stream; NULL = default stream).  The library never
+ *    allocates device memory; it synchronises only its own stream before filling host outputs.
+ *  - There is NO CPU fallback: without a CUDA device qmc_integrate* returns QMC_ECUDA.
+ *
+ * What is computed.  For a graph with P propagators (powers nu_j = 1), L loops, D = 4 - 2 eps:
+ *     I = (-1)^P Gamma(P - L D/2) J(eps),   J(eps) = sum_{l=1..P} I_l         (Eqs. 5-6; R:C1)
+ *  where I_l are the primary-sector integrals over the (P-1)-cube.  The library returns the Laurent
+ *  coefficients of J(eps) (orders k_min .. k_max = eps_order); the Gamma prefactor and any normalisation
+ *  (R:C2-C4) are applied by the caller (qmc_prefactor_series helps).
+ * ======================================================================================= */
+#ifndef QMC_FEYNMAN_H
+#define QMC_FEYNMAN_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  QMC_OK = 0,
+  QMC_EINVAL = -1,       /* bad graph (disconnected, leg on a missing vertex, L < 1, P > 9), bad N/z/m */
+  QMC_EDEPTH = -2,       /* iterated decomposition did not terminate within max_depth (R:C7) */
+  QMC_EUNSUPPORTED = -3, /* alpha_j <= -2 (needs the p >= 1 Taylor terms of Eq. 11; R:C9), beta_j = 0 on a
+                            singular variable, more than 4 singular variables in one sector, nu_j != 1 */
+  QMC_ECUDA = -4,        /* CUDA runtime error or no device */
+  QMC_ENOMEM = -5,       /* workspace / export buffer too small */
+  QMC_ECONTOUR = -6      /* reserved: contour problems are REPORTED through counters, never fatal */
+} qmc_status;
+
+/* ---- inputs (an integral is a graph, masses, propagator powers and external kinematics) ---- */
+typedef struct {
+  int32_t n_vertices, n_edges, n_legs;
+  const int32_t *edge_u, *edge_v; /* [n_edges] end points; multi-edges allowed (bubble) */
+  const double *edge_m2;          /* [n_edges] squared internal masses */
+  const int32_t *edge_nu;         /* [n_edges] propagator powers; NULL = all 1 (anything else: QMC_EUNSUPPORTED) */
+  const int32_t *leg_vertex;      /* [n_legs] vertex each external leg (all incoming) attaches to */
+} qmc_graph;
+
+typedef struct {
+  const double *gram; /* [n_legs*n_legs] p_i . p_j, momentum conservation assumed */
+} qmc_kinematics;
+
+typedef struct {
+  double lambda;     /* 0: Euclidean / real path.  > 0: contour deformation z_j = t_j - i lambda t_j (1-t_j) dF/dt_j
+                        (Eq. 14), complex path, all variables deformed with the same lambda (R:C11) */
+  int32_t transform; /* 0: x = 3y^2 - 2y^3, weight prod 6y(1-y) (Eq. 21).  1: tent/baker (R:C20) */
+  int32_t max_depth; /* decomposition recursion cap; <= 0: 64 */
+} qmc_options;
+
+typedef struct qmc_tables qmc_tables; /* opaque sector tables (Eqs. 7-9) */
+
+/* Feynman graph -> U, F -> P primary sectors (Eqs. 3-6) -> iterated sub-sectors until U^ and F^
+ * both have a constant term (Eqs. 7-9; deterministic rule R:C7) -> per-sector tables: exponents
+ * (alpha_j, beta_j) of t_j^{alpha_j + beta_j eps} and the monomial lists of U^, F^ (constants kept inside, R:C6).
+ * eps_order = highest order of J(eps) wanted.  options may be NULL (lambda 0, transform 0, depth 64). */
+int qmc_prepare(const qmc_graph *graph, const qmc_kinematics *kin, int32_t eps_order, const qmc_options *options,
+                qmc_tables **out);
+void qmc_tables_free(qmc_tables *t);
+
+/* orders k_min = -max_sector(#singular variables) .. k_max = eps_order; K = k_max - k_min + 1 */
+int qmc_tables_info(const qmc_tables *t, int32_t *n_sectors, int32_t *dim, int32_t *k_min, int32_t *k_max,
+                    int32_t *is_complex);
+
+/* Flat export of the tables so that an independent program can evaluate the SAME sectors (data, not code).
+ * Layout: 8-byte words w[] (int64 unless noted):
+ *   w[0]=0x514D4346 ('QMCF'), w[1]=version 1, w[2]=n_sectors, w[3]=dim n, w[4]=k_min, w[5]=k_max, w[6]=is_complex,
+ *   w[7..10]=a_U0,a_U1,a_F0,a_F1 with U^{a_U0+a_U1 eps} F^{a_F0+a_F1 eps}, w[11]=lambda (double);
+ *   then per sector: primary index, alpha[n], beta[n], nU, nF, nU x {coeff (double), e[n]}, nF x {coeff (double), e[n]}
+ *   (variables in the ORIGINAL order t_1..t_n of Eq. 4, monomials in the library's evaluation order).
+ * Call with buf = NULL to get the size in bytes in *len; otherwise *len is the capacity on entry. */
+int qmc_tables_export(const qmc_tables *t, void *buf, size_t *len);
+
+/* ---- outputs ---- */
+typedef struct {
+  double *coeff, *err;               /* [K][2] totals over sectors: mean over shifts (Eq. 19) and the square root
+                                        of Eq. 20, (Re, Im) separately (R:C15) */
+  double *sector_coeff, *sector_err; /* [n_sectors][K][2] the same per sector */
+  double *shift_totals;              /* [K][m][2] per-shift estimates Q_k summed over sectors (Eq. 18) */
+  double *shift_sums;                /* [n_sectors][K][m][2] per-sector per-shift estimates (parity checks) */
+  int64_t counters[4];               /* #corner evaluations with Im F^(z) > 0, with Re U^(z) <= 0,
+                                        #non-finite (point, sector) evaluations (dropped), #boundary points (R:C18) */
+  double kernel_ms;                  /* device time of the evaluation + reduction kernels (CUDA events) */
+  int32_t kernel_launches;           /* number of kernel launches made by this call */
+  int32_t mode_used;                 /* 1 fused (all sectors summed in registers), 2 per-sector */
+} qmc_result;
+
+/* Explicit control of one integration (the parity entry point). */
+typedef struct {
+  const uint64_t *z;        /* [dim] generating vector, components coprime to N; NULL: library's choice (R:C13) */
+  const double *shifts;     /* [m][dim] shift vectors in [0,1); NULL: SplitMix64 stream of `seed` (R:C14) */
+  uint64_t index_begin, index_step, index_count; /* lattice indices i = begin + c*step, c < count; count 0 = all N.
+                                                    The sum is always normalised by 1/N (Eq. 18). */
+  int32_t sector_begin, sector_end;              /* sector range; end 0 = all */
+  int32_t mode;             /* 0 auto (per-sector iff a per-sector output is requested), 1 fused, 2 per-sector */
+  int32_t tables_resident;  /* 1: reuse the table image already uploaded to this workspace by an earlier call */
+} qmc_run;
+
+size_t qmc_workspace_bytes(const qmc_tables *t, uint64_t N, int32_t m);
+
+/* S1-S8 of the hot path: lattice points x_i = {i z / N} (Eq. 17), m random shifts (Eq. 18),
+ * periodising transform (Eq. 21), per sector the subtracted (Eqs. 10-12), eps-expanded and -- for
+ * lambda > 0 -- contour-deformed (Eq. 14) integrand at every point, per-shift sums, mean and error over shifts
+ * (Eqs. 19-20).  N must be < 2^31 with every z_j coprime to it, m >= 2. */
+int qmc_integrate(const qmc_tables *t, uint64_t N, int32_t m, uint64_t seed, void *cuda_stream, void *dev_workspace,
+                  size_t dev_workspace_bytes, qmc_result *out);
+int qmc_integrate_ex(const qmc_tables *t, uint64_t N, int32_t m, uint64_t seed, const qmc_run *run, void *cuda_stream,
+                     void *dev_workspace, size_t dev_workspace_bytes, qmc_result *out);
+
+/* ---- helpers ---- */
+/* Korobov-form generating vector z = (1, a, a^2, ...) mod N with `a` minimising the P_2 figure of merit over a fixed
+ * deterministic candidate list (R:C13; "component-by-component" is the paper's own choice).  Runs on the
+ * device (needs workspace of qmc_workspace_bytes). */
+int qmc_generating_vector(uint64_t N, int32_t dim, void *cuda_stream, void *dev_workspace, size_t dev_workspace_bytes,
+                          uint64_t *z_out);
+/* m shift vectors from the SplitMix64 stream keyed by seed: Delta = (u64 >> 11) * 2^-53, shift-major (R:C14) */
+int qmc_shifts(uint64_t seed, int32_t m, int32_t dim, double *shifts_out);
+/* Laurent series of  e^{eg * eps * gamma_E} * base^{p0 + p1 eps} * Gamma(g0 + g1 eps),  g0 a non-negative integer,
+ * orders lo .. lo+n_out-1 (lo = -1 iff g0 == 0); multiply_series = 1 multiplies J (orders k_min..k_max, with errors
+ * combined in quadrature) in place of writing the bare series. */
+int qmc_prefactor_series(double eg, double base, double p0, double p1, int32_t g0, double g1, int32_t n_out,
+                         double *series_out, int32_t *lowest_order);
+/* Sustained FP64 FMA rate of the device (register-resident DFMA chains), in FLOP/s (DFMA = 2).  The roofline
+ * denominator of the evaluation kernel (MEASURED_PEAKS.json has no FP64 entry). */
+int qmc_fp64_peak(void *cuda_stream, void *dev_workspace, size_t dev_workspace_bytes, double *flops_out, double *ms_out);
+const char *qmc_strerror(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QMC_FEYNMAN_H */

@@ -1,0 +1,14 @@
+"""B200-native hot path of arXiv:1508.02512: shifted rank-1 lattice QMC over sector-decomposed Feynman integrands.
+
+    tables = qmc_prepare(workload)                 # graph, kinematics, eps_order -> sector tables   (host C++)
+    result = qmc_integrate(tables, N, m, seed)     # -> Laurent coefficients +- errors               (sm_100a CUDA)
+
+The Python layer only marshals arguments into the C-ABI library libqmcfeyn.so (include/qmc_feynman.h); it is
+imported lazily so that `import paper_1508_02512_b200` works on a box where the library has not been built yet,
+while any call fails loudly there (no CPU fallback).
+"""
+from .binding import (QmcError, Result, Tables, lib, qmc_fp64_peak, qmc_generating_vector, qmc_integrate,
+                      qmc_prefactor_series, qmc_prepare, qmc_shifts, strerror, LIB_PATH)
+
+__all__ = ["QmcError", "Result", "Tables", "lib", "qmc_fp64_peak", "qmc_generating_vector", "qmc_integrate",
+           "qmc_prefactor_series", "qmc_prepare", "qmc_shifts", "strerror", "LIB_PATH"]

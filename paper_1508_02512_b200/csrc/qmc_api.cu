@@ -1,0 +1,593 @@
+// C-ABI entry points (include/qmc_feynman.h), launch logic, small helper kernels.  sm_100a.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <numeric>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/qmc_feynman.h"
+#include "qmc_launch.h"
+#include "qmc_tables.h"
+
+#define QMC_MAX_BLOCKS 592  // upper bound of gridDim.x used for workspace sizing (148 SMs x 4)
+#define QMC_NCAND 64        // Korobov candidates of the P_2 search
+#define QMC_P2_BLOCKS 296
+
+namespace {
+
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// ---- S7 (second stage): fixed-order sum of the block partials, times 1/N -----------------------------
+// fused : partial [chunk][shift][block][nacc] -> out [nacc][shift]            (rows = n_chunks, summed)
+// persec: partial [sector][shift][block][nacc] -> out [sector][nacc][shift]   (rows = n_sectors, kept)
+__global__ void qmc_finalize_kernel(const double *partial, double *out, int rows, int m, int nblocks, int nacc,
+                                    double invN, int persec) {
+  int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  int total = (persec ? rows : 1) * nacc * m;
+  if (idx >= total) return;
+  int kap = idx % m, a = (idx / m) % nacc, row = idx / (m * nacc);
+  double s = 0.0;
+  if (persec) {
+    const double *src = partial + (((size_t)row * m + kap) * nblocks) * nacc + a;
+    for (int b = 0; b < nblocks; ++b) s += src[(size_t)b * nacc];
+  } else {
+    for (int c = 0; c < rows; ++c) {
+      const double *src = partial + (((size_t)c * m + kap) * nblocks) * nacc + a;
+      for (int b = 0; b < nblocks; ++b) s += src[(size_t)b * nacc];
+    }
+  }
+  out[idx] = s * invN;
+}
+
+// ---- generating vector: P_2 figure of merit of Korobov candidates (R:C13) ----------------------------
+// P2(z) = -1 + (1/N) sum_i prod_j (1 + 2 pi^2 B_2({i z_j / N})),  B_2(x) = x^2 - x + 1/6
+__global__ void qmc_p2_kernel(const uint32_t *zc /*[ncand][8]*/, double *partial /*[ncand][gridDim.x]*/, uint32_t N,
+                              int dim) {
+  const int cand = blockIdx.y;
+  const uint32_t *z = zc + cand * QMC_MAXDIM;
+  const double invN = 1.0 / (double)N;
+  const double c2 = 2.0 * 9.86960440108935861883;
+  double s = 0.0;
+  const uint32_t stride = gridDim.x * blockDim.x;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
+    double prod = 1.0;
+    for (int j = 0; j < dim; ++j) {
+      uint32_t r = (uint32_t)(((uint64_t)i * z[j]) % N);
+      double x = (double)r * invN;
+      prod *= 1.0 + c2 * (x * x - x + 1.0 / 6.0);
+    }
+    s += prod;
+  }
+  __shared__ double sh[8];
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += sh[w];
+    partial[(size_t)cand * gridDim.x + blockIdx.x] = t;
+  }
+}
+
+// ---- FP64 FMA peak: 8 independent register-resident DFMA chains per thread ---------------------------
+__global__ void __launch_bounds__(256) qmc_dfma_peak_kernel(double *sink, int iters, double a, double b) {
+  double x0 = threadIdx.x * 1e-3, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+      x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+    }
+  }
+  double s = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
+  if (s == 12345.678) sink[0] = s;  // never true; keeps the chains alive
+}
+
+uint64_t splitmix64(uint64_t &state) {
+  state += 0x9E3779B97F4A7C15ull;
+  uint64_t x = state;
+  x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ull;
+  x = (x ^ (x >> 27)) * 0x94D049BB133111EBull;
+  return x ^ (x >> 31);
+}
+
+uint64_t mulmod(uint64_t a, uint64_t b, uint64_t n) { return (uint64_t)(((unsigned __int128)a * b) % n); }
+
+struct DevLayout {
+  size_t image, secoff, shifts, counters, out, partial, p2z, p2partial, total;
+};
+
+DevLayout layout(const qmc_tables *t, int m) {
+  DevLayout L;
+  size_t nsec = t->sectors.size();
+  size_t o = 0;
+  L.image = o; o += align256(t->image.size());
+  L.secoff = o; o += align256((nsec + 1) * 4);
+  L.shifts = o; o += align256((size_t)m * QMC_MAXDIM * 8);
+  L.counters = o; o += 256;
+  L.out = o; o += align256(nsec * QMC_NACC_MAX * 2 * (size_t)m * 8);
+  L.partial = o; o += align256(nsec * (size_t)m * QMC_MAX_BLOCKS * QMC_NACC_MAX * 2 * 8);
+  L.p2z = o; o += align256((size_t)QMC_NCAND * QMC_MAXDIM * 4);
+  L.p2partial = o; o += align256((size_t)QMC_NCAND * QMC_P2_BLOCKS * 8);
+  L.total = o;
+  return L;
+}
+
+#define CUDA_OK(x)                      \
+  do {                                  \
+    if ((x) != cudaSuccess) {           \
+      cudaGetLastError();               \
+      return QMC_ECUDA;                 \
+    }                                   \
+  } while (0)
+
+int korobov_search(uint64_t N, int dim, cudaStream_t st, unsigned char *ws, size_t p2z_off, size_t p2p_off,
+                   uint64_t *z_out) {
+  if (dim == 1) {
+    z_out[0] = 1;
+    return QMC_OK;
+  }
+  std::vector<uint32_t> zc((size_t)QMC_NCAND * QMC_MAXDIM, 0);
+  std::vector<uint64_t> cand;
+  uint64_t state = N;
+  int guard = 0;
+  while ((int)cand.size() < QMC_NCAND && guard++ < 100000) {
+    uint64_t a = 2 + splitmix64(state) % (N - 3);
+    if (std::gcd(a, N) != 1) continue;
+    cand.push_back(a);
+  }
+  if (cand.empty()) return QMC_EINVAL;
+  int nc = (int)cand.size();
+  for (int c = 0; c < nc; ++c) {
+    uint64_t v = 1;
+    for (int j = 0; j < dim; ++j) {
+      zc[(size_t)c * QMC_MAXDIM + j] = (uint32_t)v;
+      v = mulmod(v, cand[c], N);
+    }
+  }
+  uint32_t *dz = reinterpret_cast<uint32_t *>(ws + p2z_off);
+  double *dp = reinterpret_cast<double *>(ws + p2p_off);
+  CUDA_OK(cudaMemcpyAsync(dz, zc.data(), zc.size() * 4, cudaMemcpyHostToDevice, st));
+  qmc_p2_kernel<<<dim3(QMC_P2_BLOCKS, nc), 256, 0, st>>>(dz, dp, (uint32_t)N, dim);
+  CUDA_OK(cudaGetLastError());
+  std::vector<double> part((size_t)nc * QMC_P2_BLOCKS);
+  CUDA_OK(cudaMemcpyAsync(part.data(), dp, part.size() * 8, cudaMemcpyDeviceToHost, st));
+  CUDA_OK(cudaStreamSynchronize(st));
+  int best = 0;
+  double bestv = 0.0;
+  for (int c = 0; c < nc; ++c) {
+    double s = 0.0;
+    for (int b = 0; b < QMC_P2_BLOCKS; ++b) s += part[(size_t)c * QMC_P2_BLOCKS + b];
+    double p2 = s / (double)N - 1.0;
+    if (c == 0 || p2 < bestv || (p2 == bestv && cand[c] < cand[best])) {
+      best = c;
+      bestv = p2;
+    }
+  }
+  for (int j = 0; j < dim; ++j) z_out[j] = zc[(size_t)best * QMC_MAXDIM + j];
+  return QMC_OK;
+}
+
+// Eqs. 19-20 on per-shift values v[kap] (stride in doubles)
+void mean_err(const double *v, size_t stride, int m, double *mean, double *err) {
+  double s = 0.0;
+  for (int k = 0; k < m; ++k) s += v[k * stride];
+  double q = s / m, d2 = 0.0;
+  for (int k = 0; k < m; ++k) {
+    double d = v[k * stride] - q;
+    d2 += d * d;
+  }
+  *mean = q;
+  *err = std::sqrt(d2 / ((double)m * (m - 1)));
+}
+
+}  // namespace
+
+// =====================================================================================================
+extern "C" {
+
+int qmc_prepare(const qmc_graph *graph, const qmc_kinematics *kin, int32_t eps_order, const qmc_options *options,
+                qmc_tables **out) {
+  if (!out) return QMC_EINVAL;
+  *out = nullptr;
+  qmc_tables *t = new (std::nothrow) qmc_tables;
+  if (!t) return QMC_ENOMEM;
+  int rc;
+  try {
+    rc = qmc_build_tables(graph, kin, eps_order, options, t);
+  } catch (...) {
+    rc = QMC_ENOMEM;
+  }
+  if (rc != QMC_OK) {
+    delete t;
+    return rc;
+  }
+  *out = t;
+  return QMC_OK;
+}
+
+void qmc_tables_free(qmc_tables *t) { delete t; }
+
+int qmc_tables_info(const qmc_tables *t, int32_t *n_sectors, int32_t *dim, int32_t *k_min, int32_t *k_max,
+                    int32_t *is_complex) {
+  if (!t) return QMC_EINVAL;
+  if (n_sectors) *n_sectors = (int32_t)t->sectors.size();
+  if (dim) *dim = t->n;
+  if (k_min) *k_min = t->kmin;
+  if (k_max) *k_max = t->kmax;
+  if (is_complex) *is_complex = t->lambda > 0.0 ? 1 : 0;
+  return QMC_OK;
+}
+
+int qmc_tables_export(const qmc_tables *t, void *buf, size_t *len) {
+  if (!t || !len) return QMC_EINVAL;
+  size_t words = 12;
+  for (const QmcSector &s : t->sectors) words += 1 + 2 * (size_t)t->n + 2 + (s.U.size() + s.F.size()) * (1 + (size_t)t->n);
+  size_t need = words * 8;
+  if (!buf) {
+    *len = need;
+    return QMC_OK;
+  }
+  if (*len < need) {
+    *len = need;
+    return QMC_ENOMEM;
+  }
+  int64_t *w = static_cast<int64_t *>(buf);
+  double *d = static_cast<double *>(buf);
+  size_t p = 0;
+  w[p++] = 0x514D4346;
+  w[p++] = 1;
+  w[p++] = (int64_t)t->sectors.size();
+  w[p++] = t->n;
+  w[p++] = t->kmin;
+  w[p++] = t->kmax;
+  w[p++] = t->lambda > 0.0 ? 1 : 0;
+  w[p++] = t->aU0;
+  w[p++] = t->aU1;
+  w[p++] = t->aF0;
+  w[p++] = t->aF1;
+  d[p++] = t->lambda;
+  for (const QmcSector &s : t->sectors) {
+    w[p++] = s.primary;
+    for (int j = 0; j < t->n; ++j) w[p++] = s.alpha[j];
+    for (int j = 0; j < t->n; ++j) w[p++] = s.beta[j];
+    w[p++] = (int64_t)s.U.size();
+    w[p++] = (int64_t)s.F.size();
+    for (int which = 0; which < 2; ++which)
+      for (const QmcMono &m : (which ? s.F : s.U)) {
+        d[p++] = m.c;
+        for (int j = 0; j < t->n; ++j) w[p++] = m.e[j];
+      }
+  }
+  *len = need;
+  return QMC_OK;
+}
+
+size_t qmc_workspace_bytes(const qmc_tables *t, uint64_t, int32_t m) {
+  if (!t || m < 1) return 0;
+  return layout(t, m).total;
+}
+
+int qmc_shifts(uint64_t seed, int32_t m, int32_t dim, double *shifts_out) {
+  if (m < 1 || dim < 1 || !shifts_out) return QMC_EINVAL;
+  uint64_t state = seed;
+  for (int k = 0; k < m; ++k)
+    for (int j = 0; j < dim; ++j) shifts_out[(size_t)k * dim + j] = (double)(splitmix64(state) >> 11) * (1.0 / 9007199254740992.0);
+  return QMC_OK;
+}
+
+int qmc_generating_vector(uint64_t N, int32_t dim, void *cuda_stream, void *dev_workspace, size_t dev_workspace_bytes,
+                          uint64_t *z_out) {
+  if (N < 5 || N >= (1ull << 31) || dim < 1 || dim > QMC_MAXDIM || !z_out) return QMC_EINVAL;
+  size_t p2z = 0, p2p = align256((size_t)QMC_NCAND * QMC_MAXDIM * 4);
+  if (dim > 1 && (!dev_workspace || dev_workspace_bytes < p2p + (size_t)QMC_NCAND * QMC_P2_BLOCKS * 8)) return QMC_ENOMEM;
+  return korobov_search(N, dim, static_cast<cudaStream_t>(cuda_stream), static_cast<unsigned char *>(dev_workspace), p2z,
+                        p2p, z_out);
+}
+
+int qmc_fp64_peak(void *cuda_stream, void *dev_workspace, size_t dev_workspace_bytes, double *flops_out, double *ms_out) {
+  if (!dev_workspace || dev_workspace_bytes < 8 || !flops_out) return QMC_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  int dev = 0, sms = 0;
+  CUDA_OK(cudaGetDevice(&dev));
+  CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const int iters = 4096, blocks = sms * 8;
+  cudaEvent_t e0, e1;
+  CUDA_OK(cudaEventCreate(&e0));
+  CUDA_OK(cudaEventCreate(&e1));
+  double best = 0.0, best_ms = 0.0;
+  for (int rep = 0; rep < 5; ++rep) {
+    cudaEventRecord(e0, st);
+    qmc_dfma_peak_kernel<<<blocks, 256, 0, st>>>(static_cast<double *>(dev_workspace), iters, 1.0000001, 1e-9);
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) {
+      cudaEventDestroy(e0);
+      cudaEventDestroy(e1);
+      cudaGetLastError();
+      return QMC_ECUDA;
+    }
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    double fl = (double)blocks * 256.0 * iters * 64.0 * 2.0 / (ms * 1e-3);
+    if (rep > 0 && fl > best) {
+      best = fl;
+      best_ms = ms;
+    }
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  *flops_out = best;
+  if (ms_out) *ms_out = best_ms;
+  return QMC_OK;
+}
+
+int qmc_integrate_ex(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t seed, const qmc_run *run, void *cuda_stream,
+                     void *dev_workspace, size_t dev_workspace_bytes, qmc_result *out) {
+  if (!tc || !out) return QMC_EINVAL;
+  qmc_tables *t = const_cast<qmc_tables *>(tc);  // launcher caches (resident image, generating vector)
+  const int n = t->n, nsec_all = (int)t->sectors.size();
+  if (N < 5 || N >= (1ull << 31) || m < 2) return QMC_EINVAL;  // Eq. 20 needs m >= 2
+  qmc_run r;
+  std::memset(&r, 0, sizeof r);
+  if (run) r = *run;
+  const int sb = r.sector_begin, se = r.sector_end > 0 ? r.sector_end : nsec_all;
+  if (sb < 0 || se > nsec_all || sb >= se) return QMC_EINVAL;
+  const uint64_t ibeg = r.index_begin, istep = r.index_count ? r.index_step : 1, icount = r.index_count ? r.index_count : N;
+  if (istep < 1 || ibeg >= N || icount > N) return QMC_EINVAL;
+  const bool cplx = t->lambda > 0.0;
+  const bool want_persec = out->sector_coeff || out->sector_err || out->shift_sums;
+  const int mode = r.mode ? r.mode : (want_persec ? 2 : 1);
+  if (mode != 1 && mode != 2) return QMC_EINVAL;
+  if (mode == 1 && want_persec) return QMC_EINVAL;
+  const bool persec = mode == 2;
+
+  int devcount = 0;
+  if (cudaGetDeviceCount(&devcount) != cudaSuccess || devcount < 1) {
+    cudaGetLastError();
+    return QMC_ECUDA;  // no CPU fallback
+  }
+  DevLayout L = layout(t, m);
+  if (!dev_workspace || dev_workspace_bytes < L.total) return QMC_ENOMEM;
+  unsigned char *ws = static_cast<unsigned char *>(dev_workspace);
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+
+  // ---- generating vector and shifts ---------------------------------------------------------------------
+  uint64_t z[QMC_MAXDIM] = {0};
+  if (r.z) {
+    for (int j = 0; j < n; ++j) z[j] = r.z[j];
+  } else {
+    if (t->cached_N != N) {
+      int rc = korobov_search(N, n, st, ws, L.p2z, L.p2partial, t->cached_z);
+      if (rc != QMC_OK) return rc;
+      t->cached_N = N;
+    }
+    for (int j = 0; j < n; ++j) z[j] = t->cached_z[j];
+  }
+  for (int j = 0; j < n; ++j)
+    if (z[j] == 0 || z[j] >= N || std::gcd(z[j], N) != 1) return QMC_EINVAL;
+  std::vector<double> shifts((size_t)m * n);
+  if (r.shifts) {
+    std::memcpy(shifts.data(), r.shifts, shifts.size() * 8);
+    for (double v : shifts)
+      if (!(v >= 0.0 && v < 1.0)) return QMC_EINVAL;
+  } else {
+    qmc_shifts(seed, m, n, shifts.data());
+  }
+
+  // ---- launch geometry ----------------------------------------------------------------------------------
+  int dev = 0, sms = 0, smem_optin = 0;
+  CUDA_OK(cudaGetDevice(&dev));
+  CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  CUDA_OK(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+  const int nacc = QMC_MAXSING + t->kmax + 1, nc = cplx ? 2 : 1;
+  const size_t fixed_smem = 16 + (((size_t)m * n * 8 + 15) & ~(size_t)15) + (QMC_THREADS / 32) * 8 + (size_t)3 * n * QMC_THREADS * 8;
+  const size_t per_sector_acc = persec ? (size_t)nacc * nc * QMC_THREADS * 8 : 0;
+  // sectors per chunk: as many as fit the shared-memory budget (tables + per-sector accumulators)
+  int spc = 0;
+  uint32_t tab_bytes = 0;
+  {
+    const size_t budget = (size_t)smem_optin - 1024;
+    auto fits = [&](int cnt, uint32_t &tb) {
+      // worst-case table bytes over all chunks of `cnt` sectors
+      uint32_t worst = 0;
+      for (int s0 = sb; s0 < se; s0 += cnt) {
+        int s1 = std::min(s0 + cnt, se);
+        worst = std::max(worst, t->secoff[s1] - t->secoff[s0]);
+      }
+      tb = worst;
+      size_t need = worst + (((size_t)(cnt + 1) * 4 + 15) & ~(size_t)15) + fixed_smem + per_sector_acc * cnt;
+      return need <= budget;
+    };
+    int lo = 1, hi = se - sb;
+    uint32_t tb;
+    if (!fits(1, tb)) return QMC_ENOMEM;
+    if (fits(hi, tb)) {
+      spc = hi;
+    } else {
+      while (hi - lo > 1) {
+        int mid = (lo + hi) / 2;
+        if (fits(mid, tb)) lo = mid; else hi = mid;
+      }
+      spc = lo;
+    }
+    fits(spc, tab_bytes);
+  }
+  const int nchunks = (se - sb + spc - 1) / spc;
+  const size_t smem = tab_bytes + (((size_t)(spc + 1) * 4 + 15) & ~(size_t)15) + fixed_smem + per_sector_acc * spc;
+  int bps = 0;
+  CUDA_OK(qmc_kernel_prepare(n, t->kmax, cplx, smem, &bps));
+  if (bps < 1) return QMC_ECUDA;
+  int gx = std::min<long long>({(long long)sms * bps, (long long)QMC_MAX_BLOCKS, (long long)((icount + QMC_THREADS - 1) / QMC_THREADS)});
+  gx = std::max(gx, 1);
+
+  // ---- uploads -------------------------------------------------------------------------------------------
+  if (!(r.tables_resident && t->resident_ws == dev_workspace)) {
+    CUDA_OK(cudaMemcpyAsync(ws + L.image, t->image.data(), t->image.size(), cudaMemcpyHostToDevice, st));
+    CUDA_OK(cudaMemcpyAsync(ws + L.secoff, t->secoff.data(), t->secoff.size() * 4, cudaMemcpyHostToDevice, st));
+    t->resident_ws = dev_workspace;
+  }
+  CUDA_OK(cudaMemcpyAsync(ws + L.shifts, shifts.data(), shifts.size() * 8, cudaMemcpyHostToDevice, st));
+  CUDA_OK(cudaMemsetAsync(ws + L.counters, 0, 32, st));
+
+  QmcLaunch p;
+  std::memset(&p, 0, sizeof p);
+  p.image = ws + L.image;
+  p.secoff = reinterpret_cast<const uint32_t *>(ws + L.secoff);
+  p.shifts = reinterpret_cast<const double *>(ws + L.shifts);
+  p.partial = reinterpret_cast<double *>(ws + L.partial);
+  p.counters = reinterpret_cast<unsigned long long *>(ws + L.counters);
+  p.N = (uint32_t)N;
+  p.count = (uint32_t)icount;
+  for (int j = 0; j < n; ++j) {
+    p.zeff[j] = (uint32_t)mulmod(istep % N, z[j], N);
+    p.off[j] = (uint32_t)mulmod(ibeg, z[j], N);
+  }
+  p.m = m;
+  p.kmax = t->kmax;
+  p.aU0 = t->aU0; p.aU1 = t->aU1; p.aF0 = t->aF0; p.aF1 = t->aF1;
+  p.lambda = t->lambda;
+  p.transform = t->transform;
+  p.sec_begin = sb; p.sec_end = se; p.sec_per_chunk = spc;
+  p.persec = persec ? 1 : 0;
+  p.tab_smem_bytes = (tab_bytes + 15) & ~15u;
+
+  cudaEvent_t e0, e1;
+  CUDA_OK(cudaEventCreate(&e0));
+  CUDA_OK(cudaEventCreate(&e1));
+  cudaEventRecord(e0, st);
+  cudaError_t ce = qmc_kernel_launch(n, t->kmax, cplx, dim3(gx, nchunks), smem, st, p);
+  const int rows = persec ? (se - sb) : nchunks;
+  const int nout = (persec ? (se - sb) : 1) * nacc * nc * m;
+  double *dout = reinterpret_cast<double *>(ws + L.out);
+  if (ce == cudaSuccess) {
+    qmc_finalize_kernel<<<(nout + 127) / 128, 128, 0, st>>>(p.partial, dout, rows, m, gx, nacc * nc, 1.0 / (double)N, persec ? 1 : 0);
+    ce = cudaGetLastError();
+  }
+  cudaEventRecord(e1, st);
+  std::vector<double> hout((size_t)nout);
+  unsigned long long hc[4] = {0, 0, 0, 0};
+  if (ce == cudaSuccess) ce = cudaMemcpyAsync(hout.data(), dout, hout.size() * 8, cudaMemcpyDeviceToHost, st);
+  if (ce == cudaSuccess) ce = cudaMemcpyAsync(hc, ws + L.counters, 32, cudaMemcpyDeviceToHost, st);
+  if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
+  float ms = 0.f;
+  if (ce == cudaSuccess) cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  if (ce != cudaSuccess) {
+    cudaGetLastError();
+    t->resident_ws = nullptr;
+    return QMC_ECUDA;
+  }
+  out->kernel_ms = ms;
+  out->kernel_launches = 2;
+  out->mode_used = mode;
+  for (int q = 0; q < 4; ++q) out->counters[q] = (int64_t)hc[q];
+
+  // ---- S8: statistics (Eqs. 19-20), Re and Im separately (R:C15) ---------------------------------------
+  const int K = t->kmax - t->kmin + 1;
+  auto acc_index = [&](int k_index) { return (k_index + t->kmin) + QMC_MAXSING; };  // order -> accumulator
+  // per-shift totals T[k][kap][c]
+  std::vector<double> Tt((size_t)K * m * 2, 0.0);
+  const int nrows = persec ? (se - sb) : 1;
+  for (int row = 0; row < nrows; ++row)
+    for (int k = 0; k < K; ++k)
+      for (int c = 0; c < nc; ++c) {
+        int a = acc_index(k) * nc + c;
+        const double *src = hout.data() + ((size_t)row * nacc * nc + a) * m;
+        for (int kap = 0; kap < m; ++kap) Tt[((size_t)k * m + kap) * 2 + c] += src[kap];
+      }
+  for (int k = 0; k < K; ++k)
+    for (int c = 0; c < 2; ++c) {
+      double mean, err;
+      mean_err(Tt.data() + (size_t)k * m * 2 + c, 2, m, &mean, &err);
+      if (out->coeff) out->coeff[2 * k + c] = mean;
+      if (out->err) out->err[2 * k + c] = err;
+    }
+  if (out->shift_totals) std::memcpy(out->shift_totals, Tt.data(), Tt.size() * 8);
+  if (persec)
+    for (int row = 0; row < nrows; ++row)
+      for (int k = 0; k < K; ++k)
+        for (int c = 0; c < 2; ++c) {
+          std::vector<double> v((size_t)m, 0.0);
+          if (c < nc) {
+            int a = acc_index(k) * nc + c;
+            const double *src = hout.data() + ((size_t)row * nacc * nc + a) * m;
+            for (int kap = 0; kap < m; ++kap) v[kap] = src[kap];
+          }
+          size_t o2 = ((size_t)row * K + k);
+          if (out->shift_sums)
+            for (int kap = 0; kap < m; ++kap) out->shift_sums[(o2 * m + kap) * 2 + c] = v[kap];
+          double mean, err;
+          mean_err(v.data(), 1, m, &mean, &err);
+          if (out->sector_coeff) out->sector_coeff[o2 * 2 + c] = mean;
+          if (out->sector_err) out->sector_err[o2 * 2 + c] = err;
+        }
+  return QMC_OK;
+}
+
+int qmc_integrate(const qmc_tables *t, uint64_t N, int32_t m, uint64_t seed, void *cuda_stream, void *dev_workspace,
+                  size_t dev_workspace_bytes, qmc_result *out) {
+  return qmc_integrate_ex(t, N, m, seed, nullptr, cuda_stream, dev_workspace, dev_workspace_bytes, out);
+}
+
+// Laurent series of e^{eg eps gammaE} base^{p0+p1 eps} Gamma(g0 + g1 eps)
+int qmc_prefactor_series(double eg, double base, double p0, double p1, int32_t g0, double g1, int32_t n_out,
+                         double *series_out, int32_t *lowest_order) {
+  if (n_out < 1 || n_out > 16 || g0 < 0 || !series_out || !(base > 0.0)) return QMC_EINVAL;
+  static const double zeta[17] = {0, 0, 1.6449340668482264365, 1.2020569031595942854, 1.0823232337111381915,
+                                  1.0369277551433699263, 1.0173430619844491397, 1.0083492773819228268,
+                                  1.0040773561979443394, 1.0020083928260822144, 1.0009945751278180853,
+                                  1.0004941886041194646, 1.0002460865533080483, 1.0001227133475784891,
+                                  1.0000612481350587048, 1.0000305882363070205, 1.0000152822594086519};
+  const double gammaE = 0.57721566490153286061;
+  const int n = n_out;
+  // exponent series E(eps) with exp(E) = e^{eg eps gE} base^{p1 eps} Gamma(1 + g1 eps)
+  std::vector<double> E(n, 0.0), S(n, 0.0);
+  if (n > 1) E[1] = eg * gammaE + p1 * std::log(base) - gammaE * g1;
+  double gp = g1;
+  for (int k = 2; k < n; ++k) {
+    gp *= g1;
+    E[k] = ((k & 1) ? -1.0 : 1.0) * zeta[k] * gp / k;
+  }
+  // S = exp(E): S' = E' S
+  S[0] = 1.0;
+  for (int k = 1; k < n; ++k) {
+    double s = 0.0;
+    for (int j = 1; j <= k; ++j) s += j * E[j] * S[k - j];
+    S[k] = s / k;
+  }
+  // Gamma(g0 + x) = Gamma(1 + x) prod_{q=1}^{g0-1} (q + x);  g0 = 0: Gamma(x) = Gamma(1+x)/x
+  for (int q = 1; q < g0; ++q) {
+    for (int k = n - 1; k >= 1; --k) S[k] = q * S[k] + g1 * S[k - 1];
+    S[0] *= q;
+  }
+  double scale = std::pow(base, p0);
+  int lo = 0;
+  if (g0 == 0) {
+    if (g1 == 0.0) return QMC_EINVAL;
+    scale /= g1;
+    lo = -1;
+  }
+  for (int k = 0; k < n; ++k) series_out[k] = S[k] * scale;
+  if (lowest_order) *lowest_order = lo;
+  return QMC_OK;
+}
+
+const char *qmc_strerror(int status) {
+  switch (status) {
+    case QMC_OK: return "ok";
+    case QMC_EINVAL: return "invalid argument (graph, kinematics, N, z, m or shifts)";
+    case QMC_EDEPTH: return "sector decomposition did not terminate within max_depth";
+    case QMC_EUNSUPPORTED: return "unsupported: alpha <= -2, beta = 0 on a singular variable, > 4 singular variables, nu != 1 or eps_order > 2";
+    case QMC_ECUDA: return "CUDA error or no CUDA device (there is no CPU fallback)";
+    case QMC_ENOMEM: return "workspace or buffer too small";
+    case QMC_ECONTOUR: return "contour deformation on the wrong side";
+    default: return "unknown status";
+  }
+}
+
+}  // extern "C"

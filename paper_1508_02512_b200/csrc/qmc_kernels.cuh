@@ -1,0 +1,609 @@
+// Evaluation kernel of the hot path (steps S1-S7 of DESIGN.md), sm_100a.
+//
+// One thread = one lattice point at a time (grid-stride over the points of one shift), all sectors of the
+// block's chunk evaluated for that point with the per-point quantities (t_j, ln t_j, 1/t_j) computed once.
+// Sector tables are staged in shared memory with one TMA bulk copy per block (cp.async.bulk + mbarrier) and read
+// with warp-uniform (broadcast) loads.  Everything else lives in registers: FP64 (complex) arithmetic,
+// truncated Laurent series, the 2^s corners of the subtraction.
+//
+// Per sector with s singular variables (alpha = -1), the eps-expanded subtracted integrand (Eqs. 9-12,
+// PAPER.md:94-114) is evaluated in product form:
+//   sum_k c_k eps^k = sum_{Z subset sing} g_Z(eps) prod_{j notin Z} A_j(eps) prod_{j in Z} (B_j(eps) - A_j(eps)),
+//   g_Z = G_Z exp(eps Lambda_Z),  A_j = t_j^-1 exp(eps beta_j ln t_j),  B_j = 1/(beta_j eps),
+// folded one singular variable at a time:  h <- A_j (h[Z without j] - h[Z with j]) + B_j h[Z with j].
+// (The oracle uses the expanded double-sum form instead.)
+// Real path: U^(t^Z), F^(t^Z) for all 2^s corners come from ONE pass over the monomials (partial sums per
+// "group" = set of singular variables a monomial depends on) followed by a subset-sum transform.
+// Complex path: contour deformation (Eq. 14) at every corner: gradient and Hessian of F^ from
+// the monomial table, z = t rho, det(dz/dt) by LU with row pivoting, complex U^(z), F^(z), complex logs.
+#pragma once
+#include <cstdint>
+#include <type_traits>
+#include <cuda_runtime.h>
+
+#include "qmc_tables.h"
+
+#include "qmc_launch.h"
+
+// partial layout: fused  : [chunk][shift][block][NACC*(1|2)]
+//                 persec : [sector - sec_begin][shift][block][NACC*(1|2)]
+// accumulator index a <-> order k = a - QMC_MAXSING  (so that a sector with s singular variables writes
+// a = QMC_MAXSING - s .. QMC_MAXSING + kmax with compile-time indices).
+
+namespace qmcdev {
+
+struct cd {
+  double re, im;
+};
+__device__ __forceinline__ cd operator+(cd a, cd b) { return cd{a.re + b.re, a.im + b.im}; }
+__device__ __forceinline__ cd operator-(cd a, cd b) { return cd{a.re - b.re, a.im - b.im}; }
+__device__ __forceinline__ cd operator*(cd a, cd b) {
+  return cd{a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re};
+}
+__device__ __forceinline__ cd operator*(double s, cd a) { return cd{s * a.re, s * a.im}; }
+__device__ __forceinline__ cd cinv(cd a) {
+  double d = 1.0 / (a.re * a.re + a.im * a.im);
+  return cd{a.re * d, -a.im * d};
+}
+__device__ __forceinline__ double cnorm2(cd a) { return a.re * a.re + a.im * a.im; }
+// principal log; a negative real argument carries the -i0 of F -> F - i0: arg = -pi (R:C11)
+__device__ __forceinline__ cd clog_m(cd a) {
+  double arg = (a.im == 0.0 && a.re < 0.0) ? -3.14159265358979323846 : atan2(a.im, a.re);
+  return cd{0.5 * log(cnorm2(a)), arg};
+}
+
+template <class T>
+struct Num;
+template <>
+struct Num<double> {
+  static __device__ __forceinline__ double zero() { return 0.0; }
+  static __device__ __forceinline__ double scale(double s, double a) { return s * a; }
+};
+template <>
+struct Num<cd> {
+  static __device__ __forceinline__ cd zero() { return cd{0.0, 0.0}; }
+  static __device__ __forceinline__ cd scale(double s, cd a) { return cd{s * a.re, s * a.im}; }
+};
+
+__device__ __forceinline__ double ipow_pos(double x, int e) {  // e >= 0, small
+  double r = 1.0;
+  for (int q = 0; q < e; ++q) r *= x;
+  return r;
+}
+
+// c * prod_j x_j^{e_j}; exponents are warp-uniform nibbles of w
+template <int NDIM>
+__device__ __forceinline__ double monomial(double c, uint32_t w, const double (&x)[NDIM]) {
+  double v = c;
+#pragma unroll
+  for (int j = 0; j < NDIM; ++j) {
+    int e = (w >> (4 * j)) & 15;
+    if (e) {
+      v *= x[j];
+      if (e > 1) {
+        v *= x[j];
+        for (int q = 2; q < e; ++q) v *= x[j];
+      }
+    }
+  }
+  return v;
+}
+
+// per-sector context shared by all corners
+template <int NDIM, int NS, class T>
+struct Ctx {
+  double t[NDIM];            // permuted variables (singular first)
+  double invt[NS > 0 ? NS : 1];
+  double invbeta[NS > 0 ? NS : 1];
+  double cL[NS > 0 ? NS : 1][QMC_NACC_MAX];  // (beta_j ln t_j)^p / p!
+  double G0, L0;             // regular-variable factor and log (common to all corners)
+  int aU0, aU1, aF0, aF1;
+  // real path: subset sums of U^, F^ over the groups
+  double PU[1 << NS], PF[1 << NS];
+  // complex path
+  double lambda;
+  double invt_all[NDIM];
+  const QmcSectorHdr *hdr;
+  const double *coef;
+  const uint32_t *exps;
+  unsigned cntImF, cntReU;
+};
+
+// ---- corner value g_Z(eps) = G_Z exp(eps Lambda_Z), truncated to K terms ------------------------------
+template <int NDIM, int NS, int K, int ZMASK>
+__device__ __forceinline__ void corner_series(Ctx<NDIM, NS, double> &c, double (&out)[K]) {
+  constexpr int FULL = (1 << NS) - 1;
+  double Uv = c.PU[FULL ^ ZMASK], Fv = c.PF[FULL ^ ZMASK];
+  double num = c.G0, den = 1.0;
+  {
+    double pu = ipow_pos(Uv, c.aU0 < 0 ? -c.aU0 : c.aU0), pf = ipow_pos(Fv, c.aF0 < 0 ? -c.aF0 : c.aF0);
+    if (c.aU0 >= 0) num *= pu; else den *= pu;
+    if (c.aF0 >= 0) num *= pf; else den *= pf;
+  }
+  double W = num / den;
+  double Lam = (double)c.aU1 * log(Uv) + (double)c.aF1 * log(Fv) + c.L0;
+  out[0] = W;
+#pragma unroll
+  for (int p = 1; p < K; ++p) out[p] = out[p - 1] * Lam * (1.0 / p);
+}
+
+// ZMASK is a run-time (warp-uniform) argument here: nothing below indexes a register array with it, and one
+// out-of-line copy per (NDIM, NS, K) keeps the code size and the compile time down.
+template <int NDIM, int NS, int K>
+__device__ __noinline__ void corner_series_cplx(Ctx<NDIM, NS, cd> &c, const int ZMASK, cd (&out)[K]) {
+  // tau = t with the components in Z set to 0.  Only monomials free of Z-variables survive in U^(z), F^(z) and
+  // in the derivatives w.r.t. non-Z variables; dF^/dt_a for a in Z picks the monomials linear in t_a.
+  const QmcSectorHdr *h = c.hdr;
+  const int nU = h->nU, nF = h->nF;
+  double grad[NDIM], hess[NDIM][NDIM];
+#pragma unroll
+  for (int i = 0; i < NDIM; ++i) {
+    grad[i] = 0.0;
+#pragma unroll
+    for (int k = 0; k < NDIM; ++k) hess[i][k] = 0.0;
+  }
+  // nibble mask of the Z positions
+  uint32_t zn = 0;
+#pragma unroll
+  for (int b = 0; b < NS; ++b)
+    if (ZMASK >> b & 1) zn |= 15u << (4 * b);
+  for (int mi = 0; mi < nF; ++mi) {
+    uint32_t w = c.exps[nU + mi];
+    uint32_t wz = w & zn;
+    double v0 = monomial<NDIM>(c.coef[nU + mi], w & ~zn, c.t);
+    if (wz == 0) {
+#pragma unroll
+      for (int i = 0; i < NDIM; ++i) {
+        if (i < NS && (ZMASK >> i & 1)) continue;
+        int ei = (w >> (4 * i)) & 15;
+        if (ei) {
+          double gi = (double)ei * v0 * c.invt_all[i];
+          grad[i] += gi;
+#pragma unroll
+          for (int k = i; k < NDIM; ++k) {
+            if (k < NS && (ZMASK >> k & 1)) continue;
+            int ek = ((w >> (4 * k)) & 15) - (k == i ? 1 : 0);
+            if (ek > 0) hess[i][k] += gi * (double)ek * c.invt_all[k];
+          }
+        }
+      }
+    } else if ((wz & (wz - 1)) == 0 && (wz & 0x11111111u)) {
+      // exactly one Z-variable, with exponent 1 (a single bit set, and it is the lowest bit of its nibble)
+#pragma unroll
+      for (int a = 0; a < NS; ++a)
+        if ((ZMASK >> a & 1) && (wz >> (4 * a) & 15)) grad[a] += v0;
+    }
+  }
+  // rho_i = 1 - i lambda (1 - tau_i) F_i ;  z_i = tau_i rho_i ;  J = 1 + i B
+  cd z[NDIM], rho[NDIM];
+  cd J[NDIM][NDIM];
+#pragma unroll
+  for (int i = 0; i < NDIM; ++i) {
+    const bool inZ = (i < NS) && (ZMASK >> i & 1);
+    double tau = inZ ? 0.0 : c.t[i];
+    rho[i] = cd{1.0, -c.lambda * (1.0 - tau) * grad[i]};
+    z[i] = cd{tau, tau * rho[i].im};
+#pragma unroll
+    for (int k = 0; k < NDIM; ++k) {
+      const bool kinZ = (k < NS) && (ZMASK >> k & 1);
+      if (inZ || kinZ) {
+        J[i][k] = cd{(i == k) ? 1.0 : 0.0, 0.0};  // row/column of a Z variable: its rho_i cancels rho_i^-1 (alpha=-1)
+      } else {
+        double hik = (k >= i) ? hess[i][k] : hess[k][i];
+        double b = -c.lambda * tau * (1.0 - tau) * hik;
+        if (i == k) b += -c.lambda * (1.0 - 2.0 * tau) * grad[i];
+        J[i][k] = cd{(i == k) ? 1.0 : 0.0, b};
+      }
+    }
+  }
+  // det J: Gaussian elimination with row pivoting (compare-and-swap down each column)
+  cd det = cd{1.0, 0.0};
+#pragma unroll
+  for (int col = 0; col < NDIM; ++col) {
+#pragma unroll
+    for (int r = col + 1; r < NDIM; ++r) {
+      if (cnorm2(J[r][col]) > cnorm2(J[col][col])) {
+#pragma unroll
+        for (int k = col; k < NDIM; ++k) {
+          cd tmp = J[r][k];
+          J[r][k] = J[col][k];
+          J[col][k] = tmp;
+        }
+        det = cd{-det.re, -det.im};
+      }
+    }
+    det = det * J[col][col];
+    if (col + 1 < NDIM) {
+      cd ip = cinv(J[col][col]);
+#pragma unroll
+      for (int r = col + 1; r < NDIM; ++r) {
+        cd f = J[r][col] * ip;
+#pragma unroll
+        for (int k = col + 1; k < NDIM; ++k) J[r][k] = J[r][k] - f * J[col][k];
+      }
+    }
+  }
+  // complex U^(z), F^(z): monomials free of Z variables
+  cd Uv = cd{0.0, 0.0}, Fv = cd{0.0, 0.0};
+  for (int mi = 0; mi < nU + nF; ++mi) {
+    uint32_t w = c.exps[mi];
+    if (w & zn) continue;
+    cd v = cd{c.coef[mi], 0.0};
+#pragma unroll
+    for (int j = 0; j < NDIM; ++j) {
+      int e = (w >> (4 * j)) & 15;
+      for (int q = 0; q < e; ++q) v = v * z[j];
+    }
+    if (mi < nU) Uv = Uv + v; else Fv = Fv + v;
+  }
+  if (Fv.im > 0.0) ++c.cntImF;
+  if (!(Uv.re > 0.0)) ++c.cntReU;
+  // G_Z = G0 det J prod_{j notin Z} rho_j^{alpha_j} U^{aU0} F^{aF0}
+  // Lambda_Z = aU1 ln U + aF1 ln F + sum_all beta_j ln rho_j + L0
+  cd num = cd{c.G0, 0.0} * det, den = cd{1.0, 0.0};
+  cd Lam = (double)c.aU1 * clog_m(Uv) + (double)c.aF1 * clog_m(Fv);
+  Lam.re += c.L0;
+#pragma unroll
+  for (int j = 0; j < NDIM; ++j) {
+    const bool inZ = (j < NS) && (ZMASK >> j & 1);
+    int a = h->alpha[j], b = h->beta[j];
+    if (!inZ) {
+      for (int q = 0; q < (a < 0 ? -a : a); ++q) {
+        if (a > 0) num = num * rho[j]; else den = den * rho[j];
+      }
+    }
+    if (b) Lam = Lam + (double)b * clog_m(rho[j]);
+  }
+  {
+    int eu = c.aU0 < 0 ? -c.aU0 : c.aU0, ef = c.aF0 < 0 ? -c.aF0 : c.aF0;
+    for (int q = 0; q < eu; ++q) { if (c.aU0 > 0) num = num * Uv; else den = den * Uv; }
+    for (int q = 0; q < ef; ++q) { if (c.aF0 > 0) num = num * Fv; else den = den * Fv; }
+  }
+  cd W = num * cinv(den);
+  out[0] = W;
+#pragma unroll
+  for (int p = 1; p < K; ++p) out[p] = (1.0 / p) * (out[p - 1] * Lam);
+}
+
+// ---- fold the singular variables one at a time ---------------------------------------------------------
+// Series windows: at depth d (d variables folded) index i <-> order i - d.  LEVEL = next variable to fold here.
+template <int NDIM, int NS, int K, int LEVEL, int ZMASK, class T>
+struct Fold {
+  static __device__ __forceinline__ void eval(Ctx<NDIM, NS, T> &c, T (&out)[K]) {
+    T a[K], b[K];
+    Fold<NDIM, NS, K, LEVEL + 1, ZMASK, T>::eval(c, a);
+    Fold<NDIM, NS, K, LEVEL + 1, ZMASK | (1 << LEVEL), T>::eval(c, b);
+    const double it = c.invt[LEVEL], ib = c.invbeta[LEVEL];
+    T d[K];
+#pragma unroll
+    for (int i = 0; i + 1 < K; ++i) d[i] = Num<T>::scale(it, a[i] - b[i]);
+    out[0] = Num<T>::scale(ib, b[0]);
+#pragma unroll
+    for (int i = 1; i < K; ++i) {
+      T s = Num<T>::scale(ib, b[i]) + d[i - 1];
+#pragma unroll
+      for (int p = 1; p < i; ++p) s = s + Num<T>::scale(c.cL[LEVEL][p], d[i - 1 - p]);
+      out[i] = s;
+    }
+  }
+};
+template <int NDIM, int NS, int K, int ZMASK>
+struct Fold<NDIM, NS, K, NS, ZMASK, double> {
+  static __device__ __forceinline__ void eval(Ctx<NDIM, NS, double> &c, double (&out)[K]) {
+    corner_series<NDIM, NS, K, ZMASK>(c, out);
+  }
+};
+template <int NDIM, int NS, int K, int ZMASK>
+struct Fold<NDIM, NS, K, NS, ZMASK, cd> {
+  static __device__ __forceinline__ void eval(Ctx<NDIM, NS, cd> &c, cd (&out)[K]) {
+    corner_series_cplx<NDIM, NS, K>(c, ZMASK, out);
+  }
+};
+
+// ---- one sector at one point -----------------------------------------------------------------------------
+// pt: this thread's per-point arrays in shared memory, element (a, j) at pt[(a*NDIM + j)*QMC_THREADS],
+//     a = 0: t_j, 1: ln t_j, 2: 1/t_j.
+template <int NDIM, int NS, int KMAX, class T>
+__device__ __forceinline__ void sector_eval(const QmcLaunch &p, const QmcSectorHdr *h, const double *pt, T (&res)[KMAX + NS + 1],
+                                            unsigned &cntImF, unsigned &cntReU) {
+  constexpr int K = KMAX + NS + 1;
+  constexpr bool CPLX = sizeof(T) == sizeof(cd);
+  Ctx<NDIM, NS, T> c;
+  c.hdr = h;
+  c.coef = reinterpret_cast<const double *>(h + 1);
+  c.exps = reinterpret_cast<const uint32_t *>(c.coef + (h->nU + h->nF));
+  c.aU0 = p.aU0; c.aU1 = p.aU1; c.aF0 = p.aF0; c.aF1 = p.aF1;
+  c.lambda = p.lambda;
+  c.cntImF = 0; c.cntReU = 0;
+  c.G0 = 1.0;
+  c.L0 = 0.0;
+#pragma unroll
+  for (int k = 0; k < NDIM; ++k) {
+    int j = h->perm[k];
+    double tk = pt[(0 * NDIM + j) * QMC_THREADS];
+    c.t[k] = tk;
+    if (CPLX) c.invt_all[k] = pt[(2 * NDIM + j) * QMC_THREADS];
+    if (k < NS) {
+      double L = (double)h->beta[k] * pt[(1 * NDIM + j) * QMC_THREADS];
+      c.invt[k] = pt[(2 * NDIM + j) * QMC_THREADS];
+      c.invbeta[k] = 1.0 / (double)h->beta[k];
+      c.cL[k][0] = 1.0;
+#pragma unroll
+      for (int q = 1; q < K; ++q) c.cL[k][q] = c.cL[k][q - 1] * L * (1.0 / q);
+    } else {
+      int a = h->alpha[k], b = h->beta[k];
+      if (a) c.G0 *= ipow_pos(tk, a);
+      if (b) c.L0 += (double)b * pt[(1 * NDIM + j) * QMC_THREADS];
+    }
+  }
+  if (!CPLX) {
+    // partial sums per group, then subset sums: PU[X] = sum of the monomials depending only on singular
+    // variables inside X  =  U^(t with the singular variables outside X set to 0)
+    int idx = 0;
+#pragma unroll
+    for (int g = 0; g < (1 << NS); ++g) {
+      double s = 0.0;
+      int n = h->cntU[g];
+      for (int q = 0; q < n; ++q, ++idx) s += monomial<NDIM>(c.coef[idx], c.exps[idx], c.t);
+      c.PU[g] = s;
+    }
+#pragma unroll
+    for (int g = 0; g < (1 << NS); ++g) {
+      double s = 0.0;
+      int n = h->cntF[g];
+      for (int q = 0; q < n; ++q, ++idx) s += monomial<NDIM>(c.coef[idx], c.exps[idx], c.t);
+      c.PF[g] = s;
+    }
+#pragma unroll
+    for (int b = 0; b < NS; ++b)
+#pragma unroll
+      for (int X = 0; X < (1 << NS); ++X)
+        if (X >> b & 1) {
+          c.PU[X] += c.PU[X ^ (1 << b)];
+          c.PF[X] += c.PF[X ^ (1 << b)];
+        }
+  }
+  Fold<NDIM, NS, K, 0, 0, T>::eval(c, res);
+  cntImF += c.cntImF;
+  cntReU += c.cntReU;
+}
+
+__device__ __forceinline__ bool finite_all(double v) { return fabs(v) <= 1.79769313486231570e308; }
+__device__ __forceinline__ bool finite_all(cd v) { return finite_all(v.re) && finite_all(v.im); }
+
+// TMA bulk copy global -> shared, completion on an mbarrier (sm_90+; SASS: UBLKCP)
+__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count) {
+  unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(a), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes) {
+  unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(a), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_bulk_g2s(void *dst, const void *src, unsigned bytes, uint64_t *bar) {
+  unsigned d = (unsigned)__cvta_generic_to_shared(dst), b = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(d),
+               "l"(src), "r"(bytes), "r"(b)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity) {
+  unsigned a = (unsigned)__cvta_generic_to_shared(bar), ok = 0;
+  while (!ok) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(ok)
+        : "r"(a), "r"(parity)
+        : "memory");
+  }
+}
+
+// deterministic block sum: warp shuffle tree, then pairwise tree over the warp results in shared memory
+__device__ __forceinline__ double block_sum(double v, double *scratch /*[QMC_THREADS/32]*/) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  __syncthreads();
+  if (lane == 0) scratch[wid] = v;
+  __syncthreads();
+  double r = 0.0;
+  if (wid == 0) {
+    r = (lane < QMC_THREADS / 32) ? scratch[lane] : 0.0;
+#pragma unroll
+    for (int o = (QMC_THREADS / 64); o > 0; o >>= 1) r += __shfl_down_sync(0xffffffffu, r, o);
+  }
+  return r;  // valid in thread 0
+}
+
+}  // namespace qmcdev
+
+// ================================================================================================
+template <int NDIM, int KMAX, bool CPLX>
+__global__ void __launch_bounds__(QMC_THREADS) qmc_eval_kernel(const QmcLaunch p) {
+  using namespace qmcdev;
+  typedef typename std::conditional<CPLX, cd, double>::type T;
+  constexpr int NACC = QMC_MAXSING + KMAX + 1;  // accumulator a <-> order a - QMC_MAXSING
+  constexpr int NC = CPLX ? 2 : 1;
+  constexpr int SMAX = NDIM < QMC_MAXSING ? NDIM : QMC_MAXSING;
+
+  extern __shared__ __align__(16) unsigned char smem[];
+  const int tid = threadIdx.x;
+  const int chunk = blockIdx.y;
+  const int s0 = p.sec_begin + chunk * p.sec_per_chunk;
+  const int s1 = min(s0 + p.sec_per_chunk, p.sec_end);
+  const int nsec = s1 - s0;
+
+  // shared memory carve-up
+  unsigned char *tab = smem;                                                   // table chunk
+  uint32_t *soff = reinterpret_cast<uint32_t *>(smem + p.tab_smem_bytes);     // [nsec+1] offsets
+  size_t o = p.tab_smem_bytes + (((size_t)(p.sec_per_chunk + 1) * 4 + 15) & ~(size_t)15);
+  uint64_t *bar = reinterpret_cast<uint64_t *>(smem + o);
+  o += 16;
+  double *shf = reinterpret_cast<double *>(smem + o);                          // [m][NDIM]
+  o += (((size_t)p.m * NDIM * 8) + 15) & ~(size_t)15;
+  double *scratch = reinterpret_cast<double *>(smem + o);                      // [QMC_THREADS/32]
+  o += (QMC_THREADS / 32) * 8;
+  double *ptbase = reinterpret_cast<double *>(smem + o);                       // [3][NDIM][QMC_THREADS]
+  o += (size_t)3 * NDIM * QMC_THREADS * 8;
+  double *sacc = reinterpret_cast<double *>(smem + o);                         // persec: [nsec][NACC*NC][QMC_THREADS]
+  double *pt = ptbase + tid;
+
+  // stage the chunk's tables: one TMA bulk copy, completion on an mbarrier
+  const uint32_t g0 = p.secoff[s0], g1 = p.secoff[s1];
+  if (tid == 0) {
+    mbar_init(bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (tid == 0) {
+    mbar_expect_tx(bar, g1 - g0);
+    tma_bulk_g2s(tab, p.image + g0, g1 - g0, bar);
+  }
+  for (int i = tid; i <= nsec; i += QMC_THREADS) soff[i] = p.secoff[s0 + i] - g0;
+  for (int i = tid; i < p.m * NDIM; i += QMC_THREADS) shf[i] = p.shifts[i];
+  mbar_wait(bar, 0);
+  __syncthreads();
+
+  const uint32_t N = p.N;
+  const double dN = (double)N;
+  const uint32_t stride = gridDim.x * QMC_THREADS;
+  uint32_t dz[NDIM];
+#pragma unroll
+  for (int j = 0; j < NDIM; ++j) dz[j] = (uint32_t)(((uint64_t)stride * p.zeff[j]) % N);
+
+  unsigned cntImF = 0, cntReU = 0, cntNonFinite = 0, cntBoundary = 0;
+
+  for (int kap = 0; kap < p.m; ++kap) {
+    T acc[NACC];
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) acc[a] = Num<T>::zero();
+    if (p.persec)
+      for (int i = 0; i < nsec * NACC * NC; ++i) sacc[(size_t)i * QMC_THREADS + tid] = 0.0;
+
+    uint32_t cidx = blockIdx.x * QMC_THREADS + tid;
+    uint32_t r[NDIM];
+#pragma unroll
+    for (int j = 0; j < NDIM; ++j) r[j] = (uint32_t)((p.off[j] + (uint64_t)cidx * p.zeff[j]) % N);
+
+    for (; cidx < p.count; cidx += stride) {
+      // S1-S3: lattice point (Eq. 17), shift + wrap (Eq. 18), periodising transform (Eq. 21)
+      double w = 1.0;
+      bool inside = true;
+#pragma unroll
+      for (int j = 0; j < NDIM; ++j) {
+        double u = (double)r[j] / dN;
+        double y = u + shf[kap * NDIM + j];
+        if (y >= 1.0) y -= 1.0;
+        double tj;
+        if (p.transform == 0) {
+          tj = y * y * (3.0 - 2.0 * y);
+          w *= 6.0 * y * (1.0 - y);
+        } else {
+          tj = 1.0 - fabs(2.0 * y - 1.0);
+        }
+        if (!(y > 0.0) || !(tj > 0.0)) inside = false;
+        pt[(0 * NDIM + j) * QMC_THREADS] = tj;
+        pt[(1 * NDIM + j) * QMC_THREADS] = log(tj);
+        pt[(2 * NDIM + j) * QMC_THREADS] = 1.0 / tj;
+        uint32_t rn = r[j] + dz[j];  // r, dz < N < 2^31: no wrap
+        r[j] = rn >= N ? rn - N : rn;
+      }
+      if (!inside) {
+        if (chunk == 0) ++cntBoundary;
+        continue;
+      }
+      // S4-S6: all sectors of the chunk at this point
+      for (int si = 0; si < nsec; ++si) {
+        const QmcSectorHdr *h = reinterpret_cast<const QmcSectorHdr *>(tab + soff[si]);
+        const int ns = h->nsing;
+        T contrib[NACC];
+#pragma unroll
+        for (int a = 0; a < NACC; ++a) contrib[a] = Num<T>::zero();
+        bool fin = true;
+#define QMC_CASE(NS_)                                                                   \
+  case NS_: {                                                                           \
+    if (NS_ <= SMAX) {                                                                  \
+      constexpr int NSC = NS_ <= SMAX ? NS_ : 0;                                        \
+      T res[KMAX + NSC + 1];                                                            \
+      sector_eval<NDIM, NSC, KMAX, T>(p, h, pt, res, cntImF, cntReU);                   \
+      _Pragma("unroll") for (int i = 0; i < KMAX + NSC + 1; ++i) {                      \
+        fin = fin && finite_all(res[i]);                                                \
+        contrib[QMC_MAXSING - NSC + i] = res[i];                                        \
+      }                                                                                 \
+    }                                                                                   \
+  } break;
+        switch (ns) {
+          QMC_CASE(0)
+          QMC_CASE(1)
+          QMC_CASE(2)
+          QMC_CASE(3)
+          QMC_CASE(4)
+          default:
+            break;
+        }
+#undef QMC_CASE
+        if (!fin) {
+          ++cntNonFinite;
+          continue;
+        }
+        if (!p.persec) {
+#pragma unroll
+          for (int a = 0; a < NACC; ++a) acc[a] = acc[a] + Num<T>::scale(w, contrib[a]);
+        } else {
+          double *sa = sacc + ((size_t)si * NACC * NC) * QMC_THREADS + tid;
+#pragma unroll
+          for (int a = 0; a < NACC; ++a) {
+            if (CPLX) {
+              const cd *cc = reinterpret_cast<const cd *>(&contrib[a]);
+              sa[(size_t)(2 * a) * QMC_THREADS] += w * cc->re;
+              sa[(size_t)(2 * a + 1) * QMC_THREADS] += w * cc->im;
+            } else {
+              sa[(size_t)a * QMC_THREADS] += w * *reinterpret_cast<const double *>(&contrib[a]);
+            }
+          }
+        }
+      }
+    }
+
+    // S7: block reduction -> one partial per (chunk | sector, shift, block)
+    if (!p.persec) {
+      double *dst = p.partial + (((size_t)chunk * p.m + kap) * gridDim.x + blockIdx.x) * (NACC * NC);
+#pragma unroll
+      for (int a = 0; a < NACC; ++a) {
+        if (CPLX) {
+          const cd *cc = reinterpret_cast<const cd *>(&acc[a]);
+          double sr = block_sum(cc->re, scratch);
+          double si = block_sum(cc->im, scratch);
+          if (tid == 0) {
+            dst[2 * a] = sr;
+            dst[2 * a + 1] = si;
+          }
+        } else {
+          double sr = block_sum(*reinterpret_cast<const double *>(&acc[a]), scratch);
+          if (tid == 0) dst[a] = sr;
+        }
+      }
+    } else {
+      for (int si = 0; si < nsec; ++si) {
+        double *dst = p.partial + (((size_t)(s0 - p.sec_begin + si) * p.m + kap) * gridDim.x + blockIdx.x) * (NACC * NC);
+        for (int a = 0; a < NACC * NC; ++a) {
+          double v = block_sum(sacc[((size_t)si * NACC * NC + a) * QMC_THREADS + tid], scratch);
+          if (tid == 0) dst[a] = v;
+        }
+      }
+    }
+  }
+
+  // counters (integers: order-independent)
+  unsigned c4[4] = {cntImF, cntReU, cntNonFinite, cntBoundary};
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    unsigned v = c4[q];
+#pragma unroll
+    for (int o2 = 16; o2 > 0; o2 >>= 1) v += __shfl_down_sync(0xffffffffu, v, o2);
+    if ((tid & 31) == 0 && v) atomicAdd(p.counters + q, (unsigned long long)v);
+  }
+}

@@ -1,0 +1,349 @@
+// qmc_prepare: Feynman graph -> Symanzik polynomials -> primary sectors -> iterated sub-sectors -> sector tables.
+// Host only.  arXiv:1508.02512 Sec. 2.  "P:<n>" = PAPER.md line, "R:Cxx" = DESIGN.md reading.
+//
+// Written independently of oracle/ (no shared code): polynomials are flat sorted vectors with exponents packed
+// 4 bits per variable; U comes from a deletion-contraction recursion, F from U of the graphs with two leg
+// vertices identified; the decomposition runs on an explicit stack.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+
+#include "../../include/qmc_feynman.h"
+#include "qmc_tables.h"
+
+namespace {
+
+typedef uint64_t Key;  // exponent of variable j in bits [4j, 4j+4)
+struct Term {
+  Key k;
+  double c;
+};
+typedef std::vector<Term> Poly;
+
+inline int expo(Key k, int j) { return (int)((k >> (4 * j)) & 15u); }
+inline Key unit(int j) { return (Key)1 << (4 * j); }
+
+void canonical(Poly &p) {
+  std::sort(p.begin(), p.end(), [](const Term &a, const Term &b) { return a.k < b.k; });
+  size_t w = 0;
+  for (size_t r = 0; r < p.size();) {
+    Key k = p[r].k;
+    double c = 0.0;
+    while (r < p.size() && p[r].k == k) c += p[r++].c;
+    if (c != 0.0) p[w++] = Term{k, c};
+  }
+  p.resize(w);
+}
+
+struct Edge {
+  int u, v, idx;
+};
+
+// sum over spanning trees T of prod_{e not in T} x_e, by deletion / contraction of the last edge
+void dual_kirchhoff(int nv, std::vector<Edge> edges, Key carry, Poly &out) {
+  if (edges.empty()) {
+    if (nv == 1) out.push_back(Term{carry, 1.0});
+    return;
+  }
+  Edge e = edges.back();
+  edges.pop_back();
+  // e not in the tree: factor x_e, graph without e
+  dual_kirchhoff(nv, edges, carry + unit(e.idx), out);
+  if (e.u == e.v) return;  // a self-loop is never in a tree
+  // e in the tree: contract (merge the larger label into the smaller, close the gap)
+  int keep = std::min(e.u, e.v), drop = std::max(e.u, e.v);
+  for (Edge &f : edges) {
+    if (f.u == drop) f.u = keep;
+    if (f.v == drop) f.v = keep;
+    if (f.u > drop) --f.u;
+    if (f.v > drop) --f.v;
+  }
+  dual_kirchhoff(nv - 1, edges, carry, out);
+}
+
+Poly spanning_poly(int nv, const std::vector<Edge> &edges) {
+  Poly p;
+  dual_kirchhoff(nv, edges, 0, p);
+  canonical(p);
+  return p;
+}
+
+struct Node {  // one (sub-)sector under construction
+  int primary;
+  Poly U, F;
+  int alpha[QMC_MAXDIM], beta[QMC_MAXDIM];
+  int depth;
+};
+
+bool constant_term(const Poly &p) { return !p.empty() && p.front().k == 0; }  // sorted: key 0 first
+
+// rule R:C7 step 1: divide the common monomial out of Q and book its exponents
+void pull_common(Poly &Q, int n, int a0, int a1, int *alpha, int *beta) {
+  for (int j = 0; j < n; ++j) {
+    int lo = 15;
+    for (const Term &t : Q) lo = std::min(lo, expo(t.k, j));
+    if (lo == 0 || Q.empty()) continue;
+    for (Term &t : Q) t.k -= (Key)lo << (4 * j);
+    alpha[j] += lo * a0;
+    beta[j] += lo * a1;
+  }
+  canonical(Q);
+}
+
+// rule R:C7 step 3: smallest set of variables hitting every monomial; ties -> lexicographically smallest tuple.
+// Sets are bit masks; tuple order: at the lowest differing bit, the set owning that bit is smaller.
+unsigned smallest_hitting_set(const Poly &target, int n) {
+  std::vector<unsigned> supp;
+  for (const Term &t : target) {
+    unsigned s = 0;
+    for (int j = 0; j < n; ++j)
+      if (expo(t.k, j)) s |= 1u << j;
+    supp.push_back(s);
+  }
+  unsigned best = 0;
+  int best_size = n + 1;
+  for (unsigned S = 1; S < (1u << n); ++S) {
+    int size = __builtin_popcount(S);
+    if (size > best_size) continue;
+    bool hits = true;
+    for (unsigned s : supp)
+      if (!(s & S)) {
+        hits = false;
+        break;
+      }
+    if (!hits) continue;
+    bool better = size < best_size;
+    if (!better) {
+      unsigned diff = S ^ best;
+      better = (S & (diff & (~diff + 1u))) != 0;
+    }
+    if (better) {
+      best = S;
+      best_size = size;
+    }
+  }
+  return best;
+}
+
+}  // namespace
+
+int qmc_build_tables(const qmc_graph *g, const qmc_kinematics *kin, int eps_order, const qmc_options *opt,
+                     qmc_tables *T) {
+  if (!g || !kin || !kin->gram || !T) return QMC_EINVAL;
+  const int V = g->n_vertices, P = g->n_edges, NL = g->n_legs;
+  if (V < 1 || P < 2 || NL < 0 || P - 1 > QMC_MAXDIM) return QMC_EINVAL;
+  if (eps_order < 0) return QMC_EINVAL;
+  if (eps_order > QMC_KMAX_MAX) return QMC_EUNSUPPORTED;
+  for (int e = 0; e < P; ++e) {
+    if (g->edge_u[e] < 0 || g->edge_u[e] >= V || g->edge_v[e] < 0 || g->edge_v[e] >= V) return QMC_EINVAL;
+    if (g->edge_nu && g->edge_nu[e] != 1) return QMC_EUNSUPPORTED;
+  }
+  for (int a = 0; a < NL; ++a)
+    if (g->leg_vertex[a] < 0 || g->leg_vertex[a] >= V) return QMC_EINVAL;
+  const int L = P - V + 1;
+  if (L < 1) return QMC_EINVAL;
+
+  // ---- Symanzik polynomials --------------------------------------------------------------
+  std::vector<Edge> edges;
+  for (int e = 0; e < P; ++e) edges.push_back(Edge{g->edge_u[e], g->edge_v[e], e});
+  Poly U = spanning_poly(V, edges);
+  if (U.empty()) return QMC_EINVAL;  // disconnected graph
+  // F0 = - sum_{2-forests} (p_T1)^2 prod x = sum_{a<b} (p_a.p_b) * [2-forests separating v_a, v_b]  (momentum
+  // conservation), and the bracket is the spanning polynomial of the graph with v_a and v_b identified.
+  Poly F;
+  double scale = 0.0;
+  for (int i = 0; i < NL * NL; ++i) scale = std::max(scale, std::fabs(kin->gram[i]));
+  for (int a = 0; a < NL; ++a)
+    for (int b = a + 1; b < NL; ++b) {
+      int va = g->leg_vertex[a], vb = g->leg_vertex[b];
+      double dot = kin->gram[a * NL + b];
+      if (va == vb || dot == 0.0) continue;
+      int keep = std::min(va, vb), drop = std::max(va, vb);
+      std::vector<Edge> merged = edges;
+      for (Edge &f : merged) {
+        if (f.u == drop) f.u = keep;
+        if (f.v == drop) f.v = keep;
+        if (f.u > drop) --f.u;
+        if (f.v > drop) --f.v;
+      }
+      Poly phi = spanning_poly(V - 1, merged);
+      for (const Term &t : phi) F.push_back(Term{t.k, dot * t.c});
+    }
+  canonical(F);
+  {  // kinematic zeros must be exact (R:C24): drop rounding residues of the Gram matrix
+    Poly kept;
+    for (const Term &t : F)
+      if (std::fabs(t.c) > 1e-12 * scale) kept.push_back(t);
+    F.swap(kept);
+  }
+  for (int e = 0; e < P; ++e) {  // + U * sum_e m_e^2 x_e
+    double m2 = g->edge_m2 ? g->edge_m2[e] : 0.0;
+    if (m2 == 0.0) continue;
+    for (const Term &t : U) F.push_back(Term{t.k + unit(e), m2 * t.c});
+  }
+  canonical(F);
+  if (F.empty()) return QMC_EINVAL;  // scaleless integral
+
+  // ---- exponents (Eq. 6, D = 4 - 2 eps, nu_j = 1) -----------------------------------------
+  T->n = P - 1;
+  T->P = P;
+  T->L = L;
+  T->aU0 = P - 2 * (L + 1);
+  T->aU1 = L + 1;
+  T->aF0 = -(P - 2 * L);
+  T->aF1 = -L;
+  T->lambda = opt ? opt->lambda : 0.0;
+  T->transform = opt ? opt->transform : 0;
+  if (T->lambda < 0.0 || (T->transform != 0 && T->transform != 1)) return QMC_EINVAL;
+  const int max_depth = (opt && opt->max_depth > 0) ? opt->max_depth : 64;
+  const int n = T->n;
+  T->kmax = eps_order;
+  T->sectors.clear();
+
+  // ---- primary sectors (Eqs. 3-6) and iterated decomposition (Eqs. 7-9), depth first ------------
+  std::vector<Node> stack;
+  for (int l = P - 1; l >= 0; --l) {  // pushed in reverse so that primary sector 0 is processed first
+    Node nd;
+    nd.primary = l;
+    nd.depth = 0;
+    std::memset(nd.alpha, 0, sizeof nd.alpha);
+    std::memset(nd.beta, 0, sizeof nd.beta);
+    for (int which = 0; which < 2; ++which) {
+      const Poly &Q = which ? F : U;
+      Poly &R = which ? nd.F : nd.U;
+      for (const Term &t : Q) {  // x_l = 1, the others renamed t_1..t_{P-1} in increasing order (Eq. 4)
+        Key lowmask = ((Key)1 << (4 * l)) - 1;
+        Key k = (t.k & lowmask) | ((t.k >> (4 * (l + 1))) << (4 * l));
+        R.push_back(Term{k, t.c});
+      }
+      canonical(R);
+    }
+    stack.push_back(nd);
+  }
+  int smax = 0;
+  while (!stack.empty()) {
+    Node nd = stack.back();
+    stack.pop_back();
+    pull_common(nd.U, n, T->aU0, T->aU1, nd.alpha, nd.beta);
+    pull_common(nd.F, n, T->aF0, T->aF1, nd.alpha, nd.beta);
+    const Poly *target = !constant_term(nd.U) ? &nd.U : (!constant_term(nd.F) ? &nd.F : nullptr);
+    if (!target) {  // emit
+      QmcSector s;
+      s.primary = nd.primary;
+      s.nsing = 0;
+      std::memset(s.alpha, 0, sizeof s.alpha);
+      std::memset(s.beta, 0, sizeof s.beta);
+      for (int j = 0; j < n; ++j) {
+        s.alpha[j] = nd.alpha[j];
+        s.beta[j] = nd.beta[j];
+        if (nd.alpha[j] <= -2) return QMC_EUNSUPPORTED;  // R:C9
+        if (nd.alpha[j] == -1) {
+          if (nd.beta[j] == 0) return QMC_EUNSUPPORTED;
+          ++s.nsing;
+        }
+        if (nd.alpha[j] > 127 || nd.beta[j] > 127 || nd.beta[j] < -127) return QMC_EUNSUPPORTED;
+      }
+      if (s.nsing > QMC_MAXSING) return QMC_EUNSUPPORTED;
+      smax = std::max(smax, s.nsing);
+      for (int which = 0; which < 2; ++which)
+        for (const Term &t : (which ? nd.F : nd.U)) {
+          QmcMono m;
+          m.c = t.c;
+          for (int j = 0; j < QMC_MAXDIM; ++j) m.e[j] = (uint8_t)(j < n ? expo(t.k, j) : 0);
+          (which ? s.F : s.U).push_back(m);
+        }
+      if (s.U.size() > 255 || s.F.size() > 255) return QMC_EUNSUPPORTED;
+      T->sectors.push_back(s);
+      continue;
+    }
+    if (nd.depth >= max_depth) return QMC_EDEPTH;
+    unsigned S = smallest_hitting_set(*target, n);
+    if (!S) return QMC_EDEPTH;
+    int size = __builtin_popcount(S);
+    for (int k = n - 1; k >= 0; --k) {  // children in increasing k => push in decreasing k
+      if (!(S >> k & 1u)) continue;
+      Node ch;
+      ch.primary = nd.primary;
+      ch.depth = nd.depth + 1;
+      std::memcpy(ch.alpha, nd.alpha, sizeof ch.alpha);
+      std::memcpy(ch.beta, nd.beta, sizeof ch.beta);
+      for (int j = 0; j < n; ++j)
+        if ((S >> j & 1u) && j != k) {  // t_j -> t_k t_j
+          ch.alpha[k] += nd.alpha[j];
+          ch.beta[k] += nd.beta[j];
+        }
+      ch.alpha[k] += size - 1;  // Jacobian t_k^{|S|-1} (a monomial)
+      for (int which = 0; which < 2; ++which) {
+        const Poly &Q = which ? nd.F : nd.U;
+        Poly &R = which ? ch.F : ch.U;
+        R.reserve(Q.size());
+        for (const Term &t : Q) {
+          int add = 0;
+          for (int j = 0; j < n; ++j)
+            if ((S >> j & 1u) && j != k) add += expo(t.k, j);
+          if (expo(t.k, k) + add > 15) return QMC_EUNSUPPORTED;
+          R.push_back(Term{t.k + ((Key)add << (4 * k)), t.c});
+        }
+        canonical(R);
+      }
+      stack.push_back(ch);
+    }
+  }
+  T->kmin = -smax;
+  if (T->kmax - T->kmin + 1 > QMC_MAXK) return QMC_EUNSUPPORTED;
+
+  // ---- device image -----------------------------------------------------------------------------
+  T->image.clear();
+  T->secoff.clear();
+  for (QmcSector &s : T->sectors) {
+    QmcSectorHdr h;
+    std::memset(&h, 0, sizeof h);
+    int pos = 0, inv[QMC_MAXDIM];
+    for (int pass = 0; pass < 2; ++pass)
+      for (int j = 0; j < n; ++j)
+        if ((s.alpha[j] == -1) == (pass == 0)) {
+          h.perm[pos] = (uint8_t)j;
+          inv[j] = pos;
+          h.alpha[pos] = (int8_t)s.alpha[j];
+          h.beta[pos] = (int8_t)s.beta[j];
+          ++pos;
+        }
+    h.nsing = (uint8_t)s.nsing;
+    auto group_of = [&](const QmcMono &m) {
+      int gmask = 0;
+      for (int b = 0; b < s.nsing; ++b)
+        if (m.e[h.perm[b]]) gmask |= 1 << b;
+      return gmask;
+    };
+    for (int which = 0; which < 2; ++which) {
+      std::vector<QmcMono> &M = which ? s.F : s.U;
+      std::stable_sort(M.begin(), M.end(), [&](const QmcMono &a, const QmcMono &b) { return group_of(a) < group_of(b); });
+      for (const QmcMono &m : M) {
+        uint8_t &cnt = (which ? h.cntF : h.cntU)[group_of(m)];
+        ++cnt;
+        for (int j = 0; j < n; ++j)
+          if (m.e[j] >= 2) h.flags |= 1;
+      }
+    }
+    h.nU = (uint8_t)s.U.size();
+    h.nF = (uint8_t)s.F.size();
+    T->secoff.push_back((uint32_t)T->image.size());
+    const uint8_t *hb = reinterpret_cast<const uint8_t *>(&h);
+    T->image.insert(T->image.end(), hb, hb + sizeof h);
+    for (int which = 0; which < 2; ++which)
+      for (const QmcMono &m : (which ? s.F : s.U)) {
+        const uint8_t *cb = reinterpret_cast<const uint8_t *>(&m.c);
+        T->image.insert(T->image.end(), cb, cb + 8);
+      }
+    for (int which = 0; which < 2; ++which)
+      for (const QmcMono &m : (which ? s.F : s.U)) {
+        uint32_t w = 0;
+        for (int j = 0; j < n; ++j) w |= (uint32_t)m.e[j] << (4 * inv[j]);
+        const uint8_t *wb = reinterpret_cast<const uint8_t *>(&w);
+        T->image.insert(T->image.end(), wb, wb + 4);
+      }
+    while (T->image.size() % 16) T->image.push_back(0);
+  }
+  T->secoff.push_back((uint32_t)T->image.size());
+  return QMC_OK;
+}

@@ -1,0 +1,149 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same seeded
+inputs -- same tables (exported data), same generating vector, same shifts.
+
+Tolerance (reading C19): |S_gpu - S_oracle| <= 1e-12 * max(|S_oracle|, A * 2^-10),
+A = the un-cancelled magnitude the oracle accumulates next to S.  Integer counters must match exactly.
+"""
+import numpy as np
+import pytest
+
+import qmc_inputs as qi
+import paper_1508_02512_b200 as q
+from oracle import Oracle
+
+pytestmark = pytest.mark.gpu
+
+RTOL = 1e-12
+
+
+def check(got, want, A, what):
+    tol = RTOL * np.maximum(np.abs(want), A * 2.0 ** -10)
+    bad = np.abs(got - want) > tol
+    used_floor = np.abs(want) < A * 2.0 ** -10
+    assert not bad.any(), (what, int(bad.sum()), np.abs(got - want)[bad][:5], tol[bad][:5], want[bad][:5])
+    return int(used_floor.sum())
+
+
+def parity(wl, N, m, z=None, index_range=None, sectors=None, transform=0, shifts=None, eps_order=None):
+    eo = wl.eps_order if eps_order is None else eps_order
+    t = q.qmc_prepare(wl, eps_order=eo, lam=wl.lam, transform=transform)
+    o = Oracle.from_tables(t.export())
+    if z is None:
+        z = qi.good_vector(N, t.dim)
+    sh = qi.splitmix64_shifts(wl.seed, m, t.dim) if shifts is None else shifts
+    S, A, cnt = o.integrate(N, z, sh, transform=transform, index_range=index_range, sectors=sectors)
+    r = q.qmc_integrate(t, N, m, z=z, shifts=sh, index_range=index_range, sectors=sectors, per_sector=True)
+    assert r.mode_used == 2 and r.shift_sums.shape == S.shape
+    nfloor = check(r.shift_sums, S, A, wl.name + " per-sector")
+    assert np.array_equal(r.counters, cnt), (r.counters, cnt)
+    # fused mode (the throughput mode): per-shift totals over sectors
+    f = q.qmc_integrate(t, N, m, z=z, shifts=sh, index_range=index_range, sectors=sectors, per_sector=False)
+    assert f.mode_used == 1
+    check(f.shift_totals, S.sum(axis=0), A.sum(axis=0), wl.name + " fused")
+    check(r.shift_totals, S.sum(axis=0), A.sum(axis=0), wl.name + " per-sector totals")
+    # S8: statistics
+    coeff, err = o.totals(S)
+    assert np.allclose(r.coeff, coeff, rtol=1e-10, atol=1e-13 * np.abs(A.sum(axis=0)).max())
+    assert np.allclose(f.err.real, err.real, rtol=1e-6, atol=1e-15) and np.allclose(f.err.imag, err.imag, rtol=1e-6, atol=1e-15)
+    return r, f, S, A, nfloor
+
+
+def test_config1_bubble():
+    parity(qi.bubble(), 10007, 10)
+    parity(qi.bubble(), 10007, 10, eps_order=2)
+
+
+def test_triangle_double_pole():
+    parity(qi.triangle(), 99991, 4)
+
+
+def test_config2_massless_box():
+    r, f, S, A, _ = parity(qi.massless_box(), 99991, 6)
+    # closed form within 3 sigma on the GPU result itself (level 2)
+    ex = [0.666666666666667, -1.2639198230760183, -1.2238036181980894]
+    assert np.all(np.abs(f.coeff.real - ex) <= 3 * f.err.real + 1e-13)
+
+
+def test_config2_eps1_and_tent_transform():
+    parity(qi.massless_box(), 32749, 3, eps_order=1)
+    parity(qi.massless_box(), 16381, 3, transform=1)
+
+
+def test_config3_massive_box_complex():
+    r, f, S, A, _ = parity(qi.massive_box(), 99991, 6)
+    ref = 0.29347155740583 + 0.33214829595148j       # Gauss-Legendre pin of tests/test_oracle_deformation.py
+    assert abs(f.coeff[0].real - ref.real) <= 3 * f.err[0].real and abs(f.coeff[0].imag - ref.imag) <= 3 * f.err[0].imag
+
+
+def test_config4_double_box_all_sectors_small_N():
+    parity(qi.double_box(), 16381, 2)
+
+
+def test_config4_sector_subset_many_points_per_thread():
+    # enough points that every thread walks several lattice indices (grid-stride tail included)
+    parity(qi.double_box(), 999983, 2, sectors=(120, 126))
+
+
+def test_config4_full_size_strided_indices():
+    # BASELINE size N = 999983, all 293 sectors, every 61st lattice index
+    N = 999983
+    parity(qi.double_box(), N, 2, index_range=(7, 61, (N - 7 + 60) // 61))
+
+
+def test_config5_nonplanar_vertex_complex():
+    parity(qi.nonplanar_vertex(), 16381, 4)
+    parity(qi.nonplanar_vertex(), 131071, 2, sectors=(20, 28))
+
+
+def test_paper_table1_kinematics():
+    parity(qi.double_box(-2 / 3, -2 / 3, p2=(0, 0, -1, -1)), 16381, 2, sectors=(0, 60))
+
+
+def test_edge_cases_boundary_points_and_tiny_lattices():
+    wl = qi.massless_box()
+    # a zero shift component puts lattice index 0 on the boundary: contributes exactly 0, counted
+    sh = qi.splitmix64_shifts(3, 3, 3)
+    sh[1, 2] = 0.0
+    r, f, S, A, _ = parity(wl, 1021, 3, z=qi.korobov_vector(1021, 3, 331), shifts=sh)
+    assert r.counters[3] == 1
+    parity(wl, 5, 2, z=np.array([1, 2, 3], dtype=np.uint64))
+    parity(wl, 257, 2, z=qi.korobov_vector(257, 3, 3))
+
+
+def test_invalid_arguments():
+    t = q.qmc_prepare(qi.massless_box())
+    with pytest.raises(q.QmcError) as e:
+        q.qmc_integrate(t, 1000, 4, z=[1, 10, 100])          # z_j not coprime to N
+    assert e.value.status == -1
+    with pytest.raises(q.QmcError) as e:
+        q.qmc_integrate(t, 1021, 1)                          # Eq. 20 needs m >= 2
+    assert e.value.status == -1
+
+
+def test_library_generating_vector_and_seeded_shifts():
+    t = q.qmc_prepare(qi.massless_box())
+    N = 99991
+    z = q.qmc_generating_vector(N, 3)
+    assert z[0] == 1 and all(np.gcd(int(v), N) == 1 for v in z)
+    assert int(z[2]) == (int(z[1]) * int(z[1])) % N          # Korobov form
+    a = q.qmc_integrate(t, N, 8, seed=7)
+    b = q.qmc_integrate(t, N, 8, z=z, shifts=qi.splitmix64_shifts(7, 8, 3))
+    assert np.array_equal(a.shift_totals, b.shift_totals)     # deterministic, same inputs
+    c = q.qmc_integrate(t, N, 8, seed=7)
+    assert np.array_equal(a.shift_totals, c.shift_totals)     # run-to-run bit reproducible
+    ex = [0.666666666666667, -1.2639198230760183, -1.2238036181980894]
+    assert np.all(np.abs(a.coeff.real - ex) <= 3.5 * a.err.real)
+    assert np.all(a.err.real < 1e-5)
+
+
+def test_double_box_poles_on_gpu_at_baseline_size():
+    """Level 2 at a BASELINE.json size: N = 999983, m = 20, seed 13, fused mode (the bench configuration)."""
+    t = q.qmc_prepare(qi.double_box())
+    r = q.qmc_integrate(t, 999983, 20, seed=13)
+    ex = [2.0 / 9.0, -0.8497687147780183, 0.003001503361321066]     # tests/test_oracle_closed_forms.py (mpmath)
+    assert np.all(np.abs(r.coeff.real[:3] - ex) <= 3.5 * r.err.real[:3])
+    assert np.all(r.err.real < [1e-6, 1e-5, 1e-4, 1e-3, 1e-2])
+    assert not r.counters.any()
+    # fused and per-sector modes agree at full size
+    p = q.qmc_integrate(t, 999983, 20, seed=13, per_sector=True)
+    assert np.allclose(p.shift_totals, r.shift_totals, rtol=1e-11, atol=1e-13)
