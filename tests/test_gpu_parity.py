@@ -43,8 +43,9 @@ def parity(wl, N, m, z=None, index_range=None, sectors=None, transform=0, shifts
     check(r.shift_totals, S.sum(axis=0), A.sum(axis=0), wl.name + " per-sector totals")
     # S8: statistics
     coeff, err = o.totals(S)
-    assert np.allclose(r.coeff, coeff, rtol=1e-10, atol=1e-13 * np.abs(A.sum(axis=0)).max())
-    assert np.allclose(f.err.real, err.real, rtol=1e-6, atol=1e-15) and np.allclose(f.err.imag, err.imag, rtol=1e-6, atol=1e-15)
+    atol = 1e-13 * np.abs(A.sum(axis=0)).max()   # error bars are differences of per-shift values: absolute scale
+    assert np.allclose(r.coeff, coeff, rtol=1e-10, atol=atol)
+    assert np.allclose(f.err.real, err.real, rtol=1e-6, atol=atol) and np.allclose(f.err.imag, err.imag, rtol=1e-6, atol=atol)
     return r, f, S, A, nfloor
 
 
