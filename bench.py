@@ -1,0 +1,365 @@
+"""bench.py -- FP64 integrand evaluations per second of the QMC hot path (arXiv:1508.02512) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--N 999983] [--impl reference]
+
+One "step" = one pass of the whole hot path S1-S8 (lattice points, shifts, periodising transform, all sectors with
+their subtraction corners / contour deformation, per-shift reduction, statistics) over one batch: N lattice
+points x m shifts x all sectors of the workload.  One evaluation = one (lattice point, shift, sector) triple
+(BASELINE.md M1).  Prints ONE JSON line (rank 0).  DESIGN.md "Measurement" explains every key.
+
+N > 1 GPUs (torchrun): weak scaling over shift vectors -- every rank integrates its own block of m shift vectors of
+the one SplitMix64 stream (per-GPU work fixed), the per-shift totals are all-gathered (NCCL), Eqs. 19-20 run over all
+m x N_gpus estimates.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import qmc_inputs as qi  # noqa: E402  (seeded input generators only)
+
+METRIC = "fp64_integrand_evals_per_sec_all_sectors"
+UNIT = "evals/s"
+
+# default lattice size per config for the timed step (primes from BASELINE.md; cfg4's 999983 keeps a step ~1 s)
+DEFAULT_N = {1: 10007, 2: 9999991, 3: 9999991, 4: 999983, 5: 1048573}
+
+
+def workload(cfg: int):
+    return qi.CONFIGS()[cfg - 1]
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons with NVML every 100 ms while the timed region runs."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag = index, threading.Event()
+        self.mhz, self.reasons, self.max_mhz, self.power = [], set(), None, []
+
+    def run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+            names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40,
+                     "hw_power_brake_slowdown": 0x80, "sync_boost": 0x10, "applications_clocks_setting": 0x2}
+            while not self.stop_flag.is_set():
+                self.mhz.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+                try:
+                    self.power.append(nv.nvmlDeviceGetPowerUsage(h) / 1000.0)
+                except Exception:
+                    pass
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+                time.sleep(0.1)
+        except Exception as e:  # NVML missing: report that, never fail the bench
+            self.reasons.add(f"nvml_unavailable:{type(e).__name__}")
+
+    def summary(self):
+        self.stop_flag.set()
+        self.join(timeout=2.0)
+        return {"sm_mhz": float(np.median(self.mhz)) if self.mhz else None, "sm_max_mhz": self.max_mhz,
+                "power_w_max": max(self.power) if self.power else None, "samples": len(self.mhz),
+                "reasons": sorted(self.reasons)}
+
+
+def oracle_sample(wl, N, z, shifts, target_s: float):
+    """Time the oracle (as it stands, all host cores) on a bounded sample of the same workload: the first `count`
+    lattice indices of the rule, all sectors, the first m_s shift vectors.  Returns (evals/s, cores, description)."""
+    import oracle
+    o = oracle.Oracle.from_workload(wl)       # the oracle's own decomposition: no product code on this path
+    cores = oracle.max_threads()
+    m_s = min(2, shifts.shape[0])
+    count = max(cores * 4, 64)
+    t0 = time.perf_counter()
+    o.integrate(N, z, shifts[:m_s], index_range=(0, 1, count))
+    dt = time.perf_counter() - t0
+    rate = count * m_s * o.n_sectors / dt
+    count = int(min(N, max(count, target_s * rate / (m_s * o.n_sectors))))
+    t0 = time.perf_counter()
+    o.integrate(N, z, shifts[:m_s], index_range=(0, 1, count))
+    dt = time.perf_counter() - t0
+    val = count * m_s * o.n_sectors / dt
+    return val, cores, (f"{wl.name}: lattice indices 0..{count - 1} of N={N}, all {o.n_sectors} sectors, {m_s} shifts, "
+                        f"{dt:.1f} s on {cores} threads (OpenMP), g++ -O2")
+
+
+def test_vector(N: int, dim: int) -> np.ndarray:
+    """A valid generating vector without a GPU (reference arm): tabulated Korobov multiplier, else a fixed one."""
+    if dim == 1 or (N, dim) in qi.GOOD_KOROBOV:
+        return qi.good_vector(N, dim)
+    return qi.korobov_vector(N, dim, 76 if N > 76 else 2)
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on the same workload / metric; each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    wl = workload(args.config)
+    N = args.N or DEFAULT_N[args.config]
+    z = test_vector(N, wl.dim)
+    shifts = qi.splitmix64_shifts(wl.seed, wl.m, wl.dim)
+    import oracle
+    oracle.build()
+    per_step = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    vals, desc, cores = [], "", 0
+    for i in range(args.warmup + args.steps):
+        v, cores, desc = oracle_sample(wl, N, z, shifts, per_step)
+        if i >= args.warmup:
+            vals.append(v)
+    val = float(np.mean(vals))
+    n_sectors = oracle.Oracle.from_workload(wl).n_sectors
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * N * wl.m * n_sectors / val, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl.name, "N": N, "m": wl.m, "seed": wl.seed, "n_sectors": n_sectors,
+                       "note": "ms_per_step extrapolated from the bounded sample (cost is linear in N*m)"},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def shift_block(seed: int, m: int, dim: int, rank: int, world: int) -> np.ndarray:
+    """Rank `rank`'s block of m shift vectors out of the ONE stream of m*world vectors keyed by `seed`: a world-GPU run
+    is the same estimator as a 1-GPU run with m*world shifts."""
+    return qi.splitmix64_shifts(seed, m * world, dim)[rank * m:(rank + 1) * m]
+
+
+def time_to_accuracy(q, wl, torch, target=1e-3, max_N=2 ** 27):
+    """M2: raise N through the primes below 2^k until the relative error of the eps^0 coefficient of J is <= target
+    (reading C17); wall time of everything the user waits for after qmc_prepare: generating-vector search, uploads,
+    kernels, downloads, statistics, summed over the N tried."""
+    t = q.qmc_prepare(wl, eps_order=wl.eps_order, lam=wl.lam)
+    q.qmc_integrate(t, 16381, wl.m, seed=wl.seed)          # context / module warm-up, not timed
+    tried = []
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    rel = None
+    for N in qi.primes_below_pow2(14, 27):
+        if N > max_N:
+            break
+        r = q.qmc_integrate(t, N, wl.m, seed=wl.seed)
+        c0, e0 = r.coeff[-1 - wl.eps_order], r.err[-1 - wl.eps_order]
+        rel = max(e0.real, e0.imag) / abs(c0)
+        tried.append(N)
+        if rel <= target:
+            break
+    dt = time.perf_counter() - t0
+    return {"workload": wl.name, "target_rel_err": target, "wall_s": dt, "N_reached": tried[-1], "N_tried": len(tried),
+            "rel_err": rel, "coeff_eps0": [c0.real, c0.imag], "err_eps0": [e0.real, e0.imag], "m": wl.m}
+
+
+def run_product(args):
+    import torch
+    import torch.distributed as dist
+    import paper_1508_02512_b200 as q
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the QMC hot path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = f"cuda:{local}"
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    wl = workload(args.config)
+    N = args.N or DEFAULT_N[args.config]
+    m = wl.m
+    t = q.qmc_prepare(wl, eps_order=wl.eps_order, lam=wl.lam)
+    z = q.qmc_generating_vector(N, t.dim, device=dev)           # Korobov P2 search on the device, outside the timed steps
+    shifts = shift_block(wl.seed, m, t.dim, rank, world)
+    fp, fs, corners = q.qmc_flop_model(t)
+    flops_step = (fp + fs) * N * m
+    evals_step = N * m * t.n_sectors
+
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
+    gathered = torch.zeros(world, t.K, m, 2, dtype=torch.float64, device=dev)
+
+    def step(resident):
+        q.qmc_integrate_async(t, N, m, z=z, shifts=None if resident == 2 else shifts, resident=resident, device=dev)
+        if world > 1:
+            dist.all_gather_into_tensor(gathered, q.qmc_result_device_totals(t, m).contiguous())
+
+    # ---- device-timed steps: inputs resident in HBM, CUDA events on the launching stream ---------------------
+    step(0)
+    for _ in range(max(args.warmup, 3) - 1):
+        step(2)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    eval_ms = []
+    torch.cuda.synchronize()
+    for a, b in ev:
+        flush.fill_(1)                                          # L2 flush, outside the event pair
+        a.record()
+        step(2)
+        b.record()
+        b.synchronize()
+        eval_ms.append(q.qmc_result_fetch(t, m, device=dev).eval_kernel_ms)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.summary()
+    ms_local = sum(a.elapsed_time(b) for a, b in ev)
+    res = q.qmc_result_fetch(t, m, device=dev)
+    msT = torch.tensor([ms_local], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(msT, op=dist.ReduceOp.MAX)
+    ms_per_step = float(msT.item()) / args.steps
+    value = evals_step * world / (ms_per_step * 1e-3)
+
+    # ---- end to end through the public call with HOST buffers: H2D of tables + shifts, kernels, D2H, every step ----
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        r_e2e = q.qmc_integrate(t, N, m, z=z, shifts=shifts, resident=0, device=dev)
+        if world > 1:
+            loc = torch.from_numpy(np.ascontiguousarray(r_e2e.shift_totals).view(np.float64).reshape(t.K, m, 2)).to(dev)
+            dist.all_gather_into_tensor(gathered, loc)
+            allT = gathered.cpu().numpy()
+    torch.cuda.synchronize()
+    e2e_s = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
+    e2e_val = evals_step * world * args.steps / float(e2e_s.item())
+    h2d, d2h = r_e2e.h2d_bytes, r_e2e.d2h_bytes             # counted by the library from the copies it made
+
+    # ---- combine the shifts of all ranks (Eqs. 19-20 over m*world estimates) --------------------------------
+    if world > 1:
+        allT = gathered.cpu().numpy()                      # [world, K, m, 2]
+        T = np.concatenate([allT[r] for r in range(world)], axis=1)
+        coeff, err = q.qmc_statistics(T[..., 0] + 1j * T[..., 1])
+    else:
+        coeff, err = res.coeff, res.err
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (qmc_eval_kernel): plain FP64 ALU bound -----------------------------
+    peak_flops, _ = q.qmc_fp64_peak(device=dev)
+    mean_eval_ms = float(np.mean(eval_ms))
+    achieved = flops_step / (mean_eval_ms * 1e-3) / 1e12
+    nominal = 148 * 64 * 2 * 1.965e9 / 1e12
+    roofline = {"bound": "alu", "kernel": "qmc_eval_kernel", "achieved": achieved, "peak": peak_flops / 1e12,
+                "unit": "TFLOP/s", "frac": achieved / (peak_flops / 1e12), "traffic": _traffic_from_profiles(),
+                "peak_source": "DFMA chain microbenchmark (qmc_fp64_peak) measured in this run; MEASURED_PEAKS.json has no FP64 entry",
+                "peak_nominal": nominal, "frac_of_nominal": achieved / nominal, "kernel_ms": mean_eval_ms,
+                "kernel_share_of_step": mean_eval_ms / ms_per_step,
+                "flops_per_point_shift": fp + fs, "corners_per_point": corners, "algorithmic_bytes_per_launch": 0}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl.name, "N": N, "m_per_gpu": m, "seed": wl.seed, "n_sectors": t.n_sectors,
+                       "dim": t.dim, "orders": [t.k_min, t.k_max], "complex": t.is_complex, "lambda": wl.lam,
+                       "corners_per_point": corners, "parallelism": f"shift-sharded x{world}",
+                       "l2": "flushed between steps (256 MiB fill, outside the event pairs); the kernels read <= 150 KB of tables"},
+            "corner_evals_per_sec": corners * N * m * world / (ms_per_step * 1e-3),
+            "result": {"coeff_re": [float(x) for x in coeff.real], "coeff_im": [float(x) for x in coeff.imag],
+                       "err_re": [float(x) for x in err.real], "err_im": [float(x) for x in err.imag],
+                       "counters": [int(x) for x in res.counters]},
+            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "note": "qmc_integrate with host buffers each step: tables + shifts H2D (pageable staging), kernels, statistics D2H, host wall clock"},
+            "gpu_launches": 3 * args.steps * world, "clocks": clocks, "roofline": roofline}
+
+    if world == 1 and not args.no_extras:
+        z_o = test_vector(N, wl.dim)
+        v, cores, desc = oracle_sample(wl, N, z_o, qi.splitmix64_shifts(wl.seed, m, wl.dim), 15.0)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+        line["time_to_1e-3"] = [time_to_accuracy(q, qi.double_box(), torch), time_to_accuracy(q, qi.nonplanar_vertex(), torch)]
+        line["time_to_1e-5"] = [time_to_accuracy(q, qi.nonplanar_vertex(), torch, target=1e-5, max_N=2 ** 24)]
+        line["other_workloads"] = other_workloads(q, torch, dev, args.config)
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def _traffic_from_profiles():
+    """DRAM bytes per launch of the evaluation kernel from the committed `ncu --set full` capture (profiles/), or None."""
+    p = os.path.join(ROOT, "profiles", "eval_kernel_traffic.json")
+    try:
+        with open(p) as f:
+            return json.load(f).get("dram_bytes_per_launch")
+    except Exception:
+        return None
+
+
+def other_workloads(q, torch, dev, skip_cfg):
+    """Device-timed throughput of the other multi-sector configs (context; the headline is `value`)."""
+    out = []
+    for cfg in (2, 3, 4, 5):
+        if cfg == skip_cfg:
+            continue
+        wl = workload(cfg)
+        N = DEFAULT_N[cfg]
+        t = q.qmc_prepare(wl, eps_order=wl.eps_order, lam=wl.lam)
+        z = q.qmc_generating_vector(N, t.dim, device=dev)
+        q.qmc_integrate_async(t, N, wl.m, seed=wl.seed, z=z, resident=0, device=dev)
+        q.qmc_integrate_async(t, N, wl.m, seed=wl.seed, z=z, resident=2, device=dev)
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 3
+        a.record()
+        for _ in range(reps):
+            q.qmc_integrate_async(t, N, wl.m, seed=wl.seed, z=z, resident=2, device=dev)
+        b.record()
+        b.synchronize()
+        ms = a.elapsed_time(b) / reps
+        r = q.qmc_result_fetch(t, wl.m, device=dev)
+        fp, fs, corners = q.qmc_flop_model(t)
+        out.append({"workload": wl.name, "N": N, "m": wl.m, "n_sectors": t.n_sectors, "ms_per_step": ms,
+                    "evals_per_sec": N * wl.m * t.n_sectors / (ms * 1e-3),
+                    "corner_evals_per_sec": N * wl.m * corners / (ms * 1e-3),
+                    "tflops": (fp + fs) * N * wl.m / (r.eval_kernel_ms * 1e-3) / 1e12,
+                    "coeff_eps0": [float(r.coeff[-1 - wl.eps_order].real), float(r.coeff[-1 - wl.eps_order].imag)],
+                    "err_eps0": [float(r.err[-1 - wl.eps_order].real), float(r.err[-1 - wl.eps_order].imag)]})
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5],
+                    help="BASELINE.json config (1-based); default 4 = two-loop planar double box, 293 sectors")
+    ap.add_argument("--N", type=int, default=0, help="lattice size (prime); default: DEFAULT_N[config]")
+    ap.add_argument("--impl", default="product", choices=["product", "reference"])
+    ap.add_argument("--no-extras", action="store_true", help="skip cpu_baseline, time-to-accuracy and other workloads")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_product(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -100,7 +100,9 @@ typedef struct {
   double *shift_sums;                /* [n_sectors][K][m][2] per-sector per-shift estimates (parity checks) */
   int64_t counters[4];               /* #corner evaluations with Im F^(z) > 0, with Re U^(z) <= 0,
                                         #non-finite (point, sector) evaluations (dropped), #boundary points (R:C18) */
-  double kernel_ms;                  /* device time of the evaluation + reduction kernels (CUDA events) */
+  double kernel_ms;                  /* device time of all kernels of the call: evaluation, final sum, statistics (CUDA events) */
+  double eval_kernel_ms;             /* device time of the evaluation kernel alone (S1-S7 first stage) */
+  int64_t h2d_bytes, d2h_bytes;      /* bytes this call copied host->device (tables, shifts) and device->host (results) */
   int32_t kernel_launches;           /* number of kernel launches made by this call */
   int32_t mode_used;                 /* 1 fused (all sectors summed in registers), 2 per-sector */
 } qmc_result;
@@ -113,7 +115,8 @@ typedef struct {
                                                     The sum is always normalised by 1/N (Eq. 18). */
   int32_t sector_begin, sector_end;              /* sector range; end 0 = all */
   int32_t mode;             /* 0 auto (per-sector iff a per-sector output is requested), 1 fused, 2 per-sector */
-  int32_t tables_resident;  /* 1: reuse the table image already uploaded to this workspace by an earlier call */
+  int32_t tables_resident;  /* 1: reuse the table image already uploaded to this workspace by an earlier call;
+                               2: reuse the shift vectors of that call as well (nothing is copied from the host) */
 } qmc_run;
 
 size_t qmc_workspace_bytes(const qmc_tables *t, uint64_t N, int32_t m);
@@ -127,7 +130,32 @@ int qmc_integrate(const qmc_tables *t, uint64_t N, int32_t m, uint64_t seed, voi
 int qmc_integrate_ex(const qmc_tables *t, uint64_t N, int32_t m, uint64_t seed, const qmc_run *run, void *cuda_stream,
                      void *dev_workspace, size_t dev_workspace_bytes, qmc_result *out);
 
+/* The same path in two halves, for callers that keep everything on the device (bench.py's device-timed loop):
+ * qmc_integrate_async enqueues S1-S8 on `cuda_stream` (evaluation kernel, fixed-order final sum, statistics kernel)
+ * and returns without synchronising; every result stays in the workspace.  qmc_result_fetch copies the results of
+ * the LAST qmc_integrate_async on this tables object to the host (one D2H), synchronises the stream and fills `out`
+ * exactly as qmc_integrate_ex does (qmc_integrate_ex = async + fetch).  Per-sector outputs exist only if that
+ * launch ran in mode 2. */
+int qmc_integrate_async(const qmc_tables *t, uint64_t N, int32_t m, uint64_t seed, const qmc_run *run, void *cuda_stream,
+                        void *dev_workspace, size_t dev_workspace_bytes);
+int qmc_result_fetch(const qmc_tables *t, void *cuda_stream, void *dev_workspace, size_t dev_workspace_bytes,
+                     qmc_result *out);
+
+/* Device address of the per-shift totals [K][m][2] (doubles; Eq. 18 summed over sectors) that the last
+ * qmc_integrate_async left in the workspace -- for a device-side gather across ranks. */
+int qmc_result_device_totals(const qmc_tables *t, void *dev_workspace, size_t dev_workspace_bytes, void **totals_out);
+
 /* ---- helpers ---- */
+/* Eqs. 19-20 on per-shift estimates: shift_totals [K][m][2] (host) -> coeff, err [K][2], Re and Im
+ * separately (R:C15).  Used to combine the per-shift estimates gathered from several GPUs (each rank integrates its
+ * own block of shift vectors).  m >= 2. */
+int qmc_statistics(const double *shift_totals, int32_t K, int32_t m, double *coeff, double *err);
+/* Algorithmic FP64 operation count of the evaluation (DFMA = 2, DADD = DMUL = 1, log,
+ * reciprocal, division and atan2 at the fixed costs stated there): flops per (lattice point, shift) spent once per
+ * point (S1-S3) and in all sectors [sector_begin, sector_end) (S4-S7; end 0 = all), plus the number of corner
+ * evaluations per point.  Any output may be NULL. */
+int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t sector_end, double *flops_point,
+                   double *flops_sectors, int64_t *corners);
 /* Korobov-form generating vector z = (1, a, a^2, ...) mod N with `a` minimising the P_2 figure of merit over a fixed
  * deterministic candidate list (R:C13; "component-by-component" is the paper's own choice).  Runs on the
  * device (needs workspace of qmc_workspace_bytes). */

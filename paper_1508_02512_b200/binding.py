@@ -43,7 +43,9 @@ class qmc_result(C.Structure):
     _fields_ = [("coeff", C.POINTER(C.c_double)), ("err", C.POINTER(C.c_double)),
                 ("sector_coeff", C.POINTER(C.c_double)), ("sector_err", C.POINTER(C.c_double)),
                 ("shift_totals", C.POINTER(C.c_double)), ("shift_sums", C.POINTER(C.c_double)),
-                ("counters", C.c_int64 * 4), ("kernel_ms", C.c_double), ("kernel_launches", C.c_int32),
+                ("counters", C.c_int64 * 4), ("kernel_ms", C.c_double), ("eval_kernel_ms", C.c_double),
+                ("h2d_bytes", C.c_int64), ("d2h_bytes", C.c_int64),
+                ("kernel_launches", C.c_int32),
                 ("mode_used", C.c_int32)]
 
 
@@ -82,6 +84,19 @@ def lib():
         L.qmc_integrate_ex.restype = C.c_int
         L.qmc_integrate_ex.argtypes = [C.c_void_p, C.c_uint64, C.c_int32, C.c_uint64, C.POINTER(qmc_run), C.c_void_p,
                                        C.c_void_p, C.c_size_t, C.POINTER(qmc_result)]
+        L.qmc_integrate_async.restype = C.c_int
+        L.qmc_integrate_async.argtypes = [C.c_void_p, C.c_uint64, C.c_int32, C.c_uint64, C.POINTER(qmc_run), C.c_void_p,
+                                          C.c_void_p, C.c_size_t]
+        L.qmc_result_fetch.restype = C.c_int
+        L.qmc_result_fetch.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.POINTER(qmc_result)]
+        L.qmc_result_device_totals.restype = C.c_int
+        L.qmc_result_device_totals.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.POINTER(C.c_void_p)]
+        L.qmc_statistics.restype = C.c_int
+        L.qmc_statistics.argtypes = [C.POINTER(C.c_double), C.c_int32, C.c_int32, C.POINTER(C.c_double),
+                                     C.POINTER(C.c_double)]
+        L.qmc_flop_model.restype = C.c_int
+        L.qmc_flop_model.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double),
+                                     C.POINTER(C.c_int64)]
         L.qmc_generating_vector.restype = C.c_int
         L.qmc_generating_vector.argtypes = [C.c_uint64, C.c_int32, C.c_void_p, C.c_void_p, C.c_size_t, C.POINTER(C.c_uint64)]
         L.qmc_shifts.restype = C.c_int
@@ -175,6 +190,9 @@ class Result:
     shift_sums: Optional[np.ndarray]   # [n_sectors, K, m] complex
     counters: np.ndarray         # [4]
     kernel_ms: float
+    eval_kernel_ms: float
+    h2d_bytes: int
+    d2h_bytes: int
     kernel_launches: int
     mode_used: int
 
@@ -189,9 +207,53 @@ def _workspace(t: Tables, N: int, m: int, device):
     return ws
 
 
+def _make_run(t: Tables, m: int, z, shifts, index_range, sectors, mode: int, resident: int):
+    run = qmc_run()
+    keep = []
+    if z is not None:
+        za = np.ascontiguousarray(z, dtype=np.uint64); keep.append(za)
+        run.z = _ptr(za, C.c_uint64)
+    if shifts is not None:
+        sa = np.ascontiguousarray(shifts, dtype=np.float64); keep.append(sa)
+        assert sa.shape == (m, t.dim)
+        run.shifts = _ptr(sa, C.c_double)
+    if index_range is not None:
+        run.index_begin, run.index_step, run.index_count = index_range
+    if sectors is not None:
+        run.sector_begin, run.sector_end = sectors
+    run.mode = mode
+    run.tables_resident = int(resident)
+    return run, keep
+
+
+def _make_result(t: Tables, m: int, ns: int, per_sector: bool):
+    K = t.K
+    coeff = np.zeros(K, dtype=np.complex128); err = np.zeros(K, dtype=np.complex128)
+    shift_totals = np.zeros((K, m), dtype=np.complex128)
+    res = qmc_result()
+    res.coeff = _ptr(coeff.view(np.float64), C.c_double)
+    res.err = _ptr(err.view(np.float64), C.c_double)
+    res.shift_totals = _ptr(shift_totals.view(np.float64), C.c_double)
+    sc = se = ss = None
+    if per_sector:
+        sc = np.zeros((ns, K), dtype=np.complex128); se = np.zeros((ns, K), dtype=np.complex128)
+        ss = np.zeros((ns, K, m), dtype=np.complex128)
+        res.sector_coeff = _ptr(sc.view(np.float64), C.c_double)
+        res.sector_err = _ptr(se.view(np.float64), C.c_double)
+        res.shift_sums = _ptr(ss.view(np.float64), C.c_double)
+    return res, (coeff, err, shift_totals, sc, se, ss)
+
+
+def _wrap_result(res, arrays) -> Result:
+    coeff, err, shift_totals, sc, se, ss = arrays
+    return Result(coeff, err, shift_totals, sc, se, ss, np.array(list(res.counters), dtype=np.int64),
+                  float(res.kernel_ms), float(res.eval_kernel_ms), int(res.h2d_bytes), int(res.d2h_bytes),
+                  int(res.kernel_launches), int(res.mode_used))
+
+
 def qmc_integrate(t: Tables, N: int, m: int, seed: int = 0, *, z: Optional[Sequence[int]] = None,
                   shifts: Optional[np.ndarray] = None, index_range=None, sectors=None, per_sector: bool = False,
-                  mode: int = 0, resident: bool = False, device="cuda:0", stream=None) -> Result:
+                  mode: int = 0, resident: int = 0, device="cuda:0", stream=None) -> Result:
     """qmc_integrate(tables, N, m, seed) -> Laurent coefficients and errors (qmc_integrate_ex when any of the
     explicit controls is given).  Workspace and stream come from PyTorch."""
     import torch
@@ -201,43 +263,83 @@ def qmc_integrate(t: Tables, N: int, m: int, seed: int = 0, *, z: Optional[Seque
     with torch.cuda.device(dev):
         ws = _workspace(t, N, m, dev)
         st = stream if stream is not None else torch.cuda.current_stream(dev)
-        K = t.K
         s0, s1 = sectors if sectors is not None else (0, t.n_sectors)
-        ns = s1 - s0
-        coeff = np.zeros(K, dtype=np.complex128); err = np.zeros(K, dtype=np.complex128)
-        shift_totals = np.zeros((K, m), dtype=np.complex128)
-        res = qmc_result()
-        res.coeff = _ptr(coeff.view(np.float64), C.c_double)
-        res.err = _ptr(err.view(np.float64), C.c_double)
-        res.shift_totals = _ptr(shift_totals.view(np.float64), C.c_double)
-        sc = se = ss = None
-        if per_sector:
-            sc = np.zeros((ns, K), dtype=np.complex128); se = np.zeros((ns, K), dtype=np.complex128)
-            ss = np.zeros((ns, K, m), dtype=np.complex128)
-            res.sector_coeff = _ptr(sc.view(np.float64), C.c_double)
-            res.sector_err = _ptr(se.view(np.float64), C.c_double)
-            res.shift_sums = _ptr(ss.view(np.float64), C.c_double)
-        run = qmc_run()
-        keep = []
-        if z is not None:
-            za = np.ascontiguousarray(z, dtype=np.uint64); keep.append(za)
-            run.z = _ptr(za, C.c_uint64)
-        if shifts is not None:
-            sa = np.ascontiguousarray(shifts, dtype=np.float64); keep.append(sa)
-            assert sa.shape == (m, t.dim)
-            run.shifts = _ptr(sa, C.c_double)
-        if index_range is not None:
-            run.index_begin, run.index_step, run.index_count = index_range
-        if sectors is not None:
-            run.sector_begin, run.sector_end = s0, s1
-        run.mode = mode
-        run.tables_resident = 1 if resident else 0
+        res, arrays = _make_result(t, m, s1 - s0, per_sector)
+        run, keep = _make_run(t, m, z, shifts, index_range, sectors, mode, resident)
         rc = lib().qmc_integrate_ex(t._h, N, m, seed, C.byref(run), C.c_void_p(st.cuda_stream),
                                     C.c_void_p(ws.data_ptr()), ws.numel(), C.byref(res))
         if rc:
             raise QmcError(rc, "qmc_integrate")
-    return Result(coeff, err, shift_totals, sc, se, ss, np.array(list(res.counters), dtype=np.int64),
-                  float(res.kernel_ms), int(res.kernel_launches), int(res.mode_used))
+    return _wrap_result(res, arrays)
+
+
+def qmc_integrate_async(t: Tables, N: int, m: int, seed: int = 0, *, z=None, shifts=None, index_range=None,
+                        sectors=None, mode: int = 1, resident: int = 0, device="cuda:0", stream=None) -> None:
+    """Enqueue S1-S8 on the stream and return without synchronising; results stay in the workspace of `t`
+    (qmc_result_fetch brings them to the host).  resident=2: nothing is copied from the host."""
+    import torch
+    if not torch.cuda.is_available():
+        raise QmcError(QMC_ECUDA, "qmc_integrate_async (no CUDA device; there is no CPU fallback)")
+    dev = torch.device(device)
+    with torch.cuda.device(dev):
+        ws = _workspace(t, N, m, dev)
+        st = stream if stream is not None else torch.cuda.current_stream(dev)
+        run, keep = _make_run(t, m, z, shifts, index_range, sectors, mode, resident)
+        rc = lib().qmc_integrate_async(t._h, N, m, seed, C.byref(run), C.c_void_p(st.cuda_stream),
+                                       C.c_void_p(ws.data_ptr()), ws.numel())
+        if rc:
+            raise QmcError(rc, "qmc_integrate_async")
+
+
+def qmc_result_fetch(t: Tables, m: int, *, per_sector: bool = False, n_sectors: Optional[int] = None, device="cuda:0",
+                     stream=None) -> Result:
+    """Results of the last qmc_integrate_async on `t`: one D2H copy + stream synchronisation."""
+    import torch
+    dev = torch.device(device)
+    with torch.cuda.device(dev):
+        ws = t._ws
+        if ws is None:
+            raise QmcError(QMC_EINVAL, "qmc_result_fetch (no launch on these tables)")
+        st = stream if stream is not None else torch.cuda.current_stream(dev)
+        res, arrays = _make_result(t, m, t.n_sectors if n_sectors is None else n_sectors, per_sector)
+        rc = lib().qmc_result_fetch(t._h, C.c_void_p(st.cuda_stream), C.c_void_p(ws.data_ptr()), ws.numel(), C.byref(res))
+        if rc:
+            raise QmcError(rc, "qmc_result_fetch")
+    return _wrap_result(res, arrays)
+
+
+def qmc_result_device_totals(t: Tables, m: int):
+    """torch view (float64, shape [K, m, 2]) of the per-shift totals the last qmc_integrate_async left on the device."""
+    import torch
+    ws = t._ws
+    p = C.c_void_p()
+    rc = lib().qmc_result_device_totals(t._h, C.c_void_p(ws.data_ptr()), ws.numel(), C.byref(p))
+    if rc:
+        raise QmcError(rc, "qmc_result_device_totals")
+    off = p.value - ws.data_ptr()
+    return ws[off: off + t.K * m * 16].view(torch.float64).view(t.K, m, 2)
+
+
+def qmc_statistics(shift_totals: np.ndarray):
+    """Eqs. 19-20 on per-shift estimates [K, m] (complex) -> (coeff[K], err[K])."""
+    T = np.ascontiguousarray(shift_totals, dtype=np.complex128)
+    K, m = T.shape
+    coeff = np.zeros(K, dtype=np.complex128); err = np.zeros(K, dtype=np.complex128)
+    rc = lib().qmc_statistics(_ptr(T.view(np.float64), C.c_double), K, m, _ptr(coeff.view(np.float64), C.c_double),
+                              _ptr(err.view(np.float64), C.c_double))
+    if rc:
+        raise QmcError(rc, "qmc_statistics")
+    return coeff, err
+
+
+def qmc_flop_model(t: Tables, sectors=None):
+    """(flops once per point, flops in all sectors, corner evaluations) per (lattice point, shift)."""
+    s0, s1 = sectors if sectors is not None else (0, 0)
+    fp, fs, nc = C.c_double(0), C.c_double(0), C.c_int64(0)
+    rc = lib().qmc_flop_model(t._h, s0, s1, C.byref(fp), C.byref(fs), C.byref(nc))
+    if rc:
+        raise QmcError(rc, "qmc_flop_model")
+    return float(fp.value), float(fs.value), int(nc.value)
 
 
 def qmc_shifts(seed: int, m: int, dim: int) -> np.ndarray:

@@ -87,6 +87,59 @@ __global__ void __launch_bounds__(256) qmc_dfma_peak_kernel(double *sink, int it
   if (s == 12345.678) sink[0] = s;  // never true; keeps the chains alive
 }
 
+// ---- S8: statistics over the shifts (Eqs. 19-20), Re and Im separately (R:C15) ------------
+// in : out [row][nacc*nc][m] (row = sector in per-sector mode, a single row in fused mode)
+// stat (doubles): totals [K][m][2] | coeff [K][2] | err [K][2] | sector_coeff [nrows][K][2] | sector_err [nrows][K][2]
+//                 | shift_sums [nrows][K][m][2]           (nrows = 0 in fused mode)
+// One thread per (row or total, order, Re/Im); sums run in a fixed order.
+struct StatLayout {
+  size_t totals, coeff, err, sector_coeff, sector_err, shift_sums, total;
+};
+__host__ __device__ inline StatLayout stat_layout(int nrows, int K, int m) {
+  StatLayout S;
+  size_t o = 0;
+  S.totals = o; o += (size_t)K * m * 2;
+  S.coeff = o; o += (size_t)K * 2;
+  S.err = o; o += (size_t)K * 2;
+  S.sector_coeff = o; o += (size_t)nrows * K * 2;
+  S.sector_err = o; o += (size_t)nrows * K * 2;
+  S.shift_sums = o; o += (size_t)nrows * K * m * 2;
+  S.total = o;
+  return S;
+}
+__global__ void qmc_stats_kernel(const double *out, double *stat, int nrows, int K, int m, int nacc, int nc, int acc0) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (nrows + 1) * K * 2) return;
+  const int c = idx & 1, k = (idx >> 1) % K, row = (idx >> 1) / K;
+  const StatLayout S = stat_layout(nrows, K, m);
+  const int a = (acc0 + k) * nc + c;  // accumulator of order k_min + k
+  const bool total = row == nrows;
+  const int r0 = total ? 0 : row, r1 = total ? (nrows ? nrows : 1) : row + 1;
+  double *v = total ? stat + S.totals + (size_t)k * m * 2 + c : stat + S.shift_sums + ((size_t)row * K + k) * m * 2 + c;
+  double s = 0.0;
+  for (int kap = 0; kap < m; ++kap) {
+    double x = 0.0;
+    if (c < nc)
+      for (int r = r0; r < r1; ++r) x += out[((size_t)r * nacc * nc + a) * m + kap];
+    v[2 * kap] = x;
+    s += x;
+  }
+  const double q = s / m;
+  double d2 = 0.0;
+  for (int kap = 0; kap < m; ++kap) {
+    double d = v[2 * kap] - q;
+    d2 += d * d;
+  }
+  const double e = sqrt(d2 / ((double)m * (m - 1)));
+  if (total) {
+    stat[S.coeff + 2 * k + c] = q;
+    stat[S.err + 2 * k + c] = e;
+  } else {
+    stat[S.sector_coeff + ((size_t)row * K + k) * 2 + c] = q;
+    stat[S.sector_err + ((size_t)row * K + k) * 2 + c] = e;
+  }
+}
+
 uint64_t splitmix64(uint64_t &state) {
   state += 0x9E3779B97F4A7C15ull;
   uint64_t x = state;
@@ -98,7 +151,7 @@ uint64_t splitmix64(uint64_t &state) {
 uint64_t mulmod(uint64_t a, uint64_t b, uint64_t n) { return (uint64_t)(((unsigned __int128)a * b) % n); }
 
 struct DevLayout {
-  size_t image, secoff, shifts, counters, out, partial, p2z, p2partial, total;
+  size_t image, secoff, shifts, counters, out, stat, partial, p2z, p2partial, total;
 };
 
 DevLayout layout(const qmc_tables *t, int m) {
@@ -110,6 +163,7 @@ DevLayout layout(const qmc_tables *t, int m) {
   L.shifts = o; o += align256((size_t)m * QMC_MAXDIM * 8);
   L.counters = o; o += 256;
   L.out = o; o += align256(nsec * QMC_NACC_MAX * 2 * (size_t)m * 8);
+  L.stat = o; o += align256(stat_layout((int)nsec, QMC_MAXK, m).total * 8);
   L.partial = o; o += align256(nsec * (size_t)m * QMC_MAX_BLOCKS * QMC_NACC_MAX * 2 * 8);
   L.p2z = o; o += align256((size_t)QMC_NCAND * QMC_MAXDIM * 4);
   L.p2partial = o; o += align256((size_t)QMC_NCAND * QMC_P2_BLOCKS * 8);
@@ -210,7 +264,14 @@ int qmc_prepare(const qmc_graph *graph, const qmc_kinematics *kin, int32_t eps_o
   return QMC_OK;
 }
 
-void qmc_tables_free(qmc_tables *t) { delete t; }
+void qmc_tables_free(qmc_tables *t) {
+  if (t && t->ev0) {
+    cudaEventDestroy(static_cast<cudaEvent_t>(t->ev0));
+    cudaEventDestroy(static_cast<cudaEvent_t>(t->ev1));
+    cudaEventDestroy(static_cast<cudaEvent_t>(t->evm));
+  }
+  delete t;
+}
 
 int qmc_tables_info(const qmc_tables *t, int32_t *n_sectors, int32_t *dim, int32_t *k_min, int32_t *k_max,
                     int32_t *is_complex) {
@@ -325,10 +386,11 @@ int qmc_fp64_peak(void *cuda_stream, void *dev_workspace, size_t dev_workspace_b
   return QMC_OK;
 }
 
-int qmc_integrate_ex(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t seed, const qmc_run *run, void *cuda_stream,
-                     void *dev_workspace, size_t dev_workspace_bytes, qmc_result *out) {
-  if (!tc || !out) return QMC_EINVAL;
-  qmc_tables *t = const_cast<qmc_tables *>(tc);  // launcher caches (resident image, generating vector)
+int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t seed, const qmc_run *run, void *cuda_stream,
+                        void *dev_workspace, size_t dev_workspace_bytes) {
+  if (!tc) return QMC_EINVAL;
+  qmc_tables *t = const_cast<qmc_tables *>(tc);  // launcher caches (resident image, generating vector, last launch)
+  t->last.valid = false;
   const int n = t->n, nsec_all = (int)t->sectors.size();
   if (N < 5 || N >= (1ull << 31) || m < 2) return QMC_EINVAL;  // Eq. 20 needs m >= 2
   qmc_run r;
@@ -339,10 +401,8 @@ int qmc_integrate_ex(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t seed,
   const uint64_t ibeg = r.index_begin, istep = r.index_count ? r.index_step : 1, icount = r.index_count ? r.index_count : N;
   if (istep < 1 || ibeg >= N || icount > N) return QMC_EINVAL;
   const bool cplx = t->lambda > 0.0;
-  const bool want_persec = out->sector_coeff || out->sector_err || out->shift_sums;
-  const int mode = r.mode ? r.mode : (want_persec ? 2 : 1);
+  const int mode = r.mode ? r.mode : 1;
   if (mode != 1 && mode != 2) return QMC_EINVAL;
-  if (mode == 1 && want_persec) return QMC_EINVAL;
   const bool persec = mode == 2;
 
   int devcount = 0;
@@ -354,6 +414,8 @@ int qmc_integrate_ex(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t seed,
   if (!dev_workspace || dev_workspace_bytes < L.total) return QMC_ENOMEM;
   unsigned char *ws = static_cast<unsigned char *>(dev_workspace);
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const bool image_resident = r.tables_resident >= 1 && t->resident_ws == dev_workspace;
+  const bool shifts_resident = r.tables_resident >= 2 && image_resident && t->resident_m == m && !r.shifts;
 
   // ---- generating vector and shifts ---------------------------------------------------------------------
   uint64_t z[QMC_MAXDIM] = {0};
@@ -369,13 +431,15 @@ int qmc_integrate_ex(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t seed,
   }
   for (int j = 0; j < n; ++j)
     if (z[j] == 0 || z[j] >= N || std::gcd(z[j], N) != 1) return QMC_EINVAL;
-  std::vector<double> shifts((size_t)m * n);
-  if (r.shifts) {
-    std::memcpy(shifts.data(), r.shifts, shifts.size() * 8);
-    for (double v : shifts)
-      if (!(v >= 0.0 && v < 1.0)) return QMC_EINVAL;
-  } else {
-    qmc_shifts(seed, m, n, shifts.data());
+  if (!shifts_resident) {
+    t->shifts_host.resize((size_t)m * n);
+    if (r.shifts) {
+      std::memcpy(t->shifts_host.data(), r.shifts, t->shifts_host.size() * 8);
+      for (double v : t->shifts_host)
+        if (!(v >= 0.0 && v < 1.0)) return QMC_EINVAL;
+    } else {
+      qmc_shifts(seed, m, n, t->shifts_host.data());
+    }
   }
 
   // ---- launch geometry ----------------------------------------------------------------------------------
@@ -424,13 +488,20 @@ int qmc_integrate_ex(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t seed,
   int gx = std::min<long long>({(long long)sms * bps, (long long)QMC_MAX_BLOCKS, (long long)((icount + QMC_THREADS - 1) / QMC_THREADS)});
   gx = std::max(gx, 1);
 
-  // ---- uploads -------------------------------------------------------------------------------------------
-  if (!(r.tables_resident && t->resident_ws == dev_workspace)) {
+  // ---- uploads (skipped when resident) ------------------------------------------------------------------
+  size_t h2d = 0;
+  if (!image_resident) {
+    h2d += t->image.size() + t->secoff.size() * 4;
     CUDA_OK(cudaMemcpyAsync(ws + L.image, t->image.data(), t->image.size(), cudaMemcpyHostToDevice, st));
     CUDA_OK(cudaMemcpyAsync(ws + L.secoff, t->secoff.data(), t->secoff.size() * 4, cudaMemcpyHostToDevice, st));
     t->resident_ws = dev_workspace;
+    t->resident_m = 0;
   }
-  CUDA_OK(cudaMemcpyAsync(ws + L.shifts, shifts.data(), shifts.size() * 8, cudaMemcpyHostToDevice, st));
+  if (!shifts_resident) {
+    h2d += t->shifts_host.size() * 8;
+    CUDA_OK(cudaMemcpyAsync(ws + L.shifts, t->shifts_host.data(), t->shifts_host.size() * 8, cudaMemcpyHostToDevice, st));
+    t->resident_m = m;
+  }
   CUDA_OK(cudaMemsetAsync(ws + L.counters, 0, 32, st));
 
   QmcLaunch p;
@@ -455,83 +526,126 @@ int qmc_integrate_ex(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t seed,
   p.persec = persec ? 1 : 0;
   p.tab_smem_bytes = (tab_bytes + 15) & ~15u;
 
-  cudaEvent_t e0, e1;
-  CUDA_OK(cudaEventCreate(&e0));
-  CUDA_OK(cudaEventCreate(&e1));
-  cudaEventRecord(e0, st);
+  if (!t->ev0) {
+    CUDA_OK(cudaEventCreate(reinterpret_cast<cudaEvent_t *>(&t->ev0)));
+    CUDA_OK(cudaEventCreate(reinterpret_cast<cudaEvent_t *>(&t->ev1)));
+    CUDA_OK(cudaEventCreate(reinterpret_cast<cudaEvent_t *>(&t->evm)));
+  }
+  cudaEventRecord(static_cast<cudaEvent_t>(t->ev0), st);
   cudaError_t ce = qmc_kernel_launch(n, t->kmax, cplx, dim3(gx, nchunks), smem, st, p);
+  cudaEventRecord(static_cast<cudaEvent_t>(t->evm), st);
   const int rows = persec ? (se - sb) : nchunks;
+  const int nrows = persec ? (se - sb) : 0;  // per-sector rows of the statistics block
   const int nout = (persec ? (se - sb) : 1) * nacc * nc * m;
+  const int K = t->kmax - t->kmin + 1;
   double *dout = reinterpret_cast<double *>(ws + L.out);
   if (ce == cudaSuccess) {
     qmc_finalize_kernel<<<(nout + 127) / 128, 128, 0, st>>>(p.partial, dout, rows, m, gx, nacc * nc, 1.0 / (double)N, persec ? 1 : 0);
     ce = cudaGetLastError();
   }
-  cudaEventRecord(e1, st);
-  std::vector<double> hout((size_t)nout);
+  if (ce == cudaSuccess) {
+    const int nthreads = (nrows + 1) * K * 2;
+    qmc_stats_kernel<<<(nthreads + 63) / 64, 64, 0, st>>>(dout, reinterpret_cast<double *>(ws + L.stat), nrows, K, m, nacc, nc,
+                                                          t->kmin + QMC_MAXSING);
+    ce = cudaGetLastError();
+  }
+  cudaEventRecord(static_cast<cudaEvent_t>(t->ev1), st);
+  if (ce != cudaSuccess) {
+    cudaGetLastError();
+    t->resident_ws = nullptr;
+    return QMC_ECUDA;
+  }
+  t->last.valid = true;
+  t->last.ws = dev_workspace;
+  t->last.m = m;
+  t->last.mode = mode;
+  t->last.nrows = nrows;
+  t->last.h2d = h2d;
+  return QMC_OK;
+}
+
+int qmc_result_fetch(const qmc_tables *tc, void *cuda_stream, void *dev_workspace, size_t dev_workspace_bytes,
+                     qmc_result *out) {
+  if (!tc || !out) return QMC_EINVAL;
+  qmc_tables *t = const_cast<qmc_tables *>(tc);
+  if (!t->last.valid || t->last.ws != dev_workspace) return QMC_EINVAL;
+  const int m = t->last.m, nrows = t->last.nrows, K = t->kmax - t->kmin + 1;
+  DevLayout L = layout(t, m);
+  if (dev_workspace_bytes < L.total) return QMC_ENOMEM;
+  if ((out->sector_coeff || out->sector_err || out->shift_sums) && t->last.mode != 2) return QMC_EINVAL;
+  unsigned char *ws = static_cast<unsigned char *>(dev_workspace);
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const StatLayout S = stat_layout(nrows, K, m);
+  t->stat_host.resize(S.total);
   unsigned long long hc[4] = {0, 0, 0, 0};
-  if (ce == cudaSuccess) ce = cudaMemcpyAsync(hout.data(), dout, hout.size() * 8, cudaMemcpyDeviceToHost, st);
+  // totals always; the per-sector block only when wanted
+  const size_t ncopy = (out->sector_coeff || out->sector_err || out->shift_sums) ? S.total : S.sector_coeff;
+  cudaError_t ce = cudaMemcpyAsync(t->stat_host.data(), ws + L.stat, ncopy * 8, cudaMemcpyDeviceToHost, st);
   if (ce == cudaSuccess) ce = cudaMemcpyAsync(hc, ws + L.counters, 32, cudaMemcpyDeviceToHost, st);
   if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
-  float ms = 0.f;
-  if (ce == cudaSuccess) cudaEventElapsedTime(&ms, e0, e1);
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
+  float ms = 0.f, ms_eval = 0.f;
+  if (ce == cudaSuccess) ce = cudaEventElapsedTime(&ms, static_cast<cudaEvent_t>(t->ev0), static_cast<cudaEvent_t>(t->ev1));
+  if (ce == cudaSuccess) ce = cudaEventElapsedTime(&ms_eval, static_cast<cudaEvent_t>(t->ev0), static_cast<cudaEvent_t>(t->evm));
   if (ce != cudaSuccess) {
     cudaGetLastError();
     t->resident_ws = nullptr;
     return QMC_ECUDA;
   }
   out->kernel_ms = ms;
-  out->kernel_launches = 2;
-  out->mode_used = mode;
+  out->eval_kernel_ms = ms_eval;
+  out->h2d_bytes = (int64_t)t->last.h2d;
+  out->d2h_bytes = (int64_t)(ncopy * 8 + 32);
+  out->kernel_launches = 3;
+  out->mode_used = t->last.mode;
   for (int q = 0; q < 4; ++q) out->counters[q] = (int64_t)hc[q];
-
-  // ---- S8: statistics (Eqs. 19-20), Re and Im separately (R:C15) ---------------------------------------
-  const int K = t->kmax - t->kmin + 1;
-  auto acc_index = [&](int k_index) { return (k_index + t->kmin) + QMC_MAXSING; };  // order -> accumulator
-  // per-shift totals T[k][kap][c]
-  std::vector<double> Tt((size_t)K * m * 2, 0.0);
-  const int nrows = persec ? (se - sb) : 1;
-  for (int row = 0; row < nrows; ++row)
-    for (int k = 0; k < K; ++k)
-      for (int c = 0; c < nc; ++c) {
-        int a = acc_index(k) * nc + c;
-        const double *src = hout.data() + ((size_t)row * nacc * nc + a) * m;
-        for (int kap = 0; kap < m; ++kap) Tt[((size_t)k * m + kap) * 2 + c] += src[kap];
-      }
-  for (int k = 0; k < K; ++k)
-    for (int c = 0; c < 2; ++c) {
-      double mean, err;
-      mean_err(Tt.data() + (size_t)k * m * 2 + c, 2, m, &mean, &err);
-      if (out->coeff) out->coeff[2 * k + c] = mean;
-      if (out->err) out->err[2 * k + c] = err;
-    }
-  if (out->shift_totals) std::memcpy(out->shift_totals, Tt.data(), Tt.size() * 8);
-  if (persec)
-    for (int row = 0; row < nrows; ++row)
-      for (int k = 0; k < K; ++k)
-        for (int c = 0; c < 2; ++c) {
-          std::vector<double> v((size_t)m, 0.0);
-          if (c < nc) {
-            int a = acc_index(k) * nc + c;
-            const double *src = hout.data() + ((size_t)row * nacc * nc + a) * m;
-            for (int kap = 0; kap < m; ++kap) v[kap] = src[kap];
-          }
-          size_t o2 = ((size_t)row * K + k);
-          if (out->shift_sums)
-            for (int kap = 0; kap < m; ++kap) out->shift_sums[(o2 * m + kap) * 2 + c] = v[kap];
-          double mean, err;
-          mean_err(v.data(), 1, m, &mean, &err);
-          if (out->sector_coeff) out->sector_coeff[o2 * 2 + c] = mean;
-          if (out->sector_err) out->sector_err[o2 * 2 + c] = err;
-        }
+  const double *h = t->stat_host.data();
+  if (out->shift_totals) std::memcpy(out->shift_totals, h + S.totals, (size_t)K * m * 2 * 8);
+  if (out->coeff) std::memcpy(out->coeff, h + S.coeff, (size_t)K * 2 * 8);
+  if (out->err) std::memcpy(out->err, h + S.err, (size_t)K * 2 * 8);
+  if (out->sector_coeff) std::memcpy(out->sector_coeff, h + S.sector_coeff, (size_t)nrows * K * 2 * 8);
+  if (out->sector_err) std::memcpy(out->sector_err, h + S.sector_err, (size_t)nrows * K * 2 * 8);
+  if (out->shift_sums) std::memcpy(out->shift_sums, h + S.shift_sums, (size_t)nrows * K * m * 2 * 8);
   return QMC_OK;
+}
+
+int qmc_result_device_totals(const qmc_tables *t, void *dev_workspace, size_t dev_workspace_bytes, void **totals_out) {
+  if (!t || !totals_out || !t->last.valid || t->last.ws != dev_workspace) return QMC_EINVAL;
+  DevLayout L = layout(t, t->last.m);
+  if (dev_workspace_bytes < L.total) return QMC_ENOMEM;
+  const StatLayout S = stat_layout(t->last.nrows, t->kmax - t->kmin + 1, t->last.m);
+  *totals_out = static_cast<unsigned char *>(dev_workspace) + L.stat + S.totals * 8;
+  return QMC_OK;
+}
+
+int qmc_integrate_ex(const qmc_tables *t, uint64_t N, int32_t m, uint64_t seed, const qmc_run *run, void *cuda_stream,
+                     void *dev_workspace, size_t dev_workspace_bytes, qmc_result *out) {
+  if (!t || !out) return QMC_EINVAL;
+  qmc_run r;
+  std::memset(&r, 0, sizeof r);
+  if (run) r = *run;
+  const bool want_persec = out->sector_coeff || out->sector_err || out->shift_sums;
+  if (r.mode == 0) r.mode = want_persec ? 2 : 1;
+  if (r.mode == 1 && want_persec) return QMC_EINVAL;
+  int rc = qmc_integrate_async(t, N, m, seed, &r, cuda_stream, dev_workspace, dev_workspace_bytes);
+  if (rc != QMC_OK) return rc;
+  return qmc_result_fetch(t, cuda_stream, dev_workspace, dev_workspace_bytes, out);
 }
 
 int qmc_integrate(const qmc_tables *t, uint64_t N, int32_t m, uint64_t seed, void *cuda_stream, void *dev_workspace,
                   size_t dev_workspace_bytes, qmc_result *out) {
   return qmc_integrate_ex(t, N, m, seed, nullptr, cuda_stream, dev_workspace, dev_workspace_bytes, out);
+}
+
+int qmc_statistics(const double *shift_totals, int32_t K, int32_t m, double *coeff, double *err) {
+  if (!shift_totals || K < 1 || m < 2) return QMC_EINVAL;
+  for (int k = 0; k < K; ++k)
+    for (int c = 0; c < 2; ++c) {
+      double mean, e;
+      mean_err(shift_totals + (size_t)k * m * 2 + c, 2, m, &mean, &e);
+      if (coeff) coeff[2 * k + c] = mean;
+      if (err) err[2 * k + c] = e;
+    }
+  return QMC_OK;
 }
 
 // Laurent series of e^{eg eps gammaE} base^{p0+p1 eps} Gamma(g0 + g1 eps)

@@ -1,0 +1,138 @@
+// qmc_flop_model: algorithmic FP64 operation count of the evaluation, from the sector tables (host only).
+//
+// This is the denominator-side bookkeeping of the roofline: the arithmetic the
+// product-form evaluation of Eqs. 9-12 + 14 needs, counted at the source level of the
+// scheme the kernels implement, with DFMA = 2 and DADD = DMUL = 1 and fixed costs for the library sequences
+// (fast paths of the CUDA 12.9 sm_100a FP64 routines, counted in SASS):
+//   log    : 17 DFMA + 7 DADD + 3 DMUL = 44      reciprocal: 5 DFMA = 10      division: 7 DFMA + 2 DMUL = 16
+//   atan2  : division + 19 DFMA polynomial + fix-ups = 60
+// Integer work (lattice index arithmetic, table decoding) and comparisons count as zero.  The count is
+// cross-checked against Nsight Compute's executed DFMA/DADD/DMUL thread-instruction counters (profiles/).
+#include <cstdlib>
+
+#include "../../include/qmc_feynman.h"
+#include "qmc_tables.h"
+
+namespace {
+const double F_LOG = 44.0, F_RCP = 10.0, F_DIV = 16.0, F_ATAN2 = 60.0;
+const double F_CMUL = 6.0, F_CADD = 2.0;                  // complex multiply (4 mul + 2 add), complex add
+const double F_CINV = 3.0 + F_RCP + 2.0;                  // |a|^2, reciprocal, two scalings
+const double F_CLOG = 3.0 + F_LOG + 1.0 + F_ATAN2;        // 0.5 log(|a|^2), atan2
+
+int degree(const QmcMono &m, int n) {
+  int d = 0;
+  for (int j = 0; j < n; ++j) d += m.e[j];
+  return d;
+}
+}  // namespace
+
+extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t sector_end, double *flops_point,
+                              double *flops_sectors, int64_t *corners) {
+  if (!t) return QMC_EINVAL;
+  const int n = t->n, nsec = (int)t->sectors.size();
+  const int sb = sector_begin, se = sector_end > 0 ? sector_end : nsec;
+  if (sb < 0 || se > nsec || sb >= se) return QMC_EINVAL;
+  const bool cplx = t->lambda > 0.0;
+  // S1-S3, once per (point, shift): u = r/N, y = u + Delta (wrap), t = y^2 (3 - 2y), w *= 6 y (1 - y), ln t, 1/t
+  const double per_point = n * (F_DIV + 2.0 + 4.0 + 4.0 + F_LOG + F_RCP);
+  double per_sectors = 0.0;
+  int64_t ncorners = 0;
+  const int eU = std::abs(t->aU0), eF = std::abs(t->aF0);
+  for (int si = sb; si < se; ++si) {
+    const QmcSector &s = t->sectors[si];
+    const int ns = s.nsing, K = t->kmax + ns + 1, nc = 1 << ns;
+    double f = 0.0;
+    // per-sector set-up: series (beta_j ln t_j)^p / p! of the singular variables, regular-variable factor and log
+    for (int j = 0; j < n; ++j) {
+      if (s.alpha[j] == -1) {
+        f += 1.0 + 2.0 * (K - 1);
+      } else {
+        if (s.alpha[j]) f += s.alpha[j];
+        if (s.beta[j]) f += 2.0;
+      }
+    }
+    if (!cplx) {
+      // U^, F^ at all 2^ns corners from ONE pass over the monomials (partial sums per group) + subset sums
+      for (int which = 0; which < 2; ++which)
+        for (const QmcMono &m : (which ? s.F : s.U)) f += degree(m, n) + 1.0;
+      f += 2.0 * ns * (nc / 2);
+      // per corner: integer powers, one division, two logs, Lambda, series g_Z = W exp(eps Lambda) truncated to K terms
+      f += nc * (eU + eF + 2.0 + F_DIV + 2.0 * F_LOG + 5.0 + 2.0 * (K - 1));
+      // fold (2^ns - 1 merges): d = (a - b)/t, out = b/beta + d * exp-series
+      f += (nc - 1) * (2.0 * (K - 1) + 1.0 + 2.0 * (K - 1) + (double)(K - 1) * (K - 2));
+      f += 2.0 * K;  // weight and accumulate
+    } else {
+      const double cs = 2.0;  // a real-by-complex scaling
+      for (int Z = 0; Z < nc; ++Z) {
+        // surviving monomials: those free of the variables in Z
+        auto in_Z = [&](int j) {  // j original index; singular variables are numbered in increasing original index
+          if (s.alpha[j] != -1) return false;
+          int b = 0;
+          for (int q = 0; q < j; ++q)
+            if (s.alpha[q] == -1) ++b;
+          return (Z >> b & 1) != 0;
+        };
+        int nfree = 0;
+        for (int j = 0; j < n; ++j)
+          if (!in_Z(j)) ++nfree;
+        // gradient + Hessian of F^ at the real corner point
+        for (const QmcMono &m : s.F) {
+          int zdeg = 0;
+          for (int j = 0; j < n; ++j)
+            if (in_Z(j)) zdeg += m.e[j];
+          if (zdeg > 1) continue;
+          f += degree(m, n) - zdeg;  // the monomial value
+          if (zdeg == 1) {
+            f += 1.0;  // contributes to one gradient component
+            continue;
+          }
+          for (int i = 0; i < n; ++i) {
+            if (in_Z(i) || !m.e[i]) continue;
+            f += 3.0;  // e_i * v / t_i, add
+            for (int k = i; k < n; ++k) {
+              if (in_Z(k)) continue;
+              int ek = m.e[k] - (k == i ? 1 : 0);
+              if (ek > 0) f += 3.0;
+            }
+          }
+        }
+        // rho, z, Jacobian entries
+        f += n * 4.0 + (double)nfree * nfree * 3.0 + nfree * 3.0;
+        // LU of the nfree x nfree complex block
+        for (int col = 0; col < nfree; ++col) {
+          f += F_CMUL;  // det *= pivot
+          int rem = nfree - col - 1;
+          if (rem > 0) f += F_CINV + rem * (F_CMUL + rem * (F_CMUL + F_CADD)) + rem * 6.0 /* pivot compares */;
+        }
+        // complex U^(z), F^(z)
+        for (int which = 0; which < 2; ++which)
+          for (const QmcMono &m : (which ? s.F : s.U)) {
+            bool dead = false;
+            for (int j = 0; j < n; ++j)
+              if (in_Z(j) && m.e[j]) dead = true;
+            if (dead) continue;
+            int d = degree(m, n);
+            f += (d > 0 ? cs + (d - 1) * F_CMUL : 0.0) + F_CADD;
+          }
+        // G_Z, Lambda_Z
+        f += F_CMUL;                                  // G0 det
+        for (int j = 0; j < n; ++j) {
+          if (!in_Z(j)) f += std::abs(s.alpha[j]) * F_CMUL;
+          if (s.beta[j]) f += F_CLOG + cs + F_CADD;
+        }
+        f += (eU + eF) * F_CMUL + F_CINV + F_CMUL;    // powers, W = num / den
+        f += 2.0 * F_CLOG + 2.0 * cs + F_CADD + 1.0;  // Lambda
+        f += (K - 1) * (F_CMUL + cs);                 // series
+      }
+      f += (nc - 1) * (K - 1) * (F_CADD + cs);                                                    // d = (a - b)/t
+      f += (nc - 1) * (cs + (K - 1) * (cs + F_CADD) + 0.5 * (K - 1) * (K - 2) * (cs + F_CADD));   // out
+      f += 4.0 * K;  // weight and accumulate
+    }
+    per_sectors += f;
+    ncorners += nc;
+  }
+  if (flops_point) *flops_point = per_point;
+  if (flops_sectors) *flops_sectors = per_sectors;
+  if (corners) *corners = ncorners;
+  return QMC_OK;
+}

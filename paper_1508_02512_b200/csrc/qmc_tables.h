@@ -54,8 +54,18 @@ struct qmc_tables {
   std::vector<uint32_t> secoff;   // [n_sectors + 1] byte offsets
   // launcher state (host-side caches; not thread-safe by design: one tables object per stream)
   const void *resident_ws = nullptr;  // workspace the image was last uploaded to
+  int resident_m = 0;                 // number of shift vectors resident in that workspace (0 = none)
   uint64_t cached_N = 0;              // generating vector cache
   uint64_t cached_z[QMC_MAXDIM] = {0};
+  std::vector<double> shifts_host;    // staging of the shift vectors (must outlive the async H2D copy)
+  std::vector<double> stat_host;      // staging of the fetched statistics block
+  void *ev0 = nullptr, *ev1 = nullptr, *evm = nullptr;  // cudaEvent_t: before / after all kernels, after the evaluation kernel
+  struct {
+    bool valid = false;
+    const void *ws = nullptr;
+    int m = 0, mode = 0, nrows = 0;
+    size_t h2d = 0;
+  } last;
 };
 
 // builds sectors (+ image) from a graph; returns a qmc_status
