@@ -1,0 +1,2 @@
+#include "qmc_inst2.cuh"
+QMC2_DEFINE_DIM(4)

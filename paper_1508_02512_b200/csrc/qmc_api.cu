@@ -2,6 +2,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <numeric>
@@ -151,7 +152,7 @@ uint64_t splitmix64(uint64_t &state) {
 uint64_t mulmod(uint64_t a, uint64_t b, uint64_t n) { return (uint64_t)(((unsigned __int128)a * b) % n); }
 
 struct DevLayout {
-  size_t image, secoff, shifts, counters, out, stat, partial, p2z, p2partial, total;
+  size_t image, secoff, image2, secoff2, logtab, work, shifts, counters, out, stat, partial, p2z, p2partial, total;
 };
 
 DevLayout layout(const qmc_tables *t, int m) {
@@ -160,6 +161,10 @@ DevLayout layout(const qmc_tables *t, int m) {
   size_t o = 0;
   L.image = o; o += align256(t->image.size());
   L.secoff = o; o += align256((nsec + 1) * 4);
+  L.image2 = o; o += align256(t->image2.size());
+  L.secoff2 = o; o += align256((nsec + 1) * 4);
+  L.logtab = o; o += align256(sizeof t->logtab);
+  L.work = o; o += align256((nsec + 1) * sizeof(Qmc2Work));
   L.shifts = o; o += align256((size_t)m * QMC_MAXDIM * 8);
   L.counters = o; o += 256;
   L.out = o; o += align256(nsec * QMC_NACC_MAX * 2 * (size_t)m * 8);
@@ -237,6 +242,98 @@ void mean_err(const double *v, size_t stride, int m, double *mean, double *err) 
   }
   *mean = q;
   *err = std::sqrt(d2 / ((double)m * (m - 1)));
+}
+
+// ---- version-2 launch (real path): work items = runs of sectors of one chunk ------------------------------------
+int launch_v2(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t st, uint64_t N, int m, int sb, int se,
+              bool persec, uint64_t ibeg, uint64_t istep, uint64_t icount, const uint64_t *z, int sms, int smem_optin,
+              int *gx_out, int *rows_out, size_t *h2d, cudaError_t *ce_out) {
+  const int n = t->n, nacc = QMC_MAXSING + t->kmax + 1, T = QMC2_THREADS;
+  uint32_t prog_cap = 0;
+  int max_nslots = 0;
+  for (const Qmc2Chunk &c : t->chunks)
+    if (c.sec_end > sb && c.sec_begin < se) {
+      prog_cap = std::max(prog_cap, c.prog_bytes);
+      max_nslots = std::max(max_nslots, c.nslots);
+    }
+  const size_t budget = (size_t)smem_optin - 1024;
+  const size_t fixed = prog_cap + 16 + (((size_t)m * n * 8 + 15) & ~(size_t)15) + (T / 32) * 8 + 128 * 16 + (size_t)max_nslots * T * 8;
+  const size_t accbytes = persec ? (size_t)nacc * T * 8 : 0;
+  std::vector<Qmc2Work> work;
+  uint32_t sec_cap = 0;
+  int max_nsec = 0;
+  for (const Qmc2Chunk &c : t->chunks) {
+    int a = std::max(sb, c.sec_begin);
+    const int e = std::min(se, c.sec_end);
+    while (a < e) {
+      int b = a;  // grow the run while it fits the shared-memory budget
+      while (b < e) {
+        const size_t bytes = t->secend2[b] - t->secoff2[a];
+        const size_t need = fixed + bytes + (((size_t)(b + 1 - a + 1) * 4 + 15) & ~(size_t)15) + accbytes * (b + 1 - a);
+        if (need > budget) break;
+        ++b;
+      }
+      if (b == a) return QMC_ENOMEM;
+      Qmc2Work w;
+      w.prog_off = c.prog_off;
+      w.prog_bytes = c.prog_bytes;
+      w.sec_off = t->secoff2[a];
+      w.sec_bytes = t->secend2[b - 1] - t->secoff2[a];
+      w.s0 = a;
+      w.nsec = b - a;
+      w.out_row = persec ? a - sb : (int)work.size();
+      w.pad = 0;
+      sec_cap = std::max(sec_cap, w.sec_bytes);
+      max_nsec = std::max(max_nsec, w.nsec);
+      work.push_back(w);
+      a = b;
+    }
+  }
+  const int nitems = (int)work.size();
+  const size_t smem = fixed + sec_cap + (((size_t)(max_nsec + 1) * 4 + 15) & ~(size_t)15) + accbytes * max_nsec;
+  int bps = 0;
+  CUDA_OK(qmc2_kernel_prepare(n, t->L, t->kmax, smem, &bps));
+  if (bps < 1) return QMC_ECUDA;
+  long long gx = ((long long)3 * sms * bps + nitems - 1) / nitems;
+  gx = std::min<long long>({gx, (long long)QMC_MAX_BLOCKS, (long long)((icount + T - 1) / T)});
+  gx = std::max<long long>(gx, 1);
+  // upload the work list unless the identical list is already there
+  const uint64_t key = ((uint64_t)sb << 40) ^ ((uint64_t)se << 20) ^ (persec ? 1u : 0u) ^ ((uint64_t)m << 50);
+  if (!(t->work_ws == ws && t->work_key == key)) {
+    t->work_host.assign(reinterpret_cast<const uint8_t *>(work.data()), reinterpret_cast<const uint8_t *>(work.data() + nitems));
+    CUDA_OK(cudaMemcpyAsync(ws + L.work, t->work_host.data(), t->work_host.size(), cudaMemcpyHostToDevice, st));
+    *h2d += t->work_host.size();
+    t->work_ws = ws;
+    t->work_key = key;
+  }
+  Qmc2Launch p;
+  std::memset(&p, 0, sizeof p);
+  p.image2 = ws + L.image2;
+  p.secoff2 = reinterpret_cast<const uint32_t *>(ws + L.secoff2);
+  p.work = reinterpret_cast<const Qmc2Work *>(ws + L.work);
+  p.logtab = reinterpret_cast<const double *>(ws + L.logtab);
+  p.shifts = reinterpret_cast<const double *>(ws + L.shifts);
+  p.partial = reinterpret_cast<double *>(ws + L.partial);
+  p.counters = reinterpret_cast<unsigned long long *>(ws + L.counters);
+  p.N = (uint32_t)N;
+  p.count = (uint32_t)icount;
+  for (int j = 0; j < n; ++j) {
+    p.zeff[j] = (uint32_t)mulmod(istep % N, z[j], N);
+    p.off[j] = (uint32_t)mulmod(ibeg, z[j], N);
+  }
+  p.m = m;
+  p.transform = t->transform;
+  p.persec = persec ? 1 : 0;
+  p.sm_prog_cap = prog_cap;
+  p.sm_sec_cap = (sec_cap + 15) & ~15u;
+  p.max_nsec = max_nsec;
+  p.max_nslots = max_nslots;
+  cudaEventRecord(static_cast<cudaEvent_t>(t->ev0), st);
+  *ce_out = qmc2_kernel_launch(n, t->L, t->kmax, dim3((unsigned)gx, nitems), smem, st, p);
+  cudaEventRecord(static_cast<cudaEvent_t>(t->evm), st);
+  *gx_out = (int)gx;
+  *rows_out = nitems;
+  return QMC_OK;
 }
 
 }  // namespace
@@ -448,6 +545,41 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
   CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   CUDA_OK(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
   const int nacc = QMC_MAXSING + t->kmax + 1, nc = cplx ? 2 : 1;
+  if (!t->ev0) {
+    CUDA_OK(cudaEventCreate(reinterpret_cast<cudaEvent_t *>(&t->ev0)));
+    CUDA_OK(cudaEventCreate(reinterpret_cast<cudaEvent_t *>(&t->ev1)));
+    CUDA_OK(cudaEventCreate(reinterpret_cast<cudaEvent_t *>(&t->evm)));
+  }
+  size_t h2d = 0;
+  int gx = 1, nchunks = 1;
+  cudaError_t ce = cudaSuccess;
+  double *partial = reinterpret_cast<double *>(ws + L.partial);
+  const bool use_v2 = !cplx && !t->image2.empty() && qmc2_kernel_available(n, t->L, t->kmax) && !std::getenv("QMC_FORCE_V1");
+  // ---- uploads common to both kernels (skipped when resident) ------------------------------------------------
+  if (!image_resident) {
+    h2d += t->image.size() + t->secoff.size() * 4;
+    CUDA_OK(cudaMemcpyAsync(ws + L.image, t->image.data(), t->image.size(), cudaMemcpyHostToDevice, st));
+    CUDA_OK(cudaMemcpyAsync(ws + L.secoff, t->secoff.data(), t->secoff.size() * 4, cudaMemcpyHostToDevice, st));
+    if (!t->image2.empty()) {
+      h2d += t->image2.size() + t->secoff2.size() * 4 + sizeof t->logtab;
+      CUDA_OK(cudaMemcpyAsync(ws + L.image2, t->image2.data(), t->image2.size(), cudaMemcpyHostToDevice, st));
+      CUDA_OK(cudaMemcpyAsync(ws + L.secoff2, t->secoff2.data(), t->secoff2.size() * 4, cudaMemcpyHostToDevice, st));
+      CUDA_OK(cudaMemcpyAsync(ws + L.logtab, t->logtab, sizeof t->logtab, cudaMemcpyHostToDevice, st));
+    }
+    t->resident_ws = dev_workspace;
+    t->resident_m = 0;
+  }
+  if (!shifts_resident) {
+    h2d += t->shifts_host.size() * 8;
+    CUDA_OK(cudaMemcpyAsync(ws + L.shifts, t->shifts_host.data(), t->shifts_host.size() * 8, cudaMemcpyHostToDevice, st));
+    t->resident_m = m;
+  }
+  CUDA_OK(cudaMemsetAsync(ws + L.counters, 0, 32, st));
+
+  if (use_v2) {
+    int rc = launch_v2(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, &gx, &nchunks, &h2d, &ce);
+    if (rc != QMC_OK) return rc;
+  } else {
   const size_t fixed_smem = 16 + (((size_t)m * n * 8 + 15) & ~(size_t)15) + (QMC_THREADS / 32) * 8 + (size_t)3 * n * QMC_THREADS * 8;
   const size_t per_sector_acc = persec ? (size_t)nacc * nc * QMC_THREADS * 8 : 0;
   // sectors per chunk: as many as fit the shared-memory budget (tables + per-sector accumulators)
@@ -480,29 +612,13 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
     }
     fits(spc, tab_bytes);
   }
-  const int nchunks = (se - sb + spc - 1) / spc;
+  nchunks = (se - sb + spc - 1) / spc;
   const size_t smem = tab_bytes + (((size_t)(spc + 1) * 4 + 15) & ~(size_t)15) + fixed_smem + per_sector_acc * spc;
   int bps = 0;
   CUDA_OK(qmc_kernel_prepare(n, t->kmax, cplx, smem, &bps));
   if (bps < 1) return QMC_ECUDA;
-  int gx = std::min<long long>({(long long)sms * bps, (long long)QMC_MAX_BLOCKS, (long long)((icount + QMC_THREADS - 1) / QMC_THREADS)});
+  gx = std::min<long long>({(long long)sms * bps, (long long)QMC_MAX_BLOCKS, (long long)((icount + QMC_THREADS - 1) / QMC_THREADS)});
   gx = std::max(gx, 1);
-
-  // ---- uploads (skipped when resident) ------------------------------------------------------------------
-  size_t h2d = 0;
-  if (!image_resident) {
-    h2d += t->image.size() + t->secoff.size() * 4;
-    CUDA_OK(cudaMemcpyAsync(ws + L.image, t->image.data(), t->image.size(), cudaMemcpyHostToDevice, st));
-    CUDA_OK(cudaMemcpyAsync(ws + L.secoff, t->secoff.data(), t->secoff.size() * 4, cudaMemcpyHostToDevice, st));
-    t->resident_ws = dev_workspace;
-    t->resident_m = 0;
-  }
-  if (!shifts_resident) {
-    h2d += t->shifts_host.size() * 8;
-    CUDA_OK(cudaMemcpyAsync(ws + L.shifts, t->shifts_host.data(), t->shifts_host.size() * 8, cudaMemcpyHostToDevice, st));
-    t->resident_m = m;
-  }
-  CUDA_OK(cudaMemsetAsync(ws + L.counters, 0, 32, st));
 
   QmcLaunch p;
   std::memset(&p, 0, sizeof p);
@@ -526,21 +642,17 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
   p.persec = persec ? 1 : 0;
   p.tab_smem_bytes = (tab_bytes + 15) & ~15u;
 
-  if (!t->ev0) {
-    CUDA_OK(cudaEventCreate(reinterpret_cast<cudaEvent_t *>(&t->ev0)));
-    CUDA_OK(cudaEventCreate(reinterpret_cast<cudaEvent_t *>(&t->ev1)));
-    CUDA_OK(cudaEventCreate(reinterpret_cast<cudaEvent_t *>(&t->evm)));
-  }
   cudaEventRecord(static_cast<cudaEvent_t>(t->ev0), st);
-  cudaError_t ce = qmc_kernel_launch(n, t->kmax, cplx, dim3(gx, nchunks), smem, st, p);
+  ce = qmc_kernel_launch(n, t->kmax, cplx, dim3(gx, nchunks), smem, st, p);
   cudaEventRecord(static_cast<cudaEvent_t>(t->evm), st);
+  }
   const int rows = persec ? (se - sb) : nchunks;
   const int nrows = persec ? (se - sb) : 0;  // per-sector rows of the statistics block
   const int nout = (persec ? (se - sb) : 1) * nacc * nc * m;
   const int K = t->kmax - t->kmin + 1;
   double *dout = reinterpret_cast<double *>(ws + L.out);
   if (ce == cudaSuccess) {
-    qmc_finalize_kernel<<<(nout + 127) / 128, 128, 0, st>>>(p.partial, dout, rows, m, gx, nacc * nc, 1.0 / (double)N, persec ? 1 : 0);
+    qmc_finalize_kernel<<<(nout + 127) / 128, 128, 0, st>>>(partial, dout, rows, m, gx, nacc * nc, 1.0 / (double)N, persec ? 1 : 0);
     ce = cudaGetLastError();
   }
   if (ce == cudaSuccess) {

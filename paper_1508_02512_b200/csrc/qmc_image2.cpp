@@ -1,0 +1,260 @@
+// Version-2 device image of the sector tables (real path): chunks, per-chunk slot programs, 16-byte monomial records.
+// Host only.  See qmc_tables.h for the layout and DESIGN.md "Data layout" for the rationale.
+//
+// The slot program is found by a byte-pair-encoding style pass: a monomial is a multiset of factors (initially the
+// variables t_j, repeated by exponent); the most frequent pair of factors over the chunk becomes a new slot (their
+// product, computed once per lattice point) and replaces the pair everywhere; repeat until every monomial has at
+// most two factors (mandatory) and, with the slots that are left, as many as possible have one.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+
+#include "../../include/qmc_feynman.h"
+#include "qmc_tables.h"
+
+namespace {
+
+typedef std::vector<uint8_t> Factors;  // sorted slot ids
+
+struct ChunkPlan {
+  int nslots = 0, first_prod = 0;
+  std::vector<std::pair<uint8_t, uint8_t>> prog;  // slot[first_prod + i] = slot[a] * slot[b]
+  std::vector<Factors> mono;                      // per monomial (order of collection)
+};
+
+Factors factors_of(const uint8_t *e, int n) {
+  Factors f;
+  for (int j = 0; j < n; ++j)
+    for (int q = 0; q < e[j]; ++q) f.push_back((uint8_t)j);
+  return f;
+}
+
+// replace every occurrence of the pair (a, b) in m by `nw`
+void merge_pair(Factors &m, int a, int b, int nw) {
+  for (;;) {
+    auto ia = std::find(m.begin(), m.end(), (uint8_t)a);
+    if (ia == m.end()) return;
+    auto ib = (a == b) ? std::find(ia + 1, m.end(), (uint8_t)b) : std::find(m.begin(), m.end(), (uint8_t)b);
+    if (ib == m.end()) return;
+    if (ib < ia) std::swap(ia, ib);
+    m.erase(ib);
+    m.erase(ia);
+    m.push_back((uint8_t)nw);
+  }
+}
+
+// returns false if some monomial still has more than two factors when the slots run out
+bool plan_chunk(ChunkPlan &pl, int n, int max_slots) {
+  pl.first_prod = 3 * n + 1;
+  pl.nslots = pl.first_prod;
+  pl.prog.clear();
+  for (;;) {
+    static thread_local int cnt[QMC2_MAXSLOTS][QMC2_MAXSLOTS];
+    std::memset(cnt, 0, sizeof cnt);
+    bool any_big = false;
+    for (const Factors &m : pl.mono) {
+      if (m.size() < 2) continue;
+      const int wgt = m.size() > 2 ? 64 : 1;
+      if (m.size() > 2) any_big = true;
+      std::pair<uint8_t, uint8_t> seen[128];  // each distinct pair counts once per monomial (m is sorted)
+      int nseen = 0;
+      for (size_t i = 0; i < m.size(); ++i)
+        for (size_t k = i + 1; k < m.size(); ++k) {
+          const std::pair<uint8_t, uint8_t> pr(m[i], m[k]);
+          bool dup = false;
+          for (int q = 0; q < nseen; ++q) dup = dup || seen[q] == pr;
+          if (dup || nseen >= 128) continue;
+          seen[nseen++] = pr;
+          cnt[pr.first][pr.second] += wgt;
+        }
+    }
+    int best = 0, ba = -1, bb = -1;
+    for (int a = 0; a < pl.nslots; ++a)
+      for (int b = a; b < pl.nslots; ++b)
+        if (cnt[a][b] > best) {
+          best = cnt[a][b];
+          ba = a;
+          bb = b;
+        }
+    if (ba < 0) break;                    // every monomial has at most one factor
+    if (!any_big && best < 2) break;      // optional phase: a slot must serve at least two monomials
+    if (pl.nslots >= max_slots) {
+      if (any_big) return false;
+      break;
+    }
+    const int nw = pl.nslots++;
+    pl.prog.push_back({(uint8_t)ba, (uint8_t)bb});
+    for (Factors &m : pl.mono) {
+      merge_pair(m, ba, bb, nw);
+      std::sort(m.begin(), m.end());
+    }
+  }
+  for (const Factors &m : pl.mono)
+    if (m.size() > 2) return false;
+  return true;
+}
+
+void collect(const qmc_tables *t, int s0, int s1, ChunkPlan &pl) {
+  pl.mono.clear();
+  const int n = t->n;
+  for (int si = s0; si < s1; ++si) {
+    const QmcSector &s = t->sectors[si];
+    uint8_t g[QMC_MAXDIM] = {0};
+    for (int j = 0; j < n; ++j) g[j] = (uint8_t)(s.alpha[j] > 0 ? s.alpha[j] : 0);
+    pl.mono.push_back(factors_of(g, n));  // G0 = prod over regular variables of t_j^alpha_j
+    for (const QmcMono &m : s.U) pl.mono.push_back(factors_of(m.e, n));
+    for (const QmcMono &m : s.F) pl.mono.push_back(factors_of(m.e, n));
+  }
+}
+
+double sector_cost(const QmcSector &s, int kmax) {
+  const int nc = 1 << s.nsing, K = kmax + s.nsing + 1;
+  return 4.0 * (s.U.size() + s.F.size() + 4) + nc * (30.0 + 2.0 * K) + (nc - 1) * (4.0 * K + 0.5 * K * K);
+}
+
+template <class T>
+void put(std::vector<uint8_t> &img, const T &v) {
+  const uint8_t *b = reinterpret_cast<const uint8_t *>(&v);
+  img.insert(img.end(), b, b + sizeof(T));
+}
+
+}  // namespace
+
+// table of the kernels' logarithm: z in [0.6875, 1.375) by the top bits of the high word, c_i = interval centre
+static void build_logtab(double *tab) {
+  for (int i = 0; i < 128; ++i) {
+    const uint64_t lo = ((uint64_t)(0x3fe60000u + ((uint32_t)i << 13))) << 32, hi = lo + ((uint64_t)0x2000 << 32);
+    double zl, zh;
+    std::memcpy(&zl, &lo, 8);
+    std::memcpy(&zh, &hi, 8);
+    const double invc = (double)(1.0L / (0.5L * ((long double)zl + (long double)zh)));
+    tab[2 * i] = invc;
+    tab[2 * i + 1] = (double)(-logl((long double)invc));
+  }
+}
+
+int qmc_build_image2(qmc_tables *t) {
+  build_logtab(t->logtab);
+  t->image2.clear();
+  t->secoff2.clear();
+  t->chunks.clear();
+  t->secend2.clear();
+  const int n = t->n, nsec = (int)t->sectors.size();
+  if (t->lambda > 0.0 || nsec == 0) return QMC_OK;  // complex path keeps the version-1 image
+  if (3 * n + 1 >= QMC2_MAXSLOTS) return QMC_EUNSUPPORTED;
+
+  // ---- chunk boundaries: contiguous ranges of about equal modelled cost, about 20 KB of tables each ------------
+  std::vector<double> cost(nsec);
+  double total_cost = 0.0, total_bytes = 0.0;
+  for (int i = 0; i < nsec; ++i) {
+    const QmcSector &s = t->sectors[i];
+    cost[i] = sector_cost(s, t->kmax);
+    total_cost += cost[i];
+    total_bytes += sizeof(Qmc2SectorHdr) + 16.0 * (s.U.size() + s.F.size() + 1 + n);
+  }
+  int nch = std::max(1, (int)(total_bytes / 20000.0 + 0.999));
+  std::vector<std::pair<int, int>> todo;  // ranges still to plan (processed in order)
+  {
+    int b = 0;
+    double acc = 0.0;
+    for (int c = 0; c < nch; ++c) {
+      const double target = total_cost * (c + 1) / nch;
+      int e = b;
+      while (e < nsec && (acc + cost[e] <= target || e == b)) acc += cost[e++];
+      if (c == nch - 1) e = nsec;
+      if (e > b) todo.push_back({b, e});
+      b = e;
+    }
+  }
+  // ---- plan (split a range in two when the slot budget does not suffice) and emit -----------------------------
+  t->secoff2.assign(nsec + 1, 0);
+  t->secend2.assign(nsec, 0);
+  for (size_t w = 0; w < todo.size(); ++w) {
+    const int s0 = todo[w].first, s1 = todo[w].second;
+    ChunkPlan pl;
+    collect(t, s0, s1, pl);
+    if (!plan_chunk(pl, n, QMC2_MAXSLOTS)) {
+      if (s1 - s0 == 1) return QMC_EUNSUPPORTED;
+      const int mid = (s0 + s1) / 2;
+      todo[w] = {s0, mid};
+      todo.insert(todo.begin() + w + 1, {mid, s1});
+      --w;
+      continue;
+    }
+    Qmc2Chunk ch;
+    ch.sec_begin = s0;
+    ch.sec_end = s1;
+    ch.nslots = pl.nslots;
+    ch.prog_off = (uint32_t)t->image2.size();
+    Qmc2ChunkHdr chh = {(uint32_t)pl.nslots, (uint32_t)pl.prog.size(), (uint32_t)pl.first_prod, 0u};
+    put(t->image2, chh);
+    for (auto &pr : pl.prog) {
+      put(t->image2, (uint16_t)(pr.first * QMC2_THREADS));
+      put(t->image2, (uint16_t)(pr.second * QMC2_THREADS));
+    }
+    while (t->image2.size() % 16) t->image2.push_back(0);
+    ch.prog_bytes = (uint32_t)t->image2.size() - ch.prog_off;
+    const uint16_t ONE = (uint16_t)(3 * n * QMC2_THREADS);
+    size_t mi = 0;  // index into pl.mono, same order as collect()
+    auto rec_of = [&](double c, const Factors &f) {
+      Qmc2Rec r;
+      r.c = c;
+      r.s0 = f.size() > 0 ? (uint16_t)(f[0] * QMC2_THREADS) : ONE;
+      r.s1 = f.size() > 1 ? (uint16_t)(f[1] * QMC2_THREADS) : ONE;
+      r.pad = 0;
+      return r;
+    };
+    for (int si = s0; si < s1; ++si) {
+      const QmcSector &s = t->sectors[si];
+      ch.cost += cost[si];
+      Qmc2SectorHdr h;
+      std::memset(&h, 0, sizeof h);
+      int pos_of[QMC_MAXDIM], k = 0;
+      for (int j = 0; j < n; ++j) pos_of[j] = -1;
+      for (int j = 0; j < n; ++j)
+        if (s.alpha[j] == -1) {
+          h.sing_ln[k] = (uint16_t)((n + j) * QMC2_THREADS);
+          h.sing_inv[k] = (uint16_t)((2 * n + j) * QMC2_THREADS);
+          h.beta[k] = (double)s.beta[j];
+          h.invbeta[k] = 1.0 / (double)s.beta[j];
+          pos_of[j] = k++;
+        }
+      h.nsing = (uint8_t)s.nsing;
+      std::vector<Qmc2Rec> recs;
+      recs.push_back(rec_of(1.0, pl.mono[mi++]));  // G0
+      for (int j = 0; j < n; ++j)                  // L0 = sum over regular variables of beta_j ln t_j
+        if (s.alpha[j] != -1 && s.beta[j] != 0) {
+          Qmc2Rec r;
+          r.c = (double)s.beta[j];
+          r.s0 = (uint16_t)((n + j) * QMC2_THREADS);
+          r.s1 = ONE;
+          r.pad = 0;
+          recs.push_back(r);
+          ++h.nL0;
+        }
+      for (int which = 0; which < 2; ++which) {
+        const std::vector<QmcMono> &M = which ? s.F : s.U;  // already group-sorted by qmc_build_tables
+        int gprev = 0;
+        for (const QmcMono &m : M) {
+          int g = 0;
+          for (int j = 0; j < n; ++j)
+            if (m.e[j] && pos_of[j] >= 0) g |= 1 << pos_of[j];
+          if (g < gprev) return QMC_EINVAL;  // monomials must arrive sorted by group
+          gprev = g;
+          uint8_t &c = (which ? h.cntF : h.cntU)[g];
+          if (c == 255) return QMC_EUNSUPPORTED;
+          ++c;
+          recs.push_back(rec_of(m.c, pl.mono[mi++]));
+        }
+      }
+      h.nrec = (uint16_t)recs.size();
+      t->secoff2[si] = (uint32_t)t->image2.size();
+      put(t->image2, h);
+      for (const Qmc2Rec &r : recs) put(t->image2, r);
+      t->secend2[si] = (uint32_t)t->image2.size();
+    }
+    t->chunks.push_back(ch);
+  }
+  t->secoff2[nsec] = (uint32_t)t->image2.size();
+  return QMC_OK;
+}

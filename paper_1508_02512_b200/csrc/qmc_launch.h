@@ -26,6 +26,32 @@ struct QmcLaunch {
 };
 
 
+// ---- version 2 (real path) --------------------------------------------------------------------------------
+struct Qmc2Work {  // one block column (blockIdx.y): a run of sectors of one chunk
+  uint32_t prog_off, prog_bytes;  // chunk header + slot program in image2
+  uint32_t sec_off, sec_bytes;    // the sector blocks
+  int32_t s0, nsec;               // first sector (global index), number of sectors
+  int32_t out_row;                // fused: row of the partial buffer; per-sector: row of the first sector
+  int32_t pad;
+};
+struct Qmc2Launch {
+  const uint8_t *image2;
+  const uint32_t *secoff2;       // device: [n_sectors+1]
+  const Qmc2Work *work;          // device: [gridDim.y]
+  const double *logtab;          // device: 128 x {1/c, -ln(1/c)}
+  const double *shifts;
+  double *partial;
+  unsigned long long *counters;
+  uint32_t N, count;
+  uint32_t zeff[QMC_MAXDIM], off[QMC_MAXDIM];
+  int32_t m, transform, persec;
+  uint32_t sm_prog_cap, sm_sec_cap;  // shared-memory bytes reserved for the slot program and the sector blocks
+  int32_t max_nsec, max_nslots;
+};
+cudaError_t qmc2_kernel_prepare(int ndim, int loops, int kmax, size_t smem, int *blocks_per_sm);
+cudaError_t qmc2_kernel_launch(int ndim, int loops, int kmax, dim3 grid, size_t smem, cudaStream_t st, const Qmc2Launch &p);
+bool qmc2_kernel_available(int ndim, int loops, int kmax);
+
 // implemented in qmc_dispatch.cu on top of one translation unit per dimension (qmc_inst_d<N>.cu)
 cudaError_t qmc_kernel_prepare(int ndim, int kmax, bool cplx, size_t smem, int *blocks_per_sm);
 cudaError_t qmc_kernel_launch(int ndim, int kmax, bool cplx, dim3 grid, size_t smem, cudaStream_t st, const QmcLaunch &p);

@@ -345,5 +345,5 @@ int qmc_build_tables(const qmc_graph *g, const qmc_kinematics *kin, int eps_orde
     while (T->image.size() % 16) T->image.push_back(0);
   }
   T->secoff.push_back((uint32_t)T->image.size());
-  return QMC_OK;
+  return qmc_build_image2(T);
 }

@@ -1,6 +1,7 @@
 // Internal (not part of the C ABI): host-side sector tables and the device table image.
 // Shared by qmc_prepare.cpp (host decomposer), qmc_api.cu (launcher) and the kernels.
 #pragma once
+#include <cstddef>
 #include <cstdint>
 #include <vector>
 
@@ -29,6 +30,44 @@ struct QmcSectorHdr {
 };
 static_assert(sizeof(QmcSectorHdr) == 64, "sector header must be 64 bytes");
 
+// ---- device image, version 2 (real path) ------------------------------------------------------------
+// Sectors are grouped into CHUNKS.  Every chunk owns a "slot program": each thread keeps, per lattice point, a table
+// of per-point values in shared memory (slot s of thread tid at slots[s * QMC2_THREADS + tid]):
+//   slots [0,n) t_j | [n,2n) ln t_j | [2n,3n) 1/t_j | 3n: 1.0 | 3n+1 ...: products slot[k] = slot[a] * slot[b]
+// chosen per chunk by a byte-pair-encoding style pass over the chunk's monomials (most frequent pair of factors
+// first) until every monomial is a product of at most two slots.  A monomial is then one 16-byte record.
+#define QMC2_THREADS 256
+#define QMC2_MAXSLOTS 56
+struct Qmc2Rec {        // value = c * slot[s0] * slot[s1]; s0, s1 are slot indices premultiplied by QMC2_THREADS
+  double c;
+  uint16_t s0, s1;
+  uint32_t pad;
+};
+static_assert(sizeof(Qmc2Rec) == 16, "record must be 16 bytes");
+struct Qmc2SectorHdr {  // followed by records: [G0][L0 x nL0][U^ by group][F^ by group]
+  uint8_t nsing, nL0;
+  uint16_t nrec;
+  uint32_t pad0;
+  uint16_t sing_ln[QMC_MAXSING];   // premultiplied slot index of ln t_k for singular position k
+  uint16_t sing_inv[QMC_MAXSING];  // ... of 1/t_k
+  double invbeta[QMC_MAXSING];     // 1/beta_k
+  double beta[QMC_MAXSING];        // beta_k
+  uint8_t pad1[8];
+  uint8_t cntU[1 << QMC_MAXSING];  // records per group (set of singular positions the monomial depends on); 16-byte aligned
+  uint8_t cntF[1 << QMC_MAXSING];
+};
+static_assert(offsetof(Qmc2SectorHdr, cntU) % 16 == 0, "group counts are read as one 16-byte word");
+static_assert(sizeof(Qmc2SectorHdr) == 128, "v2 sector header");
+struct Qmc2ChunkHdr {   // 16 bytes, followed by nprog x {u16 a, u16 b} (premultiplied), padded to 16 bytes
+  uint32_t nslots, nprog, first_prod, pad;
+};
+struct Qmc2Chunk {      // host description of one chunk
+  int sec_begin = 0, sec_end = 0;
+  int nslots = 0;
+  uint32_t prog_off = 0, prog_bytes = 0;  // chunk header + slot program in image2
+  double cost = 0.0;                      // modelled flops per point (load balancing)
+};
+
 // ---- host tables --------------------------------------------------------------------------------
 struct QmcMono {
   double c;
@@ -52,11 +91,20 @@ struct qmc_tables {
   // device image
   std::vector<uint8_t> image;     // concatenated sector blocks (16-byte aligned each)
   std::vector<uint32_t> secoff;   // [n_sectors + 1] byte offsets
+  // version 2 image (real path only; empty when lambda > 0)
+  std::vector<uint8_t> image2;
+  std::vector<uint32_t> secoff2;  // [n_sectors + 1] byte offsets of the sector blocks in image2
+  std::vector<uint32_t> secend2;  // [n_sectors] end offsets (a chunk header sits between the sectors of two chunks)
+  std::vector<Qmc2Chunk> chunks;
+  double logtab[256] = {0};      // 128 x {1/c_i, -ln(1/c_i)} of the kernels' table-driven logarithm
   // launcher state (host-side caches; not thread-safe by design: one tables object per stream)
   const void *resident_ws = nullptr;  // workspace the image was last uploaded to
   int resident_m = 0;                 // number of shift vectors resident in that workspace (0 = none)
   uint64_t cached_N = 0;              // generating vector cache
   uint64_t cached_z[QMC_MAXDIM] = {0};
+  std::vector<uint8_t> work_host;     // staging of the version-2 work list
+  const void *work_ws = nullptr;      // workspace / key of the work list resident on the device
+  uint64_t work_key = 0;
   std::vector<double> shifts_host;    // staging of the shift vectors (must outlive the async H2D copy)
   std::vector<double> stat_host;      // staging of the fetched statistics block
   void *ev0 = nullptr, *ev1 = nullptr, *evm = nullptr;  // cudaEvent_t: before / after all kernels, after the evaluation kernel
@@ -69,5 +117,7 @@ struct qmc_tables {
 };
 
 // builds sectors (+ image) from a graph; returns a qmc_status
+// builds image2 / secoff2 / chunks from `sectors` (real path); returns a qmc_status
+int qmc_build_image2(qmc_tables *t);
 int qmc_build_tables(const qmc_graph *g, const qmc_kinematics *kin, int eps_order, const qmc_options *opt,
                      qmc_tables *out);
