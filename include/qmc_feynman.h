@@ -171,6 +171,9 @@ int qmc_prefactor_series(double eg, double base, double p0, double p1, int32_t g
 /* Sustained FP64 FMA rate of the device (register-resident DFMA chains), in FLOP/s (DFMA = 2).  The roofline
  * denominator of the evaluation kernel (MEASURED_PEAKS.json has no FP64 entry). */
 int qmc_fp64_peak(void *cuda_stream, void *dev_workspace, size_t dev_workspace_bytes, double *flops_out, double *ms_out);
+/* Human-readable description of the device tables (chunks, slot programs, record counts) written to buf as a
+ * NUL-terminated string, truncated to len bytes.  Diagnostics only. */
+int qmc_tables_describe(const qmc_tables *t, char *buf, size_t len);
 const char *qmc_strerror(int status);
 
 #ifdef __cplusplus

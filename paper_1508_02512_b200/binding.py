@@ -106,6 +106,8 @@ def lib():
                                            C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_int32)]
         L.qmc_fp64_peak.restype = C.c_int
         L.qmc_fp64_peak.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.qmc_tables_describe.restype = C.c_int
+        L.qmc_tables_describe.argtypes = [C.c_void_p, C.c_char_p, C.c_size_t]
         L.qmc_strerror.restype = C.c_char_p
         L.qmc_strerror.argtypes = [C.c_int]
         _lib = L
@@ -153,6 +155,11 @@ class Tables:
         if rc:
             raise QmcError(rc, "qmc_tables_export")
         return buf
+
+    def describe(self) -> str:
+        buf = C.create_string_buffer(1 << 16)
+        lib().qmc_tables_describe(self._h, buf, len(buf))
+        return buf.value.decode()
 
     def workspace_bytes(self, N: int, m: int) -> int:
         return int(lib().qmc_workspace_bytes(self._h, N, m))

@@ -6,6 +6,7 @@
 #include <cstring>
 #include <new>
 #include <numeric>
+#include <string>
 #include <vector>
 
 #include <cuda_runtime.h>
@@ -254,7 +255,7 @@ int launch_v2(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
   for (const Qmc2Chunk &c : t->chunks)
     if (c.sec_end > sb && c.sec_begin < se) {
       prog_cap = std::max(prog_cap, c.prog_bytes);
-      max_nslots = std::max(max_nslots, c.nslots);
+      max_nslots = std::max(max_nslots, c.nslots + c.max_local);
     }
   const size_t budget = (size_t)smem_optin - 1024;
   const size_t fixed = prog_cap + 16 + (((size_t)m * n * 8 + 15) & ~(size_t)15) + (T / 32) * 8 + 128 * 16 + (size_t)max_nslots * T * 8;
@@ -800,6 +801,33 @@ int qmc_prefactor_series(double eg, double base, double p0, double p1, int32_t g
   }
   for (int k = 0; k < n; ++k) series_out[k] = S[k] * scale;
   if (lowest_order) *lowest_order = lo;
+  return QMC_OK;
+}
+
+int qmc_tables_describe(const qmc_tables *t, char *buf, size_t len) {
+  if (!t || !buf || len < 1) return QMC_EINVAL;
+  std::string o;
+  char line[256];
+  std::snprintf(line, sizeof line, "sectors %d dim %d loops %d orders %d..%d lambda %g image1 %zu B image2 %zu B chunks %zu\n",
+                (int)t->sectors.size(), t->n, t->L, t->kmin, t->kmax, t->lambda, t->image.size(), t->image2.size(), t->chunks.size());
+  o += line;
+  for (size_t c = 0; c < t->chunks.size(); ++c) {
+    const Qmc2Chunk &ch = t->chunks[c];
+    int nrec = 0, two = 0, nloc = 0;
+    for (int s = ch.sec_begin; s < ch.sec_end; ++s) {
+      const Qmc2SectorHdr *h = reinterpret_cast<const Qmc2SectorHdr *>(t->image2.data() + t->secoff2[s]);
+      const Qmc2Rec *r = reinterpret_cast<const Qmc2Rec *>(reinterpret_cast<const uint8_t *>(h + 1) + ((h->nlocal * 4 + 15) & ~15));
+      for (int i = 0; i < h->nrec; ++i) {
+        ++nrec;
+        if (r[i].s1 != 3 * t->n * QMC2_THREADS) ++two;
+      }
+      nloc += h->nlocal;
+    }
+    std::snprintf(line, sizeof line, "chunk %zu: sectors [%d,%d) slots %d program %u B tables %u B records %d (two-factor %d, local products %d) cost %.0f\n", c,
+                  ch.sec_begin, ch.sec_end, ch.nslots, ch.prog_bytes, t->secend2[ch.sec_end - 1] - t->secoff2[ch.sec_begin], nrec, two, nloc, ch.cost);
+    o += line;
+  }
+  std::snprintf(buf, len, "%s", o.c_str());
   return QMC_OK;
 }
 

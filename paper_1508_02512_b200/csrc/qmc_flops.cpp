@@ -8,6 +8,7 @@
 //   atan2  : division + 19 DFMA polynomial + fix-ups = 60
 // Integer work (lattice index arithmetic, table decoding) and comparisons count as zero.  The count is
 // cross-checked against Nsight Compute's executed DFMA/DADD/DMUL thread-instruction counters (profiles/).
+#include <algorithm>
 #include <cstdlib>
 
 #include "../../include/qmc_feynman.h"
@@ -52,14 +53,34 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
       }
     }
     if (!cplx) {
-      // U^, F^ at all 2^ns corners from ONE pass over the monomials (partial sums per group) + subset sums
-      for (int which = 0; which < 2; ++which)
-        for (const QmcMono &m : (which ? s.F : s.U)) f += degree(m, n) + 1.0;
-      f += 2.0 * ns * (nc / 2);
-      // per corner: integer powers, one division, two logs, Lambda, series g_Z = W exp(eps Lambda) truncated to K terms
-      f += nc * (eU + eF + 2.0 + F_DIV + 2.0 * F_LOG + 5.0 + 2.0 * (K - 1));
-      // fold (2^ns - 1 merges): d = (a - b)/t, out = b/beta + d * exp-series
-      f += (nc - 1) * (2.0 * (K - 1) + 1.0 + 2.0 * (K - 1) + (double)(K - 1) * (K - 2));
+      // version-2 scheme (qmc_kernels2.cuh).  A record c * slot * slot is DMUL + DFMA = 3.
+      auto pow_muls = [](int e) {  // multiplications of x^e by repeated squaring, e >= 0
+        int c = 0;
+        for (int q = e; q > 1; q >>= 1) c += 1 + (q & 1);
+        return (double)c;
+      };
+      const double F_RCP2 = 8.0;    // MUFU seed + 4 DFMA
+      const double F_LOG2 = 16.0;   // table-driven: 7 DFMA + DMUL + DADD
+      int nL0 = 0;
+      for (int j = 0; j < n; ++j)
+        if (s.alpha[j] != -1 && s.beta[j]) ++nL0;
+      f = 3.0 * (1 + nL0 + s.U.size() + s.F.size());   // G0, L0, U^, F^ records (replaces the set-up count above)
+      f += 2.0 * ns * (nc / 2);                        // subset sums
+      for (int j = 0; j < n; ++j)
+        if (s.alpha[j] == -1) f += 1.0 + 2.0 * std::max(0, K - 2);   // series of beta_j ln t_j
+      for (int Z = 0; Z < nc; ++Z) {
+        const int len = t->kmax + __builtin_popcount(Z) + 1;       // leaf window
+        f += F_RCP2 + (t->aU0 < 0 ? F_RCP2 : 0.0);
+        f += (t->aU0 ? pow_muls(eU) + 1.0 : 0.0) + (t->aF0 ? pow_muls(eF) + 1.0 : 0.0);
+        if (len > 1) f += pow_muls(std::abs(t->aU1)) + pow_muls(std::abs(t->aF1)) + 1.0 + F_LOG2 + 1.0;
+        f += 2.0 * (len - 1);
+      }
+      // fold: merge at level l with Z the choices of the levels below l
+      for (int l = 0; l < ns; ++l)
+        for (int Z = 0; Z < (1 << l); ++Z) {
+          const int len = ns - l + t->kmax + __builtin_popcount(Z) + 1;
+          f += 2.0 * (len - 1) + 1.0 + (double)len * (len - 1);
+        }
       f += 2.0 * K;  // weight and accumulate
     } else {
       const double cs = 2.0;  // a real-by-complex scaling

@@ -7,6 +7,7 @@
 // most two factors (mandatory) and, with the slots that are left, as many as possible have one.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 
 #include "../../include/qmc_feynman.h"
@@ -76,12 +77,10 @@ bool plan_chunk(ChunkPlan &pl, int n, int max_slots) {
           ba = a;
           bb = b;
         }
+    (void)any_big;
     if (ba < 0) break;                    // every monomial has at most one factor
-    if (!any_big && best < 2) break;      // optional phase: a slot must serve at least two monomials
-    if (pl.nslots >= max_slots) {
-      if (any_big) return false;
-      break;
-    }
+    if (best < 2) break;                  // a chunk-wide slot must serve at least two monomials
+    if (pl.nslots >= max_slots) break;    // leftovers with more than two factors get sector-local products
     const int nw = pl.nslots++;
     pl.prog.push_back({(uint8_t)ba, (uint8_t)bb});
     for (Factors &m : pl.mono) {
@@ -89,8 +88,6 @@ bool plan_chunk(ChunkPlan &pl, int n, int max_slots) {
       std::sort(m.begin(), m.end());
     }
   }
-  for (const Factors &m : pl.mono)
-    if (m.size() > 2) return false;
   return true;
 }
 
@@ -152,7 +149,13 @@ int qmc_build_image2(qmc_tables *t) {
     total_cost += cost[i];
     total_bytes += sizeof(Qmc2SectorHdr) + 16.0 * (s.U.size() + s.F.size() + 1 + n);
   }
-  int nch = std::max(1, (int)(total_bytes / 20000.0 + 0.999));
+  // defaults measured on B200 (profiles/r01b_sweep.md): 36 chunk-wide slots + up to 8 sector-local ones keep two
+  // 256-thread blocks resident per SM (2 x (44 x 2 KB + 16 KB of tables) < 227 KB); more slots halve the occupancy
+  int max_slots = std::min(QMC2_MAXSLOTS, std::max(36, 3 * n + 2));
+  double chunk_bytes = 16000.0;
+  if (const char *e = std::getenv("QMC2_SLOTS")) max_slots = std::min(QMC2_MAXSLOTS, std::max(3 * n + 2, std::atoi(e)));
+  if (const char *e = std::getenv("QMC2_CHUNK_BYTES")) chunk_bytes = std::max(1000.0, std::atof(e));
+  int nch = std::max(1, (int)(total_bytes / chunk_bytes + 0.999));
   std::vector<std::pair<int, int>> todo;  // ranges still to plan (processed in order)
   {
     int b = 0;
@@ -173,14 +176,7 @@ int qmc_build_image2(qmc_tables *t) {
     const int s0 = todo[w].first, s1 = todo[w].second;
     ChunkPlan pl;
     collect(t, s0, s1, pl);
-    if (!plan_chunk(pl, n, QMC2_MAXSLOTS)) {
-      if (s1 - s0 == 1) return QMC_EUNSUPPORTED;
-      const int mid = (s0 + s1) / 2;
-      todo[w] = {s0, mid};
-      todo.insert(todo.begin() + w + 1, {mid, s1});
-      --w;
-      continue;
-    }
+    plan_chunk(pl, n, max_slots);
     Qmc2Chunk ch;
     ch.sec_begin = s0;
     ch.sec_end = s1;
@@ -204,9 +200,31 @@ int qmc_build_image2(qmc_tables *t) {
       r.pad = 0;
       return r;
     };
-    for (int si = s0; si < s1; ++si) {
+    bool too_many_locals = false;
+    const size_t image_mark = t->image2.size();
+    for (int si = s0; si < s1 && !too_many_locals; ++si) {
       const QmcSector &s = t->sectors[si];
       ch.cost += cost[si];
+      // sector-local products for the monomials the chunk-wide slots leave with more than two factors
+      std::vector<std::pair<uint8_t, uint8_t>> local;
+      {
+        size_t cnt_m = 1 + s.U.size() + s.F.size();
+        for (size_t q = 0; q < cnt_m; ++q) {
+          Factors &f = pl.mono[mi + q];
+          while (f.size() > 2) {
+            const std::pair<uint8_t, uint8_t> pr(f[0], f[1]);
+            size_t id = 0;
+            while (id < local.size() && local[id] != pr) ++id;
+            if (id == local.size()) local.push_back(pr);
+            f.erase(f.begin(), f.begin() + 2);
+            f.insert(f.begin(), (uint8_t)(pl.nslots + id));  // may exceed the sorted order: only the first two are merged next
+          }
+        }
+        if (local.size() > QMC2_MAXLOCAL || pl.nslots + (int)local.size() > 255) {
+          too_many_locals = true;
+          break;
+        }
+      }
       Qmc2SectorHdr h;
       std::memset(&h, 0, sizeof h);
       int pos_of[QMC_MAXDIM], k = 0;
@@ -248,10 +266,27 @@ int qmc_build_image2(qmc_tables *t) {
         }
       }
       h.nrec = (uint16_t)recs.size();
+      h.nlocal = (uint8_t)local.size();
+      ch.max_local = std::max(ch.max_local, (int)local.size());
       t->secoff2[si] = (uint32_t)t->image2.size();
       put(t->image2, h);
+      for (auto &pr : local) {
+        put(t->image2, (uint16_t)(pr.first * QMC2_THREADS));
+        put(t->image2, (uint16_t)(pr.second * QMC2_THREADS));
+      }
+      while (t->image2.size() % 16) t->image2.push_back(0);
       for (const Qmc2Rec &r : recs) put(t->image2, r);
       t->secend2[si] = (uint32_t)t->image2.size();
+    }
+    if (too_many_locals) {  // split the range in two and plan again
+      t->image2.resize(ch.prog_off);
+      (void)image_mark;
+      if (s1 - s0 == 1) return QMC_EUNSUPPORTED;
+      const int mid = (s0 + s1) / 2;
+      todo[w] = {s0, mid};
+      todo.insert(todo.begin() + w + 1, {mid, s1});
+      --w;
+      continue;
     }
     t->chunks.push_back(ch);
   }

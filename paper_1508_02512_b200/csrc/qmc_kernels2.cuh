@@ -127,11 +127,20 @@ struct Fold2<NS, KMAX, K, NS, ZMASK> {
 
 // one sector at one point: out[i] = coefficient of eps^(i - NS) of the subtracted integrand (without the weight w)
 template <int NDIM, int L, int NS, int KMAX>
-__device__ __forceinline__ void sector2(const Qmc2SectorHdr *__restrict__ h, const double *__restrict__ sl,
+__device__ __forceinline__ void sector2(const Qmc2SectorHdr *__restrict__ h, double *__restrict__ sl, int local0,
                                         const double2 *__restrict__ logtab, double (&out)[KMAX + NS + 1]) {
   constexpr int K = KMAX + NS + 1, NC = 1 << NS, FULL = NC - 1;
   typedef Expo<NDIM, L> E;
-  const uint4 *rec = reinterpret_cast<const uint4 *>(h + 1);
+  const int nlocal = h->nlocal;
+  {  // sector-local products: slot[local0 + i] = slot[a] * slot[b]
+    const uint32_t *lp = reinterpret_cast<const uint32_t *>(h + 1);
+#pragma unroll 1
+    for (int i = 0; i < nlocal; ++i) {
+      const uint32_t pw = lp[i];
+      sl[local0 + i * QMC2_THREADS] = sl[pw & 0xffffu] * sl[pw >> 16];
+    }
+  }
+  const uint4 *rec = reinterpret_cast<const uint4 *>(reinterpret_cast<const unsigned char *>(h + 1) + ((nlocal * 4 + 15) & ~15));
   const double G0 = rec_sum(rec, 1, sl);
   const double L0 = rec_sum(rec, h->nL0, sl);
   Ctx2<NS, K> c;
@@ -238,7 +247,7 @@ __global__ void __launch_bounds__(QMC2_THREADS, QMC2_MIN_BLOCKS) qmc2_eval_kerne
 
   const Qmc2ChunkHdr *ch = reinterpret_cast<const Qmc2ChunkHdr *>(sprog);
   const uint32_t *prog = reinterpret_cast<const uint32_t *>(sprog + sizeof(Qmc2ChunkHdr));
-  const int nprog = ch->nprog, first_prod = ch->first_prod;
+  const int nprog = ch->nprog, first_prod = ch->first_prod, local0 = ch->nslots * T;
 
   const uint32_t N = p.N;
   const double dN = (double)N;
@@ -295,17 +304,23 @@ __global__ void __launch_bounds__(QMC2_THREADS, QMC2_MIN_BLOCKS) qmc2_eval_kerne
       // S4-S6: all sectors of the work item at this point
       for (int si = 0; si < wk.nsec; ++si) {
         const Qmc2SectorHdr *h = reinterpret_cast<const Qmc2SectorHdr *>(stab + soff[si]);
-        double contrib[NACC];
-#pragma unroll
-        for (int a = 0; a < NACC; ++a) contrib[a] = 0.0;
-#define QMC2_CASE(NS_)                                                             \
-  case NS_: {                                                                      \
-    if (NS_ <= SMAX) {                                                             \
-      constexpr int NSC = NS_ <= SMAX ? NS_ : 0;                                   \
-      double res[KMAX + NSC + 1];                                                  \
-      sector2<NDIM, L, NSC, KMAX>(h, sl, logtab, res);                             \
-      _Pragma("unroll") for (int i = 0; i < KMAX + NSC + 1; ++i) contrib[QMC_MAXSING - NSC + i] = res[i]; \
-    }                                                                              \
+#define QMC2_CASE(NS_)                                                                                       \
+  case NS_: {                                                                                                \
+    if (NS_ <= SMAX) {                                                                                       \
+      constexpr int NSC = NS_ <= SMAX ? NS_ : 0, KK = KMAX + NSC + 1;                                        \
+      double res[KK];                                                                                        \
+      sector2<NDIM, L, NSC, KMAX>(h, sl, local0, logtab, res);                                                       \
+      bool fin = true;                                                                                       \
+      _Pragma("unroll") for (int i = 0; i < KK; ++i) fin = fin && finite_hi(res[i]);                         \
+      if (!fin) {                                                                                            \
+        ++cntNonFinite;                                                                                      \
+      } else if (!p.persec) {                                                                                \
+        _Pragma("unroll") for (int i = 0; i < KK; ++i) acc[QMC_MAXSING - NSC + i] = fma(w, res[i], acc[QMC_MAXSING - NSC + i]); \
+      } else {                                                                                               \
+        double *sa = sacc + ((size_t)si * NACC + (QMC_MAXSING - NSC)) * T + tid;                             \
+        _Pragma("unroll") for (int i = 0; i < KK; ++i) sa[(size_t)i * T] += w * res[i];                      \
+      }                                                                                                      \
+    }                                                                                                        \
   } break;
         switch (h->nsing) {
           QMC2_CASE(0)
@@ -317,21 +332,6 @@ __global__ void __launch_bounds__(QMC2_THREADS, QMC2_MIN_BLOCKS) qmc2_eval_kerne
             break;
         }
 #undef QMC2_CASE
-        bool fin = true;
-#pragma unroll
-        for (int a = 0; a < NACC; ++a) fin = fin && finite_hi(contrib[a]);
-        if (!fin) {
-          ++cntNonFinite;
-          continue;
-        }
-        if (!p.persec) {
-#pragma unroll
-          for (int a = 0; a < NACC; ++a) acc[a] = fma(w, contrib[a], acc[a]);
-        } else {
-          double *sa = sacc + ((size_t)si * NACC) * T + tid;
-#pragma unroll
-          for (int a = 0; a < NACC; ++a) sa[(size_t)a * T] += w * contrib[a];
-        }
       }
     }
 

@@ -44,10 +44,12 @@ struct Qmc2Rec {        // value = c * slot[s0] * slot[s1]; s0, s1 are slot indi
   uint32_t pad;
 };
 static_assert(sizeof(Qmc2Rec) == 16, "record must be 16 bytes");
-struct Qmc2SectorHdr {  // followed by records: [G0][L0 x nL0][U^ by group][F^ by group]
+#define QMC2_MAXLOCAL 8
+struct Qmc2SectorHdr {  // followed by nlocal x {u16 a, u16 b} (sector-local products slot[nslots + i] = slot[a] * slot[b],
+                        // padded to 16 bytes), then the records: [G0][L0 x nL0][U^ by group][F^ by group]
   uint8_t nsing, nL0;
   uint16_t nrec;
-  uint32_t pad0;
+  uint8_t nlocal, pad0[3];
   uint16_t sing_ln[QMC_MAXSING];   // premultiplied slot index of ln t_k for singular position k
   uint16_t sing_inv[QMC_MAXSING];  // ... of 1/t_k
   double invbeta[QMC_MAXSING];     // 1/beta_k
@@ -63,7 +65,8 @@ struct Qmc2ChunkHdr {   // 16 bytes, followed by nprog x {u16 a, u16 b} (premult
 };
 struct Qmc2Chunk {      // host description of one chunk
   int sec_begin = 0, sec_end = 0;
-  int nslots = 0;
+  int nslots = 0;     // chunk-wide slots
+  int max_local = 0;  // largest number of sector-local product slots in the chunk
   uint32_t prog_off = 0, prog_bytes = 0;  // chunk header + slot program in image2
   double cost = 0.0;                      // modelled flops per point (load balancing)
 };
