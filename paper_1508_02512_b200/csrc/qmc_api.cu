@@ -819,7 +819,7 @@ int qmc_tables_describe(const qmc_tables *t, char *buf, size_t len) {
       const Qmc2Rec *r = reinterpret_cast<const Qmc2Rec *>(reinterpret_cast<const uint8_t *>(h + 1) + ((h->nlocal * 4 + 15) & ~15));
       for (int i = 0; i < h->nrec; ++i) {
         ++nrec;
-        if (r[i].s1 != 3 * t->n * QMC2_THREADS) ++two;
+        if (r[i].s1 != (uint32_t)(3 * t->n) * QMC2_THREADS * 8u) ++two;
       }
       nloc += h->nlocal;
     }

@@ -190,14 +190,13 @@ int qmc_build_image2(qmc_tables *t) {
     }
     while (t->image2.size() % 16) t->image2.push_back(0);
     ch.prog_bytes = (uint32_t)t->image2.size() - ch.prog_off;
-    const uint16_t ONE = (uint16_t)(3 * n * QMC2_THREADS);
+    const uint32_t ONE = (uint32_t)(3 * n) * QMC2_THREADS * 8u;
     size_t mi = 0;  // index into pl.mono, same order as collect()
     auto rec_of = [&](double c, const Factors &f) {
       Qmc2Rec r;
       r.c = c;
-      r.s0 = f.size() > 0 ? (uint16_t)(f[0] * QMC2_THREADS) : ONE;
-      r.s1 = f.size() > 1 ? (uint16_t)(f[1] * QMC2_THREADS) : ONE;
-      r.pad = 0;
+      r.s0 = f.size() > 0 ? (uint32_t)f[0] * QMC2_THREADS * 8u : ONE;
+      r.s1 = f.size() > 1 ? (uint32_t)f[1] * QMC2_THREADS * 8u : ONE;
       return r;
     };
     bool too_many_locals = false;
@@ -244,9 +243,8 @@ int qmc_build_image2(qmc_tables *t) {
         if (s.alpha[j] != -1 && s.beta[j] != 0) {
           Qmc2Rec r;
           r.c = (double)s.beta[j];
-          r.s0 = (uint16_t)((n + j) * QMC2_THREADS);
+          r.s0 = (uint32_t)(n + j) * QMC2_THREADS * 8u;
           r.s1 = ONE;
-          r.pad = 0;
           recs.push_back(r);
           ++h.nL0;
         }

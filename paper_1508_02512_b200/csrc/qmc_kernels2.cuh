@@ -38,21 +38,23 @@ __device__ __forceinline__ double fast_rcp(double x) {
 
 // ln x, absolute error ~1e-16: x = 2^e * z, z in [0.6875, 1.375), 128 sub-intervals with centre c_i;
 // tab[i] = {1/c_i rounded, -ln(that) in extended precision}; r = z/c_i - 1 (one FMA, |r| < 2^-8), degree-6 log1p.
-static __device__ __noinline__ double slow_log(double x) { return log(x); }
+// Arguments that are not positive normal numbers give NaN (the evaluation is then dropped and counted as non-finite).
+__constant__ double qmc2_logc[6] = {0.693147180559945309417, -1.0 / 6.0, 0.2, -0.25, 1.0 / 3.0, -0.5};
 __device__ __forceinline__ double fast_log(double x, const double2 *__restrict__ tab) {
   const int hi = __double2hiint(x), lo = __double2loint(x);
-  if ((unsigned)(hi - 0x00100000) >= 0x7fe00000u) return slow_log(x);  // zero, negative, subnormal, inf, nan
+  const bool ok = (unsigned)(hi - 0x00100000) < 0x7fe00000u;  // positive, normal
   const int tmp = hi - 0x3fe60000;
   const int e = tmp >> 20;
   const double2 T = tab[(tmp >> 13) & 127];
   const double z = __hiloint2double(hi - (tmp & 0xfff00000), lo);
   const double r = fma(z, T.x, -1.0);
-  const double y0 = fma((double)e, 0.693147180559945309417, T.y);
-  double q = fma(r, -1.0 / 6.0, 0.2);
-  q = fma(r, q, -0.25);
-  q = fma(r, q, 1.0 / 3.0);
-  q = fma(r, q, -0.5);
-  return fma(r * r, q, r) + y0;
+  const double y0 = fma((double)e, qmc2_logc[0], T.y);
+  double q = fma(r, qmc2_logc[1], qmc2_logc[2]);
+  q = fma(r, q, qmc2_logc[3]);
+  q = fma(r, q, qmc2_logc[4]);
+  q = fma(r, q, qmc2_logc[5]);
+  const double v = fma(r * r, q, r) + y0;
+  return ok ? v : __longlong_as_double(0x7ff8000000000000ll);
 }
 
 template <int E>
@@ -71,13 +73,14 @@ struct Expo {
 };
 
 // sum of n records: c * slot[s0] * slot[s1]
-__device__ __forceinline__ double rec_sum(const uint4 *__restrict__ &rec, int n, const double *__restrict__ sl) {
+// (sl = this thread's column of the slot table as a byte pointer; record offsets are byte offsets slot * T * 8)
+__device__ __forceinline__ double rec_sum(const uint4 *__restrict__ &rec, int n, const unsigned char *__restrict__ sl) {
   double acc = 0.0;
 #pragma unroll 1
   for (int i = 0; i < n; ++i) {
     const uint4 r = *rec++;
     const double c = __hiloint2double((int)r.y, (int)r.x);
-    acc = fma(c, sl[r.z & 0xffffu] * sl[r.z >> 16], acc);
+    acc = fma(c, *reinterpret_cast<const double *>(sl + r.z) * *reinterpret_cast<const double *>(sl + r.w), acc);
   }
   return acc;
 }
@@ -141,8 +144,9 @@ __device__ __forceinline__ void sector2(const Qmc2SectorHdr *__restrict__ h, dou
     }
   }
   const uint4 *rec = reinterpret_cast<const uint4 *>(reinterpret_cast<const unsigned char *>(h + 1) + ((nlocal * 4 + 15) & ~15));
-  const double G0 = rec_sum(rec, 1, sl);
-  const double L0 = rec_sum(rec, h->nL0, sl);
+  const unsigned char *slb = reinterpret_cast<const unsigned char *>(sl);
+  const double G0 = rec_sum(rec, 1, slb);
+  const double L0 = rec_sum(rec, h->nL0, slb);
   Ctx2<NS, K> c;
   {
     // group partial sums (records are sorted by group), then subset sums: P[X] = value with the singular variables
@@ -151,9 +155,9 @@ __device__ __forceinline__ void sector2(const Qmc2SectorHdr *__restrict__ h, dou
     const uint4 cu = *reinterpret_cast<const uint4 *>(h->cntU), cf = *reinterpret_cast<const uint4 *>(h->cntF);
     const unsigned cuw[4] = {cu.x, cu.y, cu.z, cu.w}, cfw[4] = {cf.x, cf.y, cf.z, cf.w};
 #pragma unroll
-    for (int g = 0; g < NC; ++g) PU[g] = rec_sum(rec, (cuw[g >> 2] >> (8 * (g & 3))) & 255u, sl);
+    for (int g = 0; g < NC; ++g) PU[g] = rec_sum(rec, (cuw[g >> 2] >> (8 * (g & 3))) & 255u, slb);
 #pragma unroll
-    for (int g = 0; g < NC; ++g) PF[g] = rec_sum(rec, (cfw[g >> 2] >> (8 * (g & 3))) & 255u, sl);
+    for (int g = 0; g < NC; ++g) PF[g] = rec_sum(rec, (cfw[g >> 2] >> (8 * (g & 3))) & 255u, slb);
 #pragma unroll
     for (int b = 0; b < NS; ++b)
 #pragma unroll

@@ -38,10 +38,9 @@ static_assert(sizeof(QmcSectorHdr) == 64, "sector header must be 64 bytes");
 // first) until every monomial is a product of at most two slots.  A monomial is then one 16-byte record.
 #define QMC2_THREADS 256
 #define QMC2_MAXSLOTS 56
-struct Qmc2Rec {        // value = c * slot[s0] * slot[s1]; s0, s1 are slot indices premultiplied by QMC2_THREADS
-  double c;
-  uint16_t s0, s1;
-  uint32_t pad;
+struct Qmc2Rec {        // value = c * slot[s0] * slot[s1]; s0, s1 are BYTE offsets slot * QMC2_THREADS * 8 into the
+  double c;             // thread's column of the slot table
+  uint32_t s0, s1;
 };
 static_assert(sizeof(Qmc2Rec) == 16, "record must be 16 bytes");
 #define QMC2_MAXLOCAL 8
