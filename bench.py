@@ -138,12 +138,6 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
-def shift_block(seed: int, m: int, dim: int, rank: int, world: int) -> np.ndarray:
-    """Rank `rank`'s block of m shift vectors out of the ONE stream of m*world vectors keyed by `seed`: a world-GPU run
-    is the same estimator as a 1-GPU run with m*world shifts."""
-    return qi.splitmix64_shifts(seed, m * world, dim)[rank * m:(rank + 1) * m]
-
-
 def time_to_accuracy(q, wl, torch, target=1e-3, max_N=2 ** 27):
     """M2: raise N through the primes below 2^k until the relative error of the eps^0 coefficient of J is <= target
     (reading C17); wall time of everything the user waits for after qmc_prepare: generating-vector search, uploads,
@@ -188,7 +182,8 @@ def run_product(args):
     m = wl.m
     t = q.qmc_prepare(wl, eps_order=wl.eps_order, lam=wl.lam)
     z = q.qmc_generating_vector(N, t.dim, device=dev)           # Korobov P2 search on the device, outside the timed steps
-    shifts = shift_block(wl.seed, m, t.dim, rank, world)
+    from paper_1508_02512_b200 import sharding
+    shifts = sharding.shift_block(wl.seed, m, t.dim, rank, world)
     fp, fs, corners = q.qmc_flop_model(t)
     flops_step = (fp + fs) * N * m
     evals_step = N * m * t.n_sectors
@@ -241,8 +236,7 @@ def run_product(args):
         r_e2e = q.qmc_integrate(t, N, m, z=z, shifts=shifts, resident=0, device=dev)
         if world > 1:
             loc = torch.from_numpy(np.ascontiguousarray(r_e2e.shift_totals).view(np.float64).reshape(t.K, m, 2)).to(dev)
-            dist.all_gather_into_tensor(gathered, loc)
-            allT = gathered.cpu().numpy()
+            sharding.combine(loc)
     torch.cuda.synchronize()
     e2e_s = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
     if world > 1:
@@ -252,9 +246,7 @@ def run_product(args):
 
     # ---- combine the shifts of all ranks (Eqs. 19-20 over m*world estimates) --------------------------------
     if world > 1:
-        allT = gathered.cpu().numpy()                      # [world, K, m, 2]
-        T = np.concatenate([allT[r] for r in range(world)], axis=1)
-        coeff, err = q.qmc_statistics(T[..., 0] + 1j * T[..., 1])
+        coeff, err, _ = sharding.combine(q.qmc_result_device_totals(t, m))
     else:
         coeff, err = res.coeff, res.err
 
