@@ -72,13 +72,22 @@ struct Expo {
   static constexpr int aU0 = NDIM - 1 - 2 * L, aU1 = L + 1, aF0 = -(NDIM + 1 - 2 * L), aF1 = -L;
 };
 
+// Stream of 16-byte records with the NEXT record always in flight (software pipelining: the record load overlaps
+// the slot loads and the arithmetic of the current one; reads at most one record past the sector block, still inside
+// the block's shared memory).
+struct RecStream {
+  const uint4 *p;
+  uint4 cur;
+  __device__ __forceinline__ explicit RecStream(const uint4 *q) : p(q), cur(*q) {}
+};
 // sum of n records: c * slot[s0] * slot[s1]
 // (sl = this thread's column of the slot table as a byte pointer; record offsets are byte offsets slot * T * 8)
-__device__ __forceinline__ double rec_sum(const uint4 *__restrict__ &rec, int n, const unsigned char *__restrict__ sl) {
+__device__ __forceinline__ double rec_sum(RecStream &s, int n, const unsigned char *__restrict__ sl) {
   double acc = 0.0;
 #pragma unroll 1
   for (int i = 0; i < n; ++i) {
-    const uint4 r = *rec++;
+    const uint4 r = s.cur;
+    s.cur = *(++s.p);
     const double c = __hiloint2double((int)r.y, (int)r.x);
     acc = fma(c, *reinterpret_cast<const double *>(sl + r.z) * *reinterpret_cast<const double *>(sl + r.w), acc);
   }
@@ -143,7 +152,7 @@ __device__ __forceinline__ void sector2(const Qmc2SectorHdr *__restrict__ h, dou
       sl[local0 + i * QMC2_THREADS] = sl[pw & 0xffffu] * sl[pw >> 16];
     }
   }
-  const uint4 *rec = reinterpret_cast<const uint4 *>(reinterpret_cast<const unsigned char *>(h + 1) + ((nlocal * 4 + 15) & ~15));
+  RecStream rec(reinterpret_cast<const uint4 *>(reinterpret_cast<const unsigned char *>(h + 1) + ((nlocal * 4 + 15) & ~15)));
   const unsigned char *slb = reinterpret_cast<const unsigned char *>(sl);
   const double G0 = rec_sum(rec, 1, slb);
   const double L0 = rec_sum(rec, h->nL0, slb);
@@ -292,8 +301,8 @@ __global__ void __launch_bounds__(QMC2_THREADS, QMC2_MIN_BLOCKS) qmc2_eval_kerne
         }
         if (!(y > 0.0) || !(tj > 0.0)) inside = false;
         sl[j * T] = tj;
-        sl[(NDIM + j) * T] = log(tj);
-        sl[(2 * NDIM + j) * T] = 1.0 / tj;
+        sl[(NDIM + j) * T] = fast_log(tj, logtab);   // t >= 3.7e-32 for y >= 2^-53: always a normal number
+        sl[(2 * NDIM + j) * T] = fast_rcp(tj);
         uint32_t rn = r[j] + dz[j];
         r[j] = rn >= N ? rn - N : rn;
       }
