@@ -616,7 +616,8 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
   nchunks = (se - sb + spc - 1) / spc;
   const size_t smem = tab_bytes + (((size_t)(spc + 1) * 4 + 15) & ~(size_t)15) + fixed_smem + per_sector_acc * spc;
   int bps = 0;
-  CUDA_OK(qmc_kernel_prepare(n, t->kmax, cplx, smem, &bps));
+  const int flavor = !cplx ? 0 : (-t->kmin <= 1 ? 2 : 1);  // kmin = -(largest number of singular variables)
+  CUDA_OK(qmc_kernel_prepare(n, t->kmax, flavor, smem, &bps));
   if (bps < 1) return QMC_ECUDA;
   gx = std::min<long long>({(long long)sms * bps, (long long)QMC_MAX_BLOCKS, (long long)((icount + QMC_THREADS - 1) / QMC_THREADS)});
   gx = std::max(gx, 1);
@@ -644,7 +645,7 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
   p.tab_smem_bytes = (tab_bytes + 15) & ~15u;
 
   cudaEventRecord(static_cast<cudaEvent_t>(t->ev0), st);
-  ce = qmc_kernel_launch(n, t->kmax, cplx, dim3(gx, nchunks), smem, st, p);
+  ce = qmc_kernel_launch(n, t->kmax, flavor, dim3(gx, nchunks), smem, st, p);
   cudaEventRecord(static_cast<cudaEvent_t>(t->evm), st);
   }
   const int rows = persec ? (se - sb) : nchunks;

@@ -421,13 +421,16 @@ __device__ __forceinline__ double block_sum(double v, double *scratch /*[QMC_THR
 }  // namespace qmcdev
 
 // ================================================================================================
-template <int NDIM, int KMAX, bool CPLX>
+// NSCAP: largest number of singular variables of any sector of the tables this instantiation serves (the code of the
+// larger cases is not generated: the complex instantiation with NSCAP = 1 is a fraction of the size of NSCAP = 4)
+template <int NDIM, int KMAX, bool CPLX, int NSCAP>
 __global__ void __launch_bounds__(QMC_THREADS) qmc_eval_kernel(const QmcLaunch p) {
   using namespace qmcdev;
   typedef typename std::conditional<CPLX, cd, double>::type T;
   constexpr int NACC = QMC_MAXSING + KMAX + 1;  // accumulator a <-> order a - QMC_MAXSING
   constexpr int NC = CPLX ? 2 : 1;
-  constexpr int SMAX = NDIM < QMC_MAXSING ? NDIM : QMC_MAXSING;
+  constexpr int SMAX0 = NDIM < QMC_MAXSING ? NDIM : QMC_MAXSING;
+  constexpr int SMAX = SMAX0 < NSCAP ? SMAX0 : NSCAP;
 
   extern __shared__ __align__(16) unsigned char smem[];
   const int tid = threadIdx.x;

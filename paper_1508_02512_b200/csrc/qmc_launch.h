@@ -53,5 +53,5 @@ cudaError_t qmc2_kernel_launch(int ndim, int loops, int kmax, dim3 grid, size_t 
 bool qmc2_kernel_available(int ndim, int loops, int kmax);
 
 // implemented in qmc_dispatch.cu on top of one translation unit per dimension (qmc_inst_d<N>.cu)
-cudaError_t qmc_kernel_prepare(int ndim, int kmax, bool cplx, size_t smem, int *blocks_per_sm);
-cudaError_t qmc_kernel_launch(int ndim, int kmax, bool cplx, dim3 grid, size_t smem, cudaStream_t st, const QmcLaunch &p);
+cudaError_t qmc_kernel_prepare(int ndim, int kmax, int flavor, size_t smem, int *blocks_per_sm);
+cudaError_t qmc_kernel_launch(int ndim, int kmax, int flavor, dim3 grid, size_t smem, cudaStream_t st, const QmcLaunch &p);

@@ -26,7 +26,7 @@ def check(got, want, A, what):
 
 def parity(wl, N, m, z=None, index_range=None, sectors=None, transform=0, shifts=None, eps_order=None):
     eo = wl.eps_order if eps_order is None else eps_order
-    t = q.qmc_prepare(wl, eps_order=eo, lam=wl.lam, transform=transform)
+    t = q.qmc_prepare(wl, eps_order=eo, lam=wl.lam, transform=transform)   # reads QMC2_* from the environment
     o = Oracle.from_tables(t.export())
     if z is None:
         z = qi.good_vector(N, t.dim)
@@ -148,3 +148,47 @@ def test_double_box_poles_on_gpu_at_baseline_size():
     # fused and per-sector modes agree at full size
     p = q.qmc_integrate(t, 999983, 20, seed=13, per_sector=True)
     assert np.allclose(p.shift_totals, r.shift_totals, rtol=1e-11, atol=1e-13)
+
+
+def test_v2_tables_chunk_boundaries_and_small_slot_budget(monkeypatch):
+    """Version-2 tables: sector ranges that straddle chunk boundaries, and a slot budget small enough to force
+    sector-local product slots and chunk splits (QMC2_SLOTS / QMC2_CHUNK_BYTES are read by qmc_prepare)."""
+    wl = qi.double_box()
+    t = q.qmc_prepare(wl)
+    desc = t.describe()
+    assert "chunks" in desc and t.n_sectors == 293
+    bounds = [int(l.split("[")[1].split(",")[0]) for l in desc.splitlines()[1:]]
+    assert len(bounds) > 2
+    b = bounds[2]
+    parity(wl, 16381, 2, sectors=(b - 3, b + 4))            # straddles a chunk boundary
+    parity(wl, 16381, 2, sectors=(bounds[1] - 1, bounds[3] + 1))   # spans a whole chunk plus both neighbours
+    monkeypatch.setenv("QMC2_SLOTS", "22")
+    monkeypatch.setenv("QMC2_CHUNK_BYTES", "3000")
+    t2 = q.qmc_prepare(wl)
+    d2 = t2.describe()
+    assert sum(int(l.split("local products ")[1].split(")")[0]) for l in d2.splitlines()[1:]) > 0
+    assert len(d2.splitlines()) > len(desc.splitlines())
+    parity(wl, 16381, 2, sectors=(100, 140))
+    monkeypatch.delenv("QMC2_SLOTS")
+    monkeypatch.delenv("QMC2_CHUNK_BYTES")
+
+
+def test_async_launch_resident_inputs_and_fetch():
+    """qmc_integrate_async with everything resident (the bench's device-timed step) gives bit-identical results to the
+    synchronous call, and the device view of the per-shift totals matches what fetch returns."""
+    import torch
+    wl = qi.massless_box()
+    t = q.qmc_prepare(wl)
+    N, m = 99991, 8
+    z = qi.good_vector(N, 3)
+    sh = qi.splitmix64_shifts(wl.seed, m, 3)
+    ref = q.qmc_integrate(t, N, m, z=z, shifts=sh)
+    q.qmc_integrate_async(t, N, m, z=z, shifts=sh, resident=0)
+    q.qmc_integrate_async(t, N, m, z=z, resident=2)          # nothing copied from the host
+    dev = q.qmc_result_device_totals(t, m)
+    r = q.qmc_result_fetch(t, m)
+    assert np.array_equal(r.shift_totals, ref.shift_totals) and np.array_equal(r.coeff, ref.coeff)
+    torch.cuda.synchronize()
+    d = dev.cpu().numpy()
+    assert np.array_equal(d[..., 0] + 1j * d[..., 1], ref.shift_totals)
+    assert r.h2d_bytes < ref.h2d_bytes and r.d2h_bytes > 0 and r.eval_kernel_ms > 0
