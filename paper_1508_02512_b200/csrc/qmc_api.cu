@@ -16,6 +16,7 @@
 #include "qmc_tables.h"
 
 #define QMC_MAX_BLOCKS 592  // upper bound of gridDim.x used for workspace sizing (148 SMs x 4)
+#define QMC2_MAX_WORK 8192  // blocks of one version-2 launch
 #define QMC_NCAND 64        // Korobov candidates of the P_2 search
 #define QMC_P2_BLOCKS 296
 
@@ -165,7 +166,7 @@ DevLayout layout(const qmc_tables *t, int m) {
   L.image2 = o; o += align256(t->image2.size());
   L.secoff2 = o; o += align256((nsec + 1) * 4);
   L.logtab = o; o += align256(sizeof t->logtab);
-  L.work = o; o += align256((nsec + 1) * sizeof(Qmc2Work));
+  L.work = o; o += align256((size_t)QMC2_MAX_WORK * sizeof(Qmc2Work));
   L.shifts = o; o += align256((size_t)m * QMC_MAXDIM * 8);
   L.counters = o; o += 256;
   L.out = o; o += align256(nsec * QMC_NACC_MAX * 2 * (size_t)m * 8);
@@ -260,7 +261,9 @@ int launch_v2(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
   const size_t budget = (size_t)smem_optin - 1024;
   const size_t fixed = prog_cap + 16 + (((size_t)m * n * 8 + 15) & ~(size_t)15) + (T / 32) * 8 + 128 * 16 + (size_t)max_nslots * T * 8;
   const size_t accbytes = persec ? (size_t)nacc * T * 8 : 0;
-  std::vector<Qmc2Work> work;
+  std::vector<Qmc2Work> runs;
+  std::vector<double> run_cost;
+  double total_cost = 0.0;
   uint32_t sec_cap = 0;
   int max_nsec = 0;
   for (const Qmc2Chunk &c : t->chunks) {
@@ -276,37 +279,61 @@ int launch_v2(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
       }
       if (b == a) return QMC_ENOMEM;
       Qmc2Work w;
+      std::memset(&w, 0, sizeof w);
       w.prog_off = c.prog_off;
       w.prog_bytes = c.prog_bytes;
       w.sec_off = t->secoff2[a];
       w.sec_bytes = t->secend2[b - 1] - t->secoff2[a];
       w.s0 = a;
       w.nsec = b - a;
-      w.out_row = persec ? a - sb : (int)work.size();
-      w.pad = 0;
+      w.out_row = persec ? a - sb : (int)runs.size();
+      w.count_boundary = runs.empty() ? 1 : 0;
       sec_cap = std::max(sec_cap, w.sec_bytes);
       max_nsec = std::max(max_nsec, w.nsec);
-      work.push_back(w);
+      double cst = 0.0;
+      for (int s = a; s < b; ++s) cst += t->sec_cost[s];
+      run_cost.push_back(cst);
+      total_cost += cst;
+      runs.push_back(w);
       a = b;
     }
   }
-  const int nitems = (int)work.size();
+  const int nitems = (int)runs.size();
   const size_t smem = fixed + sec_cap + (((size_t)(max_nsec + 1) * 4 + 15) & ~(size_t)15) + accbytes * max_nsec;
   int bps = 0;
   CUDA_OK(qmc2_kernel_prepare(n, t->L, t->kmax, smem, &bps));
   if (bps < 1) return QMC_ECUDA;
-  long long gx = ((long long)3 * sms * bps + nitems - 1) / nitems;
-  gx = std::min<long long>({gx, (long long)QMC_MAX_BLOCKS, (long long)((icount + T - 1) / T)});
-  gx = std::max<long long>(gx, 1);
+  // slices per run in proportion to its modelled cost: about `waves` blocks of equal cost per resident block slot
+  int waves = 16;  // measured (profiles/r01d_waves.md): short blocks interleave better than one long block per slot
+  if (const char *e = std::getenv("QMC2_WAVES")) waves = std::max(1, std::atoi(e));
+  const long long max_slices_pts = std::max<long long>(1, (long long)((icount + T - 1) / T));
+  const double nblocks_target = (double)waves * sms * bps;
+  std::vector<Qmc2Work> work;
+  int max_slices = 1;
+  for (int i = 0; i < nitems; ++i) {
+    long long ns = (long long)(nblocks_target * run_cost[i] / total_cost + 0.5);
+    ns = std::max<long long>(1, std::min<long long>({ns, (long long)QMC_MAX_BLOCKS, max_slices_pts}));
+    max_slices = std::max(max_slices, (int)ns);
+    for (int sidx = 0; sidx < (int)ns; ++sidx) {
+      Qmc2Work w = runs[i];
+      w.slice = sidx;
+      w.nslices = (int)ns;
+      work.push_back(w);
+    }
+  }
+  if (work.size() > QMC2_MAX_WORK) return QMC_ENOMEM;
   // upload the work list unless the identical list is already there
-  const uint64_t key = ((uint64_t)sb << 40) ^ ((uint64_t)se << 20) ^ (persec ? 1u : 0u) ^ ((uint64_t)m << 50);
+  const uint64_t key = ((uint64_t)sb << 40) ^ ((uint64_t)se << 20) ^ (persec ? 1u : 0u) ^ ((uint64_t)m << 50) ^ ((uint64_t)icount << 1) ^
+                       ((uint64_t)waves << 58);
   if (!(t->work_ws == ws && t->work_key == key)) {
-    t->work_host.assign(reinterpret_cast<const uint8_t *>(work.data()), reinterpret_cast<const uint8_t *>(work.data() + nitems));
+    t->work_host.assign(reinterpret_cast<const uint8_t *>(work.data()), reinterpret_cast<const uint8_t *>(work.data() + work.size()));
     CUDA_OK(cudaMemcpyAsync(ws + L.work, t->work_host.data(), t->work_host.size(), cudaMemcpyHostToDevice, st));
     *h2d += t->work_host.size();
     t->work_ws = ws;
     t->work_key = key;
   }
+  const int rows_partial = persec ? (se - sb) : nitems;
+  CUDA_OK(cudaMemsetAsync(ws + L.partial, 0, (size_t)rows_partial * m * max_slices * nacc * 8, st));
   Qmc2Launch p;
   std::memset(&p, 0, sizeof p);
   p.image2 = ws + L.image2;
@@ -329,10 +356,11 @@ int launch_v2(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
   p.sm_sec_cap = (sec_cap + 15) & ~15u;
   p.max_nsec = max_nsec;
   p.max_nslots = max_nslots;
+  p.max_slices = max_slices;
   cudaEventRecord(static_cast<cudaEvent_t>(t->ev0), st);
-  *ce_out = qmc2_kernel_launch(n, t->L, t->kmax, dim3((unsigned)gx, nitems), smem, st, p);
+  *ce_out = qmc2_kernel_launch(n, t->L, t->kmax, dim3((unsigned)work.size(), 1), smem, st, p);
   cudaEventRecord(static_cast<cudaEvent_t>(t->evm), st);
-  *gx_out = (int)gx;
+  *gx_out = max_slices;
   *rows_out = nitems;
   return QMC_OK;
 }

@@ -104,9 +104,11 @@ void collect(const qmc_tables *t, int s0, int s1, ChunkPlan &pl) {
   }
 }
 
+// relative cost of one sector at one point, fitted to measured per-chunk kernel times on B200 (cfg4, r01d):
+// time ~ 7.8 per corner (reciprocal, logarithm, series, its share of the fold) + 1 per record
 double sector_cost(const QmcSector &s, int kmax) {
-  const int nc = 1 << s.nsing, K = kmax + s.nsing + 1;
-  return 4.0 * (s.U.size() + s.F.size() + 4) + nc * (30.0 + 2.0 * K) + (nc - 1) * (4.0 * K + 0.5 * K * K);
+  const int nc = 1 << s.nsing;
+  return 7.8 * nc * (1.0 + 0.15 * kmax) + (double)(s.U.size() + s.F.size() + 2);
 }
 
 template <class T>
@@ -136,6 +138,7 @@ int qmc_build_image2(qmc_tables *t) {
   t->secoff2.clear();
   t->chunks.clear();
   t->secend2.clear();
+  t->sec_cost.clear();
   const int n = t->n, nsec = (int)t->sectors.size();
   if (t->lambda > 0.0 || nsec == 0) return QMC_OK;  // complex path keeps the version-1 image
   if (3 * n + 1 >= QMC2_MAXSLOTS) return QMC_EUNSUPPORTED;
@@ -146,6 +149,7 @@ int qmc_build_image2(qmc_tables *t) {
   for (int i = 0; i < nsec; ++i) {
     const QmcSector &s = t->sectors[i];
     cost[i] = sector_cost(s, t->kmax);
+    t->sec_cost.push_back(cost[i]);
     total_cost += cost[i];
     total_bytes += sizeof(Qmc2SectorHdr) + 16.0 * (s.U.size() + s.F.size() + 1 + n);
   }

@@ -421,10 +421,13 @@ __device__ __forceinline__ double block_sum(double v, double *scratch /*[QMC_THR
 }  // namespace qmcdev
 
 // ================================================================================================
+#ifndef QMC_V1_MIN_BLOCKS
+#define QMC_V1_MIN_BLOCKS 1
+#endif
 // NSCAP: largest number of singular variables of any sector of the tables this instantiation serves (the code of the
 // larger cases is not generated: the complex instantiation with NSCAP = 1 is a fraction of the size of NSCAP = 4)
 template <int NDIM, int KMAX, bool CPLX, int NSCAP>
-__global__ void __launch_bounds__(QMC_THREADS) qmc_eval_kernel(const QmcLaunch p) {
+__global__ void __launch_bounds__(QMC_THREADS, QMC_V1_MIN_BLOCKS) qmc_eval_kernel(const QmcLaunch p) {
   using namespace qmcdev;
   typedef typename std::conditional<CPLX, cd, double>::type T;
   constexpr int NACC = QMC_MAXSING + KMAX + 1;  // accumulator a <-> order a - QMC_MAXSING

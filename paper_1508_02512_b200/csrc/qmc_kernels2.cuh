@@ -72,22 +72,13 @@ struct Expo {
   static constexpr int aU0 = NDIM - 1 - 2 * L, aU1 = L + 1, aF0 = -(NDIM + 1 - 2 * L), aF1 = -L;
 };
 
-// Stream of 16-byte records with the NEXT record always in flight (software pipelining: the record load overlaps
-// the slot loads and the arithmetic of the current one; reads at most one record past the sector block, still inside
-// the block's shared memory).
-struct RecStream {
-  const uint4 *p;
-  uint4 cur;
-  __device__ __forceinline__ explicit RecStream(const uint4 *q) : p(q), cur(*q) {}
-};
 // sum of n records: c * slot[s0] * slot[s1]
 // (sl = this thread's column of the slot table as a byte pointer; record offsets are byte offsets slot * T * 8)
-__device__ __forceinline__ double rec_sum(RecStream &s, int n, const unsigned char *__restrict__ sl) {
+__device__ __forceinline__ double rec_sum(const uint4 *__restrict__ &rec, int n, const unsigned char *__restrict__ sl) {
   double acc = 0.0;
 #pragma unroll 1
   for (int i = 0; i < n; ++i) {
-    const uint4 r = s.cur;
-    s.cur = *(++s.p);
+    const uint4 r = *rec++;
     const double c = __hiloint2double((int)r.y, (int)r.x);
     acc = fma(c, *reinterpret_cast<const double *>(sl + r.z) * *reinterpret_cast<const double *>(sl + r.w), acc);
   }
@@ -152,7 +143,7 @@ __device__ __forceinline__ void sector2(const Qmc2SectorHdr *__restrict__ h, dou
       sl[local0 + i * QMC2_THREADS] = sl[pw & 0xffffu] * sl[pw >> 16];
     }
   }
-  RecStream rec(reinterpret_cast<const uint4 *>(reinterpret_cast<const unsigned char *>(h + 1) + ((nlocal * 4 + 15) & ~15)));
+  const uint4 *rec = reinterpret_cast<const uint4 *>(reinterpret_cast<const unsigned char *>(h + 1) + ((nlocal * 4 + 15) & ~15));
   const unsigned char *slb = reinterpret_cast<const unsigned char *>(sl);
   const double G0 = rec_sum(rec, 1, slb);
   const double L0 = rec_sum(rec, h->nL0, slb);
@@ -209,8 +200,8 @@ __device__ __forceinline__ bool finite_hi(double v) { return (__double2hiint(v) 
 #define QMC2_MIN_BLOCKS 2
 #endif
 
-// partial layout: fused  : [work item][shift][block x][NACC]
-//                 persec : [sector row][shift][block x][NACC]      (NACC = QMC_MAXSING + KMAX + 1, index a <-> order a - QMC_MAXSING)
+// partial layout: fused  : [run of sectors][shift][slice][NACC]
+//                 persec : [sector row][shift][slice][NACC]        (NACC = QMC_MAXSING + KMAX + 1, index a <-> order a - QMC_MAXSING)
 template <int NDIM, int L, int KMAX>
 __global__ void __launch_bounds__(QMC2_THREADS, QMC2_MIN_BLOCKS) qmc2_eval_kernel(const Qmc2Launch p) {
   using namespace qmc2;
@@ -220,7 +211,7 @@ __global__ void __launch_bounds__(QMC2_THREADS, QMC2_MIN_BLOCKS) qmc2_eval_kerne
 
   extern __shared__ __align__(16) unsigned char smem[];
   const int tid = threadIdx.x;
-  const Qmc2Work wk = p.work[blockIdx.y];
+  const Qmc2Work wk = p.work[blockIdx.x];
 
   // shared memory carve-up (all offsets multiples of 16)
   unsigned char *sprog = smem;
@@ -264,7 +255,7 @@ __global__ void __launch_bounds__(QMC2_THREADS, QMC2_MIN_BLOCKS) qmc2_eval_kerne
 
   const uint32_t N = p.N;
   const double dN = (double)N;
-  const uint32_t stride = gridDim.x * T;
+  const uint32_t stride = (uint32_t)wk.nslices * T;
   uint32_t dz[NDIM];
 #pragma unroll
   for (int j = 0; j < NDIM; ++j) dz[j] = (uint32_t)(((uint64_t)stride * p.zeff[j]) % N);
@@ -278,7 +269,7 @@ __global__ void __launch_bounds__(QMC2_THREADS, QMC2_MIN_BLOCKS) qmc2_eval_kerne
     if (p.persec)
       for (int i = 0; i < wk.nsec * NACC; ++i) sacc[(size_t)i * T + tid] = 0.0;
 
-    uint32_t cidx = blockIdx.x * T + tid;
+    uint32_t cidx = (uint32_t)wk.slice * T + tid;
     uint32_t r[NDIM];
 #pragma unroll
     for (int j = 0; j < NDIM; ++j) r[j] = (uint32_t)((p.off[j] + (uint64_t)cidx * p.zeff[j]) % N);
@@ -307,7 +298,7 @@ __global__ void __launch_bounds__(QMC2_THREADS, QMC2_MIN_BLOCKS) qmc2_eval_kerne
         r[j] = rn >= N ? rn - N : rn;
       }
       if (!inside) {
-        if (blockIdx.y == 0) ++cntBoundary;
+        if (wk.count_boundary) ++cntBoundary;
         continue;
       }
       for (int i = 0; i < nprog; ++i) {
@@ -350,7 +341,7 @@ __global__ void __launch_bounds__(QMC2_THREADS, QMC2_MIN_BLOCKS) qmc2_eval_kerne
 
     // S7: block reduction -> one partial per (work item | sector, shift, block)
     if (!p.persec) {
-      double *dst = p.partial + (((size_t)wk.out_row * p.m + kap) * gridDim.x + blockIdx.x) * NACC;
+      double *dst = p.partial + (((size_t)wk.out_row * p.m + kap) * p.max_slices + wk.slice) * NACC;
 #pragma unroll
       for (int a = 0; a < NACC; ++a) {
         double sr = qmcdev::block_sum(acc[a], scratch);
@@ -358,7 +349,7 @@ __global__ void __launch_bounds__(QMC2_THREADS, QMC2_MIN_BLOCKS) qmc2_eval_kerne
       }
     } else {
       for (int si = 0; si < wk.nsec; ++si) {
-        double *dst = p.partial + (((size_t)(wk.out_row + si) * p.m + kap) * gridDim.x + blockIdx.x) * NACC;
+        double *dst = p.partial + (((size_t)(wk.out_row + si) * p.m + kap) * p.max_slices + wk.slice) * NACC;
         for (int a = 0; a < NACC; ++a) {
           double v = qmcdev::block_sum(sacc[((size_t)si * NACC + a) * T + tid], scratch);
           if (tid == 0) dst[a] = v;

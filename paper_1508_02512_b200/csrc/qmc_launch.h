@@ -27,12 +27,14 @@ struct QmcLaunch {
 
 
 // ---- version 2 (real path) --------------------------------------------------------------------------------
-struct Qmc2Work {  // one block column (blockIdx.y): a run of sectors of one chunk
+struct Qmc2Work {  // one block (blockIdx.x): one slice of the lattice points of a run of sectors of one chunk
   uint32_t prog_off, prog_bytes;  // chunk header + slot program in image2
   uint32_t sec_off, sec_bytes;    // the sector blocks
   int32_t s0, nsec;               // first sector (global index), number of sectors
   int32_t out_row;                // fused: row of the partial buffer; per-sector: row of the first sector
-  int32_t pad;
+  int32_t count_boundary;         // 1 for the blocks that tally boundary points (the first run of sectors)
+  int32_t slice, nslices;         // this block takes the points slice, slice + nslices, ... (in units of blocks):
+                                  // runs get slices in proportion to their modelled cost
 };
 struct Qmc2Launch {
   const uint8_t *image2;
@@ -47,6 +49,7 @@ struct Qmc2Launch {
   int32_t m, transform, persec;
   uint32_t sm_prog_cap, sm_sec_cap;  // shared-memory bytes reserved for the slot program and the sector blocks
   int32_t max_nsec, max_nslots;
+  int32_t max_slices;            // partial buffer: [row][shift][max_slices][order], zero-filled by the launcher
 };
 cudaError_t qmc2_kernel_prepare(int ndim, int loops, int kmax, size_t smem, int *blocks_per_sm);
 cudaError_t qmc2_kernel_launch(int ndim, int loops, int kmax, dim3 grid, size_t smem, cudaStream_t st, const Qmc2Launch &p);

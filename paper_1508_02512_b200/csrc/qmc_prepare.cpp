@@ -345,5 +345,10 @@ int qmc_build_tables(const qmc_graph *g, const qmc_kinematics *kin, int eps_orde
     while (T->image.size() % 16) T->image.push_back(0);
   }
   T->secoff.push_back((uint32_t)T->image.size());
-  return qmc_build_image2(T);
+  // version-2 image (real path); graphs it cannot represent fall back to the version-1 kernel
+  if (qmc_build_image2(T) != QMC_OK) {
+    T->image2.clear();
+    T->chunks.clear();
+  }
+  return QMC_OK;
 }

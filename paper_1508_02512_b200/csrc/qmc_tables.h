@@ -98,6 +98,7 @@ struct qmc_tables {
   std::vector<uint32_t> secoff2;  // [n_sectors + 1] byte offsets of the sector blocks in image2
   std::vector<uint32_t> secend2;  // [n_sectors] end offsets (a chunk header sits between the sectors of two chunks)
   std::vector<Qmc2Chunk> chunks;
+  std::vector<double> sec_cost;   // modelled cost per sector (load balancing of the launch)
   double logtab[256] = {0};      // 128 x {1/c_i, -ln(1/c_i)} of the kernels' table-driven logarithm
   // launcher state (host-side caches; not thread-safe by design: one tables object per stream)
   const void *resident_ws = nullptr;  // workspace the image was last uploaded to

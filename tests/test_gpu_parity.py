@@ -162,7 +162,7 @@ def test_v2_tables_chunk_boundaries_and_small_slot_budget(monkeypatch):
     b = bounds[2]
     parity(wl, 16381, 2, sectors=(b - 3, b + 4))            # straddles a chunk boundary
     parity(wl, 16381, 2, sectors=(bounds[1] - 1, bounds[3] + 1))   # spans a whole chunk plus both neighbours
-    monkeypatch.setenv("QMC2_SLOTS", "22")
+    monkeypatch.setenv("QMC2_SLOTS", "26")
     monkeypatch.setenv("QMC2_CHUNK_BYTES", "3000")
     t2 = q.qmc_prepare(wl)
     d2 = t2.describe()
