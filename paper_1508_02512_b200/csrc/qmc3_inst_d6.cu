@@ -1,0 +1,2 @@
+#include "qmc_inst3.cuh"
+QMC3_DEFINE_DIM(6)

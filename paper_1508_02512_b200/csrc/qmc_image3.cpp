@@ -1,0 +1,275 @@
+// Version-3 device image of the sector tables (complex path, contour deformation Eq. 14).  Host only.
+// Layout in qmc_tables.h.  The gradient and the Hessian of F^ (needed for rho_j, z_j and the Jacobian, R:C12) are
+// emitted as polynomials of their own: d/dt_i (c prod t^e) = c e_i t^(e - 1_i), and likewise for second derivatives.
+#include <algorithm>
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+
+#include "../../include/qmc_feynman.h"
+#include "qmc_bpe.h"
+#include "qmc_tables.h"
+
+using namespace qmcbpe;
+
+namespace {
+
+struct Mono3 {
+  double c;
+  uint8_t e[QMC_MAXDIM];
+  int group;
+};
+typedef std::vector<Mono3> Poly3;
+
+// polynomials of one sector in emission order: F_1..F_n, F_11, F_12, .., F_nn, U, F
+void sector_polys(const QmcSector &s, int n, const int *pos_of, std::vector<Poly3> &out) {
+  auto group_of = [&](const uint8_t *e) {
+    int g = 0;
+    for (int j = 0; j < n; ++j)
+      if (e[j] && pos_of[j] >= 0) g |= 1 << pos_of[j];
+    return g;
+  };
+  auto push = [&](Poly3 &P, double c, const uint8_t *e) {
+    Mono3 m;
+    m.c = c;
+    std::memset(m.e, 0, sizeof m.e);
+    for (int j = 0; j < n; ++j) m.e[j] = e[j];
+    m.group = group_of(m.e);
+    P.push_back(m);
+  };
+  out.clear();
+  for (int i = 0; i < n; ++i) {
+    Poly3 P;
+    for (const QmcMono &m : s.F)
+      if (m.e[i] >= 1) {
+        uint8_t e[QMC_MAXDIM];
+        std::memcpy(e, m.e, sizeof e);
+        e[i] -= 1;
+        push(P, m.c * m.e[i], e);
+      }
+    out.push_back(P);
+  }
+  for (int i = 0; i < n; ++i)
+    for (int k = i; k < n; ++k) {
+      Poly3 P;
+      for (const QmcMono &m : s.F) {
+        uint8_t e[QMC_MAXDIM];
+        std::memcpy(e, m.e, sizeof e);
+        double c;
+        if (i == k) {
+          if (m.e[i] < 2) continue;
+          c = m.c * m.e[i] * (m.e[i] - 1);
+          e[i] -= 2;
+        } else {
+          if (m.e[i] < 1 || m.e[k] < 1) continue;
+          c = m.c * m.e[i] * m.e[k];
+          e[i] -= 1;
+          e[k] -= 1;
+        }
+        push(P, c, e);
+      }
+      out.push_back(P);
+    }
+  for (int which = 0; which < 2; ++which) {
+    Poly3 P;
+    for (const QmcMono &m : (which ? s.F : s.U)) push(P, m.c, m.e);
+    out.push_back(P);
+  }
+  for (Poly3 &P : out)
+    std::stable_sort(P.begin(), P.end(), [](const Mono3 &a, const Mono3 &b) { return a.group < b.group; });
+}
+
+void positions(const QmcSector &s, int n, int *pos_of) {
+  int k = 0;
+  for (int j = 0; j < n; ++j) pos_of[j] = (s.alpha[j] == -1) ? k++ : -1;
+}
+
+// make every monomial a product of at most two slots, adding sector-local products; false if too many are needed
+bool localise(std::vector<Factors> &mono, size_t first, size_t count, int nslots, std::vector<std::pair<uint8_t, uint8_t>> &local) {
+  for (size_t q = 0; q < count; ++q) {
+    Factors &f = mono[first + q];
+    while (f.size() > 2) {
+      const std::pair<uint8_t, uint8_t> pr(f[0], f[1]);
+      size_t id = 0;
+      while (id < local.size() && local[id] != pr) ++id;
+      if (id == local.size()) local.push_back(pr);
+      f.erase(f.begin(), f.begin() + 2);
+      f.insert(f.begin(), (uint8_t)(nslots + id));
+    }
+  }
+  return local.size() <= QMC3_MAXLOCAL && nslots + (int)local.size() <= 255;
+}
+
+}  // namespace
+
+int qmc_build_image3(qmc_tables *t) {
+  t->image3.clear();
+  t->secoff3.clear();
+  t->secend3.clear();
+  t->chunks3.clear();
+  t->chunk3_nslots_c.clear();
+  t->chunk3_max_local_c.clear();
+  const int n = t->n, nsec = (int)t->sectors.size();
+  if (!(t->lambda > 0.0) || nsec == 0) return QMC_OK;
+  const int T = QMC3_THREADS;
+  const int npoly = n + n * (n + 1) / 2 + 2, nderiv = npoly - 2;
+  int max_r = std::min(QMC3_MAXSLOTS_R, 3 * n + 1 + 20), max_c = std::min(QMC3_MAXSLOTS_C, n + 1 + 12);
+  double chunk_bytes = 16000.0;
+  if (const char *e = std::getenv("QMC3_SLOTS_R")) max_r = std::min(QMC3_MAXSLOTS_R, std::max(3 * n + 2, std::atoi(e)));
+  if (const char *e = std::getenv("QMC3_SLOTS_C")) max_c = std::min(QMC3_MAXSLOTS_C, std::max(n + 2, std::atoi(e)));
+  if (const char *e = std::getenv("QMC3_CHUNK_BYTES")) chunk_bytes = std::max(1000.0, std::atof(e));
+
+  // ---- per-sector polynomials, chunk ranges by table bytes ------------------------------------------------------
+  std::vector<std::vector<Poly3>> polys(nsec);
+  std::vector<double> bytes(nsec);
+  if (t->sec_cost.size() != (size_t)nsec) t->sec_cost.assign(nsec, 0.0);
+  for (int si = 0; si < nsec; ++si) {
+    int pos_of[QMC_MAXDIM];
+    positions(t->sectors[si], n, pos_of);
+    sector_polys(t->sectors[si], n, pos_of, polys[si]);
+    size_t nrec = 1 + n;
+    for (const Poly3 &P : polys[si]) nrec += P.size();
+    bytes[si] = sizeof(Qmc3SectorHdr) + npoly * (1 << t->sectors[si].nsing) + 64 + 16.0 * nrec;
+    t->sec_cost[si] = (double)(1 << t->sectors[si].nsing) * (nrec + 400.0);
+  }
+  std::vector<std::pair<int, int>> todo;
+  for (int b = 0; b < nsec;) {
+    int e = b;
+    double acc = 0.0;
+    while (e < nsec && (acc + bytes[e] <= chunk_bytes || e == b)) acc += bytes[e++];
+    todo.push_back({b, e});
+    b = e;
+  }
+  t->secoff3.assign(nsec + 1, 0);
+  t->secend3.assign(nsec, 0);
+  for (size_t w = 0; w < todo.size(); ++w) {
+    const int s0 = todo[w].first, s1 = todo[w].second;
+    // ---- plan the two slot programs of the chunk ------------------------------------------------------------
+    ChunkPlan pr, pc;  // monomial order: per sector [G0][derivative polynomials...] resp. [U][F]
+    for (int si = s0; si < s1; ++si) {
+      const QmcSector &s = t->sectors[si];
+      uint8_t g[QMC_MAXDIM] = {0};
+      for (int j = 0; j < n; ++j) g[j] = (uint8_t)(s.alpha[j] > 0 ? s.alpha[j] : 0);
+      pr.mono.push_back(factors_of(g, n));
+      for (int p = 0; p < nderiv; ++p)
+        for (const Mono3 &m : polys[si][p]) pr.mono.push_back(factors_of(m.e, n));
+      for (int p = nderiv; p < npoly; ++p)
+        for (const Mono3 &m : polys[si][p]) pc.mono.push_back(factors_of(m.e, n));
+    }
+    plan_chunk(pr, 3 * n + 1, max_r);
+    plan_chunk(pc, n + 1, max_c);
+    // ---- emit --------------------------------------------------------------------------------------------------
+    Qmc2Chunk ch;
+    ch.sec_begin = s0;
+    ch.sec_end = s1;
+    ch.nslots = pr.nslots;
+    ch.prog_off = (uint32_t)t->image3.size();
+    Qmc3ChunkHdr chh;
+    std::memset(&chh, 0, sizeof chh);
+    chh.nslots_r = pr.nslots; chh.nprog_r = (uint32_t)pr.prog.size(); chh.first_prod_r = pr.first_prod;
+    chh.nslots_c = pc.nslots; chh.nprog_c = (uint32_t)pc.prog.size(); chh.first_prod_c = pc.first_prod;
+    put(t->image3, chh);
+    for (auto &q : pr.prog) { put(t->image3, (uint16_t)q.first); put(t->image3, (uint16_t)q.second); }
+    while (t->image3.size() % 16) t->image3.push_back(0);
+    for (auto &q : pc.prog) { put(t->image3, (uint16_t)q.first); put(t->image3, (uint16_t)q.second); }
+    while (t->image3.size() % 16) t->image3.push_back(0);
+    ch.prog_bytes = (uint32_t)t->image3.size() - ch.prog_off;
+    const uint32_t ONE_R = (uint32_t)(3 * n) * T * 8u, ONE_C = (uint32_t)n * T * 16u;
+    auto rec_r = [&](double c, const Factors &f) {
+      Qmc2Rec r;
+      r.c = c;
+      r.s0 = f.size() > 0 ? (uint32_t)f[0] * T * 8u : ONE_R;
+      r.s1 = f.size() > 1 ? (uint32_t)f[1] * T * 8u : ONE_R;
+      return r;
+    };
+    auto rec_c = [&](double c, const Factors &f) {
+      Qmc2Rec r;
+      r.c = c;
+      r.s0 = f.size() > 0 ? (uint32_t)f[0] * T * 16u : ONE_C;
+      r.s1 = f.size() > 1 ? (uint32_t)f[1] * T * 16u : ONE_C;
+      return r;
+    };
+    size_t mr = 0, mc = 0;
+    bool split = false;
+    int max_local_c = 0;
+    for (int si = s0; si < s1 && !split; ++si) {
+      const QmcSector &s = t->sectors[si];
+      const int ng = 1 << s.nsing;
+      size_t cnt_r = 1, cnt_c = 0;
+      for (int p = 0; p < nderiv; ++p) cnt_r += polys[si][p].size();
+      for (int p = nderiv; p < npoly; ++p) cnt_c += polys[si][p].size();
+      std::vector<std::pair<uint8_t, uint8_t>> loc_r, loc_c;
+      if (!localise(pr.mono, mr, cnt_r, pr.nslots, loc_r) || !localise(pc.mono, mc, cnt_c, pc.nslots, loc_c)) {
+        split = true;
+        break;
+      }
+      Qmc3SectorHdr h;
+      std::memset(&h, 0, sizeof h);
+      h.nsing = (uint8_t)s.nsing;
+      int k = 0;
+      for (int j = 0; j < n; ++j) {
+        h.alpha[j] = (int8_t)s.alpha[j];
+        h.beta[j] = (int8_t)s.beta[j];
+        if (s.alpha[j] == -1) {
+          h.sing_var[k] = (uint8_t)j;
+          h.betas[k] = (double)s.beta[j];
+          h.invbeta[k] = 1.0 / (double)s.beta[j];
+          ++k;
+        }
+      }
+      std::vector<uint8_t> counts((size_t)npoly * ng, 0);
+      std::vector<Qmc2Rec> rr, rc;
+      rr.push_back(rec_r(1.0, pr.mono[mr++]));  // G0
+      for (int j = 0; j < n; ++j)
+        if (s.alpha[j] != -1 && s.beta[j] != 0) {  // L0 = sum over regular variables of beta_j ln t_j
+          Qmc2Rec r;
+          r.c = (double)s.beta[j];
+          r.s0 = (uint32_t)(n + j) * T * 8u;
+          r.s1 = ONE_R;
+          rr.push_back(r);
+          ++h.nL0;
+        }
+      for (int p = 0; p < npoly; ++p)
+        for (const Mono3 &m : polys[si][p]) {
+          uint8_t &c = counts[(size_t)p * ng + m.group];
+          if (c == 255) return QMC_EUNSUPPORTED;
+          ++c;
+          if (p < nderiv) rr.push_back(rec_r(m.c, pr.mono[mr++]));
+          else rc.push_back(rec_c(m.c, pc.mono[mc++]));
+        }
+      if (rr.size() > 65535 || rc.size() > 65535) return QMC_EUNSUPPORTED;
+      h.nrec_r = (uint16_t)rr.size();
+      h.nrec_c = (uint16_t)rc.size();
+      h.nlocal_r = (uint8_t)loc_r.size();
+      h.nlocal_c = (uint8_t)loc_c.size();
+      ch.max_local = std::max(ch.max_local, (int)loc_r.size());
+      max_local_c = std::max(max_local_c, (int)loc_c.size());
+      ch.cost += t->sec_cost[si];
+      t->secoff3[si] = (uint32_t)t->image3.size();
+      put(t->image3, h);
+      t->image3.insert(t->image3.end(), counts.begin(), counts.end());
+      while (t->image3.size() % 16) t->image3.push_back(0);
+      for (auto &q : loc_r) { put(t->image3, (uint16_t)q.first); put(t->image3, (uint16_t)q.second); }
+      while (t->image3.size() % 16) t->image3.push_back(0);
+      for (auto &q : loc_c) { put(t->image3, (uint16_t)q.first); put(t->image3, (uint16_t)q.second); }
+      while (t->image3.size() % 16) t->image3.push_back(0);
+      for (const Qmc2Rec &r : rr) put(t->image3, r);
+      for (const Qmc2Rec &r : rc) put(t->image3, r);
+      t->secend3[si] = (uint32_t)t->image3.size();
+    }
+    if (split) {
+      t->image3.resize(ch.prog_off);
+      if (s1 - s0 == 1) return QMC_EUNSUPPORTED;
+      const int mid = (s0 + s1) / 2;
+      todo[w] = {s0, mid};
+      todo.insert(todo.begin() + w + 1, {mid, s1});
+      --w;
+      continue;
+    }
+    t->chunks3.push_back(ch);
+    t->chunk3_nslots_c.push_back(pc.nslots);
+    t->chunk3_max_local_c.push_back(max_local_c);
+  }
+  t->secoff3[nsec] = (uint32_t)t->image3.size();
+  return QMC_OK;
+}

@@ -1,0 +1,495 @@
+// Evaluation kernel, version 3 (complex path: physical region, contour deformation), sm_100a.  Steps S1-S7 of DESIGN.md.
+//
+// Same organisation as version 2 (qmc_kernels2.cuh): one thread = one lattice point, a block = one slice of the points
+// of a run of sectors of one chunk, tables staged by TMA, monomials as 16-byte records over per-thread slot tables in
+// shared memory.  Per corner Z of a sector (real point tau = t with the variables of Z set to 0):
+//   S4  F^_i(tau), F^_ik(tau) from the record lists of the derivative polynomials (groups meeting Z are skipped);
+//       rho_i = 1 - i lambda (1 - tau_i) F^_i,  z_i = tau_i rho_i,
+//       J_ik = delta_ik [1 - i lambda (1 - 2 tau_i) F^_i] - i lambda tau_i (1 - tau_i) F^_ik   (Eq. 14; R:C12),
+//       det J by LU with row pivoting;
+//   S5  the complex slot table is refilled with z_j and the chunk's products, U^(z), F^(z) are sums of complex records;
+//       G_Z = G0 det J prod_{j notin Z} rho_j^alpha_j U^aU0 F^aF0,
+//       Lambda_Z = aU1 ln U + aF1 ln F + sum_j beta_j ln rho_j + L0   (principal logs; -i pi on the negative real axis, R:C11);
+//   S6  product form folded one singular variable at a time with exact series windows (as Fold2, complex).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "qmc_kernels2.cuh"
+
+namespace qmc3 {
+
+using qmcdev::cd;
+using qmcdev::cinv;
+using qmcdev::cnorm2;
+using qmcdev::mbar_expect_tx;
+using qmcdev::mbar_init;
+using qmcdev::mbar_wait;
+using qmcdev::tma_bulk_g2s;
+using qmc2::Expo;
+using qmc2::fast_log;
+using qmc2::fast_rcp;
+
+static __device__ __noinline__ double atan2_lib(double y, double x) { return atan2(y, x); }
+// principal log; a negative real argument carries the -i0 of F -> F - i0: arg = -pi (R:C11)
+__device__ __forceinline__ cd clog3(cd a, const double2 *__restrict__ logtab) {
+  const double arg = (a.im == 0.0 && a.re < 0.0) ? -3.14159265358979323846 : atan2_lib(a.im, a.re);
+  return cd{0.5 * fast_log(cnorm2(a), logtab), arg};
+}
+template <int E>
+__device__ __forceinline__ cd cpow_c(cd x) {  // x^E, E >= 0 compile time
+  if (E == 0) return cd{1.0, 0.0};
+  if (E == 1) return x;
+  cd h = cpow_c<E / 2>(x);
+  h = h * h;
+  return (E & 1) ? h * x : h;
+}
+
+// sum of n real records c * slot[s0] * slot[s1] (byte offsets into the thread's real column)
+__device__ __forceinline__ double rsum(const uint4 *__restrict__ &rec, int n, const unsigned char *__restrict__ sl) {
+  double acc = 0.0;
+#pragma unroll 1
+  for (int i = 0; i < n; ++i) {
+    const uint4 r = *rec++;
+    acc = fma(__hiloint2double((int)r.y, (int)r.x),
+              *reinterpret_cast<const double *>(sl + r.z) * *reinterpret_cast<const double *>(sl + r.w), acc);
+  }
+  return acc;
+}
+// sum of n complex records (byte offsets into the thread's complex column, 16 bytes per entry)
+__device__ __forceinline__ cd csum(const uint4 *__restrict__ &rec, int n, const unsigned char *__restrict__ sl) {
+  cd acc = cd{0.0, 0.0};
+#pragma unroll 1
+  for (int i = 0; i < n; ++i) {
+    const uint4 r = *rec++;
+    const double c = __hiloint2double((int)r.y, (int)r.x);
+    const double2 a = *reinterpret_cast<const double2 *>(sl + r.z), b = *reinterpret_cast<const double2 *>(sl + r.w);
+    acc.re = fma(c, a.x * b.x - a.y * b.y, acc.re);
+    acc.im = fma(c, a.x * b.y + a.y * b.x, acc.im);
+  }
+  return acc;
+}
+
+template <int NDIM, int NS, int K>
+struct Ctx3 {
+  double invt[NS > 0 ? NS : 1], invbeta[NS > 0 ? NS : 1];
+  double cL[NS > 0 ? NS : 1][K > 1 ? K - 1 : 1];
+  const Qmc3SectorHdr *h;
+  const uint8_t *counts;            // [npoly][1 << NS]
+  const uint4 *rec_deriv, *rec_c;   // first record of F_1, first complex record
+  const uint32_t *locprog_c;        // sector-local complex products
+  const uint32_t *prog_c;           // chunk complex program
+  int nprog_c, first_prod_c, local0_c;
+  const unsigned char *slr;         // this thread's real column (bytes)
+  double2 *slc;                     // this thread's complex column: element s at slc[s * QMC3_THREADS]
+  const double2 *logtab;
+  double G0, L0, lambda;
+  unsigned cntImF, cntReU;
+};
+
+// W_Z and Lambda_Z of one corner (Z = bit mask over the singular positions)
+template <int NDIM, int L, int NS, int K>
+__device__ __noinline__ void corner3(Ctx3<NDIM, NS, K> &c, const int Z, cd &Wout, cd &Lout) {
+  constexpr int NG = 1 << NS, T = QMC3_THREADS, NDERIV = NDIM + NDIM * (NDIM + 1) / 2;
+  typedef Expo<NDIM, L> E;
+  const Qmc3SectorHdr *h = c.h;
+  unsigned zv = 0;  // variables set to zero
+#pragma unroll
+  for (int k = 0; k < NS; ++k)
+    if (Z >> k & 1) zv |= 1u << h->sing_var[k];
+  // ---- S4: gradient and Hessian of F^ at tau -------------------------------------------------------------------
+  double grad[NDIM], hess[NDIM][NDIM];
+  {
+    const uint4 *rec = c.rec_deriv;
+    const uint8_t *cnt = c.counts;
+#pragma unroll
+    for (int i = 0; i < NDIM; ++i) {
+      double s = 0.0;
+#pragma unroll
+      for (int g = 0; g < NG; ++g) {
+        const int n = *cnt++;
+        if (g & Z) rec += n; else s += rsum(rec, n, c.slr);
+      }
+      grad[i] = s;
+    }
+#pragma unroll
+    for (int i = 0; i < NDIM; ++i)
+#pragma unroll
+      for (int k = i; k < NDIM; ++k) {
+        double s = 0.0;
+#pragma unroll
+        for (int g = 0; g < NG; ++g) {
+          const int n = *cnt++;
+          if (g & Z) rec += n; else s += rsum(rec, n, c.slr);
+        }
+        hess[i][k] = s;
+      }
+  }
+  // rho_i, z_i, J = 1 + i B
+  cd rho[NDIM], J[NDIM][NDIM];
+#pragma unroll
+  for (int i = 0; i < NDIM; ++i) {
+    const bool inZ = (zv >> i & 1u) != 0;
+    const double tau = inZ ? 0.0 : *reinterpret_cast<const double *>(c.slr + (size_t)i * T * 8);
+    rho[i] = cd{1.0, -c.lambda * (1.0 - tau) * grad[i]};
+    c.slc[i * T] = make_double2(tau, tau * rho[i].im);  // z_i = tau rho_i
+#pragma unroll
+    for (int k = 0; k < NDIM; ++k) {
+      const bool kinZ = (zv >> k & 1u) != 0;
+      if (inZ || kinZ) {
+        J[i][k] = cd{(i == k) ? 1.0 : 0.0, 0.0};  // row / column of a Z variable: its rho cancels rho^-1 (alpha = -1)
+      } else {
+        const double hik = (k >= i) ? hess[i][k] : hess[k][i];
+        double b = -c.lambda * tau * (1.0 - tau) * hik;
+        if (i == k) b += -c.lambda * (1.0 - 2.0 * tau) * grad[i];
+        J[i][k] = cd{(i == k) ? 1.0 : 0.0, b};
+      }
+    }
+  }
+  cd det = cd{1.0, 0.0};
+#pragma unroll
+  for (int col = 0; col < NDIM; ++col) {
+#pragma unroll
+    for (int r = col + 1; r < NDIM; ++r) {
+      if (cnorm2(J[r][col]) > cnorm2(J[col][col])) {
+#pragma unroll
+        for (int k = col; k < NDIM; ++k) {
+          cd tmp = J[r][k];
+          J[r][k] = J[col][k];
+          J[col][k] = tmp;
+        }
+        det = cd{-det.re, -det.im};
+      }
+    }
+    det = det * J[col][col];
+    if (col + 1 < NDIM) {
+      const cd ip = cinv(J[col][col]);
+#pragma unroll
+      for (int r = col + 1; r < NDIM; ++r) {
+        const cd f = J[r][col] * ip;
+#pragma unroll
+        for (int k = col + 1; k < NDIM; ++k) J[r][k] = J[r][k] - f * J[col][k];
+      }
+    }
+  }
+  // ---- S5: complex slot table over z, U^(z), F^(z) -----------------------------------------------------------------
+#pragma unroll 1
+  for (int i = 0; i < c.nprog_c; ++i) {
+    const uint32_t w = c.prog_c[i];
+    const double2 a = c.slc[(w & 0xffffu) * T], b = c.slc[(w >> 16) * T];
+    c.slc[(c.first_prod_c + i) * T] = make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+  }
+#pragma unroll 1
+  for (int i = 0; i < h->nlocal_c; ++i) {
+    const uint32_t w = c.locprog_c[i];
+    const double2 a = c.slc[(w & 0xffffu) * T], b = c.slc[(w >> 16) * T];
+    c.slc[(c.local0_c + i) * T] = make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+  }
+  cd Uv = cd{0.0, 0.0}, Fv = cd{0.0, 0.0};
+  {
+    const uint4 *rec = c.rec_c;
+    const uint8_t *cnt = c.counts + NDERIV * NG;
+    const unsigned char *slcb = reinterpret_cast<const unsigned char *>(c.slc);
+#pragma unroll
+    for (int g = 0; g < NG; ++g) {
+      const int n = *cnt++;
+      if (g & Z) rec += n; else Uv = Uv + csum(rec, n, slcb);
+    }
+#pragma unroll
+    for (int g = 0; g < NG; ++g) {
+      const int n = *cnt++;
+      if (g & Z) rec += n; else Fv = Fv + csum(rec, n, slcb);
+    }
+  }
+  if (Fv.im > 0.0) ++c.cntImF;
+  if (!(Uv.re > 0.0)) ++c.cntReU;
+  // G_Z = G0 det J prod_{j notin Z} rho_j^alpha_j U^aU0 F^aF0 ;  Lambda_Z = aU1 ln U + aF1 ln F + sum_j beta_j ln rho_j + L0
+  cd num = cd{c.G0 * det.re, c.G0 * det.im}, den = cd{1.0, 0.0};
+  cd Lam = (double)E::aU1 * clog3(Uv, c.logtab) + (double)E::aF1 * clog3(Fv, c.logtab);
+  Lam.re += c.L0;
+#pragma unroll
+  for (int j = 0; j < NDIM; ++j) {
+    const bool inZ = (zv >> j & 1u) != 0;
+    const int a = h->alpha[j], b = h->beta[j];
+    if (!inZ) {
+      if (a < 0) den = den * rho[j];
+      for (int q = 0; q < a; ++q) num = num * rho[j];
+    }
+    if (b) Lam = Lam + (double)b * clog3(rho[j], c.logtab);
+  }
+  if (E::aU0 > 0) num = num * cpow_c<(E::aU0 > 0 ? E::aU0 : 0)>(Uv);
+  if (E::aU0 < 0) den = den * cpow_c<(E::aU0 < 0 ? -E::aU0 : 0)>(Uv);
+  if (E::aF0 > 0) num = num * cpow_c<(E::aF0 > 0 ? E::aF0 : 0)>(Fv);
+  if (E::aF0 < 0) den = den * cpow_c<(E::aF0 < 0 ? -E::aF0 : 0)>(Fv);
+  Wout = num * cinv(den);
+  Lout = Lam;
+}
+
+// fold of the singular variables with exact series windows (see qmc2::Fold2), complex
+template <int NDIM, int L, int NS, int KMAX, int K, int LEVEL, int ZMASK>
+struct Fold3 {
+  static constexpr int LEN = NS - LEVEL + KMAX + __builtin_popcount(ZMASK) + 1;
+  static __device__ __forceinline__ void eval(Ctx3<NDIM, NS, K> &c, cd (&out)[LEN]) {
+    cd a[LEN - 1], b[LEN];
+    Fold3<NDIM, L, NS, KMAX, K, LEVEL + 1, ZMASK>::eval(c, a);
+    Fold3<NDIM, L, NS, KMAX, K, LEVEL + 1, ZMASK | (1 << LEVEL)>::eval(c, b);
+    const double it = c.invt[LEVEL], ib = c.invbeta[LEVEL];
+    cd d[LEN - 1];
+#pragma unroll
+    for (int i = 0; i < LEN - 1; ++i) d[i] = it * (a[i] - b[i]);
+    out[0] = ib * b[0];
+#pragma unroll
+    for (int i = 1; i < LEN; ++i) {
+      cd s = ib * b[i] + d[i - 1];
+#pragma unroll
+      for (int p = 1; p < i; ++p) s = s + c.cL[LEVEL][p] * d[i - 1 - p];
+      out[i] = s;
+    }
+  }
+};
+template <int NDIM, int L, int NS, int KMAX, int K, int ZMASK>
+struct Fold3<NDIM, L, NS, KMAX, K, NS, ZMASK> {
+  static constexpr int LEN = KMAX + __builtin_popcount(ZMASK) + 1;
+  static __device__ __forceinline__ void eval(Ctx3<NDIM, NS, K> &c, cd (&out)[LEN]) {
+    cd W, Lam;
+    corner3<NDIM, L, NS, K>(c, ZMASK, W, Lam);
+    out[0] = W;
+#pragma unroll
+    for (int p = 1; p < LEN; ++p) out[p] = (1.0 / p) * (out[p - 1] * Lam);
+  }
+};
+
+// one sector at one point: out[i] = coefficient of eps^(i - NS)
+template <int NDIM, int L, int NS, int KMAX>
+__device__ __forceinline__ void sector3(const Qmc3SectorHdr *__restrict__ h, double *__restrict__ slr_d, double2 *__restrict__ slc,
+                                        int local0_r, const uint32_t *prog_c, int nprog_c, int first_prod_c, int local0_c,
+                                        double lambda, const double2 *__restrict__ logtab, cd (&out)[KMAX + NS + 1],
+                                        unsigned &cntImF, unsigned &cntReU) {
+  constexpr int K = KMAX + NS + 1, NG = 1 << NS, T = QMC3_THREADS, NPOLY = NDIM + NDIM * (NDIM + 1) / 2 + 2;
+  Ctx3<NDIM, NS, K> c;
+  c.h = h;
+  const unsigned char *p = reinterpret_cast<const unsigned char *>(h + 1);
+  c.counts = p;
+  p += (NPOLY * NG + 15) & ~15;
+  const uint32_t *locprog_r = reinterpret_cast<const uint32_t *>(p);
+  p += (h->nlocal_r * 4 + 15) & ~15;
+  c.locprog_c = reinterpret_cast<const uint32_t *>(p);
+  p += (h->nlocal_c * 4 + 15) & ~15;
+  const uint4 *rec = reinterpret_cast<const uint4 *>(p);
+  c.rec_c = rec + h->nrec_r;
+  c.prog_c = prog_c; c.nprog_c = nprog_c; c.first_prod_c = first_prod_c; c.local0_c = local0_c;
+  c.slr = reinterpret_cast<const unsigned char *>(slr_d);
+  c.slc = slc;
+  c.logtab = logtab;
+  c.lambda = lambda;
+  c.cntImF = 0; c.cntReU = 0;
+  {  // sector-local real products
+    const int nl = h->nlocal_r;
+#pragma unroll 1
+    for (int i = 0; i < nl; ++i) {
+      const uint32_t w = locprog_r[i];
+      slr_d[(local0_r + i) * T] = slr_d[(w & 0xffffu) * T] * slr_d[(w >> 16) * T];
+    }
+  }
+  c.G0 = rsum(rec, 1, c.slr);
+  c.L0 = rsum(rec, h->nL0, c.slr);
+  c.rec_deriv = rec;
+#pragma unroll
+  for (int k = 0; k < NS; ++k) {
+    const int j = h->sing_var[k];
+    c.invt[k] = slr_d[(2 * NDIM + j) * T];
+    c.invbeta[k] = h->invbeta[k];
+    const double Lk = h->betas[k] * slr_d[(NDIM + j) * T];
+    c.cL[k][0] = 1.0;
+#pragma unroll
+    for (int q = 1; q < K - 1; ++q) c.cL[k][q] = c.cL[k][q - 1] * Lk * (1.0 / q);
+  }
+  Fold3<NDIM, L, NS, KMAX, K, 0, 0>::eval(c, out);
+  cntImF += c.cntImF;
+  cntReU += c.cntReU;
+}
+
+__device__ __forceinline__ bool finite_hi(cd v) {
+  return (__double2hiint(v.re) & 0x7ff00000) != 0x7ff00000 && (__double2hiint(v.im) & 0x7ff00000) != 0x7ff00000;
+}
+
+}  // namespace qmc3
+
+// partial layout: fused [run][shift][slice][NACC][2], persec [sector row][shift][slice][NACC][2]
+template <int NDIM, int L, int KMAX>
+__global__ void __launch_bounds__(QMC3_THREADS, 1) qmc3_eval_kernel(const Qmc3Launch q) {
+  using namespace qmc3;
+  const Qmc2Launch &p = q.b;
+  constexpr int NACC = QMC_MAXSING + KMAX + 1;
+  constexpr int SMAX = NDIM < QMC3_MAXSING ? NDIM : QMC3_MAXSING;
+  constexpr int T = QMC3_THREADS;
+
+  extern __shared__ __align__(16) unsigned char smem[];
+  const int tid = threadIdx.x;
+  const Qmc2Work wk = p.work[blockIdx.x];
+
+  unsigned char *sprog = smem;
+  unsigned char *stab = smem + p.sm_prog_cap;
+  size_t o = (size_t)p.sm_prog_cap + p.sm_sec_cap;
+  uint32_t *soff = reinterpret_cast<uint32_t *>(smem + o);
+  o += (((size_t)(p.max_nsec + 1) * 4) + 15) & ~(size_t)15;
+  uint64_t *bar = reinterpret_cast<uint64_t *>(smem + o);
+  o += 16;
+  double *shf = reinterpret_cast<double *>(smem + o);
+  o += (((size_t)p.m * NDIM * 8) + 15) & ~(size_t)15;
+  double *scratch = reinterpret_cast<double *>(smem + o);
+  o += (T / 32) * 8;
+  double2 *logtab = reinterpret_cast<double2 *>(smem + o);
+  o += 128 * 16;
+  double *slots_r = reinterpret_cast<double *>(smem + o);
+  o += (size_t)p.max_nslots * T * 8;
+  double2 *slots_c = reinterpret_cast<double2 *>(smem + o);
+  o += (size_t)q.max_nslots_c * T * 16;
+  double *sacc = reinterpret_cast<double *>(smem + o);  // persec: [nsec][NACC*2][T]
+  double *slr = slots_r + tid;
+  double2 *slc = slots_c + tid;
+
+  if (tid == 0) {
+    mbar_init(bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (tid == 0) {
+    mbar_expect_tx(bar, wk.prog_bytes + wk.sec_bytes);
+    tma_bulk_g2s(sprog, p.image2 + wk.prog_off, wk.prog_bytes, bar);
+    tma_bulk_g2s(stab, p.image2 + wk.sec_off, wk.sec_bytes, bar);
+  }
+  for (int i = tid; i <= wk.nsec; i += T) soff[i] = p.secoff2[wk.s0 + i] - wk.sec_off;
+  for (int i = tid; i < p.m * NDIM; i += T) shf[i] = p.shifts[i];
+  for (int i = tid; i < 256; i += T) reinterpret_cast<double *>(logtab)[i] = p.logtab[i];
+  slr[3 * NDIM * T] = 1.0;
+  slc[NDIM * T] = make_double2(1.0, 0.0);
+  mbar_wait(bar, 0);
+  __syncthreads();
+
+  const Qmc3ChunkHdr *ch = reinterpret_cast<const Qmc3ChunkHdr *>(sprog);
+  const uint32_t *prog_r = reinterpret_cast<const uint32_t *>(sprog + sizeof(Qmc3ChunkHdr));
+  const int nprog_r = ch->nprog_r, first_prod_r = ch->first_prod_r, local0_r = ch->nslots_r;
+  const uint32_t *prog_c = prog_r + ((nprog_r + 3) & ~3);
+  const int nprog_c = ch->nprog_c, first_prod_c = ch->first_prod_c, local0_c = ch->nslots_c;
+
+  const uint32_t N = p.N;
+  const double dN = (double)N;
+  const uint32_t stride = (uint32_t)wk.nslices * T;
+  uint32_t dz[NDIM];
+#pragma unroll
+  for (int j = 0; j < NDIM; ++j) dz[j] = (uint32_t)(((uint64_t)stride * p.zeff[j]) % N);
+
+  unsigned cntImF = 0, cntReU = 0, cntNonFinite = 0, cntBoundary = 0;
+
+  for (int kap = 0; kap < p.m; ++kap) {
+    cd acc[NACC];
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) acc[a] = cd{0.0, 0.0};
+    if (p.persec)
+      for (int i = 0; i < wk.nsec * NACC * 2; ++i) sacc[(size_t)i * T + tid] = 0.0;
+
+    uint32_t cidx = (uint32_t)wk.slice * T + tid;
+    uint32_t r[NDIM];
+#pragma unroll
+    for (int j = 0; j < NDIM; ++j) r[j] = (uint32_t)((p.off[j] + (uint64_t)cidx * p.zeff[j]) % N);
+
+    for (; cidx < p.count; cidx += stride) {
+      double w = 1.0;
+      bool inside = true;
+#pragma unroll
+      for (int j = 0; j < NDIM; ++j) {
+        double u = (double)r[j] / dN;
+        double y = u + shf[kap * NDIM + j];
+        if (y >= 1.0) y -= 1.0;
+        double tj;
+        if (p.transform == 0) {
+          tj = y * y * (3.0 - 2.0 * y);
+          w *= 6.0 * y * (1.0 - y);
+        } else {
+          tj = 1.0 - fabs(2.0 * y - 1.0);
+        }
+        if (!(y > 0.0) || !(tj > 0.0)) inside = false;
+        slr[j * T] = tj;
+        slr[(NDIM + j) * T] = fast_log(tj, logtab);
+        slr[(2 * NDIM + j) * T] = fast_rcp(tj);
+        uint32_t rn = r[j] + dz[j];
+        r[j] = rn >= N ? rn - N : rn;
+      }
+      if (!inside) {
+        if (wk.count_boundary) ++cntBoundary;
+        continue;
+      }
+      for (int i = 0; i < nprog_r; ++i) {
+        const uint32_t pw = prog_r[i];
+        slr[(first_prod_r + i) * T] = slr[(pw & 0xffffu) * T] * slr[(pw >> 16) * T];
+      }
+      for (int si = 0; si < wk.nsec; ++si) {
+        const Qmc3SectorHdr *h = reinterpret_cast<const Qmc3SectorHdr *>(stab + soff[si]);
+#define QMC3_CASE(NS_)                                                                                       \
+  case NS_: {                                                                                                \
+    if (NS_ <= SMAX) {                                                                                       \
+      constexpr int NSC = NS_ <= SMAX ? NS_ : 0, KK = KMAX + NSC + 1;                                        \
+      cd res[KK];                                                                                            \
+      sector3<NDIM, L, NSC, KMAX>(h, slr, slc, local0_r, prog_c, nprog_c, first_prod_c, local0_c, q.lambda,  \
+                                  logtab, res, cntImF, cntReU);                                              \
+      bool fin = true;                                                                                       \
+      _Pragma("unroll") for (int i = 0; i < KK; ++i) fin = fin && finite_hi(res[i]);                         \
+      if (!fin) {                                                                                            \
+        ++cntNonFinite;                                                                                      \
+      } else if (!p.persec) {                                                                                \
+        _Pragma("unroll") for (int i = 0; i < KK; ++i) {                                                     \
+          acc[QMC_MAXSING - NSC + i].re = fma(w, res[i].re, acc[QMC_MAXSING - NSC + i].re);                  \
+          acc[QMC_MAXSING - NSC + i].im = fma(w, res[i].im, acc[QMC_MAXSING - NSC + i].im);                  \
+        }                                                                                                    \
+      } else {                                                                                               \
+        double *sa = sacc + ((size_t)si * NACC + (QMC_MAXSING - NSC)) * 2 * T + tid;                         \
+        _Pragma("unroll") for (int i = 0; i < KK; ++i) {                                                     \
+          sa[(size_t)(2 * i) * T] += w * res[i].re;                                                          \
+          sa[(size_t)(2 * i + 1) * T] += w * res[i].im;                                                      \
+        }                                                                                                    \
+      }                                                                                                      \
+    }                                                                                                        \
+  } break;
+        switch (h->nsing) {
+          QMC3_CASE(0)
+          QMC3_CASE(1)
+          QMC3_CASE(2)
+          default:
+            break;
+        }
+#undef QMC3_CASE
+      }
+    }
+
+    if (!p.persec) {
+      double *dst = p.partial + (((size_t)wk.out_row * p.m + kap) * p.max_slices + wk.slice) * (NACC * 2);
+#pragma unroll
+      for (int a = 0; a < NACC; ++a) {
+        double sr = qmcdev::block_sum(acc[a].re, scratch);
+        double si = qmcdev::block_sum(acc[a].im, scratch);
+        if (tid == 0) {
+          dst[2 * a] = sr;
+          dst[2 * a + 1] = si;
+        }
+      }
+    } else {
+      for (int si = 0; si < wk.nsec; ++si) {
+        double *dst = p.partial + (((size_t)(wk.out_row + si) * p.m + kap) * p.max_slices + wk.slice) * (NACC * 2);
+        for (int a = 0; a < NACC * 2; ++a) {
+          double v = qmcdev::block_sum(sacc[((size_t)si * NACC * 2 + a) * T + tid], scratch);
+          if (tid == 0) dst[a] = v;
+        }
+      }
+    }
+  }
+
+  unsigned c4[4] = {cntImF, cntReU, cntNonFinite, cntBoundary};
+#pragma unroll
+  for (int qq = 0; qq < 4; ++qq) {
+    unsigned v = c4[qq];
+#pragma unroll
+    for (int o2 = 16; o2 > 0; o2 >>= 1) v += __shfl_down_sync(0xffffffffu, v, o2);
+    if ((tid & 31) == 0 && v) atomicAdd(p.counters + qq, (unsigned long long)v);
+  }
+}

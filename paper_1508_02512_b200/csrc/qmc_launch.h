@@ -51,6 +51,18 @@ struct Qmc2Launch {
   int32_t max_nsec, max_nslots;
   int32_t max_slices;            // partial buffer: [row][shift][max_slices][order], zero-filled by the launcher
 };
+// ---- version 3 (complex path) ------------------------------------------------------------------------------
+#define QMC3_MAXSING 2  // sectors with more singular variables go to the version-1 kernel
+struct Qmc3Launch {
+  Qmc2Launch b;          // image2 / secoff2 here mean image3 / secoff3; max_nslots = real slots (incl. local)
+  double lambda;
+  int32_t max_nslots_c;  // complex slots (incl. local)
+  int32_t pad;
+};
+cudaError_t qmc3_kernel_prepare(int ndim, int loops, int kmax, size_t smem, int *blocks_per_sm);
+cudaError_t qmc3_kernel_launch(int ndim, int loops, int kmax, dim3 grid, size_t smem, cudaStream_t st, const Qmc3Launch &p);
+bool qmc3_kernel_available(int ndim, int loops, int kmax);
+
 cudaError_t qmc2_kernel_prepare(int ndim, int loops, int kmax, size_t smem, int *blocks_per_sm);
 cudaError_t qmc2_kernel_launch(int ndim, int loops, int kmax, dim3 grid, size_t smem, cudaStream_t st, const Qmc2Launch &p);
 bool qmc2_kernel_available(int ndim, int loops, int kmax);

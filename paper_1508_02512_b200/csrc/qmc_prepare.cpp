@@ -350,5 +350,9 @@ int qmc_build_tables(const qmc_graph *g, const qmc_kinematics *kin, int eps_orde
     T->image2.clear();
     T->chunks.clear();
   }
+  if (qmc_build_image3(T) != QMC_OK) {
+    T->image3.clear();
+    T->chunks3.clear();
+  }
   return QMC_OK;
 }

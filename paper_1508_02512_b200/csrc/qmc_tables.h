@@ -70,6 +70,34 @@ struct Qmc2Chunk {      // host description of one chunk
   double cost = 0.0;                      // modelled flops per point (load balancing)
 };
 
+// ---- device image, version 3 (complex path: contour deformation) --------------------------------------
+// Same idea as version 2, with TWO slot tables per thread: a REAL one at the lattice point (t_j, ln t_j, 1/t_j, 1,
+// products) that serves the gradient and Hessian polynomials of F^ -- emitted by qmc_prepare as record lists of their
+// own -- and the regular-variable factors; and a COMPLEX one over the deformed variables z_j (z_j, 1, products),
+// refilled at every corner, that serves U^(z) and F^(z).  Records are sorted per polynomial by group; a corner Z keeps
+// the groups disjoint from Z.
+#define QMC3_THREADS 256
+#define QMC3_MAXSLOTS_R 56
+#define QMC3_MAXSLOTS_C 40
+#define QMC3_MAXLOCAL 8
+struct Qmc3ChunkHdr {  // 32 bytes; followed by program R then program C: {u16 a, u16 b} slot indices, each padded to 16 bytes
+  uint32_t nslots_r, nprog_r, first_prod_r;
+  uint32_t nslots_c, nprog_c, first_prod_c;
+  uint32_t pad[2];
+};
+struct Qmc3SectorHdr {  // 96 bytes; followed by: group counts u8 [npoly][2^nsing] (npoly = n + n(n+1)/2 + 2: F_i, F_ik (i<=k),
+                        // U, F), padded to 16 | local program R | local program C (each padded to 16) | real records
+                        // [G0][L0 x nL0][F_1..F_n][F_11, F_12, .., F_nn] | complex records [U^][F^]
+  uint8_t nsing, nL0, nlocal_r, nlocal_c;
+  uint16_t nrec_r, nrec_c;
+  uint8_t sing_var[QMC_MAXSING];   // variable index of singular position k
+  uint8_t pad0[4];
+  int8_t alpha[QMC_MAXDIM], beta[QMC_MAXDIM];  // original variable order
+  double invbeta[QMC_MAXSING];     // 1/beta of singular position k
+  double betas[QMC_MAXSING];       // beta of singular position k
+};
+static_assert(sizeof(Qmc3SectorHdr) == 96, "v3 sector header");
+
 // ---- host tables --------------------------------------------------------------------------------
 struct QmcMono {
   double c;
@@ -100,6 +128,11 @@ struct qmc_tables {
   std::vector<Qmc2Chunk> chunks;
   std::vector<double> sec_cost;   // modelled cost per sector (load balancing of the launch)
   double logtab[256] = {0};      // 128 x {1/c_i, -ln(1/c_i)} of the kernels' table-driven logarithm
+  // version 3 image (complex path only)
+  std::vector<uint8_t> image3;
+  std::vector<uint32_t> secoff3, secend3;
+  std::vector<Qmc2Chunk> chunks3;    // nslots = real slots; prog_off/prog_bytes cover the chunk header + both programs
+  std::vector<int> chunk3_nslots_c, chunk3_max_local_c;
   // launcher state (host-side caches; not thread-safe by design: one tables object per stream)
   const void *resident_ws = nullptr;  // workspace the image was last uploaded to
   int resident_m = 0;                 // number of shift vectors resident in that workspace (0 = none)
@@ -122,5 +155,7 @@ struct qmc_tables {
 // builds sectors (+ image) from a graph; returns a qmc_status
 // builds image2 / secoff2 / chunks from `sectors` (real path); returns a qmc_status
 int qmc_build_image2(qmc_tables *t);
+// builds image3 / secoff3 / chunks3 (complex path); returns a qmc_status
+int qmc_build_image3(qmc_tables *t);
 int qmc_build_tables(const qmc_graph *g, const qmc_kinematics *kin, int eps_order, const qmc_options *opt,
                      qmc_tables *out);
