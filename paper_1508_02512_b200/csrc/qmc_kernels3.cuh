@@ -30,11 +30,60 @@ using qmc2::Expo;
 using qmc2::fast_log;
 using qmc2::fast_rcp;
 
+// Shared-memory accesses by 32-bit shared address: corner3 is an out-of-line function, and through generic pointers
+// kept in a struct the compiler emits generic loads with 64-bit address arithmetic (measured: 10 % LD, 13 % R2UR).
+__device__ __forceinline__ uint32_t saddr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ double lds_f64(uint32_t a) {
+  double v;
+  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ double2 lds_f64x2(uint32_t a) {
+  double2 v;
+  asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ uint4 lds_u32x4(uint32_t a) {
+  uint4 v;
+  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ uint32_t lds_u32(uint32_t a) {
+  uint32_t v;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ uint32_t lds_u8(uint32_t a) {
+  uint32_t v;
+  asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ void sts_f64x2(uint32_t a, double x, double y) {
+  asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(a), "d"(x), "d"(y) : "memory");
+}
+// qmc2::fast_log with the table given by shared address
+__device__ __forceinline__ double fast_log_s(double x, uint32_t tab) {
+  const int hi = __double2hiint(x), lo = __double2loint(x);
+  const bool ok = (unsigned)(hi - 0x00100000) < 0x7fe00000u;
+  const int tmp = hi - 0x3fe60000;
+  const int e = tmp >> 20;
+  const double2 T = lds_f64x2(tab + (((unsigned)tmp >> 13) & 127u) * 16u);
+  const double z = __hiloint2double(hi - (tmp & 0xfff00000), lo);
+  const double r = fma(z, T.x, -1.0);
+  const double y0 = fma((double)e, qmc2::qmc2_logc[0], T.y);
+  double q = fma(r, qmc2::qmc2_logc[1], qmc2::qmc2_logc[2]);
+  q = fma(r, q, qmc2::qmc2_logc[3]);
+  q = fma(r, q, qmc2::qmc2_logc[4]);
+  q = fma(r, q, qmc2::qmc2_logc[5]);
+  const double v = fma(r * r, q, r) + y0;
+  return ok ? v : __longlong_as_double(0x7ff8000000000000ll);
+}
+
 static __device__ __noinline__ double atan2_lib(double y, double x) { return atan2(y, x); }
 // principal log; a negative real argument carries the -i0 of F -> F - i0: arg = -pi (R:C11)
-__device__ __forceinline__ cd clog3(cd a, const double2 *__restrict__ logtab) {
+__device__ __forceinline__ cd clog3(cd a, uint32_t logtab) {
   const double arg = (a.im == 0.0 && a.re < 0.0) ? -3.14159265358979323846 : atan2_lib(a.im, a.re);
-  return cd{0.5 * fast_log(cnorm2(a), logtab), arg};
+  return cd{0.5 * fast_log_s(cnorm2(a), logtab), arg};
 }
 template <int E>
 __device__ __forceinline__ cd cpow_c(cd x) {  // x^E, E >= 0 compile time
@@ -45,25 +94,26 @@ __device__ __forceinline__ cd cpow_c(cd x) {  // x^E, E >= 0 compile time
   return (E & 1) ? h * x : h;
 }
 
-// sum of n real records c * slot[s0] * slot[s1] (byte offsets into the thread's real column)
-__device__ __forceinline__ double rsum(const uint4 *__restrict__ &rec, int n, const unsigned char *__restrict__ sl) {
+// sum of n real records c * slot[s0] * slot[s1] (rec, sl: shared addresses of the records and of the thread's column)
+__device__ __forceinline__ double rsum(uint32_t &rec, int n, uint32_t sl) {
   double acc = 0.0;
 #pragma unroll 1
   for (int i = 0; i < n; ++i) {
-    const uint4 r = *rec++;
-    acc = fma(__hiloint2double((int)r.y, (int)r.x),
-              *reinterpret_cast<const double *>(sl + r.z) * *reinterpret_cast<const double *>(sl + r.w), acc);
+    const uint4 r = lds_u32x4(rec);
+    rec += 16;
+    acc = fma(__hiloint2double((int)r.y, (int)r.x), lds_f64(sl + r.z) * lds_f64(sl + r.w), acc);
   }
   return acc;
 }
-// sum of n complex records (byte offsets into the thread's complex column, 16 bytes per entry)
-__device__ __forceinline__ cd csum(const uint4 *__restrict__ &rec, int n, const unsigned char *__restrict__ sl) {
+// sum of n complex records (16 bytes per column entry)
+__device__ __forceinline__ cd csum(uint32_t &rec, int n, uint32_t sl) {
   cd acc = cd{0.0, 0.0};
 #pragma unroll 1
   for (int i = 0; i < n; ++i) {
-    const uint4 r = *rec++;
+    const uint4 r = lds_u32x4(rec);
+    rec += 16;
     const double c = __hiloint2double((int)r.y, (int)r.x);
-    const double2 a = *reinterpret_cast<const double2 *>(sl + r.z), b = *reinterpret_cast<const double2 *>(sl + r.w);
+    const double2 a = lds_f64x2(sl + r.z), b = lds_f64x2(sl + r.w);
     acc.re = fma(c, a.x * b.x - a.y * b.y, acc.re);
     acc.im = fma(c, a.x * b.y + a.y * b.x, acc.im);
   }
@@ -74,15 +124,16 @@ template <int NDIM, int NS, int K>
 struct Ctx3 {
   double invt[NS > 0 ? NS : 1], invbeta[NS > 0 ? NS : 1];
   double cL[NS > 0 ? NS : 1][K > 1 ? K - 1 : 1];
-  const Qmc3SectorHdr *h;
-  const uint8_t *counts;            // [npoly][1 << NS]
-  const uint4 *rec_deriv, *rec_c;   // first record of F_1, first complex record
-  const uint32_t *locprog_c;        // sector-local complex products
-  const uint32_t *prog_c;           // chunk complex program
-  int nprog_c, first_prod_c, local0_c;
-  const unsigned char *slr;         // this thread's real column (bytes)
-  double2 *slc;                     // this thread's complex column: element s at slc[s * QMC3_THREADS]
-  const double2 *logtab;
+  // everything below: 32-bit shared-memory addresses
+  uint32_t counts;                  // u8 [npoly][1 << NS]
+  uint32_t rec_deriv, rec_c;        // first record of F_1, first complex record
+  uint32_t locprog_c, prog_c;       // sector-local / chunk complex products {u16 a, u16 b}
+  int nprog_c, first_prod_c, local0_c, nlocal_c;
+  uint32_t slr;                     // this thread's real column; slot s at slr + s * T * 8
+  uint32_t slc;                     // this thread's complex column; slot s at slc + s * T * 16
+  uint32_t logtab;
+  unsigned zvar[NS > 0 ? NS : 1];   // variable index of singular position k
+  int alpha[NDIM], beta[NDIM];
   double G0, L0, lambda;
   unsigned cntImF, cntReU;
 };
@@ -92,23 +143,21 @@ template <int NDIM, int L, int NS, int K>
 __device__ __noinline__ void corner3(Ctx3<NDIM, NS, K> &c, const int Z, cd &Wout, cd &Lout) {
   constexpr int NG = 1 << NS, T = QMC3_THREADS, NDERIV = NDIM + NDIM * (NDIM + 1) / 2;
   typedef Expo<NDIM, L> E;
-  const Qmc3SectorHdr *h = c.h;
   unsigned zv = 0;  // variables set to zero
 #pragma unroll
   for (int k = 0; k < NS; ++k)
-    if (Z >> k & 1) zv |= 1u << h->sing_var[k];
+    if (Z >> k & 1) zv |= 1u << c.zvar[k];
   // ---- S4: gradient and Hessian of F^ at tau -------------------------------------------------------------------
   double grad[NDIM], hess[NDIM][NDIM];
   {
-    const uint4 *rec = c.rec_deriv;
-    const uint8_t *cnt = c.counts;
+    uint32_t rec = c.rec_deriv, cnt = c.counts;
 #pragma unroll
     for (int i = 0; i < NDIM; ++i) {
       double s = 0.0;
 #pragma unroll
       for (int g = 0; g < NG; ++g) {
-        const int n = *cnt++;
-        if (g & Z) rec += n; else s += rsum(rec, n, c.slr);
+        const int n = (int)lds_u8(cnt++);
+        if (g & Z) rec += 16 * n; else s += rsum(rec, n, c.slr);
       }
       grad[i] = s;
     }
@@ -119,8 +168,8 @@ __device__ __noinline__ void corner3(Ctx3<NDIM, NS, K> &c, const int Z, cd &Wout
         double s = 0.0;
 #pragma unroll
         for (int g = 0; g < NG; ++g) {
-          const int n = *cnt++;
-          if (g & Z) rec += n; else s += rsum(rec, n, c.slr);
+          const int n = (int)lds_u8(cnt++);
+          if (g & Z) rec += 16 * n; else s += rsum(rec, n, c.slr);
         }
         hess[i][k] = s;
       }
@@ -130,9 +179,9 @@ __device__ __noinline__ void corner3(Ctx3<NDIM, NS, K> &c, const int Z, cd &Wout
 #pragma unroll
   for (int i = 0; i < NDIM; ++i) {
     const bool inZ = (zv >> i & 1u) != 0;
-    const double tau = inZ ? 0.0 : *reinterpret_cast<const double *>(c.slr + (size_t)i * T * 8);
+    const double tau = inZ ? 0.0 : lds_f64(c.slr + i * T * 8);
     rho[i] = cd{1.0, -c.lambda * (1.0 - tau) * grad[i]};
-    c.slc[i * T] = make_double2(tau, tau * rho[i].im);  // z_i = tau rho_i
+    sts_f64x2(c.slc + i * T * 16, tau, tau * rho[i].im);  // z_i = tau rho_i
 #pragma unroll
     for (int k = 0; k < NDIM; ++k) {
       const bool kinZ = (zv >> k & 1u) != 0;
@@ -175,30 +224,28 @@ __device__ __noinline__ void corner3(Ctx3<NDIM, NS, K> &c, const int Z, cd &Wout
   // ---- S5: complex slot table over z, U^(z), F^(z) -----------------------------------------------------------------
 #pragma unroll 1
   for (int i = 0; i < c.nprog_c; ++i) {
-    const uint32_t w = c.prog_c[i];
-    const double2 a = c.slc[(w & 0xffffu) * T], b = c.slc[(w >> 16) * T];
-    c.slc[(c.first_prod_c + i) * T] = make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+    const uint32_t w = lds_u32(c.prog_c + 4 * i);
+    const double2 a = lds_f64x2(c.slc + (w & 0xffffu) * (T * 16)), b = lds_f64x2(c.slc + (w >> 16) * (T * 16));
+    sts_f64x2(c.slc + (c.first_prod_c + i) * (T * 16), a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
   }
 #pragma unroll 1
-  for (int i = 0; i < h->nlocal_c; ++i) {
-    const uint32_t w = c.locprog_c[i];
-    const double2 a = c.slc[(w & 0xffffu) * T], b = c.slc[(w >> 16) * T];
-    c.slc[(c.local0_c + i) * T] = make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+  for (int i = 0; i < c.nlocal_c; ++i) {
+    const uint32_t w = lds_u32(c.locprog_c + 4 * i);
+    const double2 a = lds_f64x2(c.slc + (w & 0xffffu) * (T * 16)), b = lds_f64x2(c.slc + (w >> 16) * (T * 16));
+    sts_f64x2(c.slc + (c.local0_c + i) * (T * 16), a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
   }
   cd Uv = cd{0.0, 0.0}, Fv = cd{0.0, 0.0};
   {
-    const uint4 *rec = c.rec_c;
-    const uint8_t *cnt = c.counts + NDERIV * NG;
-    const unsigned char *slcb = reinterpret_cast<const unsigned char *>(c.slc);
+    uint32_t rec = c.rec_c, cnt = c.counts + NDERIV * NG;
 #pragma unroll
     for (int g = 0; g < NG; ++g) {
-      const int n = *cnt++;
-      if (g & Z) rec += n; else Uv = Uv + csum(rec, n, slcb);
+      const int n = (int)lds_u8(cnt++);
+      if (g & Z) rec += 16 * n; else Uv = Uv + csum(rec, n, c.slc);
     }
 #pragma unroll
     for (int g = 0; g < NG; ++g) {
-      const int n = *cnt++;
-      if (g & Z) rec += n; else Fv = Fv + csum(rec, n, slcb);
+      const int n = (int)lds_u8(cnt++);
+      if (g & Z) rec += 16 * n; else Fv = Fv + csum(rec, n, c.slc);
     }
   }
   if (Fv.im > 0.0) ++c.cntImF;
@@ -210,7 +257,7 @@ __device__ __noinline__ void corner3(Ctx3<NDIM, NS, K> &c, const int Z, cd &Wout
 #pragma unroll
   for (int j = 0; j < NDIM; ++j) {
     const bool inZ = (zv >> j & 1u) != 0;
-    const int a = h->alpha[j], b = h->beta[j];
+    const int a = c.alpha[j], b = c.beta[j];
     if (!inZ) {
       if (a < 0) den = den * rho[j];
       for (int q = 0; q < a; ++q) num = num * rho[j];
@@ -267,22 +314,27 @@ __device__ __forceinline__ void sector3(const Qmc3SectorHdr *__restrict__ h, dou
                                         unsigned &cntImF, unsigned &cntReU) {
   constexpr int K = KMAX + NS + 1, NG = 1 << NS, T = QMC3_THREADS, NPOLY = NDIM + NDIM * (NDIM + 1) / 2 + 2;
   Ctx3<NDIM, NS, K> c;
-  c.h = h;
   const unsigned char *p = reinterpret_cast<const unsigned char *>(h + 1);
-  c.counts = p;
+  c.counts = saddr(p);
   p += (NPOLY * NG + 15) & ~15;
   const uint32_t *locprog_r = reinterpret_cast<const uint32_t *>(p);
   p += (h->nlocal_r * 4 + 15) & ~15;
-  c.locprog_c = reinterpret_cast<const uint32_t *>(p);
+  c.locprog_c = saddr(p);
   p += (h->nlocal_c * 4 + 15) & ~15;
-  const uint4 *rec = reinterpret_cast<const uint4 *>(p);
-  c.rec_c = rec + h->nrec_r;
-  c.prog_c = prog_c; c.nprog_c = nprog_c; c.first_prod_c = first_prod_c; c.local0_c = local0_c;
-  c.slr = reinterpret_cast<const unsigned char *>(slr_d);
-  c.slc = slc;
-  c.logtab = logtab;
+  uint32_t rec = saddr(p);
+  c.rec_c = rec + 16u * h->nrec_r;
+  c.prog_c = saddr(prog_c); c.nprog_c = nprog_c; c.first_prod_c = first_prod_c; c.local0_c = local0_c;
+  c.nlocal_c = h->nlocal_c;
+  c.slr = saddr(slr_d);
+  c.slc = saddr(slc);
+  c.logtab = saddr(logtab);
   c.lambda = lambda;
   c.cntImF = 0; c.cntReU = 0;
+#pragma unroll
+  for (int j = 0; j < NDIM; ++j) {
+    c.alpha[j] = h->alpha[j];
+    c.beta[j] = h->beta[j];
+  }
   {  // sector-local real products
     const int nl = h->nlocal_r;
 #pragma unroll 1
@@ -297,6 +349,7 @@ __device__ __forceinline__ void sector3(const Qmc3SectorHdr *__restrict__ h, dou
 #pragma unroll
   for (int k = 0; k < NS; ++k) {
     const int j = h->sing_var[k];
+    c.zvar[k] = j;
     c.invt[k] = slr_d[(2 * NDIM + j) * T];
     c.invbeta[k] = h->invbeta[k];
     const double Lk = h->betas[k] * slr_d[(NDIM + j) * T];
@@ -317,7 +370,7 @@ __device__ __forceinline__ bool finite_hi(cd v) {
 
 // partial layout: fused [run][shift][slice][NACC][2], persec [sector row][shift][slice][NACC][2]
 template <int NDIM, int L, int KMAX>
-__global__ void __launch_bounds__(QMC3_THREADS, 1) qmc3_eval_kernel(const Qmc3Launch q) {
+__global__ void __launch_bounds__(QMC3_THREADS, (NDIM <= 4 ? 2 : 1)) qmc3_eval_kernel(const Qmc3Launch q) {
   using namespace qmc3;
   const Qmc2Launch &p = q.b;
   constexpr int NACC = QMC_MAXSING + KMAX + 1;
