@@ -3,9 +3,9 @@
 // This is the denominator-side bookkeeping of the roofline: the arithmetic the
 // product-form evaluation of Eqs. 9-12 + 14 needs, counted at the source level of the
 // scheme the kernels implement, with DFMA = 2 and DADD = DMUL = 1 and fixed costs for the library sequences
-// (fast paths of the CUDA 12.9 sm_100a FP64 routines, counted in SASS):
-//   log    : 17 DFMA + 7 DADD + 3 DMUL = 44      reciprocal: 5 DFMA = 10      division: 7 DFMA + 2 DMUL = 16
-//   atan2  : division + 19 DFMA polynomial + fix-ups = 60
+// (fast paths of the CUDA 12.9 sm_100a FP64 routines, counted in SASS; the kernels' own routines in brackets):
+//   division: 7 DFMA + 2 DMUL = 16      atan2: division + 19 DFMA polynomial + fix-ups = 60
+//   [table logarithm: 7 DFMA + DMUL + DADD = 16]      [Newton reciprocal: 4 DFMA = 8]
 // Integer work (lattice index arithmetic, table decoding) and comparisons count as zero.  The count is
 // cross-checked against Nsight Compute's executed DFMA/DADD/DMUL thread-instruction counters (profiles/).
 #include <algorithm>
@@ -34,8 +34,9 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
   const int sb = sector_begin, se = sector_end > 0 ? sector_end : nsec;
   if (sb < 0 || se > nsec || sb >= se) return QMC_EINVAL;
   const bool cplx = t->lambda > 0.0;
-  // S1-S3, once per (point, shift): u = r/N, y = u + Delta (wrap), t = y^2 (3 - 2y), w *= 6 y (1 - y), ln t, 1/t
-  const double per_point = n * (F_DIV + 2.0 + 4.0 + 4.0 + F_LOG + F_RCP);
+  // S1-S3, once per (point, shift): u = r/N (IEEE division), y = u + Delta (wrap), t = y^2 (3 - 2y), w *= 6 y (1 - y),
+  // ln t (table logarithm, 16), 1/t (Newton reciprocal, 8)
+  const double per_point = n * (F_DIV + 2.0 + 4.0 + 4.0 + 16.0 + 8.0);
   double per_sectors = 0.0;
   int64_t ncorners = 0;
   const int eU = std::abs(t->aU0), eF = std::abs(t->aF0);
@@ -83,71 +84,75 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
         }
       f += 2.0 * K;  // weight and accumulate
     } else {
-      const double cs = 2.0;  // a real-by-complex scaling
+      // version-3 scheme (qmc_kernels3.cuh): real record 3, complex record 10 (complex product 6 + two FMAs)
+      auto pow_muls = [](int e) {
+        int c = 0;
+        for (int q = e; q > 1; q >>= 1) c += 1 + (q & 1);
+        return (double)c;
+      };
+      const double F_LOG2 = 16.0, F_CLOG3 = 3.0 + F_LOG2 + 1.0 + F_ATAN2;
+      int pos_of[QMC_MAXDIM], kk = 0;
+      for (int j = 0; j < n; ++j) pos_of[j] = (s.alpha[j] == -1) ? kk++ : -1;
+      int nprod_c = 0;  // complex product slots of the sector's chunk
+      for (size_t ci = 0; ci < t->chunks3.size(); ++ci)
+        if (si >= t->chunks3[ci].sec_begin && si < t->chunks3[ci].sec_end) nprod_c = t->chunk3_nslots_c[ci] - (n + 1);
+      int nL0 = 0, nbeta = 0;
+      for (int j = 0; j < n; ++j) {
+        if (s.alpha[j] != -1 && s.beta[j]) ++nL0;
+        if (s.beta[j]) ++nbeta;
+      }
+      f = 3.0 * (1 + nL0);
+      for (int j = 0; j < n; ++j)
+        if (s.alpha[j] == -1) f += 1.0 + 2.0 * std::max(0, K - 2);
       for (int Z = 0; Z < nc; ++Z) {
-        // surviving monomials: those free of the variables in Z
-        auto in_Z = [&](int j) {  // j original index; singular variables are numbered in increasing original index
-          if (s.alpha[j] != -1) return false;
-          int b = 0;
-          for (int q = 0; q < j; ++q)
-            if (s.alpha[q] == -1) ++b;
-          return (Z >> b & 1) != 0;
-        };
+        auto in_Z = [&](int j) { return pos_of[j] >= 0 && (Z >> pos_of[j] & 1); };
         int nfree = 0;
         for (int j = 0; j < n; ++j)
           if (!in_Z(j)) ++nfree;
-        // gradient + Hessian of F^ at the real corner point
+        // derivative polynomials: a monomial of d_i F (d_i d_k F) survives if what is left of it is free of Z variables
         for (const QmcMono &m : s.F) {
-          int zdeg = 0;
-          for (int j = 0; j < n; ++j)
-            if (in_Z(j)) zdeg += m.e[j];
-          if (zdeg > 1) continue;
-          f += degree(m, n) - zdeg;  // the monomial value
-          if (zdeg == 1) {
-            f += 1.0;  // contributes to one gradient component
-            continue;
-          }
           for (int i = 0; i < n; ++i) {
-            if (in_Z(i) || !m.e[i]) continue;
-            f += 3.0;  // e_i * v / t_i, add
+            if (!m.e[i]) continue;
             for (int k = i; k < n; ++k) {
-              if (in_Z(k)) continue;
-              int ek = m.e[k] - (k == i ? 1 : 0);
-              if (ek > 0) f += 3.0;
+              if (k == i ? m.e[i] < 2 : !m.e[k]) continue;
+              bool dead = false;
+              for (int j = 0; j < n; ++j)
+                if (in_Z(j) && m.e[j] - (j == i) - (j == k) > 0) dead = true;
+              if (!dead) f += 3.0;
             }
+            bool dead = false;
+            for (int j = 0; j < n; ++j)
+              if (in_Z(j) && m.e[j] - (j == i) > 0) dead = true;
+            if (!dead) f += 3.0;
           }
         }
-        // rho, z, Jacobian entries
-        f += n * 4.0 + (double)nfree * nfree * 3.0 + nfree * 3.0;
-        // LU of the nfree x nfree complex block
-        for (int col = 0; col < nfree; ++col) {
-          f += F_CMUL;  // det *= pivot
-          int rem = nfree - col - 1;
-          if (rem > 0) f += F_CINV + rem * (F_CMUL + rem * (F_CMUL + F_CADD)) + rem * 6.0 /* pivot compares */;
+        f += n * 5.0 + (double)nfree * nfree * 3.0 + nfree * 3.0;  // rho, z, Jacobian entries
+        for (int col = 0; col < n; ++col) {                         // LU of the n x n complex matrix
+          f += F_CMUL;
+          const int rem = n - col - 1;
+          if (rem > 0) f += F_CINV + rem * (F_CMUL + rem * (F_CMUL + F_CADD)) + rem * 6.0;
         }
-        // complex U^(z), F^(z)
+        f += 6.0 * nprod_c;                                         // complex slot program
         for (int which = 0; which < 2; ++which)
           for (const QmcMono &m : (which ? s.F : s.U)) {
             bool dead = false;
             for (int j = 0; j < n; ++j)
               if (in_Z(j) && m.e[j]) dead = true;
-            if (dead) continue;
-            int d = degree(m, n);
-            f += (d > 0 ? cs + (d - 1) * F_CMUL : 0.0) + F_CADD;
+            if (!dead) f += 10.0;
           }
-        // G_Z, Lambda_Z
-        f += F_CMUL;                                  // G0 det
-        for (int j = 0; j < n; ++j) {
+        f += 2.0;  // G0 det
+        for (int j = 0; j < n; ++j)
           if (!in_Z(j)) f += std::abs(s.alpha[j]) * F_CMUL;
-          if (s.beta[j]) f += F_CLOG + cs + F_CADD;
-        }
-        f += (eU + eF) * F_CMUL + F_CINV + F_CMUL;    // powers, W = num / den
-        f += 2.0 * F_CLOG + 2.0 * cs + F_CADD + 1.0;  // Lambda
-        f += (K - 1) * (F_CMUL + cs);                 // series
+        f += (pow_muls(eU) + (eU ? 1 : 0) + pow_muls(eF) + (eF ? 1 : 0)) * F_CMUL + F_CINV + F_CMUL;
+        f += (2 + nbeta) * (F_CLOG3 + 4.0) + 1.0;                   // Lambda
+        f += (t->kmax + __builtin_popcount(Z)) * 8.0;               // series
       }
-      f += (nc - 1) * (K - 1) * (F_CADD + cs);                                                    // d = (a - b)/t
-      f += (nc - 1) * (cs + (K - 1) * (cs + F_CADD) + 0.5 * (K - 1) * (K - 2) * (cs + F_CADD));   // out
-      f += 4.0 * K;  // weight and accumulate
+      for (int l = 0; l < ns; ++l)
+        for (int Z = 0; Z < (1 << l); ++Z) {
+          const int len = ns - l + t->kmax + __builtin_popcount(Z) + 1;
+          f += 4.0 * (len - 1) + 2.0 + 2.0 * len * (len - 1);
+        }
+      f += 4.0 * K;
     }
     per_sectors += f;
     ncorners += nc;
