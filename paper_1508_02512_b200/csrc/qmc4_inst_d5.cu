@@ -1,0 +1,2 @@
+#include "qmc_inst4.cuh"
+QMC4_DEFINE_DIM(5)

@@ -154,7 +154,7 @@ uint64_t splitmix64(uint64_t &state) {
 uint64_t mulmod(uint64_t a, uint64_t b, uint64_t n) { return (uint64_t)(((unsigned __int128)a * b) % n); }
 
 struct DevLayout {
-  size_t image, secoff, image2, secoff2, image3, secoff3, logtab, work, shifts, counters, out, stat, partial, p2z, p2partial, total;
+  size_t image, secoff, image2, secoff2, image3, secoff3, logtab, logtab4, work, shifts, counters, out, stat, partial, p2z, p2partial, total;
 };
 
 DevLayout layout(const qmc_tables *t, int m) {
@@ -168,6 +168,7 @@ DevLayout layout(const qmc_tables *t, int m) {
   L.image3 = o; o += align256(t->image3.size());
   L.secoff3 = o; o += align256((nsec + 1) * 4);
   L.logtab = o; o += align256(sizeof t->logtab);
+  L.logtab4 = o; o += align256(sizeof t->logtab4);
   L.work = o; o += align256((size_t)QMC2_MAX_WORK * sizeof(Qmc2Work));
   L.shifts = o; o += align256((size_t)m * QMC_MAXDIM * 8);
   L.counters = o; o += 256;
@@ -367,6 +368,148 @@ int launch_v2(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
   return QMC_OK;
 }
 
+// ---- version-4 launch (real path): one launch per run of sectors, tables in the kernel parameters ------------------
+// Runs = maximal pieces of a chunk whose tables fit QMC4_TAB_WORDS (and, in per-sector mode, whose accumulators fit
+// the shared memory).  grid = (point slices, shift vectors); slices in proportion to the modelled cost of the run.
+// The launches are independent (disjoint rows of the partial buffer): they are spread over side streams forked from
+// and joined back into the caller's stream, so that the tail of one launch overlaps the next ones.
+int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t st, uint64_t N, int m, int sb, int se,
+              bool persec, uint64_t ibeg, uint64_t istep, uint64_t icount, const uint64_t *z, int sms, int smem_optin,
+              int *gx_out, int *rows_out, int *launches_out, size_t *h2d, cudaError_t *ce_out) {
+  const int n = t->n, nacc = QMC_MAXSING + t->kmax + 1, T = QMC2_THREADS;
+  int max_nslots = 0;
+  for (const Qmc2Chunk &c : t->chunks)
+    if (c.sec_end > sb && c.sec_begin < se) max_nslots = std::max(max_nslots, c.nslots + c.max_local);
+  const size_t budget = (size_t)smem_optin - 1024;
+  const size_t fixed = (size_t)QMC4_LOG_ENTRIES * QMC4_LOG_COPIES * 16 + (((size_t)m * n * 8 + 15) & ~(size_t)15) + (T / 32) * 8 +
+                       (size_t)max_nslots * T * 8;
+  const size_t accbytes = persec ? (size_t)nacc * T * 8 : 0;
+  if (fixed + accbytes > budget) return QMC_ENOMEM;
+  struct Run { int chunk, a, b; double cost; };
+  std::vector<Run> runs;
+  double total_cost = 0.0;
+  int max_nsec = 0;
+  for (size_t ci = 0; ci < t->chunks.size(); ++ci) {
+    const Qmc2Chunk &c = t->chunks[ci];
+    int a = std::max(sb, c.sec_begin);
+    const int e = std::min(se, c.sec_end);
+    const size_t prog_words = t->prog4[ci].size() / 4;
+    while (a < e) {
+      int b = a;
+      while (b < e) {
+        const size_t words = prog_words + (t->secoff4[b + 1] - t->secoff4[a]);
+        if (words > QMC4_TAB_WORDS || b + 1 - a > QMC4_MAX_SEC || fixed + accbytes * (b + 1 - a) > budget) break;
+        ++b;
+      }
+      if (b == a) return QMC_ENOMEM;
+      Run r = {(int)ci, a, b, 0.0};
+      for (int s = a; s < b; ++s) r.cost += t->sec_cost[s];
+      total_cost += r.cost;
+      max_nsec = std::max(max_nsec, b - a);
+      runs.push_back(r);
+      a = b;
+    }
+  }
+  const int nitems = (int)runs.size();
+  const size_t smem = fixed + accbytes * max_nsec;
+  int bps = 0;
+  CUDA_OK(qmc4_kernel_prepare(n, t->L, t->kmax, smem, &bps));
+  if (bps < 1) return QMC_ECUDA;
+  int waves = 16;
+  if (const char *e = std::getenv("QMC2_WAVES")) waves = std::max(1, std::atoi(e));
+  const long long max_slices_pts = std::max<long long>(1, (long long)((icount + T - 1) / T));
+  const double nblocks_target = (double)waves * sms * bps / (double)m;  // a block serves ONE shift vector
+  std::vector<int> nsl(nitems);
+  int max_slices = 1;
+  for (int i = 0; i < nitems; ++i) {
+    long long ns = (long long)(nblocks_target * runs[i].cost / total_cost + 0.5);
+    ns = std::max<long long>(1, std::min<long long>({ns, (long long)QMC_MAX_BLOCKS, max_slices_pts}));
+    nsl[i] = (int)ns;
+    max_slices = std::max(max_slices, (int)ns);
+  }
+  const int rows_partial = persec ? (se - sb) : nitems;
+  CUDA_OK(cudaMemsetAsync(ws + L.partial, 0, (size_t)rows_partial * m * max_slices * nacc * 8, st));
+  // side streams
+  int nstreams = 4;
+  if (const char *e = std::getenv("QMC4_STREAMS")) nstreams = std::max(0, std::min(8, std::atoi(e)));
+  nstreams = std::min(nstreams, nitems);
+  if (nstreams < 2) nstreams = 0;
+  for (int q = 0; q < nstreams; ++q)
+    if (!t->side_streams[q]) {
+      CUDA_OK(cudaStreamCreateWithFlags(reinterpret_cast<cudaStream_t *>(&t->side_streams[q]), cudaStreamNonBlocking));
+    }
+  for (int q = 0; q < nstreams + 1; ++q)
+    if (!t->side_events[q]) {
+      CUDA_OK(cudaEventCreateWithFlags(reinterpret_cast<cudaEvent_t *>(&t->side_events[q]), cudaEventDisableTiming));
+    }
+  static thread_local Qmc4Launch p;  // 30 KB: not on the stack
+  std::memset(&p, 0, offsetof(Qmc4Launch, tab));
+  p.logtab = reinterpret_cast<const double *>(ws + L.logtab4);
+  p.shifts = reinterpret_cast<const double *>(ws + L.shifts);
+  p.partial = reinterpret_cast<double *>(ws + L.partial);
+  p.counters = reinterpret_cast<unsigned long long *>(ws + L.counters);
+  p.N = (uint32_t)N;
+  p.count = (uint32_t)icount;
+  for (int j = 0; j < n; ++j) {
+    p.zeff[j] = (uint32_t)mulmod(istep % N, z[j], N);
+    p.off[j] = (uint32_t)mulmod(ibeg, z[j], N);
+  }
+  p.m = m;
+  p.transform = t->transform;
+  p.persec = persec ? 1 : 0;
+  p.max_slices = max_slices;
+  p.max_nslots = (uint32_t)max_nslots;
+  cudaEventRecord(static_cast<cudaEvent_t>(t->ev0), st);
+  if (nstreams) {
+    cudaEventRecord(static_cast<cudaEvent_t>(t->side_events[nstreams]), st);
+    for (int q = 0; q < nstreams; ++q)
+      cudaStreamWaitEvent(static_cast<cudaStream_t>(t->side_streams[q]), static_cast<cudaEvent_t>(t->side_events[nstreams]), 0);
+  }
+  cudaError_t ce = cudaSuccess;
+  for (int i = 0; i < nitems && ce == cudaSuccess; ++i) {
+    const Run &r = runs[i];
+    const Qmc2Chunk &c = t->chunks[r.chunk];
+    const std::vector<uint32_t> &pg = t->prog4[r.chunk];
+    p.nsec = r.b - r.a;
+    p.out_row = persec ? r.a - sb : i;
+    p.count_boundary = i == 0 ? 1 : 0;
+    p.nslices = nsl[i];
+    p.nprog = (uint32_t)(c.nslots - (3 * n + 1));
+    p.prog_word = 0;
+    p.sec_word = (uint32_t)(pg.size() / 4);
+    p.first_prod_off = (uint32_t)(3 * n + 1) * T * 8u;
+    p.local0_off = (uint32_t)c.nslots * T * 8u;
+    uint32_t *tw = reinterpret_cast<uint32_t *>(p.tab);
+    std::memcpy(tw, pg.data(), pg.size() * 4);
+    const size_t w0 = t->secoff4[r.a], w1 = t->secoff4[r.b];
+    std::memcpy(tw + pg.size(), t->tab4.data() + w0 * 4, (w1 - w0) * 16);
+    {  // evaluation order: by number of singular variables (stable)
+      int k = 0;
+      for (int ns = 0; ns <= QMC_MAXSING; ++ns)
+        for (int s = r.a; s < r.b; ++s)
+          if (t->sectors[s].nsing == ns) {
+            p.secw[k] = (uint16_t)(p.sec_word + (t->secoff4[s] - w0));
+            p.secrow[k] = (uint16_t)(s - r.a);
+            ++k;
+          }
+    }
+    cudaStream_t ls = nstreams ? static_cast<cudaStream_t>(t->side_streams[i % nstreams]) : st;
+    ce = qmc4_kernel_launch(n, t->L, t->kmax, dim3((unsigned)nsl[i], (unsigned)m), smem, ls, p);
+    *h2d += offsetof(Qmc4Launch, tab) + pg.size() * 4 + (w1 - w0) * 16;  // the tables travel with the launch
+  }
+  if (nstreams)
+    for (int q = 0; q < nstreams; ++q) {
+      cudaEventRecord(static_cast<cudaEvent_t>(t->side_events[q]), static_cast<cudaStream_t>(t->side_streams[q]));
+      cudaStreamWaitEvent(st, static_cast<cudaEvent_t>(t->side_events[q]), 0);
+    }
+  cudaEventRecord(static_cast<cudaEvent_t>(t->evm), st);
+  *ce_out = ce;
+  *gx_out = max_slices;
+  *rows_out = nitems;
+  *launches_out = nitems;
+  return QMC_OK;
+}
+
 // ---- version-3 launch (complex path): same geometry as version 2, two slot tables per thread ------------------------------------
 int launch_v3(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t st, uint64_t N, int m, int sb, int se,
               bool persec, uint64_t ibeg, uint64_t istep, uint64_t icount, const uint64_t *z, int sms, int smem_optin,
@@ -523,6 +666,12 @@ void qmc_tables_free(qmc_tables *t) {
     cudaEventDestroy(static_cast<cudaEvent_t>(t->ev0));
     cudaEventDestroy(static_cast<cudaEvent_t>(t->ev1));
     cudaEventDestroy(static_cast<cudaEvent_t>(t->evm));
+  }
+  if (t) {
+    for (void *&q : t->side_streams)
+      if (q) cudaStreamDestroy(static_cast<cudaStream_t>(q));
+    for (void *&q : t->side_events)
+      if (q) cudaEventDestroy(static_cast<cudaEvent_t>(q));
   }
   delete t;
 }
@@ -712,6 +861,8 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
   cudaError_t ce = cudaSuccess;
   double *partial = reinterpret_cast<double *>(ws + L.partial);
   const bool use_v2 = !cplx && !t->image2.empty() && qmc2_kernel_available(n, t->L, t->kmax) && !std::getenv("QMC_FORCE_V1");
+  const bool use_v4 = use_v2 && !t->tab4.empty() && qmc4_kernel_available(n, t->L, t->kmax) && !std::getenv("QMC_FORCE_V2");
+  int eval_launches = 1;
   // ---- uploads common to both kernels (skipped when resident) ------------------------------------------------
   if (!image_resident) {
     h2d += t->image.size() + t->secoff.size() * 4;
@@ -728,6 +879,8 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
       CUDA_OK(cudaMemcpyAsync(ws + L.image2, t->image2.data(), t->image2.size(), cudaMemcpyHostToDevice, st));
       CUDA_OK(cudaMemcpyAsync(ws + L.secoff2, t->secoff2.data(), t->secoff2.size() * 4, cudaMemcpyHostToDevice, st));
       CUDA_OK(cudaMemcpyAsync(ws + L.logtab, t->logtab, sizeof t->logtab, cudaMemcpyHostToDevice, st));
+      CUDA_OK(cudaMemcpyAsync(ws + L.logtab4, t->logtab4, sizeof t->logtab4, cudaMemcpyHostToDevice, st));
+      h2d += sizeof t->logtab4;
     }
     t->resident_ws = dev_workspace;
     t->resident_m = 0;
@@ -743,6 +896,9 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
                       !std::getenv("QMC_FORCE_V1");
   if (use_v3) {
     int rc = launch_v3(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, &gx, &nchunks, &h2d, &ce);
+    if (rc != QMC_OK) return rc;
+  } else if (use_v4) {
+    int rc = launch_v4(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, &gx, &nchunks, &eval_launches, &h2d, &ce);
     if (rc != QMC_OK) return rc;
   } else if (use_v2) {
     int rc = launch_v2(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, &gx, &nchunks, &h2d, &ce);
@@ -842,6 +998,7 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
   t->last.mode = mode;
   t->last.nrows = nrows;
   t->last.h2d = h2d;
+  t->last.launches = eval_launches + 2;
   return QMC_OK;
 }
 
@@ -876,7 +1033,7 @@ int qmc_result_fetch(const qmc_tables *tc, void *cuda_stream, void *dev_workspac
   out->eval_kernel_ms = ms_eval;
   out->h2d_bytes = (int64_t)t->last.h2d;
   out->d2h_bytes = (int64_t)(ncopy * 8 + 32);
-  out->kernel_launches = 3;
+  out->kernel_launches = t->last.launches;
   out->mode_used = t->last.mode;
   for (int q = 0; q < 4; ++q) out->counters[q] = (int64_t)hc[q];
   const double *h = t->stat_host.data();

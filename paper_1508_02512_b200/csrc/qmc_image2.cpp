@@ -53,8 +53,43 @@ static void build_logtab(double *tab) {
   }
 }
 
+// the same for version 4: 64 intervals
+static void build_logtab4(double *tab) {
+  for (int i = 0; i < 64; ++i) {
+    const uint64_t lo = ((uint64_t)(0x3fe60000u + ((uint32_t)i << 14))) << 32, hi = lo + ((uint64_t)0x4000 << 32);
+    double zl, zh;
+    std::memcpy(&zl, &lo, 8);
+    std::memcpy(&zh, &hi, 8);
+    const double invc = (double)(1.0L / (0.5L * ((long double)zl + (long double)zh)));
+    tab[2 * i] = invc;
+    tab[2 * i + 1] = (double)(-logl((long double)invc));
+  }
+}
+
+namespace {
+void put32(std::vector<uint32_t> &v, uint32_t x) { v.push_back(x); }
+void putf64(std::vector<uint32_t> &v, double d) {
+  uint64_t b;
+  std::memcpy(&b, &d, 8);
+  v.push_back((uint32_t)b);
+  v.push_back((uint32_t)(b >> 32));
+}
+void pad4(std::vector<uint32_t> &v) {
+  while (v.size() % 4) v.push_back(0);
+}
+void put_rec(std::vector<uint32_t> &v, const Qmc2Rec &r) {
+  putf64(v, r.c);
+  v.push_back(r.s0);
+  v.push_back(r.s1);
+}
+}  // namespace
+
 int qmc_build_image2(qmc_tables *t) {
   build_logtab(t->logtab);
+  build_logtab4(t->logtab4);
+  t->tab4.clear();
+  t->secoff4.clear();
+  t->prog4.clear();
   t->image2.clear();
   t->secoff2.clear();
   t->chunks.clear();
@@ -115,6 +150,13 @@ int qmc_build_image2(qmc_tables *t) {
     }
     while (t->image2.size() % 16) t->image2.push_back(0);
     ch.prog_bytes = (uint32_t)t->image2.size() - ch.prog_off;
+    std::vector<uint32_t> prog4;
+    for (auto &pr : pl.prog) {
+      put32(prog4, (uint32_t)pr.first * QMC2_THREADS * 8u);
+      put32(prog4, (uint32_t)pr.second * QMC2_THREADS * 8u);
+    }
+    pad4(prog4);
+    const size_t tab4_mark = t->tab4.size();
     const uint32_t ONE = (uint32_t)(3 * n) * QMC2_THREADS * 8u;
     size_t mi = 0;  // index into pl.mono, same order as collect()
     auto rec_of = [&](double c, const Factors &f) {
@@ -200,9 +242,53 @@ int qmc_build_image2(qmc_tables *t) {
       while (t->image2.size() % 16) t->image2.push_back(0);
       for (const Qmc2Rec &r : recs) put(t->image2, r);
       t->secend2[si] = (uint32_t)t->image2.size();
+      {  // version-4 block of the same sector (layout: qmc_launch.h)
+        std::vector<uint32_t> &v = t->tab4;
+        if ((int)t->secoff4.size() <= si) t->secoff4.resize(si + 1, 0);
+        t->secoff4[si] = (uint32_t)(v.size() / 4);
+        const size_t b0 = v.size();
+        const int nc = 1 << s.nsing;
+        const uint32_t nlw = (uint32_t)((local.size() + 1) / 2);
+        put32(v, (uint32_t)s.nsing | ((uint32_t)h.nL0 << 8) | ((uint32_t)local.size() << 16));
+        put32(v, 0);         // size of the block in words (patched below)
+        put32(v, 9 + nlw);   // first record
+        put32(v, 0);
+        for (int k = 0; k < QMC_MAXSING; ++k) put32(v, (uint32_t)h.sing_ln[k] * 8u);
+        for (int k = 0; k < QMC_MAXSING; ++k) put32(v, (uint32_t)h.sing_inv[k] * 8u);
+        for (int k = 0; k < QMC_MAXSING; ++k) putf64(v, h.invbeta[k]);
+        for (int k = 0; k < QMC_MAXSING; ++k) putf64(v, h.beta[k]);
+        uint8_t extraU[16] = {0}, extraF[16] = {0};
+        for (int g = 0; g < nc; ++g) {
+          extraU[g] = h.cntU[g] ? (uint8_t)(h.cntU[g] - 1) : 0;
+          extraF[g] = h.cntF[g] ? (uint8_t)(h.cntF[g] - 1) : 0;
+        }
+        for (int q = 0; q < 4; ++q) put32(v, extraU[4 * q] | (extraU[4 * q + 1] << 8) | (extraU[4 * q + 2] << 16) | ((uint32_t)extraU[4 * q + 3] << 24));
+        for (int q = 0; q < 4; ++q) put32(v, extraF[4 * q] | (extraF[4 * q + 1] << 8) | (extraF[4 * q + 2] << 16) | ((uint32_t)extraF[4 * q + 3] << 24));
+        for (auto &pr : local) {
+          put32(v, (uint32_t)pr.first * QMC2_THREADS * 8u);
+          put32(v, (uint32_t)pr.second * QMC2_THREADS * 8u);
+        }
+        pad4(v);
+        size_t ri = 0;
+        put_rec(v, recs[ri++]);                                  // G0
+        for (int q = 0; q < h.nL0; ++q) put_rec(v, recs[ri++]);  // L0
+        const Qmc2Rec empty = {0.0, ONE, ONE};
+        std::vector<Qmc2Rec> extra;
+        for (int which = 0; which < 2; ++which)
+          for (int g = 0; g < nc; ++g) {
+            const int cnt = (which ? h.cntF : h.cntU)[g];
+            put_rec(v, cnt ? recs[ri] : empty);
+            for (int q = 1; q < cnt; ++q) extra.push_back(recs[ri + q]);
+            ri += cnt;
+          }
+        for (const Qmc2Rec &r : extra) put_rec(v, r);
+        put_rec(v, empty);  // sentinel: the kernel requests one record past the last extra one
+        v[b0 + 1] = (uint32_t)((v.size() - b0) / 4);
+      }
     }
     if (too_many_locals) {  // split the range in two and plan again
       t->image2.resize(ch.prog_off);
+      t->tab4.resize(tab4_mark);
       (void)image_mark;
       if (s1 - s0 == 1) return QMC_EUNSUPPORTED;
       const int mid = (s0 + s1) / 2;
@@ -212,7 +298,10 @@ int qmc_build_image2(qmc_tables *t) {
       continue;
     }
     t->chunks.push_back(ch);
+    t->prog4.push_back(prog4);
   }
   t->secoff2[nsec] = (uint32_t)t->image2.size();
+  t->secoff4.resize(nsec + 1, 0);
+  t->secoff4[nsec] = (uint32_t)(t->tab4.size() / 4);
   return QMC_OK;
 }

@@ -1,0 +1,344 @@
+// Evaluation kernel, version 4 (real / Euclidean path), sm_100a.  Steps S1-S7 of DESIGN.md.
+//
+// Same arithmetic scheme as version 2 (qmc_kernels2.cuh: per-point slot table in shared memory, a monomial = one record
+// c * slot * slot, group partial sums -> subset sums -> all corners of the subtraction from one pass, one reciprocal and
+// one table logarithm per corner, product form folded one singular variable at a time) with a different home for the
+// tables: the chunk's slot program and the sector tables are part of the KERNEL PARAMETER BLOCK (constant bank 0, layout
+// in qmc_launch.h).  Measured reasons (profiles/r01g_*): in version 2 the record loops were bound by the shared-memory
+// data pipe (6 wavefronts per record: 2 for the 16-byte broadcast of the record, 2 + 2 for the slot operands) and by
+// the exposed LDS -> LDS -> DMUL -> DFMA latency chain of one short loop per group, and cost 11 instructions per record.
+// Here a record is 2 uniform loads (LDCU.64), 2 LDS [R + UR], DMUL, DFMA (the coefficient is a uniform-register
+// operand), trip counts are uniform so ptxas unrolls and batches the loads, and the FIRST record of every group sits
+// in a dense array with a compile-time destination register: 2^nsing independent load/multiply chains in one basic
+// block.  The logarithm table is 64 entries x 8 interleaved copies (lane & 7 picks the copy): every lookup is a
+// conflict-free LDS.128 (4 wavefronts instead of the ~10 measured with one copy).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "qmc_kernels2.cuh"  // fast_rcp, ipow_c, Expo, Ctx2, Fold2, finite_hi
+#include "qmc_launch.h"
+
+namespace qmc4 {
+
+using qmc2::Ctx2;
+using qmc2::Expo;
+using qmc2::fast_rcp;
+using qmc2::finite_hi;
+using qmc2::Fold2;
+using qmc2::ipow_c;
+
+// ln x, absolute error ~1e-16: x = 2^e * z, z in [0.6875, 1.375), 64 sub-intervals with centre c_i;
+// tab[i] = {1/c_i rounded, -ln(that) in extended precision}; r = z/c_i - 1 (one FMA, |r| < 2^-7), degree-7 log1p.
+// `tabq` = this lane's copy of the table: entry i at tabq[i * QMC4_LOG_COPIES].
+__constant__ double qmc4_logc[7] = {0.693147180559945309417, 1.0 / 7.0, -1.0 / 6.0, 0.2, -0.25, 1.0 / 3.0, -0.5};
+__device__ __forceinline__ double fast_log(double x, const double2 *__restrict__ tabq) {
+  const int hi = __double2hiint(x), lo = __double2loint(x);
+  const bool ok = (unsigned)(hi - 0x00100000) < 0x7fe00000u;  // positive, normal
+  const int tmp = hi - 0x3fe60000;
+  const int e = tmp >> 20;
+  const double2 T = *reinterpret_cast<const double2 *>(reinterpret_cast<const unsigned char *>(tabq) +
+                                                      ((tmp >> (14 - 7)) & ((QMC4_LOG_ENTRIES - 1) << 7)));
+  const double z = __hiloint2double(hi - (tmp & 0xfff00000), lo);
+  const double r = fma(z, T.x, -1.0);
+  const double y0 = fma((double)e, qmc4_logc[0], T.y);
+  double q = fma(r, qmc4_logc[1], qmc4_logc[2]);
+  q = fma(r, q, qmc4_logc[3]);
+  q = fma(r, q, qmc4_logc[4]);
+  q = fma(r, q, qmc4_logc[5]);
+  q = fma(r, q, qmc4_logc[6]);
+  const double v = fma(r * r, q, r) + y0;
+  return ok ? v : __longlong_as_double(0x7ff8000000000000ll);
+}
+static_assert(QMC4_LOG_COPIES * 16 == 1 << 7, "fast_log index arithmetic assumes 128 bytes per table entry row");
+
+__device__ __forceinline__ double slot_at(const unsigned char *__restrict__ sl, uint32_t off) {
+  return *reinterpret_cast<const double *>(sl + off);
+}
+// value of one record: c * slot[off0] * slot[off1]
+__device__ __forceinline__ double rec_val(const uint4 r, const unsigned char *__restrict__ sl) {
+  return __hiloint2double((int)r.y, (int)r.x) * (slot_at(sl, r.z) * slot_at(sl, r.w));
+}
+__device__ __forceinline__ double rec_fma(const uint4 r, const unsigned char *__restrict__ sl, double acc) {
+  return fma(__hiloint2double((int)r.y, (int)r.x), slot_at(sl, r.z) * slot_at(sl, r.w), acc);
+}
+__device__ __forceinline__ double u2d(uint32_t lo, uint32_t hi) { return __hiloint2double((int)hi, (int)lo); }
+
+// one sector at one point: out[i] = coefficient of eps^(i - NS) of the subtracted integrand (without the weight w).
+// `o` = word offset of the sector block in p.tab (uniform).
+template <int NDIM, int L, int NS, int KMAX>
+__device__ __forceinline__ void sector4(const Qmc4Launch &p, const uint32_t o, unsigned char *__restrict__ sl,
+                                        const double2 *__restrict__ tabq, double (&out)[KMAX + NS + 1]) {
+  constexpr int K = KMAX + NS + 1, NC = 1 << NS, FULL = NC - 1, T = QMC2_THREADS;
+  typedef Expo<NDIM, L> E;
+  const uint4 h0 = p.tab[o];
+  const uint32_t nL0 = (h0.x >> 8) & 255u, nlocal = (h0.x >> 16) & 255u;
+  {  // sector-local products: slot[local0 + i] = slot[a] * slot[b]
+    const uint32_t lw = o + 9;
+#pragma unroll 1
+    for (uint32_t i = 0; i < nlocal; i += 2) {
+      const uint4 pw = p.tab[lw + (i >> 1)];
+      *reinterpret_cast<double *>(sl + p.local0_off + i * (T * 8)) = slot_at(sl, pw.x) * slot_at(sl, pw.y);
+      if (i + 1 < nlocal) *reinterpret_cast<double *>(sl + p.local0_off + (i + 1) * (T * 8)) = slot_at(sl, pw.z) * slot_at(sl, pw.w);
+    }
+  }
+  uint32_t rw = o + h0.z;  // first record
+  const double G0 = rec_val(p.tab[rw], sl);
+  ++rw;
+  double L0 = 0.0;
+#pragma unroll 2
+  for (uint32_t i = 0; i < nL0; ++i) L0 = rec_fma(p.tab[rw + i], sl, L0);
+  rw += nL0;
+  Ctx2<NS, K> c;
+  {
+    // first record of every group (dense, compile-time destination), then the extra records group by group;
+    // subset sums: P[X] = value with the singular variables outside X set to zero
+    double PU[NC], PF[NC];
+#pragma unroll
+    for (int g = 0; g < NC; ++g) PU[g] = rec_val(p.tab[rw + g], sl);
+#pragma unroll
+    for (int g = 0; g < NC; ++g) PF[g] = rec_val(p.tab[rw + NC + g], sl);
+    rw += 2 * NC;
+    const uint4 cu = p.tab[o + 7], cf = p.tab[o + 8];
+    const uint32_t cuw[4] = {cu.x, cu.y, cu.z, cu.w}, cfw[4] = {cf.x, cf.y, cf.z, cf.w};
+    // extra records: one stream across all groups, software-pipelined by one record -- the slot operands of the NEXT
+    // record are requested before the current one is accumulated, also across group boundaries (the block ends with a
+    // harmless sentinel record), so the LDCU -> LDS -> DMUL -> DFMA chain is not exposed once per group
+    uint4 rr = p.tab[rw];
+    double ra = slot_at(sl, rr.z), rb = slot_at(sl, rr.w);
+#pragma unroll
+    for (int g = 0; g < 2 * NC; ++g) {
+      const int gg = g & (NC - 1);
+      const uint32_t cnt = ((g < NC ? cuw[gg >> 2] : cfw[gg >> 2]) >> (8 * (gg & 3))) & 255u;
+      double accg = g < NC ? PU[gg] : PF[gg];
+#pragma unroll 1
+      for (uint32_t i = 0; i < cnt; ++i) {
+        const double v = ra * rb, cc = u2d(rr.x, rr.y);
+        ++rw;
+        rr = p.tab[rw];
+        ra = slot_at(sl, rr.z);
+        rb = slot_at(sl, rr.w);
+        accg = fma(cc, v, accg);
+      }
+      if (g < NC) PU[gg] = accg; else PF[gg] = accg;
+    }
+#pragma unroll
+    for (int b = 0; b < NS; ++b)
+#pragma unroll
+      for (int X = 0; X < NC; ++X)
+        if (X >> b & 1) {
+          PU[X] += PU[X ^ (1 << b)];
+          PF[X] += PF[X ^ (1 << b)];
+        }
+    // corners: W = G0 U^aU0 F^aF0 (one reciprocal), Lambda = ln(U^aU1 F^aF1) + L0 (one logarithm)
+#pragma unroll
+    for (int X = 0; X < NC; ++X) {
+      const double U = PU[X], F = PF[X];
+      const double rF = fast_rcp(F);
+      double W = G0;
+      if (E::aU0 > 0) W *= ipow_c<(E::aU0 > 0 ? E::aU0 : 0)>(U);
+      if (E::aU0 < 0) W *= ipow_c<(E::aU0 < 0 ? -E::aU0 : 0)>(fast_rcp(U));
+      if (E::aF0 > 0) W *= ipow_c<(E::aF0 > 0 ? E::aF0 : 0)>(F);
+      if (E::aF0 < 0) W *= ipow_c<(E::aF0 < 0 ? -E::aF0 : 0)>(rF);
+      c.W[X] = W;
+      if (KMAX > 0 || X != FULL) c.Lam[X] = fast_log(ipow_c<E::aU1>(U) * ipow_c<-E::aF1>(rF), tabq) + L0;
+    }
+  }
+  if (NS > 0) {
+    const uint4 sln = p.tab[o + 1], sinv = p.tab[o + 2];
+    const uint4 ib01 = p.tab[o + 3], ib23 = p.tab[o + 4], b01 = p.tab[o + 5], b23 = p.tab[o + 6];
+    const uint32_t lnw[4] = {sln.x, sln.y, sln.z, sln.w}, invw[4] = {sinv.x, sinv.y, sinv.z, sinv.w};
+    const double ibv[4] = {u2d(ib01.x, ib01.y), u2d(ib01.z, ib01.w), u2d(ib23.x, ib23.y), u2d(ib23.z, ib23.w)};
+    const double bv[4] = {u2d(b01.x, b01.y), u2d(b01.z, b01.w), u2d(b23.x, b23.y), u2d(b23.z, b23.w)};
+#pragma unroll
+    for (int k = 0; k < NS; ++k) {
+      c.invt[k] = slot_at(sl, invw[k]);
+      c.invbeta[k] = ibv[k];
+      const double Lk = bv[k] * slot_at(sl, lnw[k]);
+      c.cL[k][0] = 1.0;
+#pragma unroll
+      for (int q = 1; q < K - 1; ++q) c.cL[k][q] = c.cL[k][q - 1] * Lk * (1.0 / q);
+    }
+  }
+  Fold2<NS, KMAX, K, 0, 0>::eval(c, out);
+}
+
+}  // namespace qmc4
+
+#ifndef Q4_NOPERSEC
+#define Q4_NOPERSEC 0
+#endif
+#ifndef QMC4_MIN_BLOCKS
+#define QMC4_MIN_BLOCKS 2
+#endif
+
+// partial layout: fused  : [run of sectors][shift][slice][NACC]
+//                 persec : [sector row][shift][slice][NACC]        (NACC = QMC_MAXSING + KMAX + 1, index a <-> order a - QMC_MAXSING)
+template <int NDIM, int L, int KMAX>
+__global__ void __launch_bounds__(QMC2_THREADS, QMC4_MIN_BLOCKS) qmc4_eval_kernel(const __grid_constant__ Qmc4Launch p) {
+  using namespace qmc4;
+  constexpr int NACC = QMC_MAXSING + KMAX + 1;
+  constexpr int SMAX = NDIM < QMC_MAXSING ? NDIM : QMC_MAXSING;
+  constexpr int T = QMC2_THREADS;
+
+  extern __shared__ __align__(16) unsigned char smem[];
+  const int tid = threadIdx.x;
+
+  // shared memory carve-up (all offsets multiples of 16)
+  double2 *logtab = reinterpret_cast<double2 *>(smem);
+  size_t o = (size_t)QMC4_LOG_ENTRIES * QMC4_LOG_COPIES * 16;
+  double *shf = reinterpret_cast<double *>(smem + o);
+  o += (((size_t)p.m * NDIM * 8) + 15) & ~(size_t)15;
+  double *scratch = reinterpret_cast<double *>(smem + o);
+  o += (T / 32) * 8;
+  double *slots = reinterpret_cast<double *>(smem + o);
+  o += (size_t)p.max_nslots * T * 8;
+  double *sacc = reinterpret_cast<double *>(smem + o);  // persec: [nsec][NACC][T]
+  unsigned char *sl = reinterpret_cast<unsigned char *>(slots + tid);
+  const double2 *tabq = logtab + (tid & (QMC4_LOG_COPIES - 1));
+
+  for (int i = tid; i < QMC4_LOG_ENTRIES * QMC4_LOG_COPIES; i += T)
+    logtab[i] = reinterpret_cast<const double2 *>(p.logtab)[i / QMC4_LOG_COPIES];
+  for (int i = tid; i < p.m * NDIM; i += T) shf[i] = p.shifts[i];
+  slots[3 * NDIM * T + tid] = 1.0;  // the constant slot
+  __syncthreads();
+
+  const uint32_t N = p.N;
+  const double dN = (double)N;
+  const uint32_t stride = (uint32_t)p.nslices * T;
+  uint32_t dz[NDIM];
+#pragma unroll
+  for (int j = 0; j < NDIM; ++j) dz[j] = (uint32_t)(((uint64_t)stride * p.zeff[j]) % N);
+
+  unsigned cntNonFinite = 0, cntBoundary = 0;
+
+  // One block = one shift vector (blockIdx.y): with the shift loop inside the block, the block reduction (barriers,
+  // shuffles under `if (warp == 0)`) sat on the back edge of a loop around the table walk, and ptxas then kept the whole
+  // walk off the uniform datapath.
+  const int kap = blockIdx.y;
+  {
+    double acc[NACC];
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) acc[a] = 0.0;
+    if (p.persec)
+      for (int i = 0; i < p.nsec * NACC; ++i) sacc[(size_t)i * T + tid] = 0.0;
+
+    // The point loop has a UNIFORM trip count (threads past the end of the index range, and boundary points, carry the
+    // weight 0 at a harmless stand-in point): only then may ptxas keep the table walk on the uniform datapath.
+    const uint32_t c0 = (uint32_t)blockIdx.x * T;
+    uint32_t r[NDIM];
+#pragma unroll
+    for (int j = 0; j < NDIM; ++j) r[j] = (uint32_t)((p.off[j] + (uint64_t)(c0 + tid) * p.zeff[j]) % N);
+
+    for (uint32_t cb = c0; cb < p.count; cb += stride) {
+      // S1-S3: lattice point (Eq. 17), shift + wrap (Eq. 18), periodising transform (Eq. 21), per-point slot table
+      const bool valid = cb + tid < p.count;
+      double w = 1.0;
+      bool inside = true;
+#pragma unroll
+      for (int j = 0; j < NDIM; ++j) {
+        double u = (double)r[j] / dN;
+        double y = u + shf[kap * NDIM + j];
+        if (y >= 1.0) y -= 1.0;
+        double tj;
+        if (p.transform == 0) {
+          tj = y * y * (3.0 - 2.0 * y);
+          w *= 6.0 * y * (1.0 - y);
+        } else {
+          tj = 1.0 - fabs(2.0 * y - 1.0);
+        }
+        if (!(y > 0.0) || !(tj > 0.0)) {
+          inside = false;
+          tj = 0.5;
+        }
+        reinterpret_cast<double *>(sl)[j * T] = tj;
+        reinterpret_cast<double *>(sl)[(NDIM + j) * T] = fast_log(tj, tabq);  // t >= 3.7e-32 for y >= 2^-53: a normal number
+        reinterpret_cast<double *>(sl)[(2 * NDIM + j) * T] = fast_rcp(tj);
+        uint32_t rn = r[j] + dz[j];
+        r[j] = rn >= N ? rn - N : rn;
+      }
+      if (valid && !inside && p.count_boundary) ++cntBoundary;
+      const bool live = valid && inside;
+      if (!live) w = 0.0;
+      for (uint32_t i = 0; i < p.nprog; i += 2) {  // chunk-wide product slots
+        const uint4 pw = p.tab[p.prog_word + (i >> 1)];
+        *reinterpret_cast<double *>(sl + p.first_prod_off + i * (T * 8)) = slot_at(sl, pw.x) * slot_at(sl, pw.y);
+        if (i + 1 < p.nprog)
+          *reinterpret_cast<double *>(sl + p.first_prod_off + (i + 1) * (T * 8)) = slot_at(sl, pw.z) * slot_at(sl, pw.w);
+      }
+      // S4-S6: all sectors of the run at this point
+      for (int si = 0; si < p.nsec; ++si) {
+        // (offsets come from an array indexed by the induction variable: a loop-carried offset read from the table
+        //  itself makes ptxas give up the uniform datapath for the whole table walk)
+        const uint32_t so = p.secw[si];
+        const uint4 h0 = p.tab[so];
+#define QMC4_CASE(NS_)                                                                                       \
+  case NS_: {                                                                                                \
+    if (NS_ <= SMAX) {                                                                                       \
+      constexpr int NSC = NS_ <= SMAX ? NS_ : 0, KK = KMAX + NSC + 1;                                        \
+      double res[KK];                                                                                        \
+      sector4<NDIM, L, NSC, KMAX>(p, so, sl, tabq, res);                                                     \
+      bool fin = true;                                                                                       \
+      _Pragma("unroll") for (int i = 0; i < KK; ++i) fin = fin && finite_hi(res[i]);                         \
+      /* branch-free: a non-finite evaluation is dropped (and counted), a dead thread has w = 0 */             \
+      cntNonFinite += (live && !fin) ? 1u : 0u;                                                              \
+      const double wk = fin ? w : 0.0;                                                                       \
+      _Pragma("unroll") for (int i = 0; i < KK; ++i) res[i] = fin ? res[i] : 0.0;                            \
+      if (Q4_NOPERSEC || !p.persec) {                                                                                       \
+        _Pragma("unroll") for (int i = 0; i < KK; ++i) acc[QMC_MAXSING - NSC + i] = fma(wk, res[i], acc[QMC_MAXSING - NSC + i]); \
+      } else {                                                                                               \
+        double *sa = sacc + ((size_t)si * NACC + (QMC_MAXSING - NSC)) * T + tid;                             \
+        _Pragma("unroll") for (int i = 0; i < KK; ++i) sa[(size_t)i * T] += wk * res[i];                     \
+      }                                                                                                      \
+    }                                                                                                        \
+  } break;
+#ifdef Q4_T1
+        switch (4) {
+#else
+        switch (h0.x & 255u) {
+#endif
+          QMC4_CASE(0)
+          QMC4_CASE(1)
+          QMC4_CASE(2)
+          QMC4_CASE(3)
+          QMC4_CASE(4)
+          default:
+            break;
+        }
+#undef QMC4_CASE
+      }
+    }
+
+    // S7: block reduction -> one partial per (run | sector, shift, block)
+#ifdef Q4_T3
+    for (int a = 0; a < NACC; ++a) p.partial[(size_t)(blockIdx.x * T + tid) * NACC + a] += acc[a];
+    if (false) {
+#else
+    if (!p.persec) {
+#endif
+      double *dst = p.partial + (((size_t)p.out_row * p.m + kap) * p.max_slices + blockIdx.x) * NACC;
+#pragma unroll
+      for (int a = 0; a < NACC; ++a) {
+        double sr = qmcdev::block_sum(acc[a], scratch);
+        if (tid == 0) dst[a] = sr;
+      }
+    } else {
+      for (int si = 0; si < p.nsec; ++si) {
+        double *dst = p.partial + (((size_t)(p.out_row + p.secrow[si]) * p.m + kap) * p.max_slices + blockIdx.x) * NACC;
+        for (int a = 0; a < NACC; ++a) {
+          double v = qmcdev::block_sum(sacc[((size_t)si * NACC + a) * T + tid], scratch);
+          if (tid == 0) dst[a] = v;
+        }
+      }
+    }
+  }
+
+  unsigned c2[2] = {cntNonFinite, cntBoundary};
+#pragma unroll
+  for (int q = 0; q < 2; ++q) {
+    unsigned v = c2[q];
+#pragma unroll
+    for (int o2 = 16; o2 > 0; o2 >>= 1) v += __shfl_down_sync(0xffffffffu, v, o2);
+    if ((tid & 31) == 0 && v) atomicAdd(p.counters + 2 + q, (unsigned long long)v);
+  }
+}

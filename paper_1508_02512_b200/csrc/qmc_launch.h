@@ -70,3 +70,42 @@ bool qmc2_kernel_available(int ndim, int loops, int kmax);
 // implemented in qmc_dispatch.cu on top of one translation unit per dimension (qmc_inst_d<N>.cu)
 cudaError_t qmc_kernel_prepare(int ndim, int kmax, int flavor, size_t smem, int *blocks_per_sm);
 cudaError_t qmc_kernel_launch(int ndim, int kmax, int flavor, dim3 grid, size_t smem, cudaStream_t st, const QmcLaunch &p);
+
+// ---- version 4 (real path, tables in the kernel-parameter constant bank) -------------------------------------
+// One launch = one run of sectors of one chunk; blockIdx.x = slice of the lattice points.  The chunk's slot program and
+// the sector tables travel INSIDE the kernel parameter block (constant bank 0): every table read is a uniform load
+// (LDCU) into uniform registers, slot operands are addressed [thread column + uniform offset], the record loops run on
+// the uniform datapath and are unrolled by the compiler.  Layout of `tab` (16-byte words):
+//   [prog_word ..)  slot program: nprog x {u32 a_off, u32 b_off} (byte offsets into the thread's slot column), 2 per word
+//   [sec_word ..)   sector blocks, back to back; sector block (word offsets relative to its start):
+//     w0 = {nsing | nL0 << 8 | nlocal << 16, nwords of the block, rec_word (first record), 0}
+//     w1 = sing_ln[4]  (byte offsets of ln t_k of the singular positions)      w2 = sing_inv[4]  (of 1/t_k)
+//     w3,w4 = invbeta[4] (f64)      w5,w6 = beta[4] (f64)
+//     w7 = extra records per group of U^ (u8 x 16)      w8 = the same for F^
+//     w9.. = local program: nlocal x {u32 a_off, u32 b_off}, padded to a word
+//     records {f64 c, u32 off0, u32 off1}: [G0][L0 x nL0][first record of every group of U^: 2^nsing, c = 0 if the
+//     group is empty][the same for F^][extra records of U^ by group][extra records of F^ by group][sentinel, c = 0]
+#define QMC4_TAB_WORDS 1808  // 28 928 bytes of tables per launch (kernel parameters are limited to 32 764 bytes)
+#define QMC4_MAX_SEC 160     // sectors per launch
+#define QMC4_LOG_ENTRIES 64
+#define QMC4_LOG_COPIES 8
+struct Qmc4Launch {
+  const double *logtab;          // device: 64 x {1/c, -ln(1/c)}
+  const double *shifts;          // device: [m][ndim]
+  double *partial;               // device: [row][shift][max_slices][NACC]
+  unsigned long long *counters;  // device: [4]
+  uint32_t N, count;
+  uint32_t zeff[QMC_MAXDIM], off[QMC_MAXDIM];
+  int32_t m, transform, persec, max_slices;
+  int32_t nsec, out_row, count_boundary, nslices;
+  uint32_t nprog, prog_word, sec_word, first_prod_off;  // first_prod_off, local0_off: byte offsets in the slot column
+  uint32_t local0_off, max_nslots, pad0, pad1;
+  uint16_t secw[QMC4_MAX_SEC];  // word offset of the sector blocks in tab, in evaluation order (sorted by nsing: sectors
+                                // that run the same code path are neighbours, which the instruction cache likes)
+  uint16_t secrow[QMC4_MAX_SEC]; // per-sector mode: row of the partial buffer relative to out_row
+  uint4 tab[QMC4_TAB_WORDS];
+};
+static_assert(sizeof(Qmc4Launch) <= 32764, "kernel parameter limit");
+cudaError_t qmc4_kernel_prepare(int ndim, int loops, int kmax, size_t smem, int *blocks_per_sm);
+cudaError_t qmc4_kernel_launch(int ndim, int loops, int kmax, dim3 grid, size_t smem, cudaStream_t st, const Qmc4Launch &p);
+bool qmc4_kernel_available(int ndim, int loops, int kmax);

@@ -128,6 +128,14 @@ struct qmc_tables {
   std::vector<Qmc2Chunk> chunks;
   std::vector<double> sec_cost;   // modelled cost per sector (load balancing of the launch)
   double logtab[256] = {0};      // 128 x {1/c_i, -ln(1/c_i)} of the kernels' table-driven logarithm
+  // version 4 tables (real path; same chunks and slot programs as version 2, laid out for the kernel-parameter
+  // constant bank: see qmc_launch.h)
+  std::vector<uint32_t> tab4;       // sector blocks, 32-bit words (4 per 16-byte table word)
+  std::vector<uint32_t> secoff4;    // [n_sectors + 1] offsets into tab4 in 16-byte words
+  std::vector<std::vector<uint32_t>> prog4;  // per chunk: slot program {a_off, b_off} byte offsets, padded to 16 bytes
+  double logtab4[128] = {0};        // 64 x {1/c_i, -ln(1/c_i)}
+  void *side_streams[8] = {nullptr};  // cudaStream_t: the launches of one integration are spread over these
+  void *side_events[9] = {nullptr};   // cudaEvent_t: fork + one join per side stream
   // version 3 image (complex path only)
   std::vector<uint8_t> image3;
   std::vector<uint32_t> secoff3, secend3;
@@ -149,6 +157,7 @@ struct qmc_tables {
     const void *ws = nullptr;
     int m = 0, mode = 0, nrows = 0;
     size_t h2d = 0;
+    int launches = 3;
   } last;
 };
 
