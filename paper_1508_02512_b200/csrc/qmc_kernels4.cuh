@@ -23,7 +23,6 @@ namespace qmc4 {
 
 using qmc2::Ctx2;
 using qmc2::Expo;
-using qmc2::fast_rcp;
 using qmc2::finite_hi;
 using qmc2::Fold2;
 using qmc2::ipow_c;
@@ -51,6 +50,15 @@ __device__ __forceinline__ double fast_log(double x, const double2 *__restrict__
   return ok ? v : __longlong_as_double(0x7ff8000000000000ll);
 }
 static_assert(QMC4_LOG_COPIES * 16 == 1 << 7, "fast_log index arithmetic assumes 128 bytes per table entry row");
+
+// 1/x to ~1 ulp: MUFU.RCP64H seed (about 20 bits) + ONE cubic step r (1 + e + e^2), e = 1 - x r: 3 FP64 instructions
+// (x normal, which U^, F^ and t_j are)
+__device__ __forceinline__ double fast_rcp(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  const double e = fma(-x, r, 1.0);
+  return fma(r, fma(e, e, e), r);
+}
 
 __device__ __forceinline__ double slot_at(const unsigned char *__restrict__ sl, uint32_t off) {
   return *reinterpret_cast<const double *>(sl + off);
@@ -106,21 +114,28 @@ __device__ __forceinline__ void sector4(const Qmc4Launch &p, const uint32_t o, u
     // harmless sentinel record), so the LDCU -> LDS -> DMUL -> DFMA chain is not exposed once per group
     uint4 rr = p.tab[rw];
     double ra = slot_at(sl, rr.z), rb = slot_at(sl, rr.w);
+    constexpr int NW = (NC + 3) / 4, GW = NC < 4 ? NC : 4;  // count words per polynomial, groups per word
 #pragma unroll
-    for (int g = 0; g < 2 * NC; ++g) {
-      const int gg = g & (NC - 1);
-      const uint32_t cnt = ((g < NC ? cuw[gg >> 2] : cfw[gg >> 2]) >> (8 * (gg & 3))) & 255u;
-      double accg = g < NC ? PU[gg] : PF[gg];
+    for (int q = 0; q < 2 * NW; ++q) {
+      const uint32_t cw = q < NW ? cuw[q % NW] : cfw[q % NW];
+      if (cw != 0u) {  // (one test skips four groups without extra records)
+#pragma unroll
+        for (int k = 0; k < GW; ++k) {
+          const int gg = (q % NW) * 4 + k;
+          const uint32_t cnt = (cw >> (8 * k)) & 255u;
+          double accg = q < NW ? PU[gg] : PF[gg];
 #pragma unroll 1
-      for (uint32_t i = 0; i < cnt; ++i) {
-        const double v = ra * rb, cc = u2d(rr.x, rr.y);
-        ++rw;
-        rr = p.tab[rw];
-        ra = slot_at(sl, rr.z);
-        rb = slot_at(sl, rr.w);
-        accg = fma(cc, v, accg);
+          for (uint32_t i = 0; i < cnt; ++i) {
+            const double v = ra * rb, cc = u2d(rr.x, rr.y);
+            ++rw;
+            rr = p.tab[rw];
+            ra = slot_at(sl, rr.z);
+            rb = slot_at(sl, rr.w);
+            accg = fma(cc, v, accg);
+          }
+          if (q < NW) PU[gg] = accg; else PF[gg] = accg;
+        }
       }
-      if (g < NC) PU[gg] = accg; else PF[gg] = accg;
     }
 #pragma unroll
     for (int b = 0; b < NS; ++b)
@@ -280,15 +295,15 @@ __global__ void __launch_bounds__(QMC2_THREADS, QMC4_MIN_BLOCKS) qmc4_eval_kerne
       sector4<NDIM, L, NSC, KMAX>(p, so, sl, tabq, res);                                                     \
       bool fin = true;                                                                                       \
       _Pragma("unroll") for (int i = 0; i < KK; ++i) fin = fin && finite_hi(res[i]);                         \
-      /* branch-free: a non-finite evaluation is dropped (and counted), a dead thread has w = 0 */             \
+      /* a non-finite evaluation is dropped (and counted); a dead thread has w = 0.  Predicated, not branched */ \
       cntNonFinite += (live && !fin) ? 1u : 0u;                                                              \
-      const double wk = fin ? w : 0.0;                                                                       \
-      _Pragma("unroll") for (int i = 0; i < KK; ++i) res[i] = fin ? res[i] : 0.0;                            \
-      if (Q4_NOPERSEC || !p.persec) {                                                                                       \
-        _Pragma("unroll") for (int i = 0; i < KK; ++i) acc[QMC_MAXSING - NSC + i] = fma(wk, res[i], acc[QMC_MAXSING - NSC + i]); \
+      if (Q4_NOPERSEC || !p.persec) {                                                                        \
+        _Pragma("unroll") for (int i = 0; i < KK; ++i)                                                       \
+          if (fin) acc[QMC_MAXSING - NSC + i] = fma(w, res[i], acc[QMC_MAXSING - NSC + i]);                  \
       } else {                                                                                               \
         double *sa = sacc + ((size_t)si * NACC + (QMC_MAXSING - NSC)) * T + tid;                             \
-        _Pragma("unroll") for (int i = 0; i < KK; ++i) sa[(size_t)i * T] += wk * res[i];                     \
+        _Pragma("unroll") for (int i = 0; i < KK; ++i)                                                       \
+          if (fin) sa[(size_t)i * T] += w * res[i];                                                          \
       }                                                                                                      \
     }                                                                                                        \
   } break;
