@@ -5,7 +5,8 @@
 // scheme the kernels implement, with DFMA = 2 and DADD = DMUL = 1 and fixed costs for the library sequences
 // (fast paths of the CUDA 12.9 sm_100a FP64 routines, counted in SASS; the kernels' own routines in brackets):
 //   division: 7 DFMA + 2 DMUL = 16      atan2: division + 19 DFMA polynomial + fix-ups = 60
-//   [table logarithm: 7 DFMA + DMUL + DADD = 16]      [Newton reciprocal: 4 DFMA = 8]
+//   [table logarithm, 128 entries (complex path): 7 DFMA + DMUL + DADD = 16; 64 entries (real path): 8 DFMA + DMUL + DADD = 18]
+//   [reciprocal: Newton, 4 DFMA = 8 (complex path); one cubic step, 3 DFMA = 6 (real path)]
 // Integer work (lattice index arithmetic, table decoding) and comparisons count as zero.  The count is
 // cross-checked against Nsight Compute's executed DFMA/DADD/DMUL thread-instruction counters (profiles/).
 #include <algorithm>
@@ -35,8 +36,8 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
   if (sb < 0 || se > nsec || sb >= se) return QMC_EINVAL;
   const bool cplx = t->lambda > 0.0;
   // S1-S3, once per (point, shift): u = r/N (IEEE division), y = u + Delta (wrap), t = y^2 (3 - 2y), w *= 6 y (1 - y),
-  // ln t (table logarithm, 16), 1/t (Newton reciprocal, 8)
-  const double per_point = n * (F_DIV + 2.0 + 4.0 + 4.0 + 16.0 + 8.0);
+  // ln t (table logarithm), 1/t (reciprocal)
+  const double per_point = n * (F_DIV + 2.0 + 4.0 + 4.0 + (cplx ? 16.0 + 8.0 : 18.0 + 6.0));
   double per_sectors = 0.0;
   int64_t ncorners = 0;
   const int eU = std::abs(t->aU0), eF = std::abs(t->aF0);
@@ -54,27 +55,48 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
       }
     }
     if (!cplx) {
-      // version-2 scheme (qmc_kernels2.cuh).  A record c * slot * slot is DMUL + DFMA = 3.
+      // version-4 scheme (qmc_kernels4.cuh).  A record c * slot * slot accumulated onto its group is DMUL + DFMA = 3;
+      // the first record of a group (and G0) is two DMUL = 2.  The zero-coefficient stand-ins of empty groups and
+      // the sentinel are not counted: they are the kernel's overhead, not the method's arithmetic.
       auto pow_muls = [](int e) {  // multiplications of x^e by repeated squaring, e >= 0
         int c = 0;
         for (int q = e; q > 1; q >>= 1) c += 1 + (q & 1);
         return (double)c;
       };
-      const double F_RCP2 = 8.0;    // MUFU seed + 4 DFMA
-      const double F_LOG2 = 16.0;   // table-driven: 7 DFMA + DMUL + DADD
+      const double F_RCP2 = 6.0;    // MUFU seed + 3 DFMA
+      const double F_LOG2 = 18.0;   // table-driven: 8 DFMA + DMUL + DADD
       int nL0 = 0;
       for (int j = 0; j < n; ++j)
         if (s.alpha[j] != -1 && s.beta[j]) ++nL0;
       f = 3.0 * (1 + nL0 + s.U.size() + s.F.size());   // G0, L0, U^, F^ records (replaces the set-up count above)
+      {
+        int pos[QMC_MAXDIM], k = 0;
+        for (int j = 0; j < n; ++j) pos[j] = s.alpha[j] == -1 ? k++ : -1;
+        double first = 1.0;  // G0
+        for (int which = 0; which < 2; ++which) {
+          unsigned seen = 0;
+          for (const QmcMono &m : (which ? s.F : s.U)) {
+            int g = 0;
+            for (int j = 0; j < n; ++j)
+              if (m.e[j] && pos[j] >= 0) g |= 1 << pos[j];
+            if (!(seen >> g & 1u)) first += 1.0;
+            seen |= 1u << g;
+          }
+        }
+        f -= first;  // first records: DMUL + DMUL
+      }
       f += 2.0 * ns * (nc / 2);                        // subset sums
       for (int j = 0; j < n; ++j)
-        if (s.alpha[j] == -1) f += 1.0 + 2.0 * std::max(0, K - 2);   // series of beta_j ln t_j
+        if (s.alpha[j] == -1) f += 1.0 + 2.0 * std::max(0, K - 3);   // beta_j ln t_j, then (.)^p / p! for p = 2 .. K-2
       for (int Z = 0; Z < nc; ++Z) {
         const int len = t->kmax + __builtin_popcount(Z) + 1;       // leaf window
         f += F_RCP2 + (t->aU0 < 0 ? F_RCP2 : 0.0);
         f += (t->aU0 ? pow_muls(eU) + 1.0 : 0.0) + (t->aF0 ? pow_muls(eF) + 1.0 : 0.0);
-        if (len > 1) f += pow_muls(std::abs(t->aU1)) + pow_muls(std::abs(t->aF1)) + 1.0 + F_LOG2 + 1.0;
-        f += 2.0 * (len - 1);
+        if (len > 1) {
+          f += pow_muls(std::abs(t->aU1)) + pow_muls(std::abs(t->aF1)) + 1.0 + F_LOG2 + 1.0;
+          if (t->aF0 < 0 && eF >= 2 && std::abs(t->aF1) >= 2) f -= 1.0;  // (1/F)^2 is shared between W and the argument of the logarithm
+        }
+        if (len > 1) f += 2.0 * (len - 1) - 1.0;   // W Lambda^p / p!: two multiplications per term, one for p = 1
       }
       // fold: merge at level l with Z the choices of the levels below l
       for (int l = 0; l < ns; ++l)

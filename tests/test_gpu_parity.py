@@ -150,9 +150,10 @@ def test_double_box_poles_on_gpu_at_baseline_size():
     assert np.allclose(p.shift_totals, r.shift_totals, rtol=1e-11, atol=1e-13)
 
 
-def test_v2_tables_chunk_boundaries_and_small_slot_budget(monkeypatch):
-    """Version-2 tables: sector ranges that straddle chunk boundaries, and a slot budget small enough to force
-    sector-local product slots and chunk splits (QMC2_SLOTS / QMC2_CHUNK_BYTES are read by qmc_prepare)."""
+def test_real_path_tables_chunk_boundaries_slot_budget_and_launch_splits(monkeypatch):
+    """Real-path tables (version 4: one launch per run of sectors, tables in the kernel parameters): sector ranges that
+    straddle chunk boundaries, a slot budget small enough to force sector-local product slots and chunk splits, and
+    chunks larger than what one launch can carry (QMC2_SLOTS / QMC2_CHUNK_BYTES are read by qmc_prepare)."""
     wl = qi.double_box()
     t = q.qmc_prepare(wl)
     desc = t.describe()
@@ -170,6 +171,11 @@ def test_v2_tables_chunk_boundaries_and_small_slot_budget(monkeypatch):
     assert len(d2.splitlines()) > len(desc.splitlines())
     parity(wl, 16381, 2, sectors=(100, 140))
     monkeypatch.delenv("QMC2_SLOTS")
+    monkeypatch.setenv("QMC2_CHUNK_BYTES", "60000")       # a chunk now exceeds the 28 KB of tables one launch carries
+    t3 = q.qmc_prepare(wl)
+    nchunks3 = sum(int(l.split("[")[1].split(",")[0]) < 150 for l in t3.describe().splitlines()[1:])   # chunks meeting [0, 150)
+    r3, f3, *_ = parity(wl, 16381, 2, sectors=(0, 150))
+    assert f3.kernel_launches - 2 > nchunks3                # the launcher split chunks into several runs
     monkeypatch.delenv("QMC2_CHUNK_BYTES")
 
 
