@@ -112,8 +112,12 @@ __device__ __forceinline__ void sector4(const Qmc4Launch &p, const uint32_t o, u
     // extra records: one stream across all groups, software-pipelined by one record -- the slot operands of the NEXT
     // record are requested before the current one is accumulated, also across group boundaries (the block ends with a
     // harmless sentinel record), so the LDCU -> LDS -> DMUL -> DFMA chain is not exposed once per group
-    uint4 rr = p.tab[rw];
-    double ra = slot_at(sl, rr.z), rb = slot_at(sl, rr.w);
+    // (only the OFFSETS of the next record are requested ahead; its coefficient is loaded in its own iteration, where the
+    //  wait for the slot operands hides the latency -- carrying it across the iteration cost two UMOV per record)
+    const unsigned char *tb = reinterpret_cast<const unsigned char *>(p.tab);
+    uint32_t rwb = rw * 16u;  // byte offset of the current record: {f64 c | u32 off0, u32 off1}
+    uint2 ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);
+    double ra = slot_at(sl, ro.x), rb = slot_at(sl, ro.y);
     constexpr int NW = (NC + 3) / 4, GW = NC < 4 ? NC : 4;  // count words per polynomial, groups per word
 #pragma unroll
     for (int q = 0; q < 2 * NW; ++q) {
@@ -126,12 +130,13 @@ __device__ __forceinline__ void sector4(const Qmc4Launch &p, const uint32_t o, u
           double accg = q < NW ? PU[gg] : PF[gg];
 #pragma unroll 1
           for (uint32_t i = 0; i < cnt; ++i) {
-            const double v = ra * rb, cc = u2d(rr.x, rr.y);
-            ++rw;
-            rr = p.tab[rw];
-            ra = slot_at(sl, rr.z);
-            rb = slot_at(sl, rr.w);
-            accg = fma(cc, v, accg);
+            const uint2 rc = *reinterpret_cast<const uint2 *>(tb + rwb);
+            const double v = ra * rb;
+            rwb += 16u;
+            ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);
+            ra = slot_at(sl, ro.x);
+            rb = slot_at(sl, ro.y);
+            accg = fma(u2d(rc.x, rc.y), v, accg);
           }
           if (q < NW) PU[gg] = accg; else PF[gg] = accg;
         }
