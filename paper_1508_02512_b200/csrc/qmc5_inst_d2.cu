@@ -1,0 +1,2 @@
+#include "qmc_inst5.cuh"
+QMC5_DEFINE_DIM(2)

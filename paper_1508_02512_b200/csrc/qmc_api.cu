@@ -510,6 +510,156 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
   return QMC_OK;
 }
 
+// ---- version-5 launch (complex path): as version 4, two slot tables per thread ------------------------------------------
+int launch_v5(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t st, uint64_t N, int m, int sb, int se,
+              bool persec, uint64_t ibeg, uint64_t istep, uint64_t icount, const uint64_t *z, int sms, int smem_optin,
+              int *gx_out, int *rows_out, int *launches_out, size_t *h2d, cudaError_t *ce_out) {
+  const int n = t->n, nacc = 2 * (QMC_MAXSING + t->kmax + 1), T = QMC2_THREADS;  // accumulators: (Re, Im) per order
+  int max_r = 0, max_c = 0;
+  for (size_t ci = 0; ci < t->chunks3.size(); ++ci) {
+    const Qmc2Chunk &c = t->chunks3[ci];
+    if (c.sec_end > sb && c.sec_begin < se) {
+      max_r = std::max(max_r, c.nslots + c.max_local);
+      max_c = std::max(max_c, t->chunk3_nslots_c[ci] + t->chunk3_max_local_c[ci]);
+    }
+  }
+  const size_t budget = (size_t)smem_optin - 1024;
+  const size_t fixed = (size_t)QMC4_LOG_ENTRIES * QMC4_LOG_COPIES * 16 + (((size_t)m * n * 8 + 15) & ~(size_t)15) + (T / 32) * 8 +
+                       (size_t)max_r * T * 8 + (size_t)max_c * T * 16;
+  const size_t accbytes = persec ? (size_t)nacc * T * 8 : 0;
+  if (fixed + accbytes > budget) return QMC_ENOMEM;
+  struct Run { int chunk, a, b; double cost; };
+  std::vector<Run> runs;
+  double total_cost = 0.0;
+  int max_nsec = 0;
+  for (size_t ci = 0; ci < t->chunks3.size(); ++ci) {
+    const Qmc2Chunk &c = t->chunks3[ci];
+    int a = std::max(sb, c.sec_begin);
+    const int e = std::min(se, c.sec_end);
+    const size_t prog_words = (t->prog5r[ci].size() + t->prog5c[ci].size()) / 4;
+    while (a < e) {
+      int b = a;
+      while (b < e) {
+        const size_t words = prog_words + (t->secoff5[b + 1] - t->secoff5[a]);
+        if (words > QMC4_TAB_WORDS || b + 1 - a > QMC4_MAX_SEC || fixed + accbytes * (b + 1 - a) > budget) break;
+        ++b;
+      }
+      if (b == a) return QMC_ENOMEM;
+      Run r = {(int)ci, a, b, 0.0};
+      for (int s = a; s < b; ++s) r.cost += t->sec_cost[s];
+      total_cost += r.cost;
+      max_nsec = std::max(max_nsec, b - a);
+      runs.push_back(r);
+      a = b;
+    }
+  }
+  const int nitems = (int)runs.size();
+  const size_t smem = fixed + accbytes * max_nsec;
+  int bps = 0;
+  CUDA_OK(qmc5_kernel_prepare(n, t->L, t->kmax, smem, &bps));
+  if (bps < 1) return QMC_ECUDA;
+  int waves = 16;
+  if (const char *e = std::getenv("QMC2_WAVES")) waves = std::max(1, std::atoi(e));
+  const long long max_slices_pts = std::max<long long>(1, (long long)((icount + T - 1) / T));
+  const double nblocks_target = (double)waves * sms * bps / (double)m;
+  std::vector<int> nsl(nitems);
+  int max_slices = 1;
+  for (int i = 0; i < nitems; ++i) {
+    long long ns = (long long)(nblocks_target * runs[i].cost / total_cost + 0.5);
+    ns = std::max<long long>(1, std::min<long long>({ns, (long long)QMC_MAX_BLOCKS, max_slices_pts}));
+    nsl[i] = (int)ns;
+    max_slices = std::max(max_slices, (int)ns);
+  }
+  const int rows_partial = persec ? (se - sb) : nitems;
+  CUDA_OK(cudaMemsetAsync(ws + L.partial, 0, (size_t)rows_partial * m * max_slices * nacc * 8, st));
+  int nstreams = 4;
+  if (const char *e = std::getenv("QMC4_STREAMS")) nstreams = std::max(0, std::min(8, std::atoi(e)));
+  nstreams = std::min(nstreams, nitems);
+  if (nstreams < 2) nstreams = 0;
+  for (int q = 0; q < nstreams; ++q)
+    if (!t->side_streams[q]) {
+      CUDA_OK(cudaStreamCreateWithFlags(reinterpret_cast<cudaStream_t *>(&t->side_streams[q]), cudaStreamNonBlocking));
+    }
+  for (int q = 0; q < nstreams + 1; ++q)
+    if (!t->side_events[q]) {
+      CUDA_OK(cudaEventCreateWithFlags(reinterpret_cast<cudaEvent_t *>(&t->side_events[q]), cudaEventDisableTiming));
+    }
+  static thread_local Qmc5Launch p;
+  std::memset(&p, 0, offsetof(Qmc5Launch, tab));
+  p.logtab = reinterpret_cast<const double *>(ws + L.logtab4);
+  p.shifts = reinterpret_cast<const double *>(ws + L.shifts);
+  p.partial = reinterpret_cast<double *>(ws + L.partial);
+  p.counters = reinterpret_cast<unsigned long long *>(ws + L.counters);
+  p.N = (uint32_t)N;
+  p.count = (uint32_t)icount;
+  for (int j = 0; j < n; ++j) {
+    p.zeff[j] = (uint32_t)mulmod(istep % N, z[j], N);
+    p.off[j] = (uint32_t)mulmod(ibeg, z[j], N);
+  }
+  p.m = m;
+  p.transform = t->transform;
+  p.persec = persec ? 1 : 0;
+  p.max_slices = max_slices;
+  p.max_nslots_r = (uint32_t)max_r;
+  p.max_nslots_c = (uint32_t)max_c;
+  p.lambda = t->lambda;
+  cudaEventRecord(static_cast<cudaEvent_t>(t->ev0), st);
+  if (nstreams) {
+    cudaEventRecord(static_cast<cudaEvent_t>(t->side_events[nstreams]), st);
+    for (int q = 0; q < nstreams; ++q)
+      cudaStreamWaitEvent(static_cast<cudaStream_t>(t->side_streams[q]), static_cast<cudaEvent_t>(t->side_events[nstreams]), 0);
+  }
+  cudaError_t ce = cudaSuccess;
+  for (int i = 0; i < nitems && ce == cudaSuccess; ++i) {
+    const Run &r = runs[i];
+    const Qmc2Chunk &c = t->chunks3[r.chunk];
+    const std::vector<uint32_t> &pgr = t->prog5r[r.chunk], &pgc = t->prog5c[r.chunk];
+    const int nslots_c = t->chunk3_nslots_c[r.chunk];
+    p.nsec = r.b - r.a;
+    p.out_row = persec ? r.a - sb : i;
+    p.count_boundary = i == 0 ? 1 : 0;
+    p.nslices = nsl[i];
+    p.nprog_r = (uint32_t)(c.nslots - (3 * n + 1));
+    p.prog_r_word = 0;
+    p.first_prod_r_off = (uint32_t)(3 * n + 1) * T * 8u;
+    p.local0_r_off = (uint32_t)c.nslots * T * 8u;
+    p.nprog_c = (uint32_t)(nslots_c - (n + 1));
+    p.prog_c_word = (uint32_t)(pgr.size() / 4);
+    p.first_prod_c_off = (uint32_t)(n + 1) * T * 16u;
+    p.local0_c_off = (uint32_t)nslots_c * T * 16u;
+    const uint32_t sec_word = (uint32_t)((pgr.size() + pgc.size()) / 4);
+    uint32_t *tw = reinterpret_cast<uint32_t *>(p.tab);
+    std::memcpy(tw, pgr.data(), pgr.size() * 4);
+    std::memcpy(tw + pgr.size(), pgc.data(), pgc.size() * 4);
+    const size_t w0 = t->secoff5[r.a], w1 = t->secoff5[r.b];
+    std::memcpy(tw + pgr.size() + pgc.size(), t->tab5.data() + w0 * 4, (w1 - w0) * 16);
+    {
+      int k = 0;
+      for (int ns = 0; ns <= QMC_MAXSING; ++ns)
+        for (int s = r.a; s < r.b; ++s)
+          if (t->sectors[s].nsing == ns) {
+            p.secw[k] = (uint16_t)(sec_word + (t->secoff5[s] - w0));
+            p.secrow[k] = (uint16_t)(s - r.a);
+            ++k;
+          }
+    }
+    cudaStream_t ls = nstreams ? static_cast<cudaStream_t>(t->side_streams[i % nstreams]) : st;
+    ce = qmc5_kernel_launch(n, t->L, t->kmax, dim3((unsigned)nsl[i], (unsigned)m), smem, ls, p);
+    *h2d += offsetof(Qmc5Launch, tab) + (pgr.size() + pgc.size()) * 4 + (w1 - w0) * 16;
+  }
+  if (nstreams)
+    for (int q = 0; q < nstreams; ++q) {
+      cudaEventRecord(static_cast<cudaEvent_t>(t->side_events[q]), static_cast<cudaStream_t>(t->side_streams[q]));
+      cudaStreamWaitEvent(st, static_cast<cudaEvent_t>(t->side_events[q]), 0);
+    }
+  cudaEventRecord(static_cast<cudaEvent_t>(t->evm), st);
+  *ce_out = ce;
+  *gx_out = max_slices;
+  *rows_out = nitems;
+  *launches_out = nitems;
+  return QMC_OK;
+}
+
 // ---- version-3 launch (complex path): same geometry as version 2, two slot tables per thread ------------------------------------
 int launch_v3(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t st, uint64_t N, int m, int sb, int se,
               bool persec, uint64_t ibeg, uint64_t istep, uint64_t icount, const uint64_t *z, int sms, int smem_optin,
@@ -873,6 +1023,8 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
       CUDA_OK(cudaMemcpyAsync(ws + L.image3, t->image3.data(), t->image3.size(), cudaMemcpyHostToDevice, st));
       CUDA_OK(cudaMemcpyAsync(ws + L.secoff3, t->secoff3.data(), t->secoff3.size() * 4, cudaMemcpyHostToDevice, st));
       CUDA_OK(cudaMemcpyAsync(ws + L.logtab, t->logtab, sizeof t->logtab, cudaMemcpyHostToDevice, st));
+      CUDA_OK(cudaMemcpyAsync(ws + L.logtab4, t->logtab4, sizeof t->logtab4, cudaMemcpyHostToDevice, st));
+      h2d += sizeof t->logtab4;
     }
     if (!t->image2.empty()) {
       h2d += t->image2.size() + t->secoff2.size() * 4 + sizeof t->logtab;
@@ -894,7 +1046,11 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
 
   const bool use_v3 = cplx && !t->image3.empty() && -t->kmin <= QMC3_MAXSING && qmc3_kernel_available(n, t->L, t->kmax) &&
                       !std::getenv("QMC_FORCE_V1");
-  if (use_v3) {
+  const bool use_v5 = use_v3 && !t->tab5.empty() && qmc5_kernel_available(n, t->L, t->kmax) && !std::getenv("QMC_FORCE_V3");
+  if (use_v5) {
+    int rc = launch_v5(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, &gx, &nchunks, &eval_launches, &h2d, &ce);
+    if (rc != QMC_OK) return rc;
+  } else if (use_v3) {
     int rc = launch_v3(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, &gx, &nchunks, &h2d, &ce);
     if (rc != QMC_OK) return rc;
   } else if (use_v4) {

@@ -5,8 +5,7 @@
 // scheme the kernels implement, with DFMA = 2 and DADD = DMUL = 1 and fixed costs for the library sequences
 // (fast paths of the CUDA 12.9 sm_100a FP64 routines, counted in SASS; the kernels' own routines in brackets):
 //   division: 7 DFMA + 2 DMUL = 16      atan2: division + 19 DFMA polynomial + fix-ups = 60
-//   [table logarithm, 128 entries (complex path): 7 DFMA + DMUL + DADD = 16; 64 entries (real path): 8 DFMA + DMUL + DADD = 18]
-//   [reciprocal: Newton, 4 DFMA = 8 (complex path); one cubic step, 3 DFMA = 6 (real path)]
+//   [table logarithm, 64 entries: 8 DFMA + DMUL + DADD = 18]      [reciprocal: MUFU seed + one cubic step, 3 DFMA = 6]
 // Integer work (lattice index arithmetic, table decoding) and comparisons count as zero.  The count is
 // cross-checked against Nsight Compute's executed DFMA/DADD/DMUL thread-instruction counters (profiles/).
 #include <algorithm>
@@ -37,7 +36,7 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
   const bool cplx = t->lambda > 0.0;
   // S1-S3, once per (point, shift): u = r/N (IEEE division), y = u + Delta (wrap), t = y^2 (3 - 2y), w *= 6 y (1 - y),
   // ln t (table logarithm), 1/t (reciprocal)
-  const double per_point = n * (F_DIV + 2.0 + 4.0 + 4.0 + (cplx ? 16.0 + 8.0 : 18.0 + 6.0));
+  const double per_point = n * (F_DIV + 2.0 + 4.0 + 4.0 + 18.0 + 6.0);
   double per_sectors = 0.0;
   int64_t ncorners = 0;
   const int eU = std::abs(t->aU0), eF = std::abs(t->aF0);
@@ -106,13 +105,14 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
         }
       f += 2.0 * K;  // weight and accumulate
     } else {
-      // version-3 scheme (qmc_kernels3.cuh): real record 3, complex record 10 (complex product 6 + two FMAs)
+      // version-5 scheme (qmc_kernels5.cuh; the arithmetic of version 3): real record 3, complex record 10 (complex
+      // product 6 + two FMAs)
       auto pow_muls = [](int e) {
         int c = 0;
         for (int q = e; q > 1; q >>= 1) c += 1 + (q & 1);
         return (double)c;
       };
-      const double F_LOG2 = 16.0, F_CLOG3 = 3.0 + F_LOG2 + 1.0 + F_ATAN2;
+      const double F_LOG2 = 18.0, F_CLOG3 = 3.0 + F_LOG2 + 1.0 + F_ATAN2;  // 64-entry table logarithm of |a|^2, atan2
       int pos_of[QMC_MAXDIM], kk = 0;
       for (int j = 0; j < n; ++j) pos_of[j] = (s.alpha[j] == -1) ? kk++ : -1;
       int nprod_c = 0;  // complex product slots of the sector's chunk

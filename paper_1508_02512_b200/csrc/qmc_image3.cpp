@@ -102,7 +102,29 @@ bool localise(std::vector<Factors> &mono, size_t first, size_t count, int nslots
 
 }  // namespace
 
+namespace {
+void put32(std::vector<uint32_t> &v, uint32_t x) { v.push_back(x); }
+void putf64(std::vector<uint32_t> &v, double d) {
+  uint64_t b;
+  std::memcpy(&b, &d, 8);
+  v.push_back((uint32_t)b);
+  v.push_back((uint32_t)(b >> 32));
+}
+void pad4(std::vector<uint32_t> &v) {
+  while (v.size() % 4) v.push_back(0);
+}
+void put_rec(std::vector<uint32_t> &v, const Qmc2Rec &r) {
+  putf64(v, r.c);
+  v.push_back(r.s0);
+  v.push_back(r.s1);
+}
+}  // namespace
+
 int qmc_build_image3(qmc_tables *t) {
+  t->tab5.clear();
+  t->secoff5.clear();
+  t->prog5r.clear();
+  t->prog5c.clear();
   t->image3.clear();
   t->secoff3.clear();
   t->secend3.clear();
@@ -174,6 +196,12 @@ int qmc_build_image3(qmc_tables *t) {
     for (auto &q : pc.prog) { put(t->image3, (uint16_t)q.first); put(t->image3, (uint16_t)q.second); }
     while (t->image3.size() % 16) t->image3.push_back(0);
     ch.prog_bytes = (uint32_t)t->image3.size() - ch.prog_off;
+    std::vector<uint32_t> p5r, p5c;
+    for (auto &q : pr.prog) { put32(p5r, (uint32_t)q.first * T * 8u); put32(p5r, (uint32_t)q.second * T * 8u); }
+    pad4(p5r);
+    for (auto &q : pc.prog) { put32(p5c, (uint32_t)q.first * T * 16u); put32(p5c, (uint32_t)q.second * T * 16u); }
+    pad4(p5c);
+    const size_t tab5_mark = t->tab5.size();
     const uint32_t ONE_R = (uint32_t)(3 * n) * T * 8u, ONE_C = (uint32_t)n * T * 16u;
     auto rec_r = [&](double c, const Factors &f) {
       Qmc2Rec r;
@@ -256,9 +284,72 @@ int qmc_build_image3(qmc_tables *t) {
       for (const Qmc2Rec &r : rr) put(t->image3, r);
       for (const Qmc2Rec &r : rc) put(t->image3, r);
       t->secend3[si] = (uint32_t)t->image3.size();
+      {  // version-5 block of the same sector (layout: qmc_launch.h)
+        std::vector<uint32_t> &v = t->tab5;
+        if ((int)t->secoff5.size() <= si) t->secoff5.resize(si + 1, 0);
+        t->secoff5[si] = (uint32_t)(v.size() / 4);
+        const size_t b0 = v.size();
+        const uint32_t nlr = (uint32_t)((loc_r.size() + 1) / 2), nlc = (uint32_t)((loc_c.size() + 1) / 2);
+        put32(v, (uint32_t)s.nsing | ((uint32_t)h.nL0 << 8) | ((uint32_t)loc_r.size() << 16) | ((uint32_t)loc_c.size() << 24));
+        put32(v, 0);                // size of the block in words (patched below)
+        put32(v, 8 + nlr + nlc);    // first real record (G0)
+        put32(v, 0);
+        auto pack4 = [](const int8_t *a) {
+          return (uint32_t)(uint8_t)a[0] | ((uint32_t)(uint8_t)a[1] << 8) | ((uint32_t)(uint8_t)a[2] << 16) | ((uint32_t)(uint8_t)a[3] << 24);
+        };
+        put32(v, (uint32_t)h.sing_var[0] | ((uint32_t)h.sing_var[1] << 8) | ((uint32_t)h.sing_var[2] << 16) | ((uint32_t)h.sing_var[3] << 24));
+        put32(v, 0);
+        put32(v, pack4(h.alpha));
+        put32(v, pack4(h.alpha + 4));
+        put32(v, pack4(h.beta));
+        put32(v, pack4(h.beta + 4));
+        put32(v, 0);
+        put32(v, 0);
+        for (int q = 0; q < QMC_MAXSING; ++q) putf64(v, h.invbeta[q]);
+        for (int q = 0; q < QMC_MAXSING; ++q) putf64(v, h.betas[q]);
+        const size_t dir = v.size();
+        for (int q = 0; q < 4; ++q) put32(v, 0);  // corner directory (patched below)
+        for (auto &q : loc_r) { put32(v, (uint32_t)q.first * T * 8u); put32(v, (uint32_t)q.second * T * 8u); }
+        pad4(v);
+        for (auto &q : loc_c) { put32(v, (uint32_t)q.first * T * 16u); put32(v, (uint32_t)q.second * T * 16u); }
+        pad4(v);
+        for (int q = 0; q < 1 + h.nL0; ++q) put_rec(v, rr[q]);  // G0, L0
+        const Qmc2Rec empty_r = {0.0, ONE_R, ONE_R}, empty_c = {0.0, ONE_C, ONE_C};
+        for (int Z = 0; Z < ng; ++Z) {
+          v[dir + Z] = (uint32_t)((v.size() - b0) / 4);
+          // counts of the surviving records per polynomial, then the records: a monomial survives iff its group is
+          // disjoint from Z
+          std::vector<uint8_t> cz(npoly, 0);
+          std::vector<Qmc2Rec> zr, zc;
+          size_t ir = 1 + h.nL0, ic = 0;
+          for (int p = 0; p < npoly; ++p)
+            for (const Mono3 &m : polys[si][p]) {
+              const bool keep = (m.group & Z) == 0;
+              if (p < nderiv) {
+                if (keep) { zr.push_back(rr[ir]); ++cz[p]; }
+                ++ir;
+              } else {
+                if (keep) { zc.push_back(rc[ic]); ++cz[p]; }
+                ++ic;
+              }
+            }
+          for (int p = 0; p < npoly; p += 4) {
+            uint32_t w = 0;
+            for (int q = 0; q < 4 && p + q < npoly; ++q) w |= (uint32_t)cz[p + q] << (8 * q);
+            put32(v, w);
+          }
+          pad4(v);
+          for (const Qmc2Rec &r : zr) put_rec(v, r);
+          put_rec(v, empty_r);
+          for (const Qmc2Rec &r : zc) put_rec(v, r);
+          put_rec(v, empty_c);
+        }
+        v[b0 + 1] = (uint32_t)((v.size() - b0) / 4);
+      }
     }
     if (split) {
       t->image3.resize(ch.prog_off);
+      t->tab5.resize(tab5_mark);
       if (s1 - s0 == 1) return QMC_EUNSUPPORTED;
       const int mid = (s0 + s1) / 2;
       todo[w] = {s0, mid};
@@ -267,9 +358,13 @@ int qmc_build_image3(qmc_tables *t) {
       continue;
     }
     t->chunks3.push_back(ch);
+    t->prog5r.push_back(p5r);
+    t->prog5c.push_back(p5c);
     t->chunk3_nslots_c.push_back(pc.nslots);
     t->chunk3_max_local_c.push_back(max_local_c);
   }
   t->secoff3[nsec] = (uint32_t)t->image3.size();
+  t->secoff5.resize(nsec + 1, 0);
+  t->secoff5[nsec] = (uint32_t)(t->tab5.size() / 4);
   return QMC_OK;
 }

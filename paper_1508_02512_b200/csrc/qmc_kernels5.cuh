@@ -1,0 +1,470 @@
+// Evaluation kernel, version 5 (complex path: physical region, contour deformation), sm_100a.  Steps S1-S7 of DESIGN.md.
+//
+// The arithmetic of version 3 (qmc_kernels3.cuh: real slot table at the lattice point for the derivative polynomials of
+// F^, complex slot table over the deformed variables for U^(z), F^(z), Eq. 14 with its Jacobian determinant by LU, complex
+// table logarithms, product form folded over the singular variables) with the tables where version 4 keeps them: in the
+// kernel parameter block (constant bank 0; layout in qmc_launch.h).  Every table read is a uniform load, the record
+// loops run on the uniform datapath, and every corner of a sector owns a flat record stream (records needed by several
+// corners are duplicated by the table builder), walked with the next record's slot operands in flight.  The corner is
+// inlined inside a `for Z` loop with a uniform trip count (one copy of the corner code per number of singular
+// variables); its results go to compile-time registers through a uniform `switch (Z)`.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "qmc_kernels4.cuh"  // fast_log (64 x 8 table), fast_rcp, slot_at, u2d
+
+namespace qmc5 {
+
+using qmc2::Expo;
+using qmc4::fast_log;
+using qmc4::fast_rcp;
+using qmc4::slot_at;
+using qmc4::u2d;
+using qmcdev::cd;
+using qmcdev::cinv;
+using qmcdev::cnorm2;
+
+__device__ __forceinline__ double2 cslot_at(const unsigned char *__restrict__ sl, uint32_t off) {
+  return *reinterpret_cast<const double2 *>(sl + off);
+}
+static __device__ __noinline__ double atan2_lib(double y, double x) { return atan2(y, x); }
+// principal log; a negative real argument carries the -i0 of F -> F - i0: arg = -pi (R:C11)
+__device__ __forceinline__ cd clog5(cd a, const double2 *__restrict__ tabq) {
+  const double arg = (a.im == 0.0 && a.re < 0.0) ? -3.14159265358979323846 : atan2_lib(a.im, a.re);
+  return cd{0.5 * fast_log(cnorm2(a), tabq), arg};
+}
+template <int E>
+__device__ __forceinline__ cd cpow_c(cd x) {  // x^E, E >= 0 compile time
+  if (E == 0) return cd{1.0, 0.0};
+  if (E == 1) return x;
+  cd h = cpow_c<E / 2>(x);
+  h = h * h;
+  return (E & 1) ? h * x : h;
+}
+__device__ __forceinline__ int sext8(uint32_t w, int k) { return (int)(int8_t)((w >> (8 * k)) & 255u); }
+
+// W_Z and Lambda_Z of one corner.  Z (bit mask over the singular positions) is warp-uniform; `cw` = word offset of the
+// corner block in p.tab.
+template <int NDIM, int L, int NS>
+__device__ __forceinline__ void corner5(const Qmc5Launch &p, const uint32_t cw, const int Z, const uint32_t singvar,
+                                        const uint32_t alo, const uint32_t ahi, const uint32_t blo, const uint32_t bhi,
+                                        const uint32_t lcw, const uint32_t nlocal_c,
+                                        const double G0, const double L0, unsigned char *__restrict__ slr,
+                                        unsigned char *__restrict__ slc, const double2 *__restrict__ tabq, cd &Wout, cd &Lout,
+                                        unsigned &cntImF, unsigned &cntReU) {
+  constexpr int T = QMC2_THREADS, NDERIV = NDIM + NDIM * (NDIM + 1) / 2, NPOLY = NDERIV + 2, CW = (NPOLY + 15) / 16;
+  typedef Expo<NDIM, L> E;
+  uint32_t zv = 0;  // variables set to zero
+#pragma unroll
+  for (int k = 0; k < NS; ++k)
+    if (Z >> k & 1) zv |= 1u << ((singvar >> (8 * k)) & 255u);
+  uint32_t cnt[CW * 4];
+#pragma unroll
+  for (int q = 0; q < CW; ++q) {
+    const uint4 w = p.tab[cw + q];
+    cnt[4 * q] = w.x; cnt[4 * q + 1] = w.y; cnt[4 * q + 2] = w.z; cnt[4 * q + 3] = w.w;
+  }
+  const unsigned char *tb = reinterpret_cast<const unsigned char *>(p.tab);
+  uint32_t rwb = (cw + CW) * 16u;  // byte offset of the current record
+  // ---- S4: gradient and Hessian of F^ at tau: one software-pipelined stream of real records --------------------------
+  double dv[NDERIV];
+  {
+    uint2 ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);
+    double ra = slot_at(slr, ro.x), rb = slot_at(slr, ro.y);
+#pragma unroll
+    for (int q = 0; q < NDERIV; ++q) {
+      const uint32_t n = (cnt[q >> 2] >> (8 * (q & 3))) & 255u;
+      double acc = 0.0;
+#pragma unroll 1
+      for (uint32_t i = 0; i < n; ++i) {
+        const uint2 rc = *reinterpret_cast<const uint2 *>(tb + rwb);
+        const double v = ra * rb;
+        rwb += 16u;
+        ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);
+        ra = slot_at(slr, ro.x);
+        rb = slot_at(slr, ro.y);
+        acc = fma(u2d(rc.x, rc.y), v, acc);
+      }
+      dv[q] = acc;
+    }
+    rwb += 16u;  // the real sentinel
+  }
+  // rho_i, z_i, J = 1 + i B
+  cd rho[NDIM], J[NDIM][NDIM];
+#pragma unroll
+  for (int i = 0; i < NDIM; ++i) {
+    const bool inZ = (zv >> i & 1u) != 0;
+    const double tau = inZ ? 0.0 : slot_at(slr, i * T * 8);
+    rho[i] = cd{1.0, -p.lambda * (1.0 - tau) * dv[i]};
+    *reinterpret_cast<double2 *>(slc + i * T * 16) = make_double2(tau, tau * rho[i].im);  // z_i = tau rho_i
+#pragma unroll
+    for (int k = 0; k < NDIM; ++k) {
+      const bool kinZ = (zv >> k & 1u) != 0;
+      if (inZ || kinZ) {
+        J[i][k] = cd{(i == k) ? 1.0 : 0.0, 0.0};  // row / column of a Z variable: its rho cancels rho^-1 (alpha = -1)
+      } else {
+        const int a = i < k ? i : k, b = i < k ? k : i;  // Hessian entry (a <= b) in emission order
+        const double hik = dv[NDIM + a * NDIM - a * (a - 1) / 2 + (b - a)];
+        double bb = -p.lambda * tau * (1.0 - tau) * hik;
+        if (i == k) bb += -p.lambda * (1.0 - 2.0 * tau) * dv[i];
+        J[i][k] = cd{(i == k) ? 1.0 : 0.0, bb};
+      }
+    }
+  }
+  cd det = cd{1.0, 0.0};
+#pragma unroll
+  for (int col = 0; col < NDIM; ++col) {
+#pragma unroll
+    for (int r = col + 1; r < NDIM; ++r) {
+      if (cnorm2(J[r][col]) > cnorm2(J[col][col])) {
+#pragma unroll
+        for (int k = col; k < NDIM; ++k) {
+          cd tmp = J[r][k];
+          J[r][k] = J[col][k];
+          J[col][k] = tmp;
+        }
+        det = cd{-det.re, -det.im};
+      }
+    }
+    det = det * J[col][col];
+    if (col + 1 < NDIM) {
+      const cd ip = cinv(J[col][col]);
+#pragma unroll
+      for (int r = col + 1; r < NDIM; ++r) {
+        const cd f = J[r][col] * ip;
+#pragma unroll
+        for (int k = col + 1; k < NDIM; ++k) J[r][k] = J[r][k] - f * J[col][k];
+      }
+    }
+  }
+  // ---- S5: complex slot table over z, U^(z), F^(z) -----------------------------------------------------------------
+  for (uint32_t i = 0; i < p.nprog_c; i += 2) {
+    const uint4 pw = p.tab[p.prog_c_word + (i >> 1)];
+    {
+      const double2 a = cslot_at(slc, pw.x), b = cslot_at(slc, pw.y);
+      *reinterpret_cast<double2 *>(slc + p.first_prod_c_off + i * (T * 16)) = make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+    }
+    if (i + 1 < p.nprog_c) {
+      const double2 a = cslot_at(slc, pw.z), b = cslot_at(slc, pw.w);
+      *reinterpret_cast<double2 *>(slc + p.first_prod_c_off + (i + 1) * (T * 16)) = make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+    }
+  }
+  for (uint32_t i = 0; i < nlocal_c; i += 2) {  // sector-local complex products
+    const uint4 pw = p.tab[lcw + (i >> 1)];
+    {
+      const double2 a = cslot_at(slc, pw.x), b = cslot_at(slc, pw.y);
+      *reinterpret_cast<double2 *>(slc + p.local0_c_off + i * (T * 16)) = make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+    }
+    if (i + 1 < nlocal_c) {
+      const double2 a = cslot_at(slc, pw.z), b = cslot_at(slc, pw.w);
+      *reinterpret_cast<double2 *>(slc + p.local0_c_off + (i + 1) * (T * 16)) = make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+    }
+  }
+  cd UF[2];
+  {
+    uint2 ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);
+    double2 ra = cslot_at(slc, ro.x), rb = cslot_at(slc, ro.y);
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+      const uint32_t n = (cnt[(NDERIV + q) >> 2] >> (8 * ((NDERIV + q) & 3))) & 255u;
+      cd acc = cd{0.0, 0.0};
+#pragma unroll 1
+      for (uint32_t i = 0; i < n; ++i) {
+        const uint2 rc = *reinterpret_cast<const uint2 *>(tb + rwb);
+        const double vr = ra.x * rb.x - ra.y * rb.y, vi = ra.x * rb.y + ra.y * rb.x;
+        rwb += 16u;
+        ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);
+        ra = cslot_at(slc, ro.x);
+        rb = cslot_at(slc, ro.y);
+        const double c = u2d(rc.x, rc.y);
+        acc.re = fma(c, vr, acc.re);
+        acc.im = fma(c, vi, acc.im);
+      }
+      UF[q] = acc;
+    }
+  }
+  const cd Uv = UF[0], Fv = UF[1];
+  if (Fv.im > 0.0) ++cntImF;
+  if (!(Uv.re > 0.0)) ++cntReU;
+  // G_Z = G0 det J prod_{j notin Z} rho_j^alpha_j U^aU0 F^aF0 ;  Lambda_Z = aU1 ln U + aF1 ln F + sum_j beta_j ln rho_j + L0
+  cd num = cd{G0 * det.re, G0 * det.im}, den = cd{1.0, 0.0};
+  cd Lam = (double)E::aU1 * clog5(Uv, tabq) + (double)E::aF1 * clog5(Fv, tabq);
+  Lam.re += L0;
+#pragma unroll
+  for (int j = 0; j < NDIM; ++j) {
+    const bool inZ = (zv >> j & 1u) != 0;
+    const int a = sext8(j < 4 ? alo : ahi, j & 3), b = sext8(j < 4 ? blo : bhi, j & 3);
+    if (!inZ) {
+      if (a < 0) den = den * rho[j];
+      for (int q = 0; q < a; ++q) num = num * rho[j];
+    }
+    if (b) Lam = Lam + (double)b * clog5(rho[j], tabq);
+  }
+  if (E::aU0 > 0) num = num * cpow_c<(E::aU0 > 0 ? E::aU0 : 0)>(Uv);
+  if (E::aU0 < 0) den = den * cpow_c<(E::aU0 < 0 ? -E::aU0 : 0)>(Uv);
+  if (E::aF0 > 0) num = num * cpow_c<(E::aF0 > 0 ? E::aF0 : 0)>(Fv);
+  if (E::aF0 < 0) den = den * cpow_c<(E::aF0 < 0 ? -E::aF0 : 0)>(Fv);
+  Wout = num * cinv(den);
+  Lout = Lam;
+}
+
+template <int NS, int K>
+struct Ctx5 {
+  double invt[NS > 0 ? NS : 1], invbeta[NS > 0 ? NS : 1];
+  double cL[NS > 0 ? NS : 1][K > 1 ? K - 1 : 1];
+  cd W[1 << NS], Lam[1 << NS];  // index Z = set of singular positions set to zero
+};
+
+// fold of the singular variables with exact series windows (see qmc2::Fold2), complex
+template <int NS, int KMAX, int K, int LEVEL, int ZMASK>
+struct Fold5 {
+  static constexpr int LEN = NS - LEVEL + KMAX + __builtin_popcount(ZMASK) + 1;
+  static __device__ __forceinline__ void eval(const Ctx5<NS, K> &c, cd (&out)[LEN]) {
+    cd a[LEN - 1], b[LEN];
+    Fold5<NS, KMAX, K, LEVEL + 1, ZMASK>::eval(c, a);
+    Fold5<NS, KMAX, K, LEVEL + 1, ZMASK | (1 << LEVEL)>::eval(c, b);
+    const double it = c.invt[LEVEL], ib = c.invbeta[LEVEL];
+    cd d[LEN - 1];
+#pragma unroll
+    for (int i = 0; i < LEN - 1; ++i) d[i] = it * (a[i] - b[i]);
+    out[0] = ib * b[0];
+#pragma unroll
+    for (int i = 1; i < LEN; ++i) {
+      cd s = ib * b[i] + d[i - 1];
+#pragma unroll
+      for (int p = 1; p < i; ++p) s = s + c.cL[LEVEL][p] * d[i - 1 - p];
+      out[i] = s;
+    }
+  }
+};
+template <int NS, int KMAX, int K, int ZMASK>
+struct Fold5<NS, KMAX, K, NS, ZMASK> {
+  static constexpr int LEN = KMAX + __builtin_popcount(ZMASK) + 1;
+  static __device__ __forceinline__ void eval(const Ctx5<NS, K> &c, cd (&out)[LEN]) {
+    out[0] = c.W[ZMASK];
+#pragma unroll
+    for (int p = 1; p < LEN; ++p) out[p] = (1.0 / p) * (out[p - 1] * c.Lam[ZMASK]);
+  }
+};
+
+// one sector at one point: out[i] = coefficient of eps^(i - NS).  `o` = word offset of the sector block (uniform).
+template <int NDIM, int L, int NS, int KMAX>
+__device__ __forceinline__ void sector5(const Qmc5Launch &p, const uint32_t o, unsigned char *__restrict__ slr,
+                                        unsigned char *__restrict__ slc, const double2 *__restrict__ tabq,
+                                        cd (&out)[KMAX + NS + 1], unsigned &cntImF, unsigned &cntReU) {
+  constexpr int K = KMAX + NS + 1, NG = 1 << NS, T = QMC2_THREADS;
+  const uint4 h0 = p.tab[o], h1 = p.tab[o + 1], h2 = p.tab[o + 2];
+  const uint32_t nL0 = (h0.x >> 8) & 255u, nlocal_r = (h0.x >> 16) & 255u, nlocal_c = (h0.x >> 24) & 255u;
+  const uint32_t lrw = o + 8, lcw = lrw + ((nlocal_r + 1) >> 1);
+  for (uint32_t i = 0; i < nlocal_r; i += 2) {  // sector-local real products
+    const uint4 pw = p.tab[lrw + (i >> 1)];
+    *reinterpret_cast<double *>(slr + p.local0_r_off + i * (T * 8)) = slot_at(slr, pw.x) * slot_at(slr, pw.y);
+    if (i + 1 < nlocal_r) *reinterpret_cast<double *>(slr + p.local0_r_off + (i + 1) * (T * 8)) = slot_at(slr, pw.z) * slot_at(slr, pw.w);
+  }
+  uint32_t rw = o + h0.z;
+  const double G0 = qmc4::rec_val(p.tab[rw], slr);
+  ++rw;
+  double L0 = 0.0;
+#pragma unroll 2
+  for (uint32_t i = 0; i < nL0; ++i) L0 = qmc4::rec_fma(p.tab[rw + i], slr, L0);
+  Ctx5<NS, K> c;
+  const uint4 cdir = p.tab[o + 7];
+  const uint32_t cws[4] = {cdir.x, cdir.y, cdir.z, cdir.w};
+#pragma unroll 1
+  for (int Z = 0; Z < NG; ++Z) {
+    cd W, Lam;
+    const uint32_t cw = o + (Z == 0 ? cws[0] : Z == 1 ? cws[1] : Z == 2 ? cws[2] : cws[3]);
+    corner5<NDIM, L, NS>(p, cw, Z, h1.x, h1.z, h1.w, h2.x, h2.y, lcw, nlocal_c, G0, L0, slr, slc, tabq, W, Lam, cntImF, cntReU);
+#pragma unroll
+    for (int q = 0; q < NG; ++q)
+      if (Z == q) {  // warp-uniform: the results land in compile-time registers
+        c.W[q] = W;
+        c.Lam[q] = Lam;
+      }
+  }
+  if (NS > 0) {
+    const uint4 ib01 = p.tab[o + 3], ib23 = p.tab[o + 4], b01 = p.tab[o + 5], b23 = p.tab[o + 6];
+    const double ibv[4] = {u2d(ib01.x, ib01.y), u2d(ib01.z, ib01.w), u2d(ib23.x, ib23.y), u2d(ib23.z, ib23.w)};
+    const double bv[4] = {u2d(b01.x, b01.y), u2d(b01.z, b01.w), u2d(b23.x, b23.y), u2d(b23.z, b23.w)};
+#pragma unroll
+    for (int k = 0; k < NS; ++k) {
+      const uint32_t j = (h1.x >> (8 * k)) & 255u;
+      c.invt[k] = slot_at(slr, (2 * NDIM + j) * (T * 8));
+      c.invbeta[k] = ibv[k];
+      const double Lk = bv[k] * slot_at(slr, (NDIM + j) * (T * 8));
+      c.cL[k][0] = 1.0;
+#pragma unroll
+      for (int q = 1; q < K - 1; ++q) c.cL[k][q] = c.cL[k][q - 1] * Lk * (1.0 / q);
+    }
+  }
+  Fold5<NS, KMAX, K, 0, 0>::eval(c, out);
+}
+
+__device__ __forceinline__ bool finite_hi(cd v) {
+  return (__double2hiint(v.re) & 0x7ff00000) != 0x7ff00000 && (__double2hiint(v.im) & 0x7ff00000) != 0x7ff00000;
+}
+
+}  // namespace qmc5
+
+// partial layout: fused [run][shift][slice][NACC][2], persec [sector row][shift][slice][NACC][2]
+template <int NDIM, int L, int KMAX>
+__global__ void __launch_bounds__(QMC2_THREADS, (NDIM <= 4 ? 2 : 1)) qmc5_eval_kernel(const __grid_constant__ Qmc5Launch p) {
+  using namespace qmc5;
+  constexpr int NACC = QMC_MAXSING + KMAX + 1;
+  constexpr int SMAX = NDIM < QMC3_MAXSING ? NDIM : QMC3_MAXSING;
+  constexpr int T = QMC2_THREADS;
+
+  extern __shared__ __align__(16) unsigned char smem[];
+  const int tid = threadIdx.x;
+  double2 *logtab = reinterpret_cast<double2 *>(smem);
+  size_t o = (size_t)QMC4_LOG_ENTRIES * QMC4_LOG_COPIES * 16;
+  double *shf = reinterpret_cast<double *>(smem + o);
+  o += (((size_t)p.m * NDIM * 8) + 15) & ~(size_t)15;
+  double *scratch = reinterpret_cast<double *>(smem + o);
+  o += (T / 32) * 8;
+  double *slots_r = reinterpret_cast<double *>(smem + o);
+  o += (size_t)p.max_nslots_r * T * 8;
+  double2 *slots_c = reinterpret_cast<double2 *>(smem + o);
+  o += (size_t)p.max_nslots_c * T * 16;
+  double *sacc = reinterpret_cast<double *>(smem + o);  // persec: [nsec][NACC*2][T]
+  unsigned char *slr = reinterpret_cast<unsigned char *>(slots_r + tid);
+  unsigned char *slc = reinterpret_cast<unsigned char *>(slots_c + tid);
+  const double2 *tabq = logtab + (tid & (QMC4_LOG_COPIES - 1));
+
+  for (int i = tid; i < QMC4_LOG_ENTRIES * QMC4_LOG_COPIES; i += T)
+    logtab[i] = reinterpret_cast<const double2 *>(p.logtab)[i / QMC4_LOG_COPIES];
+  for (int i = tid; i < p.m * NDIM; i += T) shf[i] = p.shifts[i];
+  slots_r[3 * NDIM * T + tid] = 1.0;                     // the constant slots
+  slots_c[NDIM * T + tid] = make_double2(1.0, 0.0);
+  __syncthreads();
+
+  const uint32_t N = p.N;
+  const double dN = (double)N;
+  const uint32_t stride = (uint32_t)p.nslices * T;
+  uint32_t dz[NDIM];
+#pragma unroll
+  for (int j = 0; j < NDIM; ++j) dz[j] = (uint32_t)(((uint64_t)stride * p.zeff[j]) % N);
+
+  unsigned cntImF = 0, cntReU = 0, cntNonFinite = 0, cntBoundary = 0;
+  const int kap = blockIdx.y;  // one block = one shift vector (see qmc_kernels4.cuh)
+  {
+    cd acc[NACC];
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) acc[a] = cd{0.0, 0.0};
+    if (p.persec)
+      for (int i = 0; i < p.nsec * NACC * 2; ++i) sacc[(size_t)i * T + tid] = 0.0;
+
+    const uint32_t c0 = (uint32_t)blockIdx.x * T;
+    uint32_t r[NDIM];
+#pragma unroll
+    for (int j = 0; j < NDIM; ++j) r[j] = (uint32_t)((p.off[j] + (uint64_t)(c0 + tid) * p.zeff[j]) % N);
+
+    for (uint32_t cb = c0; cb < p.count; cb += stride) {  // uniform trip count; dead threads carry the weight 0
+      const bool valid = cb + tid < p.count;
+      double w = 1.0;
+      bool inside = true;
+#pragma unroll
+      for (int j = 0; j < NDIM; ++j) {
+        double u = (double)r[j] / dN;
+        double y = u + shf[kap * NDIM + j];
+        if (y >= 1.0) y -= 1.0;
+        double tj;
+        if (p.transform == 0) {
+          tj = y * y * (3.0 - 2.0 * y);
+          w *= 6.0 * y * (1.0 - y);
+        } else {
+          tj = 1.0 - fabs(2.0 * y - 1.0);
+        }
+        if (!(y > 0.0) || !(tj > 0.0)) {
+          inside = false;
+          tj = 0.5;
+        }
+        reinterpret_cast<double *>(slr)[j * T] = tj;
+        reinterpret_cast<double *>(slr)[(NDIM + j) * T] = fast_log(tj, tabq);
+        reinterpret_cast<double *>(slr)[(2 * NDIM + j) * T] = fast_rcp(tj);
+        uint32_t rn = r[j] + dz[j];
+        r[j] = rn >= N ? rn - N : rn;
+      }
+      if (valid && !inside && p.count_boundary) ++cntBoundary;
+      const bool live = valid && inside;
+      if (!live) w = 0.0;
+      for (uint32_t i = 0; i < p.nprog_r; i += 2) {  // chunk-wide real product slots
+        const uint4 pw = p.tab[p.prog_r_word + (i >> 1)];
+        *reinterpret_cast<double *>(slr + p.first_prod_r_off + i * (T * 8)) = slot_at(slr, pw.x) * slot_at(slr, pw.y);
+        if (i + 1 < p.nprog_r)
+          *reinterpret_cast<double *>(slr + p.first_prod_r_off + (i + 1) * (T * 8)) = slot_at(slr, pw.z) * slot_at(slr, pw.w);
+      }
+      for (int si = 0; si < p.nsec; ++si) {
+        const uint32_t so = p.secw[si];
+        const uint4 h0 = p.tab[so];
+        unsigned dImF = 0, dReU = 0;
+#define QMC5_CASE(NS_)                                                                                       \
+  case NS_: {                                                                                                \
+    if (NS_ <= SMAX) {                                                                                       \
+      constexpr int NSC = NS_ <= SMAX ? NS_ : 0, KK = KMAX + NSC + 1;                                        \
+      cd res[KK];                                                                                            \
+      sector5<NDIM, L, NSC, KMAX>(p, so, slr, slc, tabq, res, dImF, dReU);                                   \
+      bool fin = true;                                                                                       \
+      _Pragma("unroll") for (int i = 0; i < KK; ++i) fin = fin && finite_hi(res[i]);                         \
+      cntNonFinite += (live && !fin) ? 1u : 0u;                                                              \
+      if (!p.persec) {                                                                                       \
+        _Pragma("unroll") for (int i = 0; i < KK; ++i) if (fin) {                                            \
+          acc[QMC_MAXSING - NSC + i].re = fma(w, res[i].re, acc[QMC_MAXSING - NSC + i].re);                  \
+          acc[QMC_MAXSING - NSC + i].im = fma(w, res[i].im, acc[QMC_MAXSING - NSC + i].im);                  \
+        }                                                                                                    \
+      } else {                                                                                               \
+        double *sa = sacc + ((size_t)si * NACC + (QMC_MAXSING - NSC)) * 2 * T + tid;                         \
+        _Pragma("unroll") for (int i = 0; i < KK; ++i) if (fin) {                                            \
+          sa[(size_t)(2 * i) * T] += w * res[i].re;                                                          \
+          sa[(size_t)(2 * i + 1) * T] += w * res[i].im;                                                      \
+        }                                                                                                    \
+      }                                                                                                      \
+    }                                                                                                        \
+  } break;
+        switch (h0.x & 255u) {
+          QMC5_CASE(0)
+          QMC5_CASE(1)
+          QMC5_CASE(2)
+          default:
+            break;
+        }
+#undef QMC5_CASE
+        if (live) {  // the contour counters tally evaluated points only
+          cntImF += dImF;
+          cntReU += dReU;
+        }
+      }
+    }
+
+    if (!p.persec) {
+      double *dst = p.partial + (((size_t)p.out_row * p.m + kap) * p.max_slices + blockIdx.x) * (NACC * 2);
+#pragma unroll
+      for (int a = 0; a < NACC; ++a) {
+        double sr = qmcdev::block_sum(acc[a].re, scratch);
+        double si = qmcdev::block_sum(acc[a].im, scratch);
+        if (tid == 0) {
+          dst[2 * a] = sr;
+          dst[2 * a + 1] = si;
+        }
+      }
+    } else {
+      for (int si = 0; si < p.nsec; ++si) {
+        double *dst = p.partial + (((size_t)(p.out_row + p.secrow[si]) * p.m + kap) * p.max_slices + blockIdx.x) * (NACC * 2);
+        for (int a = 0; a < NACC * 2; ++a) {
+          double v = qmcdev::block_sum(sacc[((size_t)si * NACC * 2 + a) * T + tid], scratch);
+          if (tid == 0) dst[a] = v;
+        }
+      }
+    }
+  }
+
+  unsigned c4[4] = {cntImF, cntReU, cntNonFinite, cntBoundary};
+#pragma unroll
+  for (int qq = 0; qq < 4; ++qq) {
+    unsigned v = c4[qq];
+#pragma unroll
+    for (int o2 = 16; o2 > 0; o2 >>= 1) v += __shfl_down_sync(0xffffffffu, v, o2);
+    if ((tid & 31) == 0 && v) atomicAdd(p.counters + qq, (unsigned long long)v);
+  }
+}

@@ -109,3 +109,39 @@ static_assert(sizeof(Qmc4Launch) <= 32764, "kernel parameter limit");
 cudaError_t qmc4_kernel_prepare(int ndim, int loops, int kmax, size_t smem, int *blocks_per_sm);
 cudaError_t qmc4_kernel_launch(int ndim, int loops, int kmax, dim3 grid, size_t smem, cudaStream_t st, const Qmc4Launch &p);
 bool qmc4_kernel_available(int ndim, int loops, int kmax);
+
+// ---- version 5 (complex path, tables in the kernel-parameter constant bank) ---------------------------------------
+// The complex-path counterpart of version 4: one launch = one run of sectors of one chunk, grid = (slices, shifts).
+// Layout of `tab` (16-byte words): [prog_r_word ..) real slot program, [prog_c_word ..) complex slot program, each
+// {u32 a_off, u32 b_off} byte offsets into the thread's real (8-byte entries) resp. complex (16-byte entries) column,
+// two per word; then the sector blocks (word offsets relative to the block):
+//   w0 = {nsing | nL0 << 8 | nlocal_r << 16 | nlocal_c << 24, nwords, first real record (G0), 0}
+//   w1 = {variable index of the singular positions (u8 x 4), 0, alpha[0..3] (i8 x 4), alpha[4..7]}
+//   w2 = {beta[0..3] (i8 x 4), beta[4..7], 0, 0}      w3,w4 = 1/beta of the singular positions (f64 x 4)      w5,w6 = beta (f64 x 4)
+//   w7 = word offsets of the corner blocks Z = 0..3
+//   w8.. = local real program, local complex program (each padded to a word), then records [G0][L0 x nL0]
+//   corner block Z: u8 counts[npoly] (npoly = n + n(n+1)/2 + 2: F_i, F_ik (i <= k), U, F; padded to a word) of the
+//     records that survive at the corner (monomials free of the variables of Z), then the real records of the
+//     derivative polynomials, a real sentinel, the complex records of U^ and F^, a complex sentinel.
+//   A record is duplicated into every corner block that needs it: each corner is one flat stream without skips.
+struct Qmc5Launch {
+  const double *logtab;          // device: 64 x {1/c, -ln(1/c)}
+  const double *shifts;
+  double *partial;               // [row][shift][max_slices][NACC][2]
+  unsigned long long *counters;
+  uint32_t N, count;
+  uint32_t zeff[QMC_MAXDIM], off[QMC_MAXDIM];
+  int32_t m, transform, persec, max_slices;
+  int32_t nsec, out_row, count_boundary, nslices;
+  uint32_t nprog_r, prog_r_word, first_prod_r_off, local0_r_off;  // *_off: byte offsets in the real column
+  uint32_t nprog_c, prog_c_word, first_prod_c_off, local0_c_off;  // ... in the complex column
+  uint32_t max_nslots_r, max_nslots_c, pad0, pad1;
+  double lambda;
+  uint16_t secw[QMC4_MAX_SEC];
+  uint16_t secrow[QMC4_MAX_SEC];
+  uint4 tab[QMC4_TAB_WORDS];
+};
+static_assert(sizeof(Qmc5Launch) <= 32764, "kernel parameter limit");
+cudaError_t qmc5_kernel_prepare(int ndim, int loops, int kmax, size_t smem, int *blocks_per_sm);
+cudaError_t qmc5_kernel_launch(int ndim, int loops, int kmax, dim3 grid, size_t smem, cudaStream_t st, const Qmc5Launch &p);
+bool qmc5_kernel_available(int ndim, int loops, int kmax);

@@ -134,6 +134,9 @@ struct qmc_tables {
   std::vector<uint32_t> secoff4;    // [n_sectors + 1] offsets into tab4 in 16-byte words
   std::vector<std::vector<uint32_t>> prog4;  // per chunk: slot program {a_off, b_off} byte offsets, padded to 16 bytes
   double logtab4[128] = {0};        // 64 x {1/c_i, -ln(1/c_i)}
+  // version 5 tables (complex path; same chunks and slot programs as version 3, laid out for the constant bank)
+  std::vector<uint32_t> tab5, secoff5;             // sector blocks (32-bit words) and their offsets in 16-byte words
+  std::vector<std::vector<uint32_t>> prog5r, prog5c;  // per chunk: real / complex slot programs {a_off, b_off}
   void *side_streams[8] = {nullptr};  // cudaStream_t: the launches of one integration are spread over these
   void *side_events[9] = {nullptr};   // cudaEvent_t: fork + one join per side stream
   // version 3 image (complex path only)
