@@ -282,7 +282,8 @@ int qmc_build_image2(qmc_tables *t) {
             ri += cnt;
           }
         for (const Qmc2Rec &r : extra) put_rec(v, r);
-        put_rec(v, empty);  // sentinel: the kernel requests one record past the last extra one
+        put_rec(v, empty);  // sentinels: the kernel requests operands one record and offsets two records past the last
+        put_rec(v, empty);
         v[b0 + 1] = (uint32_t)((v.size() - b0) / 4);
       }
     }

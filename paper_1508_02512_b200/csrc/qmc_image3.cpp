@@ -341,7 +341,9 @@ int qmc_build_image3(qmc_tables *t) {
           pad4(v);
           for (const Qmc2Rec &r : zr) put_rec(v, r);
           put_rec(v, empty_r);
+          put_rec(v, empty_r);  // the kernel requests offsets two records ahead
           for (const Qmc2Rec &r : zc) put_rec(v, r);
+          put_rec(v, empty_c);
           put_rec(v, empty_c);
         }
         v[b0 + 1] = (uint32_t)((v.size() - b0) / 4);

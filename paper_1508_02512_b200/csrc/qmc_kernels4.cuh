@@ -118,6 +118,7 @@ __device__ __forceinline__ void sector4(const Qmc4Launch &p, const uint32_t o, u
     uint32_t rwb = rw * 16u;  // byte offset of the current record: {f64 c | u32 off0, u32 off1}
     uint2 ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);
     double ra = slot_at(sl, ro.x), rb = slot_at(sl, ro.y);
+    ro = *reinterpret_cast<const uint2 *>(tb + rwb + 24);  // offsets run TWO records ahead, operands one (two sentinels)
     constexpr int NW = (NC + 3) / 4, GW = NC < 4 ? NC : 4;  // count words per polynomial, groups per word
 #pragma unroll
     for (int q = 0; q < 2 * NW; ++q) {
@@ -133,9 +134,9 @@ __device__ __forceinline__ void sector4(const Qmc4Launch &p, const uint32_t o, u
             const uint2 rc = *reinterpret_cast<const uint2 *>(tb + rwb);
             const double v = ra * rb;
             rwb += 16u;
-            ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);
             ra = slot_at(sl, ro.x);
             rb = slot_at(sl, ro.y);
+            ro = *reinterpret_cast<const uint2 *>(tb + rwb + 24);
             accg = fma(u2d(rc.x, rc.y), v, accg);
           }
           if (q < NW) PU[gg] = accg; else PF[gg] = accg;

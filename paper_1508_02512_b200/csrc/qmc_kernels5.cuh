@@ -70,8 +70,11 @@ __device__ __forceinline__ void corner5(const Qmc5Launch &p, const uint32_t cw, 
   // ---- S4: gradient and Hessian of F^ at tau: one software-pipelined stream of real records --------------------------
   double dv[NDERIV];
   {
+    // offsets two records ahead (uniform registers), operands one record ahead: neither the uniform load nor the LDS
+    // sits on the critical path of an iteration (the block ends with TWO sentinel records)
     uint2 ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);
     double ra = slot_at(slr, ro.x), rb = slot_at(slr, ro.y);
+    ro = *reinterpret_cast<const uint2 *>(tb + rwb + 24);
 #pragma unroll
     for (int q = 0; q < NDERIV; ++q) {
       const uint32_t n = (cnt[q >> 2] >> (8 * (q & 3))) & 255u;
@@ -81,14 +84,14 @@ __device__ __forceinline__ void corner5(const Qmc5Launch &p, const uint32_t cw, 
         const uint2 rc = *reinterpret_cast<const uint2 *>(tb + rwb);
         const double v = ra * rb;
         rwb += 16u;
-        ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);
         ra = slot_at(slr, ro.x);
         rb = slot_at(slr, ro.y);
+        ro = *reinterpret_cast<const uint2 *>(tb + rwb + 24);
         acc = fma(u2d(rc.x, rc.y), v, acc);
       }
       dv[q] = acc;
     }
-    rwb += 16u;  // the real sentinel
+    rwb += 32u;  // the two real sentinels
   }
   // rho_i, z_i, J = 1 + i B
   cd rho[NDIM], J[NDIM][NDIM];
@@ -165,6 +168,7 @@ __device__ __forceinline__ void corner5(const Qmc5Launch &p, const uint32_t cw, 
   {
     uint2 ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);
     double2 ra = cslot_at(slc, ro.x), rb = cslot_at(slc, ro.y);
+    ro = *reinterpret_cast<const uint2 *>(tb + rwb + 24);
 #pragma unroll
     for (int q = 0; q < 2; ++q) {
       const uint32_t n = (cnt[(NDERIV + q) >> 2] >> (8 * ((NDERIV + q) & 3))) & 255u;
@@ -174,9 +178,9 @@ __device__ __forceinline__ void corner5(const Qmc5Launch &p, const uint32_t cw, 
         const uint2 rc = *reinterpret_cast<const uint2 *>(tb + rwb);
         const double vr = ra.x * rb.x - ra.y * rb.y, vi = ra.x * rb.y + ra.y * rb.x;
         rwb += 16u;
-        ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);
         ra = cslot_at(slc, ro.x);
         rb = cslot_at(slc, ro.y);
+        ro = *reinterpret_cast<const uint2 *>(tb + rwb + 24);
         const double c = u2d(rc.x, rc.y);
         acc.re = fma(c, vr, acc.re);
         acc.im = fma(c, vi, acc.im);

@@ -84,7 +84,7 @@ cudaError_t qmc_kernel_launch(int ndim, int kmax, int flavor, dim3 grid, size_t 
 //     w7 = extra records per group of U^ (u8 x 16)      w8 = the same for F^
 //     w9.. = local program: nlocal x {u32 a_off, u32 b_off}, padded to a word
 //     records {f64 c, u32 off0, u32 off1}: [G0][L0 x nL0][first record of every group of U^: 2^nsing, c = 0 if the
-//     group is empty][the same for F^][extra records of U^ by group][extra records of F^ by group][sentinel, c = 0]
+//     group is empty][the same for F^][extra records of U^ by group][extra records of F^ by group][two sentinels, c = 0]
 #define QMC4_TAB_WORDS 1808  // 28 928 bytes of tables per launch (kernel parameters are limited to 32 764 bytes)
 #define QMC4_MAX_SEC 160     // sectors per launch
 #define QMC4_LOG_ENTRIES 64
@@ -122,7 +122,7 @@ bool qmc4_kernel_available(int ndim, int loops, int kmax);
 //   w8.. = local real program, local complex program (each padded to a word), then records [G0][L0 x nL0]
 //   corner block Z: u8 counts[npoly] (npoly = n + n(n+1)/2 + 2: F_i, F_ik (i <= k), U, F; padded to a word) of the
 //     records that survive at the corner (monomials free of the variables of Z), then the real records of the
-//     derivative polynomials, a real sentinel, the complex records of U^ and F^, a complex sentinel.
+//     derivative polynomials, two real sentinels, the complex records of U^ and F^, two complex sentinels.
 //   A record is duplicated into every corner block that needs it: each corner is one flat stream without skips.
 struct Qmc5Launch {
   const double *logtab;          // device: 64 x {1/c, -ln(1/c)}
