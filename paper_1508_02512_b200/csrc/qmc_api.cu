@@ -1308,6 +1308,15 @@ int qmc_tables_describe(const qmc_tables *t, char *buf, size_t len) {
                   ch.sec_begin, ch.sec_end, ch.nslots, ch.prog_bytes, t->secend2[ch.sec_end - 1] - t->secoff2[ch.sec_begin], nrec, two, nloc, ch.cost);
     o += line;
   }
+  for (size_t c = 0; c < t->chunks3.size(); ++c) {  // complex path
+    const Qmc2Chunk &ch = t->chunks3[c];
+    std::snprintf(line, sizeof line,
+                  "complex chunk %zu: sectors [%d,%d) real slots %d (+%d local) complex slots %d (+%d local) tables %u B (version 5: %u B) cost %.0f\n",
+                  c, ch.sec_begin, ch.sec_end, ch.nslots, ch.max_local, t->chunk3_nslots_c[c], t->chunk3_max_local_c[c],
+                  t->secend3[ch.sec_end - 1] - t->secoff3[ch.sec_begin],
+                  t->secoff5.empty() ? 0u : (t->secoff5[ch.sec_end] - t->secoff5[ch.sec_begin]) * 16u, ch.cost);
+    o += line;
+  }
   std::snprintf(buf, len, "%s", o.c_str());
   return QMC_OK;
 }

@@ -198,3 +198,22 @@ def test_async_launch_resident_inputs_and_fetch():
     d = dev.cpu().numpy()
     assert np.array_equal(d[..., 0] + 1j * d[..., 1], ref.shift_totals)
     assert r.h2d_bytes < ref.h2d_bytes and r.d2h_bytes > 0 and r.eval_kernel_ms > 0
+
+
+def test_complex_path_tables_launch_splits_and_local_slots(monkeypatch):
+    """Complex-path tables (version 5): small chunks (several launches per step, sector ranges that straddle them) and
+    slot budgets small enough to force sector-local real and complex product slots (QMC3_* are read by qmc_prepare)."""
+    wl = qi.nonplanar_vertex()
+    t = q.qmc_prepare(wl, lam=wl.lam)
+    n0 = len(t.describe().splitlines())
+    monkeypatch.setenv("QMC3_CHUNK_BYTES", "6000")
+    monkeypatch.setenv("QMC3_SLOTS_R", "26")
+    monkeypatch.setenv("QMC3_SLOTS_C", "10")
+    t2 = q.qmc_prepare(wl, lam=wl.lam)
+    d2 = t2.describe()
+    assert len(d2.splitlines()) > n0 and "local) complex slots 10 (+" in d2 and "(+0 local) tables" not in d2.splitlines()[1]
+    r, f, *_ = parity(wl, 16381, 2, sectors=(3, 31))
+    assert f.kernel_launches - 2 >= 3
+    monkeypatch.delenv("QMC3_CHUNK_BYTES")
+    monkeypatch.delenv("QMC3_SLOTS_R")
+    monkeypatch.delenv("QMC3_SLOTS_C")
