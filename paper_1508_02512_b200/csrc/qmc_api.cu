@@ -16,7 +16,6 @@
 #include "qmc_tables.h"
 
 #define QMC_MAX_BLOCKS 592  // upper bound of gridDim.x used for workspace sizing (148 SMs x 4)
-#define QMC2_MAX_WORK 8192  // blocks of one version-2 launch
 #define QMC_NCAND 64        // Korobov candidates of the P_2 search
 #define QMC_P2_BLOCKS 296
 
@@ -154,7 +153,7 @@ uint64_t splitmix64(uint64_t &state) {
 uint64_t mulmod(uint64_t a, uint64_t b, uint64_t n) { return (uint64_t)(((unsigned __int128)a * b) % n); }
 
 struct DevLayout {
-  size_t image, secoff, image2, secoff2, image3, secoff3, logtab, logtab4, work, shifts, counters, out, stat, partial, p2z, p2partial, total;
+  size_t image, secoff, logtab4, shifts, counters, out, stat, partial, p2z, p2partial, total;
 };
 
 DevLayout layout(const qmc_tables *t, int m) {
@@ -163,13 +162,7 @@ DevLayout layout(const qmc_tables *t, int m) {
   size_t o = 0;
   L.image = o; o += align256(t->image.size());
   L.secoff = o; o += align256((nsec + 1) * 4);
-  L.image2 = o; o += align256(t->image2.size());
-  L.secoff2 = o; o += align256((nsec + 1) * 4);
-  L.image3 = o; o += align256(t->image3.size());
-  L.secoff3 = o; o += align256((nsec + 1) * 4);
-  L.logtab = o; o += align256(sizeof t->logtab);
   L.logtab4 = o; o += align256(sizeof t->logtab4);
-  L.work = o; o += align256((size_t)QMC2_MAX_WORK * sizeof(Qmc2Work));
   L.shifts = o; o += align256((size_t)m * QMC_MAXDIM * 8);
   L.counters = o; o += 256;
   L.out = o; o += align256(nsec * QMC_NACC_MAX * 2 * (size_t)m * 8);
@@ -247,125 +240,6 @@ void mean_err(const double *v, size_t stride, int m, double *mean, double *err) 
   }
   *mean = q;
   *err = std::sqrt(d2 / ((double)m * (m - 1)));
-}
-
-// ---- version-2 launch (real path): work items = runs of sectors of one chunk ------------------------------------
-int launch_v2(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t st, uint64_t N, int m, int sb, int se,
-              bool persec, uint64_t ibeg, uint64_t istep, uint64_t icount, const uint64_t *z, int sms, int smem_optin,
-              int *gx_out, int *rows_out, size_t *h2d, cudaError_t *ce_out) {
-  const int n = t->n, nacc = QMC_MAXSING + t->kmax + 1, T = QMC2_THREADS;
-  uint32_t prog_cap = 0;
-  int max_nslots = 0;
-  for (const Qmc2Chunk &c : t->chunks)
-    if (c.sec_end > sb && c.sec_begin < se) {
-      prog_cap = std::max(prog_cap, c.prog_bytes);
-      max_nslots = std::max(max_nslots, c.nslots + c.max_local);
-    }
-  const size_t budget = (size_t)smem_optin - 1024;
-  const size_t fixed = prog_cap + 16 + (((size_t)m * n * 8 + 15) & ~(size_t)15) + (T / 32) * 8 + 128 * 16 + (size_t)max_nslots * T * 8;
-  const size_t accbytes = persec ? (size_t)nacc * T * 8 : 0;
-  std::vector<Qmc2Work> runs;
-  std::vector<double> run_cost;
-  double total_cost = 0.0;
-  uint32_t sec_cap = 0;
-  int max_nsec = 0;
-  for (const Qmc2Chunk &c : t->chunks) {
-    int a = std::max(sb, c.sec_begin);
-    const int e = std::min(se, c.sec_end);
-    while (a < e) {
-      int b = a;  // grow the run while it fits the shared-memory budget
-      while (b < e) {
-        const size_t bytes = t->secend2[b] - t->secoff2[a];
-        const size_t need = fixed + bytes + (((size_t)(b + 1 - a + 1) * 4 + 15) & ~(size_t)15) + accbytes * (b + 1 - a);
-        if (need > budget) break;
-        ++b;
-      }
-      if (b == a) return QMC_ENOMEM;
-      Qmc2Work w;
-      std::memset(&w, 0, sizeof w);
-      w.prog_off = c.prog_off;
-      w.prog_bytes = c.prog_bytes;
-      w.sec_off = t->secoff2[a];
-      w.sec_bytes = t->secend2[b - 1] - t->secoff2[a];
-      w.s0 = a;
-      w.nsec = b - a;
-      w.out_row = persec ? a - sb : (int)runs.size();
-      w.count_boundary = runs.empty() ? 1 : 0;
-      sec_cap = std::max(sec_cap, w.sec_bytes);
-      max_nsec = std::max(max_nsec, w.nsec);
-      double cst = 0.0;
-      for (int s = a; s < b; ++s) cst += t->sec_cost[s];
-      run_cost.push_back(cst);
-      total_cost += cst;
-      runs.push_back(w);
-      a = b;
-    }
-  }
-  const int nitems = (int)runs.size();
-  const size_t smem = fixed + sec_cap + (((size_t)(max_nsec + 1) * 4 + 15) & ~(size_t)15) + accbytes * max_nsec;
-  int bps = 0;
-  CUDA_OK(qmc2_kernel_prepare(n, t->L, t->kmax, smem, &bps));
-  if (bps < 1) return QMC_ECUDA;
-  // slices per run in proportion to its modelled cost: about `waves` blocks of equal cost per resident block slot
-  int waves = 16;  // measured (profiles/r01d_waves.md): short blocks interleave better than one long block per slot
-  if (const char *e = std::getenv("QMC2_WAVES")) waves = std::max(1, std::atoi(e));
-  const long long max_slices_pts = std::max<long long>(1, (long long)((icount + T - 1) / T));
-  const double nblocks_target = (double)waves * sms * bps;
-  std::vector<Qmc2Work> work;
-  int max_slices = 1;
-  for (int i = 0; i < nitems; ++i) {
-    long long ns = (long long)(nblocks_target * run_cost[i] / total_cost + 0.5);
-    ns = std::max<long long>(1, std::min<long long>({ns, (long long)QMC_MAX_BLOCKS, max_slices_pts}));
-    max_slices = std::max(max_slices, (int)ns);
-    for (int sidx = 0; sidx < (int)ns; ++sidx) {
-      Qmc2Work w = runs[i];
-      w.slice = sidx;
-      w.nslices = (int)ns;
-      work.push_back(w);
-    }
-  }
-  if (work.size() > QMC2_MAX_WORK) return QMC_ENOMEM;
-  // upload the work list unless the identical list is already there
-  const uint64_t key = ((uint64_t)sb << 40) ^ ((uint64_t)se << 20) ^ (persec ? 1u : 0u) ^ ((uint64_t)m << 50) ^ ((uint64_t)icount << 1) ^
-                       ((uint64_t)waves << 58);
-  if (!(t->work_ws == ws && t->work_key == key)) {
-    t->work_host.assign(reinterpret_cast<const uint8_t *>(work.data()), reinterpret_cast<const uint8_t *>(work.data() + work.size()));
-    CUDA_OK(cudaMemcpyAsync(ws + L.work, t->work_host.data(), t->work_host.size(), cudaMemcpyHostToDevice, st));
-    *h2d += t->work_host.size();
-    t->work_ws = ws;
-    t->work_key = key;
-  }
-  const int rows_partial = persec ? (se - sb) : nitems;
-  CUDA_OK(cudaMemsetAsync(ws + L.partial, 0, (size_t)rows_partial * m * max_slices * nacc * 8, st));
-  Qmc2Launch p;
-  std::memset(&p, 0, sizeof p);
-  p.image2 = ws + L.image2;
-  p.secoff2 = reinterpret_cast<const uint32_t *>(ws + L.secoff2);
-  p.work = reinterpret_cast<const Qmc2Work *>(ws + L.work);
-  p.logtab = reinterpret_cast<const double *>(ws + L.logtab);
-  p.shifts = reinterpret_cast<const double *>(ws + L.shifts);
-  p.partial = reinterpret_cast<double *>(ws + L.partial);
-  p.counters = reinterpret_cast<unsigned long long *>(ws + L.counters);
-  p.N = (uint32_t)N;
-  p.count = (uint32_t)icount;
-  for (int j = 0; j < n; ++j) {
-    p.zeff[j] = (uint32_t)mulmod(istep % N, z[j], N);
-    p.off[j] = (uint32_t)mulmod(ibeg, z[j], N);
-  }
-  p.m = m;
-  p.transform = t->transform;
-  p.persec = persec ? 1 : 0;
-  p.sm_prog_cap = prog_cap;
-  p.sm_sec_cap = (sec_cap + 15) & ~15u;
-  p.max_nsec = max_nsec;
-  p.max_nslots = max_nslots;
-  p.max_slices = max_slices;
-  cudaEventRecord(static_cast<cudaEvent_t>(t->ev0), st);
-  *ce_out = qmc2_kernel_launch(n, t->L, t->kmax, dim3((unsigned)work.size(), 1), smem, st, p);
-  cudaEventRecord(static_cast<cudaEvent_t>(t->evm), st);
-  *gx_out = max_slices;
-  *rows_out = nitems;
-  return QMC_OK;
 }
 
 // ---- version-4 launch (real path): one launch per run of sectors, tables in the kernel parameters ------------------
@@ -660,132 +534,6 @@ int launch_v5(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
   return QMC_OK;
 }
 
-// ---- version-3 launch (complex path): same geometry as version 2, two slot tables per thread ------------------------------------
-int launch_v3(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t st, uint64_t N, int m, int sb, int se,
-              bool persec, uint64_t ibeg, uint64_t istep, uint64_t icount, const uint64_t *z, int sms, int smem_optin,
-              int *gx_out, int *rows_out, size_t *h2d, cudaError_t *ce_out) {
-  const int n = t->n, nacc = 2 * (QMC_MAXSING + t->kmax + 1), T = QMC3_THREADS;  // accumulators: (Re, Im) per order
-  uint32_t prog_cap = 0;
-  int max_nslots = 0;
-  int max_nslots_c = 0;
-  for (size_t ci = 0; ci < t->chunks3.size(); ++ci) {
-    const Qmc2Chunk &c = t->chunks3[ci];
-    if (c.sec_end > sb && c.sec_begin < se) {
-      prog_cap = std::max(prog_cap, c.prog_bytes);
-      max_nslots = std::max(max_nslots, c.nslots + c.max_local);
-      max_nslots_c = std::max(max_nslots_c, t->chunk3_nslots_c[ci] + t->chunk3_max_local_c[ci]);
-    }
-  }
-  const size_t budget = (size_t)smem_optin - 1024;
-  const size_t fixed = prog_cap + 16 + (((size_t)m * n * 8 + 15) & ~(size_t)15) + (T / 32) * 8 + 128 * 16 + (size_t)max_nslots * T * 8 + (size_t)max_nslots_c * T * 16;
-  const size_t accbytes = persec ? (size_t)nacc * T * 8 : 0;
-  std::vector<Qmc2Work> runs;
-  std::vector<double> run_cost;
-  double total_cost = 0.0;
-  uint32_t sec_cap = 0;
-  int max_nsec = 0;
-  for (const Qmc2Chunk &c : t->chunks3) {
-    int a = std::max(sb, c.sec_begin);
-    const int e = std::min(se, c.sec_end);
-    while (a < e) {
-      int b = a;  // grow the run while it fits the shared-memory budget
-      while (b < e) {
-        const size_t bytes = t->secend3[b] - t->secoff3[a];
-        const size_t need = fixed + bytes + (((size_t)(b + 1 - a + 1) * 4 + 15) & ~(size_t)15) + accbytes * (b + 1 - a);
-        if (need > budget) break;
-        ++b;
-      }
-      if (b == a) return QMC_ENOMEM;
-      Qmc2Work w;
-      std::memset(&w, 0, sizeof w);
-      w.prog_off = c.prog_off;
-      w.prog_bytes = c.prog_bytes;
-      w.sec_off = t->secoff3[a];
-      w.sec_bytes = t->secend3[b - 1] - t->secoff3[a];
-      w.s0 = a;
-      w.nsec = b - a;
-      w.out_row = persec ? a - sb : (int)runs.size();
-      w.count_boundary = runs.empty() ? 1 : 0;
-      sec_cap = std::max(sec_cap, w.sec_bytes);
-      max_nsec = std::max(max_nsec, w.nsec);
-      double cst = 0.0;
-      for (int s = a; s < b; ++s) cst += t->sec_cost[s];
-      run_cost.push_back(cst);
-      total_cost += cst;
-      runs.push_back(w);
-      a = b;
-    }
-  }
-  const int nitems = (int)runs.size();
-  const size_t smem = fixed + sec_cap + (((size_t)(max_nsec + 1) * 4 + 15) & ~(size_t)15) + accbytes * max_nsec;
-  int bps = 0;
-  CUDA_OK(qmc3_kernel_prepare(n, t->L, t->kmax, smem, &bps));
-  if (bps < 1) return QMC_ECUDA;
-  // slices per run in proportion to its modelled cost: about `waves` blocks of equal cost per resident block slot
-  int waves = 16;  // measured (profiles/r01d_waves.md): short blocks interleave better than one long block per slot
-  if (const char *e = std::getenv("QMC2_WAVES")) waves = std::max(1, std::atoi(e));
-  const long long max_slices_pts = std::max<long long>(1, (long long)((icount + T - 1) / T));
-  const double nblocks_target = (double)waves * sms * bps;
-  std::vector<Qmc2Work> work;
-  int max_slices = 1;
-  for (int i = 0; i < nitems; ++i) {
-    long long ns = (long long)(nblocks_target * run_cost[i] / total_cost + 0.5);
-    ns = std::max<long long>(1, std::min<long long>({ns, (long long)QMC_MAX_BLOCKS, max_slices_pts}));
-    max_slices = std::max(max_slices, (int)ns);
-    for (int sidx = 0; sidx < (int)ns; ++sidx) {
-      Qmc2Work w = runs[i];
-      w.slice = sidx;
-      w.nslices = (int)ns;
-      work.push_back(w);
-    }
-  }
-  if (work.size() > QMC2_MAX_WORK) return QMC_ENOMEM;
-  // upload the work list unless the identical list is already there
-  const uint64_t key = ((uint64_t)sb << 40) ^ ((uint64_t)se << 20) ^ (persec ? 1u : 0u) ^ ((uint64_t)m << 50) ^ ((uint64_t)icount << 1) ^
-                       ((uint64_t)waves << 58);
-  if (!(t->work_ws == ws && t->work_key == key)) {
-    t->work_host.assign(reinterpret_cast<const uint8_t *>(work.data()), reinterpret_cast<const uint8_t *>(work.data() + work.size()));
-    CUDA_OK(cudaMemcpyAsync(ws + L.work, t->work_host.data(), t->work_host.size(), cudaMemcpyHostToDevice, st));
-    *h2d += t->work_host.size();
-    t->work_ws = ws;
-    t->work_key = key;
-  }
-  const int rows_partial = persec ? (se - sb) : nitems;
-  CUDA_OK(cudaMemsetAsync(ws + L.partial, 0, (size_t)rows_partial * m * max_slices * nacc * 8, st));
-  Qmc3Launch q;
-  std::memset(&q, 0, sizeof q);
-  Qmc2Launch &p = q.b;
-  q.lambda = t->lambda;
-  q.max_nslots_c = max_nslots_c;
-  p.image2 = ws + L.image3;
-  p.secoff2 = reinterpret_cast<const uint32_t *>(ws + L.secoff3);
-  p.work = reinterpret_cast<const Qmc2Work *>(ws + L.work);
-  p.logtab = reinterpret_cast<const double *>(ws + L.logtab);
-  p.shifts = reinterpret_cast<const double *>(ws + L.shifts);
-  p.partial = reinterpret_cast<double *>(ws + L.partial);
-  p.counters = reinterpret_cast<unsigned long long *>(ws + L.counters);
-  p.N = (uint32_t)N;
-  p.count = (uint32_t)icount;
-  for (int j = 0; j < n; ++j) {
-    p.zeff[j] = (uint32_t)mulmod(istep % N, z[j], N);
-    p.off[j] = (uint32_t)mulmod(ibeg, z[j], N);
-  }
-  p.m = m;
-  p.transform = t->transform;
-  p.persec = persec ? 1 : 0;
-  p.sm_prog_cap = prog_cap;
-  p.sm_sec_cap = (sec_cap + 15) & ~15u;
-  p.max_nsec = max_nsec;
-  p.max_nslots = max_nslots;
-  p.max_slices = max_slices;
-  cudaEventRecord(static_cast<cudaEvent_t>(t->ev0), st);
-  *ce_out = qmc3_kernel_launch(n, t->L, t->kmax, dim3((unsigned)work.size(), 1), smem, st, q);
-  cudaEventRecord(static_cast<cudaEvent_t>(t->evm), st);
-  *gx_out = max_slices;
-  *rows_out = nitems;
-  return QMC_OK;
-}
-
 }  // namespace
 
 // =====================================================================================================
@@ -967,8 +715,8 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
   if (!dev_workspace || dev_workspace_bytes < L.total) return QMC_ENOMEM;
   unsigned char *ws = static_cast<unsigned char *>(dev_workspace);
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  const bool image_resident = r.tables_resident >= 1 && t->resident_ws == dev_workspace;
-  const bool shifts_resident = r.tables_resident >= 2 && image_resident && t->resident_m == m && !r.shifts;
+  const bool image_resident_ws = r.tables_resident >= 1 && t->resident_ws == dev_workspace;
+  const bool shifts_resident = r.tables_resident >= 2 && image_resident_ws && t->resident_m == m && !r.shifts;
 
   // ---- generating vector and shifts ---------------------------------------------------------------------
   uint64_t z[QMC_MAXDIM] = {0};
@@ -1010,32 +758,25 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
   int gx = 1, nchunks = 1;
   cudaError_t ce = cudaSuccess;
   double *partial = reinterpret_cast<double *>(ws + L.partial);
-  const bool use_v2 = !cplx && !t->image2.empty() && qmc2_kernel_available(n, t->L, t->kmax) && !std::getenv("QMC_FORCE_V1");
-  const bool use_v4 = use_v2 && !t->tab4.empty() && qmc4_kernel_available(n, t->L, t->kmax) && !std::getenv("QMC_FORCE_V2");
+  const bool use_v4 = !cplx && !t->tab4.empty() && qmc4_kernel_available(n, t->L, t->kmax) && !std::getenv("QMC_FORCE_V1");
+  const bool use_v5 = cplx && !t->tab5.empty() && -t->kmin <= QMC3_MAXSING && qmc5_kernel_available(n, t->L, t->kmax) &&
+                      !std::getenv("QMC_FORCE_V1");
   int eval_launches = 1;
-  // ---- uploads common to both kernels (skipped when resident) ------------------------------------------------
-  if (!image_resident) {
-    h2d += t->image.size() + t->secoff.size() * 4;
-    CUDA_OK(cudaMemcpyAsync(ws + L.image, t->image.data(), t->image.size(), cudaMemcpyHostToDevice, st));
-    CUDA_OK(cudaMemcpyAsync(ws + L.secoff, t->secoff.data(), t->secoff.size() * 4, cudaMemcpyHostToDevice, st));
-    if (!t->image3.empty()) {
-      h2d += t->image3.size() + t->secoff3.size() * 4 + sizeof t->logtab;
-      CUDA_OK(cudaMemcpyAsync(ws + L.image3, t->image3.data(), t->image3.size(), cudaMemcpyHostToDevice, st));
-      CUDA_OK(cudaMemcpyAsync(ws + L.secoff3, t->secoff3.data(), t->secoff3.size() * 4, cudaMemcpyHostToDevice, st));
-      CUDA_OK(cudaMemcpyAsync(ws + L.logtab, t->logtab, sizeof t->logtab, cudaMemcpyHostToDevice, st));
+  // ---- uploads (skipped when resident).  Versions 4 and 5 carry their tables in the kernel parameters: only the
+  // logarithm table lives in the workspace; the version-1 image is uploaded for the generic fallback kernel only.
+  const int kind = (use_v4 || use_v5) ? 4 : 1;  // what has to be in the workspace: the logarithm table, or the version-1 image
+  if (!(image_resident_ws && t->resident_kind == kind)) {
+    if (use_v4 || use_v5) {
       CUDA_OK(cudaMemcpyAsync(ws + L.logtab4, t->logtab4, sizeof t->logtab4, cudaMemcpyHostToDevice, st));
       h2d += sizeof t->logtab4;
-    }
-    if (!t->image2.empty()) {
-      h2d += t->image2.size() + t->secoff2.size() * 4 + sizeof t->logtab;
-      CUDA_OK(cudaMemcpyAsync(ws + L.image2, t->image2.data(), t->image2.size(), cudaMemcpyHostToDevice, st));
-      CUDA_OK(cudaMemcpyAsync(ws + L.secoff2, t->secoff2.data(), t->secoff2.size() * 4, cudaMemcpyHostToDevice, st));
-      CUDA_OK(cudaMemcpyAsync(ws + L.logtab, t->logtab, sizeof t->logtab, cudaMemcpyHostToDevice, st));
-      CUDA_OK(cudaMemcpyAsync(ws + L.logtab4, t->logtab4, sizeof t->logtab4, cudaMemcpyHostToDevice, st));
-      h2d += sizeof t->logtab4;
+    } else {
+      h2d += t->image.size() + t->secoff.size() * 4;
+      CUDA_OK(cudaMemcpyAsync(ws + L.image, t->image.data(), t->image.size(), cudaMemcpyHostToDevice, st));
+      CUDA_OK(cudaMemcpyAsync(ws + L.secoff, t->secoff.data(), t->secoff.size() * 4, cudaMemcpyHostToDevice, st));
     }
     t->resident_ws = dev_workspace;
-    t->resident_m = 0;
+    t->resident_kind = kind;
+    if (!shifts_resident) t->resident_m = 0;
   }
   if (!shifts_resident) {
     h2d += t->shifts_host.size() * 8;
@@ -1044,20 +785,11 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
   }
   CUDA_OK(cudaMemsetAsync(ws + L.counters, 0, 32, st));
 
-  const bool use_v3 = cplx && !t->image3.empty() && -t->kmin <= QMC3_MAXSING && qmc3_kernel_available(n, t->L, t->kmax) &&
-                      !std::getenv("QMC_FORCE_V1");
-  const bool use_v5 = use_v3 && !t->tab5.empty() && qmc5_kernel_available(n, t->L, t->kmax) && !std::getenv("QMC_FORCE_V3");
   if (use_v5) {
     int rc = launch_v5(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, &gx, &nchunks, &eval_launches, &h2d, &ce);
     if (rc != QMC_OK) return rc;
-  } else if (use_v3) {
-    int rc = launch_v3(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, &gx, &nchunks, &h2d, &ce);
-    if (rc != QMC_OK) return rc;
   } else if (use_v4) {
     int rc = launch_v4(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, &gx, &nchunks, &eval_launches, &h2d, &ce);
-    if (rc != QMC_OK) return rc;
-  } else if (use_v2) {
-    int rc = launch_v2(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, &gx, &nchunks, &h2d, &ce);
     if (rc != QMC_OK) return rc;
   } else {
   const size_t fixed_smem = 16 + (((size_t)m * n * 8 + 15) & ~(size_t)15) + (QMC_THREADS / 32) * 8 + (size_t)3 * n * QMC_THREADS * 8;

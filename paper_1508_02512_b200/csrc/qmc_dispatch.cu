@@ -24,58 +24,6 @@ cudaError_t qmc_kernel_launch(int ndim, int kmax, int flavor, dim3 grid, size_t 
   return ops(ndim, kmax, flavor, 1, grid, smem, st, &p, nullptr);
 }
 
-// ---- version 2 (real path) ---------------------------------------------------------------------------------
-#define QMC2_DECL(N) \
-  cudaError_t qmc2_ops_d##N(int, int, int, dim3, size_t, cudaStream_t, const Qmc2Launch *, int *);
-QMC2_DECL(1) QMC2_DECL(2) QMC2_DECL(3) QMC2_DECL(4) QMC2_DECL(5) QMC2_DECL(6)
-
-static cudaError_t ops2(int ndim, int loops, int kmax, int op, dim3 grid, size_t smem, cudaStream_t st, const Qmc2Launch *p, int *bps) {
-  switch (ndim) {
-    case 1: return qmc2_ops_d1(loops, kmax, op, grid, smem, st, p, bps);
-    case 2: return qmc2_ops_d2(loops, kmax, op, grid, smem, st, p, bps);
-    case 3: return qmc2_ops_d3(loops, kmax, op, grid, smem, st, p, bps);
-    case 4: return qmc2_ops_d4(loops, kmax, op, grid, smem, st, p, bps);
-    case 5: return qmc2_ops_d5(loops, kmax, op, grid, smem, st, p, bps);
-    case 6: return qmc2_ops_d6(loops, kmax, op, grid, smem, st, p, bps);
-    default: return cudaErrorInvalidValue;
-  }
-}
-bool qmc2_kernel_available(int ndim, int loops, int kmax) {
-  return ndim >= 1 && ndim <= 6 && loops >= 1 && loops <= 2 && loops <= ndim && kmax >= 0 && kmax <= 2;
-}
-cudaError_t qmc2_kernel_prepare(int ndim, int loops, int kmax, size_t smem, int *blocks_per_sm) {
-  return ops2(ndim, loops, kmax, 0, dim3(1), smem, nullptr, nullptr, blocks_per_sm);
-}
-cudaError_t qmc2_kernel_launch(int ndim, int loops, int kmax, dim3 grid, size_t smem, cudaStream_t st, const Qmc2Launch &p) {
-  return ops2(ndim, loops, kmax, 1, grid, smem, st, &p, nullptr);
-}
-
-// ---- version 3 (complex path) ------------------------------------------------------------------------------
-#define QMC3_DECL(N) \
-  cudaError_t qmc3_ops_d##N(int, int, int, dim3, size_t, cudaStream_t, const Qmc3Launch *, int *);
-QMC3_DECL(1) QMC3_DECL(2) QMC3_DECL(3) QMC3_DECL(4) QMC3_DECL(5) QMC3_DECL(6)
-
-static cudaError_t ops3(int ndim, int loops, int kmax, int op, dim3 grid, size_t smem, cudaStream_t st, const Qmc3Launch *p, int *bps) {
-  switch (ndim) {
-    case 1: return qmc3_ops_d1(loops, kmax, op, grid, smem, st, p, bps);
-    case 2: return qmc3_ops_d2(loops, kmax, op, grid, smem, st, p, bps);
-    case 3: return qmc3_ops_d3(loops, kmax, op, grid, smem, st, p, bps);
-    case 4: return qmc3_ops_d4(loops, kmax, op, grid, smem, st, p, bps);
-    case 5: return qmc3_ops_d5(loops, kmax, op, grid, smem, st, p, bps);
-    case 6: return qmc3_ops_d6(loops, kmax, op, grid, smem, st, p, bps);
-    default: return cudaErrorInvalidValue;
-  }
-}
-bool qmc3_kernel_available(int ndim, int loops, int kmax) {
-  return ndim >= 1 && ndim <= 6 && loops >= 1 && loops <= 2 && loops <= ndim && kmax >= 0 && kmax <= 2;
-}
-cudaError_t qmc3_kernel_prepare(int ndim, int loops, int kmax, size_t smem, int *blocks_per_sm) {
-  return ops3(ndim, loops, kmax, 0, dim3(1), smem, nullptr, nullptr, blocks_per_sm);
-}
-cudaError_t qmc3_kernel_launch(int ndim, int loops, int kmax, dim3 grid, size_t smem, cudaStream_t st, const Qmc3Launch &p) {
-  return ops3(ndim, loops, kmax, 1, grid, smem, st, &p, nullptr);
-}
-
 // ---- version 4 (real path, constant-bank tables) -------------------------------------------------------------
 #define QMC4_DECL(N) \
   cudaError_t qmc4_ops_d##N(int, int, int, dim3, size_t, cudaStream_t, const Qmc4Launch *, int *);

@@ -40,20 +40,8 @@ double sector_cost(const QmcSector &s, int kmax) {
 
 }  // namespace
 
-// table of the kernels' logarithm: z in [0.6875, 1.375) by the top bits of the high word, c_i = interval centre
-static void build_logtab(double *tab) {
-  for (int i = 0; i < 128; ++i) {
-    const uint64_t lo = ((uint64_t)(0x3fe60000u + ((uint32_t)i << 13))) << 32, hi = lo + ((uint64_t)0x2000 << 32);
-    double zl, zh;
-    std::memcpy(&zl, &lo, 8);
-    std::memcpy(&zh, &hi, 8);
-    const double invc = (double)(1.0L / (0.5L * ((long double)zl + (long double)zh)));
-    tab[2 * i] = invc;
-    tab[2 * i + 1] = (double)(-logl((long double)invc));
-  }
-}
-
-// the same for version 4: 64 intervals
+// table of the kernels' logarithm: z in [0.6875, 1.375), 64 intervals by the top bits of the high word, c_i = interval centre;
+// tab[i] = {1/c_i rounded, -ln(that) in extended precision}
 static void build_logtab4(double *tab) {
   for (int i = 0; i < 64; ++i) {
     const uint64_t lo = ((uint64_t)(0x3fe60000u + ((uint32_t)i << 14))) << 32, hi = lo + ((uint64_t)0x4000 << 32);
@@ -85,7 +73,6 @@ void put_rec(std::vector<uint32_t> &v, const Qmc2Rec &r) {
 }  // namespace
 
 int qmc_build_image2(qmc_tables *t) {
-  build_logtab(t->logtab);
   build_logtab4(t->logtab4);
   t->tab4.clear();
   t->secoff4.clear();

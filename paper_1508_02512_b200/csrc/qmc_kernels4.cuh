@@ -1,22 +1,29 @@
-// Evaluation kernel, version 4 (real / Euclidean path), sm_100a.  Steps S1-S7 of DESIGN.md.
+// Evaluation kernel of the real (Euclidean) path, "version 4", sm_100a.  Steps S1-S7 of DESIGN.md.
 //
-// Same arithmetic scheme as version 2 (qmc_kernels2.cuh: per-point slot table in shared memory, a monomial = one record
-// c * slot * slot, group partial sums -> subset sums -> all corners of the subtraction from one pass, one reciprocal and
-// one table logarithm per corner, product form folded one singular variable at a time) with a different home for the
-// tables: the chunk's slot program and the sector tables are part of the KERNEL PARAMETER BLOCK (constant bank 0, layout
-// in qmc_launch.h).  Measured reasons (profiles/r01g_*): in version 2 the record loops were bound by the shared-memory
-// data pipe (6 wavefronts per record: 2 for the 16-byte broadcast of the record, 2 + 2 for the slot operands) and by
-// the exposed LDS -> LDS -> DMUL -> DFMA latency chain of one short loop per group, and cost 11 instructions per record.
-// Here a record is 2 uniform loads (LDCU.64), 2 LDS [R + UR], DMUL, DFMA (the coefficient is a uniform-register
-// operand), trip counts are uniform so ptxas unrolls and batches the loads, and the FIRST record of every group sits
-// in a dense array with a compile-time destination register: 2^nsing independent load/multiply chains in one basic
-// block.  The logarithm table is 64 entries x 8 interleaved copies (lane & 7 picks the copy): every lookup is a
-// conflict-free LDS.128 (4 wavefronts instead of the ~10 measured with one copy).
+// One thread = one lattice point at a time.  Per point the thread fills its column of a shared-memory slot table
+// (t_j, ln t_j, 1/t_j, 1, then the chunk's product slots chosen by the byte-pair-encoding pass of qmc_image2.cpp); a
+// monomial of U^ or F^ is then ONE record c * slot * slot.  Per sector with s singular variables:
+//   1. partial sums of U^, F^ per group (= set of singular variables a monomial depends on), subset sums -> the values
+//      at all 2^s corners t^Z of the subtraction (Eqs. 11-12) from one pass over the records;
+//   2. per corner: W_Z = G0 U^aU0 F^aF0 with one reciprocal, Lambda_Z = ln(U^aU1 F^aF1) + L0 with ONE table-driven
+//      logarithm (exponents are compile-time: they depend only on the dimension and the loop number, Eq. 6);
+//   3. the product form of the eps-expanded subtracted integrand, folded one singular variable at a time with series
+//      windows of exactly the needed length (qmc_fold.cuh).
+// The chunk's slot program and the sector tables are part of the KERNEL PARAMETER BLOCK (constant bank 0, layout in
+// qmc_launch.h).  Measured reasons (profiles/r01i_eval_kernel_ncu.md): with the tables in shared memory (the round's
+// earlier kernel) the record loops were bound by the shared-memory data pipe (6 wavefronts per record: 2 for the
+// 16-byte broadcast of the record, 2 + 2 for the slot operands) and by the exposed LDS -> LDS -> DMUL -> DFMA latency
+// chain of one short loop per group, at 11 instructions per record.  Here a record is 2 uniform loads (LDCU.64), 2 LDS
+// [R + UR], DMUL, DFMA (the coefficient is a uniform-register operand), trip counts are uniform, the FIRST record of
+// every group sits in a dense array with a compile-time destination register (2^nsing independent load/multiply chains
+// in one basic block), and all further records are one stream walked with the next operands in flight.  The logarithm
+// table is 64 entries x 8 interleaved copies (lane & 7 picks the copy): every lookup is a conflict-free LDS.128
+// (4 wavefronts instead of the ~10 measured with one copy).
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
 
-#include "qmc_kernels2.cuh"  // fast_rcp, ipow_c, Expo, Ctx2, Fold2, finite_hi
+#include "qmc_fold.cuh"  // ipow_c, Expo, Ctx2, Fold2, finite_hi
 #include "qmc_launch.h"
 
 namespace qmc4 {

@@ -1,13 +1,22 @@
-// Evaluation kernel, version 5 (complex path: physical region, contour deformation), sm_100a.  Steps S1-S7 of DESIGN.md.
+// Evaluation kernel of the complex path (physical region, contour deformation), "version 5", sm_100a.  Steps S1-S7.
 //
-// The arithmetic of version 3 (qmc_kernels3.cuh: real slot table at the lattice point for the derivative polynomials of
-// F^, complex slot table over the deformed variables for U^(z), F^(z), Eq. 14 with its Jacobian determinant by LU, complex
-// table logarithms, product form folded over the singular variables) with the tables where version 4 keeps them: in the
-// kernel parameter block (constant bank 0; layout in qmc_launch.h).  Every table read is a uniform load, the record
-// loops run on the uniform datapath, and every corner of a sector owns a flat record stream (records needed by several
-// corners are duplicated by the table builder), walked with the next record's slot operands in flight.  The corner is
-// inlined inside a `for Z` loop with a uniform trip count (one copy of the corner code per number of singular
-// variables); its results go to compile-time registers through a uniform `switch (Z)`.
+// One thread = one lattice point; two slot tables per thread in shared memory: a REAL one at the lattice point (t_j,
+// ln t_j, 1/t_j, 1, products) that serves the gradient and Hessian polynomials of F^ -- emitted by qmc_prepare as record
+// lists of their own -- and a COMPLEX one over the deformed variables z_j, refilled at every corner, that serves U^(z),
+// F^(z).  Per corner Z of a sector (real point tau = t with the variables of Z set to 0):
+//   S4  F^_i(tau), F^_ik(tau) from the record lists of the derivative polynomials;
+//       rho_i = 1 - i lambda (1 - tau_i) F^_i,  z_i = tau_i rho_i,
+//       J_ik = delta_ik [1 - i lambda (1 - 2 tau_i) F^_i] - i lambda tau_i (1 - tau_i) F^_ik   (Eq. 14; R:C12),
+//       det J by LU with row pivoting;
+//   S5  U^(z), F^(z) as sums of complex records;  G_Z = G0 det J prod_{j notin Z} rho_j^alpha_j U^aU0 F^aF0,
+//       Lambda_Z = aU1 ln U + aF1 ln F + sum_j beta_j ln rho_j + L0   (principal logs; -i pi on the negative real axis, R:C11);
+//   S6  product form folded one singular variable at a time with exact series windows (as qmc_fold.cuh, complex).
+// The tables are in the kernel parameter block (constant bank 0; layout in qmc_launch.h) like those of the real path:
+// every table read is a uniform load, the record loops run on the uniform datapath, and every corner of a sector owns a
+// flat record stream (records needed by several corners are duplicated by the table builder), walked with the next
+// record's slot operands in flight.  The corner is inlined inside a `for Z` loop with a uniform trip count (one copy of
+// the corner code per number of singular variables); its results go to compile-time registers through a uniform
+// `if (Z == q)` chain.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>

@@ -30,7 +30,8 @@ struct QmcSectorHdr {
 };
 static_assert(sizeof(QmcSectorHdr) == 64, "sector header must be 64 bytes");
 
-// ---- device image, version 2 (real path) ------------------------------------------------------------
+// ---- planning image of the real path ("version 2": host only; chunk sizes, describe(); the kernels read the
+// version-4 tables built from the same plan, qmc_launch.h) ------------------------------------------------
 // Sectors are grouped into CHUNKS.  Every chunk owns a "slot program": each thread keeps, per lattice point, a table
 // of per-point values in shared memory (slot s of thread tid at slots[s * QMC2_THREADS + tid]):
 //   slots [0,n) t_j | [n,2n) ln t_j | [2n,3n) 1/t_j | 3n: 1.0 | 3n+1 ...: products slot[k] = slot[a] * slot[b]
@@ -70,7 +71,7 @@ struct Qmc2Chunk {      // host description of one chunk
   double cost = 0.0;                      // modelled flops per point (load balancing)
 };
 
-// ---- device image, version 3 (complex path: contour deformation) --------------------------------------
+// ---- planning image of the complex path ("version 3": host only; the kernels read the version-5 tables) ------
 // Same idea as version 2, with TWO slot tables per thread: a REAL one at the lattice point (t_j, ln t_j, 1/t_j, 1,
 // products) that serves the gradient and Hessian polynomials of F^ -- emitted by qmc_prepare as record lists of their
 // own -- and the regular-variable factors; and a COMPLEX one over the deformed variables z_j (z_j, 1, products),
@@ -121,13 +122,12 @@ struct qmc_tables {
   // device image
   std::vector<uint8_t> image;     // concatenated sector blocks (16-byte aligned each)
   std::vector<uint32_t> secoff;   // [n_sectors + 1] byte offsets
-  // version 2 image (real path only; empty when lambda > 0)
+  // planning image of the real path (host only; empty when lambda > 0)
   std::vector<uint8_t> image2;
   std::vector<uint32_t> secoff2;  // [n_sectors + 1] byte offsets of the sector blocks in image2
   std::vector<uint32_t> secend2;  // [n_sectors] end offsets (a chunk header sits between the sectors of two chunks)
   std::vector<Qmc2Chunk> chunks;
   std::vector<double> sec_cost;   // modelled cost per sector (load balancing of the launch)
-  double logtab[256] = {0};      // 128 x {1/c_i, -ln(1/c_i)} of the kernels' table-driven logarithm
   // version 4 tables (real path; same chunks and slot programs as version 2, laid out for the kernel-parameter
   // constant bank: see qmc_launch.h)
   std::vector<uint32_t> tab4;       // sector blocks, 32-bit words (4 per 16-byte table word)
@@ -139,19 +139,17 @@ struct qmc_tables {
   std::vector<std::vector<uint32_t>> prog5r, prog5c;  // per chunk: real / complex slot programs {a_off, b_off}
   void *side_streams[8] = {nullptr};  // cudaStream_t: the launches of one integration are spread over these
   void *side_events[9] = {nullptr};   // cudaEvent_t: fork + one join per side stream
-  // version 3 image (complex path only)
+  // planning image of the complex path (host only)
   std::vector<uint8_t> image3;
   std::vector<uint32_t> secoff3, secend3;
   std::vector<Qmc2Chunk> chunks3;    // nslots = real slots; prog_off/prog_bytes cover the chunk header + both programs
   std::vector<int> chunk3_nslots_c, chunk3_max_local_c;
   // launcher state (host-side caches; not thread-safe by design: one tables object per stream)
   const void *resident_ws = nullptr;  // workspace the image was last uploaded to
+  int resident_kind = 0;              // 4: logarithm table (versions 4, 5), 1: version-1 image
   int resident_m = 0;                 // number of shift vectors resident in that workspace (0 = none)
   uint64_t cached_N = 0;              // generating vector cache
   uint64_t cached_z[QMC_MAXDIM] = {0};
-  std::vector<uint8_t> work_host;     // staging of the version-2 work list
-  const void *work_ws = nullptr;      // workspace / key of the work list resident on the device
-  uint64_t work_key = 0;
   std::vector<double> shifts_host;    // staging of the shift vectors (must outlive the async H2D copy)
   std::vector<double> stat_host;      // staging of the fetched statistics block
   void *ev0 = nullptr, *ev1 = nullptr, *evm = nullptr;  // cudaEvent_t: before / after all kernels, after the evaluation kernel
