@@ -17,7 +17,7 @@ from typing import List, Sequence, Tuple
 import numpy as np
 
 __all__ = [
-    "Workload", "CONFIGS", "bubble", "massless_box", "massive_box", "double_box", "nonplanar_vertex",
+    "Workload", "CONFIGS", "bubble", "massless_box", "massive_box", "gghh_box_scan", "double_box", "nonplanar_vertex",
     "triangle", "four_point_gram", "splitmix64_shifts", "korobov_vector", "good_vector", "GOOD_KOROBOV", "PRIMES",
     "primes_below_pow2",
 ]
@@ -90,6 +90,19 @@ def massive_box(s: float = 5.0, t: float = -1.5, m2: float = 1.0, mh2: float = 0
     """Config 3: one-loop box, four equal internal masses, p3^2=p4^2=mh2, physical region for s > 4 m2."""
     return Workload("cfg3_massive_box", 4, [(0, 1, m2), (1, 2, m2), (2, 3, m2), (3, 0, m2)], [0, 1, 2, 3],
                     four_point_gram([0, 0, mh2, mh2], s, t), lam, 0, (99991, 999983, 9999991), 16, 11)
+
+
+def gghh_box_scan(n_points: int = 1000, s_min: float = 70000.0, s_max: float = 500000.0, t: float = -6000.0,
+                  mt: float = 172.0, mh: float = 125.0, lam: float = 0.5):
+    """The paper's kinematic scan of the one-loop box I_A of gg -> HH (Eq. 22: 1000 values of s in
+    [70000, 500000] at t = -6000, M_t = 172, M_H = 125; threshold at s = 4 M_t^2 = 118336), in units of M_t^2: the graph of
+    config 3 at other kinematics.  Yields (s, Workload)."""
+    mt2 = mt * mt
+    for i in range(n_points):
+        s = s_min + (s_max - s_min) * i / max(n_points - 1, 1)
+        wl = massive_box(s=s / mt2, t=t / mt2, m2=1.0, mh2=mh * mh / mt2, lam=lam)
+        wl.name = "gghh_box_scan"
+        yield s, wl
 
 
 def double_box(s: float = -3.0, t: float = -1.0, p2: Sequence[float] = (0, 0, 0, 0), eps_order: int = 0) -> Workload:

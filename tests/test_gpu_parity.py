@@ -217,3 +217,23 @@ def test_complex_path_tables_launch_splits_and_local_slots(monkeypatch):
     monkeypatch.delenv("QMC3_CHUNK_BYTES")
     monkeypatch.delenv("QMC3_SLOTS_R")
     monkeypatch.delenv("QMC3_SLOTS_C")
+
+
+def test_kinematic_scan_points_of_the_papers_box():
+    """three points of the paper's s-scan of the one-loop box: parity with the oracle,
+    a vanishing imaginary part below the threshold s = 4 M_t^2, and lambda-independence above it."""
+    pts = dict((round(s), wl) for s, wl in qi.gghh_box_scan(44))     # s = 70000, 80000, ..., 500000
+    below, above = pts[110000], pts[200000]
+    r, *_ = parity(below, 16381, 4)
+    assert abs(r.coeff[-1].imag) < 5 * r.err[-1].imag + 1e-9 and r.coeff[-1].real > 0
+    parity(above, 16381, 4)
+    N, m = 99991, 16
+    z = qi.good_vector(N, 3)
+    vals = []
+    for lam in (0.25, 0.5):
+        t = q.qmc_prepare(above, eps_order=0, lam=lam)
+        vals.append(q.qmc_integrate(t, N, m, z=z, seed=11))
+    d = vals[0].coeff[-1] - vals[1].coeff[-1]
+    sig = np.hypot(abs(vals[0].err[-1]), abs(vals[1].err[-1]))
+    assert abs(d) < 6 * sig and abs(vals[0].coeff[-1].imag) > 0.1
+    assert not vals[0].counters[:2].any() and not vals[1].counters[:2].any()

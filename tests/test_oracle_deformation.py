@@ -192,3 +192,26 @@ def test_config5_lambda_independence_and_euclidean_limit():
     for k in range(2):
         assert abs(cc[k].imag) <= 4 * ec[k].imag + 1e-12
         assert abs(cc[k].real - cr[k].real) <= 4 * np.hypot(ec[k].real, er[k].real)
+
+
+def test_kinematic_scan_points_threshold_and_lambda_independence():
+    """points of the paper's s-scan of the one-loop box on the oracle: the imaginary part
+    vanishes below the threshold s = 4 M_t^2 = 118336 and is there above it, and the value does not depend
+    on lambda (Eq. 14: any deformation that keeps Im F < 0 gives the same integral)."""
+    pts = dict((round(s), wl) for s, wl in qi.gghh_box_scan(44))
+    N, m = 16381, 6
+    z = qi.good_vector(N, 3)
+    sh = qi.splitmix64_shifts(11, m, 3)
+    res = {}
+    for s_phys, lam in ((110000, 0.5), (200000, 0.25), (200000, 0.5)):
+        wl = pts[s_phys]
+        o = Oracle.from_workload(wl, lam=lam)
+        S, A, cnt = o.integrate(N, z, sh)
+        assert cnt[0] == 0 and cnt[2] == 0
+        res[(s_phys, lam)] = o.totals(S)
+    c, e = res[(110000, 0.5)]
+    assert abs(c[-1].imag) <= 5 * e[-1].imag + 1e-9 and c[-1].real > 0.3
+    (c1, e1), (c2, e2) = res[(200000, 0.25)], res[(200000, 0.5)]
+    assert abs((c1[-1] - c2[-1]).real) <= 5 * np.hypot(e1[-1].real, e2[-1].real)
+    assert abs((c1[-1] - c2[-1]).imag) <= 5 * np.hypot(e1[-1].imag, e2[-1].imag)
+    assert c1[-1].imag > 0.3      # J_0(s = 200000) = 0.13976 + 0.34363 i on the GPU at N = 99991 (profiles/r01n)
