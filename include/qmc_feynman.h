@@ -19,6 +19,10 @@
  *    qmc_workspace_bytes() bytes (e.g. a torch tensor's data_ptr()), `cuda_stream` is a cudaStream_t
  *    (e.g. torch.cuda.current_stream().cuda_stream; NULL = default stream).  The library never
  *    allocates device memory; it synchronises only its own stream before filling host outputs.
+ *    The evaluation is one kernel launch per run of sectors (the sector tables travel in the kernel
+ *    parameters); the launches of one call are spread over up to 8 internal non-blocking streams
+ *    owned by the qmc_tables object (created on first use, destroyed by qmc_tables_free), forked from
+ *    and joined back into `cuda_stream` with events: to the caller the call is ordered on `cuda_stream`.
  *  - There is NO CPU fallback: without a CUDA device qmc_integrate* returns QMC_ECUDA.
  *
  * What is computed.  For a graph with P propagators (powers nu_j = 1), L loops, D = 4 - 2 eps:
@@ -102,7 +106,8 @@ typedef struct {
                                         #non-finite (point, sector) evaluations (dropped), #boundary points (R:C18) */
   double kernel_ms;                  /* device time of all kernels of the call: evaluation, final sum, statistics (CUDA events) */
   double eval_kernel_ms;             /* device time of the evaluation kernel alone (S1-S7 first stage) */
-  int64_t h2d_bytes, d2h_bytes;      /* bytes this call copied host->device (tables, shifts) and device->host (results) */
+  int64_t h2d_bytes, d2h_bytes;      /* bytes this call moved host->device (shifts, logarithm table, and the kernel parameter
+                                        blocks that carry the sector tables) and device->host (results) */
   int32_t kernel_launches;           /* number of kernel launches made by this call */
   int32_t mode_used;                 /* 1 fused (all sectors summed in registers), 2 per-sector */
 } qmc_result;
@@ -115,7 +120,7 @@ typedef struct {
                                                     The sum is always normalised by 1/N (Eq. 18). */
   int32_t sector_begin, sector_end;              /* sector range; end 0 = all */
   int32_t mode;             /* 0 auto (per-sector iff a per-sector output is requested), 1 fused, 2 per-sector */
-  int32_t tables_resident;  /* 1: reuse the table image already uploaded to this workspace by an earlier call;
+  int32_t tables_resident;  /* 1: reuse what an earlier call left in this workspace (the logarithm table);
                                2: reuse the shift vectors of that call as well (nothing is copied from the host) */
 } qmc_run;
 
