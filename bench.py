@@ -314,6 +314,8 @@ def run_product(args):
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
         line["time_to_1e-3"] = [time_to_accuracy(q, qi.double_box(), torch), time_to_accuracy(q, qi.nonplanar_vertex(), torch)]
         line["time_to_1e-5"] = [time_to_accuracy(q, qi.nonplanar_vertex(), torch, target=1e-5, max_N=2 ** 24)]
+        # the paper's own two-loop integrals in the physical region (Tables 2-3: 19 s and 20 s on a K20)
+        line["time_to_1e-3"] += [time_to_accuracy(q, qi.paper_IC(), torch), time_to_accuracy(q, qi.paper_ID(), torch)]
         line["other_workloads"] = other_workloads(q, torch, dev, args.config)
         line["kinematic_scan"] = kinematic_scan(q, torch)
     print(json.dumps(line), flush=True)

@@ -26,8 +26,9 @@
 //   O9  mean, standard error over shifts                      P:161-170, Eqs. 19-20 (R:C15)
 //
 // Pins (tests/test_oracle_*.py, -m "not gpu"): closed forms (bubble, triangle, massless
-// box, double-box poles), the paper's Table 1, brute-force quadrature,
-// Kirchhoff matrix-tree counts, lattice exactness, tiling identity, invariants.
+// box, double-box poles), the paper's Table 1 and, for the complex path, its
+// Tables 2 and 3, brute-force quadrature, Kirchhoff matrix-tree
+// counts, lattice exactness, tiling identity, invariants.
 // No function here is "parity unpinned" except the final VALUE of config 5 (no closed form
 // in the container; pinned by invariants only -- see DESIGN.md).
 // =====================================================================================

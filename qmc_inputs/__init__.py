@@ -17,7 +17,7 @@ from typing import List, Sequence, Tuple
 import numpy as np
 
 __all__ = [
-    "Workload", "CONFIGS", "bubble", "massless_box", "massive_box", "gghh_box_scan", "double_box", "nonplanar_vertex",
+    "Workload", "CONFIGS", "bubble", "massless_box", "massive_box", "gghh_box_scan", "paper_IC", "paper_ID", "double_box", "nonplanar_vertex",
     "triangle", "four_point_gram", "splitmix64_shifts", "korobov_vector", "good_vector", "GOOD_KOROBOV", "PRIMES",
     "primes_below_pow2",
 ]
@@ -103,6 +103,32 @@ def gghh_box_scan(n_points: int = 1000, s_min: float = 70000.0, s_max: float = 5
         wl = massive_box(s=s / mt2, t=t / mt2, m2=1.0, mh2=mh * mh / mt2, lam=lam)
         wl.name = "gghh_box_scan"
         yield s, wl
+
+
+def _gghh_two_loop(name: str, edges, lam: float, s: float, t: float, mt: float, mh: float) -> Workload:
+    mt2 = mt * mt
+    g = four_point_gram([0.0, 0.0, mh * mh / mt2, mh * mh / mt2], s / mt2, t / mt2)
+    wl = Workload(name, 6, edges, [0, 1, 4, 5], g, lam, 0, primes_below_pow2(14, 27), 20, 5)
+    wl.meta["s_over_mt2"] = s / mt2
+    return wl
+
+
+def paper_IC(lam: float = 0.3, s: float = 160000.0, t: float = -6000.0, mt: float = 172.0, mh: float = 125.0) -> Workload:
+    """The paper's planar two-loop master integral I_C of gg -> HH (Eq. 25; Table 2), in
+    units of M_t^2.  Propagators of Eq. 25 in order: k1, k1-p1, k1+p2 (massless), k1-k2-p1, k2, k1+p2-k2-p3, k1-k2+p2
+    (mass M_t).  With k2' = k1 - k2 the rung is line 5; vertices: 0 (p1; lines 1, 2), 1 (p2; lines 1, 3),
+    2 (lines 2, 4, 5), 3 (lines 3, 5, 7), 4 (p3 leaves; lines 6, 7), 5 (p4 leaves; lines 4, 6)."""
+    edges = [(0, 1, 0.0), (0, 2, 0.0), (1, 3, 0.0), (2, 5, 1.0), (2, 3, 1.0), (4, 5, 1.0), (3, 4, 1.0)]
+    return _gghh_two_loop("paper_IC_planar_double_box", edges, lam, s, t, mt, mh)
+
+
+def paper_ID(lam: float = 0.3, s: float = 160000.0, t: float = -6000.0, mt: float = 172.0, mh: float = 125.0) -> Workload:
+    """The paper's non-planar two-loop master integral I_D (Eq. 27; Table 3), in units of
+    M_t^2.  Propagators of Eq. 27 in order: k1, k1+p1, k1-p2 (massless), k1+p1-k2, k2, k2-p4, k1+p1-k2-p3 (mass M_t).
+    Vertices: 0 (p1; lines 1, 2), 1 (p2; lines 1, 3), 2 (lines 2, 4, 5), 3 (lines 3, 6, 7), 4 (p3 leaves; lines 4, 7),
+    5 (p4 leaves; lines 5, 6): lines 5 and 6 carry both loop momenta -- non-planar."""
+    edges = [(0, 1, 0.0), (0, 2, 0.0), (1, 3, 0.0), (2, 4, 1.0), (2, 5, 1.0), (5, 3, 1.0), (4, 3, 1.0)]
+    return _gghh_two_loop("paper_ID_nonplanar_double_box", edges, lam, s, t, mt, mh)
 
 
 def double_box(s: float = -3.0, t: float = -1.0, p2: Sequence[float] = (0, 0, 0, 0), eps_order: int = 0) -> Workload:

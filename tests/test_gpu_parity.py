@@ -237,3 +237,20 @@ def test_kinematic_scan_points_of_the_papers_box():
     sig = np.hypot(abs(vals[0].err[-1]), abs(vals[1].err[-1]))
     assert abs(d) < 6 * sig and abs(vals[0].coeff[-1].imag) > 0.1
     assert not vals[0].counters[:2].any() and not vals[1].counters[:2].any()
+
+
+@pytest.mark.parametrize("which", ["table2_IC", "table3_ID"])
+def test_paper_tables_2_and_3_on_gpu(which):
+    """the paper's own two-loop integrals in the physical region (Eqs. 25, 27; Tables 2, 3):
+    per-sector parity with the oracle at a small lattice, then the printed P_2, P_1, P_0 at N = 1048573."""
+    from test_oracle_paper_table23 import compare, laurent_P, load_table
+    wl, table = (qi.paper_IC(), load_table("paper_table2.txt")) if which == "table2_IC" else (qi.paper_ID(), load_table("paper_table3.txt"))
+    parity(wl, 16381, 2, sectors=(0, 12))
+    parity(wl, 16381, 2, sectors=(30, 46))
+    t = q.qmc_prepare(wl, eps_order=0, lam=wl.lam)
+    assert (t.k_min, t.k_max, t.is_complex) == (-2, 0, True)
+    r = q.qmc_integrate(t, 1048573, 20, seed=5)
+    assert r.counters[0] == 0 and r.counters[2] == 0
+    P = laurent_P(r.shift_totals, wl.meta["s_over_mt2"])
+    assert max(P[0][1], P[0][2]) / abs(P[0][0]) < 2e-3          # the finite part to the paper's O(1e-3)
+    compare(P, table, 5.0)
