@@ -250,7 +250,7 @@ void mean_err(const double *v, size_t stride, int m, double *mean, double *err) 
 int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t st, uint64_t N, int m, int sb, int se,
               bool persec, uint64_t ibeg, uint64_t istep, uint64_t icount, const uint64_t *z, int sms, int smem_optin,
               int *gx_out, int *rows_out, int *launches_out, size_t *h2d, cudaError_t *ce_out) {
-  const int n = t->n, nacc = QMC_MAXSING + t->kmax + 1, T = QMC2_THREADS;
+  const int n = t->n, nacc = QMC_MAXSING + t->kmax + 1, T = t->threads_real;
   int max_nslots = 0;
   for (const Qmc2Chunk &c : t->chunks)
     if (c.sec_end > sb && c.sec_begin < se) max_nslots = std::max(max_nslots, c.nslots + c.max_local);
@@ -287,7 +287,7 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
   const int nitems = (int)runs.size();
   const size_t smem = fixed + accbytes * max_nsec;
   int bps = 0;
-  CUDA_OK(qmc4_kernel_prepare(n, t->L, t->kmax, smem, &bps));
+  CUDA_OK(qmc4_kernel_prepare(n, t->L, t->kmax, T, smem, &bps));
   if (bps < 1) return QMC_ECUDA;
   int waves = 16;
   if (const char *e = std::getenv("QMC2_WAVES")) waves = std::max(1, std::atoi(e));
@@ -368,7 +368,7 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
           }
     }
     cudaStream_t ls = nstreams ? static_cast<cudaStream_t>(t->side_streams[i % nstreams]) : st;
-    ce = qmc4_kernel_launch(n, t->L, t->kmax, dim3((unsigned)nsl[i], (unsigned)m), smem, ls, p);
+    ce = qmc4_kernel_launch(n, t->L, t->kmax, T, dim3((unsigned)nsl[i], (unsigned)m), smem, ls, p);
     *h2d += offsetof(Qmc4Launch, tab) + pg.size() * 4 + (w1 - w0) * 16;  // the tables travel with the launch
   }
   if (nstreams)
@@ -388,7 +388,7 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
 int launch_v5(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t st, uint64_t N, int m, int sb, int se,
               bool persec, uint64_t ibeg, uint64_t istep, uint64_t icount, const uint64_t *z, int sms, int smem_optin,
               int *gx_out, int *rows_out, int *launches_out, size_t *h2d, cudaError_t *ce_out) {
-  const int n = t->n, nacc = 2 * (QMC_MAXSING + t->kmax + 1), T = QMC2_THREADS;  // accumulators: (Re, Im) per order
+  const int n = t->n, nacc = 2 * (QMC_MAXSING + t->kmax + 1), T = QMC3_THREADS;  // accumulators: (Re, Im) per order
   int max_r = 0, max_c = 0;
   for (size_t ci = 0; ci < t->chunks3.size(); ++ci) {
     const Qmc2Chunk &c = t->chunks3[ci];

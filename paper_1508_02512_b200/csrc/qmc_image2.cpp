@@ -65,10 +65,11 @@ void putf64(std::vector<uint32_t> &v, double d) {
 void pad4(std::vector<uint32_t> &v) {
   while (v.size() % 4) v.push_back(0);
 }
-void put_rec(std::vector<uint32_t> &v, const Qmc2Rec &r) {
+// record of the planning image (offsets = slot * QMC2_THREADS * 8) -> record for T threads per block
+void put_rec(std::vector<uint32_t> &v, const Qmc2Rec &r, uint32_t T) {
   putf64(v, r.c);
-  v.push_back(r.s0);
-  v.push_back(r.s1);
+  v.push_back(r.s0 / (QMC2_THREADS * 8u) * T * 8u);
+  v.push_back(r.s1 / (QMC2_THREADS * 8u) * T * 8u);
 }
 }  // namespace
 
@@ -77,6 +78,18 @@ int qmc_build_image2(qmc_tables *t) {
   t->tab4.clear();
   t->secoff4.clear();
   t->prog4.clear();
+  {
+    // Threads per block of the real-path kernel, measured on B200 (kernels): tables dominated by sectors
+    // with three or four singular variables execute long straight-line code paths, and one 512-thread block per SM (all
+    // 16 warps walking the same sectors) fetches instructions better than four independent 128-thread blocks
+    // (cfg4: 247 / 261 / 304 ms at 512 / 256 / 128 threads); tables of short paths prefer the small blocks (cfg2: 23.4 /
+    // 22.4 / 21.6 ms).
+    int big = 0;
+    for (const QmcSector &s : t->sectors) big += s.nsing >= 3;
+    t->threads_real = 2 * big >= (int)t->sectors.size() ? 512 : 128;
+    if (const char *e = std::getenv("QMC4_THREADS")) t->threads_real = std::atoi(e) == 128 ? 128 : 512;
+  }
+  const uint32_t T4 = (uint32_t)t->threads_real;
   t->image2.clear();
   t->secoff2.clear();
   t->chunks.clear();
@@ -139,8 +152,8 @@ int qmc_build_image2(qmc_tables *t) {
     ch.prog_bytes = (uint32_t)t->image2.size() - ch.prog_off;
     std::vector<uint32_t> prog4;
     for (auto &pr : pl.prog) {
-      put32(prog4, (uint32_t)pr.first * QMC2_THREADS * 8u);
-      put32(prog4, (uint32_t)pr.second * QMC2_THREADS * 8u);
+      put32(prog4, (uint32_t)pr.first * T4 * 8u);
+      put32(prog4, (uint32_t)pr.second * T4 * 8u);
     }
     pad4(prog4);
     const size_t tab4_mark = t->tab4.size();
@@ -240,8 +253,8 @@ int qmc_build_image2(qmc_tables *t) {
         put32(v, 0);         // size of the block in words (patched below)
         put32(v, 9 + nlw);   // first record
         put32(v, 0);
-        for (int k = 0; k < QMC_MAXSING; ++k) put32(v, (uint32_t)h.sing_ln[k] * 8u);
-        for (int k = 0; k < QMC_MAXSING; ++k) put32(v, (uint32_t)h.sing_inv[k] * 8u);
+        for (int k = 0; k < QMC_MAXSING; ++k) put32(v, (uint32_t)(h.sing_ln[k] / QMC2_THREADS) * T4 * 8u);
+        for (int k = 0; k < QMC_MAXSING; ++k) put32(v, (uint32_t)(h.sing_inv[k] / QMC2_THREADS) * T4 * 8u);
         for (int k = 0; k < QMC_MAXSING; ++k) putf64(v, h.invbeta[k]);
         for (int k = 0; k < QMC_MAXSING; ++k) putf64(v, h.beta[k]);
         uint8_t extraU[16] = {0}, extraF[16] = {0};
@@ -252,25 +265,25 @@ int qmc_build_image2(qmc_tables *t) {
         for (int q = 0; q < 4; ++q) put32(v, extraU[4 * q] | (extraU[4 * q + 1] << 8) | (extraU[4 * q + 2] << 16) | ((uint32_t)extraU[4 * q + 3] << 24));
         for (int q = 0; q < 4; ++q) put32(v, extraF[4 * q] | (extraF[4 * q + 1] << 8) | (extraF[4 * q + 2] << 16) | ((uint32_t)extraF[4 * q + 3] << 24));
         for (auto &pr : local) {
-          put32(v, (uint32_t)pr.first * QMC2_THREADS * 8u);
-          put32(v, (uint32_t)pr.second * QMC2_THREADS * 8u);
+          put32(v, (uint32_t)pr.first * T4 * 8u);
+          put32(v, (uint32_t)pr.second * T4 * 8u);
         }
         pad4(v);
         size_t ri = 0;
-        put_rec(v, recs[ri++]);                                  // G0
-        for (int q = 0; q < h.nL0; ++q) put_rec(v, recs[ri++]);  // L0
+        put_rec(v, recs[ri++], T4);                                  // G0
+        for (int q = 0; q < h.nL0; ++q) put_rec(v, recs[ri++], T4);  // L0
         const Qmc2Rec empty = {0.0, ONE, ONE};
         std::vector<Qmc2Rec> extra;
         for (int which = 0; which < 2; ++which)
           for (int g = 0; g < nc; ++g) {
             const int cnt = (which ? h.cntF : h.cntU)[g];
-            put_rec(v, cnt ? recs[ri] : empty);
+            put_rec(v, cnt ? recs[ri] : empty, T4);
             for (int q = 1; q < cnt; ++q) extra.push_back(recs[ri + q]);
             ri += cnt;
           }
-        for (const Qmc2Rec &r : extra) put_rec(v, r);
-        put_rec(v, empty);  // sentinels: the kernel requests operands one record and offsets two records past the last
-        put_rec(v, empty);
+        for (const Qmc2Rec &r : extra) put_rec(v, r, T4);
+        put_rec(v, empty, T4);  // sentinels: the kernel requests operands one record and offsets two records past the last
+        put_rec(v, empty, T4);
         v[b0 + 1] = (uint32_t)((v.size() - b0) / 4);
       }
     }

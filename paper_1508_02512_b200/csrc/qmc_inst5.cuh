@@ -8,9 +8,9 @@ static cudaError_t qmc5_op(int op, dim3 grid, size_t smem, cudaStream_t st, cons
   if (op == 0) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(bps, kern, QMC2_THREADS, smem);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(bps, kern, QMC3_THREADS, smem);
   }
-  kern<<<grid, QMC2_THREADS, smem, st>>>(*p);
+  kern<<<grid, QMC3_THREADS, smem, st>>>(*p);
   return cudaGetLastError();
 }
 

@@ -67,6 +67,24 @@ __device__ __forceinline__ double fast_rcp(double x) {
   return fma(r, fma(e, e, e), r);
 }
 
+// sum of v over the block (valid in thread 0): warp shuffle tree, then pairwise over the warps; fixed order
+template <int T>
+__device__ __forceinline__ double block_sum_t(double v, double *scratch /*[T / 32]*/) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  __syncthreads();
+  if (lane == 0) scratch[wid] = v;
+  __syncthreads();
+  double r = 0.0;
+  if (wid == 0) {
+    r = (lane < T / 32) ? scratch[lane] : 0.0;
+#pragma unroll
+    for (int o = (T / 64); o > 0; o >>= 1) r += __shfl_down_sync(0xffffffffu, r, o);
+  }
+  return r;
+}
+
 __device__ __forceinline__ double slot_at(const unsigned char *__restrict__ sl, uint32_t off) {
   return *reinterpret_cast<const double *>(sl + off);
 }
@@ -81,10 +99,10 @@ __device__ __forceinline__ double u2d(uint32_t lo, uint32_t hi) { return __hiloi
 
 // one sector at one point: out[i] = coefficient of eps^(i - NS) of the subtracted integrand (without the weight w).
 // `o` = word offset of the sector block in p.tab (uniform).
-template <int NDIM, int L, int NS, int KMAX>
+template <int NDIM, int L, int NS, int KMAX, int T>
 __device__ __forceinline__ void sector4(const Qmc4Launch &p, const uint32_t o, unsigned char *__restrict__ sl,
                                         const double2 *__restrict__ tabq, double (&out)[KMAX + NS + 1]) {
-  constexpr int K = KMAX + NS + 1, NC = 1 << NS, FULL = NC - 1, T = QMC2_THREADS;
+  constexpr int K = KMAX + NS + 1, NC = 1 << NS, FULL = NC - 1;
   typedef Expo<NDIM, L> E;
   const uint4 h0 = p.tab[o];
   const uint32_t nL0 = (h0.x >> 8) & 255u, nlocal = (h0.x >> 16) & 255u;
@@ -196,18 +214,15 @@ __device__ __forceinline__ void sector4(const Qmc4Launch &p, const uint32_t o, u
 #ifndef Q4_NOPERSEC
 #define Q4_NOPERSEC 0
 #endif
-#ifndef QMC4_MIN_BLOCKS
-#define QMC4_MIN_BLOCKS 2
-#endif
 
 // partial layout: fused  : [run of sectors][shift][slice][NACC]
 //                 persec : [sector row][shift][slice][NACC]        (NACC = QMC_MAXSING + KMAX + 1, index a <-> order a - QMC_MAXSING)
-template <int NDIM, int L, int KMAX>
-__global__ void __launch_bounds__(QMC2_THREADS, QMC4_MIN_BLOCKS) qmc4_eval_kernel(const __grid_constant__ Qmc4Launch p) {
+// T = threads per block (128 or 512; 512 registers-worth of threads per SM either way: 128 registers per thread)
+template <int NDIM, int L, int KMAX, int T>
+__global__ void __launch_bounds__(T, 512 / T) qmc4_eval_kernel(const __grid_constant__ Qmc4Launch p) {
   using namespace qmc4;
   constexpr int NACC = QMC_MAXSING + KMAX + 1;
   constexpr int SMAX = NDIM < QMC_MAXSING ? NDIM : QMC_MAXSING;
-  constexpr int T = QMC2_THREADS;
 
   extern __shared__ __align__(16) unsigned char smem[];
   const int tid = threadIdx.x;
@@ -305,7 +320,7 @@ __global__ void __launch_bounds__(QMC2_THREADS, QMC4_MIN_BLOCKS) qmc4_eval_kerne
     if (NS_ <= SMAX) {                                                                                       \
       constexpr int NSC = NS_ <= SMAX ? NS_ : 0, KK = KMAX + NSC + 1;                                        \
       double res[KK];                                                                                        \
-      sector4<NDIM, L, NSC, KMAX>(p, so, sl, tabq, res);                                                     \
+      sector4<NDIM, L, NSC, KMAX, T>(p, so, sl, tabq, res);                                                     \
       bool fin = true;                                                                                       \
       _Pragma("unroll") for (int i = 0; i < KK; ++i) fin = fin && finite_hi(res[i]);                         \
       /* a non-finite evaluation is dropped (and counted); a dead thread has w = 0.  Predicated, not branched */ \
@@ -347,14 +362,14 @@ __global__ void __launch_bounds__(QMC2_THREADS, QMC4_MIN_BLOCKS) qmc4_eval_kerne
       double *dst = p.partial + (((size_t)p.out_row * p.m + kap) * p.max_slices + blockIdx.x) * NACC;
 #pragma unroll
       for (int a = 0; a < NACC; ++a) {
-        double sr = qmcdev::block_sum(acc[a], scratch);
+        double sr = block_sum_t<T>(acc[a], scratch);
         if (tid == 0) dst[a] = sr;
       }
     } else {
       for (int si = 0; si < p.nsec; ++si) {
         double *dst = p.partial + (((size_t)(p.out_row + p.secrow[si]) * p.m + kap) * p.max_slices + blockIdx.x) * NACC;
         for (int a = 0; a < NACC; ++a) {
-          double v = qmcdev::block_sum(sacc[((size_t)si * NACC + a) * T + tid], scratch);
+          double v = block_sum_t<T>(sacc[((size_t)si * NACC + a) * T + tid], scratch);
           if (tid == 0) dst[a] = v;
         }
       }

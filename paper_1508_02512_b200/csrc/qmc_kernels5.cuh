@@ -62,7 +62,7 @@ __device__ __forceinline__ void corner5(const Qmc5Launch &p, const uint32_t cw, 
                                         const double G0, const double L0, unsigned char *__restrict__ slr,
                                         unsigned char *__restrict__ slc, const double2 *__restrict__ tabq, cd &Wout, cd &Lout,
                                         unsigned &cntImF, unsigned &cntReU) {
-  constexpr int T = QMC2_THREADS, NDERIV = NDIM + NDIM * (NDIM + 1) / 2, NPOLY = NDERIV + 2, CW = (NPOLY + 15) / 16;
+  constexpr int T = QMC3_THREADS, NDERIV = NDIM + NDIM * (NDIM + 1) / 2, NPOLY = NDERIV + 2, CW = (NPOLY + 15) / 16;
   typedef Expo<NDIM, L> E;
   uint32_t zv = 0;  // variables set to zero
 #pragma unroll
@@ -266,7 +266,7 @@ template <int NDIM, int L, int NS, int KMAX>
 __device__ __forceinline__ void sector5(const Qmc5Launch &p, const uint32_t o, unsigned char *__restrict__ slr,
                                         unsigned char *__restrict__ slc, const double2 *__restrict__ tabq,
                                         cd (&out)[KMAX + NS + 1], unsigned &cntImF, unsigned &cntReU) {
-  constexpr int K = KMAX + NS + 1, NG = 1 << NS, T = QMC2_THREADS;
+  constexpr int K = KMAX + NS + 1, NG = 1 << NS, T = QMC3_THREADS;
   const uint4 h0 = p.tab[o], h1 = p.tab[o + 1], h2 = p.tab[o + 2];
   const uint32_t nL0 = (h0.x >> 8) & 255u, nlocal_r = (h0.x >> 16) & 255u, nlocal_c = (h0.x >> 24) & 255u;
   const uint32_t lrw = o + 8, lcw = lrw + ((nlocal_r + 1) >> 1);
@@ -322,11 +322,11 @@ __device__ __forceinline__ bool finite_hi(cd v) {
 
 // partial layout: fused [run][shift][slice][NACC][2], persec [sector row][shift][slice][NACC][2]
 template <int NDIM, int L, int KMAX>
-__global__ void __launch_bounds__(QMC2_THREADS, (NDIM <= 4 ? 2 : 1)) qmc5_eval_kernel(const __grid_constant__ Qmc5Launch p) {
+__global__ void __launch_bounds__(QMC3_THREADS, (NDIM <= 4 ? 512 : 256) / QMC3_THREADS) qmc5_eval_kernel(const __grid_constant__ Qmc5Launch p) {
   using namespace qmc5;
   constexpr int NACC = QMC_MAXSING + KMAX + 1;
   constexpr int SMAX = NDIM < QMC3_MAXSING ? NDIM : QMC3_MAXSING;
-  constexpr int T = QMC2_THREADS;
+  constexpr int T = QMC3_THREADS;
 
   extern __shared__ __align__(16) unsigned char smem[];
   const int tid = threadIdx.x;
@@ -454,8 +454,8 @@ __global__ void __launch_bounds__(QMC2_THREADS, (NDIM <= 4 ? 2 : 1)) qmc5_eval_k
       double *dst = p.partial + (((size_t)p.out_row * p.m + kap) * p.max_slices + blockIdx.x) * (NACC * 2);
 #pragma unroll
       for (int a = 0; a < NACC; ++a) {
-        double sr = qmcdev::block_sum(acc[a].re, scratch);
-        double si = qmcdev::block_sum(acc[a].im, scratch);
+        double sr = qmc4::block_sum_t<T>(acc[a].re, scratch);
+        double si = qmc4::block_sum_t<T>(acc[a].im, scratch);
         if (tid == 0) {
           dst[2 * a] = sr;
           dst[2 * a + 1] = si;
@@ -465,7 +465,7 @@ __global__ void __launch_bounds__(QMC2_THREADS, (NDIM <= 4 ? 2 : 1)) qmc5_eval_k
       for (int si = 0; si < p.nsec; ++si) {
         double *dst = p.partial + (((size_t)(p.out_row + p.secrow[si]) * p.m + kap) * p.max_slices + blockIdx.x) * (NACC * 2);
         for (int a = 0; a < NACC * 2; ++a) {
-          double v = qmcdev::block_sum(sacc[((size_t)si * NACC * 2 + a) * T + tid], scratch);
+          double v = qmc4::block_sum_t<T>(sacc[((size_t)si * NACC * 2 + a) * T + tid], scratch);
           if (tid == 0) dst[a] = v;
         }
       }

@@ -67,8 +67,9 @@ struct Qmc4Launch {
   uint4 tab[QMC4_TAB_WORDS];
 };
 static_assert(sizeof(Qmc4Launch) <= 32764, "kernel parameter limit");
-cudaError_t qmc4_kernel_prepare(int ndim, int loops, int kmax, size_t smem, int *blocks_per_sm);
-cudaError_t qmc4_kernel_launch(int ndim, int loops, int kmax, dim3 grid, size_t smem, cudaStream_t st, const Qmc4Launch &p);
+cudaError_t qmc4_kernel_prepare(int ndim, int loops, int kmax, int threads, size_t smem, int *blocks_per_sm);
+cudaError_t qmc4_kernel_launch(int ndim, int loops, int kmax, int threads, dim3 grid, size_t smem, cudaStream_t st,
+                               const Qmc4Launch &p);
 bool qmc4_kernel_available(int ndim, int loops, int kmax);
 
 // ---- version 5 (complex path, tables in the kernel-parameter constant bank) ---------------------------------------

@@ -37,7 +37,7 @@ static_assert(sizeof(QmcSectorHdr) == 64, "sector header must be 64 bytes");
 //   slots [0,n) t_j | [n,2n) ln t_j | [2n,3n) 1/t_j | 3n: 1.0 | 3n+1 ...: products slot[k] = slot[a] * slot[b]
 // chosen per chunk by a byte-pair-encoding style pass over the chunk's monomials (most frequent pair of factors
 // first) until every monomial is a product of at most two slots.  A monomial is then one 16-byte record.
-#define QMC2_THREADS 256
+#define QMC2_THREADS 256   // planning image only; the real-path kernel runs 128 or 512 threads per block (qmc_tables::threads_real)
 #define QMC2_MAXSLOTS 56
 struct Qmc2Rec {        // value = c * slot[s0] * slot[s1]; s0, s1 are BYTE offsets slot * QMC2_THREADS * 8 into the
   double c;             // thread's column of the slot table
@@ -77,7 +77,7 @@ struct Qmc2Chunk {      // host description of one chunk
 // own -- and the regular-variable factors; and a COMPLEX one over the deformed variables z_j (z_j, 1, products),
 // refilled at every corner, that serves U^(z) and F^(z).  Records are sorted per polynomial by group; a corner Z keeps
 // the groups disjoint from Z.
-#define QMC3_THREADS 256
+#define QMC3_THREADS 128
 #define QMC3_MAXSLOTS_R 56
 #define QMC3_MAXSLOTS_C 40
 #define QMC3_MAXLOCAL 8
@@ -130,6 +130,8 @@ struct qmc_tables {
   std::vector<double> sec_cost;   // modelled cost per sector (load balancing of the launch)
   // version 4 tables (real path; same chunks and slot programs as version 2, laid out for the kernel-parameter
   // constant bank: see qmc_launch.h)
+  int threads_real = 512;           // threads per block of the real-path kernel: the slot offsets in tab4 / prog4 are
+                                    // premultiplied by it (chosen by qmc_build_image2, see there)
   std::vector<uint32_t> tab4;       // sector blocks, 32-bit words (4 per 16-byte table word)
   std::vector<uint32_t> secoff4;    // [n_sectors + 1] offsets into tab4 in 16-byte words
   std::vector<std::vector<uint32_t>> prog4;  // per chunk: slot program {a_off, b_off} byte offsets, padded to 16 bytes
