@@ -56,6 +56,26 @@ __device__ __forceinline__ double fast_log(double x, const double2 *__restrict__
   const double v = fma(r * r, q, r) + y0;
   return ok ? v : __longlong_as_double(0x7ff8000000000000ll);
 }
+// the same without the argument test: `worst` collects max (hi - 0x00100000) as unsigned over a sector's corners, and the
+// sector's result is dropped as a whole when worst >= 0x7fe00000 (some argument was not a positive normal number) --
+// what the NaN of fast_log achieved through `finite_hi` of the results, at 2 instead of 4 integer instructions per corner
+__device__ __forceinline__ double fast_log_unchecked(double x, const double2 *__restrict__ tabq, unsigned &worst) {
+  const int hi = __double2hiint(x), lo = __double2loint(x);
+  worst = max(worst, (unsigned)(hi - 0x00100000));
+  const int tmp = hi - 0x3fe60000;
+  const int e = tmp >> 20;
+  const double2 T = *reinterpret_cast<const double2 *>(reinterpret_cast<const unsigned char *>(tabq) +
+                                                      ((tmp >> (14 - 7)) & ((QMC4_LOG_ENTRIES - 1) << 7)));
+  const double z = __hiloint2double(hi - (tmp & 0xfff00000), lo);
+  const double r = fma(z, T.x, -1.0);
+  const double y0 = fma((double)e, qmc4_logc[0], T.y);
+  double q = fma(r, qmc4_logc[1], qmc4_logc[2]);
+  q = fma(r, q, qmc4_logc[3]);
+  q = fma(r, q, qmc4_logc[4]);
+  q = fma(r, q, qmc4_logc[5]);
+  q = fma(r, q, qmc4_logc[6]);
+  return fma(r * r, q, r) + y0;
+}
 static_assert(QMC4_LOG_COPIES * 16 == 1 << 7, "fast_log index arithmetic assumes 128 bytes per table entry row");
 
 // 1/x to ~1 ulp: MUFU.RCP64H seed (about 20 bits) + ONE cubic step r (1 + e + e^2), e = 1 - x r: 3 FP64 instructions
@@ -100,8 +120,9 @@ __device__ __forceinline__ double u2d(uint32_t lo, uint32_t hi) { return __hiloi
 // one sector at one point: out[i] = coefficient of eps^(i - NS) of the subtracted integrand (without the weight w).
 // `o` = word offset of the sector block in p.tab (uniform).
 template <int NDIM, int L, int NS, int KMAX, int T>
-__device__ __forceinline__ void sector4(const Qmc4Launch &p, const uint32_t o, unsigned char *__restrict__ sl,
+__device__ __forceinline__ bool sector4(const Qmc4Launch &p, const uint32_t o, unsigned char *__restrict__ sl,
                                         const double2 *__restrict__ tabq, double (&out)[KMAX + NS + 1]) {
+  unsigned worst = 0;  // fast_log_unchecked
   constexpr int K = KMAX + NS + 1, NC = 1 << NS, FULL = NC - 1;
   typedef Expo<NDIM, L> E;
   const uint4 h0 = p.tab[o];
@@ -127,10 +148,16 @@ __device__ __forceinline__ void sector4(const Qmc4Launch &p, const uint32_t o, u
     // first record of every group (dense, compile-time destination), then the extra records group by group;
     // subset sums: P[X] = value with the singular variables outside X set to zero
     double PU[NC], PF[NC];
+    const unsigned char *tb = reinterpret_cast<const unsigned char *>(p.tab);
+    {
+      // (pointer + compile-time offset, not p.tab[rw + g]: the 32-bit index sum may wrap, so ptxas computed every record's
+      //  address with its own UIADD3 + ULEA and then ran out of uniform registers -- 4 extra instructions per record)
+      const unsigned char *fr = tb + rw * 16u;
 #pragma unroll
-    for (int g = 0; g < NC; ++g) PU[g] = rec_val(p.tab[rw + g], sl);
+      for (int g = 0; g < NC; ++g) PU[g] = rec_val(*reinterpret_cast<const uint4 *>(fr + g * 16), sl);
 #pragma unroll
-    for (int g = 0; g < NC; ++g) PF[g] = rec_val(p.tab[rw + NC + g], sl);
+      for (int g = 0; g < NC; ++g) PF[g] = rec_val(*reinterpret_cast<const uint4 *>(fr + (NC + g) * 16), sl);
+    }
     rw += 2 * NC;
     const uint4 cu = p.tab[o + 7], cf = p.tab[o + 8];
     const uint32_t cuw[4] = {cu.x, cu.y, cu.z, cu.w}, cfw[4] = {cf.x, cf.y, cf.z, cf.w};
@@ -139,7 +166,6 @@ __device__ __forceinline__ void sector4(const Qmc4Launch &p, const uint32_t o, u
     // harmless sentinel record), so the LDCU -> LDS -> DMUL -> DFMA chain is not exposed once per group
     // (only the OFFSETS of the next record are requested ahead; its coefficient is loaded in its own iteration, where the
     //  wait for the slot operands hides the latency -- carrying it across the iteration cost two UMOV per record)
-    const unsigned char *tb = reinterpret_cast<const unsigned char *>(p.tab);
     uint32_t rwb = rw * 16u;  // byte offset of the current record: {f64 c | u32 off0, u32 off1}
     uint2 ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);
     double ra = slot_at(sl, ro.x), rb = slot_at(sl, ro.y);
@@ -187,7 +213,7 @@ __device__ __forceinline__ void sector4(const Qmc4Launch &p, const uint32_t o, u
       if (E::aF0 > 0) W *= ipow_c<(E::aF0 > 0 ? E::aF0 : 0)>(F);
       if (E::aF0 < 0) W *= ipow_c<(E::aF0 < 0 ? -E::aF0 : 0)>(rF);
       c.W[X] = W;
-      if (KMAX > 0 || X != FULL) c.Lam[X] = fast_log(ipow_c<E::aU1>(U) * ipow_c<-E::aF1>(rF), tabq) + L0;
+      if (KMAX > 0 || X != FULL) c.Lam[X] = fast_log_unchecked(ipow_c<E::aU1>(U) * ipow_c<-E::aF1>(rF), tabq, worst) + L0;
     }
   }
   if (NS > 0) {
@@ -207,6 +233,7 @@ __device__ __forceinline__ void sector4(const Qmc4Launch &p, const uint32_t o, u
     }
   }
   Fold2<NS, KMAX, K, 0, 0>::eval(c, out);
+  return worst < 0x7fe00000u;
 }
 
 }  // namespace qmc4
@@ -320,8 +347,7 @@ __global__ void __launch_bounds__(T, 512 / T) qmc4_eval_kernel(const __grid_cons
     if (NS_ <= SMAX) {                                                                                       \
       constexpr int NSC = NS_ <= SMAX ? NS_ : 0, KK = KMAX + NSC + 1;                                        \
       double res[KK];                                                                                        \
-      sector4<NDIM, L, NSC, KMAX, T>(p, so, sl, tabq, res);                                                     \
-      bool fin = true;                                                                                       \
+      bool fin = sector4<NDIM, L, NSC, KMAX, T>(p, so, sl, tabq, res);                                       \
       _Pragma("unroll") for (int i = 0; i < KK; ++i) fin = fin && finite_hi(res[i]);                         \
       /* a non-finite evaluation is dropped (and counted); a dead thread has w = 0.  Predicated, not branched */ \
       cntNonFinite += (live && !fin) ? 1u : 0u;                                                              \
