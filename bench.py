@@ -97,6 +97,10 @@ def oracle_sample(wl, N, z, shifts, target_s: float):
     o.integrate(N, z, shifts[:m_s], index_range=(0, 1, count))
     dt = time.perf_counter() - t0
     val = count * m_s * o.n_sectors / dt
+    c1 = max(64, count // (4 * cores))
+    t0 = time.perf_counter()
+    o.integrate(N, z, shifts[:m_s], index_range=(0, 1, c1), threads=1)
+    oracle_sample.single_thread = c1 * m_s * o.n_sectors / (time.perf_counter() - t0)
     return val, cores, (f"{wl.name}: lattice indices 0..{count - 1} of N={N}, all {o.n_sectors} sectors, {m_s} shifts, "
                         f"{dt:.1f} s on {cores} threads (OpenMP), g++ -O2")
 
@@ -160,6 +164,31 @@ def time_to_accuracy(q, wl, torch, target=1e-3, max_N=2 ** 27):
     dt = time.perf_counter() - t0
     return {"workload": wl.name, "target_rel_err": target, "wall_s": dt, "N_reached": tried[-1], "N_tried": len(tried),
             "rel_err": rel, "coeff_eps0": [c0.real, c0.imag], "err_eps0": [e0.real, e0.imag], "m": wl.m}
+
+
+def convergence(q, wl, k_lo=14, k_hi=20):
+    """error estimate of the eps^0 coefficient of J against N over the primes below 2^k, and the
+    least-squares slope of log(error) against log(N) (the paper claims "close to O(n^-1)")."""
+    t = q.qmc_prepare(wl, eps_order=wl.eps_order, lam=wl.lam)
+    Ns, rels = [], []
+    for N in qi.primes_below_pow2(k_lo, k_hi):
+        r = q.qmc_integrate(t, N, wl.m, seed=wl.seed)
+        c0, e0 = r.coeff[-1 - wl.eps_order], r.err[-1 - wl.eps_order]
+        Ns.append(int(N))
+        rels.append(float(max(e0.real, e0.imag) / abs(c0)))
+    slope = float(np.polyfit(np.log(Ns), np.log(rels), 1)[0])
+    return {"workload": wl.name, "m": wl.m, "N": Ns, "rel_err_eps0": rels, "fitted_exponent": slope}
+
+
+def per_sector_mode(q, t, N, m, z, shifts, dev, torch):
+    """the per-sector (parity) mode of the kernel next to the fused (throughput) mode the headline times."""
+    q.qmc_integrate(t, N, m, z=z, shifts=shifts, per_sector=True, device=dev)
+    r = q.qmc_integrate(t, N, m, z=z, shifts=shifts, per_sector=True, device=dev)
+    f = q.qmc_integrate(t, N, m, z=z, shifts=shifts, device=dev)
+    tot = r.shift_sums.sum(axis=0)
+    scale = np.abs(r.shift_sums).sum(axis=0)
+    return {"eval_kernel_ms": float(r.eval_kernel_ms), "fused_eval_kernel_ms": float(f.eval_kernel_ms),
+            "max_rel_diff_of_totals": float(np.max(np.abs(tot - f.shift_totals) / np.maximum(scale, 1e-300)))}
 
 
 def kinematic_scan(q, torch, n_points=1000, N=99991, m=16):
@@ -311,7 +340,8 @@ def run_product(args):
     if world == 1 and not args.no_extras:
         z_o = test_vector(N, wl.dim)
         v, cores, desc = oracle_sample(wl, N, z_o, qi.splitmix64_shifts(wl.seed, m, wl.dim), 15.0)
-        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+                                "single_thread_value": oracle_sample.single_thread}
         def extra(fn, *a, **k):       # the context numbers must not take the headline line down with them
             try:
                 return fn(*a, **k)
@@ -321,7 +351,11 @@ def run_product(args):
         # (Tables 2-3: 19 s and 20 s on a K20)
         line["time_to_1e-3"] = [extra(time_to_accuracy, q, w, torch)
                                 for w in (qi.double_box(), qi.nonplanar_vertex(), qi.paper_IC(), qi.paper_ID())]
-        line["time_to_1e-5"] = [extra(time_to_accuracy, q, qi.nonplanar_vertex(), torch, target=1e-5, max_N=2 ** 24)]
+        line["time_to_1e-5"] = [extra(time_to_accuracy, q, w, torch, target=1e-5, max_N=2 ** 24)
+                                for w in (qi.double_box(), qi.nonplanar_vertex())]
+        line["time_to_1e-6"] = [extra(time_to_accuracy, q, qi.nonplanar_vertex(), torch, target=1e-6, max_N=2 ** 24)]
+        line["convergence"] = [extra(convergence, q, w) for w in (qi.massless_box(), qi.double_box(), qi.nonplanar_vertex())]
+        line["per_sector_mode"] = extra(per_sector_mode, q, t, N, m, z, shifts, dev, torch)
         line["other_workloads"] = extra(other_workloads, q, torch, dev, args.config)
         line["kinematic_scan"] = extra(kinematic_scan, q, torch)
     print(json.dumps(line), flush=True)
