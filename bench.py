@@ -180,6 +180,28 @@ def convergence(q, wl, k_lo=14, k_hi=20):
     return {"workload": wl.name, "m": wl.m, "N": Ns, "rel_err_eps0": rels, "fitted_exponent": slope}
 
 
+def cbc_vs_korobov(q, dev):
+    """error estimate of the eps^0 coefficient with the component-by-component vector the paper names
+    (host construction, timed) next to the Korobov-form vector of the P_2 search (reading C13), same N,
+    shifts and kernels."""
+    out = []
+    for wl, N in ((qi.massless_box(), 1048573), (qi.double_box(), 262139), (qi.nonplanar_vertex(), 262139)):
+        t = q.qmc_prepare(wl, eps_order=wl.eps_order, lam=wl.lam)
+        t0 = time.perf_counter()
+        zc = q.qmc_cbc_vector(N, t.dim)
+        t_cbc = time.perf_counter() - t0
+        zk = q.qmc_generating_vector(N, t.dim, device=dev)
+        sh = qi.splitmix64_shifts(wl.seed, wl.m, t.dim)
+        row = {"workload": wl.name, "N": N, "m": wl.m, "cbc_construction_s": t_cbc}
+        for name, z in (("cbc", zc), ("korobov", zk)):
+            r = q.qmc_integrate(t, N, wl.m, z=z, shifts=sh, device=dev)
+            c0, e0 = r.coeff[-1 - wl.eps_order], r.err[-1 - wl.eps_order]
+            row[name] = {"z": [int(v) for v in z], "coeff_eps0": [c0.real, c0.imag],
+                         "rel_err_eps0": float(max(e0.real, e0.imag) / abs(c0))}
+        out.append(row)
+    return out
+
+
 def per_sector_mode(q, t, N, m, z, shifts, dev, torch):
     """the per-sector (parity) mode of the kernel next to the fused (throughput) mode the headline times."""
     q.qmc_integrate(t, N, m, z=z, shifts=shifts, per_sector=True, device=dev)
@@ -355,6 +377,7 @@ def run_product(args):
                                 for w in (qi.double_box(), qi.nonplanar_vertex())]
         line["time_to_1e-6"] = [extra(time_to_accuracy, q, qi.nonplanar_vertex(), torch, target=1e-6, max_N=2 ** 24)]
         line["convergence"] = [extra(convergence, q, w) for w in (qi.massless_box(), qi.double_box(), qi.nonplanar_vertex())]
+        line["cbc_vs_korobov"] = extra(cbc_vs_korobov, q, dev)
         line["per_sector_mode"] = extra(per_sector_mode, q, t, N, m, z, shifts, dev, torch)
         line["other_workloads"] = extra(other_workloads, q, torch, dev, args.config)
         line["kinematic_scan"] = extra(kinematic_scan, q, torch)

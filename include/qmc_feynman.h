@@ -166,6 +166,14 @@ int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t sector_end
  * device (needs workspace of qmc_workspace_bytes). */
 int qmc_generating_vector(uint64_t N, int32_t dim, void *cuda_stream, void *dev_workspace, size_t dev_workspace_bytes,
                           uint64_t *z_out);
+/* Generating vector by the component-by-component construction the paper names (refs [29, 30]): z_1 = 1, then
+ * z_d = argmin over z in [1, (N-1)/2] of  e^2(z_1..z_d) = -1 + (1/N) sum_i prod_j (1 + 2 pi^2 B_2({i z_j / N}))  (the P_2
+ * criterion of R:C13 with unit weights; ties -> smaller z; R:C25).  HOST function, O(dim N log N): the candidates of one
+ * component are one cyclic convolution over the multiplicative group of the prime N (FFT), which only screens; the
+ * decision is taken on plain O(N) sums of the closest candidates.  N an odd prime below 2^26, 1 <= dim <= 16, else
+ * QMC_EINVAL; QMC_ENOMEM if the host work arrays (about 50 N bytes) cannot be allocated.  z_out[dim] caller-owned;
+ * e2_out[dim] (NULL = not wanted) receives the criterion after each component. */
+int qmc_cbc_vector(uint64_t N, int32_t dim, uint64_t *z_out, double *e2_out);
 /* m shift vectors from the SplitMix64 stream keyed by seed: Delta = (u64 >> 11) * 2^-53, shift-major (R:C14) */
 int qmc_shifts(uint64_t seed, int32_t m, int32_t dim, double *shifts_out);
 /* Laurent series of  e^{eg * eps * gamma_E} * base^{p0 + p1 eps} * Gamma(g0 + g1 eps),  g0 a non-negative integer,

@@ -9,6 +9,9 @@ criterion nor the weights; reading C25 fixes them the way reading C13 
 
     z_1 = 1;  for d = 2..s:  z_d = argmin over z in {1, .., (N-1)/2} of e^2(z_1, .., z_{d-1}, z),  ties -> smaller z
     (N an odd prime; omega(x) = omega(1-x) makes z and N-z exactly equivalent, so only the lower half is searched).
+    A tie is a value within TIE_TOL * (1 + minimum) of the minimum: e^2 is the difference of two O(1 + e^2) numbers, so
+    the mathematically exact ties of the construction (z and its inverse give the same rule in two dimensions) come out
+    of any floating-point evaluation with rounding noise of about 1e-15 (1 + e^2) and must not be decided by it.
 
 This file is the DEFINITION written out: every candidate's criterion is the plain O(N) sum, O(N^2) per component.
 No FFT, no primitive roots, no reuse across candidates beyond the running product over the components already fixed.
@@ -22,6 +25,9 @@ pairs (z_1, z_2) for small N in pure Python loops; the Fibonacci lattices in two
 from __future__ import annotations
 
 import numpy as np
+
+
+TIE_TOL = 1e-11
 
 
 def omega_from_remainder(r, N: int):
@@ -49,14 +55,13 @@ def cbc_vector(N: int, s: int, chunk: int = 256):
     e2 = [float(-1.0 + prod.sum() / N)]
     half = (N - 1) // 2
     for _ in range(1, s):
-        best_val, best_z = None, None
+        vals = np.empty(half)                                # vals[c - 1] = e^2(z_1..z_{d-1}, c)
         for c0 in range(1, half + 1, chunk):
             cand = np.arange(c0, min(c0 + chunk, half + 1), dtype=np.int64)
             r = (cand[:, None] * i[None, :]) % N             # [candidates, lattice points]
-            vals = -1.0 + ((1.0 + omega_from_remainder(r, N)) * prod[None, :]).sum(axis=1) / N
-            k = int(np.argmin(vals))                         # first minimum = smallest z of the chunk
-            if best_val is None or vals[k] < best_val:
-                best_val, best_z = float(vals[k]), int(cand[k])
+            vals[c0 - 1:c0 - 1 + len(cand)] = -1.0 + ((1.0 + omega_from_remainder(r, N)) * prod[None, :]).sum(axis=1) / N
+        best = float(vals.min())
+        best_z = int(np.nonzero(vals <= best + TIE_TOL * (1.0 + best))[0][0]) + 1   # smallest z among the ties
         z.append(best_z)
         prod = prod * (1.0 + omega_from_remainder((i * best_z) % N, N))
         e2.append(float(-1.0 + prod.sum() / N))

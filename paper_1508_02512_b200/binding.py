@@ -97,6 +97,8 @@ def lib():
         L.qmc_flop_model.restype = C.c_int
         L.qmc_flop_model.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double),
                                      C.POINTER(C.c_int64)]
+        L.qmc_cbc_vector.restype = C.c_int
+        L.qmc_cbc_vector.argtypes = [C.c_uint64, C.c_int32, C.POINTER(C.c_uint64), C.POINTER(C.c_double)]
         L.qmc_generating_vector.restype = C.c_int
         L.qmc_generating_vector.argtypes = [C.c_uint64, C.c_int32, C.c_void_p, C.c_void_p, C.c_size_t, C.POINTER(C.c_uint64)]
         L.qmc_shifts.restype = C.c_int
@@ -368,6 +370,16 @@ def qmc_generating_vector(N: int, dim: int, device="cuda:0") -> np.ndarray:
     if rc:
         raise QmcError(rc, "qmc_generating_vector")
     return z
+
+
+def qmc_cbc_vector(N: int, dim: int, with_criterion: bool = False):
+    """Component-by-component generating vector (host function of the library)."""
+    z = np.zeros(dim, dtype=np.uint64)
+    e2 = np.zeros(dim, dtype=np.float64)
+    rc = lib().qmc_cbc_vector(N, dim, _ptr(z, C.c_uint64), _ptr(e2, C.c_double))
+    if rc != 0:
+        raise QmcError(rc, "qmc_cbc_vector")
+    return (z, e2) if with_criterion else z
 
 
 def qmc_prefactor_series(eg: float, base: float, p0: float, p1: float, g0: int, g1: float, n_out: int):

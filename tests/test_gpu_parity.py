@@ -254,3 +254,14 @@ def test_paper_tables_2_and_3_on_gpu(which):
     P = laurent_P(r.shift_totals, wl.meta["s_over_mt2"])
     assert max(P[0][1], P[0][2]) / abs(P[0][0]) < 2e-3          # the finite part to the paper's O(1e-3)
     compare(P, table, 5.0)
+
+
+def test_cbc_generating_vectors_through_the_kernels():
+    """the library's component-by-component vectors drive the same kernels -- parity
+    against the oracle on the massless box and the non-planar vertex, closed form of the box within 3 sigma."""
+    N = 65521
+    z3 = q.qmc_cbc_vector(N, 3)
+    r, f, S, A, _ = parity(qi.massless_box(), N, 6, z=z3)
+    ex = [0.666666666666667, -1.2639198230760183, -1.2238036181980894]
+    assert np.all(np.abs(f.coeff.real - ex) <= 3.5 * f.err.real + 1e-13)
+    parity(qi.nonplanar_vertex(), 16381, 3, z=q.qmc_cbc_vector(16381, 5))

@@ -140,3 +140,39 @@ def test_no_cpu_fallback():
     res = q.binding.qmc_result()
     rc = q.lib().qmc_integrate(t._h, 10007, 10, 1, None, None, 0, ctypes.byref(res))
     assert rc in (-4, -5)
+
+
+# ---------------------------------------------------------------- component-by-component construction
+@pytest.mark.parametrize("N,dim", [(3, 3), (89, 2), (251, 5), (1009, 6), (4093, 6), (8191, 3)])
+def test_cbc_vector_matches_oracle_definition(N, dim):
+    # product: FFT over the multiplicative group + exact re-evaluation of the closest candidates (qmc_cbc.cpp);
+    # oracle: the O(N^2) definition (oracle/cbc.py).  Integer result: bit-exact.  Criterion: a difference of O(1 + e^2)
+    # numbers in both, so compared on that scale.
+    from oracle.cbc import cbc_vector
+    z, e2 = q.qmc_cbc_vector(N, dim, with_criterion=True)
+    zo, eo = cbc_vector(N, dim)
+    assert np.array_equal(z, zo)
+    assert np.all(np.abs(e2 - eo) <= 1e-13 * (1.0 + eo))
+
+
+def test_cbc_vector_at_a_production_size_is_a_local_optimum():
+    # N too large for the O(N^2) oracle: check what holds at any size -- range, coprimality, the reported criterion
+    # against the oracle's one-pass definition, and that no sampled candidate for any component beats the chosen one
+    from oracle.cbc import criterion
+    N, dim = 65521, 6
+    z, e2 = q.qmc_cbc_vector(N, dim, with_criterion=True)
+    assert z[0] == 1 and np.all(z >= 1) and np.all(z <= (N - 1) // 2)
+    for d in range(1, dim + 1):
+        assert abs(criterion(N, z[:d]) - e2[d - 1]) <= 1e-12 * (1.0 + e2[d - 1])
+    rng = np.random.default_rng(5)
+    for d in range(2, dim + 1):
+        for c in rng.integers(1, (N - 1) // 2 + 1, size=40):
+            assert criterion(N, list(z[:d - 1]) + [int(c)]) >= e2[d - 1] - 1e-11 * (1.0 + e2[d - 1])
+    assert np.all(np.diff(e2) > 0)          # every new factor (1 + omega) adds non-negative dual-lattice terms
+
+
+def test_cbc_vector_error_codes():
+    for N, dim in ((1, 2), (2, 2), (91, 3), (1 << 26, 2), (101, 0), (101, 17)):
+        with pytest.raises(q.QmcError) as e:
+            q.qmc_cbc_vector(N, dim)
+        assert e.value.status == -1         # QMC_EINVAL
