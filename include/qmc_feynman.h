@@ -68,7 +68,8 @@ typedef struct {
 typedef struct {
   double lambda;     /* 0: Euclidean / real path.  > 0: contour deformation z_j = t_j - i lambda t_j (1-t_j) dF/dt_j
                         (Eq. 14), complex path, all variables deformed with the same lambda (R:C11) */
-  int32_t transform; /* 0: x = 3y^2 - 2y^3, weight prod 6y(1-y) (Eq. 21).  1: tent/baker (R:C20) */
+  int32_t transform; /* 0: x = 3y^2 - 2y^3, weight prod 6y(1-y) (Eq. 21).  1: tent/baker (R:C20).
+                        2: x = 10y^3 - 15y^4 + 6y^5, weight prod 30y^2(1-y)^2 -- the next member of Eq. 21's family */
   int32_t max_depth; /* decomposition recursion cap; <= 0: 64 */
 } qmc_options;
 

@@ -349,6 +349,11 @@ bool lattice_point(uint64_t N, const uint64_t* z, int n, uint64_t i, const doubl
     if (transform == 0) {
       t[j] = v * v * (3.0 - 2.0 * v);  // Eq. 21: x = 3y^2 - 2y^3
       w *= 6.0 * v * (1.0 - v);
+    } else if (transform == 2) {
+      // next member of the family of Eq. 21, x(y) = int_0^y (u(1-u))^r du / B(r+1, r+1) with r = 2 (Eq. 21 is r = 1;
+      // SURVEY 8(f) f4, R:C20): x = 10y^3 - 15y^4 + 6y^5, weight dx/dy = 30 y^2 (1-y)^2
+      t[j] = v * v * v * (10.0 + v * (6.0 * v - 15.0));
+      w *= 30.0 * (v * (1.0 - v)) * (v * (1.0 - v));
     } else {
       t[j] = 1.0 - std::fabs(2.0 * v - 1.0);  // tent / baker (R:C20), weight 1
     }

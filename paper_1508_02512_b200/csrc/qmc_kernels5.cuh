@@ -386,6 +386,10 @@ __global__ void __launch_bounds__(QMC3_THREADS, (NDIM <= 4 ? 512 : 256) / QMC3_T
         if (p.transform == 0) {
           tj = y * y * (3.0 - 2.0 * y);
           w *= 6.0 * y * (1.0 - y);
+        } else if (p.transform == 2) {  // r = 2 member of the family of Eq. 21: x = 10y^3 - 15y^4 + 6y^5, dx/dy = 30 y^2 (1-y)^2
+          const double yq = y * (1.0 - y);
+          tj = y * y * y * (10.0 + y * (6.0 * y - 15.0));
+          w *= 30.0 * yq * yq;
         } else {
           tj = 1.0 - fabs(2.0 * y - 1.0);
         }

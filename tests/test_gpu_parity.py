@@ -265,3 +265,13 @@ def test_cbc_generating_vectors_through_the_kernels():
     ex = [0.666666666666667, -1.2639198230760183, -1.2238036181980894]
     assert np.all(np.abs(f.coeff.real - ex) <= 3.5 * f.err.real + 1e-13)
     parity(qi.nonplanar_vertex(), 16381, 3, z=q.qmc_cbc_vector(16381, 5))
+
+
+def test_second_order_periodising_transform_on_gpu():
+    """transform = 2 (the r = 2 member of Eq. 21's family, R:C20) through all three kernels: real path (box, double-box
+    sector subset), complex path (massive box), and the closed form of the box within 3.5 sigma."""
+    r, f, S, A, _ = parity(qi.massless_box(), 65521, 6, transform=2)
+    ex = [0.666666666666667, -1.2639198230760183, -1.2238036181980894]
+    assert np.all(np.abs(f.coeff.real - ex) <= 3.5 * f.err.real + 1e-13)
+    parity(qi.massive_box(), 16381, 3, transform=2)
+    parity(qi.double_box(), 10007, 2, transform=2, sectors=(100, 130))

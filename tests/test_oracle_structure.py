@@ -191,6 +191,34 @@ def test_tent_transform():
     assert np.mean(np.prod(t, axis=1)) == pytest.approx(0.25, rel=1e-5)
 
 
+@pytest.mark.parametrize("dim", [1, 2, 3])
+def test_second_order_periodising_transform(dim):
+    # transform = 2 (R:C20; the r = 2 member of Eq. 21's family): x = 10y^3 - 15y^4 + 6y^5, weight 30 y^2 (1-y)^2.
+    # Pins: x(0) = 0, x(1/2) = 1/2, x -> 1; dx/dy = weight (central differences on y itself); the same monomial
+    # integrals as Eq. 21; symmetry x(1-y) = 1 - x(y)
+    N = 32749
+    z = qi.good_vector(N, dim)
+    sh = qi.splitmix64_shifts(11, 1, dim)[0]
+    y, t, w, _ = lattice(N, z, 0, N, sh, transform=2)
+    assert np.mean(w * np.prod(t, axis=1)) == pytest.approx(2.0 ** -dim, rel=1e-8)
+    assert np.mean(w * np.prod(t * t, axis=1)) == pytest.approx(3.0 ** -dim, rel=1e-8)
+    assert np.mean(w) == pytest.approx(1.0, rel=1e-8)
+    if dim == 1:
+        order = np.argsort(y[:, 0])
+        ys, ts, ws = y[order, 0], t[order, 0], w[order]
+        assert np.all(np.diff(ts) > 0) and ts[0] > 0 and ts[-1] < 1
+        k = np.arange(1, N - 1)
+        slope = (ts[k + 1] - ts[k - 1]) / (ys[k + 1] - ys[k - 1])
+        assert np.allclose(slope, ws[k], rtol=0, atol=5e-8)
+        x = lambda v: 10 * v ** 3 - 15 * v ** 4 + 6 * v ** 5          # the polynomial in its expanded form
+        assert np.allclose(ts, x(ys), rtol=1e-13, atol=1e-300)
+        assert np.allclose(x(1.0 - ys), 1.0 - ts, rtol=0, atol=3e-14)   # expanded form: terms of size 10 cancel
+        one = lattice(3, [1], 0, 3, np.array([0.5]), transform=2)       # y = 1/2, 5/6, 1/6
+        assert one[1][0, 0] == 0.5 and one[2][0] == pytest.approx(30.0 / 16.0, rel=1e-15)
+    y0, t0, w0, ins = lattice(N, z, 0, 1, np.zeros(dim), transform=2)
+    assert w0[0] == 0.0 and ins[0] == 0
+
+
 def test_primes_and_vectors_are_valid():
     for nominal, p in qi.PRIMES.items():
         assert sympy.isprime(p) and sympy.prevprime(nominal + 1) == p
