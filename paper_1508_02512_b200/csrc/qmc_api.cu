@@ -330,6 +330,7 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
   }
   p.m = m;
   p.transform = t->transform;
+  qmc_transform_poly(t->transform, p.tc, p.wc);
   p.persec = persec ? 1 : 0;
   p.max_slices = max_slices;
   p.max_nslots = (uint32_t)max_nslots;
@@ -472,6 +473,7 @@ int launch_v5(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
   }
   p.m = m;
   p.transform = t->transform;
+  qmc_transform_poly(t->transform, p.tc, p.wc);
   p.persec = persec ? 1 : 0;
   p.max_slices = max_slices;
   p.max_nslots_r = (uint32_t)max_r;
@@ -851,6 +853,7 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
   p.aU0 = t->aU0; p.aU1 = t->aU1; p.aF0 = t->aF0; p.aF1 = t->aF1;
   p.lambda = t->lambda;
   p.transform = t->transform;
+  qmc_transform_poly(t->transform, p.tc, p.wc);
   p.sec_begin = sb; p.sec_end = se; p.sec_per_chunk = spc;
   p.persec = persec ? 1 : 0;
   p.tab_smem_bytes = (tab_bytes + 15) & ~15u;

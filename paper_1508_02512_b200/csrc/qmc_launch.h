@@ -7,6 +7,20 @@
 
 #define QMC_THREADS 256
 
+// The polynomial periodising transforms as data, so that S3 of the kernels has no branch between them (a branch between
+// Eq. 21 and its r = 2 sibling cost the complex kernel registers in its hot loop: cfg3 25 -> 32 ms):
+//   t = y^2 (tc[0] + y (tc[1] + y (tc[2] + y tc[3]))),   weight factor = q (wc[0] + q wc[1]),  q = y (1 - y)
+//   transform 0 (Eq. 21): tc = {3, -2, 0, 0}, wc = {6, 0};   transform 2 (R:C20): tc = {0, 10, -15, 6}, wc = {0, 30}.
+// The coefficients sit in the kernel parameters (constant bank operands of the FMAs: no registers).  transform 1 (tent)
+// keeps its branch.
+inline void qmc_transform_poly(int transform, double *tc, double *wc) {
+  if (transform == 2) {
+    tc[0] = 0.0, tc[1] = 10.0, tc[2] = -15.0, tc[3] = 6.0, wc[0] = 0.0, wc[1] = 30.0;
+  } else {
+    tc[0] = 3.0, tc[1] = -2.0, tc[2] = 0.0, tc[3] = 0.0, wc[0] = 6.0, wc[1] = 0.0;
+  }
+}
+
 struct QmcLaunch {
   const uint8_t *image;          // device: sector blocks
   const uint32_t *secoff;        // device: [n_sectors+1] byte offsets into image
@@ -19,6 +33,7 @@ struct QmcLaunch {
   int32_t m, kmax;
   int32_t aU0, aU1, aF0, aF1;
   double lambda;
+  double tc[4], wc[2];           // periodising transform (see qmc_transform_poly)
   int32_t transform;
   int32_t sec_begin, sec_end, sec_per_chunk;
   int32_t persec;                // 0: fused (all sectors of the chunk summed), 1: per-sector sums
@@ -61,6 +76,7 @@ struct Qmc4Launch {
   int32_t nsec, out_row, count_boundary, nslices;
   uint32_t nprog, prog_word, sec_word, first_prod_off;  // first_prod_off, local0_off: byte offsets in the slot column
   uint32_t local0_off, max_nslots, pad0, pad1;
+  double tc[4], wc[2];           // periodising transform (see qmc_transform_poly)
   uint16_t secw[QMC4_MAX_SEC];  // word offset of the sector blocks in tab, in evaluation order (sorted by nsing: sectors
                                 // that run the same code path are neighbours, which the instruction cache likes)
   uint16_t secrow[QMC4_MAX_SEC]; // per-sector mode: row of the partial buffer relative to out_row
@@ -99,6 +115,7 @@ struct Qmc5Launch {
   uint32_t nprog_c, prog_c_word, first_prod_c_off, local0_c_off;  // ... in the complex column
   uint32_t max_nslots_r, max_nslots_c, pad0, pad1;
   double lambda;
+  double tc[4], wc[2];           // periodising transform (see qmc_transform_poly)
   uint16_t secw[QMC4_MAX_SEC];
   uint16_t secrow[QMC4_MAX_SEC];
   uint4 tab[QMC4_TAB_WORDS];
