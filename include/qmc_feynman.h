@@ -71,6 +71,9 @@ typedef struct {
   int32_t transform; /* 0: x = 3y^2 - 2y^3, weight prod 6y(1-y) (Eq. 21).  1: tent/baker (R:C20).
                         2: x = 10y^3 - 15y^4 + 6y^5, weight prod 30y^2(1-y)^2 -- the next member of Eq. 21's family */
   int32_t max_depth; /* decomposition recursion cap; <= 0: 64 */
+  int32_t lattice;   /* generating vector of qmc_integrate when the caller passes none: 0 = Korobov-form P_2 search on the
+                        device (R:C13), 1 = component-by-component construction (R:C25; qmc_cbc_vector on the host,
+                        N an odd prime below 2^26, cached per N in the tables object) */
 } qmc_options;
 
 typedef struct qmc_tables qmc_tables; /* opaque sector tables (Eqs. 7-9) */

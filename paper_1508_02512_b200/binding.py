@@ -36,7 +36,7 @@ class qmc_kinematics(C.Structure):
 
 
 class qmc_options(C.Structure):
-    _fields_ = [("lambda_", C.c_double), ("transform", C.c_int32), ("max_depth", C.c_int32)]
+    _fields_ = [("lambda_", C.c_double), ("transform", C.c_int32), ("max_depth", C.c_int32), ("lattice", C.c_int32)]
 
 
 class qmc_result(C.Structure):
@@ -168,7 +168,7 @@ class Tables:
 
 
 def qmc_prepare(wl=None, *, n_vertices=None, edges=None, leg_vertex=None, gram=None, eps_order: int = 0,
-                lam: float = 0.0, transform: int = 0, max_depth: int = 0) -> Tables:
+                lam: float = 0.0, transform: int = 0, max_depth: int = 0, lattice: int = 0) -> Tables:
     """qmc_prepare(graph, kinematics, eps_order) -> sector tables.  `wl` is a qmc_inputs.Workload, or pass the
     graph explicitly (edges = [(u, v, m^2), ...])."""
     if wl is not None:
@@ -181,7 +181,7 @@ def qmc_prepare(wl=None, *, n_vertices=None, edges=None, leg_vertex=None, gram=N
     g = qmc_graph(n_vertices, len(edges), len(lv), _ptr(eu, C.c_int32), _ptr(ev, C.c_int32), _ptr(m2, C.c_double), None,
                   _ptr(lv, C.c_int32))
     k = qmc_kinematics(_ptr(gr, C.c_double))
-    o = qmc_options(lam, transform, max_depth)
+    o = qmc_options(lam, transform, max_depth, lattice)
     h = C.c_void_p()
     rc = lib().qmc_prepare(C.byref(g), C.byref(k), eps_order, C.byref(o), C.byref(h))
     if rc:

@@ -726,7 +726,8 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
     for (int j = 0; j < n; ++j) z[j] = r.z[j];
   } else {
     if (t->cached_N != N) {
-      int rc = korobov_search(N, n, st, ws, L.p2z, L.p2partial, t->cached_z);
+      int rc = t->lattice == 1 ? qmc_cbc_vector(N, n, t->cached_z, nullptr)
+                               : korobov_search(N, n, st, ws, L.p2z, L.p2partial, t->cached_z);
       if (rc != QMC_OK) return rc;
       t->cached_N = N;
     }

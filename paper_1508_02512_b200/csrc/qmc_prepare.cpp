@@ -194,7 +194,8 @@ int qmc_build_tables(const qmc_graph *g, const qmc_kinematics *kin, int eps_orde
   T->aF1 = -L;
   T->lambda = opt ? opt->lambda : 0.0;
   T->transform = opt ? opt->transform : 0;
-  if (T->lambda < 0.0 || (T->transform < 0 || T->transform > 2)) return QMC_EINVAL;
+  T->lattice = opt ? opt->lattice : 0;
+  if (T->lambda < 0.0 || (T->transform < 0 || T->transform > 2) || (T->lattice != 0 && T->lattice != 1)) return QMC_EINVAL;
   const int max_depth = (opt && opt->max_depth > 0) ? opt->max_depth : 64;
   const int n = T->n;
   T->kmax = eps_order;

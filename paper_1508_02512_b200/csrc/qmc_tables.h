@@ -118,6 +118,7 @@ struct qmc_tables {
   int aU0 = 0, aU1 = 0, aF0 = 0, aF1 = 0;
   double lambda = 0.0;
   int transform = 0;
+  int lattice = 0;  // qmc_options::lattice
   std::vector<QmcSector> sectors;
   // device image
   std::vector<uint8_t> image;     // concatenated sector blocks (16-byte aligned each)

@@ -265,6 +265,14 @@ def test_cbc_generating_vectors_through_the_kernels():
     ex = [0.666666666666667, -1.2639198230760183, -1.2238036181980894]
     assert np.all(np.abs(f.coeff.real - ex) <= 3.5 * f.err.real + 1e-13)
     parity(qi.nonplanar_vertex(), 16381, 3, z=q.qmc_cbc_vector(16381, 5))
+    # qmc_options.lattice = 1: qmc_integrate builds (and caches) the CBC vector itself
+    t = q.qmc_prepare(qi.massless_box(), lattice=1)
+    a = q.qmc_integrate(t, N, 6, seed=7)
+    b = q.qmc_integrate(q.qmc_prepare(qi.massless_box()), N, 6, z=z3, shifts=qi.splitmix64_shifts(7, 6, 3))
+    assert np.array_equal(a.shift_totals, b.shift_totals)
+    with pytest.raises(q.QmcError) as e:
+        q.qmc_integrate(t, 65535, 6, seed=7)              # CBC needs a prime N
+    assert e.value.status == -1
 
 
 def test_second_order_periodising_transform_on_gpu():
@@ -275,3 +283,17 @@ def test_second_order_periodising_transform_on_gpu():
     assert np.all(np.abs(f.coeff.real - ex) <= 3.5 * f.err.real + 1e-13)
     parity(qi.massive_box(), 16381, 3, transform=2)
     parity(qi.double_box(), 10007, 2, transform=2, sectors=(100, 130))
+
+
+def test_maximum_baseline_sizes_strided_indices():
+    """The largest lattices BASELINE.json names (cfg4: N = 99999989, cfg2 / cfg3: N = 9999991): i * z_j reaches 2^53, so
+    the remainder must be integer arithmetic on both sides.  Sampled outputs: a strided subset of the
+    lattice indices that the oracle can compute one by one, all sectors, the launch geometry of the full rule."""
+    N = qi.PRIMES[10 ** 8]
+    z = qi.korobov_vector(N, 6, 34567891)
+    step = 65537
+    parity(qi.double_box(), N, 2, z=z, index_range=(N - 1 - step * 1500, step, 1501))   # includes the last index N - 1
+    N = qi.PRIMES[10 ** 7]
+    z = qi.korobov_vector(N, 3, 2345677)
+    parity(qi.massless_box(), N, 3, z=z, index_range=(5, 4099, (N - 5 + 4098) // 4099))
+    parity(qi.massive_box(), N, 2, z=z, index_range=(11, 8191, (N - 11 + 8190) // 8191))

@@ -105,6 +105,10 @@ def test_prepare_error_codes():
     with pytest.raises(q.QmcError) as e:                                  # tree graph: L < 1
         q.qmc_prepare(n_vertices=3, edges=[(0, 1, 0.0), (1, 2, 0.0)], leg_vertex=[0, 2], gram=np.zeros((2, 2)))
     assert e.value.status == -1
+    for bad in (dict(transform=3), dict(transform=-1), dict(lattice=2), dict(lam=-0.1)):
+        with pytest.raises(q.QmcError) as e:                              # options out of range
+            q.qmc_prepare(qi.massless_box(), **bad)
+        assert e.value.status == -1
     with pytest.raises(q.QmcError) as e:
         q.qmc_prepare(qi.double_box(), max_depth=2)                       # depth cap
     assert e.value.status == -2
