@@ -151,7 +151,7 @@ int qmc_build_image3(qmc_tables *t) {
     sector_polys(t->sectors[si], n, pos_of, polys[si]);
     size_t nrec = 1 + n;
     for (const Poly3 &P : polys[si]) nrec += P.size();
-    bytes[si] = sizeof(Qmc3SectorHdr) + npoly * (1 << t->sectors[si].nsing) + 64 + 16.0 * nrec;
+    bytes[si] = sizeof(Qmc3SectorHdr) + npoly * (1 << t->sectors[si].nsing) + 64 + 16.0 * (nrec + nderiv / 2);
     t->sec_cost[si] = (double)(1 << t->sectors[si].nsing) * (nrec + 400.0);
   }
   std::vector<std::pair<int, int>> todo;
@@ -322,7 +322,7 @@ int qmc_build_image3(qmc_tables *t) {
           std::vector<uint8_t> cz(npoly, 0);
           std::vector<Qmc2Rec> zr, zc;
           size_t ir = 1 + h.nL0, ic = 0;
-          for (int p = 0; p < npoly; ++p)
+          for (int p = 0; p < npoly; ++p) {
             for (const Mono3 &m : polys[si][p]) {
               const bool keep = (m.group & Z) == 0;
               if (p < nderiv) {
@@ -333,6 +333,10 @@ int qmc_build_image3(qmc_tables *t) {
                 ++ic;
               }
             }
+            // the kernel walks the real stream two records at a time: every derivative polynomial gets an even count
+            // (one zero-coefficient record where needed)
+            if (n >= QMC5_PAIR_MIN_DIM && p < nderiv && (cz[p] & 1)) { zr.push_back(empty_r); ++cz[p]; }
+          }
           for (int p = 0; p < npoly; p += 4) {
             uint32_t w = 0;
             for (int q = 0; q < 4 && p + q < npoly; ++q) w |= (uint32_t)cz[p + q] << (8 * q);
@@ -340,8 +344,7 @@ int qmc_build_image3(qmc_tables *t) {
           }
           pad4(v);
           for (const Qmc2Rec &r : zr) put_rec(v, r);
-          put_rec(v, empty_r);
-          put_rec(v, empty_r);  // the kernel requests offsets two records ahead
+          for (int q = 0; q < (n >= QMC5_PAIR_MIN_DIM ? 4 : 2); ++q) put_rec(v, empty_r);  // offsets run two (pairs of) records ahead
           for (const Qmc2Rec &r : zc) put_rec(v, r);
           put_rec(v, empty_c);
           put_rec(v, empty_c);

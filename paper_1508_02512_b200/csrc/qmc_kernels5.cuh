@@ -79,28 +79,60 @@ __device__ __forceinline__ void corner5(const Qmc5Launch &p, const uint32_t cw, 
   // ---- S4: gradient and Hessian of F^ at tau: one software-pipelined stream of real records --------------------------
   double dv[NDERIV];
   {
-    // offsets two records ahead (uniform registers), operands one record ahead: neither the uniform load nor the LDS
-    // sits on the critical path of an iteration (the block ends with TWO sentinel records)
-    uint2 ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);
-    double ra = slot_at(slr, ro.x), rb = slot_at(slr, ro.y);
-    ro = *reinterpret_cast<const uint2 *>(tb + rwb + 24);
-#pragma unroll
-    for (int q = 0; q < NDERIV; ++q) {
-      const uint32_t n = (cnt[q >> 2] >> (8 * (q & 3))) & 255u;
-      double acc = 0.0;
-#pragma unroll 1
-      for (uint32_t i = 0; i < n; ++i) {
-        const uint2 rc = *reinterpret_cast<const uint2 *>(tb + rwb);
-        const double v = ra * rb;
-        rwb += 16u;
-        ra = slot_at(slr, ro.x);
-        rb = slot_at(slr, ro.y);
-        ro = *reinterpret_cast<const uint2 *>(tb + rwb + 24);
-        acc = fma(u2d(rc.x, rc.y), v, acc);
+    if (NDIM >= QMC5_PAIR_MIN_DIM) {
+      // Two records per iteration (the table builder pads every derivative polynomial to an even count): operands one
+      // PAIR ahead, offsets two pairs ahead (the stream ends with FOUR sentinel records).  With two warps per scheduler
+      // one record of lead did not cover the LDS latency: the DMUL of the single-record loop took half of the loop's
+      // samples waiting for its operands (profiles/r01p_final.md).
+      uint2 roA = *reinterpret_cast<const uint2 *>(tb + rwb + 8), roB = *reinterpret_cast<const uint2 *>(tb + rwb + 24);
+      double a0 = slot_at(slr, roA.x), b0 = slot_at(slr, roA.y), a1 = slot_at(slr, roB.x), b1 = slot_at(slr, roB.y);
+      roA = *reinterpret_cast<const uint2 *>(tb + rwb + 40);
+      roB = *reinterpret_cast<const uint2 *>(tb + rwb + 56);
+  #pragma unroll
+      for (int q = 0; q < NDERIV; ++q) {
+        const uint32_t n = (cnt[q >> 2] >> (8 * (q & 3))) & 255u;
+        double acc0 = 0.0, acc1 = 0.0;
+  #pragma unroll 1
+        for (uint32_t i = 0; i < n; i += 2) {
+          const uint2 rc0 = *reinterpret_cast<const uint2 *>(tb + rwb), rc1 = *reinterpret_cast<const uint2 *>(tb + rwb + 16);
+          const double v0 = a0 * b0, v1 = a1 * b1;
+          rwb += 32u;
+          a0 = slot_at(slr, roA.x);
+          b0 = slot_at(slr, roA.y);
+          a1 = slot_at(slr, roB.x);
+          b1 = slot_at(slr, roB.y);
+          roA = *reinterpret_cast<const uint2 *>(tb + rwb + 40);
+          roB = *reinterpret_cast<const uint2 *>(tb + rwb + 56);
+          acc0 = fma(u2d(rc0.x, rc0.y), v0, acc0);
+          acc1 = fma(u2d(rc1.x, rc1.y), v1, acc1);
+        }
+        dv[q] = acc0 + acc1;
       }
-      dv[q] = acc;
+      rwb += 64u;  // the four real sentinels
+    } else {
+      // offsets two records ahead (uniform registers), operands one record ahead: neither the uniform load nor the LDS
+      // sits on the critical path of an iteration (the block ends with TWO sentinel records)
+      uint2 ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);
+      double ra = slot_at(slr, ro.x), rb = slot_at(slr, ro.y);
+      ro = *reinterpret_cast<const uint2 *>(tb + rwb + 24);
+  #pragma unroll
+      for (int q = 0; q < NDERIV; ++q) {
+        const uint32_t n = (cnt[q >> 2] >> (8 * (q & 3))) & 255u;
+        double acc = 0.0;
+  #pragma unroll 1
+        for (uint32_t i = 0; i < n; ++i) {
+          const uint2 rc = *reinterpret_cast<const uint2 *>(tb + rwb);
+          const double v = ra * rb;
+          rwb += 16u;
+          ra = slot_at(slr, ro.x);
+          rb = slot_at(slr, ro.y);
+          ro = *reinterpret_cast<const uint2 *>(tb + rwb + 24);
+          acc = fma(u2d(rc.x, rc.y), v, acc);
+        }
+        dv[q] = acc;
+      }
+      rwb += 32u;  // the two real sentinels
     }
-    rwb += 32u;  // the two real sentinels
   }
   // rho_i, z_i, J = 1 + i B
   cd rho[NDIM], J[NDIM][NDIM];

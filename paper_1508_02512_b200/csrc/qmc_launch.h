@@ -100,7 +100,8 @@ bool qmc4_kernel_available(int ndim, int loops, int kmax);
 //   w8.. = local real program, local complex program (each padded to a word), then records [G0][L0 x nL0]
 //   corner block Z: u8 counts[npoly] (npoly = n + n(n+1)/2 + 2: F_i, F_ik (i <= k), U, F; padded to a word) of the
 //     records that survive at the corner (monomials free of the variables of Z), then the real records of the
-//     derivative polynomials, two real sentinels, the complex records of U^ and F^, two complex sentinels.
+//     derivative polynomials (each padded to an even count with a zero-coefficient record), four real sentinels, the
+//     complex records of U^ and F^, two complex sentinels.
 //   A record is duplicated into every corner block that needs it: each corner is one flat stream without skips.
 struct Qmc5Launch {
   const double *logtab;          // device: 64 x {1/c, -ln(1/c)}

@@ -78,6 +78,11 @@ struct Qmc2Chunk {      // host description of one chunk
 // refilled at every corner, that serves U^(z) and F^(z).  Records are sorted per polynomial by group; a corner Z keeps
 // the groups disjoint from Z.
 #define QMC3_THREADS 128
+// complex path, n >= QMC5_PAIR_MIN_DIM: the derivative-polynomial record stream is walked two records at a time (every
+// polynomial padded to an even count, four sentinels); below, one at a time (two sentinels).  Measured on B200: the pair
+// walk gains on the long polynomials of n = 5 (cfg5 229.4 -> 223.4 ms) and loses to its padding on the short ones of
+// n = 3 (cfg3 25.3 -> 26.4 ms).
+#define QMC5_PAIR_MIN_DIM 5
 #define QMC3_MAXSLOTS_R 56
 #define QMC3_MAXSLOTS_C 40
 #define QMC3_MAXLOCAL 8
