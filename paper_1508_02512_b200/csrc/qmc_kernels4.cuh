@@ -337,13 +337,14 @@ __global__ void __launch_bounds__(T, 512 / T) qmc4_eval_kernel(const __grid_cons
         if (i + 1 < p.nprog)
           *reinterpret_cast<double *>(sl + p.first_prod_off + (i + 1) * (T * 8)) = slot_at(sl, pw.z) * slot_at(sl, pw.w);
       }
-      // S4-S6: all sectors of the run at this point.  The barrier re-aligns the block's warps once per point: the kernel
-      // is close to its instruction-fetch ceiling (profiles/r01p_final.md: GPC instruction-cache requests at 77 % of
-      // their sustained rate, SM instruction-cache hit rate 87 %), and warps that walk the same sector at about the
-      // same time share the fetched lines.  Measured on cfg4: 248.0 ms without, 241.5 ms with one barrier per point,
-      // 244.8 / 249.0 / 255.1 / 268.3 ms with one per 16 / 8 / 4 / 1 sectors (finer alignment costs the overlap of
-      // table-walk and arithmetic phases between warps).
-      if (T >= 256) __syncthreads();
+      // S4-S6: all sectors of the run at this point.  A barrier every fourth point re-aligns the block's warps: the
+      // kernel was close to its instruction-fetch ceiling (profiles/r01p_final.md: GPC instruction-cache requests at
+      // 77 % of their sustained rate, SM instruction-cache hit rate 87 %), and warps that walk the same sector at about
+      // the same time share the fetched lines -- while between two barriers they drift apart again, which keeps the
+      // table-walk phase of one warp over the arithmetic phase of another.  Measured on cfg4 (ms per step): no barrier
+      // 248.0; one per 64 / 16 / 8 / 4 / 2 / 1 points 246.6 / 239.3 / 234.5 / 232.0 / 234.5 / 242.0; one per 16 / 8 / 4 / 1
+      // sectors 244.8 / 249.0 / 255.1 / 268.3.
+      if (T >= 256 && (((cb - c0) / stride) & 3u) == 0u) __syncthreads();
       for (int si = 0; si < p.nsec; ++si) {
         // (offsets come from an array indexed by the induction variable: a loop-carried offset read from the table
         //  itself makes ptxas give up the uniform datapath for the whole table walk)
