@@ -344,6 +344,7 @@ __global__ void __launch_bounds__(T, 512 / T) qmc4_eval_kernel(const __grid_cons
       // table-walk phase of one warp over the arithmetic phase of another.  Measured on cfg4 (ms per step): no barrier
       // 248.0; one per 64 / 16 / 8 / 4 / 2 / 1 points 246.6 / 239.3 / 234.5 / 232.0 / 234.5 / 242.0; one per 16 / 8 / 4 / 1
       // sectors 244.8 / 249.0 / 255.1 / 268.3.
+      // (barriers among groups of 8 or 4 warps instead of the whole block: 232.7-237.0 ms, no gain)
       if (T >= 256 && (((cb - c0) / stride) & 3u) == 0u) __syncthreads();
       for (int si = 0; si < p.nsec; ++si) {
         // (offsets come from an array indexed by the induction variable: a loop-carried offset read from the table
