@@ -74,6 +74,12 @@ typedef struct {
   int32_t lattice;   /* generating vector of qmc_integrate when the caller passes none: 0 = Korobov-form P_2 search on the
                         device (R:C13), 1 = component-by-component construction (R:C25; qmc_cbc_vector on the host,
                         N an odd prime below 2^26, cached per N in the tables object) */
+  /* Layout of the device tables; 0 = the defaults measured on B200.  They change how the
+   * sectors are grouped into chunks and how many per-point product slots a chunk may use, never the result. */
+  int32_t slot_budget;       /* real path: chunk-wide slots of the slot program (default 36) */
+  int32_t chunk_bytes;       /* target bytes of sector tables per chunk (both paths) */
+  int32_t threads;           /* real path: threads per block, 128 or 512 (default: chosen from the tables) */
+  int32_t slot_budget_cplx_real, slot_budget_cplx; /* complex path: real / complex slots per chunk */
 } qmc_options;
 
 typedef struct qmc_tables qmc_tables; /* opaque sector tables (Eqs. 7-9) */
@@ -126,6 +132,11 @@ typedef struct {
   int32_t mode;             /* 0 auto (per-sector iff a per-sector output is requested), 1 fused, 2 per-sector */
   int32_t tables_resident;  /* 1: reuse what an earlier call left in this workspace (the logarithm table);
                                2: reuse the shift vectors of that call as well (nothing is copied from the host) */
+  int32_t kernel;           /* 0: the table-driven kernels (real path: qmc4_eval_kernel, complex path: qmc5_eval_kernel) where
+                               the tables allow them, else the generic kernel; 1: the generic kernel (qmc_eval_kernel) */
+  int32_t waves;            /* launch geometry: blocks per resident block slot over all launches of a step (0 = 16) */
+  int32_t streams;          /* internal side streams the launches of a step are spread over, 0..8 (0 = default 4;
+                               -1 = none: all launches in order on cuda_stream) */
 } qmc_run;
 
 size_t qmc_workspace_bytes(const qmc_tables *t, uint64_t N, int32_t m);

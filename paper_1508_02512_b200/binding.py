@@ -36,7 +36,9 @@ class qmc_kinematics(C.Structure):
 
 
 class qmc_options(C.Structure):
-    _fields_ = [("lambda_", C.c_double), ("transform", C.c_int32), ("max_depth", C.c_int32), ("lattice", C.c_int32)]
+    _fields_ = [("lambda_", C.c_double), ("transform", C.c_int32), ("max_depth", C.c_int32), ("lattice", C.c_int32),
+                ("slot_budget", C.c_int32), ("chunk_bytes", C.c_int32), ("threads", C.c_int32),
+                ("slot_budget_cplx_real", C.c_int32), ("slot_budget_cplx", C.c_int32)]
 
 
 class qmc_result(C.Structure):
@@ -53,7 +55,7 @@ class qmc_run(C.Structure):
     _fields_ = [("z", C.POINTER(C.c_uint64)), ("shifts", C.POINTER(C.c_double)),
                 ("index_begin", C.c_uint64), ("index_step", C.c_uint64), ("index_count", C.c_uint64),
                 ("sector_begin", C.c_int32), ("sector_end", C.c_int32), ("mode", C.c_int32),
-                ("tables_resident", C.c_int32)]
+                ("tables_resident", C.c_int32), ("kernel", C.c_int32), ("waves", C.c_int32), ("streams", C.c_int32)]
 
 
 _lib = None
@@ -168,9 +170,11 @@ class Tables:
 
 
 def qmc_prepare(wl=None, *, n_vertices=None, edges=None, leg_vertex=None, gram=None, eps_order: int = 0,
-                lam: float = 0.0, transform: int = 0, max_depth: int = 0, lattice: int = 0) -> Tables:
+                lam: float = 0.0, transform: int = 0, max_depth: int = 0, lattice: int = 0, slot_budget: int = 0,
+                chunk_bytes: int = 0, threads: int = 0, slot_budget_cplx_real: int = 0, slot_budget_cplx: int = 0) -> Tables:
     """qmc_prepare(graph, kinematics, eps_order) -> sector tables.  `wl` is a qmc_inputs.Workload, or pass the
-    graph explicitly (edges = [(u, v, m^2), ...])."""
+    graph explicitly (edges = [(u, v, m^2), ...]).  slot_budget .. slot_budget_cplx are the table-layout fields of
+    qmc_options (0 = the library's defaults)."""
     if wl is not None:
         n_vertices, edges, leg_vertex, gram = wl.n_vertices, wl.edges, wl.leg_vertex, wl.gram
     eu = np.ascontiguousarray([e[0] for e in edges], dtype=np.int32)
@@ -181,7 +185,8 @@ def qmc_prepare(wl=None, *, n_vertices=None, edges=None, leg_vertex=None, gram=N
     g = qmc_graph(n_vertices, len(edges), len(lv), _ptr(eu, C.c_int32), _ptr(ev, C.c_int32), _ptr(m2, C.c_double), None,
                   _ptr(lv, C.c_int32))
     k = qmc_kinematics(_ptr(gr, C.c_double))
-    o = qmc_options(lam, transform, max_depth, lattice)
+    o = qmc_options(lam, transform, max_depth, lattice, slot_budget, chunk_bytes, threads, slot_budget_cplx_real,
+                    slot_budget_cplx)
     h = C.c_void_p()
     rc = lib().qmc_prepare(C.byref(g), C.byref(k), eps_order, C.byref(o), C.byref(h))
     if rc:
@@ -216,8 +221,10 @@ def _workspace(t: Tables, N: int, m: int, device):
     return ws
 
 
-def _make_run(t: Tables, m: int, z, shifts, index_range, sectors, mode: int, resident: int):
+def _make_run(t: Tables, m: int, z, shifts, index_range, sectors, mode: int, resident: int, kernel: int = 0,
+              waves: int = 0, streams: int = 0):
     run = qmc_run()
+    run.kernel, run.waves, run.streams = kernel, waves, streams
     keep = []
     if z is not None:
         za = np.ascontiguousarray(z, dtype=np.uint64); keep.append(za)
@@ -262,7 +269,8 @@ def _wrap_result(res, arrays) -> Result:
 
 def qmc_integrate(t: Tables, N: int, m: int, seed: int = 0, *, z: Optional[Sequence[int]] = None,
                   shifts: Optional[np.ndarray] = None, index_range=None, sectors=None, per_sector: bool = False,
-                  mode: int = 0, resident: int = 0, device="cuda:0", stream=None) -> Result:
+                  mode: int = 0, resident: int = 0, kernel: int = 0, waves: int = 0, streams: int = 0,
+                  device="cuda:0", stream=None) -> Result:
     """qmc_integrate(tables, N, m, seed) -> Laurent coefficients and errors (qmc_integrate_ex when any of the
     explicit controls is given).  Workspace and stream come from PyTorch."""
     import torch
@@ -274,7 +282,7 @@ def qmc_integrate(t: Tables, N: int, m: int, seed: int = 0, *, z: Optional[Seque
         st = stream if stream is not None else torch.cuda.current_stream(dev)
         s0, s1 = sectors if sectors is not None else (0, t.n_sectors)
         res, arrays = _make_result(t, m, s1 - s0, per_sector)
-        run, keep = _make_run(t, m, z, shifts, index_range, sectors, mode, resident)
+        run, keep = _make_run(t, m, z, shifts, index_range, sectors, mode, resident, kernel, waves, streams)
         rc = lib().qmc_integrate_ex(t._h, N, m, seed, C.byref(run), C.c_void_p(st.cuda_stream),
                                     C.c_void_p(ws.data_ptr()), ws.numel(), C.byref(res))
         if rc:
@@ -283,7 +291,8 @@ def qmc_integrate(t: Tables, N: int, m: int, seed: int = 0, *, z: Optional[Seque
 
 
 def qmc_integrate_async(t: Tables, N: int, m: int, seed: int = 0, *, z=None, shifts=None, index_range=None,
-                        sectors=None, mode: int = 1, resident: int = 0, device="cuda:0", stream=None) -> None:
+                        sectors=None, mode: int = 1, resident: int = 0, kernel: int = 0, waves: int = 0, streams: int = 0,
+                        device="cuda:0", stream=None) -> None:
     """Enqueue S1-S8 on the stream and return without synchronising; results stay in the workspace of `t`
     (qmc_result_fetch brings them to the host).  resident=2: nothing is copied from the host."""
     import torch
@@ -293,7 +302,7 @@ def qmc_integrate_async(t: Tables, N: int, m: int, seed: int = 0, *, z=None, shi
     with torch.cuda.device(dev):
         ws = _workspace(t, N, m, dev)
         st = stream if stream is not None else torch.cuda.current_stream(dev)
-        run, keep = _make_run(t, m, z, shifts, index_range, sectors, mode, resident)
+        run, keep = _make_run(t, m, z, shifts, index_range, sectors, mode, resident, kernel, waves, streams)
         rc = lib().qmc_integrate_async(t._h, N, m, seed, C.byref(run), C.c_void_p(st.cuda_stream),
                                        C.c_void_p(ws.data_ptr()), ws.numel())
         if rc:

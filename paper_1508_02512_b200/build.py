@@ -20,7 +20,7 @@ NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
-SOURCES = ["qmc_prepare.cpp", "qmc_flops.cpp", "qmc_image2.cpp", "qmc_image3.cpp", "qmc_cbc.cpp", "qmc_api.cu", "qmc_dispatch.cu"] + [f"qmc_inst_d{d}.cu" for d in range(1, 7)] + [f"qmc4_inst_d{d}.cu" for d in range(1, 7)] + [f"qmc5_inst_d{d}.cu" for d in range(1, 7)]
+SOURCES = ["qmc_prepare.cpp", "qmc_flops.cpp", "qmc_image4.cpp", "qmc_image3.cpp", "qmc_cbc.cpp", "qmc_api.cu", "qmc_dispatch.cu"] + [f"qmc_inst_d{d}.cu" for d in range(1, 7)] + [f"qmc4_inst_d{d}.cu" for d in range(1, 7)] + [f"qmc5_inst_d{d}.cu" for d in range(1, 7)]
 HEADERS = ["qmc_tables.h", "qmc_launch.h", "qmc_kernels.cuh", "qmc_inst.cuh", "qmc_fold.cuh", "qmc_kernels4.cuh", "qmc_inst4.cuh", "qmc_kernels5.cuh", "qmc_inst5.cuh", "qmc_bpe.h", os.path.join("..", "..", "include", "qmc_feynman.h")]
 
 

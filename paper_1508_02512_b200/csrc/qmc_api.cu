@@ -249,25 +249,27 @@ void mean_err(const double *v, size_t stride, int m, double *mean, double *err) 
 // and joined back into the caller's stream, so that the tail of one launch overlaps the next ones.
 int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t st, uint64_t N, int m, int sb, int se,
               bool persec, uint64_t ibeg, uint64_t istep, uint64_t icount, const uint64_t *z, int sms, int smem_optin,
-              int *gx_out, int *rows_out, int *launches_out, size_t *h2d, cudaError_t *ce_out) {
+              int waves_opt, int streams_opt, int *gx_out, int *rows_out, int *launches_out, size_t *h2d, cudaError_t *ce_out) {
   const int n = t->n, nacc = QMC_MAXSING + t->kmax + 1, T = t->threads_real;
-  int max_nslots = 0;
-  for (const Qmc2Chunk &c : t->chunks)
-    if (c.sec_end > sb && c.sec_begin < se) max_nslots = std::max(max_nslots, c.nslots + c.max_local);
   const size_t budget = (size_t)smem_optin - 1024;
-  const size_t fixed = (size_t)QMC4_LOG_ENTRIES * QMC4_LOG_COPIES * 16 + (((size_t)m * n * 8 + 15) & ~(size_t)15) + (T / 32) * 8 +
-                       (size_t)max_nslots * T * 8;
+  // shared memory of a launch: logarithm table, shift vectors, reduction scratch, the chunk's slot columns (+ per-sector
+  // accumulators in per-sector mode)
+  auto fixed_of = [&](const Qmc2Chunk &c) {
+    return (size_t)QMC4_LOG_ENTRIES * QMC4_LOG_COPIES * 16 + (((size_t)m * n * 8 + 15) & ~(size_t)15) + (T / 32) * 8 +
+           (size_t)(c.nslots + c.max_local) * T * 8;
+  };
   const size_t accbytes = persec ? (size_t)nacc * T * 8 : 0;
-  if (fixed + accbytes > budget) return QMC_ENOMEM;
-  struct Run { int chunk, a, b; double cost; };
+  struct Run { int chunk, a, b; double cost; size_t smem; };
   std::vector<Run> runs;
   double total_cost = 0.0;
-  int max_nsec = 0;
+  size_t smem = 0;
   for (size_t ci = 0; ci < t->chunks.size(); ++ci) {
     const Qmc2Chunk &c = t->chunks[ci];
     int a = std::max(sb, c.sec_begin);
     const int e = std::min(se, c.sec_end);
     const size_t prog_words = t->prog4[ci].size() / 4;
+    const size_t fixed = fixed_of(c);
+    if (a < e && fixed + accbytes > budget) return QMC_ENOMEM;
     while (a < e) {
       int b = a;
       while (b < e) {
@@ -276,21 +278,19 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
         ++b;
       }
       if (b == a) return QMC_ENOMEM;
-      Run r = {(int)ci, a, b, 0.0};
+      Run r = {(int)ci, a, b, 0.0, fixed + accbytes * (b - a)};
       for (int s = a; s < b; ++s) r.cost += t->sec_cost[s];
       total_cost += r.cost;
-      max_nsec = std::max(max_nsec, b - a);
+      smem = std::max(smem, r.smem);
       runs.push_back(r);
       a = b;
     }
   }
   const int nitems = (int)runs.size();
-  const size_t smem = fixed + accbytes * max_nsec;
   int bps = 0;
   CUDA_OK(qmc4_kernel_prepare(n, t->L, t->kmax, T, smem, &bps));
   if (bps < 1) return QMC_ECUDA;
-  int waves = 16;
-  if (const char *e = std::getenv("QMC2_WAVES")) waves = std::max(1, std::atoi(e));
+  const int waves = waves_opt > 0 ? waves_opt : 16;
   const long long max_slices_pts = std::max<long long>(1, (long long)((icount + T - 1) / T));
   const double nblocks_target = (double)waves * sms * bps / (double)m;  // a block serves ONE shift vector
   std::vector<int> nsl(nitems);
@@ -304,8 +304,7 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
   const int rows_partial = persec ? (se - sb) : nitems;
   CUDA_OK(cudaMemsetAsync(ws + L.partial, 0, (size_t)rows_partial * m * max_slices * nacc * 8, st));
   // side streams
-  int nstreams = 4;
-  if (const char *e = std::getenv("QMC4_STREAMS")) nstreams = std::max(0, std::min(8, std::atoi(e)));
+  int nstreams = streams_opt < 0 ? 0 : (streams_opt == 0 ? 4 : std::min(8, streams_opt));
   nstreams = std::min(nstreams, nitems);
   if (nstreams < 2) nstreams = 0;
   for (int q = 0; q < nstreams; ++q)
@@ -333,7 +332,9 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
   qmc_transform_poly(t->transform, p.tc, p.wc);
   p.persec = persec ? 1 : 0;
   p.max_slices = max_slices;
-  p.max_nslots = (uint32_t)max_nslots;
+  p.dN = (double)N;
+  p.invN = 1.0 / (double)N;
+  p.sync_every = 4;  // measured on B200 (kernels): a block barrier every fourth point
   cudaEventRecord(static_cast<cudaEvent_t>(t->ev0), st);
   if (nstreams) {
     cudaEventRecord(static_cast<cudaEvent_t>(t->side_events[nstreams]), st);
@@ -349,10 +350,13 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
     p.out_row = persec ? r.a - sb : i;
     p.count_boundary = i == 0 ? 1 : 0;
     p.nslices = nsl[i];
-    p.nprog = (uint32_t)(c.nslots - (3 * n + 1));
+    p.max_nslots = (uint32_t)(c.nslots + c.max_local);
+    p.nconst = (uint32_t)c.nconst;
+    for (int q = 0; q < c.nconst; ++q) p.cval[q] = t->const4[r.chunk][q];
+    p.nprog = (uint32_t)(c.nslots - (3 * n + 2 + c.nconst));
     p.prog_word = 0;
     p.sec_word = (uint32_t)(pg.size() / 4);
-    p.first_prod_off = (uint32_t)(3 * n + 1) * T * 8u;
+    p.first_prod_off = (uint32_t)(3 * n + 2 + c.nconst) * T * 8u;
     p.local0_off = (uint32_t)c.nslots * T * 8u;
     uint32_t *tw = reinterpret_cast<uint32_t *>(p.tab);
     std::memcpy(tw, pg.data(), pg.size() * 4);
@@ -369,7 +373,7 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
           }
     }
     cudaStream_t ls = nstreams ? static_cast<cudaStream_t>(t->side_streams[i % nstreams]) : st;
-    ce = qmc4_kernel_launch(n, t->L, t->kmax, T, dim3((unsigned)nsl[i], (unsigned)m), smem, ls, p);
+    ce = qmc4_kernel_launch(n, t->L, t->kmax, T, dim3((unsigned)nsl[i], (unsigned)m), r.smem, ls, p);
     *h2d += offsetof(Qmc4Launch, tab) + pg.size() * 4 + (w1 - w0) * 16;  // the tables travel with the launch
   }
   if (nstreams)
@@ -388,7 +392,7 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
 // ---- version-5 launch (complex path): as version 4, two slot tables per thread ------------------------------------------
 int launch_v5(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t st, uint64_t N, int m, int sb, int se,
               bool persec, uint64_t ibeg, uint64_t istep, uint64_t icount, const uint64_t *z, int sms, int smem_optin,
-              int *gx_out, int *rows_out, int *launches_out, size_t *h2d, cudaError_t *ce_out) {
+              int waves_opt, int streams_opt, int *gx_out, int *rows_out, int *launches_out, size_t *h2d, cudaError_t *ce_out) {
   const int n = t->n, nacc = 2 * (QMC_MAXSING + t->kmax + 1), T = QMC3_THREADS;  // accumulators: (Re, Im) per order
   int max_r = 0, max_c = 0;
   for (size_t ci = 0; ci < t->chunks3.size(); ++ci) {
@@ -433,8 +437,7 @@ int launch_v5(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
   int bps = 0;
   CUDA_OK(qmc5_kernel_prepare(n, t->L, t->kmax, smem, &bps));
   if (bps < 1) return QMC_ECUDA;
-  int waves = 16;
-  if (const char *e = std::getenv("QMC2_WAVES")) waves = std::max(1, std::atoi(e));
+  const int waves = waves_opt > 0 ? waves_opt : 16;
   const long long max_slices_pts = std::max<long long>(1, (long long)((icount + T - 1) / T));
   const double nblocks_target = (double)waves * sms * bps / (double)m;
   std::vector<int> nsl(nitems);
@@ -447,8 +450,7 @@ int launch_v5(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
   }
   const int rows_partial = persec ? (se - sb) : nitems;
   CUDA_OK(cudaMemsetAsync(ws + L.partial, 0, (size_t)rows_partial * m * max_slices * nacc * 8, st));
-  int nstreams = 4;
-  if (const char *e = std::getenv("QMC4_STREAMS")) nstreams = std::max(0, std::min(8, std::atoi(e)));
+  int nstreams = streams_opt < 0 ? 0 : (streams_opt == 0 ? 4 : std::min(8, streams_opt));
   nstreams = std::min(nstreams, nitems);
   if (nstreams < 2) nstreams = 0;
   for (int q = 0; q < nstreams; ++q)
@@ -761,9 +763,11 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
   int gx = 1, nchunks = 1;
   cudaError_t ce = cudaSuccess;
   double *partial = reinterpret_cast<double *>(ws + L.partial);
-  const bool use_v4 = !cplx && !t->tab4.empty() && qmc4_kernel_available(n, t->L, t->kmax) && !std::getenv("QMC_FORCE_V1");
+  if (r.kernel != 0 && r.kernel != 1) return QMC_EINVAL;
+  if (n > 6) return QMC_EUNSUPPORTED;  // every kernel family is instantiated for 1..6 integration variables
+  const bool use_v4 = !cplx && !t->tab4.empty() && qmc4_kernel_available(n, t->L, t->kmax) && r.kernel == 0;
   const bool use_v5 = cplx && !t->tab5.empty() && -t->kmin <= QMC3_MAXSING && qmc5_kernel_available(n, t->L, t->kmax) &&
-                      !std::getenv("QMC_FORCE_V1");
+                      r.kernel == 0;
   int eval_launches = 1;
   // ---- uploads (skipped when resident).  Versions 4 and 5 carry their tables in the kernel parameters: only the
   // logarithm table lives in the workspace; the version-1 image is uploaded for the generic fallback kernel only.
@@ -789,10 +793,10 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
   CUDA_OK(cudaMemsetAsync(ws + L.counters, 0, 32, st));
 
   if (use_v5) {
-    int rc = launch_v5(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, &gx, &nchunks, &eval_launches, &h2d, &ce);
+    int rc = launch_v5(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, r.waves, r.streams, &gx, &nchunks, &eval_launches, &h2d, &ce);
     if (rc != QMC_OK) return rc;
   } else if (use_v4) {
-    int rc = launch_v4(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, &gx, &nchunks, &eval_launches, &h2d, &ce);
+    int rc = launch_v4(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, r.waves, r.streams, &gx, &nchunks, &eval_launches, &h2d, &ce);
     if (rc != QMC_OK) return rc;
   } else {
   const size_t fixed_smem = 16 + (((size_t)m * n * 8 + 15) & ~(size_t)15) + (QMC_THREADS / 32) * 8 + (size_t)3 * n * QMC_THREADS * 8;
@@ -1025,23 +1029,15 @@ int qmc_tables_describe(const qmc_tables *t, char *buf, size_t len) {
   if (!t || !buf || len < 1) return QMC_EINVAL;
   std::string o;
   char line[256];
-  std::snprintf(line, sizeof line, "sectors %d dim %d loops %d orders %d..%d lambda %g image1 %zu B image2 %zu B chunks %zu\n",
-                (int)t->sectors.size(), t->n, t->L, t->kmin, t->kmax, t->lambda, t->image.size(), t->image2.size(), t->chunks.size());
+  std::snprintf(line, sizeof line, "sectors %d dim %d loops %d orders %d..%d lambda %g generic image %zu B real-path tables %zu B chunks %zu threads %d\n",
+                (int)t->sectors.size(), t->n, t->L, t->kmin, t->kmax, t->lambda, t->image.size(), t->tab4.size() * 4, t->chunks.size(),
+                t->threads_real);
   o += line;
   for (size_t c = 0; c < t->chunks.size(); ++c) {
     const Qmc2Chunk &ch = t->chunks[c];
-    int nrec = 0, two = 0, nloc = 0;
-    for (int s = ch.sec_begin; s < ch.sec_end; ++s) {
-      const Qmc2SectorHdr *h = reinterpret_cast<const Qmc2SectorHdr *>(t->image2.data() + t->secoff2[s]);
-      const Qmc2Rec *r = reinterpret_cast<const Qmc2Rec *>(reinterpret_cast<const uint8_t *>(h + 1) + ((h->nlocal * 4 + 15) & ~15));
-      for (int i = 0; i < h->nrec; ++i) {
-        ++nrec;
-        if (r[i].s1 != (uint32_t)(3 * t->n) * QMC2_THREADS * 8u) ++two;
-      }
-      nloc += h->nlocal;
-    }
-    std::snprintf(line, sizeof line, "chunk %zu: sectors [%d,%d) slots %d program %u B tables %u B records %d (two-factor %d, local products %d) cost %.0f\n", c,
-                  ch.sec_begin, ch.sec_end, ch.nslots, ch.prog_bytes, t->secend2[ch.sec_end - 1] - t->secoff2[ch.sec_begin], nrec, two, nloc, ch.cost);
+    std::snprintf(line, sizeof line, "chunk %zu: sectors [%d,%d) slots %d (constants %d, products %d) tables %u B records %d local products %d (max %d) cost %.0f\n", c,
+                  ch.sec_begin, ch.sec_end, ch.nslots, ch.nconst, ch.nslots - (3 * t->n + 2 + ch.nconst), ch.tab_words * 16u, ch.nrec,
+                  ch.nlocal, ch.max_local, ch.cost);
     o += line;
   }
   for (size_t c = 0; c < t->chunks3.size(); ++c) {  // complex path

@@ -36,7 +36,11 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
   const bool cplx = t->lambda > 0.0;
   // S1-S3, once per (point, shift): u = r/N (IEEE division), y = u + Delta (wrap), t = y^2 (3 - 2y), w *= 6 y (1 - y),
   // ln t (table logarithm), 1/t (reciprocal)
-  const double per_point = n * (F_DIV + 2.0 + 4.0 + 4.0 + 18.0 + 6.0);
+  // (real path: r / N as r * RN(1/N) with one FMA correction, 5 flops; complex path: the division routine)
+  double per_point = n * ((cplx ? F_DIV : 5.0) + 2.0 + 4.0 + 4.0 + 18.0 + 6.0);
+  if (!cplx)  // the chunks' product slots, once per point and chunk touched
+    for (const Qmc2Chunk &c : t->chunks)
+      if (c.sec_end > sb && c.sec_begin < se) per_point += (double)(c.nslots - (3 * n + 2 + c.nconst));
   double per_sectors = 0.0;
   int64_t ncorners = 0;
   const int eU = std::abs(t->aU0), eF = std::abs(t->aF0);
@@ -54,54 +58,70 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
       }
     }
     if (!cplx) {
-      // version-4 scheme (qmc_kernels4.cuh).  A record c * slot * slot accumulated onto its group is DMUL + DFMA = 3;
-      // the first record of a group (and G0) is two DMUL = 2.  The zero-coefficient stand-ins of empty groups and
-      // the sentinel are not counted: they are the kernel's overhead, not the method's arithmetic.
-      auto pow_muls = [](int e) {  // multiplications of x^e by repeated squaring, e >= 0
+      // version-4 scheme (qmc_kernels4.cuh, qmc_image4.cpp).  A monomial record slot * slot accumulated onto its group is
+      // one DFMA = 2; the first record of a group is one DMUL = 1.  The 0 * 0 stand-ins of empty groups and the sentinels
+      // are not counted: they are the kernel's overhead, not the method's arithmetic.
+      auto pow_muls = [](int e) {  // multiplications of x^e by repeated squaring (ipow_c), e >= 0
         int c = 0;
         for (int q = e; q > 1; q >>= 1) c += 1 + (q & 1);
         return (double)c;
       };
       const double F_RCP2 = 6.0;    // MUFU seed + 3 DFMA
-      const double F_LOG2 = 18.0;   // table-driven: 8 DFMA + DMUL + DADD
+      const double F_LOG2 = 18.0;   // table-driven: 9 DFMA
       int nL0 = 0;
       for (int j = 0; j < n; ++j)
         if (s.alpha[j] != -1 && s.beta[j]) ++nL0;
-      f = 3.0 * (1 + nL0 + s.U.size() + s.F.size());   // G0, L0, U^, F^ records (replaces the set-up count above)
+      const int nlocal = t->tab4.empty() ? 0 : (int)((t->tab4[(size_t)t->secoff4[si] * 4] >> 16) & 255u);
+      f = 1.0 * nlocal;                        // sector-local product slots
+      f += 3.0 + 2.0 * nL0;                    // G0' = c * slot * slot, times the weight; L0 = constant + sum beta_j ln t_j (FMAs)
       {
         int pos[QMC_MAXDIM], k = 0;
         for (int j = 0; j < n; ++j) pos[j] = s.alpha[j] == -1 ? k++ : -1;
-        double first = 1.0;  // G0
         for (int which = 0; which < 2; ++which) {
           unsigned seen = 0;
           for (const QmcMono &m : (which ? s.F : s.U)) {
             int g = 0;
             for (int j = 0; j < n; ++j)
               if (m.e[j] && pos[j] >= 0) g |= 1 << pos[j];
-            if (!(seen >> g & 1u)) first += 1.0;
+            f += (seen >> g & 1u) ? 2.0 : 1.0;   // first record of a group: DMUL; further records: DFMA
             seen |= 1u << g;
           }
         }
-        f -= first;  // first records: DMUL + DMUL
       }
-      f += 2.0 * ns * (nc / 2);                        // subset sums
+      f += (double)ns * nc;                            // subset sums: ns * 2^(ns-1) additions per polynomial
       for (int j = 0; j < n; ++j)
-        if (s.alpha[j] == -1) f += 1.0 + 2.0 * std::max(0, K - 3);   // beta_j ln t_j, then (.)^p / p! for p = 2 .. K-2
+        if (s.alpha[j] == -1) f += 2.0 + 2.0 * std::max(0, K - 3);   // t_j / beta_j, beta_j ln t_j, then (.)^p / p! for p = 2 .. K-2
+      // W = U^aU0 F^aF0 and the argument U^aU1 F^aF1 of the logarithm from U, 1/F (1/U), a = U/F (corner_powers)
+      const int P = std::min(t->aU1, -t->aF1), Q = (t->aU0 > 0 && t->aF0 < 0) ? std::min(t->aU0, -t->aF0) : 0;
+      auto factors_w = [&]() {
+        double c = 0.0;
+        int terms = 0;
+        if (Q > 0) { c += pow_muls(Q); ++terms; }
+        if (t->aU0 - Q > 0) { c += pow_muls(t->aU0 - Q); ++terms; }
+        if (t->aU0 < 0) { c += pow_muls(-t->aU0); ++terms; }
+        if (-t->aF0 - Q > 0) { c += pow_muls(-t->aF0 - Q); ++terms; }
+        if (t->aF0 > 0) { c += pow_muls(t->aF0); ++terms; }
+        return c + std::max(0, terms - 1);
+      };
+      auto factors_arg = [&]() {
+        double c = pow_muls(P) - (Q > 0 ? pow_muls(std::min(P, Q)) : 0.0);  // powers of a shared with W
+        int terms = 1;
+        if (t->aU1 - P > 0) { c += pow_muls(t->aU1 - P); ++terms; }
+        if (-t->aF1 - P > 0) { c += pow_muls(-t->aF1 - P); ++terms; }
+        return c + (terms - 1);
+      };
       for (int Z = 0; Z < nc; ++Z) {
         const int len = t->kmax + __builtin_popcount(Z) + 1;       // leaf window
         f += F_RCP2 + (t->aU0 < 0 ? F_RCP2 : 0.0);
-        f += (t->aU0 ? pow_muls(eU) + 1.0 : 0.0) + (t->aF0 ? pow_muls(eF) + 1.0 : 0.0);
-        if (len > 1) {
-          f += pow_muls(std::abs(t->aU1)) + pow_muls(std::abs(t->aF1)) + 1.0 + F_LOG2 + 1.0;
-          if (t->aF0 < 0 && eF >= 2 && std::abs(t->aF1) >= 2) f -= 1.0;  // (1/F)^2 is shared between W and the argument of the logarithm
-        }
-        if (len > 1) f += 2.0 * (len - 1) - 1.0;   // W Lambda^p / p!: two multiplications per term, one for p = 1
+        const bool need_a = Q > 0 || len > 1;
+        f += (need_a ? 1.0 : 0.0) + factors_w();
+        if (len > 1) f += factors_arg() + F_LOG2 + 1.0 + 2.0 * (len - 1) - 1.0;   // logarithm + L0; W Lambda^p / p!: two multiplications per term, one for p = 1
       }
-      // fold: merge at level l with Z the choices of the levels below l
+      // fold: merge at level l with Z the choices of the levels below l: (len-1) differences, one product, len (len-1) / 2 FMAs
       for (int l = 0; l < ns; ++l)
         for (int Z = 0; Z < (1 << l); ++Z) {
           const int len = ns - l + t->kmax + __builtin_popcount(Z) + 1;
-          f += 2.0 * (len - 1) + 1.0 + (double)len * (len - 1);
+          f += (len - 1) + 1.0 + (double)len * (len - 1);
         }
       f += 2.0 * K;  // weight and accumulate
     } else {

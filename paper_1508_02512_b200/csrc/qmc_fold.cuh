@@ -29,13 +29,17 @@ struct Expo {
 // per-sector state shared by the fold
 template <int NS, int K>
 struct Ctx2 {
-  double invt[NS > 0 ? NS : 1], invbeta[NS > 0 ? NS : 1];
+  double bt[NS > 0 ? NS : 1];                     // t_k / beta_k
   double cL[NS > 0 ? NS : 1][K > 1 ? K - 1 : 1];  // (beta_k ln t_k)^p / p!, p = 0 .. K-2
   double W[1 << NS], Lam[1 << NS];                // index X = set of singular variables NOT set to zero
 };
 
-// Fold2<LEVEL, ZMASK>: series of sum over Z' subset of {LEVEL..NS-1} of
-//   g_{ZMASK u Z'} prod_{j >= LEVEL, j notin Z'} A_j prod_{j in Z'} (B_j - A_j),  A_j = t_j^-1 e^{eps beta_j ln t_j}, B_j = 1/(beta_j eps)
+// The subtracted, eps-expanded integrand in product form is
+//   sum_Z g_Z prod_{j notin Z} A_j prod_{j in Z} (B_j - A_j),   A_j = t_j^-1 e^{eps beta_j ln t_j},  B_j = 1/(beta_j eps).
+// With prod_j t_j^-1 taken out (it sits in the sector's G0', qmc_image4.cpp) the factors are
+//   a_j = e^{eps beta_j ln t_j}   and   b_j - a_j,  b_j = (t_j / beta_j) / eps:
+// no multiplication by 1/t_j inside the fold.
+// Fold2<LEVEL, ZMASK>: series of sum over Z' subset of {LEVEL..NS-1} of g_{ZMASK u Z'} prod_{j >= LEVEL, j notin Z'} a_j prod_{j in Z'} (b_j - a_j)
 // window: orders -(NS-LEVEL) .. KMAX + popcount(ZMASK)  (what the remaining factors of levels < LEVEL can still use).
 template <int NS, int KMAX, int K, int LEVEL, int ZMASK>
 struct Fold2 {
@@ -44,14 +48,14 @@ struct Fold2 {
     double a[LEN - 1], b[LEN];
     Fold2<NS, KMAX, K, LEVEL + 1, ZMASK>::eval(c, a);
     Fold2<NS, KMAX, K, LEVEL + 1, ZMASK | (1 << LEVEL)>::eval(c, b);
-    const double it = c.invt[LEVEL], ib = c.invbeta[LEVEL];
+    const double bt = c.bt[LEVEL];
     double d[LEN - 1];
 #pragma unroll
-    for (int i = 0; i < LEN - 1; ++i) d[i] = it * (a[i] - b[i]);
-    out[0] = ib * b[0];
+    for (int i = 0; i < LEN - 1; ++i) d[i] = a[i] - b[i];
+    out[0] = bt * b[0];
 #pragma unroll
     for (int i = 1; i < LEN; ++i) {
-      double s = fma(ib, b[i], d[i - 1]);
+      double s = fma(bt, b[i], d[i - 1]);
 #pragma unroll
       for (int p = 1; p < i; ++p) s = fma(c.cL[LEVEL][p], d[i - 1 - p], s);
       out[i] = s;
@@ -65,7 +69,7 @@ struct Fold2<NS, KMAX, K, NS, ZMASK> {
     constexpr int X = ((1 << NS) - 1) ^ ZMASK;
     out[0] = c.W[X];
 #pragma unroll
-    for (int p = 1; p < LEN; ++p) out[p] = out[p - 1] * c.Lam[X] * (1.0 / p);
+    for (int p = 1; p < LEN; ++p) out[p] = out[p - 1] * (c.Lam[X] * (1.0 / p));
   }
 };
 

@@ -120,7 +120,7 @@ void put_rec(std::vector<uint32_t> &v, const Qmc2Rec &r) {
 }
 }  // namespace
 
-int qmc_build_image3(qmc_tables *t) {
+int qmc_build_image3(qmc_tables *t, int slots_r_opt, int slots_c_opt, int chunk_bytes_opt) {
   t->tab5.clear();
   t->secoff5.clear();
   t->prog5r.clear();
@@ -137,9 +137,9 @@ int qmc_build_image3(qmc_tables *t) {
   const int npoly = n + n * (n + 1) / 2 + 2, nderiv = npoly - 2;
   int max_r = std::min(QMC3_MAXSLOTS_R, 3 * n + 1 + 20), max_c = std::min(QMC3_MAXSLOTS_C, n + 1 + 12);
   double chunk_bytes = 16000.0;
-  if (const char *e = std::getenv("QMC3_SLOTS_R")) max_r = std::min(QMC3_MAXSLOTS_R, std::max(3 * n + 2, std::atoi(e)));
-  if (const char *e = std::getenv("QMC3_SLOTS_C")) max_c = std::min(QMC3_MAXSLOTS_C, std::max(n + 2, std::atoi(e)));
-  if (const char *e = std::getenv("QMC3_CHUNK_BYTES")) chunk_bytes = std::max(1000.0, std::atof(e));
+  if (slots_r_opt > 0) max_r = std::min(QMC3_MAXSLOTS_R, std::max(3 * n + 2, slots_r_opt));
+  if (slots_c_opt > 0) max_c = std::min(QMC3_MAXSLOTS_C, std::max(n + 2, slots_c_opt));
+  if (chunk_bytes_opt > 0) chunk_bytes = std::max(1000.0, (double)chunk_bytes_opt);
 
   // ---- per-sector polynomials, chunk ranges by table bytes ------------------------------------------------------
   std::vector<std::vector<Poly3>> polys(nsec);

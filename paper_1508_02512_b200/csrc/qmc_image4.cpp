@@ -1,0 +1,349 @@
+// Sector tables of the real (Euclidean) path, "version 4": chunks, per-chunk slot programs, 8-byte monomial records.
+// Host only.  Layout: qmc_launch.h; rationale: DESIGN.md "Data layout".
+//
+// Every thread keeps, per lattice point, a column of per-point values ("slots") in shared memory:
+//   [0,n) t_j | [n,2n) ln t_j | [2n,3n) 1/t_j | 3n: 1.0 | 3n+1: 0.0 | coefficient constants | chunk products | sector-local products
+// A monomial c * prod t_j^e_j is a multiset of FACTORS: the variables repeated by exponent and -- when c != 1 -- one
+// symbol for the constant c, which owns a slot of its own.  A byte-pair-encoding style pass over the chunk's monomials
+// (most frequent pair of factors first) turns pairs of factors into product slots, computed once per lattice point,
+// until every monomial is a product of at most two slots.  A monomial is then ONE 8-byte record {u32 off0, u32 off1}:
+// value = slot[off0] * slot[off1], accumulated with a single FMA -- the coefficient travels inside a slot.
+// To keep the constants few, every sector's U^ and F^ are divided by their most frequent |coefficient| c_U, c_F
+// (U^ = c_U U', F^ = c_F F'): W picks up the factor c_U^aU0 c_F^aF0 (folded into the coefficient of G0) and Lambda the
+// constant aU1 ln c_U + aF1 ln c_F (folded into L0).  On the double box every coefficient of U' is 1 and F' has one
+// monomial with coefficient 1/3.
+#include <algorithm>
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+
+#include "../../include/qmc_feynman.h"
+#include "qmc_bpe.h"
+#include "qmc_tables.h"
+
+using namespace qmcbpe;
+
+namespace {
+
+// relative cost of one sector at one point, fitted to measured per-chunk kernel times on B200:
+// time ~ 7.8 per corner (reciprocal, logarithm, series, its share of the fold) + 1 per record
+double sector_cost(const QmcSector &s, int kmax) {
+  const int nc = 1 << s.nsing;
+  return 7.8 * nc * (1.0 + 0.15 * kmax) + (double)(s.U.size() + s.F.size() + 2);
+}
+
+// most frequent |coefficient| of a polynomial (ties: the one met first)
+double common_coefficient(const std::vector<QmcMono> &M) {
+  double best = 1.0;
+  int best_cnt = 0;
+  for (size_t i = 0; i < M.size(); ++i) {
+    const double a = std::fabs(M[i].c);
+    int cnt = 0;
+    for (const QmcMono &m : M) cnt += std::fabs(m.c) == a;
+    if (cnt > best_cnt) {
+      best_cnt = cnt;
+      best = a;
+    }
+  }
+  return best;
+}
+
+double ipow(double x, int e) {
+  double r = 1.0;
+  for (int i = 0; i < std::abs(e); ++i) r *= x;
+  return e < 0 ? 1.0 / r : r;
+}
+
+struct ChunkConsts {
+  std::vector<double> val;  // constants other than 1.0, slot 3n + 2 + index
+  int id(double c) {
+    for (size_t i = 0; i < val.size(); ++i)
+      if (val[i] == c) return (int)i;
+    val.push_back(c);
+    return (int)val.size() - 1;
+  }
+};
+
+// factors of all monomials of sectors [s0, s1), in the order [G0', U^ ..., F^ ...] per sector.
+// G0' = prod_{regular j} t_j^alpha_j * prod_{singular j} 1/t_j  (the 1/t_j of the plus-distribution terms, Eq. 12, factored out
+// of the fold: qmc_fold.cuh)
+bool collect(const qmc_tables *t, int s0, int s1, ChunkPlan &pl, ChunkConsts &cc, std::vector<double> &cU, std::vector<double> &cF) {
+  pl.mono.clear();
+  cc.val.clear();
+  cU.clear();
+  cF.clear();
+  const int n = t->n;
+  for (int si = s0; si < s1; ++si) {
+    const QmcSector &s = t->sectors[si];
+    Factors g;
+    for (int j = 0; j < n; ++j) {
+      if (s.alpha[j] == -1) g.push_back((uint8_t)(2 * n + j));
+      for (int q = 0; q < s.alpha[j]; ++q) g.push_back((uint8_t)j);
+    }
+    std::sort(g.begin(), g.end());
+    pl.mono.push_back(g);
+    const double cu = common_coefficient(s.U), cf = common_coefficient(s.F);
+    cU.push_back(cu);
+    cF.push_back(cf);
+    for (int which = 0; which < 2; ++which)
+      for (const QmcMono &m : (which ? s.F : s.U)) {
+        Factors f = factors_of(m.e, n);
+        const double c = m.c / (which ? cf : cu);
+        if (c != 1.0) {
+          const int id = cc.id(c);
+          if (id >= QMC4_MAXCONST) return false;
+          f.push_back((uint8_t)(3 * n + 2 + id));
+        }
+        std::sort(f.begin(), f.end());
+        pl.mono.push_back(f);
+      }
+  }
+  return true;
+}
+
+void put32(std::vector<uint32_t> &v, uint32_t x) { v.push_back(x); }
+void putf64(std::vector<uint32_t> &v, double d) {
+  uint64_t b;
+  std::memcpy(&b, &d, 8);
+  v.push_back((uint32_t)b);
+  v.push_back((uint32_t)(b >> 32));
+}
+void pad4(std::vector<uint32_t> &v) {
+  while (v.size() % 4) v.push_back(0);
+}
+
+}  // namespace
+
+// table of the kernels' logarithm: z in [0.6875, 1.375), 64 intervals by the top bits of the high word, c_i = interval centre;
+// tab[i] = {1/c_i rounded, -ln(that) in extended precision}
+static void build_logtab4(double *tab) {
+  for (int i = 0; i < 64; ++i) {
+    const uint64_t lo = ((uint64_t)(0x3fe60000u + ((uint32_t)i << 14))) << 32, hi = lo + ((uint64_t)0x4000 << 32);
+    double zl, zh;
+    std::memcpy(&zl, &lo, 8);
+    std::memcpy(&zh, &hi, 8);
+    const double invc = (double)(1.0L / (0.5L * ((long double)zl + (long double)zh)));
+    tab[2 * i] = invc;
+    tab[2 * i + 1] = (double)(-logl((long double)invc));
+  }
+}
+
+int qmc_build_tables4(qmc_tables *t, int slot_budget, int chunk_bytes_opt, int threads_opt) {
+  build_logtab4(t->logtab4);
+  t->tab4.clear();
+  t->secoff4.clear();
+  t->prog4.clear();
+  t->const4.clear();
+  t->chunks.clear();
+  t->sec_cost.clear();
+  {
+    // Threads per block of the real-path kernel, measured on B200 (kernels): tables dominated by sectors
+    // with three or four singular variables execute long straight-line code paths, and one 512-thread block per SM (all
+    // 16 warps walking the same sectors) fetches instructions better than four independent 128-thread blocks; tables of
+    // short paths prefer the small blocks.
+    int big = 0;
+    for (const QmcSector &s : t->sectors) big += s.nsing >= 3;
+    t->threads_real = 2 * big >= (int)t->sectors.size() ? 512 : 128;
+    if (threads_opt == 128 || threads_opt == 512) t->threads_real = threads_opt;
+  }
+  const uint32_t T4 = (uint32_t)t->threads_real;
+  const int n = t->n, nsec = (int)t->sectors.size();
+  if (t->lambda > 0.0 || nsec == 0) return QMC_OK;
+  if (3 * n + 2 >= QMC2_MAXSLOTS) return QMC_EUNSUPPORTED;
+
+  // ---- chunk boundaries: contiguous ranges of about equal modelled cost, about chunk_bytes of tables each ------
+  std::vector<double> cost(nsec);
+  double total_cost = 0.0, total_bytes = 0.0;
+  for (int i = 0; i < nsec; ++i) {
+    const QmcSector &s = t->sectors[i];
+    cost[i] = sector_cost(s, t->kmax);
+    t->sec_cost.push_back(cost[i]);
+    total_cost += cost[i];
+    total_bytes += 16.0 * (11 + n) + 8.0 * (s.U.size() + s.F.size() + (2 << s.nsing) + 2);
+  }
+  // 40 chunk-wide slots (+ the coefficient constants) + up to 8 sector-local ones: 49 columns of 8 T bytes = 196 KB at
+  // T = 512 (one block per SM); measured on B200 (cfg4): 32 / 36 / 40 slots -> 232 / 211 / 205 ms per step
+  const int max_slots_base = slot_budget > 0 ? slot_budget : 40;
+  const double chunk_bytes = chunk_bytes_opt > 0 ? std::max(1000.0, (double)chunk_bytes_opt) : 24000.0;
+  int nch = std::max(1, (int)(total_bytes / chunk_bytes + 0.999));
+  std::vector<std::pair<int, int>> todo;  // ranges still to plan (processed in order)
+  {
+    int b = 0;
+    double acc = 0.0;
+    for (int c = 0; c < nch; ++c) {
+      const double target = total_cost * (c + 1) / nch;
+      int e = b;
+      while (e < nsec && (acc + cost[e] <= target || e == b)) acc += cost[e++];
+      if (c == nch - 1) e = nsec;
+      if (e > b) todo.push_back({b, e});
+      b = e;
+    }
+  }
+  // ---- plan (split a range in two when the slot budget does not suffice) and emit -----------------------------
+  t->secoff4.assign(nsec + 1, 0);
+  for (size_t w = 0; w < todo.size(); ++w) {
+    const int s0 = todo[w].first, s1 = todo[w].second;
+    ChunkPlan pl;
+    ChunkConsts cc;
+    std::vector<double> cU, cF;
+    if (!collect(t, s0, s1, pl, cc, cU, cF)) return QMC_EUNSUPPORTED;
+    const int nconst = (int)cc.val.size();
+    const int first_prod = 3 * n + 2 + nconst;
+    const int max_slots = std::min(QMC2_MAXSLOTS - QMC2_MAXLOCAL, std::max(max_slots_base + std::min(nconst, 6), first_prod + 1));
+    plan_chunk(pl, first_prod, max_slots);
+    Qmc2Chunk ch;
+    ch.sec_begin = s0;
+    ch.sec_end = s1;
+    ch.nslots = pl.nslots;
+    ch.nconst = nconst;
+    std::vector<uint32_t> prog4;
+    for (auto &pr : pl.prog) {
+      put32(prog4, (uint32_t)pr.first * T4 * 8u);
+      put32(prog4, (uint32_t)pr.second * T4 * 8u);
+    }
+    pad4(prog4);
+    const size_t tab4_mark = t->tab4.size();
+    const uint32_t ONE = (uint32_t)(3 * n) * T4 * 8u, ZERO = (uint32_t)(3 * n + 1) * T4 * 8u;
+    size_t mi = 0;  // index into pl.mono, same order as collect()
+    auto put_rec = [&](std::vector<uint32_t> &v, const Factors &f) {
+      v.push_back(f.size() > 0 ? (uint32_t)f[0] * T4 * 8u : ONE);
+      v.push_back(f.size() > 1 ? (uint32_t)f[1] * T4 * 8u : ONE);
+    };
+    bool too_many_locals = false;
+    for (int si = s0; si < s1 && !too_many_locals; ++si) {
+      const QmcSector &s = t->sectors[si];
+      ch.cost += cost[si];
+      // sector-local products for the monomials the chunk-wide slots leave with more than two factors
+      std::vector<std::pair<uint8_t, uint8_t>> local;
+      {
+        const size_t cnt_m = 1 + s.U.size() + s.F.size();
+        for (size_t q = 0; q < cnt_m; ++q) {
+          Factors &f = pl.mono[mi + q];
+          while (f.size() > 2) {
+            const std::pair<uint8_t, uint8_t> pr(f[0], f[1]);
+            size_t id = 0;
+            while (id < local.size() && local[id] != pr) ++id;
+            if (id == local.size()) local.push_back(pr);
+            f.erase(f.begin(), f.begin() + 2);
+            f.insert(f.begin(), (uint8_t)(pl.nslots + id));  // may exceed the sorted order: only the first two are merged next
+          }
+        }
+        if (local.size() > QMC2_MAXLOCAL || pl.nslots + (int)local.size() > QMC2_MAXSLOTS) {
+          too_many_locals = true;
+          break;
+        }
+      }
+      int pos_of[QMC_MAXDIM], k = 0;
+      uint32_t sing_ln[QMC_MAXSING] = {0}, sing_t[QMC_MAXSING] = {0};
+      double invbeta[QMC_MAXSING] = {0}, beta[QMC_MAXSING] = {0};
+      for (int j = 0; j < n; ++j) pos_of[j] = -1;
+      for (int j = 0; j < n; ++j)
+        if (s.alpha[j] == -1) {
+          sing_ln[k] = (uint32_t)(n + j) * T4 * 8u;
+          sing_t[k] = (uint32_t)j * T4 * 8u;
+          beta[k] = (double)s.beta[j];
+          invbeta[k] = 1.0 / (double)s.beta[j];
+          pos_of[j] = k++;
+        }
+      const int nc = 1 << s.nsing;
+      // group-sorted monomials (qmc_build_tables sorted them); counts per group
+      int cntU[1 << QMC_MAXSING] = {0}, cntF[1 << QMC_MAXSING] = {0};
+      const Factors &g0f = pl.mono[mi++];
+      std::vector<const Factors *> recs;  // U^ then F^, group-sorted
+      for (int which = 0; which < 2; ++which) {
+        int gprev = 0;
+        for (const QmcMono &m : (which ? s.F : s.U)) {
+          int g = 0;
+          for (int j = 0; j < n; ++j)
+            if (m.e[j] && pos_of[j] >= 0) g |= 1 << pos_of[j];
+          if (g < gprev) return QMC_EINVAL;  // monomials must arrive sorted by group
+          gprev = g;
+          int &c = (which ? cntF : cntU)[g];
+          if (c == 255) return QMC_EUNSUPPORTED;
+          ++c;
+          recs.push_back(&pl.mono[mi++]);
+        }
+      }
+      ch.nrec += (int)recs.size();
+      ch.nlocal += (int)local.size();
+      ch.max_local = std::max(ch.max_local, (int)local.size());
+      // ---- the sector block (layout: qmc_launch.h) ----
+      std::vector<uint32_t> &v = t->tab4;
+      t->secoff4[si] = (uint32_t)(v.size() / 4);
+      const size_t b0 = v.size();
+      int nL0 = 0;
+      for (int j = 0; j < n; ++j)
+        if (s.alpha[j] != -1 && s.beta[j] != 0) ++nL0;
+      const uint32_t nlw = (uint32_t)((local.size() + 1) / 2);
+      put32(v, (uint32_t)s.nsing | ((uint32_t)nL0 << 8) | ((uint32_t)local.size() << 16));
+      put32(v, 0);                              // size of the block in words (patched below)
+      put32(v, 11 + (uint32_t)nL0 + nlw);       // first dense record
+      put32(v, 0);
+      for (int q = 0; q < QMC_MAXSING; ++q) put32(v, sing_ln[q]);
+      for (int q = 0; q < QMC_MAXSING; ++q) put32(v, sing_t[q]);
+      for (int q = 0; q < QMC_MAXSING; ++q) putf64(v, invbeta[q]);
+      for (int q = 0; q < QMC_MAXSING; ++q) putf64(v, beta[q]);
+      const double cu = cU[si - s0], cf = cF[si - s0];
+      putf64(v, ipow(cu, t->aU0) * ipow(cf, t->aF0));  // w7: coefficient of G0', then its two slots
+      put_rec(v, g0f);
+      putf64(v, t->aU1 * std::log(cu) + t->aF1 * std::log(cf));  // w8: constant of L0
+      put32(v, 0);
+      put32(v, 0);
+      uint8_t extraU[16] = {0}, extraF[16] = {0};
+      for (int g = 0; g < nc; ++g) {
+        extraU[g] = cntU[g] ? (uint8_t)(cntU[g] - 1) : 0;
+        extraF[g] = cntF[g] ? (uint8_t)(cntF[g] - 1) : 0;
+      }
+      for (int q = 0; q < 4; ++q) put32(v, extraU[4 * q] | (extraU[4 * q + 1] << 8) | (extraU[4 * q + 2] << 16) | ((uint32_t)extraU[4 * q + 3] << 24));
+      for (int q = 0; q < 4; ++q) put32(v, extraF[4 * q] | (extraF[4 * q + 1] << 8) | (extraF[4 * q + 2] << 16) | ((uint32_t)extraF[4 * q + 3] << 24));
+      for (int j = 0; j < n; ++j)  // L0 = constant + sum over regular variables of beta_j ln t_j
+        if (s.alpha[j] != -1 && s.beta[j] != 0) {
+          putf64(v, (double)s.beta[j]);
+          put32(v, (uint32_t)(n + j) * T4 * 8u);
+          put32(v, 0);
+        }
+      for (auto &pr : local) {
+        put32(v, (uint32_t)pr.first * T4 * 8u);
+        put32(v, (uint32_t)pr.second * T4 * 8u);
+      }
+      pad4(v);
+      // dense first records (one per group; an empty group reads the 0.0 slot), then the extra records group by group
+      std::vector<const Factors *> extra;
+      size_t ri = 0;
+      for (int which = 0; which < 2; ++which)
+        for (int g = 0; g < nc; ++g) {
+          const int cnt = (which ? cntF : cntU)[g];
+          if (cnt) {
+            put_rec(v, *recs[ri]);
+          } else {
+            v.push_back(ZERO);
+            v.push_back(ZERO);
+          }
+          for (int q = 1; q < cnt; ++q) extra.push_back(recs[ri + q]);
+          ri += cnt;
+        }
+      for (const Factors *f : extra) put_rec(v, *f);
+      for (int q = 0; q < 2; ++q) {  // sentinels: the kernel requests operands one record and offsets two records past the last
+        v.push_back(ONE);
+        v.push_back(ONE);
+      }
+      pad4(v);
+      v[b0 + 1] = (uint32_t)((v.size() - b0) / 4);
+    }
+    if (too_many_locals) {  // split the range in two and plan again
+      t->tab4.resize(tab4_mark);
+      if (s1 - s0 == 1) return QMC_EUNSUPPORTED;
+      const int mid = (s0 + s1) / 2;
+      todo[w] = {s0, mid};
+      todo.insert(todo.begin() + w + 1, {mid, s1});
+      --w;
+      continue;
+    }
+    ch.tab_words = (uint32_t)((t->tab4.size() - tab4_mark) / 4);
+    t->chunks.push_back(ch);
+    t->prog4.push_back(prog4);
+    t->const4.push_back(cc.val);
+  }
+  t->secoff4[nsec] = (uint32_t)(t->tab4.size() / 4);
+  return QMC_OK;
+}

@@ -1,24 +1,22 @@
 // Evaluation kernel of the real (Euclidean) path, "version 4", sm_100a.  Steps S1-S7 of DESIGN.md.
 //
 // One thread = one lattice point at a time.  Per point the thread fills its column of a shared-memory slot table
-// (t_j, ln t_j, 1/t_j, 1, then the chunk's product slots chosen by the byte-pair-encoding pass of qmc_image2.cpp); a
-// monomial of U^ or F^ is then ONE record c * slot * slot.  Per sector with s singular variables:
+// (t_j, ln t_j, 1/t_j, 1, 0, coefficient constants, then the chunk's product slots chosen by the byte-pair-encoding pass of
+// qmc_image4.cpp); a monomial of U^ or F^ is then ONE 8-byte record: slot * slot, accumulated with one FMA (the
+// coefficient lives in a slot).  Per sector with s singular variables:
 //   1. partial sums of U^, F^ per group (= set of singular variables a monomial depends on), subset sums -> the values
 //      at all 2^s corners t^Z of the subtraction (Eqs. 11-12) from one pass over the records;
-//   2. per corner: W_Z = G0 U^aU0 F^aF0 with one reciprocal, Lambda_Z = ln(U^aU1 F^aF1) + L0 with ONE table-driven
+//   2. per corner: W_Z = U^aU0 F^aF0 with one reciprocal, Lambda_Z = ln(U^aU1 F^aF1) + L0 with ONE table-driven
 //      logarithm (exponents are compile-time: they depend only on the dimension and the loop number, Eq. 6);
 //   3. the product form of the eps-expanded subtracted integrand, folded one singular variable at a time with series
-//      windows of exactly the needed length (qmc_fold.cuh).
+//      windows of exactly the needed length (qmc_fold.cuh); the common factor G0' = c prod_reg t^alpha prod_sing 1/t
+//      multiplies the weight once per sector.
 // The chunk's slot program and the sector tables are part of the KERNEL PARAMETER BLOCK (constant bank 0, layout in
-// qmc_launch.h).  Measured reasons (profiles/r01i_eval_kernel_ncu.md): with the tables in shared memory (the round's
-// earlier kernel) the record loops were bound by the shared-memory data pipe (6 wavefronts per record: 2 for the
-// 16-byte broadcast of the record, 2 + 2 for the slot operands) and by the exposed LDS -> LDS -> DMUL -> DFMA latency
-// chain of one short loop per group, at 11 instructions per record.  Here a record is 2 uniform loads (LDCU.64), 2 LDS
-// [R + UR], DMUL, DFMA (the coefficient is a uniform-register operand), trip counts are uniform, the FIRST record of
-// every group sits in a dense array with a compile-time destination register (2^nsing independent load/multiply chains
-// in one basic block), and all further records are one stream walked with the next operands in flight.  The logarithm
-// table is 64 entries x 8 interleaved copies (lane & 7 picks the copy): every lookup is a conflict-free LDS.128
-// (4 wavefronts instead of the ~10 measured with one copy).
+// qmc_launch.h): a record is one uniform load (LDCU.64; two records per LDCU.128 in the dense part), 2 LDS [R + UR] and one
+// DFMA; trip counts are uniform; the FIRST record of every group sits in a dense array with a compile-time destination
+// register (2^nsing independent load/multiply chains in one basic block), and all further records are one stream walked
+// with the next operands in flight.  The logarithm table is 64 entries x 8 interleaved copies (lane & 7 picks the copy):
+// every lookup is a conflict-free LDS.128.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -74,7 +72,8 @@ __device__ __forceinline__ double fast_log_unchecked(double x, const double2 *__
   q = fma(r, q, qmc4_logc[4]);
   q = fma(r, q, qmc4_logc[5]);
   q = fma(r, q, qmc4_logc[6]);
-  return fma(r * r, q, r) + y0;
+  // r + r^2 q + y0 as r (1 + r q) + y0: two FMAs instead of DMUL + DFMA + DADD (1 + r q carries 2^-53, times |r| < 2^-7)
+  return fma(r, fma(r, q, 1.0), y0);
 }
 static_assert(QMC4_LOG_COPIES * 16 == 1 << 7, "fast_log index arithmetic assumes 128 bytes per table entry row");
 
@@ -108,27 +107,49 @@ __device__ __forceinline__ double block_sum_t(double v, double *scratch /*[T / 3
 __device__ __forceinline__ double slot_at(const unsigned char *__restrict__ sl, uint32_t off) {
   return *reinterpret_cast<const double *>(sl + off);
 }
-// value of one record: c * slot[off0] * slot[off1]
+__device__ __forceinline__ double u2d(uint32_t lo, uint32_t hi) { return __hiloint2double((int)hi, (int)lo); }
+// 16-byte records {f64 c, u32 off0, u32 off1} of the complex path's real streams (qmc_kernels5.cuh): c * slot[off0] * slot[off1]
 __device__ __forceinline__ double rec_val(const uint4 r, const unsigned char *__restrict__ sl) {
   return __hiloint2double((int)r.y, (int)r.x) * (slot_at(sl, r.z) * slot_at(sl, r.w));
 }
 __device__ __forceinline__ double rec_fma(const uint4 r, const unsigned char *__restrict__ sl, double acc) {
   return fma(__hiloint2double((int)r.y, (int)r.x), slot_at(sl, r.z) * slot_at(sl, r.w), acc);
 }
-__device__ __forceinline__ double u2d(uint32_t lo, uint32_t hi) { return __hiloint2double((int)hi, (int)lo); }
 
-// one sector at one point: out[i] = coefficient of eps^(i - NS) of the subtracted integrand (without the weight w).
-// `o` = word offset of the sector block in p.tab (uniform).
+// W = U^aU0 F^aF0 and the argument U^aU1 F^aF1 of the logarithm (aU1 > 0 > aF1) from U, 1/F (and 1/U when aU0 < 0), with
+// a = U / F shared between the two where both want it (double box: a, a^2, a^2 U, (1/F)^2, a (1/F)^2: five products)
+template <class E>
+__device__ __forceinline__ void corner_powers(double U, double F, double rF, double rU, double &W, double &arg) {
+  constexpr int P = E::aU1 < -E::aF1 ? E::aU1 : -E::aF1;                              // arg = a^P U^(aU1-P) rF^(-aF1-P)
+  constexpr int Q = (E::aU0 > 0 && E::aF0 < 0) ? (E::aU0 < -E::aF0 ? E::aU0 : -E::aF0) : 0;  // W = a^Q U^(aU0-Q) rF^(-aF0-Q)
+  const double a = U * rF;
+  double w = 1.0, g = 1.0;
+  bool wset = false;
+  if (Q > 0) { w = ipow_c<Q>(a); wset = true; }
+  if (E::aU0 - Q > 0) { const double x = ipow_c<(E::aU0 - Q > 0 ? E::aU0 - Q : 0)>(U); w = wset ? w * x : x; wset = true; }
+  if (E::aU0 < 0) { const double x = ipow_c<(E::aU0 < 0 ? -E::aU0 : 0)>(rU); w = wset ? w * x : x; wset = true; }
+  if (-E::aF0 - Q > 0) { const double x = ipow_c<(-E::aF0 - Q > 0 ? -E::aF0 - Q : 0)>(rF); w = wset ? w * x : x; wset = true; }
+  if (E::aF0 > 0) { const double x = ipow_c<(E::aF0 > 0 ? E::aF0 : 0)>(F); w = wset ? w * x : x; wset = true; }
+  W = w;
+  g = ipow_c<P>(a);
+  if (E::aU1 - P > 0) g *= ipow_c<(E::aU1 - P > 0 ? E::aU1 - P : 0)>(U);
+  if (-E::aF1 - P > 0) g *= ipow_c<(-E::aF1 - P > 0 ? -E::aF1 - P : 0)>(rF);
+  arg = g;
+}
+
+// one sector at one point: out[i] = coefficient of eps^(i - NS) of the subtracted integrand without the weight w and
+// without the sector's common factor G0' (returned in g0).  `o` = word offset of the sector block in p.tab (uniform).
 template <int NDIM, int L, int NS, int KMAX, int T>
 __device__ __forceinline__ bool sector4(const Qmc4Launch &p, const uint32_t o, unsigned char *__restrict__ sl,
-                                        const double2 *__restrict__ tabq, double (&out)[KMAX + NS + 1]) {
+                                        const double2 *__restrict__ tabq, double (&out)[KMAX + NS + 1], double &g0) {
   unsigned worst = 0;  // fast_log_unchecked
   constexpr int K = KMAX + NS + 1, NC = 1 << NS, FULL = NC - 1;
   typedef Expo<NDIM, L> E;
+  const unsigned char *tb = reinterpret_cast<const unsigned char *>(p.tab);
   const uint4 h0 = p.tab[o];
   const uint32_t nL0 = (h0.x >> 8) & 255u, nlocal = (h0.x >> 16) & 255u;
   {  // sector-local products: slot[local0 + i] = slot[a] * slot[b]
-    const uint32_t lw = o + 9;
+    const uint32_t lw = o + 11 + nL0;
 #pragma unroll 1
     for (uint32_t i = 0; i < nlocal; i += 2) {
       const uint4 pw = p.tab[lw + (i >> 1)];
@@ -136,40 +157,49 @@ __device__ __forceinline__ bool sector4(const Qmc4Launch &p, const uint32_t o, u
       if (i + 1 < nlocal) *reinterpret_cast<double *>(sl + p.local0_off + (i + 1) * (T * 8)) = slot_at(sl, pw.z) * slot_at(sl, pw.w);
     }
   }
-  uint32_t rw = o + h0.z;  // first record
-  const double G0 = rec_val(p.tab[rw], sl);
-  ++rw;
-  double L0 = 0.0;
+  {
+    const uint4 g = p.tab[o + 7];
+    g0 = u2d(g.x, g.y) * (slot_at(sl, g.z) * slot_at(sl, g.w));
+  }
+  double L0 = u2d(p.tab[o + 8].x, p.tab[o + 8].y);
 #pragma unroll 2
-  for (uint32_t i = 0; i < nL0; ++i) L0 = rec_fma(p.tab[rw + i], sl, L0);
-  rw += nL0;
+  for (uint32_t i = 0; i < nL0; ++i) {
+    const uint4 r = p.tab[o + 11 + i];
+    L0 = fma(u2d(r.x, r.y), slot_at(sl, r.z), L0);
+  }
   Ctx2<NS, K> c;
   {
     // first record of every group (dense, compile-time destination), then the extra records group by group;
     // subset sums: P[X] = value with the singular variables outside X set to zero
     double PU[NC], PF[NC];
-    const unsigned char *tb = reinterpret_cast<const unsigned char *>(p.tab);
-    {
-      // (pointer + compile-time offset, not p.tab[rw + g]: the 32-bit index sum may wrap, so ptxas computed every record's
-      //  address with its own UIADD3 + ULEA and then ran out of uniform registers -- 4 extra instructions per record)
-      const unsigned char *fr = tb + rw * 16u;
+    const unsigned char *fr = tb + (o + h0.z) * 16u;
+    if (NC == 1) {
+      const uint4 q = *reinterpret_cast<const uint4 *>(fr);
+      PU[0] = slot_at(sl, q.x) * slot_at(sl, q.y);
+      PF[0] = slot_at(sl, q.z) * slot_at(sl, q.w);
+    } else {
 #pragma unroll
-      for (int g = 0; g < NC; ++g) PU[g] = rec_val(*reinterpret_cast<const uint4 *>(fr + g * 16), sl);
+      for (int g = 0; g < NC; g += 2) {
+        const uint4 q = *reinterpret_cast<const uint4 *>(fr + g * 8);
+        PU[g] = slot_at(sl, q.x) * slot_at(sl, q.y);
+        PU[g + 1] = slot_at(sl, q.z) * slot_at(sl, q.w);
+      }
 #pragma unroll
-      for (int g = 0; g < NC; ++g) PF[g] = rec_val(*reinterpret_cast<const uint4 *>(fr + (NC + g) * 16), sl);
+      for (int g = 0; g < NC; g += 2) {
+        const uint4 q = *reinterpret_cast<const uint4 *>(fr + (NC + g) * 8);
+        PF[g] = slot_at(sl, q.x) * slot_at(sl, q.y);
+        PF[g + 1] = slot_at(sl, q.z) * slot_at(sl, q.w);
+      }
     }
-    rw += 2 * NC;
-    const uint4 cu = p.tab[o + 7], cf = p.tab[o + 8];
+    const uint4 cu = p.tab[o + 9], cf = p.tab[o + 10];
     const uint32_t cuw[4] = {cu.x, cu.y, cu.z, cu.w}, cfw[4] = {cf.x, cf.y, cf.z, cf.w};
     // extra records: one stream across all groups, software-pipelined by one record -- the slot operands of the NEXT
-    // record are requested before the current one is accumulated, also across group boundaries (the block ends with a
-    // harmless sentinel record), so the LDCU -> LDS -> DMUL -> DFMA chain is not exposed once per group
-    // (only the OFFSETS of the next record are requested ahead; its coefficient is loaded in its own iteration, where the
-    //  wait for the slot operands hides the latency -- carrying it across the iteration cost two UMOV per record)
-    uint32_t rwb = rw * 16u;  // byte offset of the current record: {f64 c | u32 off0, u32 off1}
-    uint2 ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);
+    // record are requested before the current one is accumulated, also across group boundaries (the block ends with two
+    // harmless sentinel records), so the LDCU -> LDS -> DFMA chain is not exposed once per group
+    uint32_t rwb = (o + h0.z) * 16u + 2u * NC * 8u;  // byte offset of the current record {u32 off0, u32 off1}
+    uint2 ro = *reinterpret_cast<const uint2 *>(tb + rwb);
     double ra = slot_at(sl, ro.x), rb = slot_at(sl, ro.y);
-    ro = *reinterpret_cast<const uint2 *>(tb + rwb + 24);  // offsets run TWO records ahead, operands one (two sentinels)
+    ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);  // offsets run TWO records ahead, operands one (two sentinels)
     constexpr int NW = (NC + 3) / 4, GW = NC < 4 ? NC : 4;  // count words per polynomial, groups per word
 #pragma unroll
     for (int q = 0; q < 2 * NW; ++q) {
@@ -182,13 +212,11 @@ __device__ __forceinline__ bool sector4(const Qmc4Launch &p, const uint32_t o, u
           double accg = q < NW ? PU[gg] : PF[gg];
 #pragma unroll 1
           for (uint32_t i = 0; i < cnt; ++i) {
-            const uint2 rc = *reinterpret_cast<const uint2 *>(tb + rwb);
-            const double v = ra * rb;
-            rwb += 16u;
+            accg = fma(ra, rb, accg);
+            rwb += 8u;
             ra = slot_at(sl, ro.x);
             rb = slot_at(sl, ro.y);
-            ro = *reinterpret_cast<const uint2 *>(tb + rwb + 24);
-            accg = fma(u2d(rc.x, rc.y), v, accg);
+            ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);
           }
           if (q < NW) PU[gg] = accg; else PF[gg] = accg;
         }
@@ -202,34 +230,31 @@ __device__ __forceinline__ bool sector4(const Qmc4Launch &p, const uint32_t o, u
           PU[X] += PU[X ^ (1 << b)];
           PF[X] += PF[X ^ (1 << b)];
         }
-    // corners: W = G0 U^aU0 F^aF0 (one reciprocal), Lambda = ln(U^aU1 F^aF1) + L0 (one logarithm)
+    // corners: W = U^aU0 F^aF0 (one reciprocal), Lambda = ln(U^aU1 F^aF1) + L0 (one logarithm)
 #pragma unroll
     for (int X = 0; X < NC; ++X) {
       const double U = PU[X], F = PF[X];
       const double rF = fast_rcp(F);
-      double W = G0;
-      if (E::aU0 > 0) W *= ipow_c<(E::aU0 > 0 ? E::aU0 : 0)>(U);
-      if (E::aU0 < 0) W *= ipow_c<(E::aU0 < 0 ? -E::aU0 : 0)>(fast_rcp(U));
-      if (E::aF0 > 0) W *= ipow_c<(E::aF0 > 0 ? E::aF0 : 0)>(F);
-      if (E::aF0 < 0) W *= ipow_c<(E::aF0 < 0 ? -E::aF0 : 0)>(rF);
+      const double rU = E::aU0 < 0 ? fast_rcp(U) : 0.0;
+      double W, arg;
+      corner_powers<E>(U, F, rF, rU, W, arg);
       c.W[X] = W;
-      if (KMAX > 0 || X != FULL) c.Lam[X] = fast_log_unchecked(ipow_c<E::aU1>(U) * ipow_c<-E::aF1>(rF), tabq, worst) + L0;
+      if (KMAX > 0 || X != FULL) c.Lam[X] = fast_log_unchecked(arg, tabq, worst) + L0;
     }
   }
   if (NS > 0) {
-    const uint4 sln = p.tab[o + 1], sinv = p.tab[o + 2];
+    const uint4 sln = p.tab[o + 1], st = p.tab[o + 2];
     const uint4 ib01 = p.tab[o + 3], ib23 = p.tab[o + 4], b01 = p.tab[o + 5], b23 = p.tab[o + 6];
-    const uint32_t lnw[4] = {sln.x, sln.y, sln.z, sln.w}, invw[4] = {sinv.x, sinv.y, sinv.z, sinv.w};
+    const uint32_t lnw[4] = {sln.x, sln.y, sln.z, sln.w}, tw[4] = {st.x, st.y, st.z, st.w};
     const double ibv[4] = {u2d(ib01.x, ib01.y), u2d(ib01.z, ib01.w), u2d(ib23.x, ib23.y), u2d(ib23.z, ib23.w)};
     const double bv[4] = {u2d(b01.x, b01.y), u2d(b01.z, b01.w), u2d(b23.x, b23.y), u2d(b23.z, b23.w)};
 #pragma unroll
     for (int k = 0; k < NS; ++k) {
-      c.invt[k] = slot_at(sl, invw[k]);
-      c.invbeta[k] = ibv[k];
+      c.bt[k] = ibv[k] * slot_at(sl, tw[k]);
       const double Lk = bv[k] * slot_at(sl, lnw[k]);
       c.cL[k][0] = 1.0;
 #pragma unroll
-      for (int q = 1; q < K - 1; ++q) c.cL[k][q] = c.cL[k][q - 1] * Lk * (1.0 / q);
+      for (int q = 1; q < K - 1; ++q) c.cL[k][q] = c.cL[k][q - 1] * (Lk * (1.0 / q));
     }
   }
   Fold2<NS, KMAX, K, 0, 0>::eval(c, out);
@@ -237,10 +262,6 @@ __device__ __forceinline__ bool sector4(const Qmc4Launch &p, const uint32_t o, u
 }
 
 }  // namespace qmc4
-
-#ifndef Q4_NOPERSEC
-#define Q4_NOPERSEC 0
-#endif
 
 // partial layout: fused  : [run of sectors][shift][slice][NACC]
 //                 persec : [sector row][shift][slice][NACC]        (NACC = QMC_MAXSING + KMAX + 1, index a <-> order a - QMC_MAXSING)
@@ -270,11 +291,13 @@ __global__ void __launch_bounds__(T, 512 / T) qmc4_eval_kernel(const __grid_cons
   for (int i = tid; i < QMC4_LOG_ENTRIES * QMC4_LOG_COPIES; i += T)
     logtab[i] = reinterpret_cast<const double2 *>(p.logtab)[i / QMC4_LOG_COPIES];
   for (int i = tid; i < p.m * NDIM; i += T) shf[i] = p.shifts[i];
-  slots[3 * NDIM * T + tid] = 1.0;  // the constant slot
+  slots[3 * NDIM * T + tid] = 1.0;        // the constant slots: 1, 0, the chunk's coefficient constants
+  slots[(3 * NDIM + 1) * T + tid] = 0.0;
+  for (uint32_t i = 0; i < p.nconst; ++i) slots[(3 * NDIM + 2 + i) * T + tid] = p.cval[i];
   __syncthreads();
 
   const uint32_t N = p.N;
-  const double dN = (double)N;
+
   const uint32_t stride = (uint32_t)p.nslices * T;
   uint32_t dz[NDIM];
 #pragma unroll
@@ -300,6 +323,7 @@ __global__ void __launch_bounds__(T, 512 / T) qmc4_eval_kernel(const __grid_cons
 #pragma unroll
     for (int j = 0; j < NDIM; ++j) r[j] = (uint32_t)((p.off[j] + (uint64_t)(c0 + tid) * p.zeff[j]) % N);
 
+    uint32_t since_sync = 0;
     for (uint32_t cb = c0; cb < p.count; cb += stride) {
       // S1-S3: lattice point (Eq. 17), shift + wrap (Eq. 18), periodising transform (Eq. 21), per-point slot table
       const bool valid = cb + tid < p.count;
@@ -307,7 +331,10 @@ __global__ void __launch_bounds__(T, 512 / T) qmc4_eval_kernel(const __grid_cons
       bool inside = true;
 #pragma unroll
       for (int j = 0; j < NDIM; ++j) {
-        double u = (double)r[j] / dN;
+        // u = r / N correctly rounded (the oracle's IEEE division) without the division routine: q = r * RN(1/N),
+        // remainder by FMA (exact), one correction -- Markstein's theorem (r, N integers below 2^31: no exception case)
+        const double rd = (double)r[j], q0 = rd * p.invN;
+        const double u = fma(fma(-q0, p.dN, rd), p.invN, q0);
         double y = u + shf[kap * NDIM + j];
         if (y >= 1.0) y -= 1.0;
         double tj;
@@ -337,15 +364,13 @@ __global__ void __launch_bounds__(T, 512 / T) qmc4_eval_kernel(const __grid_cons
         if (i + 1 < p.nprog)
           *reinterpret_cast<double *>(sl + p.first_prod_off + (i + 1) * (T * 8)) = slot_at(sl, pw.z) * slot_at(sl, pw.w);
       }
-      // S4-S6: all sectors of the run at this point.  A barrier every fourth point re-aligns the block's warps: the
-      // kernel was close to its instruction-fetch ceiling (profiles/r01p_final.md: GPC instruction-cache requests at
-      // 77 % of their sustained rate, SM instruction-cache hit rate 87 %), and warps that walk the same sector at about
-      // the same time share the fetched lines -- while between two barriers they drift apart again, which keeps the
-      // table-walk phase of one warp over the arithmetic phase of another.  Measured on cfg4 (ms per step): no barrier
-      // 248.0; one per 64 / 16 / 8 / 4 / 2 / 1 points 246.6 / 239.3 / 234.5 / 232.0 / 234.5 / 242.0; one per 16 / 8 / 4 / 1
-      // sectors 244.8 / 249.0 / 255.1 / 268.3.
-      // (barriers among groups of 8 or 4 warps instead of the whole block: 232.7-237.0 ms, no gain)
-      if (T >= 256 && (((cb - c0) / stride) & 3u) == 0u) __syncthreads();
+      // S4-S6: all sectors of the run at this point.  A barrier every few points (p.sync_every, kernels)
+      // re-aligns the block's warps so that they share fetched instruction lines, while between two barriers they drift
+      // apart again, which keeps the table-walk phase of one warp over the arithmetic phase of another.
+      if (T >= 256 && p.sync_every) {
+        if (since_sync == 0) __syncthreads();
+        since_sync = since_sync + 1 == p.sync_every ? 0 : since_sync + 1;
+      }
       for (int si = 0; si < p.nsec; ++si) {
         // (offsets come from an array indexed by the induction variable: a loop-carried offset read from the table
         //  itself makes ptxas give up the uniform datapath for the whole table walk)
@@ -355,26 +380,24 @@ __global__ void __launch_bounds__(T, 512 / T) qmc4_eval_kernel(const __grid_cons
   case NS_: {                                                                                                \
     if (NS_ <= SMAX) {                                                                                       \
       constexpr int NSC = NS_ <= SMAX ? NS_ : 0, KK = KMAX + NSC + 1;                                        \
-      double res[KK];                                                                                        \
-      bool fin = sector4<NDIM, L, NSC, KMAX, T>(p, so, sl, tabq, res);                                       \
+      double res[KK], g0;                                                                                    \
+      bool fin = sector4<NDIM, L, NSC, KMAX, T>(p, so, sl, tabq, res, g0);                                   \
+      const double wg = w * g0;                                                                              \
+      fin = fin && finite_hi(g0);                                                                            \
       _Pragma("unroll") for (int i = 0; i < KK; ++i) fin = fin && finite_hi(res[i]);                         \
       /* a non-finite evaluation is dropped (and counted); a dead thread has w = 0.  Predicated, not branched */ \
       cntNonFinite += (live && !fin) ? 1u : 0u;                                                              \
-      if (Q4_NOPERSEC || !p.persec) {                                                                        \
+      if (!p.persec) {                                                                                       \
         _Pragma("unroll") for (int i = 0; i < KK; ++i)                                                       \
-          if (fin) acc[QMC_MAXSING - NSC + i] = fma(w, res[i], acc[QMC_MAXSING - NSC + i]);                  \
+          if (fin) acc[QMC_MAXSING - NSC + i] = fma(wg, res[i], acc[QMC_MAXSING - NSC + i]);                 \
       } else {                                                                                               \
         double *sa = sacc + ((size_t)si * NACC + (QMC_MAXSING - NSC)) * T + tid;                             \
         _Pragma("unroll") for (int i = 0; i < KK; ++i)                                                       \
-          if (fin) sa[(size_t)i * T] += w * res[i];                                                          \
+          if (fin) sa[(size_t)i * T] += wg * res[i];                                                         \
       }                                                                                                      \
     }                                                                                                        \
   } break;
-#ifdef Q4_T1
-        switch (4) {
-#else
         switch (h0.x & 255u) {
-#endif
           QMC4_CASE(0)
           QMC4_CASE(1)
           QMC4_CASE(2)
@@ -388,12 +411,7 @@ __global__ void __launch_bounds__(T, 512 / T) qmc4_eval_kernel(const __grid_cons
     }
 
     // S7: block reduction -> one partial per (run | sector, shift, block)
-#ifdef Q4_T3
-    for (int a = 0; a < NACC; ++a) p.partial[(size_t)(blockIdx.x * T + tid) * NACC + a] += acc[a];
-    if (false) {
-#else
     if (!p.persec) {
-#endif
       double *dst = p.partial + (((size_t)p.out_row * p.m + kap) * p.max_slices + blockIdx.x) * NACC;
 #pragma unroll
       for (int a = 0; a < NACC; ++a) {

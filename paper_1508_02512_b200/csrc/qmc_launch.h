@@ -51,17 +51,21 @@ cudaError_t qmc_kernel_launch(int ndim, int kmax, int flavor, dim3 grid, size_t 
 // One launch = one run of sectors of one chunk; blockIdx.x = slice of the lattice points.  The chunk's slot program and
 // the sector tables travel INSIDE the kernel parameter block (constant bank 0): every table read is a uniform load
 // (LDCU) into uniform registers, slot operands are addressed [thread column + uniform offset], the record loops run on
-// the uniform datapath and are unrolled by the compiler.  Layout of `tab` (16-byte words):
-//   [prog_word ..)  slot program: nprog x {u32 a_off, u32 b_off} (byte offsets into the thread's slot column), 2 per word
+// the uniform datapath.  A monomial record is 8 bytes {u32 off0, u32 off1}: value = slot[off0] * slot[off1] (byte offsets
+// into the thread's slot column; the coefficient lives in a slot, qmc_image4.cpp).  Layout of `tab` (16-byte words):
+//   [prog_word ..)  slot program: nprog x {u32 a_off, u32 b_off}, 2 per word
 //   [sec_word ..)   sector blocks, back to back; sector block (word offsets relative to its start):
-//     w0 = {nsing | nL0 << 8 | nlocal << 16, nwords of the block, rec_word (first record), 0}
-//     w1 = sing_ln[4]  (byte offsets of ln t_k of the singular positions)      w2 = sing_inv[4]  (of 1/t_k)
-//     w3,w4 = invbeta[4] (f64)      w5,w6 = beta[4] (f64)
-//     w7 = extra records per group of U^ (u8 x 16)      w8 = the same for F^
-//     w9.. = local program: nlocal x {u32 a_off, u32 b_off}, padded to a word
-//     records {f64 c, u32 off0, u32 off1}: [G0][L0 x nL0][first record of every group of U^: 2^nsing, c = 0 if the
-//     group is empty][the same for F^][extra records of U^ by group][extra records of F^ by group][two sentinels, c = 0]
-#define QMC4_TAB_WORDS 1808  // 28 928 bytes of tables per launch (kernel parameters are limited to 32 764 bytes)
+//     w0 = {nsing | nL0 << 8 | nlocal << 16, nwords of the block, first dense record word, 0}
+//     w1 = sing_ln[4]  (byte offsets of ln t_k of the singular positions)      w2 = sing_t[4]  (of t_k)
+//     w3,w4 = 1/beta[4] (f64)      w5,w6 = beta[4] (f64)
+//     w7 = {f64 coefficient of G0', u32 off0, u32 off1}: G0' = c * slot * slot = c_U^aU0 c_F^aF0 prod_reg t^alpha prod_sing 1/t
+//     w8 = {f64 constant of L0 = aU1 ln c_U + aF1 ln c_F, 0, 0}
+//     w9 = extra records per group of U^ (u8 x 16)      w10 = the same for F^
+//     w11.. = nL0 x {f64 beta_j, u32 offset of ln t_j, 0} (regular variables), then the local program nlocal x {u32 a_off,
+//     u32 b_off} padded to a word, then the records: [first record of every group of U^: 2^nsing, the 0.0 slot twice if
+//     the group is empty][the same for F^][extra records of U^ by group][extra records of F^ by group][two sentinels],
+//     padded to a word
+#define QMC4_TAB_WORDS 1800  // 28 800 bytes of tables per launch (kernel parameters are limited to 32 764 bytes)
 #define QMC4_MAX_SEC 160     // sectors per launch
 #define QMC4_LOG_ENTRIES 64
 #define QMC4_LOG_COPIES 8
@@ -75,8 +79,10 @@ struct Qmc4Launch {
   int32_t m, transform, persec, max_slices;
   int32_t nsec, out_row, count_boundary, nslices;
   uint32_t nprog, prog_word, sec_word, first_prod_off;  // first_prod_off, local0_off: byte offsets in the slot column
-  uint32_t local0_off, max_nslots, pad0, pad1;
+  uint32_t local0_off, max_nslots, nconst, sync_every;  // sync_every: block barrier every that many points (0 = never)
   double tc[4], wc[2];           // periodising transform (see qmc_transform_poly)
+  double dN, invN;               // (double)N and RN(1 / N): constant-bank operands of the lattice-point division (S1)
+  double cval[QMC4_MAXCONST];    // values of the coefficient-constant slots 3n + 2 ..
   uint16_t secw[QMC4_MAX_SEC];  // word offset of the sector blocks in tab, in evaluation order (sorted by nsing: sectors
                                 // that run the same code path are neighbours, which the instruction cache likes)
   uint16_t secrow[QMC4_MAX_SEC]; // per-sector mode: row of the partial buffer relative to out_row

@@ -346,14 +346,26 @@ int qmc_build_tables(const qmc_graph *g, const qmc_kinematics *kin, int eps_orde
     while (T->image.size() % 16) T->image.push_back(0);
   }
   T->secoff.push_back((uint32_t)T->image.size());
-  // version-2 image (real path); graphs it cannot represent fall back to the version-1 kernel
-  if (qmc_build_image2(T) != QMC_OK) {
-    T->image2.clear();
+  // table-driven kernels: real path (version 4) and complex path (version 5).  What a builder cannot represent falls back
+  // to the generic kernel: on failure EVERYTHING the builder left behind is dropped, so that qmc_integrate sees no
+  // half-built tables
+  if (qmc_build_tables4(T, opt ? opt->slot_budget : 0, opt ? opt->chunk_bytes : 0, opt ? opt->threads : 0) != QMC_OK) {
+    T->tab4.clear();
+    T->secoff4.clear();
+    T->prog4.clear();
+    T->const4.clear();
     T->chunks.clear();
   }
-  if (qmc_build_image3(T) != QMC_OK) {
+  if (qmc_build_image3(T, opt ? opt->slot_budget_cplx_real : 0, opt ? opt->slot_budget_cplx : 0, opt ? opt->chunk_bytes : 0) != QMC_OK) {
     T->image3.clear();
     T->chunks3.clear();
+    T->tab5.clear();
+    T->secoff5.clear();
+    T->prog5r.clear();
+    T->prog5c.clear();
+    T->chunk3_nslots_c.clear();
+    T->chunk3_max_local_c.clear();
   }
+  if (T->sec_cost.size() != T->sectors.size()) T->sec_cost.assign(T->sectors.size(), 1.0);
   return QMC_OK;
 }

@@ -30,44 +30,28 @@ struct QmcSectorHdr {
 };
 static_assert(sizeof(QmcSectorHdr) == 64, "sector header must be 64 bytes");
 
-// ---- planning image of the real path ("version 2": host only; chunk sizes, describe(); the kernels read the
-// version-4 tables built from the same plan, qmc_launch.h) ------------------------------------------------
-// Sectors are grouped into CHUNKS.  Every chunk owns a "slot program": each thread keeps, per lattice point, a table
-// of per-point values in shared memory (slot s of thread tid at slots[s * QMC2_THREADS + tid]):
-//   slots [0,n) t_j | [n,2n) ln t_j | [2n,3n) 1/t_j | 3n: 1.0 | 3n+1 ...: products slot[k] = slot[a] * slot[b]
+// ---- real path ("version 4" tables, built by qmc_image4.cpp; layout of the kernel-side tables: qmc_launch.h) ----------
+// Sectors are grouped into CHUNKS.  Every chunk owns a "slot program": each thread keeps, per lattice point, a column
+// of per-point values in shared memory (slot s of thread tid at slots[s * T + tid]):
+//   [0,n) t_j | [n,2n) ln t_j | [2n,3n) 1/t_j | 3n: 1.0 | 3n+1: 0.0 | 3n+2 ..: coefficient constants | products slot[k] = slot[a] * slot[b]
 // chosen per chunk by a byte-pair-encoding style pass over the chunk's monomials (most frequent pair of factors
-// first) until every monomial is a product of at most two slots.  A monomial is then one 16-byte record.
-#define QMC2_THREADS 256   // planning image only; the real-path kernel runs 128 or 512 threads per block (qmc_tables::threads_real)
+// first) until every monomial is a product of at most two slots.  A monomial is then one 8-byte record.
 #define QMC2_MAXSLOTS 56
-struct Qmc2Rec {        // value = c * slot[s0] * slot[s1]; s0, s1 are BYTE offsets slot * QMC2_THREADS * 8 into the
-  double c;             // thread's column of the slot table
+#define QMC2_MAXLOCAL 8
+#define QMC4_MAXCONST 12   // distinct coefficient constants (other than 1) per chunk
+struct Qmc2Rec {        // complex-path record: value = c * slot[s0] * slot[s1]; s0, s1 are BYTE offsets into the thread's column
+  double c;
   uint32_t s0, s1;
 };
 static_assert(sizeof(Qmc2Rec) == 16, "record must be 16 bytes");
-#define QMC2_MAXLOCAL 8
-struct Qmc2SectorHdr {  // followed by nlocal x {u16 a, u16 b} (sector-local products slot[nslots + i] = slot[a] * slot[b],
-                        // padded to 16 bytes), then the records: [G0][L0 x nL0][U^ by group][F^ by group]
-  uint8_t nsing, nL0;
-  uint16_t nrec;
-  uint8_t nlocal, pad0[3];
-  uint16_t sing_ln[QMC_MAXSING];   // premultiplied slot index of ln t_k for singular position k
-  uint16_t sing_inv[QMC_MAXSING];  // ... of 1/t_k
-  double invbeta[QMC_MAXSING];     // 1/beta_k
-  double beta[QMC_MAXSING];        // beta_k
-  uint8_t pad1[8];
-  uint8_t cntU[1 << QMC_MAXSING];  // records per group (set of singular positions the monomial depends on); 16-byte aligned
-  uint8_t cntF[1 << QMC_MAXSING];
-};
-static_assert(offsetof(Qmc2SectorHdr, cntU) % 16 == 0, "group counts are read as one 16-byte word");
-static_assert(sizeof(Qmc2SectorHdr) == 128, "v2 sector header");
-struct Qmc2ChunkHdr {   // 16 bytes, followed by nprog x {u16 a, u16 b} (premultiplied), padded to 16 bytes
-  uint32_t nslots, nprog, first_prod, pad;
-};
 struct Qmc2Chunk {      // host description of one chunk
   int sec_begin = 0, sec_end = 0;
-  int nslots = 0;     // chunk-wide slots
+  int nslots = 0;     // chunk-wide slots (base + constants + products)
+  int nconst = 0;     // coefficient constants (real path)
   int max_local = 0;  // largest number of sector-local product slots in the chunk
-  uint32_t prog_off = 0, prog_bytes = 0;  // chunk header + slot program in image2
+  int nrec = 0, nlocal = 0;               // monomial records / sector-local products over the chunk (describe)
+  uint32_t tab_words = 0;                 // 16-byte words of sector blocks (real path)
+  uint32_t prog_off = 0, prog_bytes = 0;  // complex path: chunk header + slot programs in image3
   double cost = 0.0;                      // modelled flops per point (load balancing)
 };
 
@@ -128,19 +112,15 @@ struct qmc_tables {
   // device image
   std::vector<uint8_t> image;     // concatenated sector blocks (16-byte aligned each)
   std::vector<uint32_t> secoff;   // [n_sectors + 1] byte offsets
-  // planning image of the real path (host only; empty when lambda > 0)
-  std::vector<uint8_t> image2;
-  std::vector<uint32_t> secoff2;  // [n_sectors + 1] byte offsets of the sector blocks in image2
-  std::vector<uint32_t> secend2;  // [n_sectors] end offsets (a chunk header sits between the sectors of two chunks)
-  std::vector<Qmc2Chunk> chunks;
+  std::vector<Qmc2Chunk> chunks;  // real path (empty when lambda > 0)
   std::vector<double> sec_cost;   // modelled cost per sector (load balancing of the launch)
-  // version 4 tables (real path; same chunks and slot programs as version 2, laid out for the kernel-parameter
-  // constant bank: see qmc_launch.h)
+  // version 4 tables (real path; laid out for the kernel-parameter constant bank: see qmc_launch.h)
   int threads_real = 512;           // threads per block of the real-path kernel: the slot offsets in tab4 / prog4 are
-                                    // premultiplied by it (chosen by qmc_build_image2, see there)
+                                    // premultiplied by it (chosen by qmc_build_tables4, see there)
   std::vector<uint32_t> tab4;       // sector blocks, 32-bit words (4 per 16-byte table word)
   std::vector<uint32_t> secoff4;    // [n_sectors + 1] offsets into tab4 in 16-byte words
   std::vector<std::vector<uint32_t>> prog4;  // per chunk: slot program {a_off, b_off} byte offsets, padded to 16 bytes
+  std::vector<std::vector<double>> const4;   // per chunk: values of the coefficient-constant slots
   double logtab4[128] = {0};        // 64 x {1/c_i, -ln(1/c_i)}
   // version 5 tables (complex path; same chunks and slot programs as version 3, laid out for the constant bank)
   std::vector<uint32_t> tab5, secoff5;             // sector blocks (32-bit words) and their offsets in 16-byte words
@@ -171,9 +151,10 @@ struct qmc_tables {
 };
 
 // builds sectors (+ image) from a graph; returns a qmc_status
-// builds image2 / secoff2 / chunks from `sectors` (real path); returns a qmc_status
-int qmc_build_image2(qmc_tables *t);
+// builds tab4 / secoff4 / prog4 / const4 / chunks from `sectors` (real path); returns a qmc_status.
+// slot_budget, chunk_bytes, threads: 0 = the measured defaults (qmc_tuning in qmc_feynman.h)
+int qmc_build_tables4(qmc_tables *t, int slot_budget, int chunk_bytes, int threads);
 // builds image3 / secoff3 / chunks3 (complex path); returns a qmc_status
-int qmc_build_image3(qmc_tables *t);
+int qmc_build_image3(qmc_tables *t, int slots_r, int slots_c, int chunk_bytes);  // 0 = the measured defaults
 int qmc_build_tables(const qmc_graph *g, const qmc_kinematics *kin, int eps_order, const qmc_options *opt,
                      qmc_tables *out);

@@ -24,20 +24,21 @@ def check(got, want, A, what):
     return int(used_floor.sum())
 
 
-def parity(wl, N, m, z=None, index_range=None, sectors=None, transform=0, shifts=None, eps_order=None):
+def parity(wl, N, m, z=None, index_range=None, sectors=None, transform=0, shifts=None, eps_order=None, kernel=0, **layout):
+    """`layout`: table-layout fields of qmc_options (slot_budget, chunk_bytes, ...); kernel = 1: the generic kernel."""
     eo = wl.eps_order if eps_order is None else eps_order
-    t = q.qmc_prepare(wl, eps_order=eo, lam=wl.lam, transform=transform)   # reads QMC2_* from the environment
+    t = q.qmc_prepare(wl, eps_order=eo, lam=wl.lam, transform=transform, **layout)
     o = Oracle.from_tables(t.export())
     if z is None:
         z = qi.good_vector(N, t.dim)
     sh = qi.splitmix64_shifts(wl.seed, m, t.dim) if shifts is None else shifts
     S, A, cnt = o.integrate(N, z, sh, transform=transform, index_range=index_range, sectors=sectors)
-    r = q.qmc_integrate(t, N, m, z=z, shifts=sh, index_range=index_range, sectors=sectors, per_sector=True)
+    r = q.qmc_integrate(t, N, m, z=z, shifts=sh, index_range=index_range, sectors=sectors, per_sector=True, kernel=kernel)
     assert r.mode_used == 2 and r.shift_sums.shape == S.shape
     nfloor = check(r.shift_sums, S, A, wl.name + " per-sector")
     assert np.array_equal(r.counters, cnt), (r.counters, cnt)
     # fused mode (the throughput mode): per-shift totals over sectors
-    f = q.qmc_integrate(t, N, m, z=z, shifts=sh, index_range=index_range, sectors=sectors, per_sector=False)
+    f = q.qmc_integrate(t, N, m, z=z, shifts=sh, index_range=index_range, sectors=sectors, per_sector=False, kernel=kernel)
     assert f.mode_used == 1
     check(f.shift_totals, S.sum(axis=0), A.sum(axis=0), wl.name + " fused")
     check(r.shift_totals, S.sum(axis=0), A.sum(axis=0), wl.name + " per-sector totals")
@@ -150,10 +151,10 @@ def test_double_box_poles_on_gpu_at_baseline_size():
     assert np.allclose(p.shift_totals, r.shift_totals, rtol=1e-11, atol=1e-13)
 
 
-def test_real_path_tables_chunk_boundaries_slot_budget_and_launch_splits(monkeypatch):
+def test_real_path_tables_chunk_boundaries_slot_budget_and_launch_splits():
     """Real-path tables (version 4: one launch per run of sectors, tables in the kernel parameters): sector ranges that
     straddle chunk boundaries, a slot budget small enough to force sector-local product slots and chunk splits, and
-    chunks larger than what one launch can carry (QMC2_SLOTS / QMC2_CHUNK_BYTES are read by qmc_prepare)."""
+    chunks larger than what one launch can carry (qmc_options.slot_budget / chunk_bytes)."""
     wl = qi.double_box()
     t = q.qmc_prepare(wl)
     desc = t.describe()
@@ -163,20 +164,16 @@ def test_real_path_tables_chunk_boundaries_slot_budget_and_launch_splits(monkeyp
     b = bounds[2]
     parity(wl, 16381, 2, sectors=(b - 3, b + 4))            # straddles a chunk boundary
     parity(wl, 16381, 2, sectors=(bounds[1] - 1, bounds[3] + 1))   # spans a whole chunk plus both neighbours
-    monkeypatch.setenv("QMC2_SLOTS", "26")
-    monkeypatch.setenv("QMC2_CHUNK_BYTES", "3000")
-    t2 = q.qmc_prepare(wl)
+    t2 = q.qmc_prepare(wl, slot_budget=26, chunk_bytes=3000)
     d2 = t2.describe()
-    assert sum(int(l.split("local products ")[1].split(")")[0]) for l in d2.splitlines()[1:]) > 0
+    assert sum(int(l.split("local products ")[1].split(" ")[0]) for l in d2.splitlines()[1:]) > 0
     assert len(d2.splitlines()) > len(desc.splitlines())
-    parity(wl, 16381, 2, sectors=(100, 140))
-    monkeypatch.delenv("QMC2_SLOTS")
-    monkeypatch.setenv("QMC2_CHUNK_BYTES", "60000")       # a chunk now exceeds the 28 KB of tables one launch carries
-    t3 = q.qmc_prepare(wl)
+    parity(wl, 16381, 2, sectors=(100, 140), slot_budget=26, chunk_bytes=3000)
+    t3 = q.qmc_prepare(wl, chunk_bytes=60000)             # a chunk now exceeds the 28 KB of tables one launch carries
     nchunks3 = sum(int(l.split("[")[1].split(",")[0]) < 150 for l in t3.describe().splitlines()[1:])   # chunks meeting [0, 150)
-    r3, f3, *_ = parity(wl, 16381, 2, sectors=(0, 150))
+    r3, f3, *_ = parity(wl, 16381, 2, sectors=(0, 150), chunk_bytes=60000)
     assert f3.kernel_launches - 2 > nchunks3                # the launcher split chunks into several runs
-    monkeypatch.delenv("QMC2_CHUNK_BYTES")
+    parity(wl, 16381, 2, sectors=(100, 140), threads=128)   # the other block size of the kernel
 
 
 def test_async_launch_resident_inputs_and_fetch():
@@ -200,23 +197,19 @@ def test_async_launch_resident_inputs_and_fetch():
     assert r.h2d_bytes < ref.h2d_bytes and r.d2h_bytes > 0 and r.eval_kernel_ms > 0
 
 
-def test_complex_path_tables_launch_splits_and_local_slots(monkeypatch):
+def test_complex_path_tables_launch_splits_and_local_slots():
     """Complex-path tables (version 5): small chunks (several launches per step, sector ranges that straddle them) and
-    slot budgets small enough to force sector-local real and complex product slots (QMC3_* are read by qmc_prepare)."""
+    slot budgets small enough to force sector-local real and complex product slots (qmc_options.chunk_bytes,
+    slot_budget_cplx_real, slot_budget_cplx)."""
     wl = qi.nonplanar_vertex()
     t = q.qmc_prepare(wl, lam=wl.lam)
     n0 = len(t.describe().splitlines())
-    monkeypatch.setenv("QMC3_CHUNK_BYTES", "6000")
-    monkeypatch.setenv("QMC3_SLOTS_R", "26")
-    monkeypatch.setenv("QMC3_SLOTS_C", "10")
-    t2 = q.qmc_prepare(wl, lam=wl.lam)
+    lay = dict(chunk_bytes=6000, slot_budget_cplx_real=26, slot_budget_cplx=10)
+    t2 = q.qmc_prepare(wl, lam=wl.lam, **lay)
     d2 = t2.describe()
     assert len(d2.splitlines()) > n0 and "local) complex slots 10 (+" in d2 and "(+0 local) tables" not in d2.splitlines()[1]
-    r, f, *_ = parity(wl, 16381, 2, sectors=(3, 31))
+    r, f, *_ = parity(wl, 16381, 2, sectors=(3, 31), **lay)
     assert f.kernel_launches - 2 >= 3
-    monkeypatch.delenv("QMC3_CHUNK_BYTES")
-    monkeypatch.delenv("QMC3_SLOTS_R")
-    monkeypatch.delenv("QMC3_SLOTS_C")
 
 
 def test_kinematic_scan_points_of_the_papers_box():
