@@ -80,6 +80,8 @@ typedef struct {
   int32_t chunk_bytes;       /* target bytes of sector tables per chunk (both paths) */
   int32_t threads;           /* real path: threads per block, 128 or 512 (default: chosen from the tables) */
   int32_t slot_budget_cplx_real, slot_budget_cplx; /* complex path: real / complex slots per chunk */
+  int32_t dense_template;    /* real path: dense-position template of the sector tables, 1 = lean, 2 = two-loop sized
+                                (default: the one with the lower modelled cost) */
 } qmc_options;
 
 typedef struct qmc_tables qmc_tables; /* opaque sector tables (Eqs. 7-9) */

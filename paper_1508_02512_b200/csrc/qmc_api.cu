@@ -288,7 +288,7 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
   }
   const int nitems = (int)runs.size();
   int bps = 0;
-  CUDA_OK(qmc4_kernel_prepare(n, t->L, t->kmax, T, smem, &bps));
+  CUDA_OK(qmc4_kernel_prepare(n, t->L, t->kmax, T, t->tpl_real, smem, &bps));
   if (bps < 1) return QMC_ECUDA;
   const int waves = waves_opt > 0 ? waves_opt : 16;
   const long long max_slices_pts = std::max<long long>(1, (long long)((icount + T - 1) / T));
@@ -335,6 +335,7 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
   p.dN = (double)N;
   p.invN = 1.0 / (double)N;
   p.sync_every = 4;  // measured on B200 (kernels): a block barrier every fourth point
+  if (const char *e = std::getenv("QMC_TMP_SYNC")) p.sync_every = (uint32_t)std::atoi(e);  // TEMPORARY experiment knob
   cudaEventRecord(static_cast<cudaEvent_t>(t->ev0), st);
   if (nstreams) {
     cudaEventRecord(static_cast<cudaEvent_t>(t->side_events[nstreams]), st);
@@ -353,10 +354,10 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
     p.max_nslots = (uint32_t)(c.nslots + c.max_local);
     p.nconst = (uint32_t)c.nconst;
     for (int q = 0; q < c.nconst; ++q) p.cval[q] = t->const4[r.chunk][q];
-    p.nprog = (uint32_t)(c.nslots - (3 * n + 2 + c.nconst));
+    p.nprog = (uint32_t)(c.nslots - (2 * n + 2 + c.nconst));
     p.prog_word = 0;
     p.sec_word = (uint32_t)(pg.size() / 4);
-    p.first_prod_off = (uint32_t)(3 * n + 2 + c.nconst) * T * 8u;
+    p.first_prod_off = (uint32_t)(2 * n + 2 + c.nconst) * T * 8u;
     p.local0_off = (uint32_t)c.nslots * T * 8u;
     uint32_t *tw = reinterpret_cast<uint32_t *>(p.tab);
     std::memcpy(tw, pg.data(), pg.size() * 4);
@@ -364,16 +365,19 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
     std::memcpy(tw + pg.size(), t->tab4.data() + w0 * 4, (w1 - w0) * 16);
     {  // evaluation order: by number of singular variables (stable)
       int k = 0;
-      for (int ns = 0; ns <= QMC_MAXSING; ++ns)
+      for (int ns = 0; ns <= QMC_MAXSING; ++ns) {
+        p.nsb[ns] = k;
         for (int s = r.a; s < r.b; ++s)
           if (t->sectors[s].nsing == ns) {
             p.secw[k] = (uint16_t)(p.sec_word + (t->secoff4[s] - w0));
             p.secrow[k] = (uint16_t)(s - r.a);
             ++k;
           }
+      }
+      p.nsb[QMC_MAXSING + 1] = k;
     }
     cudaStream_t ls = nstreams ? static_cast<cudaStream_t>(t->side_streams[i % nstreams]) : st;
-    ce = qmc4_kernel_launch(n, t->L, t->kmax, T, dim3((unsigned)nsl[i], (unsigned)m), r.smem, ls, p);
+    ce = qmc4_kernel_launch(n, t->L, t->kmax, T, t->tpl_real, dim3((unsigned)nsl[i], (unsigned)m), r.smem, ls, p);
     *h2d += offsetof(Qmc4Launch, tab) + pg.size() * 4 + (w1 - w0) * 16;  // the tables travel with the launch
   }
   if (nstreams)
@@ -1029,15 +1033,15 @@ int qmc_tables_describe(const qmc_tables *t, char *buf, size_t len) {
   if (!t || !buf || len < 1) return QMC_EINVAL;
   std::string o;
   char line[256];
-  std::snprintf(line, sizeof line, "sectors %d dim %d loops %d orders %d..%d lambda %g generic image %zu B real-path tables %zu B chunks %zu threads %d\n",
+  std::snprintf(line, sizeof line, "sectors %d dim %d loops %d orders %d..%d lambda %g generic image %zu B real-path tables %zu B chunks %zu threads %d template %d\n",
                 (int)t->sectors.size(), t->n, t->L, t->kmin, t->kmax, t->lambda, t->image.size(), t->tab4.size() * 4, t->chunks.size(),
-                t->threads_real);
+                t->threads_real, t->tpl_real);
   o += line;
   for (size_t c = 0; c < t->chunks.size(); ++c) {
     const Qmc2Chunk &ch = t->chunks[c];
-    std::snprintf(line, sizeof line, "chunk %zu: sectors [%d,%d) slots %d (constants %d, products %d) tables %u B records %d local products %d (max %d) cost %.0f\n", c,
-                  ch.sec_begin, ch.sec_end, ch.nslots, ch.nconst, ch.nslots - (3 * t->n + 2 + ch.nconst), ch.tab_words * 16u, ch.nrec,
-                  ch.nlocal, ch.max_local, ch.cost);
+    std::snprintf(line, sizeof line, "chunk %zu: sectors [%d,%d) slots %d (constants %d, products %d) tables %u B records %d (beyond the dense positions %d) local products %d (max local slots %d) cost %.0f\n", c,
+                  ch.sec_begin, ch.sec_end, ch.nslots, ch.nconst, ch.nslots - (2 * t->n + 2 + ch.nconst), ch.tab_words * 16u, ch.nrec,
+                  ch.noverflow, ch.nlocal, ch.max_local, ch.cost);
     o += line;
   }
   for (size_t c = 0; c < t->chunks3.size(); ++c) {  // complex path

@@ -40,7 +40,7 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
   double per_point = n * ((cplx ? F_DIV : 5.0) + 2.0 + 4.0 + 4.0 + 18.0 + 6.0);
   if (!cplx)  // the chunks' product slots, once per point and chunk touched
     for (const Qmc2Chunk &c : t->chunks)
-      if (c.sec_end > sb && c.sec_begin < se) per_point += (double)(c.nslots - (3 * n + 2 + c.nconst));
+      if (c.sec_end > sb && c.sec_begin < se) per_point += (double)(c.nslots - (2 * n + 2 + c.nconst));
   double per_sectors = 0.0;
   int64_t ncorners = 0;
   const int eU = std::abs(t->aU0), eF = std::abs(t->aF0);
@@ -73,7 +73,8 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
         if (s.alpha[j] != -1 && s.beta[j]) ++nL0;
       const int nlocal = t->tab4.empty() ? 0 : (int)((t->tab4[(size_t)t->secoff4[si] * 4] >> 16) & 255u);
       f = 1.0 * nlocal;                        // sector-local product slots
-      f += 3.0 + 2.0 * nL0;                    // G0' = c * slot * slot, times the weight; L0 = constant + sum beta_j ln t_j (FMAs)
+      f += 3.0 + 2.0 * nL0;                    // G0 = c * slot * slot, times the weight; L0 = constant + sum beta_j ln t_j (FMAs)
+      if (ns > 0) f += (ns - 1) + F_RCP2 + 1.0;  // 1 / prod t_k of the singular variables, times G0
       {
         int pos[QMC_MAXDIM], k = 0;
         for (int j = 0; j < n; ++j) pos[j] = s.alpha[j] == -1 ? k++ : -1;

@@ -2,12 +2,16 @@
 // Host only.  Layout: qmc_launch.h; rationale: DESIGN.md "Data layout".
 //
 // Every thread keeps, per lattice point, a column of per-point values ("slots") in shared memory:
-//   [0,n) t_j | [n,2n) ln t_j | [2n,3n) 1/t_j | 3n: 1.0 | 3n+1: 0.0 | coefficient constants | chunk products | sector-local products
+//   [0,n) t_j | [n,2n) ln t_j | 2n: 1.0 | 2n+1: 0.0 | coefficient constants | chunk products | sector-local products
 // A monomial c * prod t_j^e_j is a multiset of FACTORS: the variables repeated by exponent and -- when c != 1 -- one
 // symbol for the constant c, which owns a slot of its own.  A byte-pair-encoding style pass over the chunk's monomials
 // (most frequent pair of factors first) turns pairs of factors into product slots, computed once per lattice point,
 // until every monomial is a product of at most two slots.  A monomial is then ONE 8-byte record {u32 off0, u32 off1}:
 // value = slot[off0] * slot[off1], accumulated with a single FMA -- the coefficient travels inside a slot.
+// The records of a sector sit at DENSE POSITIONS: group g of polynomial q owns qmc4_cap(nsing, q, popcount g) positions
+// (qmc_tables.h), which the kernel evaluates in straight-line code.  A group with more monomials than positions sums the
+// overflow into a sector-local slot first ("fused" local entries slot = a*b + c*d; further monomials chain slot = slot*1 +
+// c*d), and its last position reads that slot.
 // To keep the constants few, every sector's U^ and F^ are divided by their most frequent |coefficient| c_U, c_F
 // (U^ = c_U U', F^ = c_F F'): W picks up the factor c_U^aU0 c_F^aF0 (folded into the coefficient of G0) and Lambda the
 // constant aU1 ln c_U + aF1 ln c_F (folded into L0).  On the double box every coefficient of U' is 1 and F' has one
@@ -64,9 +68,9 @@ struct ChunkConsts {
   }
 };
 
-// factors of all monomials of sectors [s0, s1), in the order [G0', U^ ..., F^ ...] per sector.
-// G0' = prod_{regular j} t_j^alpha_j * prod_{singular j} 1/t_j  (the 1/t_j of the plus-distribution terms, Eq. 12, factored out
-// of the fold: qmc_fold.cuh)
+// factors of all monomials of sectors [s0, s1), in the order [G0, U^ ..., F^ ...] per sector.
+// G0 = prod_{regular j} t_j^alpha_j  (the kernel multiplies the 1/t_j of the singular variables, Eq. 12, factored out of the
+// fold, qmc_fold.cuh, onto it)
 bool collect(const qmc_tables *t, int s0, int s1, ChunkPlan &pl, ChunkConsts &cc, std::vector<double> &cU, std::vector<double> &cF) {
   pl.mono.clear();
   cc.val.clear();
@@ -76,10 +80,8 @@ bool collect(const qmc_tables *t, int s0, int s1, ChunkPlan &pl, ChunkConsts &cc
   for (int si = s0; si < s1; ++si) {
     const QmcSector &s = t->sectors[si];
     Factors g;
-    for (int j = 0; j < n; ++j) {
-      if (s.alpha[j] == -1) g.push_back((uint8_t)(2 * n + j));
+    for (int j = 0; j < n; ++j)
       for (int q = 0; q < s.alpha[j]; ++q) g.push_back((uint8_t)j);
-    }
     std::sort(g.begin(), g.end());
     pl.mono.push_back(g);
     const double cu = common_coefficient(s.U), cf = common_coefficient(s.F);
@@ -92,7 +94,7 @@ bool collect(const qmc_tables *t, int s0, int s1, ChunkPlan &pl, ChunkConsts &cc
         if (c != 1.0) {
           const int id = cc.id(c);
           if (id >= QMC4_MAXCONST) return false;
-          f.push_back((uint8_t)(3 * n + 2 + id));
+          f.push_back((uint8_t)(2 * n + 2 + id));
         }
         std::sort(f.begin(), f.end());
         pl.mono.push_back(f);
@@ -128,7 +130,7 @@ static void build_logtab4(double *tab) {
   }
 }
 
-int qmc_build_tables4(qmc_tables *t, int slot_budget, int chunk_bytes_opt, int threads_opt) {
+int qmc_build_tables4(qmc_tables *t, int slot_budget, int chunk_bytes_opt, int threads_opt, int tpl_opt) {
   build_logtab4(t->logtab4);
   t->tab4.clear();
   t->secoff4.clear();
@@ -143,13 +145,40 @@ int qmc_build_tables4(qmc_tables *t, int slot_budget, int chunk_bytes_opt, int t
     // short paths prefer the small blocks.
     int big = 0;
     for (const QmcSector &s : t->sectors) big += s.nsing >= 3;
-    t->threads_real = 2 * big >= (int)t->sectors.size() ? 512 : 128;
-    if (threads_opt == 128 || threads_opt == 512) t->threads_real = threads_opt;
+    t->threads_real = 2 * big >= (int)t->sectors.size() ? QMC4_TBIG : 128;
+    if (threads_opt == 128) t->threads_real = 128;
+    if (threads_opt == 512) t->threads_real = QMC4_TBIG;
   }
   const uint32_t T4 = (uint32_t)t->threads_real;
   const int n = t->n, nsec = (int)t->sectors.size();
   if (t->lambda > 0.0 || nsec == 0) return QMC_OK;
-  if (3 * n + 2 >= QMC2_MAXSLOTS) return QMC_EUNSUPPORTED;
+  {
+    // dense-position template (qmc_tables.h): the one with the lower modelled instruction count over all sectors --
+    // 3.5 per position (its share of the table load, two slot loads, one multiply-add), 13 per monomial beyond a group's
+    // positions (a fused sector-local entry)
+    double cost_tpl[2] = {0.0, 0.0};
+    for (const QmcSector &s : t->sectors) {
+      int pos_of[QMC_MAXDIM], k = 0;
+      for (int j = 0; j < n; ++j) pos_of[j] = s.alpha[j] == -1 ? k++ : -1;
+      for (int which = 0; which < 2; ++which) {
+        int cnt[1 << QMC_MAXSING] = {0};
+        for (const QmcMono &m : (which ? s.F : s.U)) {
+          int g = 0;
+          for (int j = 0; j < n; ++j)
+            if (m.e[j] && pos_of[j] >= 0) g |= 1 << pos_of[j];
+          ++cnt[g];
+        }
+        for (int tpl = 0; tpl < 2; ++tpl)
+          for (int g = 0; g < (1 << s.nsing); ++g) {
+            const int cap = qmc4_cap(tpl, s.nsing, which, qmc4_popc(g));
+            cost_tpl[tpl] += 3.5 * cap + 13.0 * std::max(0, cnt[g] - cap);
+          }
+      }
+    }
+    t->tpl_real = cost_tpl[1] < cost_tpl[0] ? 1 : 0;
+    if (tpl_opt == 1 || tpl_opt == 2) t->tpl_real = tpl_opt - 1;
+  }
+  if (2 * n + 2 >= QMC2_MAXSLOTS) return QMC_EUNSUPPORTED;
 
   // ---- chunk boundaries: contiguous ranges of about equal modelled cost, about chunk_bytes of tables each ------
   std::vector<double> cost(nsec);
@@ -159,10 +188,11 @@ int qmc_build_tables4(qmc_tables *t, int slot_budget, int chunk_bytes_opt, int t
     cost[i] = sector_cost(s, t->kmax);
     t->sec_cost.push_back(cost[i]);
     total_cost += cost[i];
-    total_bytes += 16.0 * (11 + n) + 8.0 * (s.U.size() + s.F.size() + (2 << s.nsing) + 2);
+    total_bytes += 16.0 * (11 + n) + 8.0 * qmc4_pos(t->tpl_real, s.nsing, 1, 1 << s.nsing);
   }
   // 40 chunk-wide slots (+ the coefficient constants) + up to 8 sector-local ones: 49 columns of 8 T bytes = 196 KB at
-  // T = 512 (one block per SM); measured on B200 (cfg4): 32 / 36 / 40 slots -> 232 / 211 / 205 ms per step
+  // T = 512 (one block per SM, and room for the accumulators of the per-sector mode); the more slots, the fewer
+  // sector-local products and chunks (measured on B200, cfg4)
   const int max_slots_base = slot_budget > 0 ? slot_budget : 40;
   const double chunk_bytes = chunk_bytes_opt > 0 ? std::max(1000.0, (double)chunk_bytes_opt) : 24000.0;
   int nch = std::max(1, (int)(total_bytes / chunk_bytes + 0.999));
@@ -188,7 +218,7 @@ int qmc_build_tables4(qmc_tables *t, int slot_budget, int chunk_bytes_opt, int t
     std::vector<double> cU, cF;
     if (!collect(t, s0, s1, pl, cc, cU, cF)) return QMC_EUNSUPPORTED;
     const int nconst = (int)cc.val.size();
-    const int first_prod = 3 * n + 2 + nconst;
+    const int first_prod = 2 * n + 2 + nconst;
     const int max_slots = std::min(QMC2_MAXSLOTS - QMC2_MAXLOCAL, std::max(max_slots_base + std::min(nconst, 6), first_prod + 1));
     plan_chunk(pl, first_prod, max_slots);
     Qmc2Chunk ch;
@@ -203,7 +233,7 @@ int qmc_build_tables4(qmc_tables *t, int slot_budget, int chunk_bytes_opt, int t
     }
     pad4(prog4);
     const size_t tab4_mark = t->tab4.size();
-    const uint32_t ONE = (uint32_t)(3 * n) * T4 * 8u, ZERO = (uint32_t)(3 * n + 1) * T4 * 8u;
+    const uint32_t ONE = (uint32_t)(2 * n) * T4 * 8u, ZERO = (uint32_t)(2 * n + 1) * T4 * 8u;
     size_t mi = 0;  // index into pl.mono, same order as collect()
     auto put_rec = [&](std::vector<uint32_t> &v, const Factors &f) {
       v.push_back(f.size() > 0 ? (uint32_t)f[0] * T4 * 8u : ONE);
@@ -245,11 +275,11 @@ int qmc_build_tables4(qmc_tables *t, int slot_budget, int chunk_bytes_opt, int t
           invbeta[k] = 1.0 / (double)s.beta[j];
           pos_of[j] = k++;
         }
-      const int nc = 1 << s.nsing;
-      // group-sorted monomials (qmc_build_tables sorted them); counts per group
-      int cntU[1 << QMC_MAXSING] = {0}, cntF[1 << QMC_MAXSING] = {0};
+      for (; k < QMC_MAXSING; ++k) sing_ln[k] = sing_t[k] = ONE;
+      const int ns = s.nsing, nc = 1 << ns;
+      // monomials per group (qmc_build_tables sorted them by group)
+      std::vector<const Factors *> grp[2][1 << QMC_MAXSING];
       const Factors &g0f = pl.mono[mi++];
-      std::vector<const Factors *> recs;  // U^ then F^, group-sorted
       for (int which = 0; which < 2; ++which) {
         int gprev = 0;
         for (const QmcMono &m : (which ? s.F : s.U)) {
@@ -258,46 +288,76 @@ int qmc_build_tables4(qmc_tables *t, int slot_budget, int chunk_bytes_opt, int t
             if (m.e[j] && pos_of[j] >= 0) g |= 1 << pos_of[j];
           if (g < gprev) return QMC_EINVAL;  // monomials must arrive sorted by group
           gprev = g;
-          int &c = (which ? cntF : cntU)[g];
-          if (c == 255) return QMC_EUNSUPPORTED;
-          ++c;
-          recs.push_back(&pl.mono[mi++]);
+          grp[which][g].push_back(&pl.mono[mi++]);
         }
       }
-      ch.nrec += (int)recs.size();
+      // dense positions; overflowing groups sum their surplus into a sector-local slot (fused entries)
+      struct Fused { uint32_t a, b, c, d, dst; };
+      std::vector<Fused> fused;
+      std::vector<uint32_t> posrec;  // {off0, off1} per position
+      auto off_of = [&](const Factors &f, int i) { return (int)f.size() > i ? (uint32_t)f[i] * T4 * 8u : ONE; };
+      int nlocal_slots = (int)local.size();
+      for (int which = 0; which < 2 && !too_many_locals; ++which)
+        for (int g = 0; g < nc; ++g) {
+          const int cap = qmc4_cap(t->tpl_real, ns, which, qmc4_popc(g));
+          const std::vector<const Factors *> &R = grp[which][g];
+          const int cnt = (int)R.size();
+          ch.nrec += cnt;
+          if (cap < 1) return QMC_EUNSUPPORTED;
+          if (cnt <= cap) {
+            for (int q = 0; q < cap; ++q) {
+              posrec.push_back(q < cnt ? off_of(*R[q], 0) : ZERO);
+              posrec.push_back(q < cnt ? off_of(*R[q], 1) : ZERO);
+            }
+          } else {
+            for (int q = 0; q < cap - 1; ++q) {
+              posrec.push_back(off_of(*R[q], 0));
+              posrec.push_back(off_of(*R[q], 1));
+            }
+            if (nlocal_slots >= QMC2_MAXLOCAL || pl.nslots + nlocal_slots >= QMC2_MAXSLOTS) {
+              too_many_locals = true;
+              break;
+            }
+            const uint32_t dst = (uint32_t)(pl.nslots + nlocal_slots) * T4 * 8u;
+            ++nlocal_slots;
+            int q = cap - 1;
+            fused.push_back({off_of(*R[q], 0), off_of(*R[q], 1), off_of(*R[q + 1], 0), off_of(*R[q + 1], 1), dst});
+            for (q += 2; q < cnt; ++q) fused.push_back({dst, ONE, off_of(*R[q], 0), off_of(*R[q], 1), dst});
+            posrec.push_back(dst);
+            posrec.push_back(ONE);
+            ch.noverflow += cnt - cap;
+          }
+        }
+      if (too_many_locals) break;
+      if (posrec.size() % 4) {  // pad to a whole 16-byte word
+        posrec.push_back(ONE);
+        posrec.push_back(ONE);
+      }
       ch.nlocal += (int)local.size();
-      ch.max_local = std::max(ch.max_local, (int)local.size());
+      ch.max_local = std::max(ch.max_local, nlocal_slots);
       // ---- the sector block (layout: qmc_launch.h) ----
       std::vector<uint32_t> &v = t->tab4;
       t->secoff4[si] = (uint32_t)(v.size() / 4);
       const size_t b0 = v.size();
-      int nL0 = 0;
-      for (int j = 0; j < n; ++j)
-        if (s.alpha[j] != -1 && s.beta[j] != 0) ++nL0;
+      const int nL0 = n - ns;  // one record per regular variable
       const uint32_t nlw = (uint32_t)((local.size() + 1) / 2);
-      put32(v, (uint32_t)s.nsing | ((uint32_t)nL0 << 8) | ((uint32_t)local.size() << 16));
-      put32(v, 0);                              // size of the block in words (patched below)
-      put32(v, 11 + (uint32_t)nL0 + nlw);       // first dense record
+      put32(v, (uint32_t)ns | ((uint32_t)nL0 << 8) | ((uint32_t)local.size() << 16) | ((uint32_t)fused.size() << 24));
+      put32(v, 0);                                                    // size of the block in words (patched below)
+      put32(v, 9 + (uint32_t)nL0 + nlw + 2u * (uint32_t)fused.size());  // first dense position
       put32(v, 0);
       for (int q = 0; q < QMC_MAXSING; ++q) put32(v, sing_ln[q]);
       for (int q = 0; q < QMC_MAXSING; ++q) put32(v, sing_t[q]);
       for (int q = 0; q < QMC_MAXSING; ++q) putf64(v, invbeta[q]);
       for (int q = 0; q < QMC_MAXSING; ++q) putf64(v, beta[q]);
       const double cu = cU[si - s0], cf = cF[si - s0];
-      putf64(v, ipow(cu, t->aU0) * ipow(cf, t->aF0));  // w7: coefficient of G0', then its two slots
-      put_rec(v, g0f);
+      putf64(v, ipow(cu, t->aU0) * ipow(cf, t->aF0));  // w7: coefficient of G0, then its two slots
+      v.push_back(off_of(g0f, 0));
+      v.push_back(off_of(g0f, 1));
       putf64(v, t->aU1 * std::log(cu) + t->aF1 * std::log(cf));  // w8: constant of L0
       put32(v, 0);
       put32(v, 0);
-      uint8_t extraU[16] = {0}, extraF[16] = {0};
-      for (int g = 0; g < nc; ++g) {
-        extraU[g] = cntU[g] ? (uint8_t)(cntU[g] - 1) : 0;
-        extraF[g] = cntF[g] ? (uint8_t)(cntF[g] - 1) : 0;
-      }
-      for (int q = 0; q < 4; ++q) put32(v, extraU[4 * q] | (extraU[4 * q + 1] << 8) | (extraU[4 * q + 2] << 16) | ((uint32_t)extraU[4 * q + 3] << 24));
-      for (int q = 0; q < 4; ++q) put32(v, extraF[4 * q] | (extraF[4 * q + 1] << 8) | (extraF[4 * q + 2] << 16) | ((uint32_t)extraF[4 * q + 3] << 24));
-      for (int j = 0; j < n; ++j)  // L0 = constant + sum over regular variables of beta_j ln t_j
-        if (s.alpha[j] != -1 && s.beta[j] != 0) {
+      for (int j = 0; j < n; ++j)  // w9..: L0 = constant + sum over regular variables of beta_j ln t_j
+        if (s.alpha[j] != -1) {
           putf64(v, (double)s.beta[j]);
           put32(v, (uint32_t)(n + j) * T4 * 8u);
           put32(v, 0);
@@ -307,27 +367,11 @@ int qmc_build_tables4(qmc_tables *t, int slot_budget, int chunk_bytes_opt, int t
         put32(v, (uint32_t)pr.second * T4 * 8u);
       }
       pad4(v);
-      // dense first records (one per group; an empty group reads the 0.0 slot), then the extra records group by group
-      std::vector<const Factors *> extra;
-      size_t ri = 0;
-      for (int which = 0; which < 2; ++which)
-        for (int g = 0; g < nc; ++g) {
-          const int cnt = (which ? cntF : cntU)[g];
-          if (cnt) {
-            put_rec(v, *recs[ri]);
-          } else {
-            v.push_back(ZERO);
-            v.push_back(ZERO);
-          }
-          for (int q = 1; q < cnt; ++q) extra.push_back(recs[ri + q]);
-          ri += cnt;
-        }
-      for (const Factors *f : extra) put_rec(v, *f);
-      for (int q = 0; q < 2; ++q) {  // sentinels: the kernel requests operands one record and offsets two records past the last
-        v.push_back(ONE);
-        v.push_back(ONE);
+      for (const Fused &fu : fused) {
+        put32(v, fu.a); put32(v, fu.b); put32(v, fu.c); put32(v, fu.d);
+        put32(v, fu.dst); put32(v, 0); put32(v, 0); put32(v, 0);
       }
-      pad4(v);
+      for (uint32_t x : posrec) v.push_back(x);
       v[b0 + 1] = (uint32_t)((v.size() - b0) / 4);
     }
     if (too_many_locals) {  // split the range in two and plan again

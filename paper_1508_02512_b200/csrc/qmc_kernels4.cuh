@@ -1,7 +1,7 @@
 // Evaluation kernel of the real (Euclidean) path, "version 4", sm_100a.  Steps S1-S7 of DESIGN.md.
 //
 // One thread = one lattice point at a time.  Per point the thread fills its column of a shared-memory slot table
-// (t_j, ln t_j, 1/t_j, 1, 0, coefficient constants, then the chunk's product slots chosen by the byte-pair-encoding pass of
+// (t_j, ln t_j, 1, 0, coefficient constants, then the chunk's product slots chosen by the byte-pair-encoding pass of
 // qmc_image4.cpp); a monomial of U^ or F^ is then ONE 8-byte record: slot * slot, accumulated with one FMA (the
 // coefficient lives in a slot).  Per sector with s singular variables:
 //   1. partial sums of U^, F^ per group (= set of singular variables a monomial depends on), subset sums -> the values
@@ -13,10 +13,10 @@
 //      multiplies the weight once per sector.
 // The chunk's slot program and the sector tables are part of the KERNEL PARAMETER BLOCK (constant bank 0, layout in
 // qmc_launch.h): a record is one uniform load (LDCU.64; two records per LDCU.128 in the dense part), 2 LDS [R + UR] and one
-// DFMA; trip counts are uniform; the FIRST record of every group sits in a dense array with a compile-time destination
-// register (2^nsing independent load/multiply chains in one basic block), and all further records are one stream walked
-// with the next operands in flight.  The logarithm table is 64 entries x 8 interleaved copies (lane & 7 picks the copy):
-// every lookup is a conflict-free LDS.128.
+// DFMA; the records of a sector sit at DENSE POSITIONS (a fixed number per group, qmc_tables.h) with compile-time
+// destination registers: one basic block of independent load / multiply-add chains without a loop or a branch; what a
+// group has beyond its positions was summed into a sector-local slot before (fused local entries).  The logarithm table
+// is 64 entries x 8 interleaved copies (lane & 7 picks the copy): every lookup is a conflict-free LDS.128.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -99,7 +99,7 @@ __device__ __forceinline__ double block_sum_t(double v, double *scratch /*[T / 3
   if (wid == 0) {
     r = (lane < T / 32) ? scratch[lane] : 0.0;
 #pragma unroll
-    for (int o = (T / 64); o > 0; o >>= 1) r += __shfl_down_sync(0xffffffffu, r, o);
+    for (int o = (T > 512 ? 16 : T / 64); o > 0; o >>= 1) r += __shfl_down_sync(0xffffffffu, r, o);
   }
   return r;
 }
@@ -115,6 +115,31 @@ __device__ __forceinline__ double rec_val(const uint4 r, const unsigned char *__
 __device__ __forceinline__ double rec_fma(const uint4 r, const unsigned char *__restrict__ sl, double acc) {
   return fma(__hiloint2double((int)r.y, (int)r.x), slot_at(sl, r.z) * slot_at(sl, r.w), acc);
 }
+
+// dense positions of group G (and, recursively, of the groups after it) of polynomial WHICH: P[G] = sum over the group's
+// qmc4_cap positions of slot * slot; `fr` = first dense position of the sector (uniform), record index compile-time
+template <int TPL, int NS, int WHICH, int G>
+struct Dense4 {
+  static __device__ __forceinline__ void eval(const unsigned char *__restrict__ fr, const unsigned char *__restrict__ sl,
+                                              double (&P)[1 << NS]) {
+    constexpr int CAP = qmc4_cap(TPL, NS, WHICH, qmc4_popc(G)), P0 = qmc4_pos(TPL, NS, WHICH, G);
+    // a group with singular variable 0 starts from the sum of the group without it: the first level of the subset sums
+    // (P[X] += P[X ^ 1]) rides on the first multiply-add instead of costing an addition of its own
+    double acc = (G & 1) ? P[G ^ 1] : 0.0;
+#pragma unroll
+    for (int k = 0; k < CAP; ++k) {
+      const uint4 q = *reinterpret_cast<const uint4 *>(fr + ((P0 + k) >> 1) * 16);
+      const uint32_t oa = ((P0 + k) & 1) ? q.z : q.x, ob = ((P0 + k) & 1) ? q.w : q.y;
+      acc = (k == 0 && !(G & 1)) ? slot_at(sl, oa) * slot_at(sl, ob) : fma(slot_at(sl, oa), slot_at(sl, ob), acc);
+    }
+    P[G] = acc;
+    Dense4<TPL, NS, WHICH, G + 1>::eval(fr, sl, P);
+  }
+};
+template <int TPL, int NS, int WHICH>
+struct Dense4<TPL, NS, WHICH, 1 << NS> {
+  static __device__ __forceinline__ void eval(const unsigned char *__restrict__, const unsigned char *__restrict__, double (&)[1 << NS]) {}
+};
 
 // W = U^aU0 F^aF0 and the argument U^aU1 F^aF1 of the logarithm (aU1 > 0 > aF1) from U, 1/F (and 1/U when aU0 < 0), with
 // a = U / F shared between the two where both want it (double box: a, a^2, a^2 U, (1/F)^2, a (1/F)^2: five products)
@@ -139,7 +164,7 @@ __device__ __forceinline__ void corner_powers(double U, double F, double rF, dou
 
 // one sector at one point: out[i] = coefficient of eps^(i - NS) of the subtracted integrand without the weight w and
 // without the sector's common factor G0' (returned in g0).  `o` = word offset of the sector block in p.tab (uniform).
-template <int NDIM, int L, int NS, int KMAX, int T>
+template <int NDIM, int L, int NS, int KMAX, int T, int TPL>
 __device__ __forceinline__ bool sector4(const Qmc4Launch &p, const uint32_t o, unsigned char *__restrict__ sl,
                                         const double2 *__restrict__ tabq, double (&out)[KMAX + NS + 1], double &g0) {
   unsigned worst = 0;  // fast_log_unchecked
@@ -147,83 +172,54 @@ __device__ __forceinline__ bool sector4(const Qmc4Launch &p, const uint32_t o, u
   typedef Expo<NDIM, L> E;
   const unsigned char *tb = reinterpret_cast<const unsigned char *>(p.tab);
   const uint4 h0 = p.tab[o];
-  const uint32_t nL0 = (h0.x >> 8) & 255u, nlocal = (h0.x >> 16) & 255u;
+  constexpr uint32_t nL0 = NDIM - NS;  // one record per regular variable (beta_j = 0 where ln t_j does not enter)
+  const uint32_t nlocal = (h0.x >> 16) & 255u, nfused = h0.x >> 24;
   {  // sector-local products: slot[local0 + i] = slot[a] * slot[b]
-    const uint32_t lw = o + 11 + nL0;
+    const uint32_t lw = o + 9 + nL0;
 #pragma unroll 1
     for (uint32_t i = 0; i < nlocal; i += 2) {
       const uint4 pw = p.tab[lw + (i >> 1)];
       *reinterpret_cast<double *>(sl + p.local0_off + i * (T * 8)) = slot_at(sl, pw.x) * slot_at(sl, pw.y);
       if (i + 1 < nlocal) *reinterpret_cast<double *>(sl + p.local0_off + (i + 1) * (T * 8)) = slot_at(sl, pw.z) * slot_at(sl, pw.w);
     }
+    // fused entries: slot[dst] = slot[a] * slot[b] + slot[c] * slot[d] -- the monomials of a group beyond its dense positions
+    const uint32_t fw = lw + ((nlocal + 1) >> 1);
+#pragma unroll 1
+    for (uint32_t i = 0; i < nfused; ++i) {
+      const uint4 e = p.tab[fw + 2 * i];
+      const uint32_t dst = p.tab[fw + 2 * i + 1].x;
+      *reinterpret_cast<double *>(sl + dst) = fma(slot_at(sl, e.x), slot_at(sl, e.y), slot_at(sl, e.z) * slot_at(sl, e.w));
+    }
   }
   {
     const uint4 g = p.tab[o + 7];
     g0 = u2d(g.x, g.y) * (slot_at(sl, g.z) * slot_at(sl, g.w));
+    if (NS > 0) {  // the 1/t_k of the singular variables (Eq. 12), factored out of the fold: one reciprocal of their product
+      const uint4 st = p.tab[o + 2];
+      const uint32_t tw[4] = {st.x, st.y, st.z, st.w};
+      double pt = slot_at(sl, tw[0]);
+#pragma unroll
+      for (int k = 1; k < NS; ++k) pt *= slot_at(sl, tw[k]);
+      g0 *= fast_rcp(pt);
+    }
   }
   double L0 = u2d(p.tab[o + 8].x, p.tab[o + 8].y);
-#pragma unroll 2
+#pragma unroll
   for (uint32_t i = 0; i < nL0; ++i) {
-    const uint4 r = p.tab[o + 11 + i];
+    const uint4 r = p.tab[o + 9 + i];
     L0 = fma(u2d(r.x, r.y), slot_at(sl, r.z), L0);
   }
   Ctx2<NS, K> c;
   {
-    // first record of every group (dense, compile-time destination), then the extra records group by group;
+    // dense positions (qmc_tables.h: qmc4_cap): every group of U^ and F^ owns a fixed number of records with compile-time
+    // destination registers -- one basic block of independent load / multiply-add chains, no loop, no branch;
     // subset sums: P[X] = value with the singular variables outside X set to zero
     double PU[NC], PF[NC];
     const unsigned char *fr = tb + (o + h0.z) * 16u;
-    if (NC == 1) {
-      const uint4 q = *reinterpret_cast<const uint4 *>(fr);
-      PU[0] = slot_at(sl, q.x) * slot_at(sl, q.y);
-      PF[0] = slot_at(sl, q.z) * slot_at(sl, q.w);
-    } else {
+    Dense4<TPL, NS, 0, 0>::eval(fr, sl, PU);
+    Dense4<TPL, NS, 1, 0>::eval(fr, sl, PF);
 #pragma unroll
-      for (int g = 0; g < NC; g += 2) {
-        const uint4 q = *reinterpret_cast<const uint4 *>(fr + g * 8);
-        PU[g] = slot_at(sl, q.x) * slot_at(sl, q.y);
-        PU[g + 1] = slot_at(sl, q.z) * slot_at(sl, q.w);
-      }
-#pragma unroll
-      for (int g = 0; g < NC; g += 2) {
-        const uint4 q = *reinterpret_cast<const uint4 *>(fr + (NC + g) * 8);
-        PF[g] = slot_at(sl, q.x) * slot_at(sl, q.y);
-        PF[g + 1] = slot_at(sl, q.z) * slot_at(sl, q.w);
-      }
-    }
-    const uint4 cu = p.tab[o + 9], cf = p.tab[o + 10];
-    const uint32_t cuw[4] = {cu.x, cu.y, cu.z, cu.w}, cfw[4] = {cf.x, cf.y, cf.z, cf.w};
-    // extra records: one stream across all groups, software-pipelined by one record -- the slot operands of the NEXT
-    // record are requested before the current one is accumulated, also across group boundaries (the block ends with two
-    // harmless sentinel records), so the LDCU -> LDS -> DFMA chain is not exposed once per group
-    uint32_t rwb = (o + h0.z) * 16u + 2u * NC * 8u;  // byte offset of the current record {u32 off0, u32 off1}
-    uint2 ro = *reinterpret_cast<const uint2 *>(tb + rwb);
-    double ra = slot_at(sl, ro.x), rb = slot_at(sl, ro.y);
-    ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);  // offsets run TWO records ahead, operands one (two sentinels)
-    constexpr int NW = (NC + 3) / 4, GW = NC < 4 ? NC : 4;  // count words per polynomial, groups per word
-#pragma unroll
-    for (int q = 0; q < 2 * NW; ++q) {
-      const uint32_t cw = q < NW ? cuw[q % NW] : cfw[q % NW];
-      if (cw != 0u) {  // (one test skips four groups without extra records)
-#pragma unroll
-        for (int k = 0; k < GW; ++k) {
-          const int gg = (q % NW) * 4 + k;
-          const uint32_t cnt = (cw >> (8 * k)) & 255u;
-          double accg = q < NW ? PU[gg] : PF[gg];
-#pragma unroll 1
-          for (uint32_t i = 0; i < cnt; ++i) {
-            accg = fma(ra, rb, accg);
-            rwb += 8u;
-            ra = slot_at(sl, ro.x);
-            rb = slot_at(sl, ro.y);
-            ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);
-          }
-          if (q < NW) PU[gg] = accg; else PF[gg] = accg;
-        }
-      }
-    }
-#pragma unroll
-    for (int b = 0; b < NS; ++b)
+    for (int b = 1; b < NS; ++b)  // (level b = 0 is done by Dense4)
 #pragma unroll
       for (int X = 0; X < NC; ++X)
         if (X >> b & 1) {
@@ -266,8 +262,8 @@ __device__ __forceinline__ bool sector4(const Qmc4Launch &p, const uint32_t o, u
 // partial layout: fused  : [run of sectors][shift][slice][NACC]
 //                 persec : [sector row][shift][slice][NACC]        (NACC = QMC_MAXSING + KMAX + 1, index a <-> order a - QMC_MAXSING)
 // T = threads per block (128 or 512; 512 registers-worth of threads per SM either way: 128 registers per thread)
-template <int NDIM, int L, int KMAX, int T>
-__global__ void __launch_bounds__(T, 512 / T) qmc4_eval_kernel(const __grid_constant__ Qmc4Launch p) {
+template <int NDIM, int L, int KMAX, int T, int TPL>
+__global__ void __launch_bounds__(T, T >= 256 ? 1 : 512 / T) qmc4_eval_kernel(const __grid_constant__ Qmc4Launch p) {
   using namespace qmc4;
   constexpr int NACC = QMC_MAXSING + KMAX + 1;
   constexpr int SMAX = NDIM < QMC_MAXSING ? NDIM : QMC_MAXSING;
@@ -291,9 +287,9 @@ __global__ void __launch_bounds__(T, 512 / T) qmc4_eval_kernel(const __grid_cons
   for (int i = tid; i < QMC4_LOG_ENTRIES * QMC4_LOG_COPIES; i += T)
     logtab[i] = reinterpret_cast<const double2 *>(p.logtab)[i / QMC4_LOG_COPIES];
   for (int i = tid; i < p.m * NDIM; i += T) shf[i] = p.shifts[i];
-  slots[3 * NDIM * T + tid] = 1.0;        // the constant slots: 1, 0, the chunk's coefficient constants
-  slots[(3 * NDIM + 1) * T + tid] = 0.0;
-  for (uint32_t i = 0; i < p.nconst; ++i) slots[(3 * NDIM + 2 + i) * T + tid] = p.cval[i];
+  slots[2 * NDIM * T + tid] = 1.0;        // the constant slots: 1, 0, the chunk's coefficient constants
+  slots[(2 * NDIM + 1) * T + tid] = 0.0;
+  for (uint32_t i = 0; i < p.nconst; ++i) slots[(2 * NDIM + 2 + i) * T + tid] = p.cval[i];
   __syncthreads();
 
   const uint32_t N = p.N;
@@ -351,7 +347,6 @@ __global__ void __launch_bounds__(T, 512 / T) qmc4_eval_kernel(const __grid_cons
         }
         reinterpret_cast<double *>(sl)[j * T] = tj;
         reinterpret_cast<double *>(sl)[(NDIM + j) * T] = fast_log(tj, tabq);  // t >= 3.7e-32 for y >= 2^-53: a normal number
-        reinterpret_cast<double *>(sl)[(2 * NDIM + j) * T] = fast_rcp(tj);
         uint32_t rn = r[j] + dz[j];
         r[j] = rn >= N ? rn - N : rn;
       }
@@ -371,17 +366,16 @@ __global__ void __launch_bounds__(T, 512 / T) qmc4_eval_kernel(const __grid_cons
         if (since_sync == 0) __syncthreads();
         since_sync = since_sync + 1 == p.sync_every ? 0 : since_sync + 1;
       }
-      for (int si = 0; si < p.nsec; ++si) {
-        // (offsets come from an array indexed by the induction variable: a loop-carried offset read from the table
-        //  itself makes ptxas give up the uniform datapath for the whole table walk)
-        const uint32_t so = p.secw[si];
-        const uint4 h0 = p.tab[so];
-#define QMC4_CASE(NS_)                                                                                       \
-  case NS_: {                                                                                                \
-    if (NS_ <= SMAX) {                                                                                       \
-      constexpr int NSC = NS_ <= SMAX ? NS_ : 0, KK = KMAX + NSC + 1;                                        \
+      // (sectors are sorted by their number of singular variables: p.nsb[ns] .. p.nsb[ns + 1] run the code path of ns;
+      //  offsets come from an array indexed by the induction variable: a loop-carried offset read from the table
+      //  itself makes ptxas give up the uniform datapath for the whole table walk)
+#define QMC4_CLASS(NS_)                                                                                      \
+  if (NS_ <= SMAX) {                                                                                         \
+    constexpr int NSC = NS_ <= SMAX ? NS_ : 0, KK = KMAX + NSC + 1;                                          \
+    for (int si = p.nsb[NS_]; si < p.nsb[NS_ + 1]; ++si) {                                                   \
+      const uint32_t so = p.secw[si];                                                                        \
       double res[KK], g0;                                                                                    \
-      bool fin = sector4<NDIM, L, NSC, KMAX, T>(p, so, sl, tabq, res, g0);                                   \
+      bool fin = sector4<NDIM, L, NSC, KMAX, T, TPL>(p, so, sl, tabq, res, g0);                                   \
       const double wg = w * g0;                                                                              \
       fin = fin && finite_hi(g0);                                                                            \
       _Pragma("unroll") for (int i = 0; i < KK; ++i) fin = fin && finite_hi(res[i]);                         \
@@ -396,18 +390,13 @@ __global__ void __launch_bounds__(T, 512 / T) qmc4_eval_kernel(const __grid_cons
           if (fin) sa[(size_t)i * T] += wg * res[i];                                                         \
       }                                                                                                      \
     }                                                                                                        \
-  } break;
-        switch (h0.x & 255u) {
-          QMC4_CASE(0)
-          QMC4_CASE(1)
-          QMC4_CASE(2)
-          QMC4_CASE(3)
-          QMC4_CASE(4)
-          default:
-            break;
-        }
-#undef QMC4_CASE
-      }
+  }
+      QMC4_CLASS(0)
+      QMC4_CLASS(1)
+      QMC4_CLASS(2)
+      QMC4_CLASS(3)
+      QMC4_CLASS(4)
+#undef QMC4_CLASS
     }
 
     // S7: block reduction -> one partial per (run | sector, shift, block)

@@ -55,16 +55,16 @@ cudaError_t qmc_kernel_launch(int ndim, int kmax, int flavor, dim3 grid, size_t 
 // into the thread's slot column; the coefficient lives in a slot, qmc_image4.cpp).  Layout of `tab` (16-byte words):
 //   [prog_word ..)  slot program: nprog x {u32 a_off, u32 b_off}, 2 per word
 //   [sec_word ..)   sector blocks, back to back; sector block (word offsets relative to its start):
-//     w0 = {nsing | nL0 << 8 | nlocal << 16, nwords of the block, first dense record word, 0}
+//     w0 = {nsing | nL0 << 8 | nlocal << 16 | nfused << 24, nwords of the block, first dense position word, 0}
 //     w1 = sing_ln[4]  (byte offsets of ln t_k of the singular positions)      w2 = sing_t[4]  (of t_k)
 //     w3,w4 = 1/beta[4] (f64)      w5,w6 = beta[4] (f64)
-//     w7 = {f64 coefficient of G0', u32 off0, u32 off1}: G0' = c * slot * slot = c_U^aU0 c_F^aF0 prod_reg t^alpha prod_sing 1/t
+//     w7 = {f64 coefficient of G0, u32 off0, u32 off1}: G0 = c * slot * slot = c_U^aU0 c_F^aF0 prod_reg t^alpha
 //     w8 = {f64 constant of L0 = aU1 ln c_U + aF1 ln c_F, 0, 0}
-//     w9 = extra records per group of U^ (u8 x 16)      w10 = the same for F^
-//     w11.. = nL0 x {f64 beta_j, u32 offset of ln t_j, 0} (regular variables), then the local program nlocal x {u32 a_off,
-//     u32 b_off} padded to a word, then the records: [first record of every group of U^: 2^nsing, the 0.0 slot twice if
-//     the group is empty][the same for F^][extra records of U^ by group][extra records of F^ by group][two sentinels],
-//     padded to a word
+//     w9.. = (n - nsing) x {f64 beta_j, u32 offset of ln t_j, 0} (one per regular variable), then the local program nlocal x {u32 a_off,
+//     u32 b_off} padded to a word (slot[local0 + i] = slot[a] * slot[b]), then nfused x 2 words {a, b, c, d}{dst, 0, 0, 0}
+//     (slot[dst] = slot[a] * slot[b] + slot[c] * slot[d]: the overflow of groups with more monomials than dense positions),
+//     then the dense positions: for U^ then F^, group by group, qmc4_cap(nsing, polynomial, popcount of the group) records
+//     (qmc_tables.h; an unused position is the 0.0 slot twice), padded to a word
 #define QMC4_TAB_WORDS 1800  // 28 800 bytes of tables per launch (kernel parameters are limited to 32 764 bytes)
 #define QMC4_MAX_SEC 160     // sectors per launch
 #define QMC4_LOG_ENTRIES 64
@@ -83,14 +83,15 @@ struct Qmc4Launch {
   double tc[4], wc[2];           // periodising transform (see qmc_transform_poly)
   double dN, invN;               // (double)N and RN(1 / N): constant-bank operands of the lattice-point division (S1)
   double cval[QMC4_MAXCONST];    // values of the coefficient-constant slots 3n + 2 ..
-  uint16_t secw[QMC4_MAX_SEC];  // word offset of the sector blocks in tab, in evaluation order (sorted by nsing: sectors
-                                // that run the same code path are neighbours, which the instruction cache likes)
+  int32_t nsb[QMC_MAXSING + 2];  // evaluation positions [nsb[ns], nsb[ns + 1]) hold the sectors with ns singular variables
+  uint16_t secw[QMC4_MAX_SEC];  // word offset of the sector blocks in tab, in evaluation order (sorted by nsing: one code
+                                // path per class, no dispatch per sector)
   uint16_t secrow[QMC4_MAX_SEC]; // per-sector mode: row of the partial buffer relative to out_row
   uint4 tab[QMC4_TAB_WORDS];
 };
 static_assert(sizeof(Qmc4Launch) <= 32764, "kernel parameter limit");
-cudaError_t qmc4_kernel_prepare(int ndim, int loops, int kmax, int threads, size_t smem, int *blocks_per_sm);
-cudaError_t qmc4_kernel_launch(int ndim, int loops, int kmax, int threads, dim3 grid, size_t smem, cudaStream_t st,
+cudaError_t qmc4_kernel_prepare(int ndim, int loops, int kmax, int threads, int tpl, size_t smem, int *blocks_per_sm);
+cudaError_t qmc4_kernel_launch(int ndim, int loops, int kmax, int threads, int tpl, dim3 grid, size_t smem, cudaStream_t st,
                                const Qmc4Launch &p);
 bool qmc4_kernel_available(int ndim, int loops, int kmax);
 

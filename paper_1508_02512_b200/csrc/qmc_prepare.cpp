@@ -349,7 +349,7 @@ int qmc_build_tables(const qmc_graph *g, const qmc_kinematics *kin, int eps_orde
   // table-driven kernels: real path (version 4) and complex path (version 5).  What a builder cannot represent falls back
   // to the generic kernel: on failure EVERYTHING the builder left behind is dropped, so that qmc_integrate sees no
   // half-built tables
-  if (qmc_build_tables4(T, opt ? opt->slot_budget : 0, opt ? opt->chunk_bytes : 0, opt ? opt->threads : 0) != QMC_OK) {
+  if (qmc_build_tables4(T, opt ? opt->slot_budget : 0, opt ? opt->chunk_bytes : 0, opt ? opt->threads : 0, opt ? opt->dense_template : 0) != QMC_OK) {
     T->tab4.clear();
     T->secoff4.clear();
     T->prog4.clear();

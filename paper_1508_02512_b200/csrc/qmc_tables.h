@@ -33,12 +33,41 @@ static_assert(sizeof(QmcSectorHdr) == 64, "sector header must be 64 bytes");
 // ---- real path ("version 4" tables, built by qmc_image4.cpp; layout of the kernel-side tables: qmc_launch.h) ----------
 // Sectors are grouped into CHUNKS.  Every chunk owns a "slot program": each thread keeps, per lattice point, a column
 // of per-point values in shared memory (slot s of thread tid at slots[s * T + tid]):
-//   [0,n) t_j | [n,2n) ln t_j | [2n,3n) 1/t_j | 3n: 1.0 | 3n+1: 0.0 | 3n+2 ..: coefficient constants | products slot[k] = slot[a] * slot[b]
+//   [0,n) t_j | [n,2n) ln t_j | 2n: 1.0 | 2n+1: 0.0 | 2n+2 ..: coefficient constants | products slot[k] = slot[a] * slot[b]
 // chosen per chunk by a byte-pair-encoding style pass over the chunk's monomials (most frequent pair of factors
 // first) until every monomial is a product of at most two slots.  A monomial is then one 8-byte record.
 #define QMC2_MAXSLOTS 56
 #define QMC2_MAXLOCAL 8
+#ifndef QMC4_TBIG
+#define QMC4_TBIG 512  // threads per block of the real-path kernel for tables dominated by sectors with 3-4 singular variables
+#endif
 #define QMC4_MAXCONST 12   // distinct coefficient constants (other than 1) per chunk
+// Real-path walk: DENSE POSITIONS per group of a sector's U^ and F^ (group = set of singular variables a monomial depends
+// on), by (template, number of singular variables, polynomial, popcount of the group).  The kernel evaluates every position
+// in straight-line code with a compile-time destination register; a group with fewer monomials fills up with 0 * 0 records,
+// a group with more sums its overflow into a sector-local slot first (qmc_image4.cpp).  Two templates, chosen per tables
+// object by modelled cost: 0 = lean (one-loop sized polynomials: one or two monomials per group), 1 = tuned on the group
+// statistics of the two-loop planar double box.  Any shape is exact under either.
+#if defined(__CUDACC__)
+#define QMC_HD __host__ __device__
+#else
+#define QMC_HD
+#endif
+QMC_HD constexpr int qmc4_cap(int tpl, int nsing, int poly, int popc) {
+  constexpr int capU1[5][5] = {{6, 0, 0, 0, 0}, {8, 10, 0, 0, 0}, {4, 4, 7, 0, 0}, {2, 2, 3, 5, 0}, {1, 1, 1, 2, 5}};
+  constexpr int capF1[5][5] = {{6, 0, 0, 0, 0}, {8, 3, 0, 0, 0}, {6, 2, 2, 0, 0}, {4, 2, 2, 1, 0}, {3, 1, 1, 1, 1}};
+  constexpr int capU0[5][5] = {{3, 0, 0, 0, 0}, {2, 2, 0, 0, 0}, {2, 1, 1, 0, 0}, {2, 1, 1, 1, 0}, {1, 1, 1, 1, 1}};
+  constexpr int capF0[5][5] = {{3, 0, 0, 0, 0}, {2, 1, 0, 0, 0}, {2, 1, 1, 0, 0}, {2, 1, 1, 1, 0}, {2, 1, 1, 1, 1}};
+  return tpl ? (poly ? capF1[nsing][popc] : capU1[nsing][popc]) : (poly ? capF0[nsing][popc] : capU0[nsing][popc]);
+}
+QMC_HD constexpr int qmc4_popc(int g) { return (g & 1) + ((g >> 1) & 1) + ((g >> 2) & 1) + ((g >> 3) & 1); }
+// index of the first dense position of group g of polynomial poly (U^ positions first, then F^); g = 2^nsing: the total
+QMC_HD constexpr int qmc4_pos(int tpl, int nsing, int poly, int g) {
+  int p = 0;
+  for (int q = 0; q <= poly; ++q)
+    for (int h = 0; h < (q < poly ? (1 << nsing) : g); ++h) p += qmc4_cap(tpl, nsing, q, qmc4_popc(h));
+  return p;
+}
 struct Qmc2Rec {        // complex-path record: value = c * slot[s0] * slot[s1]; s0, s1 are BYTE offsets into the thread's column
   double c;
   uint32_t s0, s1;
@@ -49,7 +78,7 @@ struct Qmc2Chunk {      // host description of one chunk
   int nslots = 0;     // chunk-wide slots (base + constants + products)
   int nconst = 0;     // coefficient constants (real path)
   int max_local = 0;  // largest number of sector-local product slots in the chunk
-  int nrec = 0, nlocal = 0;               // monomial records / sector-local products over the chunk (describe)
+  int nrec = 0, nlocal = 0, noverflow = 0;  // monomial records / sector-local products / monomials beyond the dense positions (describe)
   uint32_t tab_words = 0;                 // 16-byte words of sector blocks (real path)
   uint32_t prog_off = 0, prog_bytes = 0;  // complex path: chunk header + slot programs in image3
   double cost = 0.0;                      // modelled flops per point (load balancing)
@@ -115,6 +144,7 @@ struct qmc_tables {
   std::vector<Qmc2Chunk> chunks;  // real path (empty when lambda > 0)
   std::vector<double> sec_cost;   // modelled cost per sector (load balancing of the launch)
   // version 4 tables (real path; laid out for the kernel-parameter constant bank: see qmc_launch.h)
+  int tpl_real = 1;                 // dense-position template of the real-path tables (qmc4_cap)
   int threads_real = 512;           // threads per block of the real-path kernel: the slot offsets in tab4 / prog4 are
                                     // premultiplied by it (chosen by qmc_build_tables4, see there)
   std::vector<uint32_t> tab4;       // sector blocks, 32-bit words (4 per 16-byte table word)
@@ -153,7 +183,7 @@ struct qmc_tables {
 // builds sectors (+ image) from a graph; returns a qmc_status
 // builds tab4 / secoff4 / prog4 / const4 / chunks from `sectors` (real path); returns a qmc_status.
 // slot_budget, chunk_bytes, threads: 0 = the measured defaults (qmc_tuning in qmc_feynman.h)
-int qmc_build_tables4(qmc_tables *t, int slot_budget, int chunk_bytes, int threads);
+int qmc_build_tables4(qmc_tables *t, int slot_budget, int chunk_bytes, int threads, int dense_template);
 // builds image3 / secoff3 / chunks3 (complex path); returns a qmc_status
 int qmc_build_image3(qmc_tables *t, int slots_r, int slots_c, int chunk_bytes);  // 0 = the measured defaults
 int qmc_build_tables(const qmc_graph *g, const qmc_kinematics *kin, int eps_order, const qmc_options *opt,
