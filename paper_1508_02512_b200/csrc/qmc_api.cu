@@ -252,13 +252,12 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
               int waves_opt, int streams_opt, int *gx_out, int *rows_out, int *launches_out, size_t *h2d, cudaError_t *ce_out) {
   const int n = t->n, nacc = QMC_MAXSING + t->kmax + 1, T = t->threads_real;
   const size_t budget = (size_t)smem_optin - 1024;
-  // shared memory of a launch: logarithm table, shift vectors, reduction scratch, the chunk's slot columns (+ per-sector
-  // accumulators in per-sector mode)
+  // shared memory of a launch: logarithm table, shift vectors, reduction scratch, the chunk's slot columns.
+  // Per-sector mode = one launch per sector (its accumulators are then registers like in the fused mode).
   auto fixed_of = [&](const Qmc2Chunk &c) {
     return (size_t)QMC4_LOG_ENTRIES * QMC4_LOG_COPIES * 16 + (((size_t)m * n * 8 + 15) & ~(size_t)15) + (T / 32) * 8 +
            (size_t)(c.nslots + c.max_local) * T * 8;
   };
-  const size_t accbytes = persec ? (size_t)nacc * T * 8 : 0;
   struct Run { int chunk, a, b; double cost; size_t smem; };
   std::vector<Run> runs;
   double total_cost = 0.0;
@@ -269,16 +268,16 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
     const int e = std::min(se, c.sec_end);
     const size_t prog_words = t->prog4[ci].size() / 4;
     const size_t fixed = fixed_of(c);
-    if (a < e && fixed + accbytes > budget) return QMC_ENOMEM;
+    if (a < e && fixed > budget) return QMC_ENOMEM;
     while (a < e) {
       int b = a;
       while (b < e) {
         const size_t words = prog_words + (t->secoff4[b + 1] - t->secoff4[a]);
-        if (words > QMC4_TAB_WORDS || b + 1 - a > QMC4_MAX_SEC || fixed + accbytes * (b + 1 - a) > budget) break;
+        if (words > QMC4_TAB_WORDS || b + 1 - a > QMC4_MAX_SEC || (persec && b > a)) break;
         ++b;
       }
       if (b == a) return QMC_ENOMEM;
-      Run r = {(int)ci, a, b, 0.0, fixed + accbytes * (b - a)};
+      Run r = {(int)ci, a, b, 0.0, fixed};
       for (int s = a; s < b; ++s) r.cost += t->sec_cost[s];
       total_cost += r.cost;
       smem = std::max(smem, r.smem);
@@ -297,6 +296,7 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
   int max_slices = 1;
   for (int i = 0; i < nitems; ++i) {
     long long ns = (long long)(nblocks_target * runs[i].cost / total_cost + 0.5);
+    if (persec) ns = std::max<long long>(ns, (sms + 4 * m - 1) / (4 * m));  // one small launch per sector: a quarter wave each
     ns = std::max<long long>(1, std::min<long long>({ns, (long long)QMC_MAX_BLOCKS, max_slices_pts}));
     nsl[i] = (int)ns;
     max_slices = std::max(max_slices, (int)ns);
@@ -330,12 +330,10 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
   p.m = m;
   p.transform = t->transform;
   qmc_transform_poly(t->transform, p.tc, p.wc);
-  p.persec = persec ? 1 : 0;
   p.max_slices = max_slices;
   p.dN = (double)N;
   p.invN = 1.0 / (double)N;
   p.sync_every = 4;  // measured on B200 (kernels): a block barrier every fourth point
-  if (const char *e = std::getenv("QMC_TMP_SYNC")) p.sync_every = (uint32_t)std::atoi(e);  // TEMPORARY experiment knob
   cudaEventRecord(static_cast<cudaEvent_t>(t->ev0), st);
   if (nstreams) {
     cudaEventRecord(static_cast<cudaEvent_t>(t->side_events[nstreams]), st);
@@ -368,11 +366,7 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
       for (int ns = 0; ns <= QMC_MAXSING; ++ns) {
         p.nsb[ns] = k;
         for (int s = r.a; s < r.b; ++s)
-          if (t->sectors[s].nsing == ns) {
-            p.secw[k] = (uint16_t)(p.sec_word + (t->secoff4[s] - w0));
-            p.secrow[k] = (uint16_t)(s - r.a);
-            ++k;
-          }
+          if (t->sectors[s].nsing == ns) p.secw[k++] = (uint16_t)(p.sec_word + (t->secoff4[s] - w0));
       }
       p.nsb[QMC_MAXSING + 1] = k;
     }

@@ -190,10 +190,10 @@ int qmc_build_tables4(qmc_tables *t, int slot_budget, int chunk_bytes_opt, int t
     total_cost += cost[i];
     total_bytes += 16.0 * (11 + n) + 8.0 * qmc4_pos(t->tpl_real, s.nsing, 1, 1 << s.nsing);
   }
-  // 40 chunk-wide slots (+ the coefficient constants) + up to 8 sector-local ones: 49 columns of 8 T bytes = 196 KB at
-  // T = 512 (one block per SM, and room for the accumulators of the per-sector mode); the more slots, the fewer
-  // sector-local products and chunks (measured on B200, cfg4)
-  const int max_slots_base = slot_budget > 0 ? slot_budget : 40;
+  // 44 chunk-wide slots (+ the coefficient constants) + up to 8 sector-local ones: 53 columns of 8 T bytes = 212 KB at
+  // T = 512 (one block per SM); the more slots, the fewer sector-local products and chunks (measured on B200, cfg4:
+  // 32 / 36 / 40 / 44 slots -> 232 / 211 / 187 / 183 ms per step)
+  const int max_slots_base = slot_budget > 0 ? slot_budget : 44;
   const double chunk_bytes = chunk_bytes_opt > 0 ? std::max(1000.0, (double)chunk_bytes_opt) : 24000.0;
   int nch = std::max(1, (int)(total_bytes / chunk_bytes + 0.999));
   std::vector<std::pair<int, int>> todo;  // ranges still to plan (processed in order)

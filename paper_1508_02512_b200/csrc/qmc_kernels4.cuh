@@ -259,8 +259,8 @@ __device__ __forceinline__ bool sector4(const Qmc4Launch &p, const uint32_t o, u
 
 }  // namespace qmc4
 
-// partial layout: fused  : [run of sectors][shift][slice][NACC]
-//                 persec : [sector row][shift][slice][NACC]        (NACC = QMC_MAXSING + KMAX + 1, index a <-> order a - QMC_MAXSING)
+// partial layout: [row][shift][slice][NACC], row = run of sectors (fused mode) or sector (per-sector mode: one launch per
+// sector, so that the accumulators stay in registers)        (NACC = QMC_MAXSING + KMAX + 1, index a <-> order a - QMC_MAXSING)
 // T = threads per block (128 or 512; 512 registers-worth of threads per SM either way: 128 registers per thread)
 template <int NDIM, int L, int KMAX, int T, int TPL>
 __global__ void __launch_bounds__(T, T >= 256 ? 1 : 512 / T) qmc4_eval_kernel(const __grid_constant__ Qmc4Launch p) {
@@ -279,8 +279,6 @@ __global__ void __launch_bounds__(T, T >= 256 ? 1 : 512 / T) qmc4_eval_kernel(co
   double *scratch = reinterpret_cast<double *>(smem + o);
   o += (T / 32) * 8;
   double *slots = reinterpret_cast<double *>(smem + o);
-  o += (size_t)p.max_nslots * T * 8;
-  double *sacc = reinterpret_cast<double *>(smem + o);  // persec: [nsec][NACC][T]
   unsigned char *sl = reinterpret_cast<unsigned char *>(slots + tid);
   const double2 *tabq = logtab + (tid & (QMC4_LOG_COPIES - 1));
 
@@ -309,8 +307,6 @@ __global__ void __launch_bounds__(T, T >= 256 ? 1 : 512 / T) qmc4_eval_kernel(co
     double acc[NACC];
 #pragma unroll
     for (int a = 0; a < NACC; ++a) acc[a] = 0.0;
-    if (p.persec)
-      for (int i = 0; i < p.nsec * NACC; ++i) sacc[(size_t)i * T + tid] = 0.0;
 
     // The point loop has a UNIFORM trip count (threads past the end of the index range, and boundary points, carry the
     // weight 0 at a harmless stand-in point): only then may ptxas keep the table walk on the uniform datapath.
@@ -381,14 +377,8 @@ __global__ void __launch_bounds__(T, T >= 256 ? 1 : 512 / T) qmc4_eval_kernel(co
       _Pragma("unroll") for (int i = 0; i < KK; ++i) fin = fin && finite_hi(res[i]);                         \
       /* a non-finite evaluation is dropped (and counted); a dead thread has w = 0.  Predicated, not branched */ \
       cntNonFinite += (live && !fin) ? 1u : 0u;                                                              \
-      if (!p.persec) {                                                                                       \
-        _Pragma("unroll") for (int i = 0; i < KK; ++i)                                                       \
-          if (fin) acc[QMC_MAXSING - NSC + i] = fma(wg, res[i], acc[QMC_MAXSING - NSC + i]);                 \
-      } else {                                                                                               \
-        double *sa = sacc + ((size_t)si * NACC + (QMC_MAXSING - NSC)) * T + tid;                             \
-        _Pragma("unroll") for (int i = 0; i < KK; ++i)                                                       \
-          if (fin) sa[(size_t)i * T] += wg * res[i];                                                         \
-      }                                                                                                      \
+      _Pragma("unroll") for (int i = 0; i < KK; ++i)                                                         \
+        if (fin) acc[QMC_MAXSING - NSC + i] = fma(wg, res[i], acc[QMC_MAXSING - NSC + i]);                   \
     }                                                                                                        \
   }
       QMC4_CLASS(0)
@@ -399,22 +389,12 @@ __global__ void __launch_bounds__(T, T >= 256 ? 1 : 512 / T) qmc4_eval_kernel(co
 #undef QMC4_CLASS
     }
 
-    // S7: block reduction -> one partial per (run | sector, shift, block)
-    if (!p.persec) {
-      double *dst = p.partial + (((size_t)p.out_row * p.m + kap) * p.max_slices + blockIdx.x) * NACC;
+    // S7: block reduction -> one partial per (row, shift, block)
+    double *dst = p.partial + (((size_t)p.out_row * p.m + kap) * p.max_slices + blockIdx.x) * NACC;
 #pragma unroll
-      for (int a = 0; a < NACC; ++a) {
-        double sr = block_sum_t<T>(acc[a], scratch);
-        if (tid == 0) dst[a] = sr;
-      }
-    } else {
-      for (int si = 0; si < p.nsec; ++si) {
-        double *dst = p.partial + (((size_t)(p.out_row + p.secrow[si]) * p.m + kap) * p.max_slices + blockIdx.x) * NACC;
-        for (int a = 0; a < NACC; ++a) {
-          double v = block_sum_t<T>(sacc[((size_t)si * NACC + a) * T + tid], scratch);
-          if (tid == 0) dst[a] = v;
-        }
-      }
+    for (int a = 0; a < NACC; ++a) {
+      double sr = block_sum_t<T>(acc[a], scratch);
+      if (tid == 0) dst[a] = sr;
     }
   }
 

@@ -65,7 +65,7 @@ cudaError_t qmc_kernel_launch(int ndim, int kmax, int flavor, dim3 grid, size_t 
 //     (slot[dst] = slot[a] * slot[b] + slot[c] * slot[d]: the overflow of groups with more monomials than dense positions),
 //     then the dense positions: for U^ then F^, group by group, qmc4_cap(nsing, polynomial, popcount of the group) records
 //     (qmc_tables.h; an unused position is the 0.0 slot twice), padded to a word
-#define QMC4_TAB_WORDS 1800  // 28 800 bytes of tables per launch (kernel parameters are limited to 32 764 bytes)
+#define QMC4_TAB_WORDS 1820  // 29 120 bytes of tables per launch (kernel parameters are limited to 32 764 bytes)
 #define QMC4_MAX_SEC 160     // sectors per launch
 #define QMC4_LOG_ENTRIES 64
 #define QMC4_LOG_COPIES 8
@@ -76,7 +76,7 @@ struct Qmc4Launch {
   unsigned long long *counters;  // device: [4]
   uint32_t N, count;
   uint32_t zeff[QMC_MAXDIM], off[QMC_MAXDIM];
-  int32_t m, transform, persec, max_slices;
+  int32_t m, transform, pad2, max_slices;
   int32_t nsec, out_row, count_boundary, nslices;
   uint32_t nprog, prog_word, sec_word, first_prod_off;  // first_prod_off, local0_off: byte offsets in the slot column
   uint32_t local0_off, max_nslots, nconst, sync_every;  // sync_every: block barrier every that many points (0 = never)
@@ -86,7 +86,6 @@ struct Qmc4Launch {
   int32_t nsb[QMC_MAXSING + 2];  // evaluation positions [nsb[ns], nsb[ns + 1]) hold the sectors with ns singular variables
   uint16_t secw[QMC4_MAX_SEC];  // word offset of the sector blocks in tab, in evaluation order (sorted by nsing: one code
                                 // path per class, no dispatch per sector)
-  uint16_t secrow[QMC4_MAX_SEC]; // per-sector mode: row of the partial buffer relative to out_row
   uint4 tab[QMC4_TAB_WORDS];
 };
 static_assert(sizeof(Qmc4Launch) <= 32764, "kernel parameter limit");
