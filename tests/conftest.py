@@ -17,3 +17,14 @@ def oracle_mod():
     import oracle
     oracle.build()
     return oracle
+
+
+def pytest_sessionfinish(session, exitstatus):
+    """Reading C19: the parity tests list every use of the A-floor; keep the list where gpurun brings it back."""
+    mod = sys.modules.get("test_gpu_parity")
+    if mod is not None and getattr(mod, "NFLOOR", None):
+        import json
+        out = os.path.join(ROOT, "gpurun_out")
+        os.makedirs(out, exist_ok=True)
+        with open(os.path.join(out, "parity_floor.json"), "w") as f:
+            json.dump(mod.NFLOOR, f, indent=1)

@@ -214,4 +214,4 @@ def test_kinematic_scan_points_threshold_and_lambda_independence():
     (c1, e1), (c2, e2) = res[(200000, 0.25)], res[(200000, 0.5)]
     assert abs((c1[-1] - c2[-1]).real) <= 5 * np.hypot(e1[-1].real, e2[-1].real)
     assert abs((c1[-1] - c2[-1]).imag) <= 5 * np.hypot(e1[-1].imag, e2[-1].imag)
-    assert c1[-1].imag > 0.3      # J_0(s = 200000) = 0.13976 + 0.34363 i on the GPU at N = 99991 (profiles/r01n)
+    assert c1[-1].imag > 0.3      # above the threshold s = 4 M_t^2 the integral has an absorptive part
