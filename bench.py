@@ -31,8 +31,11 @@ import qmc_inputs as qi  # noqa: E402  (seeded input generators only)
 METRIC = "fp64_integrand_evals_per_sec_all_sectors"
 UNIT = "evals/s"
 
-# default lattice size per config for the timed step (primes from BASELINE.md; cfg4's 999983 keeps a step ~1 s)
-DEFAULT_N = {1: 10007, 2: 9999991, 3: 9999991, 4: 999983, 5: 1048573}
+# default lattice size per config for the timed step (primes from BASELINE.md).  cfg4: the middle one of the three sizes
+# BASELINE.json lists (a step is ~1.8 s, so the driver's 25 device-timed + 20 end-to-end steps take ~1.5 min); the largest,
+# 99999989 (~18 s per step), is timed once beside it (`largest_size`)
+DEFAULT_N = {1: 10007, 2: 9999991, 3: 9999991, 4: 9999991, 5: 1048573}
+LARGEST_N = {4: 99999989}
 
 
 def workload(cfg: int):
@@ -80,21 +83,36 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(self.reasons)}
 
 
+def host_cores() -> int:
+    """Threads the oracle is run with, set explicitly (an inherited OMP_NUM_THREADS=1 made the two arms differ in round 1)."""
+    try:
+        return max(1, len(os.sched_getaffinity(0)))
+    except Exception:
+        return max(1, os.cpu_count() or 1)
+
+
+def config_of(wl, N, n_sectors, world):
+    """The `config` object: the same keys in the product arm and in the reference arm."""
+    return {"workload": wl.name, "N": int(N), "m": int(wl.m), "seed": int(wl.seed), "n_sectors": int(n_sectors), "dim": int(wl.dim),
+            "lambda": float(wl.lam), "parallelism": f"shift-sharded x{world}",
+            "l2": "flushed between steps (256 MiB fill, outside the event pairs); the tables (<= 300 KB) travel in the kernel parameters, nothing else is read"}
+
+
 def oracle_sample(wl, N, z, shifts, target_s: float):
     """Time the oracle (as it stands, all host cores) on a bounded sample of the same workload: the first `count`
     lattice indices of the rule, all sectors, the first m_s shift vectors.  Returns (evals/s, cores, description)."""
     import oracle
     o = oracle.Oracle.from_workload(wl)       # the oracle's own decomposition: no product code on this path
-    cores = oracle.max_threads()
+    cores = host_cores()
     m_s = min(2, shifts.shape[0])
     count = max(cores * 4, 64)
     t0 = time.perf_counter()
-    o.integrate(N, z, shifts[:m_s], index_range=(0, 1, count))
+    o.integrate(N, z, shifts[:m_s], index_range=(0, 1, count), threads=cores)
     dt = time.perf_counter() - t0
     rate = count * m_s * o.n_sectors / dt
     count = int(min(N, max(count, target_s * rate / (m_s * o.n_sectors))))
     t0 = time.perf_counter()
-    o.integrate(N, z, shifts[:m_s], index_range=(0, 1, count))
+    o.integrate(N, z, shifts[:m_s], index_range=(0, 1, count), threads=cores)
     dt = time.perf_counter() - t0
     val = count * m_s * o.n_sectors / dt
     c1 = max(64, count // (4 * cores))
@@ -134,8 +152,8 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * N * wl.m * n_sectors / val, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": wl.name, "N": N, "m": wl.m, "seed": wl.seed, "n_sectors": n_sectors,
-                       "note": "ms_per_step extrapolated from the bounded sample (cost is linear in N*m)"},
+            "config": config_of(wl, N, n_sectors, 1),
+            "note": "ms_per_step extrapolated from the bounded sample (cost is linear in N*m)",
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -145,7 +163,8 @@ def run_reference(args):
 def time_to_accuracy(q, wl, torch, target=1e-3, max_N=2 ** 27, transform=0):
     """M2: raise N through the primes below 2^k until the relative error of the eps^0 coefficient of J is <= target
     (reading C17); wall time of everything the user waits for after qmc_prepare: generating-vector search, uploads,
-    kernels, downloads, statistics, summed over the N tried."""
+    kernels, downloads, statistics, summed over the N tried.  `rel_err` is the ESTIMATED standard error of Eq. 20 over the
+    coefficient (what the paper calls accuracy), not a deviation from a known value."""
     t = q.qmc_prepare(wl, eps_order=wl.eps_order, lam=wl.lam, transform=transform)
     q.qmc_integrate(t, 16381, wl.m, seed=wl.seed)          # context / module warm-up, not timed
     tried = []
@@ -199,6 +218,21 @@ def cbc_vs_korobov(q, dev):
             row[name] = {"z": [int(v) for v in z], "coeff_eps0": [c0.real, c0.imag],
                          "rel_err_eps0": float(max(e0.real, e0.imag) / abs(c0))}
         out.append(row)
+    return out
+
+
+def closed_form_check(q, dev):
+    """ACTUAL deviations from known values (next to the estimated errors): the massless box through eps^0 (closed form,
+    tests/test_oracle_closed_forms.py) and the three leading poles of the double box (mpmath values of the same file)."""
+    out = []
+    for wl, N, exact in ((qi.massless_box(), 999983, [0.666666666666667, -1.2639198230760183, -1.2238036181980894]),
+                         (qi.double_box(), 999983, [2.0 / 9.0, -0.8497687147780183, 0.003001503361321066])):
+        t = q.qmc_prepare(wl, eps_order=wl.eps_order)
+        r = q.qmc_integrate(t, N, wl.m, seed=wl.seed, device=dev)
+        k = len(exact)
+        out.append({"workload": wl.name, "N": N, "m": wl.m, "orders": list(range(t.k_min, t.k_min + k)),
+                    "exact": exact, "value": [float(x) for x in r.coeff.real[:k]], "estimated_err": [float(x) for x in r.err.real[:k]],
+                    "deviation_in_sigma": [float(abs(v - e) / max(s, 1e-300)) for v, e, s in zip(r.coeff.real[:k], exact, r.err.real[:k])]})
     return out
 
 
@@ -258,6 +292,7 @@ def run_product(args):
     N = args.N or DEFAULT_N[args.config]
     m = wl.m
     t = q.qmc_prepare(wl, eps_order=wl.eps_order, lam=wl.lam)
+    geo = dict(waves=args.waves, streams=args.streams)           # launch geometry (0 = the library's defaults)
     z = q.qmc_generating_vector(N, t.dim, device=dev)           # Korobov P2 search on the device, outside the timed steps
     from paper_1508_02512_b200 import sharding
     shifts = sharding.shift_block(wl.seed, m, t.dim, rank, world)
@@ -269,7 +304,7 @@ def run_product(args):
     gathered = torch.zeros(world, t.K, m, 2, dtype=torch.float64, device=dev)
 
     def step(resident):
-        q.qmc_integrate_async(t, N, m, z=z, shifts=None if resident == 2 else shifts, resident=resident, device=dev)
+        q.qmc_integrate_async(t, N, m, z=z, shifts=None if resident == 2 else shifts, resident=resident, device=dev, **geo)
         if world > 1:
             dist.all_gather_into_tensor(gathered, q.qmc_result_device_totals(t, m).contiguous())
 
@@ -310,7 +345,7 @@ def run_product(args):
         dist.barrier()
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        r_e2e = q.qmc_integrate(t, N, m, z=z, shifts=shifts, resident=0, device=dev)
+        r_e2e = q.qmc_integrate(t, N, m, z=z, shifts=shifts, resident=0, device=dev, **geo)
         if world > 1:
             loc = torch.from_numpy(np.ascontiguousarray(r_e2e.shift_totals).view(np.float64).reshape(t.K, m, 2)).to(dev)
             sharding.combine(loc)
@@ -337,7 +372,7 @@ def run_product(args):
     mean_eval_ms = float(np.mean(eval_ms))
     achieved = flops_step / (mean_eval_ms * 1e-3) / 1e12
     nominal = 148 * 64 * 2 * 1.965e9 / 1e12
-    roofline = {"bound": "alu", "kernel": EVAL_KERNEL_NOTE if not t.is_complex else "qmc3_eval_kernel", "achieved": achieved, "peak": peak_flops / 1e12,
+    roofline = {"bound": "alu", "kernel": EVAL_KERNEL_NOTE if not t.is_complex else EVAL_KERNEL_NOTE.replace("qmc4", "qmc5"), "achieved": achieved, "peak": peak_flops / 1e12,
                 "unit": "TFLOP/s", "frac": achieved / (peak_flops / 1e12), "traffic": _traffic_from_profiles(),
                 "peak_source": "DFMA chain microbenchmark (qmc_fp64_peak) measured in this run; MEASURED_PEAKS.json has no FP64 entry",
                 "peak_nominal": nominal, "frac_of_nominal": achieved / nominal, "kernel_ms": mean_eval_ms,
@@ -347,10 +382,9 @@ def run_product(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": wl.name, "N": N, "m_per_gpu": m, "seed": wl.seed, "n_sectors": t.n_sectors,
-                       "dim": t.dim, "orders": [t.k_min, t.k_max], "complex": t.is_complex, "lambda": wl.lam,
-                       "corners_per_point": corners, "parallelism": f"shift-sharded x{world}",
-                       "l2": "flushed between steps (256 MiB fill, outside the event pairs); the tables (<= 300 KB) travel in the kernel parameters, nothing else is read"},
+            "config": config_of(wl, N, t.n_sectors, world),
+            "workload_info": {"orders": [t.k_min, t.k_max], "complex": t.is_complex, "corners_per_point": corners,
+                              "m_per_gpu": m, "tables": t.describe().splitlines()[0]},
             "corner_evals_per_sec": corners * N * m * world / (ms_per_step * 1e-3),
             "result": {"coeff_re": [float(x) for x in coeff.real], "coeff_im": [float(x) for x in coeff.imag],
                        "err_re": [float(x) for x in err.real], "err_im": [float(x) for x in err.imag],
@@ -359,7 +393,25 @@ def run_product(args):
                     "note": "qmc_integrate with host buffers each step: tables + shifts H2D (pageable staging), kernels, statistics D2H, host wall clock"},
             "gpu_launches": int(res.kernel_launches) * args.steps * world, "clocks": clocks, "roofline": roofline}
 
+    if world == 1 and not args.no_extras and args.config in LARGEST_N and N != LARGEST_N[args.config]:
+        # the largest lattice BASELINE.json lists for this config: one device-timed step (inputs resident), same kernels
+        NL = LARGEST_N[args.config]
+        zl = q.qmc_generating_vector(NL, t.dim, device=dev)
+        q.qmc_integrate_async(t, NL, m, z=zl, shifts=shifts, resident=0, device=dev, **geo)
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        flush.fill_(1)
+        a.record()
+        q.qmc_integrate_async(t, NL, m, z=zl, resident=2, device=dev, **geo)
+        b.record()
+        b.synchronize()
+        rl = q.qmc_result_fetch(t, m, device=dev)
+        msl = a.elapsed_time(b)
+        line["largest_size"] = {"N": NL, "steps": 1, "ms_per_step": msl, "value": NL * m * t.n_sectors / (msl * 1e-3), "unit": UNIT,
+                                "roofline_frac": (fp + fs) * NL * m / (rl.eval_kernel_ms * 1e-3) / peak_flops,
+                                "coeff_re": [float(x) for x in rl.coeff.real], "err_re": [float(x) for x in rl.err.real]}
     if world == 1 and not args.no_extras:
+        line["closed_form_check"] = closed_form_check(q, dev)
         z_o = test_vector(N, wl.dim)
         v, cores, desc = oracle_sample(wl, N, z_o, qi.splitmix64_shifts(wl.seed, m, wl.dim), 15.0)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
@@ -381,7 +433,7 @@ def run_product(args):
         line["convergence"] = [extra(convergence, q, w, tr) for w in (qi.massless_box(), qi.double_box(), qi.nonplanar_vertex())
                                for tr in (0, 2)]
         line["cbc_vs_korobov"] = extra(cbc_vs_korobov, q, dev)
-        line["per_sector_mode"] = extra(per_sector_mode, q, t, N, m, z, shifts, dev, torch)
+        line["per_sector_mode"] = extra(per_sector_mode, q, t, min(N, 999983), m, q.qmc_generating_vector(min(N, 999983), t.dim, device=dev), shifts, dev, torch)
         line["other_workloads"] = extra(other_workloads, q, torch, dev, args.config)
         line["kinematic_scan"] = extra(kinematic_scan, q, torch)
     print(json.dumps(line), flush=True)
@@ -445,6 +497,8 @@ def main():
     ap.add_argument("--N", type=int, default=0, help="lattice size (prime); default: DEFAULT_N[config]")
     ap.add_argument("--impl", default="product", choices=["product", "reference"])
     ap.add_argument("--no-extras", action="store_true", help="skip cpu_baseline, time-to-accuracy and other workloads")
+    ap.add_argument("--waves", type=int, default=0, help="qmc_run.waves: blocks per resident block slot over a step (0 = library default 16)")
+    ap.add_argument("--streams", type=int, default=0, help="qmc_run.streams: side streams of a step (0 = default 4, -1 = none: launches in order)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
