@@ -23,6 +23,10 @@
 
 #include "qmc_kernels4.cuh"  // fast_log (64 x 8 table), fast_rcp, slot_at, u2d
 
+#ifndef QMC5_MINB
+#define QMC5_MINB(NDIM) ((NDIM) <= 4 ? 4 : 2)  // resident 128-thread blocks per SM the register budget is sized for
+#endif
+
 namespace qmc5 {
 
 using qmc2::Expo;
@@ -42,6 +46,20 @@ static __device__ __noinline__ double atan2_lib(double y, double x) { return ata
 __device__ __forceinline__ cd clog5(cd a, const double2 *__restrict__ tabq) {
   const double arg = (a.im == 0.0 && a.re < 0.0) ? -3.14159265358979323846 : atan2_lib(a.im, a.re);
   return cd{0.5 * fast_log(cnorm2(a), tabq), arg};
+}
+// phase of a to about 1e-5 in single precision, with the convention of clog5 on the negative real axis; only ever used to
+// fix a winding number (|values| of U^, F^, rho_j are far inside the single-precision range; outside it the estimate falls
+// back to the double-precision routine)
+__device__ __forceinline__ float arg_estimate(cd a) {
+  if (a.im == 0.0 && a.re < 0.0) return -3.14159265f;
+  const float x = (float)a.re, y = (float)a.im;
+  const float ax = fabsf(x), ay = fabsf(y), mx = fmaxf(ax, ay), mn = fminf(ax, ay);
+  if (!(mx > 1e-30f && mx < 1e30f)) return (float)atan2_lib(a.im, a.re);
+  const float t = mn * __frcp_rn(mx), s = t * t;
+  float p = t * (0.99997726f + s * (-0.33262347f + s * (0.19354346f + s * (-0.11643287f + s * (0.05265332f + s * -0.01172120f)))));
+  if (ay > ax) p = 1.57079633f - p;
+  if (x < 0.0f) p = 3.14159265f - p;
+  return y < 0.0f ? -p : p;
 }
 template <int E>
 __device__ __forceinline__ cd cpow_c(cd x) {  // x^E, E >= 0 compile time
@@ -232,10 +250,13 @@ __device__ __forceinline__ void corner5(const Qmc5Launch &p, const uint32_t cw, 
   const cd Uv = UF[0], Fv = UF[1];
   if (Fv.im > 0.0) ++cntImF;
   if (!(Uv.re > 0.0)) ++cntReU;
-  // G_Z = G0 det J prod_{j notin Z} rho_j^alpha_j U^aU0 F^aF0 ;  Lambda_Z = aU1 ln U + aF1 ln F + sum_j beta_j ln rho_j + L0
+  // G_Z = G0 det J prod_{j notin Z} rho_j^alpha_j U^aU0 F^aF0 ;  Lambda_Z = aU1 ln U + aF1 ln F + sum_j beta_j ln rho_j + L0.
+  // The 2 + n principal logarithms are taken as ONE: Lambda_Z - L0 = ln Q + 2 pi i k with Q = U^aU1 F^aF1 prod_j rho_j^beta_j
+  // (complex products) and the winding number k fixed by single-precision estimates of the same phases: the sum of the
+  // principal phases, known to 1e-3, differs from the principal phase of Q by an exact multiple of 2 pi.
   cd num = cd{G0 * det.re, G0 * det.im}, den = cd{1.0, 0.0};
-  cd Lam = (double)E::aU1 * clog5(Uv, tabq) + (double)E::aF1 * clog5(Fv, tabq);
-  Lam.re += L0;
+  cd qn = cpow_c<(E::aU1 > 0 ? E::aU1 : 0)>(Uv), qd = cpow_c<(E::aF1 < 0 ? -E::aF1 : 0)>(Fv);
+  float th = (float)E::aU1 * arg_estimate(Uv) + (float)E::aF1 * arg_estimate(Fv);
 #pragma unroll
   for (int j = 0; j < NDIM; ++j) {
     const bool inZ = (zv >> j & 1u) != 0;
@@ -244,8 +265,15 @@ __device__ __forceinline__ void corner5(const Qmc5Launch &p, const uint32_t cw, 
       if (a < 0) den = den * rho[j];
       for (int q = 0; q < a; ++q) num = num * rho[j];
     }
-    if (b) Lam = Lam + (double)b * clog5(rho[j], tabq);
+    if (b) {
+      th += (float)b * arg_estimate(rho[j]);
+      for (int q = 0; q < b; ++q) qn = qn * rho[j];
+      for (int q = 0; q < -b; ++q) qd = qd * rho[j];
+    }
   }
+  cd Lam = clog5(qn * cinv(qd), tabq);
+  Lam.im = fma((double)rintf((th - (float)Lam.im) * 0.15915494f), 6.28318530717958647692, Lam.im);
+  Lam.re += L0;
   if (E::aU0 > 0) num = num * cpow_c<(E::aU0 > 0 ? E::aU0 : 0)>(Uv);
   if (E::aU0 < 0) den = den * cpow_c<(E::aU0 < 0 ? -E::aU0 : 0)>(Uv);
   if (E::aF0 > 0) num = num * cpow_c<(E::aF0 > 0 ? E::aF0 : 0)>(Fv);
@@ -354,7 +382,7 @@ __device__ __forceinline__ bool finite_hi(cd v) {
 
 // partial layout: fused [run][shift][slice][NACC][2], persec [sector row][shift][slice][NACC][2]
 template <int NDIM, int L, int KMAX>
-__global__ void __launch_bounds__(QMC3_THREADS, (NDIM <= 4 ? 512 : 256) / QMC3_THREADS) qmc5_eval_kernel(const __grid_constant__ Qmc5Launch p) {
+__global__ void __launch_bounds__(QMC3_THREADS, QMC5_MINB(NDIM)) qmc5_eval_kernel(const __grid_constant__ Qmc5Launch p) {
   using namespace qmc5;
   constexpr int NACC = QMC_MAXSING + KMAX + 1;
   constexpr int SMAX = NDIM < QMC3_MAXSING ? NDIM : QMC3_MAXSING;
