@@ -361,3 +361,22 @@ def test_maximum_baseline_sizes_strided_indices():
     z = qi.korobov_vector(N, 3, 2345677)
     parity(qi.massless_box(), N, 3, z=z, index_range=(5, 4099, (N - 5 + 4098) // 4099))
     parity(qi.massive_box(), N, 2, z=z, index_range=(11, 8191, (N - 11 + 8190) // 8191))
+
+
+def test_index_blocks_of_two_ranks_add_to_the_full_lattice():
+    """the lattice split into contiguous index ranges (sharding.index_block) -- the two half-sums, each
+    normalised by 1/N, add to the single-rank totals within the C19 tolerance (here: evaluated one after the other on one
+    GPU; the all_reduce itself is covered by tests/test_multi_rank.py)."""
+    from paper_1508_02512_b200 import sharding
+    wl = qi.double_box()
+    t = q.qmc_prepare(wl)
+    N, m = 131071, 4
+    z = qi.korobov_vector(N, 6, 60941)
+    sh = qi.splitmix64_shifts(wl.seed, m, 6)
+    full = q.qmc_integrate(t, N, m, z=z, shifts=sh)
+    parts = [q.qmc_integrate(t, N, m, z=z, shifts=sh, index_range=sharding.index_block(N, r, 2)) for r in range(2)]
+    tot = parts[0].shift_totals + parts[1].shift_totals
+    scale = np.abs(parts[0].shift_totals) + np.abs(parts[1].shift_totals)
+    assert np.all(np.abs(tot - full.shift_totals) <= 1e-12 * np.maximum(np.abs(full.shift_totals), scale))
+    coeff, err = q.qmc_statistics(tot)
+    assert np.allclose(coeff, full.coeff, rtol=1e-11, atol=1e-14)

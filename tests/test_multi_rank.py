@@ -65,3 +65,55 @@ def test_single_process_path_and_argument_checks():
         pass
     c2, e2 = q.qmc_statistics(T)
     assert np.array_equal(c2, coeff) and np.array_equal(e2, err)
+
+
+# ---- contiguous lattice-index ranges, one all_reduce(SUM) ---------------------------------------------------
+
+def fake_index_totals(N, begin, count):
+    """Per-shift totals a rank would hold for its index block: (1/N) sum over its indices of a function of (index, shift,
+    order) -- additive over blocks like the kernels' sums (Eq. 18)."""
+    i = np.arange(begin, begin + count, dtype=np.float64)[None, None, :]
+    k = np.arange(1, K + 1, dtype=np.float64)[:, None, None]
+    kap = np.arange(M, dtype=np.float64)[None, :, None]
+    return (np.cos(0.001 * i * k + kap) + 1j * np.sin(0.002 * i + k * kap)).sum(axis=2) / N
+
+
+def _index_worker(rank, world, port, out, N):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        b, step, c = sharding.index_block(N, rank, world)
+        coeff, err, T = sharding.reduce_index_blocks(fake_index_totals(N, b, c))
+        torch.save({"block": (b, step, c), "coeff": coeff, "err": err, "T": T}, os.path.join(out, f"i{rank}.pt"))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_index_range_sharding_allreduce_world2(tmp_path):
+    world, N = 2, 10007
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    mp.spawn(_index_worker, args=(world, port, str(tmp_path), N), nprocs=world, join=True)
+    res = [torch.load(os.path.join(str(tmp_path), f"i{r}.pt"), weights_only=False) for r in range(world)]
+    # the blocks tile 0..N-1 exactly once, contiguous, balanced to one index
+    assert res[0]["block"] == (0, 1, 5004) and res[1]["block"] == (5004, 1, 5003)
+    want = fake_index_totals(N, 0, N)                              # what one rank over the whole lattice would hold
+    for r in range(world):
+        assert np.allclose(res[r]["T"], want, rtol=1e-12, atol=1e-15)   # the two half-sums add to the single-rank totals
+        c, e = q.qmc_statistics(res[r]["T"])
+        assert np.array_equal(c, res[r]["coeff"]) and np.array_equal(e, res[r]["err"])
+    assert np.array_equal(res[0]["T"], res[1]["T"])                # every rank holds the same answer
+
+
+def test_index_blocks_tile_the_lattice():
+    for N, world in ((10007, 1), (10007, 3), (99991, 8), (16, 16)):
+        blocks = [sharding.index_block(N, r, world) for r in range(world)]
+        assert blocks[0][0] == 0 and sum(b[2] for b in blocks) == N
+        for a, b in zip(blocks, blocks[1:]):
+            assert a[0] + a[2] == b[0] and 0 <= a[2] - b[2] <= 1
+    try:
+        sharding.index_block(4, 0, 5)
+        assert False
+    except ValueError:
+        pass
