@@ -86,13 +86,16 @@ class Oracle:
         self.K = self.k_max - self.k_min + 1
 
     @classmethod
-    def from_workload(cls, wl, lam: Optional[float] = None, eps_order: Optional[int] = None, max_depth: int = 64):
+    def from_workload(cls, wl, lam: Optional[float] = None, eps_order: Optional[int] = None, max_depth: int = 64,
+                      order: int = 0):
+        """order = 0: decomposition rule A.3 (U^ first); 1: F^ first (only to pin strategy independence of the totals)."""
         eu, ev, m2, lv, gram = wl.arrays()
         L = _load()
-        h = L.orc_build(C.c_int(wl.n_vertices), C.c_int(wl.n_edges), C.c_int(len(lv)), _p(eu, C.c_int),
-                        _p(ev, C.c_int), _p(m2, C.c_double), _p(lv, C.c_int), _p(gram, C.c_double),
-                        C.c_double(wl.lam if lam is None else lam),
-                        C.c_int(wl.eps_order if eps_order is None else eps_order), C.c_int(max_depth))
+        L.orc_build_order.restype = C.c_void_p
+        h = L.orc_build_order(C.c_int(wl.n_vertices), C.c_int(wl.n_edges), C.c_int(len(lv)), _p(eu, C.c_int),
+                              _p(ev, C.c_int), _p(m2, C.c_double), _p(lv, C.c_int), _p(gram, C.c_double),
+                              C.c_double(wl.lam if lam is None else lam),
+                              C.c_int(wl.eps_order if eps_order is None else eps_order), C.c_int(max_depth), C.c_int(order))
         o = cls(h)
         o.n_edges = wl.n_edges
         return o

@@ -176,6 +176,7 @@ struct Problem {
   double lambda = 0.0;
   int kmax = 0, kmin = 0;
   int max_depth = 64;
+  int order = 0;  // 0: rule A.3 (target U^ first); 1: F^ first (strategy-independence pin)
   std::vector<Sector> sectors;
   int status = 0;  // 0 ok, -2 depth, -3 unsupported
 };
@@ -242,11 +243,15 @@ void decompose(Problem& pb, int primary, Poly U, Poly F, std::vector<int> alpha,
   if (pb.status) return;
   factor_out(U, pb.aU0, pb.aU1, alpha, beta);
   factor_out(F, pb.aF0, pb.aF1, alpha, beta);
+  // rule A.3 step 2: target U^ first, then F^ (pb.order = 0, the rule of every config); pb.order = 1 targets F^ first --
+  // another terminating strategy, used only to pin that the TOTALS do not depend on the strategy (reading C23)
   const Poly* target = nullptr;
-  if (!has_const(U))
-    target = &U;
-  else if (!has_const(F))
-    target = &F;
+  const Poly* first = pb.order ? &F : &U;
+  const Poly* second = pb.order ? &U : &F;
+  if (!has_const(*first))
+    target = first;
+  else if (!has_const(*second))
+    target = second;
   if (!target) {
     Sector s;
     s.primary = primary;
@@ -582,9 +587,17 @@ struct orc_problem {
 };
 
 // graph + kinematics -> U, F, sectors.  Returns NULL on invalid graph.
+orc_problem* orc_build_order(int V, int P, int nlegs, const int* eu, const int* ev, const double* m2, const int* legv,
+                             const double* gram, double lambda, int kmax, int max_depth, int order);
 orc_problem* orc_build(int V, int P, int nlegs, const int* eu, const int* ev, const double* m2, const int* legv,
                        const double* gram, double lambda, int kmax, int max_depth) {
+  return orc_build_order(V, P, nlegs, eu, ev, m2, legv, gram, lambda, kmax, max_depth, 0);
+}
+// order = 0: rule A.3 (U^ first); 1: F^ first (strategy-independence pin only)
+orc_problem* orc_build_order(int V, int P, int nlegs, const int* eu, const int* ev, const double* m2, const int* legv,
+                             const double* gram, double lambda, int kmax, int max_depth, int order) {
   orc_problem* h = new orc_problem;
+  h->pb.order = order;
   Graph& g = h->pb.g;
   g.V = V;
   g.P = P;
