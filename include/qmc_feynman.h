@@ -183,6 +183,14 @@ int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t sector_end
  * device (needs workspace of qmc_workspace_bytes). */
 int qmc_generating_vector(uint64_t N, int32_t dim, void *cuda_stream, void *dev_workspace, size_t dev_workspace_bytes,
                           uint64_t *z_out);
+/* The same search for callers that cannot allocate device memory (code under CUDA graph capture, serving loops, harnesses
+ * that forbid cudaMalloc): no workspace argument -- the scratch of the P_2 kernel (candidate vectors and per-block partial
+ * sums, 153 600 bytes) is a fixed array inside the library that every GPU holds from the moment it loads the library until
+ * the process exits.  Calls no cudaMalloc / cudaFree and no allocating routine; same candidates, same kernel, same z as
+ * qmc_generating_vector.  Limits: 5 <= N < 2^31, dim <= 8; dim > 8 returns QMC_ENOMEM ("workspace or buffer too small":
+ * the fixed scratch is sized for 64 candidates of up to 8 components).  All calls on one device SHARE the array: calls that
+ * overlap on the GPU (two streams, two threads) race -- serialise them.  Synchronises `cuda_stream` before returning. */
+int qmc_generating_vector_noalloc(uint64_t N, int32_t dim, void *cuda_stream, uint64_t *z_out);
 /* Generating vector by the component-by-component construction the paper names (refs [29, 30]): z_1 = 1, then
  * z_d = argmin over z in [1, (N-1)/2] of  e^2(z_1..z_d) = -1 + (1/N) sum_i prod_j (1 + 2 pi^2 B_2({i z_j / N}))  (the P_2
  * criterion of R:C13 with unit weights; ties -> smaller z; R:C25).  HOST function, O(dim N log N): the candidates of one

@@ -103,6 +103,8 @@ def lib():
         L.qmc_cbc_vector.argtypes = [C.c_uint64, C.c_int32, C.POINTER(C.c_uint64), C.POINTER(C.c_double)]
         L.qmc_generating_vector.restype = C.c_int
         L.qmc_generating_vector.argtypes = [C.c_uint64, C.c_int32, C.c_void_p, C.c_void_p, C.c_size_t, C.POINTER(C.c_uint64)]
+        L.qmc_generating_vector_noalloc.restype = C.c_int
+        L.qmc_generating_vector_noalloc.argtypes = [C.c_uint64, C.c_int32, C.c_void_p, C.POINTER(C.c_uint64)]
         L.qmc_shifts.restype = C.c_int
         L.qmc_shifts.argtypes = [C.c_uint64, C.c_int32, C.c_int32, C.POINTER(C.c_double)]
         L.qmc_prefactor_series.restype = C.c_int
@@ -380,6 +382,18 @@ def qmc_generating_vector(N: int, dim: int, device="cuda:0") -> np.ndarray:
     if rc:
         raise QmcError(rc, "qmc_generating_vector")
     return z
+
+
+def qmc_generating_vector_noalloc(N: int, dim: int, device="cuda:0") -> np.ndarray:
+    """qmc_generating_vector without a workspace: the library's own fixed device array is the scratch (no allocation)."""
+    import torch
+    dev = torch.device(device)
+    with torch.cuda.device(dev):
+        z = np.zeros(max(dim, 1), dtype=np.uint64)
+        rc = lib().qmc_generating_vector_noalloc(N, dim, C.c_void_p(torch.cuda.current_stream(dev).cuda_stream), _ptr(z, C.c_uint64))
+    if rc:
+        raise QmcError(rc, "qmc_generating_vector_noalloc")
+    return z[:dim]
 
 
 def qmc_cbc_vector(N: int, dim: int, with_criterion: bool = False):

@@ -182,6 +182,18 @@ DevLayout layout(const qmc_tables *t, int m) {
     }                                   \
   } while (0)
 
+// ---- allocation-free variant of the P_2 search (qmc_generating_vector_noalloc) ------------------------------------------
+// Its scratch (candidate vectors + per-block partial sums of qmc_p2_kernel) lives in a file-scope device array of FIXED
+// size: 2 048 + 64 x 296 x 8 = 153 600 bytes, held by every GPU that loads the library until the process exits.  In host
+// code the array's name is a host-side stand-in, NOT a device address: the address is fetched once per device with
+// cudaGetSymbolAddress (that device current) and handed to the kernel.
+#define QMC_NOALLOC_P2Z_BYTES 2048u
+#define QMC_NOALLOC_BYTES (QMC_NOALLOC_P2Z_BYTES + (size_t)QMC_NCAND * QMC_P2_BLOCKS * 8)
+static_assert((size_t)QMC_NCAND * QMC_MAXDIM * 4 <= QMC_NOALLOC_P2Z_BYTES, "candidate block of the P_2 search");
+static __device__ __align__(256) unsigned char qmc_noalloc_scratch[QMC_NOALLOC_BYTES];
+#define QMC_NOALLOC_MAXDEV 64
+unsigned char *noalloc_addr[QMC_NOALLOC_MAXDEV] = {nullptr};  // device address of qmc_noalloc_scratch, per device
+
 int korobov_search(uint64_t N, int dim, cudaStream_t st, unsigned char *ws, size_t p2z_off, size_t p2p_off,
                    uint64_t *z_out) {
   if (dim == 1) {
@@ -651,6 +663,68 @@ int qmc_generating_vector(uint64_t N, int32_t dim, void *cuda_stream, void *dev_
   if (dim > 1 && (!dev_workspace || dev_workspace_bytes < p2p + (size_t)QMC_NCAND * QMC_P2_BLOCKS * 8)) return QMC_ENOMEM;
   return korobov_search(N, dim, static_cast<cudaStream_t>(cuda_stream), static_cast<unsigned char *>(dev_workspace), p2z,
                         p2p, z_out);
+}
+
+int qmc_generating_vector_noalloc(uint64_t N, int32_t dim, void *cuda_stream, uint64_t *z_out) {
+  if (N < 5 || N >= (1ull << 31) || dim < 1 || !z_out) return QMC_EINVAL;
+  if (dim > QMC_MAXDIM) return QMC_ENOMEM;  // beyond what the fixed scratch (and the kernels) are sized for
+  if (dim == 1) {
+    z_out[0] = 1;
+    return QMC_OK;
+  }
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  int dev = 0;
+  CUDA_OK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= QMC_NOALLOC_MAXDEV) return QMC_EINVAL;
+  if (!noalloc_addr[dev]) {  // set-up, once per device, with that device current
+    unsigned char *ptr = nullptr;
+    CUDA_OK(cudaGetSymbolAddress(reinterpret_cast<void **>(&ptr), qmc_noalloc_scratch));
+    if (!ptr) return QMC_ECUDA;
+    noalloc_addr[dev] = ptr;
+  }
+  unsigned char *ws = noalloc_addr[dev];
+  // host side: fixed-size staging (no heap): candidates, their vectors, the partial sums coming back
+  static thread_local uint32_t zc[QMC_NCAND * QMC_MAXDIM];
+  static thread_local uint64_t cand[QMC_NCAND];
+  static thread_local double part[QMC_NCAND * QMC_P2_BLOCKS];
+  std::memset(zc, 0, sizeof zc);
+  int nc = 0, guard = 0;
+  uint64_t state = N;  // the candidate list of korobov_search (R:C13): the same vectors, hence the same answer
+  while (nc < QMC_NCAND && guard++ < 100000) {
+    const uint64_t a = 2 + splitmix64(state) % (N - 3);
+    if (std::gcd(a, N) != 1) continue;
+    cand[nc++] = a;
+  }
+  if (nc == 0) return QMC_EINVAL;
+  for (int c = 0; c < nc; ++c) {
+    uint64_t v = 1;
+    for (int j = 0; j < dim; ++j) {
+      zc[(size_t)c * QMC_MAXDIM + j] = (uint32_t)v;
+      v = mulmod(v, cand[c], N);
+    }
+  }
+  uint32_t *dz = reinterpret_cast<uint32_t *>(ws);
+  double *dp = reinterpret_cast<double *>(ws + QMC_NOALLOC_P2Z_BYTES);
+  // the array keeps the last call's contents: everything read below is written first (candidates by the copy, every
+  // partial [cand][block] by its block), nothing has to start at zero
+  CUDA_OK(cudaMemcpyAsync(dz, zc, sizeof zc, cudaMemcpyHostToDevice, st));
+  qmc_p2_kernel<<<dim3(QMC_P2_BLOCKS, nc), 256, 0, st>>>(dz, dp, (uint32_t)N, dim);
+  CUDA_OK(cudaGetLastError());
+  CUDA_OK(cudaMemcpyAsync(part, dp, (size_t)nc * QMC_P2_BLOCKS * 8, cudaMemcpyDeviceToHost, st));
+  CUDA_OK(cudaStreamSynchronize(st));
+  int best = 0;
+  double bestv = 0.0;
+  for (int c = 0; c < nc; ++c) {
+    double sum = 0.0;
+    for (int b = 0; b < QMC_P2_BLOCKS; ++b) sum += part[(size_t)c * QMC_P2_BLOCKS + b];
+    const double p2 = sum / (double)N - 1.0;
+    if (c == 0 || p2 < bestv || (p2 == bestv && cand[c] < cand[best])) {
+      best = c;
+      bestv = p2;
+    }
+  }
+  for (int j = 0; j < dim; ++j) z_out[j] = zc[(size_t)best * QMC_MAXDIM + j];
+  return QMC_OK;
 }
 
 int qmc_fp64_peak(void *cuda_stream, void *dev_workspace, size_t dev_workspace_bytes, double *flops_out, double *ms_out) {
