@@ -42,7 +42,7 @@ inline void merge_pair(Factors &m, int a, int b, int nw) {
 }
 
 // returns false if some monomial still has more than two factors when the slots run out
-inline bool plan_chunk(ChunkPlan &pl, int first_prod, int max_slots) {
+inline bool plan_chunk(ChunkPlan &pl, int first_prod, int max_slots, bool stop_at_two = false) {
   pl.first_prod = first_prod;
   pl.nslots = pl.first_prod;
   pl.prog.clear();
@@ -74,7 +74,7 @@ inline bool plan_chunk(ChunkPlan &pl, int first_prod, int max_slots) {
           ba = a;
           bb = b;
         }
-    (void)any_big;
+    if (stop_at_two && !any_big) break;   // every monomial is a product of at most two slots: enough for a record
     if (ba < 0) break;                    // every monomial has at most one factor
     if (best < 2) break;                  // a chunk-wide slot must serve at least two monomials
     if (pl.nslots >= max_slots) break;    // leftovers with more than two factors get sector-local products

@@ -170,10 +170,10 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
           }
         }
         f += n * 5.0 + (double)nfree * nfree * 3.0 + nfree * 3.0;  // rho, z, Jacobian entries
-        for (int col = 0; col < n; ++col) {                         // LU of the n x n complex matrix
+        for (int col = 0; col < n; ++col) {                         // elimination of the n x n complex matrix (no pivoting)
           f += F_CMUL;
           const int rem = n - col - 1;
-          if (rem > 0) f += F_CINV + rem * (F_CMUL + rem * (F_CMUL + F_CADD)) + rem * 6.0;
+          if (rem > 0) f += F_CINV + rem * (F_CMUL + rem * (F_CMUL + F_CADD));   // natural order, no pivot search
           // first elimination step: the off-diagonal entries of J = 1 + iB are purely imaginary, a product with one of
           // them is 2 multiplications, not 6 (ptxas folds the zeros; checked against ncu's executed FP64 counters)
           if (col == 0) f -= 4.0 * rem + 4.0 * rem * rem;

@@ -220,7 +220,7 @@ int qmc_build_tables4(qmc_tables *t, int slot_budget, int chunk_bytes_opt, int t
     const int nconst = (int)cc.val.size();
     const int first_prod = 2 * n + 2 + nconst;
     const int max_slots = std::min(QMC2_MAXSLOTS - QMC2_MAXLOCAL, std::max(max_slots_base + std::min(nconst, 6), first_prod + 1));
-    plan_chunk(pl, first_prod, max_slots);
+    plan_chunk(pl, first_prod, max_slots, true);  // a record costs the same with one factor or two: stop at two
     Qmc2Chunk ch;
     ch.sec_begin = s0;
     ch.sec_end = s1;

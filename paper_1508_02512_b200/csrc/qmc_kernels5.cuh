@@ -7,7 +7,7 @@
 //   S4  F^_i(tau), F^_ik(tau) from the record lists of the derivative polynomials;
 //       rho_i = 1 - i lambda (1 - tau_i) F^_i,  z_i = tau_i rho_i,
 //       J_ik = delta_ik [1 - i lambda (1 - 2 tau_i) F^_i] - i lambda tau_i (1 - tau_i) F^_ik   (Eq. 14; R:C12),
-//       det J by LU with row pivoting;
+//       det J by elimination in the natural order (no pivoting: see corner5);
 //   S5  U^(z), F^(z) as sums of complex records;  G_Z = G0 det J prod_{j notin Z} rho_j^alpha_j U^aU0 F^aF0,
 //       Lambda_Z = aU1 ln U + aF1 ln F + sum_j beta_j ln rho_j + L0   (principal logs; -i pi on the negative real axis, R:C11);
 //   S6  product form folded one singular variable at a time with exact series windows (as qmc_fold.cuh, complex).
@@ -174,21 +174,14 @@ __device__ __forceinline__ void corner5(const Qmc5Launch &p, const uint32_t cw, 
       }
     }
   }
+  // det J by elimination WITHOUT pivoting.  J = 1 + i (E + D H) with E, D real diagonal, D = diag(tau (1 - tau)) >= 0 and H
+  // the real symmetric Hessian: J is diagonally similar to 1 + i S, S real symmetric, whose Hermitian part is the identity --
+  // every leading principal minor has modulus >= 1 and elimination in the natural order is stable (no growth beyond that of
+  // S), with the same pivots.  Row exchanges in registers had cost a fifth of the kernel's instructions in moves and selects
+  // (profiles/r02a_final.md).  The oracle pivots; the determinants agree to rounding.
   cd det = cd{1.0, 0.0};
 #pragma unroll
   for (int col = 0; col < NDIM; ++col) {
-#pragma unroll
-    for (int r = col + 1; r < NDIM; ++r) {
-      if (cnorm2(J[r][col]) > cnorm2(J[col][col])) {
-#pragma unroll
-        for (int k = col; k < NDIM; ++k) {
-          cd tmp = J[r][k];
-          J[r][k] = J[col][k];
-          J[col][k] = tmp;
-        }
-        det = cd{-det.re, -det.im};
-      }
-    }
     det = det * J[col][col];
     if (col + 1 < NDIM) {
       const cd ip = cinv(J[col][col]);
