@@ -507,9 +507,9 @@ int launch_v5(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
     p.out_row = persec ? r.a - sb : i;
     p.count_boundary = i == 0 ? 1 : 0;
     p.nslices = nsl[i];
-    p.nprog_r = (uint32_t)(c.nslots - (3 * n + 1));
+    p.nprog_r = (uint32_t)(c.nslots - (2 * n + 1));
     p.prog_r_word = 0;
-    p.first_prod_r_off = (uint32_t)(3 * n + 1) * T * 8u;
+    p.first_prod_r_off = (uint32_t)(2 * n + 1) * T * 8u;
     p.local0_r_off = (uint32_t)c.nslots * T * 8u;
     p.nprog_c = (uint32_t)(nslots_c - (n + 1));
     p.prog_c_word = (uint32_t)(pgr.size() / 4);

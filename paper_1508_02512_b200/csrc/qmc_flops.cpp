@@ -35,9 +35,9 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
   if (sb < 0 || se > nsec || sb >= se) return QMC_EINVAL;
   const bool cplx = t->lambda > 0.0;
   // S1-S3, once per (point, shift): u = r/N (IEEE division), y = u + Delta (wrap), t = y^2 (3 - 2y), w *= 6 y (1 - y),
-  // ln t (table logarithm), 1/t (reciprocal)
+  // ln t (table logarithm)
   // (real path: r / N as r * RN(1/N) with one FMA correction, 5 flops; complex path: the division routine)
-  double per_point = n * ((cplx ? F_DIV : 5.0) + 2.0 + 4.0 + 4.0 + 18.0 + 6.0);
+  double per_point = n * ((cplx ? F_DIV : 5.0) + 2.0 + 4.0 + 4.0 + 18.0);
   if (!cplx)  // the chunks' product slots, once per point and chunk touched
     for (const Qmc2Chunk &c : t->chunks)
       if (c.sec_end > sb && c.sec_begin < se) per_point += (double)(c.nslots - (2 * n + 2 + c.nconst));
@@ -145,8 +145,9 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
         if (s.beta[j]) ++nbeta;
       }
       f = 3.0 * (1 + nL0);
+      if (ns > 0) f += (ns - 1) + 6.0 + 1.0;   // 1 / prod t_k of the singular variables, onto G0
       for (int j = 0; j < n; ++j)
-        if (s.alpha[j] == -1) f += 1.0 + 2.0 * std::max(0, K - 2);
+        if (s.alpha[j] == -1) f += 2.0 + 2.0 * std::max(0, K - 3);   // t_k / beta_k, beta_k ln t_k, (.)^p / p!
       for (int Z = 0; Z < nc; ++Z) {
         auto in_Z = [&](int j) { return pos_of[j] >= 0 && (Z >> pos_of[j] & 1); };
         int nfree = 0;
@@ -196,7 +197,7 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
       for (int l = 0; l < ns; ++l)
         for (int Z = 0; Z < (1 << l); ++Z) {
           const int len = ns - l + t->kmax + __builtin_popcount(Z) + 1;
-          f += 4.0 * (len - 1) + 2.0 + 2.0 * len * (len - 1);
+          f += 2.0 * (len - 1) + 2.0 + 2.0 * len * (len - 1);
         }
       f += 4.0 * K;
     }

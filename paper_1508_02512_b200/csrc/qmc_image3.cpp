@@ -135,9 +135,16 @@ int qmc_build_image3(qmc_tables *t, int slots_r_opt, int slots_c_opt, int chunk_
   if (!(t->lambda > 0.0) || nsec == 0) return QMC_OK;
   const int T = QMC3_THREADS;
   const int npoly = n + n * (n + 1) / 2 + 2, nderiv = npoly - 2;
-  int max_r = std::min(QMC3_MAXSLOTS_R, 3 * n + 1 + 20), max_c = std::min(QMC3_MAXSLOTS_C, n + 1 + 12);
+  int max_r = std::min(QMC3_MAXSLOTS_R, 2 * n + 1 + 20), max_c = std::min(QMC3_MAXSLOTS_C, n + 1 + 12);
+  if (n == 5) {
+    // n = 5 runs three 128-thread blocks per SM (168 registers, qmc_kernels5.cuh), which needs <= 75 KB of shared memory per
+    // block: 8 KB logarithm table + 1 KB per real slot + 2 KB per complex slot.  Measured on B200 (cfg5, ms per step):
+    // budgets 31/18 (two blocks) 202; 24/14 151; 21/14 152; 19/13 153; 21/15 (76 KB: two blocks again) 203
+    max_r = 2 * n + 1 + 13;
+    max_c = n + 1 + 8;
+  }
   double chunk_bytes = 16000.0;
-  if (slots_r_opt > 0) max_r = std::min(QMC3_MAXSLOTS_R, std::max(3 * n + 2, slots_r_opt));
+  if (slots_r_opt > 0) max_r = std::min(QMC3_MAXSLOTS_R, std::max(2 * n + 2, slots_r_opt));
   if (slots_c_opt > 0) max_c = std::min(QMC3_MAXSLOTS_C, std::max(n + 2, slots_c_opt));
   if (chunk_bytes_opt > 0) chunk_bytes = std::max(1000.0, (double)chunk_bytes_opt);
 
@@ -178,7 +185,7 @@ int qmc_build_image3(qmc_tables *t, int slots_r_opt, int slots_c_opt, int chunk_
       for (int p = nderiv; p < npoly; ++p)
         for (const Mono3 &m : polys[si][p]) pc.mono.push_back(factors_of(m.e, n));
     }
-    plan_chunk(pr, 3 * n + 1, max_r);
+    plan_chunk(pr, 2 * n + 1, max_r);
     plan_chunk(pc, n + 1, max_c);
     // ---- emit --------------------------------------------------------------------------------------------------
     Qmc2Chunk ch;
@@ -202,7 +209,7 @@ int qmc_build_image3(qmc_tables *t, int slots_r_opt, int slots_c_opt, int chunk_
     for (auto &q : pc.prog) { put32(p5c, (uint32_t)q.first * T * 16u); put32(p5c, (uint32_t)q.second * T * 16u); }
     pad4(p5c);
     const size_t tab5_mark = t->tab5.size();
-    const uint32_t ONE_R = (uint32_t)(3 * n) * T * 8u, ONE_C = (uint32_t)n * T * 16u;
+    const uint32_t ONE_R = (uint32_t)(2 * n) * T * 8u, ONE_C = (uint32_t)n * T * 16u;
     auto rec_r = [&](double c, const Factors &f) {
       Qmc2Rec r;
       r.c = c;

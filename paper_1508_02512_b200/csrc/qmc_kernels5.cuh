@@ -1,7 +1,7 @@
 // Evaluation kernel of the complex path (physical region, contour deformation), "version 5", sm_100a.  Steps S1-S7.
 //
 // One thread = one lattice point; two slot tables per thread in shared memory: a REAL one at the lattice point (t_j,
-// ln t_j, 1/t_j, 1, products) that serves the gradient and Hessian polynomials of F^ -- emitted by qmc_prepare as record
+// ln t_j, 1, products) that serves the gradient and Hessian polynomials of F^ -- emitted by qmc_prepare as record
 // lists of their own -- and a COMPLEX one over the deformed variables z_j, refilled at every corner, that serves U^(z),
 // F^(z).  Per corner Z of a sector (real point tau = t with the variables of Z set to 0):
 //   S4  F^_i(tau), F^_ik(tau) from the record lists of the derivative polynomials;
@@ -24,7 +24,9 @@
 #include "qmc_kernels4.cuh"  // fast_log (64 x 8 table), fast_rcp, slot_at, u2d
 
 #ifndef QMC5_MINB
-#define QMC5_MINB(NDIM) ((NDIM) <= 4 ? 4 : 2)  // resident 128-thread blocks per SM the register budget is sized for
+// resident 128-thread blocks per SM the register budget is sized for: n <= 4: 4 (128 registers); n = 5: 3 (168 registers,
+// 92 bytes of spills; needs <= 75 KB of shared memory per block: the slot budgets of qmc_image3.cpp); n = 6: 2 (255)
+#define QMC5_MINB(NDIM) ((NDIM) <= 4 ? 4 : (NDIM) == 5 ? 3 : 2)
 #endif
 
 namespace qmc5 {
@@ -277,7 +279,7 @@ __device__ __forceinline__ void corner5(const Qmc5Launch &p, const uint32_t cw, 
 
 template <int NS, int K>
 struct Ctx5 {
-  double invt[NS > 0 ? NS : 1], invbeta[NS > 0 ? NS : 1];
+  double bt[NS > 0 ? NS : 1];  // t_k / beta_k (the 1/t_k of Eq. 12 are factored out of the fold: one reciprocal onto G0)
   double cL[NS > 0 ? NS : 1][K > 1 ? K - 1 : 1];
   cd W[1 << NS], Lam[1 << NS];  // index Z = set of singular positions set to zero
 };
@@ -290,14 +292,14 @@ struct Fold5 {
     cd a[LEN - 1], b[LEN];
     Fold5<NS, KMAX, K, LEVEL + 1, ZMASK>::eval(c, a);
     Fold5<NS, KMAX, K, LEVEL + 1, ZMASK | (1 << LEVEL)>::eval(c, b);
-    const double it = c.invt[LEVEL], ib = c.invbeta[LEVEL];
+    const double bt = c.bt[LEVEL];
     cd d[LEN - 1];
 #pragma unroll
-    for (int i = 0; i < LEN - 1; ++i) d[i] = it * (a[i] - b[i]);
-    out[0] = ib * b[0];
+    for (int i = 0; i < LEN - 1; ++i) d[i] = a[i] - b[i];
+    out[0] = bt * b[0];
 #pragma unroll
     for (int i = 1; i < LEN; ++i) {
-      cd s = ib * b[i] + d[i - 1];
+      cd s = bt * b[i] + d[i - 1];
 #pragma unroll
       for (int p = 1; p < i; ++p) s = s + c.cL[LEVEL][p] * d[i - 1 - p];
       out[i] = s;
@@ -329,7 +331,13 @@ __device__ __forceinline__ void sector5(const Qmc5Launch &p, const uint32_t o, u
     if (i + 1 < nlocal_r) *reinterpret_cast<double *>(slr + p.local0_r_off + (i + 1) * (T * 8)) = slot_at(slr, pw.z) * slot_at(slr, pw.w);
   }
   uint32_t rw = o + h0.z;
-  const double G0 = qmc4::rec_val(p.tab[rw], slr);
+  double G0 = qmc4::rec_val(p.tab[rw], slr);
+  if (NS > 0) {  // the 1/t_k of the singular variables (Eq. 12), factored out of the fold: one reciprocal of their product
+    double pt = slot_at(slr, (h1.x & 255u) * (T * 8));
+#pragma unroll
+    for (int k = 1; k < NS; ++k) pt *= slot_at(slr, ((h1.x >> (8 * k)) & 255u) * (T * 8));
+    G0 *= fast_rcp(pt);
+  }
   ++rw;
   double L0 = 0.0;
 #pragma unroll 2
@@ -356,8 +364,7 @@ __device__ __forceinline__ void sector5(const Qmc5Launch &p, const uint32_t o, u
 #pragma unroll
     for (int k = 0; k < NS; ++k) {
       const uint32_t j = (h1.x >> (8 * k)) & 255u;
-      c.invt[k] = slot_at(slr, (2 * NDIM + j) * (T * 8));
-      c.invbeta[k] = ibv[k];
+      c.bt[k] = ibv[k] * slot_at(slr, j * (T * 8));
       const double Lk = bv[k] * slot_at(slr, (NDIM + j) * (T * 8));
       c.cL[k][0] = 1.0;
 #pragma unroll
@@ -401,7 +408,7 @@ __global__ void __launch_bounds__(QMC3_THREADS, QMC5_MINB(NDIM)) qmc5_eval_kerne
   for (int i = tid; i < QMC4_LOG_ENTRIES * QMC4_LOG_COPIES; i += T)
     logtab[i] = reinterpret_cast<const double2 *>(p.logtab)[i / QMC4_LOG_COPIES];
   for (int i = tid; i < p.m * NDIM; i += T) shf[i] = p.shifts[i];
-  slots_r[3 * NDIM * T + tid] = 1.0;                     // the constant slots
+  slots_r[2 * NDIM * T + tid] = 1.0;                     // the constant slots
   slots_c[NDIM * T + tid] = make_double2(1.0, 0.0);
   __syncthreads();
 
@@ -449,7 +456,6 @@ __global__ void __launch_bounds__(QMC3_THREADS, QMC5_MINB(NDIM)) qmc5_eval_kerne
         }
         reinterpret_cast<double *>(slr)[j * T] = tj;
         reinterpret_cast<double *>(slr)[(NDIM + j) * T] = fast_log(tj, tabq);
-        reinterpret_cast<double *>(slr)[(2 * NDIM + j) * T] = fast_rcp(tj);
         uint32_t rn = r[j] + dz[j];
         r[j] = rn >= N ? rn - N : rn;
       }

@@ -85,7 +85,7 @@ struct Qmc2Chunk {      // host description of one chunk
 };
 
 // ---- planning image of the complex path ("version 3": host only; the kernels read the version-5 tables) ------
-// Same idea as version 2, with TWO slot tables per thread: a REAL one at the lattice point (t_j, ln t_j, 1/t_j, 1,
+// Same idea as version 2, with TWO slot tables per thread: a REAL one at the lattice point (t_j, ln t_j, 1,
 // products) that serves the gradient and Hessian polynomials of F^ -- emitted by qmc_prepare as record lists of their
 // own -- and the regular-variable factors; and a COMPLEX one over the deformed variables z_j (z_j, 1, products),
 // refilled at every corner, that serves U^(z) and F^(z).  Records are sorted per polynomial by group; a corner Z keeps
