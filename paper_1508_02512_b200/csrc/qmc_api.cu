@@ -1107,9 +1107,9 @@ int qmc_tables_describe(const qmc_tables *t, char *buf, size_t len) {
   o += line;
   for (size_t c = 0; c < t->chunks.size(); ++c) {
     const Qmc2Chunk &ch = t->chunks[c];
-    std::snprintf(line, sizeof line, "chunk %zu: sectors [%d,%d) slots %d (constants %d, products %d) tables %u B records %d (beyond the dense positions %d) local products %d (max local slots %d) cost %.0f\n", c,
+    std::snprintf(line, sizeof line, "chunk %zu: sectors [%d,%d) slots %d (constants %d, products %d) tables %u B records %d (one-factor %d, beyond the dense positions %d) local products %d (max local slots %d) cost %.0f\n", c,
                   ch.sec_begin, ch.sec_end, ch.nslots, ch.nconst, ch.nslots - (2 * t->n + 2 + ch.nconst), ch.tab_words * 16u, ch.nrec,
-                  ch.noverflow, ch.nlocal, ch.max_local, ch.cost);
+                  ch.nsingle, ch.noverflow, ch.nlocal, ch.max_local, ch.cost);
     o += line;
   }
   for (size_t c = 0; c < t->chunks3.size(); ++c) {  // complex path

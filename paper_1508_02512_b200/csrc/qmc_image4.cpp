@@ -303,6 +303,7 @@ int qmc_build_tables4(qmc_tables *t, int slot_budget, int chunk_bytes_opt, int t
           const std::vector<const Factors *> &R = grp[which][g];
           const int cnt = (int)R.size();
           ch.nrec += cnt;
+          for (const Factors *f : R) ch.nsingle += f->size() < 2;
           if (cap < 1) return QMC_EUNSUPPORTED;
           if (cnt <= cap) {
             for (int q = 0; q < cap; ++q) {

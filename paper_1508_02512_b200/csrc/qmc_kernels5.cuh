@@ -41,7 +41,7 @@ using qmcdev::cnorm2;
 
 // 1 / a with the MUFU.RCP64H + cubic-step reciprocal of the real path (|a|^2 is a normal number: pivots of 1 + iS have
 // modulus >= 1, U^, F^, rho_j are O(1)) instead of the IEEE division routine: six of them per corner
-__device__ __forceinline__ cd cinv(cd a) {
+__device__ __forceinline__ cd cinv5(cd a) {
   const double d = fast_rcp(a.re * a.re + a.im * a.im);
   return cd{a.re * d, -a.im * d};
 }
@@ -191,7 +191,7 @@ __device__ __forceinline__ void corner5(const Qmc5Launch &p, const uint32_t cw, 
   for (int col = 0; col < NDIM; ++col) {
     det = det * J[col][col];
     if (col + 1 < NDIM) {
-      const cd ip = cinv(J[col][col]);
+      const cd ip = cinv5(J[col][col]);
 #pragma unroll
       for (int r = col + 1; r < NDIM; ++r) {
         const cd f = J[r][col] * ip;
@@ -271,14 +271,14 @@ __device__ __forceinline__ void corner5(const Qmc5Launch &p, const uint32_t cw, 
       for (int q = 0; q < -b; ++q) qd = qd * rho[j];
     }
   }
-  cd Lam = clog5(qn * cinv(qd), tabq);
+  cd Lam = clog5(qn * cinv5(qd), tabq);
   Lam.im = fma((double)rintf((th - (float)Lam.im) * 0.15915494f), 6.28318530717958647692, Lam.im);
   Lam.re += L0;
   if (E::aU0 > 0) num = num * cpow_c<(E::aU0 > 0 ? E::aU0 : 0)>(Uv);
   if (E::aU0 < 0) den = den * cpow_c<(E::aU0 < 0 ? -E::aU0 : 0)>(Uv);
   if (E::aF0 > 0) num = num * cpow_c<(E::aF0 > 0 ? E::aF0 : 0)>(Fv);
   if (E::aF0 < 0) den = den * cpow_c<(E::aF0 < 0 ? -E::aF0 : 0)>(Fv);
-  Wout = num * cinv(den);
+  Wout = num * cinv5(den);
   Lout = Lam;
 }
 

@@ -78,7 +78,7 @@ struct Qmc2Chunk {      // host description of one chunk
   int nslots = 0;     // chunk-wide slots (base + constants + products)
   int nconst = 0;     // coefficient constants (real path)
   int max_local = 0;  // largest number of sector-local product slots in the chunk
-  int nrec = 0, nlocal = 0, noverflow = 0;  // monomial records / sector-local products / monomials beyond the dense positions (describe)
+  int nrec = 0, nsingle = 0, nlocal = 0, noverflow = 0;  // monomial records / sector-local products / monomials beyond the dense positions (describe)
   uint32_t tab_words = 0;                 // 16-byte words of sector blocks (real path)
   uint32_t prog_off = 0, prog_bytes = 0;  // complex path: chunk header + slot programs in image3
   double cost = 0.0;                      // modelled flops per point (load balancing)
