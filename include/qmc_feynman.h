@@ -199,6 +199,24 @@ int qmc_generating_vector_noalloc(uint64_t N, int32_t dim, void *cuda_stream, ui
  * QMC_EINVAL; QMC_ENOMEM if the host work arrays (about 50 N bytes) cannot be allocated.  z_out[dim] caller-owned;
  * e2_out[dim] (NULL = not wanted) receives the criterion after each component. */
 int qmc_cbc_vector(uint64_t N, int32_t dim, uint64_t *z_out, double *e2_out);
+/* Embedded lattice sequence (P:172 names better lattices as the source of the O(1/n) rate; R:C26): rules with
+ * N = 2^k points, k_min <= k <= k_max, that share ONE generating vector with odd components.  The even lattice indices of level
+ * k + 1 are the points of level k ({2i z / 2^(k+1)} = {i z / 2^k}, Eq. 17), so raising N re-uses every point already evaluated.
+ * qmc_embedded_vector: Korobov form z = (1, a, a^2, ...) mod 2^k_max, `a` odd, minimising over a fixed list of 64 candidates the
+ * worst level of P_2(z mod 2^k; 2^k) / ((k ln 2)^dim / 4^k) (the P_2 criterion of R:C13 per level, relative to its expected rate).
+ * Runs on the device (workspace as for qmc_generating_vector).  3 <= k_min <= k_max <= 30, dim <= 8. */
+int qmc_embedded_vector(int32_t k_min, int32_t k_max, int32_t dim, void *cuda_stream, void *dev_workspace,
+                        size_t dev_workspace_bytes, uint64_t *z_out);
+/* S1-S8 over the levels k_min, k_min + 1, ... of an embedded sequence with generating vector z (odd components, z mod 2^k at
+ * level k) and the m shift vectors of `seed`: level k_min evaluates all 2^k_min indices, every further level only its odd indices
+ * (qmc_run.index_begin = 1, index_step = 2), and the per-shift estimates combine as Q_k = Q_{k-1} / 2 + (odd part), each part
+ * carrying the 1/N of Eq. 18 of its own level.  Stops after the first level whose estimated relative error of the highest order
+ * kept (R:C17) is <= target_rel_err (<= 0: runs to k_max).  Fused mode; `out` receives coeff, err, shift_totals [K][m][2] of
+ * the level reached (per-sector outputs must be NULL), the counters and times summed over the levels; *k_reached the level,
+ * *points_evaluated = 2^k_reached lattice points per shift (a restart at every level would cost 2^(k+1) - 2^k_min). */
+int qmc_integrate_embedded(const qmc_tables *t, int32_t k_min, int32_t k_max, double target_rel_err, int32_t m, uint64_t seed,
+                           const uint64_t *z, void *cuda_stream, void *dev_workspace, size_t dev_workspace_bytes,
+                           qmc_result *out, int32_t *k_reached, int64_t *points_evaluated);
 /* m shift vectors from the SplitMix64 stream keyed by seed: Delta = (u64 >> 11) * 2^-53, shift-major (R:C14) */
 int qmc_shifts(uint64_t seed, int32_t m, int32_t dim, double *shifts_out);
 /* Laurent series of  e^{eg * eps * gamma_E} * base^{p0 + p1 eps} * Gamma(g0 + g1 eps),  g0 a non-negative integer,

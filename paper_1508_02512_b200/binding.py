@@ -105,6 +105,12 @@ def lib():
         L.qmc_generating_vector.argtypes = [C.c_uint64, C.c_int32, C.c_void_p, C.c_void_p, C.c_size_t, C.POINTER(C.c_uint64)]
         L.qmc_generating_vector_noalloc.restype = C.c_int
         L.qmc_generating_vector_noalloc.argtypes = [C.c_uint64, C.c_int32, C.c_void_p, C.POINTER(C.c_uint64)]
+        L.qmc_embedded_vector.restype = C.c_int
+        L.qmc_embedded_vector.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_size_t, C.POINTER(C.c_uint64)]
+        L.qmc_integrate_embedded.restype = C.c_int
+        L.qmc_integrate_embedded.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_int32, C.c_uint64, C.POINTER(C.c_uint64),
+                                             C.c_void_p, C.c_void_p, C.c_size_t, C.POINTER(qmc_result), C.POINTER(C.c_int32),
+                                             C.POINTER(C.c_int64)]
         L.qmc_shifts.restype = C.c_int
         L.qmc_shifts.argtypes = [C.c_uint64, C.c_int32, C.c_int32, C.POINTER(C.c_double)]
         L.qmc_prefactor_series.restype = C.c_int
@@ -394,6 +400,40 @@ def qmc_generating_vector_noalloc(N: int, dim: int, device="cuda:0") -> np.ndarr
     if rc:
         raise QmcError(rc, "qmc_generating_vector_noalloc")
     return z[:dim]
+
+
+def qmc_embedded_vector(k_min: int, k_max: int, dim: int, device="cuda:0") -> np.ndarray:
+    """Generating vector (odd components) shared by the lattices N = 2^k, k_min <= k <= k_max (embedded sequence)."""
+    import torch
+    dev = torch.device(device)
+    with torch.cuda.device(dev):
+        ws = torch.empty(1 << 20, dtype=torch.uint8, device=dev)
+        z = np.zeros(dim, dtype=np.uint64)
+        rc = lib().qmc_embedded_vector(k_min, k_max, dim, C.c_void_p(torch.cuda.current_stream(dev).cuda_stream),
+                                       C.c_void_p(ws.data_ptr()), ws.numel(), _ptr(z, C.c_uint64))
+    if rc:
+        raise QmcError(rc, "qmc_embedded_vector")
+    return z
+
+
+def qmc_integrate_embedded(t: Tables, k_min: int, k_max: int, m: int, seed: int, z, target_rel_err: float = 0.0,
+                           device="cuda:0", stream=None):
+    """qmc_integrate_embedded: levels 2^k_min .. of an embedded lattice sequence, each level evaluating only its new (odd)
+    indices.  Returns (Result, k_reached, points_evaluated_per_shift)."""
+    import torch
+    dev = torch.device(device)
+    with torch.cuda.device(dev):
+        ws = _workspace(t, 1 << k_max, m, dev)
+        st = stream if stream is not None else torch.cuda.current_stream(dev)
+        res, arrays = _make_result(t, m, 0, False)
+        za = np.ascontiguousarray(z, dtype=np.uint64)
+        kr, npts = C.c_int32(0), C.c_int64(0)
+        rc = lib().qmc_integrate_embedded(t._h, k_min, k_max, float(target_rel_err), m, seed, _ptr(za, C.c_uint64),
+                                          C.c_void_p(st.cuda_stream), C.c_void_p(ws.data_ptr()), ws.numel(), C.byref(res),
+                                          C.byref(kr), C.byref(npts))
+        if rc:
+            raise QmcError(rc, "qmc_integrate_embedded")
+    return _wrap_result(res, arrays), int(kr.value), int(npts.value)
 
 
 def qmc_cbc_vector(N: int, dim: int, with_criterion: bool = False):

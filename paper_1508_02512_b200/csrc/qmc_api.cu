@@ -727,6 +727,116 @@ int qmc_generating_vector_noalloc(uint64_t N, int32_t dim, void *cuda_stream, ui
   return QMC_OK;
 }
 
+// ---- embedded lattice sequence (R:C26) --------------------------------------------------------------
+// N = 2^k with ODD generating-vector components: the even indices of level k + 1 are the lattice of level k
+// ({2i z / 2^(k+1)} = {i z / 2^k}), so raising N re-uses every point already evaluated and only the odd indices are new.
+int qmc_embedded_vector(int32_t k_min, int32_t k_max, int32_t dim, void *cuda_stream, void *dev_workspace,
+                        size_t dev_workspace_bytes, uint64_t *z_out) {
+  if (k_min < 3 || k_max < k_min || k_max > 30 || dim < 1 || dim > QMC_MAXDIM || !z_out) return QMC_EINVAL;
+  if (dim == 1) {
+    z_out[0] = 1;
+    return QMC_OK;
+  }
+  const size_t p2z = 0, p2p = align256((size_t)QMC_NCAND * QMC_MAXDIM * 4);
+  if (!dev_workspace || dev_workspace_bytes < p2p + (size_t)QMC_NCAND * QMC_P2_BLOCKS * 8) return QMC_ENOMEM;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  unsigned char *ws = static_cast<unsigned char *>(dev_workspace);
+  const uint64_t Nmax = 1ull << k_max;
+  // candidates: Korobov form z = (1, a, a^2, ...) mod 2^k_max with odd a from a SplitMix64 stream keyed by (k_max, dim)
+  std::vector<uint64_t> cand;
+  uint64_t state = ((uint64_t)k_max << 8) | (uint64_t)dim;
+  while ((int)cand.size() < QMC_NCAND) cand.push_back((splitmix64(state) % Nmax) | 1ull);
+  std::vector<uint64_t> zfull((size_t)QMC_NCAND * QMC_MAXDIM, 0);
+  for (int c = 0; c < QMC_NCAND; ++c) {
+    uint64_t v = 1;
+    for (int j = 0; j < dim; ++j) {
+      zfull[(size_t)c * QMC_MAXDIM + j] = v;
+      v = mulmod(v, cand[c], Nmax);
+    }
+  }
+  // criterion: the worst level of P_2(z mod 2^k; 2^k) relative to the reference rate (k ln 2)^dim / 4^k
+  std::vector<double> worst(QMC_NCAND, 0.0), part((size_t)QMC_NCAND * QMC_P2_BLOCKS);
+  std::vector<uint32_t> zc((size_t)QMC_NCAND * QMC_MAXDIM);
+  uint32_t *dz = reinterpret_cast<uint32_t *>(ws + p2z);
+  double *dp = reinterpret_cast<double *>(ws + p2p);
+  for (int k = k_min; k <= k_max; ++k) {
+    const uint64_t N = 1ull << k;
+    for (size_t i = 0; i < zc.size(); ++i) zc[i] = (uint32_t)(zfull[i] & (N - 1));
+    CUDA_OK(cudaMemcpyAsync(dz, zc.data(), zc.size() * 4, cudaMemcpyHostToDevice, st));
+    qmc_p2_kernel<<<dim3(QMC_P2_BLOCKS, QMC_NCAND), 256, 0, st>>>(dz, dp, (uint32_t)N, dim);
+    CUDA_OK(cudaGetLastError());
+    CUDA_OK(cudaMemcpyAsync(part.data(), dp, part.size() * 8, cudaMemcpyDeviceToHost, st));
+    CUDA_OK(cudaStreamSynchronize(st));
+    const double ref = std::pow((double)k * 0.6931471805599453, (double)dim) / ((double)N * (double)N);
+    for (int c = 0; c < QMC_NCAND; ++c) {
+      double sum = 0.0;
+      for (int b = 0; b < QMC_P2_BLOCKS; ++b) sum += part[(size_t)c * QMC_P2_BLOCKS + b];
+      worst[c] = std::max(worst[c], (sum / (double)N - 1.0) / ref);
+    }
+  }
+  int best = 0;
+  for (int c = 1; c < QMC_NCAND; ++c)
+    if (worst[c] < worst[best] || (worst[c] == worst[best] && cand[c] < cand[best])) best = c;
+  for (int j = 0; j < dim; ++j) z_out[j] = zfull[(size_t)best * QMC_MAXDIM + j];
+  return QMC_OK;
+}
+
+int qmc_integrate_embedded(const qmc_tables *t, int32_t k_min, int32_t k_max, double target_rel_err, int32_t m, uint64_t seed,
+                           const uint64_t *z, void *cuda_stream, void *dev_workspace, size_t dev_workspace_bytes,
+                           qmc_result *out, int32_t *k_reached, int64_t *points_evaluated) {
+  if (!t || !out || !z || k_min < 3 || k_max < k_min || k_max > 30 || m < 2) return QMC_EINVAL;
+  if (out->sector_coeff || out->sector_err || out->shift_sums) return QMC_EINVAL;  // totals only
+  const int n = t->n, K = t->kmax - t->kmin + 1;
+  for (int j = 0; j < n; ++j)
+    if (!(z[j] & 1ull)) return QMC_EINVAL;  // odd components: coprime to every 2^k
+  std::vector<double> T((size_t)K * m * 2, 0.0), part((size_t)K * m * 2), coeff((size_t)K * 2), err((size_t)K * 2);
+  int64_t npts = 0, counters[4] = {0, 0, 0, 0};
+  double kms = 0.0, ems = 0.0;
+  int64_t h2d = 0, d2h = 0;
+  int launches = 0, kr = k_min;
+  for (int k = k_min; k <= k_max; ++k) {
+    const uint64_t N = 1ull << k;
+    uint64_t zk[QMC_MAXDIM] = {0};
+    for (int j = 0; j < n; ++j) zk[j] = z[j] & (N - 1);
+    qmc_run run;
+    std::memset(&run, 0, sizeof run);
+    run.z = zk;
+    run.mode = 1;
+    run.tables_resident = k > k_min ? 2 : 0;  // the logarithm table and the shift vectors of the first level stay in the workspace
+    if (k > k_min) {  // only the odd indices are new
+      run.index_begin = 1;
+      run.index_step = 2;
+      run.index_count = N / 2;
+    }
+    qmc_result r;
+    std::memset(&r, 0, sizeof r);
+    r.shift_totals = part.data();
+    const int rc = qmc_integrate_ex(t, N, m, seed, &run, cuda_stream, dev_workspace, dev_workspace_bytes, &r);
+    if (rc != QMC_OK) return rc;
+    // Eq. 18 at level k: (1/N) sum over all indices = half of the level below + the odd part (both already carry their 1/N)
+    for (size_t i = 0; i < T.size(); ++i) T[i] = (k > k_min ? 0.5 * T[i] : 0.0) + part[i];
+    npts += (int64_t)(k > k_min ? N / 2 : N);
+    for (int q = 0; q < 4; ++q) counters[q] += r.counters[q];
+    kms += r.kernel_ms; ems += r.eval_kernel_ms; h2d += r.h2d_bytes; d2h += r.d2h_bytes; launches += r.kernel_launches;
+    qmc_statistics(T.data(), K, m, coeff.data(), err.data());
+    kr = k;
+    if (target_rel_err > 0.0) {  // reading C17 on the highest order kept (eps^k_max)
+      const double re = coeff[2 * (K - 1)], im = coeff[2 * (K - 1) + 1];
+      const double mod = std::sqrt(re * re + im * im);
+      if (mod > 0.0 && std::max(err[2 * (K - 1)], err[2 * (K - 1) + 1]) <= target_rel_err * mod) break;
+    }
+  }
+  if (out->coeff) std::memcpy(out->coeff, coeff.data(), coeff.size() * 8);
+  if (out->err) std::memcpy(out->err, err.data(), err.size() * 8);
+  if (out->shift_totals) std::memcpy(out->shift_totals, T.data(), T.size() * 8);
+  for (int q = 0; q < 4; ++q) out->counters[q] = counters[q];
+  out->kernel_ms = kms; out->eval_kernel_ms = ems; out->h2d_bytes = h2d; out->d2h_bytes = d2h;
+  out->kernel_launches = launches; out->mode_used = 1;
+  if (k_reached) *k_reached = kr;
+  if (points_evaluated) *points_evaluated = npts;
+  return QMC_OK;
+}
+
 int qmc_fp64_peak(void *cuda_stream, void *dev_workspace, size_t dev_workspace_bytes, double *flops_out, double *ms_out) {
   if (!dev_workspace || dev_workspace_bytes < 8 || !flops_out) return QMC_EINVAL;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);

@@ -380,3 +380,28 @@ def test_index_blocks_of_two_ranks_add_to_the_full_lattice():
     assert np.all(np.abs(tot - full.shift_totals) <= 1e-12 * np.maximum(np.abs(full.shift_totals), scale))
     coeff, err = q.qmc_statistics(tot)
     assert np.allclose(coeff, full.coeff, rtol=1e-11, atol=1e-14)
+
+
+def test_embedded_lattice_sequence():
+    """SURVEY 8(f) f4, reading C26: lattices N = 2^k that share one generating vector with odd components.  (1) the library's
+    vector: odd, Korobov form; (2) the odd-index half of a level against the oracle (per sector, C19 tolerance); (3) walking up
+    the levels (each evaluating only its new points) gives the estimate of a direct run at N = 2^k on the same vector and
+    shifts; (4) the early stop; on the real path and on the complex path."""
+    z = q.qmc_embedded_vector(10, 18, 3)
+    assert all(int(v) & 1 for v in z) and int(z[2]) == (int(z[1]) * int(z[1])) % (1 << 18)
+    for wl, zz in ((qi.massless_box(), z), (qi.massive_box(), z)):
+        N = 1 << 12
+        parity(wl, N, 3, z=zz % N, index_range=(1, 2, N // 2))                 # the new points of level 12
+        t = q.qmc_prepare(wl, eps_order=wl.eps_order, lam=wl.lam)
+        m = 8
+        r, k, npts = q.qmc_integrate_embedded(t, 10, 15, m, wl.seed, zz)        # target 0: runs to k_max
+        assert (k, npts) == (15, 1 << 15)
+        d = q.qmc_integrate(t, 1 << 15, m, z=zz % (1 << 15), seed=wl.seed)      # all 2^15 points in one go
+        scale = np.maximum(np.abs(d.shift_totals), np.abs(d.shift_totals).max())
+        assert np.all(np.abs(r.shift_totals - d.shift_totals) <= 1e-12 * scale)
+        assert np.allclose(r.coeff, d.coeff, rtol=1e-11, atol=1e-14) and np.allclose(r.err.real, d.err.real, rtol=1e-6, atol=1e-16)
+        r2, k2, n2 = q.qmc_integrate_embedded(t, 10, 18, m, wl.seed, zz, target_rel_err=1e-5)
+        c0, e0 = r2.coeff[-1], r2.err[-1]
+        assert k2 < 18 and n2 == 1 << k2 and max(e0.real, e0.imag) <= 1e-5 * abs(c0)
+    with pytest.raises(q.QmcError):
+        q.qmc_integrate_embedded(q.qmc_prepare(qi.massless_box()), 10, 12, 4, 1, np.array([1, 2, 5], dtype=np.uint64))   # even component

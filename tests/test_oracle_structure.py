@@ -244,3 +244,24 @@ def test_statistics_match_numpy():
     assert np.allclose(mean, T.mean(axis=1), rtol=0, atol=1e-15)
     assert np.allclose(err.real, T.real.std(axis=1, ddof=1) / 4.0, rtol=1e-13)
     assert np.allclose(err.imag, T.imag.std(axis=1, ddof=1) / 4.0, rtol=1e-13)
+
+
+def test_embedded_lattice_identity_on_the_oracle():
+    """SURVEY 8(f) f4 / reading C26: with odd generating-vector components the even indices of the N = 2^(k+1) lattice are the
+    points of the N = 2^k lattice ({2i z / 2N} = {i z / N}, Eq. 17), so per shift
+    Q(2N) = Q(N) / 2 + (1/2N) sum over odd i -- checked on the oracle's own sums for a sector-decomposed integrand."""
+    from oracle import Oracle
+    wl = qi.massless_box()
+    o = Oracle.from_workload(wl)
+    z = np.array([1, 1237, 1237 * 1237 % 4096], dtype=np.uint64)          # odd components
+    sh = qi.splitmix64_shifts(5, 3, 3)
+    N = 2048
+    S1, A1, _ = o.integrate(N, z % N, sh)
+    S2, A2, _ = o.integrate(2 * N, z % (2 * N), sh)
+    Sodd, Aodd, _ = o.integrate(2 * N, z % (2 * N), sh, index_range=(1, 2, N))
+    assert np.all(np.abs(0.5 * S1 + Sodd - S2) <= 1e-13 * np.maximum(np.abs(S2), A2))
+    # and the points themselves: lattice index 2i at 2N = lattice index i at N
+    import oracle as orc
+    y_even = orc.lattice(2 * N, z % (2 * N), 0, 2 * N, sh[0])[0]
+    y_half = orc.lattice(N, z % N, 0, N, sh[0])[0]
+    assert np.array_equal(np.asarray(y_even)[::2], np.asarray(y_half))
