@@ -204,6 +204,30 @@ def time_to_accuracy_embedded(q, wl, torch, target=1e-5, k_min=14, k_max=22, tra
             "coeff_eps0": [c0.real, c0.imag], "err_eps0": [e0.real, e0.imag], "m": wl.m, "z": [int(v) for v in z]}
 
 
+def allocation_vs_uniform(q, torch, target=1e-5):
+    """SURVEY 8(f) f4, reading C27: per-sector lattice sizes by variance (qmc_integrate_allocated) against the uniform embedded
+    sequence at the same target, same vector and shifts: wall time and integrand evaluations per shift vector."""
+    out = []
+    for wl in (qi.double_box(), qi.nonplanar_vertex()):
+        t = q.qmc_prepare(wl, eps_order=wl.eps_order, lam=wl.lam)
+        z = q.qmc_embedded_vector(13, 24, t.dim)
+        q.qmc_integrate(t, 16381, wl.m, seed=wl.seed)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        r, lev, ev = q.qmc_integrate_allocated(t, 13, 24, wl.m, wl.seed, z, target)
+        ta = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        u, k, npts = q.qmc_integrate_embedded(t, 13, 24, wl.m, wl.seed, z, target_rel_err=target)
+        tu = time.perf_counter() - t0
+        rel = lambda x: float(max(x.err[-1].real, x.err[-1].imag) / abs(x.coeff[-1]))
+        out.append({"workload": wl.name, "target_rel_err": target, "m": wl.m,
+                    "allocated": {"wall_s": ta, "rel_err": rel(r), "evals_per_shift": ev, "launches": r.kernel_launches,
+                                  "sectors_per_level": {int(a): int(b) for a, b in zip(*np.unique(lev, return_counts=True))}},
+                    "uniform": {"wall_s": tu, "rel_err": rel(u), "evals_per_shift": npts * t.n_sectors, "N": 1 << k},
+                    "difference_in_sigma": float(abs(r.coeff[-1] - u.coeff[-1]) / np.hypot(abs(r.err[-1]), abs(u.err[-1])))})
+    return out
+
+
 def convergence(q, wl, transform=0, k_lo=14, k_hi=20):
     """error estimate of the eps^0 coefficient of J against N over the primes below 2^k, and the
     least-squares slope of log(error) against log(N) (the paper claims "close to O(n^-1)")."""
@@ -451,6 +475,7 @@ def run_product(args):
                                 for w, tr in ((qi.nonplanar_vertex(), 0), (qi.nonplanar_vertex(), 2), (qi.double_box(), 2))]
         line["time_to_1e-5_embedded"] = [extra(time_to_accuracy_embedded, q, w, torch, target=1e-5, transform=tr)
                                          for w in (qi.double_box(), qi.nonplanar_vertex()) for tr in (0, 2)]
+        line["allocation_vs_uniform"] = extra(allocation_vs_uniform, q, torch)
         line["convergence"] = [extra(convergence, q, w, tr) for w in (qi.massless_box(), qi.double_box(), qi.nonplanar_vertex())
                                for tr in (0, 2)]
         line["cbc_vs_korobov"] = extra(cbc_vs_korobov, q, dev)

@@ -139,6 +139,10 @@ typedef struct {
   int32_t waves;            /* launch geometry: blocks per resident block slot over all launches of a step (0 = 16) */
   int32_t streams;          /* internal side streams the launches of a step are spread over, 0..8 (0 = default 4;
                                -1 = none: all launches in order on cuda_stream) */
+  const uint8_t *sector_mask; /* [n_sectors] (indexed by sector number), NULL = every sector of [sector_begin, sector_end):
+                               only sectors with a non-zero entry are evaluated.  Fused mode with the table-driven kernels
+                               only (else QMC_EUNSUPPORTED): a launch serves the selected sectors of its chunk, whatever
+                               their positions (qmc_integrate_allocated: one call per lattice size) */
 } qmc_run;
 
 size_t qmc_workspace_bytes(const qmc_tables *t, uint64_t N, int32_t m);
@@ -217,6 +221,19 @@ int qmc_embedded_vector(int32_t k_min, int32_t k_max, int32_t dim, void *cuda_st
 int qmc_integrate_embedded(const qmc_tables *t, int32_t k_min, int32_t k_max, double target_rel_err, int32_t m, uint64_t seed,
                            const uint64_t *z, void *cuda_stream, void *dev_workspace, size_t dev_workspace_bytes,
                            qmc_result *out, int32_t *k_reached, int64_t *points_evaluated);
+/* Per-sector lattice sizes by variance (R:C27), on an embedded sequence (z as for qmc_integrate_embedded):
+ * (1) every sector at N0 = 2^k0 in per-sector mode -> per-sector error estimates e_s of the highest order kept (Eq. 20 per sector);
+ * (2) sizes N_s = (a_s/c_s)^(1/3) (sum_r a_r^(1/3) c_r^(2/3))^(1/2) / tau, a_s = e_s^2 N0^2, c_s = modelled cost of the sector,
+ *     tau = target_rel_err |coefficient|: the cheapest sizes that meet sum_s e_s(N_s)^2 <= tau^2 if errors fall like 1/N,
+ *     rounded up to powers of two in [2^k0, 2^k_max];
+ * (3) maximal runs of neighbouring sectors with one size are evaluated in fused mode; all sectors share the shift vectors, the
+ *     per-shift totals T_k = sum over runs are unbiased whatever the sizes, and Eqs. 19-20 on them give the error bar (R:C16);
+ * (4) while that error is above the target every run climbs one level (only its odd indices are new).
+ * levels_out [n_sectors] (NULL = not wanted): log2 of the final size per sector; *evals_per_shift: integrand evaluations per
+ * shift vector over all stages (a uniform rule costs n_sectors 2^k).  target_rel_err > 0; per-sector outputs must be NULL. */
+int qmc_integrate_allocated(const qmc_tables *t, int32_t k0, int32_t k_max, double target_rel_err, int32_t m, uint64_t seed,
+                            const uint64_t *z, void *cuda_stream, void *dev_workspace, size_t dev_workspace_bytes,
+                            qmc_result *out, int32_t *levels_out, int64_t *evals_per_shift);
 /* m shift vectors from the SplitMix64 stream keyed by seed: Delta = (u64 >> 11) * 2^-53, shift-major (R:C14) */
 int qmc_shifts(uint64_t seed, int32_t m, int32_t dim, double *shifts_out);
 /* Laurent series of  e^{eg * eps * gamma_E} * base^{p0 + p1 eps} * Gamma(g0 + g1 eps),  g0 a non-negative integer,

@@ -55,7 +55,8 @@ class qmc_run(C.Structure):
     _fields_ = [("z", C.POINTER(C.c_uint64)), ("shifts", C.POINTER(C.c_double)),
                 ("index_begin", C.c_uint64), ("index_step", C.c_uint64), ("index_count", C.c_uint64),
                 ("sector_begin", C.c_int32), ("sector_end", C.c_int32), ("mode", C.c_int32),
-                ("tables_resident", C.c_int32), ("kernel", C.c_int32), ("waves", C.c_int32), ("streams", C.c_int32)]
+                ("tables_resident", C.c_int32), ("kernel", C.c_int32), ("waves", C.c_int32), ("streams", C.c_int32),
+                ("sector_mask", C.POINTER(C.c_uint8))]
 
 
 _lib = None
@@ -111,6 +112,10 @@ def lib():
         L.qmc_integrate_embedded.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_int32, C.c_uint64, C.POINTER(C.c_uint64),
                                              C.c_void_p, C.c_void_p, C.c_size_t, C.POINTER(qmc_result), C.POINTER(C.c_int32),
                                              C.POINTER(C.c_int64)]
+        L.qmc_integrate_allocated.restype = C.c_int
+        L.qmc_integrate_allocated.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_int32, C.c_uint64, C.POINTER(C.c_uint64),
+                                              C.c_void_p, C.c_void_p, C.c_size_t, C.POINTER(qmc_result), C.POINTER(C.c_int32),
+                                              C.POINTER(C.c_int64)]
         L.qmc_shifts.restype = C.c_int
         L.qmc_shifts.argtypes = [C.c_uint64, C.c_int32, C.c_int32, C.POINTER(C.c_double)]
         L.qmc_prefactor_series.restype = C.c_int
@@ -231,10 +236,14 @@ def _workspace(t: Tables, N: int, m: int, device):
 
 
 def _make_run(t: Tables, m: int, z, shifts, index_range, sectors, mode: int, resident: int, kernel: int = 0,
-              waves: int = 0, streams: int = 0):
+              waves: int = 0, streams: int = 0, sector_mask=None):
     run = qmc_run()
     run.kernel, run.waves, run.streams = kernel, waves, streams
     keep = []
+    if sector_mask is not None:
+        ma = np.ascontiguousarray(sector_mask, dtype=np.uint8); keep.append(ma)
+        assert ma.shape == (t.n_sectors,)
+        run.sector_mask = _ptr(ma, C.c_uint8)
     if z is not None:
         za = np.ascontiguousarray(z, dtype=np.uint64); keep.append(za)
         run.z = _ptr(za, C.c_uint64)
@@ -278,7 +287,7 @@ def _wrap_result(res, arrays) -> Result:
 
 def qmc_integrate(t: Tables, N: int, m: int, seed: int = 0, *, z: Optional[Sequence[int]] = None,
                   shifts: Optional[np.ndarray] = None, index_range=None, sectors=None, per_sector: bool = False,
-                  mode: int = 0, resident: int = 0, kernel: int = 0, waves: int = 0, streams: int = 0,
+                  mode: int = 0, resident: int = 0, kernel: int = 0, waves: int = 0, streams: int = 0, sector_mask=None,
                   device="cuda:0", stream=None) -> Result:
     """qmc_integrate(tables, N, m, seed) -> Laurent coefficients and errors (qmc_integrate_ex when any of the
     explicit controls is given).  Workspace and stream come from PyTorch."""
@@ -291,7 +300,7 @@ def qmc_integrate(t: Tables, N: int, m: int, seed: int = 0, *, z: Optional[Seque
         st = stream if stream is not None else torch.cuda.current_stream(dev)
         s0, s1 = sectors if sectors is not None else (0, t.n_sectors)
         res, arrays = _make_result(t, m, s1 - s0, per_sector)
-        run, keep = _make_run(t, m, z, shifts, index_range, sectors, mode, resident, kernel, waves, streams)
+        run, keep = _make_run(t, m, z, shifts, index_range, sectors, mode, resident, kernel, waves, streams, sector_mask)
         rc = lib().qmc_integrate_ex(t._h, N, m, seed, C.byref(run), C.c_void_p(st.cuda_stream),
                                     C.c_void_p(ws.data_ptr()), ws.numel(), C.byref(res))
         if rc:
@@ -434,6 +443,26 @@ def qmc_integrate_embedded(t: Tables, k_min: int, k_max: int, m: int, seed: int,
         if rc:
             raise QmcError(rc, "qmc_integrate_embedded")
     return _wrap_result(res, arrays), int(kr.value), int(npts.value)
+
+
+def qmc_integrate_allocated(t: Tables, k0: int, k_max: int, m: int, seed: int, z, target_rel_err: float,
+                            device="cuda:0", stream=None):
+    """qmc_integrate_allocated: per-sector lattice sizes by variance.  Returns (Result, levels[n_sectors], evals_per_shift)."""
+    import torch
+    dev = torch.device(device)
+    with torch.cuda.device(dev):
+        ws = _workspace(t, 1 << k_max, m, dev)
+        st = stream if stream is not None else torch.cuda.current_stream(dev)
+        res, arrays = _make_result(t, m, 0, False)
+        za = np.ascontiguousarray(z, dtype=np.uint64)
+        lev = np.zeros(t.n_sectors, dtype=np.int32)
+        ev = C.c_int64(0)
+        rc = lib().qmc_integrate_allocated(t._h, k0, k_max, float(target_rel_err), m, seed, _ptr(za, C.c_uint64),
+                                           C.c_void_p(st.cuda_stream), C.c_void_p(ws.data_ptr()), ws.numel(), C.byref(res),
+                                           _ptr(lev, C.c_int32), C.byref(ev))
+        if rc:
+            raise QmcError(rc, "qmc_integrate_allocated")
+    return _wrap_result(res, arrays), lev, int(ev.value)
 
 
 def qmc_cbc_vector(N: int, dim: int, with_criterion: bool = False):

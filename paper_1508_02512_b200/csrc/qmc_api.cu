@@ -261,7 +261,8 @@ void mean_err(const double *v, size_t stride, int m, double *mean, double *err) 
 // and joined back into the caller's stream, so that the tail of one launch overlaps the next ones.
 int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t st, uint64_t N, int m, int sb, int se,
               bool persec, uint64_t ibeg, uint64_t istep, uint64_t icount, const uint64_t *z, int sms, int smem_optin,
-              int waves_opt, int streams_opt, int *gx_out, int *rows_out, int *launches_out, size_t *h2d, cudaError_t *ce_out) {
+              int waves_opt, int streams_opt, const uint8_t *mask, int *gx_out, int *rows_out, int *launches_out, size_t *h2d,
+              cudaError_t *ce_out) {
   const int n = t->n, nacc = QMC_MAXSING + t->kmax + 1, T = t->threads_real;
   const size_t budget = (size_t)smem_optin - 1024;
   // shared memory of a launch: logarithm table, shift vectors, reduction scratch, the chunk's slot columns.
@@ -290,7 +291,8 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
       }
       if (b == a) return QMC_ENOMEM;
       Run r = {(int)ci, a, b, 0.0, fixed};
-      for (int s = a; s < b; ++s) r.cost += t->sec_cost[s];
+      for (int s = a; s < b; ++s)
+        if (!mask || mask[s]) r.cost += t->sec_cost[s];
       total_cost += r.cost;
       smem = std::max(smem, r.smem);
       runs.push_back(r);
@@ -307,7 +309,7 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
   std::vector<int> nsl(nitems);
   int max_slices = 1;
   for (int i = 0; i < nitems; ++i) {
-    long long ns = (long long)(nblocks_target * runs[i].cost / total_cost + 0.5);
+    long long ns = total_cost > 0.0 ? (long long)(nblocks_target * runs[i].cost / total_cost + 0.5) : 1;
     if (persec) ns = std::max<long long>(ns, (sms + 4 * m - 1) / (4 * m));  // one small launch per sector: a quarter wave each
     ns = std::max<long long>(1, std::min<long long>({ns, (long long)QMC_MAX_BLOCKS, max_slices_pts}));
     nsl[i] = (int)ns;
@@ -378,9 +380,10 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
       for (int ns = 0; ns <= QMC_MAXSING; ++ns) {
         p.nsb[ns] = k;
         for (int s = r.a; s < r.b; ++s)
-          if (t->sectors[s].nsing == ns) p.secw[k++] = (uint16_t)(p.sec_word + (t->secoff4[s] - w0));
+          if (t->sectors[s].nsing == ns && (!mask || mask[s])) p.secw[k++] = (uint16_t)(p.sec_word + (t->secoff4[s] - w0));
       }
       p.nsb[QMC_MAXSING + 1] = k;
+      if (k == 0) continue;  // no sector of this run is selected (qmc_run.sector_mask): its row of partials stays zero
     }
     cudaStream_t ls = nstreams ? static_cast<cudaStream_t>(t->side_streams[i % nstreams]) : st;
     ce = qmc4_kernel_launch(n, t->L, t->kmax, T, t->tpl_real, dim3((unsigned)nsl[i], (unsigned)m), r.smem, ls, p);
@@ -402,7 +405,8 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
 // ---- version-5 launch (complex path): as version 4, two slot tables per thread ------------------------------------------
 int launch_v5(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t st, uint64_t N, int m, int sb, int se,
               bool persec, uint64_t ibeg, uint64_t istep, uint64_t icount, const uint64_t *z, int sms, int smem_optin,
-              int waves_opt, int streams_opt, int *gx_out, int *rows_out, int *launches_out, size_t *h2d, cudaError_t *ce_out) {
+              int waves_opt, int streams_opt, const uint8_t *mask, int *gx_out, int *rows_out, int *launches_out, size_t *h2d,
+              cudaError_t *ce_out) {
   const int n = t->n, nacc = 2 * (QMC_MAXSING + t->kmax + 1), T = QMC3_THREADS;  // accumulators: (Re, Im) per order
   int max_r = 0, max_c = 0;
   for (size_t ci = 0; ci < t->chunks3.size(); ++ci) {
@@ -435,7 +439,8 @@ int launch_v5(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
       }
       if (b == a) return QMC_ENOMEM;
       Run r = {(int)ci, a, b, 0.0};
-      for (int s = a; s < b; ++s) r.cost += t->sec_cost[s];
+      for (int s = a; s < b; ++s)
+        if (!mask || mask[s]) r.cost += t->sec_cost[s];
       total_cost += r.cost;
       max_nsec = std::max(max_nsec, b - a);
       runs.push_back(r);
@@ -453,7 +458,7 @@ int launch_v5(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
   std::vector<int> nsl(nitems);
   int max_slices = 1;
   for (int i = 0; i < nitems; ++i) {
-    long long ns = (long long)(nblocks_target * runs[i].cost / total_cost + 0.5);
+    long long ns = total_cost > 0.0 ? (long long)(nblocks_target * runs[i].cost / total_cost + 0.5) : 1;
     ns = std::max<long long>(1, std::min<long long>({ns, (long long)QMC_MAX_BLOCKS, max_slices_pts}));
     nsl[i] = (int)ns;
     max_slices = std::max(max_slices, (int)ns);
@@ -525,11 +530,13 @@ int launch_v5(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
       int k = 0;
       for (int ns = 0; ns <= QMC_MAXSING; ++ns)
         for (int s = r.a; s < r.b; ++s)
-          if (t->sectors[s].nsing == ns) {
+          if (t->sectors[s].nsing == ns && (!mask || mask[s])) {
             p.secw[k] = (uint16_t)(sec_word + (t->secoff5[s] - w0));
             p.secrow[k] = (uint16_t)(s - r.a);
             ++k;
           }
+      p.nsec = k;
+      if (k == 0) continue;  // no sector of this run is selected (qmc_run.sector_mask)
     }
     cudaStream_t ls = nstreams ? static_cast<cudaStream_t>(t->side_streams[i % nstreams]) : st;
     ce = qmc5_kernel_launch(n, t->L, t->kmax, dim3((unsigned)nsl[i], (unsigned)m), smem, ls, p);
@@ -837,6 +844,178 @@ int qmc_integrate_embedded(const qmc_tables *t, int32_t k_min, int32_t k_max, do
   return QMC_OK;
 }
 
+// ---- per-sector lattice sizes by variance (R:C27) ----------------------------------------------------
+int qmc_integrate_allocated(const qmc_tables *t, int32_t k0, int32_t k_max, double target_rel_err, int32_t m, uint64_t seed,
+                            const uint64_t *z, void *cuda_stream, void *dev_workspace, size_t dev_workspace_bytes,
+                            qmc_result *out, int32_t *levels_out, int64_t *evals_per_shift) {
+  if (!t || !out || !z || k0 < 3 || k_max < k0 || k_max > 30 || m < 2 || !(target_rel_err > 0.0)) return QMC_EINVAL;
+  if (out->sector_coeff || out->sector_err || out->shift_sums) return QMC_EINVAL;  // totals only
+  const int n = t->n, K = t->kmax - t->kmin + 1, nsec = (int)t->sectors.size();
+  for (int j = 0; j < n; ++j)
+    if (!(z[j] & 1ull)) return QMC_EINVAL;
+  const size_t TS = (size_t)K * m * 2;
+  auto zmod = [&](int k, uint64_t *zk) {
+    for (int j = 0; j < n; ++j) zk[j] = z[j] & ((1ull << k) - 1);
+  };
+  int64_t counters[4] = {0, 0, 0, 0}, evals = 0, h2d = 0, d2h = 0;
+  double kms = 0.0, ems = 0.0;
+  int launches = 0;
+  auto book = [&](const qmc_result &r) {
+    for (int q = 0; q < 4; ++q) counters[q] += r.counters[q];
+    kms += r.kernel_ms; ems += r.eval_kernel_ms; h2d += r.h2d_bytes; d2h += r.d2h_bytes; launches += r.kernel_launches;
+  };
+  // ---- stage 1: every sector at level k0, per-sector mode: S[sector][order][shift]
+  std::vector<double> S((size_t)nsec * TS), T0(TS), coeff((size_t)K * 2), err((size_t)K * 2);
+  {
+    uint64_t zk[QMC_MAXDIM] = {0};
+    zmod(k0, zk);
+    qmc_run run;
+    std::memset(&run, 0, sizeof run);
+    run.z = zk;
+    run.mode = 2;
+    qmc_result r;
+    std::memset(&r, 0, sizeof r);
+    r.shift_sums = S.data();
+    r.shift_totals = T0.data();
+    const int rc = qmc_integrate_ex(t, 1ull << k0, m, seed, &run, cuda_stream, dev_workspace, dev_workspace_bytes, &r);
+    if (rc != QMC_OK) return rc;
+    book(r);
+    evals += (int64_t)nsec << k0;
+  }
+  qmc_statistics(T0.data(), K, m, coeff.data(), err.data());
+  const double c0 = std::hypot(coeff[2 * (K - 1)], coeff[2 * (K - 1) + 1]);
+  const double tau = target_rel_err * c0;
+  // ---- stage 2: lattice size per sector.  With error ~ e_s N0 / N (the O(1/n) rate the paper quotes) and cost c_s N the
+  // cheapest sizes that meet sum_s e_s(N_s)^2 <= tau^2 are  N_s = (a_s / c_s)^(1/3) (sum_r a_r^(1/3) c_r^(2/3))^(1/2) / tau,
+  // a_s = e_s^2 N0^2 (Lagrange multiplier); rounded up to a power of two in [2^k0, 2^k_max]
+  std::vector<int> lev(nsec, k0);
+  {
+    std::vector<double> a(nsec, 0.0);
+    double sum = 0.0;
+    const double N0 = (double)(1ull << k0);
+    for (int s = 0; s < nsec; ++s) {
+      double e2 = 0.0;
+      for (int c = 0; c < 2; ++c) {  // Re and Im separately (R:C15): the larger of the two
+        double mean, e;
+        mean_err(S.data() + (size_t)s * TS + (size_t)(K - 1) * m * 2 + c, 2, m, &mean, &e);
+        e2 = std::max(e2, e * e);
+      }
+      a[s] = e2 * N0 * N0;
+      sum += std::cbrt(a[s]) * std::pow(t->sec_cost[s], 2.0 / 3.0);
+    }
+    for (int s = 0; s < nsec && tau > 0.0; ++s) {
+      const double Ns = std::cbrt(a[s] / t->sec_cost[s]) * std::sqrt(sum) / tau;
+      int k = k0;
+      while (k < k_max && (double)(1ull << k) < Ns) ++k;
+      lev[s] = k;
+    }
+  }
+  // ---- stage 3: one CLASS per lattice size, evaluated in fused mode through qmc_run.sector_mask (a launch then serves the
+  // class's sectors of a chunk wherever they sit: the per-point work S1-S3 is shared by all of them); per-class per-shift totals.
+  // Kernels without mask support (the generic one): classes = maximal runs of neighbouring sectors of one size instead.
+  struct Run { int a, b, k; std::vector<double> T; std::vector<uint8_t> mask; };
+  std::vector<Run> runs;
+  {
+    std::vector<uint8_t> probe(nsec, 0);
+    uint64_t zk[QMC_MAXDIM] = {0};
+    zmod(k0, zk);
+    qmc_run run;
+    std::memset(&run, 0, sizeof run);
+    run.z = zk;
+    run.mode = 1;
+    run.sector_mask = probe.data();
+    const bool masks = qmc_integrate_async(t, 1ull << k0, m, seed, &run, cuda_stream, dev_workspace, dev_workspace_bytes) == QMC_OK;
+    if (masks) {
+      for (int k = k0; k <= k_max; ++k) {
+        Run R = {0, nsec, k, std::vector<double>(TS, 0.0), std::vector<uint8_t>(nsec, 0)};
+        bool any = false;
+        for (int s = 0; s < nsec; ++s)
+          if (lev[s] == k) R.mask[s] = 1, any = true;
+        if (any) runs.push_back(R);
+      }
+    } else {
+      for (int s = 0; s < nsec;) {
+        int e = s;
+        while (e < nsec && lev[e] == lev[s]) ++e;
+        runs.push_back({s, e, lev[s], std::vector<double>(TS, 0.0), std::vector<uint8_t>()});
+        s = e;
+      }
+    }
+  }
+  std::vector<double> part(TS), T(TS);
+  auto integrate_run = [&](Run &R, int k, bool odd_only) -> int {
+    uint64_t zk[QMC_MAXDIM] = {0};
+    zmod(k, zk);
+    qmc_run run;
+    std::memset(&run, 0, sizeof run);
+    run.z = zk;
+    run.mode = 1;
+    run.sector_begin = R.a;
+    run.sector_end = R.b;
+    run.sector_mask = R.mask.empty() ? nullptr : R.mask.data();
+    if (odd_only) {
+      run.index_begin = 1;
+      run.index_step = 2;
+      run.index_count = (1ull << k) / 2;
+    }
+    qmc_result r;
+    std::memset(&r, 0, sizeof r);
+    r.shift_totals = part.data();
+    const int rc = qmc_integrate_ex(t, 1ull << k, m, seed, &run, cuda_stream, dev_workspace, dev_workspace_bytes, &r);
+    if (rc != QMC_OK) return rc;
+    book(r);
+    for (size_t i = 0; i < TS; ++i) R.T[i] = (odd_only ? 0.5 * R.T[i] : 0.0) + part[i];
+    int64_t nsel = R.b - R.a;
+    if (!R.mask.empty()) {
+      nsel = 0;
+      for (uint8_t v : R.mask) nsel += v != 0;
+    }
+    evals += nsel * (int64_t)((1ull << k) / (odd_only ? 2 : 1));
+    return QMC_OK;
+  };
+  for (Run &R : runs) {
+    if (R.k == k0) {  // stage 1 already holds these sectors at their level
+      for (int s = R.a; s < R.b; ++s)
+        if (R.mask.empty() || R.mask[s])
+          for (size_t i = 0; i < TS; ++i) R.T[i] += S[(size_t)s * TS + i];
+    } else {
+      const int rc = integrate_run(R, R.k, false);
+      if (rc != QMC_OK) return rc;
+    }
+  }
+  // ---- stage 4: Eqs. 19-20 on the per-shift totals over all runs; while the error is above the target every run climbs one
+  // level of the embedded sequence (only its odd indices are new)
+  for (;;) {
+    std::fill(T.begin(), T.end(), 0.0);
+    for (const Run &R : runs)
+      for (size_t i = 0; i < TS; ++i) T[i] += R.T[i];
+    qmc_statistics(T.data(), K, m, coeff.data(), err.data());
+    const double mod = std::hypot(coeff[2 * (K - 1)], coeff[2 * (K - 1) + 1]);
+    if (mod > 0.0 && std::max(err[2 * (K - 1)], err[2 * (K - 1) + 1]) <= target_rel_err * mod) break;
+    bool any = false;
+    for (Run &R : runs)
+      if (R.k < k_max) {
+        const int rc = integrate_run(R, R.k + 1, true);
+        if (rc != QMC_OK) return rc;
+        ++R.k;
+        any = true;
+      }
+    if (!any) break;
+  }
+  if (out->coeff) std::memcpy(out->coeff, coeff.data(), coeff.size() * 8);
+  if (out->err) std::memcpy(out->err, err.data(), err.size() * 8);
+  if (out->shift_totals) std::memcpy(out->shift_totals, T.data(), TS * 8);
+  for (int q = 0; q < 4; ++q) out->counters[q] = counters[q];
+  out->kernel_ms = kms; out->eval_kernel_ms = ems; out->h2d_bytes = h2d; out->d2h_bytes = d2h;
+  out->kernel_launches = launches; out->mode_used = 1;
+  if (levels_out)
+    for (const Run &R : runs)
+      for (int s = R.a; s < R.b; ++s)
+        if (R.mask.empty() || R.mask[s]) levels_out[s] = R.k;
+  if (evals_per_shift) *evals_per_shift = evals;
+  return QMC_OK;
+}
+
 int qmc_fp64_peak(void *cuda_stream, void *dev_workspace, size_t dev_workspace_bytes, double *flops_out, double *ms_out) {
   if (!dev_workspace || dev_workspace_bytes < 8 || !flops_out) return QMC_EINVAL;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
@@ -951,6 +1130,7 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
   const bool use_v5 = cplx && !t->tab5.empty() && -t->kmin <= QMC3_MAXSING && qmc5_kernel_available(n, t->L, t->kmax) &&
                       r.kernel == 0;
   int eval_launches = 1;
+  if (r.sector_mask && (persec || !(use_v4 || use_v5))) return QMC_EUNSUPPORTED;  // fused mode of the table-driven kernels only
   // ---- uploads (skipped when resident).  Versions 4 and 5 carry their tables in the kernel parameters: only the
   // logarithm table lives in the workspace; the version-1 image is uploaded for the generic fallback kernel only.
   const int kind = (use_v4 || use_v5) ? 4 : 1;  // what has to be in the workspace: the logarithm table, or the version-1 image
@@ -975,10 +1155,10 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
   CUDA_OK(cudaMemsetAsync(ws + L.counters, 0, 32, st));
 
   if (use_v5) {
-    int rc = launch_v5(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, r.waves, r.streams, &gx, &nchunks, &eval_launches, &h2d, &ce);
+    int rc = launch_v5(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, r.waves, r.streams, r.sector_mask, &gx, &nchunks, &eval_launches, &h2d, &ce);
     if (rc != QMC_OK) return rc;
   } else if (use_v4) {
-    int rc = launch_v4(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, r.waves, r.streams, &gx, &nchunks, &eval_launches, &h2d, &ce);
+    int rc = launch_v4(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, r.waves, r.streams, r.sector_mask, &gx, &nchunks, &eval_launches, &h2d, &ce);
     if (rc != QMC_OK) return rc;
   } else {
   const size_t fixed_smem = 16 + (((size_t)m * n * 8 + 15) & ~(size_t)15) + (QMC_THREADS / 32) * 8 + (size_t)3 * n * QMC_THREADS * 8;

@@ -405,3 +405,48 @@ def test_embedded_lattice_sequence():
         assert k2 < 18 and n2 == 1 << k2 and max(e0.real, e0.imag) <= 1e-5 * abs(c0)
     with pytest.raises(q.QmcError):
         q.qmc_integrate_embedded(q.qmc_prepare(qi.massless_box()), 10, 12, 4, 1, np.array([1, 2, 5], dtype=np.uint64))   # even component
+
+
+def test_sector_mask_selects_sectors_in_fused_mode():
+    """qmc_run.sector_mask: a fused launch that serves an arbitrary subset of sectors -- the per-shift totals are the sum of
+    the oracle's per-sector values over the selected sectors (C19 tolerance); real path, complex path, empty chunks; the
+    generic kernel refuses masks."""
+    rng = np.random.default_rng(3)
+    for wl, N in ((qi.double_box(), 16381), (qi.nonplanar_vertex(), 16381)):
+        t = q.qmc_prepare(wl, eps_order=wl.eps_order, lam=wl.lam)
+        o = Oracle.from_tables(t.export())
+        z = qi.good_vector(N, t.dim)
+        sh = qi.splitmix64_shifts(wl.seed, 2, t.dim)
+        S, A, cnt = o.integrate(N, z, sh)
+        for mask in (rng.random(t.n_sectors) < 0.3, np.arange(t.n_sectors) % 7 == 3, np.arange(t.n_sectors) >= t.n_sectors - 2):
+            r = q.qmc_integrate(t, N, 2, z=z, shifts=sh, sector_mask=mask.astype(np.uint8))
+            check(r.shift_totals, S[mask].sum(axis=0), A[mask].sum(axis=0), wl.name + " masked")
+        with pytest.raises(q.QmcError) as e:
+            q.qmc_integrate(t, N, 2, z=z, shifts=sh, sector_mask=np.ones(t.n_sectors, dtype=np.uint8), kernel=1)
+        assert e.value.status == -3
+
+
+def test_per_sector_lattice_sizes_by_variance():
+    """SURVEY 8(f) f4, reading C27 (qmc_integrate_allocated): sizes differ between sectors, the target is met, the result agrees
+    with the uniform embedded sequence within errors and with the closed forms (how the evaluation counts compare depends on
+    the target: bench.py reports it, `allocation_vs_uniform`)."""
+    wl = qi.double_box()
+    t = q.qmc_prepare(wl)
+    z = q.qmc_embedded_vector(12, 22, 6)
+    r, lev, ev = q.qmc_integrate_allocated(t, 13, 22, wl.m, wl.seed, z, 2e-4)
+    u, k, npts = q.qmc_integrate_embedded(t, 13, 22, wl.m, wl.seed, z, target_rel_err=2e-4)
+    assert r.err[-1].real <= 2e-4 * abs(r.coeff[-1]) and lev.min() >= 13 and lev.max() > lev.min() + 3
+    assert ev >= t.n_sectors << 13                                                   # stage 1 alone
+    assert abs(r.coeff[-1] - u.coeff[-1]) <= 4 * np.hypot(r.err[-1].real, u.err[-1].real)
+    ex = [2.0 / 9.0, -0.8497687147780183, 0.003001503361321066]                     # the three analytic poles
+    assert np.all(np.abs(r.coeff.real[:3] - ex) <= 4 * r.err.real[:3])
+    wl = qi.massless_box()
+    t = q.qmc_prepare(wl)
+    r, lev, ev = q.qmc_integrate_allocated(t, 10, 20, wl.m, wl.seed, q.qmc_embedded_vector(10, 20, 3), 1e-7)
+    ex = [0.666666666666667, -1.2639198230760183, -1.2238036181980894]
+    assert np.all(np.abs(r.coeff.real - ex) <= 4 * r.err.real) and r.err[-1].real <= 1e-7 * abs(r.coeff[-1])
+    wl = qi.massive_box()                                                            # complex path
+    t = q.qmc_prepare(wl, lam=wl.lam)
+    r, lev, ev = q.qmc_integrate_allocated(t, 10, 20, wl.m, wl.seed, q.qmc_embedded_vector(10, 20, 3), 1e-6)
+    ref = 0.29347155740583 + 0.33214829595148j
+    assert abs(r.coeff[0].real - ref.real) <= 4 * r.err[0].real and abs(r.coeff[0].imag - ref.imag) <= 4 * r.err[0].imag
