@@ -92,6 +92,17 @@ typedef struct qmc_tables qmc_tables; /* opaque sector tables (Eqs. 7-9
  * eps_order = highest order of J(eps) wanted.  options may be NULL (lambda 0, transform 0, depth 64). */
 int qmc_prepare(const qmc_graph *graph, const qmc_kinematics *kin, int32_t eps_order, const qmc_options *options,
                 qmc_tables **out);
+/* Kinematic scans (Fig. 2: the paper's 1000-point scan of the one-loop box): ONE graph at n_points
+ * kinematic points `kinematics[0 .. n_points)`.  The tables hold the sectors of all points one after the other (the exponent
+ * structure of a point's sectors does not depend on the kinematics, only the coefficients do); every point must decompose into
+ * the same number of sectors (a coefficient that vanishes at one point only changes the decomposition: QMC_EINVAL).
+ * qmc_tables_info reports the total number of sectors, qmc_tables_batch_info the points and the sectors per point.
+ * Integrate with qmc_run.mode = 3: one call evaluates all points (one fused launch per point and chunk, spread over the side
+ * streams, ONE final sum, ONE statistics pass, ONE copy back) on the same lattice and shift vectors, and returns per POINT
+ * what mode 2 returns per sector: sector_coeff / sector_err [n_points][K][2], shift_sums [n_points][K][m][2]. */
+int qmc_prepare_batch(const qmc_graph *graph, const qmc_kinematics *kinematics, int32_t n_points, int32_t eps_order,
+                      const qmc_options *options, qmc_tables **out);
+int qmc_tables_batch_info(const qmc_tables *t, int32_t *n_points, int32_t *sectors_per_point);
 void qmc_tables_free(qmc_tables *t);
 
 /* orders k_min = -max_sector(#singular variables) .. k_max = eps_order; K = k_max - k_min + 1 */
@@ -131,7 +142,8 @@ typedef struct {
   uint64_t index_begin, index_step, index_count; /* lattice indices i = begin + c*step, c < count; count 0 = all N.
                                                     The sum is always normalised by 1/N (Eq. 18). */
   int32_t sector_begin, sector_end;              /* sector range; end 0 = all */
-  int32_t mode;             /* 0 auto (per-sector iff a per-sector output is requested), 1 fused, 2 per-sector */
+  int32_t mode;             /* 0 auto (per-sector iff a per-sector output is requested), 1 fused, 2 per-sector,
+                               3 per kinematic point of a batch (qmc_prepare_batch): fused within a point */
   int32_t tables_resident;  /* 1: reuse what an earlier call left in this workspace (the logarithm table);
                                2: reuse the shift vectors of that call as well (nothing is copied from the host) */
   int32_t kernel;           /* 0: the table-driven kernels (real path: qmc4_eval_kernel, complex path: qmc5_eval_kernel) where

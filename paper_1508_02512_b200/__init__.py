@@ -9,9 +9,9 @@ while any call fails loudly there (no CPU fallback).
 """
 from . import binding
 from .binding import (QmcError, Result, Tables, lib, qmc_flop_model, qmc_fp64_peak, qmc_cbc_vector, qmc_generating_vector, qmc_generating_vector_noalloc, qmc_embedded_vector, qmc_integrate_embedded, qmc_integrate_allocated,
-                      qmc_integrate, qmc_integrate_async, qmc_prefactor_series, qmc_prepare, qmc_result_device_totals, qmc_result_fetch,
+                      qmc_integrate, qmc_integrate_async, qmc_prefactor_series, qmc_prepare, qmc_prepare_batch, qmc_result_device_totals, qmc_result_fetch,
                       qmc_shifts, qmc_statistics, strerror, LIB_PATH)
 
 __all__ = ["QmcError", "Result", "Tables", "lib", "qmc_flop_model", "qmc_fp64_peak", "qmc_cbc_vector", "qmc_generating_vector", "qmc_generating_vector_noalloc", "qmc_embedded_vector", "qmc_integrate_embedded", "qmc_integrate_allocated",
-           "qmc_integrate", "qmc_integrate_async", "qmc_prefactor_series", "qmc_prepare", "qmc_result_device_totals", "qmc_result_fetch",
+           "qmc_integrate", "qmc_integrate_async", "qmc_prefactor_series", "qmc_prepare", "qmc_prepare_batch", "qmc_result_device_totals", "qmc_result_fetch",
            "qmc_shifts", "qmc_statistics", "strerror", "LIB_PATH", "binding"]

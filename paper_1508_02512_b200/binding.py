@@ -73,6 +73,11 @@ def lib():
         L.qmc_prepare.restype = C.c_int
         L.qmc_prepare.argtypes = [C.POINTER(qmc_graph), C.POINTER(qmc_kinematics), C.c_int32, C.POINTER(qmc_options),
                                   C.POINTER(C.c_void_p)]
+        L.qmc_prepare_batch.restype = C.c_int
+        L.qmc_prepare_batch.argtypes = [C.POINTER(qmc_graph), C.POINTER(qmc_kinematics), C.c_int32, C.c_int32, C.POINTER(qmc_options),
+                                        C.POINTER(C.c_void_p)]
+        L.qmc_tables_batch_info.restype = C.c_int
+        L.qmc_tables_batch_info.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
         L.qmc_tables_free.restype = None
         L.qmc_tables_free.argtypes = [C.c_void_p]
         L.qmc_tables_info.restype = C.c_int
@@ -151,6 +156,9 @@ class Tables:
         self.n_sectors, self.dim, self.k_min, self.k_max, cx = (int(x.value) for x in v)
         self.is_complex = bool(cx)
         self.K = self.k_max - self.k_min + 1
+        npts, spp = C.c_int32(1), C.c_int32(0)
+        lib().qmc_tables_batch_info(self._h, C.byref(npts), C.byref(spp))
+        self.n_points, self.sectors_per_point = int(npts.value), int(spp.value)   # > 1 point: qmc_prepare_batch
         self._ws = None
 
     def __del__(self):
@@ -205,6 +213,31 @@ def qmc_prepare(wl=None, *, n_vertices=None, edges=None, leg_vertex=None, gram=N
     rc = lib().qmc_prepare(C.byref(g), C.byref(k), eps_order, C.byref(o), C.byref(h))
     if rc:
         raise QmcError(rc, "qmc_prepare")
+    return Tables(h.value)
+
+
+def qmc_prepare_batch(wls, *, eps_order: int = 0, lam: float = 0.0, transform: int = 0, max_depth: int = 0, lattice: int = 0,
+                      slot_budget: int = 0, chunk_bytes: int = 0, threads: int = 0, slot_budget_cplx_real: int = 0,
+                      slot_budget_cplx: int = 0, dense_template: int = 0) -> Tables:
+    """qmc_prepare_batch: ONE graph (taken from wls[0]) at the kinematic points of the workloads `wls` (their Gram matrices).
+    Integrate with qmc_integrate(..., mode=3): results per kinematic point."""
+    w0 = wls[0]
+    eu = np.ascontiguousarray([e[0] for e in w0.edges], dtype=np.int32)
+    ev = np.ascontiguousarray([e[1] for e in w0.edges], dtype=np.int32)
+    m2 = np.ascontiguousarray([e[2] for e in w0.edges], dtype=np.float64)
+    lv = np.ascontiguousarray(w0.leg_vertex, dtype=np.int32)
+    grams = [np.ascontiguousarray(w.gram, dtype=np.float64) for w in wls]
+    for w in wls:
+        assert w.edges == w0.edges and list(w.leg_vertex) == list(w0.leg_vertex), "a batch is one graph at several kinematic points"
+    g = qmc_graph(w0.n_vertices, len(w0.edges), len(lv), _ptr(eu, C.c_int32), _ptr(ev, C.c_int32), _ptr(m2, C.c_double), None,
+                  _ptr(lv, C.c_int32))
+    kins = (qmc_kinematics * len(wls))(*[qmc_kinematics(_ptr(gr, C.c_double)) for gr in grams])
+    o = qmc_options(lam, transform, max_depth, lattice, slot_budget, chunk_bytes, threads, slot_budget_cplx_real,
+                    slot_budget_cplx, dense_template)
+    h = C.c_void_p()
+    rc = lib().qmc_prepare_batch(C.byref(g), kins, len(wls), eps_order, C.byref(o), C.byref(h))
+    if rc:
+        raise QmcError(rc, "qmc_prepare_batch")
     return Tables(h.value)
 
 
@@ -299,7 +332,8 @@ def qmc_integrate(t: Tables, N: int, m: int, seed: int = 0, *, z: Optional[Seque
         ws = _workspace(t, N, m, dev)
         st = stream if stream is not None else torch.cuda.current_stream(dev)
         s0, s1 = sectors if sectors is not None else (0, t.n_sectors)
-        res, arrays = _make_result(t, m, s1 - s0, per_sector)
+        rows = t.n_points if mode == 3 else s1 - s0       # mode 3: one row of results per kinematic point of a batch
+        res, arrays = _make_result(t, m, rows, per_sector or mode == 3)
         run, keep = _make_run(t, m, z, shifts, index_range, sectors, mode, resident, kernel, waves, streams, sector_mask)
         rc = lib().qmc_integrate_ex(t._h, N, m, seed, C.byref(run), C.c_void_p(st.cuda_stream),
                                     C.c_void_p(ws.data_ptr()), ws.numel(), C.byref(res))

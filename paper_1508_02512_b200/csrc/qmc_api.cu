@@ -16,6 +16,7 @@
 #include "qmc_tables.h"
 
 #define QMC_MAX_BLOCKS 592  // upper bound of gridDim.x used for workspace sizing (148 SMs x 4)
+#define QMC_MAX_BLOCKS_BATCH 32  // the same for a batch of kinematic points (one small run per point)
 #define QMC_NCAND 64        // Korobov candidates of the P_2 search
 #define QMC_P2_BLOCKS 296
 
@@ -41,6 +42,21 @@ __global__ void qmc_finalize_kernel(const double *partial, double *out, int rows
       const double *src = partial + (((size_t)c * m + kap) * nblocks) * nacc + a;
       for (int b = 0; b < nblocks; ++b) s += src[(size_t)b * nacc];
     }
+  }
+  out[idx] = s * invN;
+}
+
+// batch of kinematic points (mode 3): partial [run][shift][block][nacc], the runs of row r are [run_begin[r], run_begin[r + 1])
+// -> out [row][nacc][shift]
+__global__ void qmc_finalize_rows_kernel(const double *partial, double *out, const int *run_begin, int nrows, int m, int nblocks,
+                                         int nacc, double invN) {
+  int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= nrows * nacc * m) return;
+  int kap = idx % m, a = (idx / m) % nacc, row = idx / (m * nacc);
+  double s = 0.0;
+  for (int c = run_begin[row]; c < run_begin[row + 1]; ++c) {
+    const double *src = partial + (((size_t)c * m + kap) * nblocks) * nacc + a;
+    for (int b = 0; b < nblocks; ++b) s += src[(size_t)b * nacc];
   }
   out[idx] = s * invN;
 }
@@ -153,7 +169,7 @@ uint64_t splitmix64(uint64_t &state) {
 uint64_t mulmod(uint64_t a, uint64_t b, uint64_t n) { return (uint64_t)(((unsigned __int128)a * b) % n); }
 
 struct DevLayout {
-  size_t image, secoff, logtab4, shifts, counters, out, stat, partial, p2z, p2partial, total;
+  size_t image, secoff, logtab4, shifts, counters, out, stat, partial, p2z, p2partial, runbegin, total;
 };
 
 DevLayout layout(const qmc_tables *t, int m) {
@@ -167,9 +183,10 @@ DevLayout layout(const qmc_tables *t, int m) {
   L.counters = o; o += 256;
   L.out = o; o += align256(nsec * QMC_NACC_MAX * 2 * (size_t)m * 8);
   L.stat = o; o += align256(stat_layout((int)nsec, QMC_MAXK, m).total * 8);
-  L.partial = o; o += align256(nsec * (size_t)m * QMC_MAX_BLOCKS * QMC_NACC_MAX * 2 * 8);
+  L.partial = o; o += align256(nsec * (size_t)m * (t->n_rows > 1 ? QMC_MAX_BLOCKS_BATCH : QMC_MAX_BLOCKS) * QMC_NACC_MAX * 2 * 8);
   L.p2z = o; o += align256((size_t)QMC_NCAND * QMC_MAXDIM * 4);
   L.p2partial = o; o += align256((size_t)QMC_NCAND * QMC_P2_BLOCKS * 8);
+  L.runbegin = o; o += align256((nsec + 2) * 4);
   L.total = o;
   return L;
 }
@@ -261,8 +278,8 @@ void mean_err(const double *v, size_t stride, int m, double *mean, double *err) 
 // and joined back into the caller's stream, so that the tail of one launch overlaps the next ones.
 int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t st, uint64_t N, int m, int sb, int se,
               bool persec, uint64_t ibeg, uint64_t istep, uint64_t icount, const uint64_t *z, int sms, int smem_optin,
-              int waves_opt, int streams_opt, const uint8_t *mask, int *gx_out, int *rows_out, int *launches_out, size_t *h2d,
-              cudaError_t *ce_out) {
+              int waves_opt, int streams_opt, const uint8_t *mask, const int *rowmap, std::vector<int> *row_of_run, int *gx_out,
+              int *rows_out, int *launches_out, size_t *h2d, cudaError_t *ce_out) {
   const int n = t->n, nacc = QMC_MAXSING + t->kmax + 1, T = t->threads_real;
   const size_t budget = (size_t)smem_optin - 1024;
   // shared memory of a launch: logarithm table, shift vectors, reduction scratch, the chunk's slot columns.
@@ -287,6 +304,7 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
       while (b < e) {
         const size_t words = prog_words + (t->secoff4[b + 1] - t->secoff4[a]);
         if (words > QMC4_TAB_WORDS || b + 1 - a > QMC4_MAX_SEC || (persec && b > a)) break;
+        if (rowmap && b > a && rowmap[b] != rowmap[a]) break;  // a run never mixes kinematic points
         ++b;
       }
       if (b == a) return QMC_ENOMEM;
@@ -311,7 +329,8 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
   for (int i = 0; i < nitems; ++i) {
     long long ns = total_cost > 0.0 ? (long long)(nblocks_target * runs[i].cost / total_cost + 0.5) : 1;
     if (persec) ns = std::max<long long>(ns, (sms + 4 * m - 1) / (4 * m));  // one small launch per sector: a quarter wave each
-    ns = std::max<long long>(1, std::min<long long>({ns, (long long)QMC_MAX_BLOCKS, max_slices_pts}));
+    if (rowmap) ns = std::max<long long>(ns, (2LL * sms * bps + (long long)m * 4 - 1) / ((long long)m * 4));  // one small launch per point
+    ns = std::max<long long>(1, std::min<long long>({ns, (long long)(rowmap ? QMC_MAX_BLOCKS_BATCH : QMC_MAX_BLOCKS), max_slices_pts}));
     nsl[i] = (int)ns;
     max_slices = std::max(max_slices, (int)ns);
   }
@@ -395,6 +414,10 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
       cudaStreamWaitEvent(st, static_cast<cudaEvent_t>(t->side_events[q]), 0);
     }
   cudaEventRecord(static_cast<cudaEvent_t>(t->evm), st);
+  if (rowmap && row_of_run) {
+    row_of_run->clear();
+    for (const Run &r : runs) row_of_run->push_back(rowmap[r.a]);
+  }
   *ce_out = ce;
   *gx_out = max_slices;
   *rows_out = nitems;
@@ -405,8 +428,8 @@ int launch_v4(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
 // ---- version-5 launch (complex path): as version 4, two slot tables per thread ------------------------------------------
 int launch_v5(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t st, uint64_t N, int m, int sb, int se,
               bool persec, uint64_t ibeg, uint64_t istep, uint64_t icount, const uint64_t *z, int sms, int smem_optin,
-              int waves_opt, int streams_opt, const uint8_t *mask, int *gx_out, int *rows_out, int *launches_out, size_t *h2d,
-              cudaError_t *ce_out) {
+              int waves_opt, int streams_opt, const uint8_t *mask, const int *rowmap, std::vector<int> *row_of_run, int *gx_out,
+              int *rows_out, int *launches_out, size_t *h2d, cudaError_t *ce_out) {
   const int n = t->n, nacc = 2 * (QMC_MAXSING + t->kmax + 1), T = QMC3_THREADS;  // accumulators: (Re, Im) per order
   int max_r = 0, max_c = 0;
   for (size_t ci = 0; ci < t->chunks3.size(); ++ci) {
@@ -435,6 +458,7 @@ int launch_v5(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
       while (b < e) {
         const size_t words = prog_words + (t->secoff5[b + 1] - t->secoff5[a]);
         if (words > QMC4_TAB_WORDS || b + 1 - a > QMC4_MAX_SEC || fixed + accbytes * (b + 1 - a) > budget) break;
+        if (rowmap && b > a && rowmap[b] != rowmap[a]) break;  // a run never mixes kinematic points
         ++b;
       }
       if (b == a) return QMC_ENOMEM;
@@ -459,7 +483,8 @@ int launch_v5(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
   int max_slices = 1;
   for (int i = 0; i < nitems; ++i) {
     long long ns = total_cost > 0.0 ? (long long)(nblocks_target * runs[i].cost / total_cost + 0.5) : 1;
-    ns = std::max<long long>(1, std::min<long long>({ns, (long long)QMC_MAX_BLOCKS, max_slices_pts}));
+    if (rowmap) ns = std::max<long long>(ns, (2LL * sms * bps + (long long)m * 4 - 1) / ((long long)m * 4));  // one small launch per point
+    ns = std::max<long long>(1, std::min<long long>({ns, (long long)(rowmap ? QMC_MAX_BLOCKS_BATCH : QMC_MAX_BLOCKS), max_slices_pts}));
     nsl[i] = (int)ns;
     max_slices = std::max(max_slices, (int)ns);
   }
@@ -548,6 +573,10 @@ int launch_v5(qmc_tables *t, const DevLayout &L, unsigned char *ws, cudaStream_t
       cudaStreamWaitEvent(st, static_cast<cudaEvent_t>(t->side_events[q]), 0);
     }
   cudaEventRecord(static_cast<cudaEvent_t>(t->evm), st);
+  if (rowmap && row_of_run) {
+    row_of_run->clear();
+    for (const Run &r : runs) row_of_run->push_back(rowmap[r.a]);
+  }
   *ce_out = ce;
   *gx_out = max_slices;
   *rows_out = nitems;
@@ -577,6 +606,33 @@ int qmc_prepare(const qmc_graph *graph, const qmc_kinematics *kin, int32_t eps_o
     return rc;
   }
   *out = t;
+  return QMC_OK;
+}
+
+int qmc_prepare_batch(const qmc_graph *graph, const qmc_kinematics *kinematics, int32_t n_points, int32_t eps_order,
+                      const qmc_options *options, qmc_tables **out) {
+  if (!out) return QMC_EINVAL;
+  *out = nullptr;
+  qmc_tables *t = new (std::nothrow) qmc_tables;
+  if (!t) return QMC_ENOMEM;
+  int rc;
+  try {
+    rc = qmc_build_tables_batch(graph, kinematics, n_points, eps_order, options, t);
+  } catch (...) {
+    rc = QMC_ENOMEM;
+  }
+  if (rc != QMC_OK) {
+    delete t;
+    return rc;
+  }
+  *out = t;
+  return QMC_OK;
+}
+
+int qmc_tables_batch_info(const qmc_tables *t, int32_t *n_points, int32_t *sectors_per_point) {
+  if (!t) return QMC_EINVAL;
+  if (n_points) *n_points = t->n_rows;
+  if (sectors_per_point) *sectors_per_point = t->n_rows > 0 ? (int32_t)(t->sectors.size() / t->n_rows) : 0;
   return QMC_OK;
 }
 
@@ -1068,8 +1124,10 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
   if (istep < 1 || ibeg >= N || icount > N) return QMC_EINVAL;
   const bool cplx = t->lambda > 0.0;
   const int mode = r.mode ? r.mode : 1;
-  if (mode != 1 && mode != 2) return QMC_EINVAL;
+  if (mode != 1 && mode != 2 && mode != 3) return QMC_EINVAL;
   const bool persec = mode == 2;
+  const bool batch = mode == 3;  // fused within a kinematic point, one row of results per point (qmc_prepare_batch)
+  if (batch && (t->row_of_sector.size() != t->sectors.size() || sb != 0 || se != nsec_all || r.sector_mask)) return QMC_EINVAL;
 
   int devcount = 0;
   if (cudaGetDeviceCount(&devcount) != cudaSuccess || devcount < 1) {
@@ -1130,7 +1188,9 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
   const bool use_v5 = cplx && !t->tab5.empty() && -t->kmin <= QMC3_MAXSING && qmc5_kernel_available(n, t->L, t->kmax) &&
                       r.kernel == 0;
   int eval_launches = 1;
-  if (r.sector_mask && (persec || !(use_v4 || use_v5))) return QMC_EUNSUPPORTED;  // fused mode of the table-driven kernels only
+  if ((r.sector_mask || batch) && (persec || !(use_v4 || use_v5))) return QMC_EUNSUPPORTED;  // fused mode of the table-driven kernels only
+  std::vector<int> row_of_run;
+  const int *rowmap = batch ? t->row_of_sector.data() : nullptr;
   // ---- uploads (skipped when resident).  Versions 4 and 5 carry their tables in the kernel parameters: only the
   // logarithm table lives in the workspace; the version-1 image is uploaded for the generic fallback kernel only.
   const int kind = (use_v4 || use_v5) ? 4 : 1;  // what has to be in the workspace: the logarithm table, or the version-1 image
@@ -1155,10 +1215,10 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
   CUDA_OK(cudaMemsetAsync(ws + L.counters, 0, 32, st));
 
   if (use_v5) {
-    int rc = launch_v5(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, r.waves, r.streams, r.sector_mask, &gx, &nchunks, &eval_launches, &h2d, &ce);
+    int rc = launch_v5(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, r.waves, r.streams, r.sector_mask, rowmap, &row_of_run, &gx, &nchunks, &eval_launches, &h2d, &ce);
     if (rc != QMC_OK) return rc;
   } else if (use_v4) {
-    int rc = launch_v4(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, r.waves, r.streams, r.sector_mask, &gx, &nchunks, &eval_launches, &h2d, &ce);
+    int rc = launch_v4(t, L, ws, st, N, m, sb, se, persec, ibeg, istep, icount, z, sms, smem_optin, r.waves, r.streams, r.sector_mask, rowmap, &row_of_run, &gx, &nchunks, &eval_launches, &h2d, &ce);
     if (rc != QMC_OK) return rc;
   } else {
   const size_t fixed_smem = 16 + (((size_t)m * n * 8 + 15) & ~(size_t)15) + (QMC_THREADS / 32) * 8 + (size_t)3 * n * QMC_THREADS * 8;
@@ -1230,11 +1290,23 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
   cudaEventRecord(static_cast<cudaEvent_t>(t->evm), st);
   }
   const int rows = persec ? (se - sb) : nchunks;
-  const int nrows = persec ? (se - sb) : 0;  // per-sector rows of the statistics block
-  const int nout = (persec ? (se - sb) : 1) * nacc * nc * m;
+  const int nrows = persec ? (se - sb) : (batch ? t->n_rows : 0);  // rows of the statistics block: sectors, or kinematic points
+  const int nout = (nrows ? nrows : 1) * nacc * nc * m;
   const int K = t->kmax - t->kmin + 1;
   double *dout = reinterpret_cast<double *>(ws + L.out);
-  if (ce == cudaSuccess) {
+  if (ce == cudaSuccess && batch) {
+    // runs are in sector order, hence in row order: row r owns the runs [run_begin[r], run_begin[r + 1])
+    t->run_begin_host.assign(t->n_rows + 1, 0);
+    for (int rr : row_of_run) ++t->run_begin_host[rr + 1];
+    for (int q = 0; q < t->n_rows; ++q) t->run_begin_host[q + 1] += t->run_begin_host[q];
+    int *drb = reinterpret_cast<int *>(ws + L.runbegin);
+    ce = cudaMemcpyAsync(drb, t->run_begin_host.data(), t->run_begin_host.size() * 4, cudaMemcpyHostToDevice, st);
+    h2d += t->run_begin_host.size() * 4;
+    if (ce == cudaSuccess) {
+      qmc_finalize_rows_kernel<<<(nout + 127) / 128, 128, 0, st>>>(partial, dout, drb, nrows, m, gx, nacc * nc, 1.0 / (double)N);
+      ce = cudaGetLastError();
+    }
+  } else if (ce == cudaSuccess) {
     qmc_finalize_kernel<<<(nout + 127) / 128, 128, 0, st>>>(partial, dout, rows, m, gx, nacc * nc, 1.0 / (double)N, persec ? 1 : 0);
     ce = cudaGetLastError();
   }
@@ -1268,7 +1340,7 @@ int qmc_result_fetch(const qmc_tables *tc, void *cuda_stream, void *dev_workspac
   const int m = t->last.m, nrows = t->last.nrows, K = t->kmax - t->kmin + 1;
   DevLayout L = layout(t, m);
   if (dev_workspace_bytes < L.total) return QMC_ENOMEM;
-  if ((out->sector_coeff || out->sector_err || out->shift_sums) && t->last.mode != 2) return QMC_EINVAL;
+  if ((out->sector_coeff || out->sector_err || out->shift_sums) && t->last.mode != 2 && t->last.mode != 3) return QMC_EINVAL;
   unsigned char *ws = static_cast<unsigned char *>(dev_workspace);
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   const StatLayout S = stat_layout(nrows, K, m);
@@ -1322,6 +1394,7 @@ int qmc_integrate_ex(const qmc_tables *t, uint64_t N, int32_t m, uint64_t seed, 
   const bool want_persec = out->sector_coeff || out->sector_err || out->shift_sums;
   if (r.mode == 0) r.mode = want_persec ? 2 : 1;
   if (r.mode == 1 && want_persec) return QMC_EINVAL;
+  if (r.mode == 3 && !want_persec) return QMC_EINVAL;  // a batch returns its results per kinematic point (the sector_* outputs)
   int rc = qmc_integrate_async(t, N, m, seed, &r, cuda_stream, dev_workspace, dev_workspace_bytes);
   if (rc != QMC_OK) return rc;
   return qmc_result_fetch(t, cuda_stream, dev_workspace, dev_workspace_bytes, out);

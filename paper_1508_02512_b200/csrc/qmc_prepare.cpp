@@ -127,8 +127,9 @@ unsigned smallest_hitting_set(const Poly &target, int n) {
 
 }  // namespace
 
-int qmc_build_tables(const qmc_graph *g, const qmc_kinematics *kin, int eps_order, const qmc_options *opt,
-                     qmc_tables *T) {
+// graph + kinematics -> T->sectors (appended), exponents, kmin (the most negative so far); no table images yet
+static int qmc_build_sectors(const qmc_graph *g, const qmc_kinematics *kin, int eps_order, const qmc_options *opt,
+                             qmc_tables *T) {
   if (!g || !kin || !kin->gram || !T) return QMC_EINVAL;
   const int V = g->n_vertices, P = g->n_edges, NL = g->n_legs;
   if (V < 1 || P < 2 || NL < 0 || P - 1 > QMC_MAXDIM) return QMC_EINVAL;
@@ -199,7 +200,6 @@ int qmc_build_tables(const qmc_graph *g, const qmc_kinematics *kin, int eps_orde
   const int max_depth = (opt && opt->max_depth > 0) ? opt->max_depth : 64;
   const int n = T->n;
   T->kmax = eps_order;
-  T->sectors.clear();
 
   // ---- primary sectors (Eqs. 3-6) and iterated decomposition (Eqs. 7-9), depth first ------------
   std::vector<Node> stack;
@@ -221,7 +221,7 @@ int qmc_build_tables(const qmc_graph *g, const qmc_kinematics *kin, int eps_orde
     }
     stack.push_back(nd);
   }
-  int smax = 0;
+  int smax = -T->kmin;  // (a batch appends the sectors of several kinematic points: kmin = the most negative of all)
   while (!stack.empty()) {
     Node nd = stack.back();
     stack.pop_back();
@@ -292,7 +292,12 @@ int qmc_build_tables(const qmc_graph *g, const qmc_kinematics *kin, int eps_orde
   }
   T->kmin = -smax;
   if (T->kmax - T->kmin + 1 > QMC_MAXK) return QMC_EUNSUPPORTED;
+  return QMC_OK;
+}
 
+// T->sectors -> the generic table image and the tables of the table-driven kernels
+static int qmc_finish_tables(qmc_tables *T, const qmc_options *opt) {
+  const int n = T->n;
   // ---- device image -----------------------------------------------------------------------------
   T->image.clear();
   T->secoff.clear();
@@ -368,4 +373,39 @@ int qmc_build_tables(const qmc_graph *g, const qmc_kinematics *kin, int eps_orde
   }
   if (T->sec_cost.size() != T->sectors.size()) T->sec_cost.assign(T->sectors.size(), 1.0);
   return QMC_OK;
+}
+
+int qmc_build_tables(const qmc_graph *g, const qmc_kinematics *kin, int eps_order, const qmc_options *opt,
+                     qmc_tables *T) {
+  if (!T) return QMC_EINVAL;
+  T->sectors.clear();
+  T->kmin = 0;
+  T->row_of_sector.clear();
+  T->n_rows = 1;
+  const int rc = qmc_build_sectors(g, kin, eps_order, opt, T);
+  if (rc != QMC_OK) return rc;
+  return qmc_finish_tables(T, opt);
+}
+
+// Kinematic points as a batch: ONE graph at n_points kinematic points.  The sectors of all points are
+// concatenated (row_of_sector = point); the exponent structure of a point's tables does not depend on the kinematics unless a
+// coefficient vanishes, so every point must decompose into the same number of sectors (else QMC_EINVAL).
+int qmc_build_tables_batch(const qmc_graph *g, const qmc_kinematics *kins, int n_points, int eps_order, const qmc_options *opt,
+                           qmc_tables *T) {
+  if (!T || !kins || n_points < 1) return QMC_EINVAL;
+  T->sectors.clear();
+  T->kmin = 0;
+  T->row_of_sector.clear();
+  size_t per_point = 0;
+  for (int p = 0; p < n_points; ++p) {
+    const size_t before = T->sectors.size();
+    const int rc = qmc_build_sectors(g, &kins[p], eps_order, opt, T);
+    if (rc != QMC_OK) return rc;
+    const size_t cnt = T->sectors.size() - before;
+    if (p == 0) per_point = cnt;
+    if (cnt != per_point || cnt == 0) return QMC_EINVAL;
+    for (size_t i = 0; i < cnt; ++i) T->row_of_sector.push_back(p);
+  }
+  T->n_rows = n_points;
+  return qmc_finish_tables(T, opt);
 }

@@ -138,6 +138,8 @@ struct qmc_tables {
   int transform = 0;
   int lattice = 0;  // qmc_options::lattice
   std::vector<QmcSector> sectors;
+  std::vector<int> row_of_sector;  // batch of kinematic points (qmc_prepare_batch): kinematic point of every sector; else empty
+  int n_rows = 1;                  // kinematic points in the batch
   // device image
   std::vector<uint8_t> image;     // concatenated sector blocks (16-byte aligned each)
   std::vector<uint32_t> secoff;   // [n_sectors + 1] byte offsets
@@ -170,6 +172,7 @@ struct qmc_tables {
   uint64_t cached_z[QMC_MAXDIM] = {0};
   std::vector<double> shifts_host;    // staging of the shift vectors (must outlive the async H2D copy)
   std::vector<double> stat_host;      // staging of the fetched statistics block
+  std::vector<int> run_begin_host;    // batch mode: first run of every kinematic point (must outlive the async H2D copy)
   void *ev0 = nullptr, *ev1 = nullptr, *evm = nullptr;  // cudaEvent_t: before / after all kernels, after the evaluation kernel
   struct {
     bool valid = false;
@@ -188,3 +191,5 @@ int qmc_build_tables4(qmc_tables *t, int slot_budget, int chunk_bytes, int threa
 int qmc_build_image3(qmc_tables *t, int slots_r, int slots_c, int chunk_bytes);  // 0 = the measured defaults
 int qmc_build_tables(const qmc_graph *g, const qmc_kinematics *kin, int eps_order, const qmc_options *opt,
                      qmc_tables *out);
+int qmc_build_tables_batch(const qmc_graph *g, const qmc_kinematics *kins, int n_points, int eps_order, const qmc_options *opt,
+                           qmc_tables *out);

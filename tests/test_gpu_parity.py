@@ -450,3 +450,29 @@ def test_per_sector_lattice_sizes_by_variance():
     r, lev, ev = q.qmc_integrate_allocated(t, 10, 20, wl.m, wl.seed, q.qmc_embedded_vector(10, 20, 3), 1e-6)
     ref = 0.29347155740583 + 0.33214829595148j
     assert abs(r.coeff[0].real - ref.real) <= 4 * r.err[0].real and abs(r.coeff[0].imag - ref.imag) <= 4 * r.err[0].imag
+
+
+def test_batched_kinematic_points():
+    """kinematic points as a batch (qmc_prepare_batch + qmc_run.mode = 3): ONE call evaluates all points.  Per
+    point and per shift the batch result equals the oracle's totals of that point (its own decomposition at that point's
+    kinematics; C19 tolerance), and the result of the one-call-per-point path to the same tolerance (the two split the lattice
+    into different numbers of slices, so the partial sums group differently) -- complex path (the paper's box scan, points on
+    both sides of the threshold) and real path (the massless box at four kinematic points)."""
+    N, m = 16381, 4
+    z = qi.good_vector(N, 3)
+    for pts, lam, seed in (([wl for s, wl in qi.gghh_box_scan(44)][2:9], 0.5, 11),
+                           ([qi.massless_box(-3, -2), qi.massless_box(-1, -1), qi.massless_box(-2, -5), qi.massless_box(-0.3, -4)], 0.0, 7)):
+        sh = qi.splitmix64_shifts(seed, m, 3)
+        t = q.qmc_prepare_batch(pts, lam=lam)
+        assert t.n_points == len(pts) and t.n_sectors == t.n_points * t.sectors_per_point
+        r = q.qmc_integrate(t, N, m, z=z, shifts=sh, mode=3)
+        assert r.mode_used == 3 and r.shift_sums.shape == (len(pts), t.K, m)
+        for p, wl in enumerate(pts):
+            o = Oracle.from_workload(wl, lam=lam)
+            S, A, cnt = o.integrate(N, z, sh)
+            check(r.shift_sums[p], S.sum(axis=0), A.sum(axis=0), f"{wl.name} point {p}")
+            one = q.qmc_integrate(q.qmc_prepare(wl, lam=lam), N, m, z=z, shifts=sh)
+            check(one.shift_totals, r.shift_sums[p], A.sum(axis=0), f"{wl.name} point {p}: one call per point")
+            assert np.allclose(one.coeff, r.sector_coeff[p], rtol=1e-11, atol=1e-13 * np.abs(A).max())
+    with pytest.raises(q.QmcError):
+        q.qmc_integrate(t, N, m, z=z, shifts=sh, mode=3, sectors=(0, 4))         # a batch is integrated as a whole
