@@ -145,7 +145,11 @@ typedef struct {
   int32_t mode;             /* 0 auto (per-sector iff a per-sector output is requested), 1 fused, 2 per-sector,
                                3 per kinematic point of a batch (qmc_prepare_batch): fused within a point */
   int32_t tables_resident;  /* 1: reuse what an earlier call left in this workspace (the logarithm table);
-                               2: reuse the shift vectors of that call as well (nothing is copied from the host) */
+                               2: reuse the shift vectors of that call as well (nothing is copied from the host) -- only if
+                               they are the ones this call asks for: the same m and, unless that call passed them explicitly,
+                               the same seed; otherwise they are generated and uploaded again.
+                               A qmc_tables object carries launcher state (events, side streams, staging buffers, what is
+                               resident): it serves ONE stream and ONE host thread at a time -- use one object per stream. */
   int32_t kernel;           /* 0: the table-driven kernels (real path: qmc4_eval_kernel, complex path: qmc5_eval_kernel) where
                                the tables allow them, else the generic kernel; 1: the generic kernel (qmc_eval_kernel) */
   int32_t waves;            /* launch geometry: blocks per resident block slot over all launches of a step (0 = 16) */

@@ -1139,7 +1139,10 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
   unsigned char *ws = static_cast<unsigned char *>(dev_workspace);
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   const bool image_resident_ws = r.tables_resident >= 1 && t->resident_ws == dev_workspace;
-  const bool shifts_resident = r.tables_resident >= 2 && image_resident_ws && t->resident_m == m && !r.shifts;
+  // resident shift vectors are reused only if they are the ones this call asks for: the same count and -- unless they were
+  // passed explicitly by the call that left them -- the same seed (a different seed re-generates and re-uploads them)
+  const bool shifts_resident = r.tables_resident >= 2 && image_resident_ws && t->resident_m == m && !r.shifts &&
+                               (t->resident_explicit || t->resident_seed == seed);
 
   // ---- generating vector and shifts ---------------------------------------------------------------------
   uint64_t z[QMC_MAXDIM] = {0};
@@ -1211,6 +1214,8 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
     h2d += t->shifts_host.size() * 8;
     CUDA_OK(cudaMemcpyAsync(ws + L.shifts, t->shifts_host.data(), t->shifts_host.size() * 8, cudaMemcpyHostToDevice, st));
     t->resident_m = m;
+    t->resident_seed = seed;
+    t->resident_explicit = r.shifts != nullptr;
   }
   CUDA_OK(cudaMemsetAsync(ws + L.counters, 0, 32, st));
 

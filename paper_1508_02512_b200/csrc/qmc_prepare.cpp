@@ -361,7 +361,14 @@ static int qmc_finish_tables(qmc_tables *T, const qmc_options *opt) {
     T->const4.clear();
     T->chunks.clear();
   }
-  if (qmc_build_image3(T, opt ? opt->slot_budget_cplx_real : 0, opt ? opt->slot_budget_cplx : 0, opt ? opt->chunk_bytes : 0) != QMC_OK) {
+  // complex path: the default slot budgets first; a graph whose sectors need more sector-local products than a launch has
+  // room for (the paper's non-planar I_D at six variables) gets larger budgets before the generic kernel is the answer
+  int rc3 = qmc_build_image3(T, opt ? opt->slot_budget_cplx_real : 0, opt ? opt->slot_budget_cplx : 0, opt ? opt->chunk_bytes : 0);
+  if (rc3 != QMC_OK && !(opt && (opt->slot_budget_cplx_real > 0 || opt->slot_budget_cplx > 0))) {
+    const int retry[3][2] = {{40, 0}, {48, 26}, {56, 32}};
+    for (int q = 0; q < 3 && rc3 != QMC_OK; ++q) rc3 = qmc_build_image3(T, retry[q][0], retry[q][1], opt ? opt->chunk_bytes : 0);
+  }
+  if (rc3 != QMC_OK) {
     T->image3.clear();
     T->chunks3.clear();
     T->tab5.clear();

@@ -168,6 +168,8 @@ struct qmc_tables {
   const void *resident_ws = nullptr;  // workspace the image was last uploaded to
   int resident_kind = 0;              // 4: logarithm table (versions 4, 5), 1: version-1 image
   int resident_m = 0;                 // number of shift vectors resident in that workspace (0 = none)
+  uint64_t resident_seed = 0;         // seed that produced them ...
+  bool resident_explicit = false;     // ... or: they were passed explicitly (qmc_run.shifts)
   uint64_t cached_N = 0;              // generating vector cache
   uint64_t cached_z[QMC_MAXDIM] = {0};
   std::vector<double> shifts_host;    // staging of the shift vectors (must outlive the async H2D copy)

@@ -476,3 +476,37 @@ def test_batched_kinematic_points():
             assert np.allclose(one.coeff, r.sector_coeff[p], rtol=1e-11, atol=1e-13 * np.abs(A).max())
     with pytest.raises(q.QmcError):
         q.qmc_integrate(t, N, m, z=z, shifts=sh, mode=3, sectors=(0, 4))         # a batch is integrated as a whole
+
+
+def test_resident_shifts_are_keyed_by_their_seed():
+    """with tables_resident = 2 a different seed must not silently reuse the previous call's shift vectors."""
+    wl = qi.massless_box()
+    t = q.qmc_prepare(wl)
+    N, m = 16381, 4
+    z = qi.good_vector(N, 3)
+    a7 = q.qmc_integrate(t, N, m, z=z, seed=7)
+    q.qmc_integrate_async(t, N, m, z=z, seed=7, resident=0)
+    q.qmc_integrate_async(t, N, m, z=z, seed=8, resident=2)              # another seed: re-generated, not reused
+    r8 = q.qmc_result_fetch(t, m)
+    a8 = q.qmc_integrate(t, N, m, z=z, seed=8)
+    assert np.array_equal(r8.shift_totals, a8.shift_totals) and not np.array_equal(r8.shift_totals, a7.shift_totals)
+    q.qmc_integrate_async(t, N, m, z=z, seed=8, resident=2)              # the same seed: reused (nothing but the tables travels)
+    r8b = q.qmc_result_fetch(t, m)
+    assert np.array_equal(r8b.shift_totals, a8.shift_totals) and r8b.h2d_bytes < r8.h2d_bytes
+
+
+def test_two_ranks_on_two_gpus():
+    """the N > 1 path on hardware -- skipped unless two GPUs are visible (one GPU per call on this pool; the
+    sharding logic itself is covered by the world-size-2 gloo tests)."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    from paper_1508_02512_b200 import sharding
+    wl = qi.massless_box()
+    N, m = 99991, 4
+    z = qi.good_vector(N, 3)
+    full = q.qmc_integrate(q.qmc_prepare(wl), N, m, z=z, seed=wl.seed, device="cuda:0")
+    parts = [q.qmc_integrate(q.qmc_prepare(wl), N, m, z=z, seed=wl.seed, index_range=sharding.index_block(N, r, 2), device=f"cuda:{r}")
+             for r in range(2)]
+    tot = parts[0].shift_totals + parts[1].shift_totals
+    assert np.allclose(tot, full.shift_totals, rtol=1e-11, atol=1e-13)

@@ -180,3 +180,17 @@ def test_cbc_vector_error_codes():
         with pytest.raises(q.QmcError) as e:
             q.qmc_cbc_vector(N, dim)
         assert e.value.status == -1         # QMC_EINVAL
+
+
+def test_every_workload_gets_table_driven_tables():
+    """A graph the record builders cannot represent silently runs on the (correct, several times slower) generic kernel: the
+    parity tests cannot see that.  Every config, the triangle, the Table-1 kinematics and the paper's I_C / I_D (the latter
+    needs the larger slot budgets qmc_prepare retries with) must come out of qmc_prepare with table-driven chunks."""
+    for wl in qi.CONFIGS() + [qi.triangle(), qi.double_box(-2 / 3, -2 / 3, p2=(0, 0, -1, -1)), qi.paper_IC(), qi.paper_ID()]:
+        t = q.qmc_prepare(wl, eps_order=wl.eps_order, lam=wl.lam)
+        lines = t.describe().splitlines()[1:]
+        kind = "complex chunk" if wl.lam > 0 else "chunk"
+        assert lines and all(l.startswith(kind) for l in lines), (wl.name, t.describe()[:200])
+    # a budget that is too small on purpose still falls back (and says so: no chunks)
+    t = q.qmc_prepare(qi.double_box(), slot_budget=15, chunk_bytes=1000)
+    assert len(t.describe().splitlines()) == 1
