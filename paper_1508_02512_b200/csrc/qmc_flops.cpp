@@ -126,8 +126,7 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
         }
       f += 2.0 * K;  // weight and accumulate
     } else {
-      // version-5 scheme (qmc_kernels5.cuh; the arithmetic of version 3): real record 3, complex record 10 (complex
-      // product 6 + two FMAs)
+      // version-5 scheme (qmc_kernels5.cuh)
       auto pow_muls = [](int e) {
         int c = 0;
         for (int q = e; q > 1; q >>= 1) c += 1 + (q & 1);
@@ -148,28 +147,14 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
       if (ns > 0) f += (ns - 1) + 6.0 + 1.0;   // 1 / prod t_k of the singular variables, onto G0
       for (int j = 0; j < n; ++j)
         if (s.alpha[j] == -1) f += 2.0 + 2.0 * std::max(0, K - 3);   // t_k / beta_k, beta_k ln t_k, (.)^p / p!
+      // record streams of all corners (derivative polynomials, U^(z), F^(z)): constants 0, real one-factor record 2 (an FMA),
+      // real two-factor 3, complex one-factor 4, complex two-factor 10 -- counted by the table builder (qmc_image3.cpp)
+      if ((size_t)si < t->rec_flops5.size()) f += t->rec_flops5[si];
       for (int Z = 0; Z < nc; ++Z) {
         auto in_Z = [&](int j) { return pos_of[j] >= 0 && (Z >> pos_of[j] & 1); };
         int nfree = 0;
         for (int j = 0; j < n; ++j)
           if (!in_Z(j)) ++nfree;
-        // derivative polynomials: a monomial of d_i F (d_i d_k F) survives if what is left of it is free of Z variables
-        for (const QmcMono &m : s.F) {
-          for (int i = 0; i < n; ++i) {
-            if (!m.e[i]) continue;
-            for (int k = i; k < n; ++k) {
-              if (k == i ? m.e[i] < 2 : !m.e[k]) continue;
-              bool dead = false;
-              for (int j = 0; j < n; ++j)
-                if (in_Z(j) && m.e[j] - (j == i) - (j == k) > 0) dead = true;
-              if (!dead) f += 3.0;
-            }
-            bool dead = false;
-            for (int j = 0; j < n; ++j)
-              if (in_Z(j) && m.e[j] - (j == i) > 0) dead = true;
-            if (!dead) f += 3.0;
-          }
-        }
         f += n * 5.0 + (double)nfree * nfree * 3.0 + nfree * 3.0;  // rho, z, Jacobian entries
         for (int col = 0; col < n; ++col) {                         // elimination of the n x n complex matrix (no pivoting)
           f += F_CMUL;
@@ -180,13 +165,6 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
           if (col == 0) f -= 4.0 * rem + 4.0 * rem * rem;
         }
         f += 6.0 * nprod_c;                                         // complex slot program
-        for (int which = 0; which < 2; ++which)
-          for (const QmcMono &m : (which ? s.F : s.U)) {
-            bool dead = false;
-            for (int j = 0; j < n; ++j)
-              if (in_Z(j) && m.e[j]) dead = true;
-            if (!dead) f += 10.0;
-          }
         f += 2.0;  // G0 det
         for (int j = 0; j < n; ++j)
           if (!in_Z(j)) f += std::abs(s.alpha[j]) * F_CMUL;

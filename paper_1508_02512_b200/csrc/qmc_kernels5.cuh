@@ -93,71 +93,58 @@ __device__ __forceinline__ void corner5(const Qmc5Launch &p, const uint32_t cw, 
 #pragma unroll
   for (int k = 0; k < NS; ++k)
     if (Z >> k & 1) zv |= 1u << ((singvar >> (8 * k)) & 255u);
-  uint32_t cnt[CW * 4];
+  // corner block: counts of stream A (one-factor records) and of stream B (two-factor records) per polynomial, the constant
+  // terms c0[NPOLY], then the four streams (real A, real B, complex A, complex B), each closed by two sentinels
+  constexpr int C0W = (NPOLY + 1) / 2;
+  uint32_t cntA[CW * 4], cntB[CW * 4];
 #pragma unroll
   for (int q = 0; q < CW; ++q) {
-    const uint4 w = p.tab[cw + q];
-    cnt[4 * q] = w.x; cnt[4 * q + 1] = w.y; cnt[4 * q + 2] = w.z; cnt[4 * q + 3] = w.w;
+    const uint4 w = p.tab[cw + q], x = p.tab[cw + CW + q];
+    cntA[4 * q] = w.x; cntA[4 * q + 1] = w.y; cntA[4 * q + 2] = w.z; cntA[4 * q + 3] = w.w;
+    cntB[4 * q] = x.x; cntB[4 * q + 1] = x.y; cntB[4 * q + 2] = x.z; cntB[4 * q + 3] = x.w;
   }
   const unsigned char *tb = reinterpret_cast<const unsigned char *>(p.tab);
-  uint32_t rwb = (cw + CW) * 16u;  // byte offset of the current record
-  // ---- S4: gradient and Hessian of F^ at tau: one software-pipelined stream of real records --------------------------
+  const unsigned char *c0p = tb + (cw + 2 * CW) * 16u;  // c0[NPOLY] (f64)
+  uint32_t rwb = (cw + 2 * CW + C0W) * 16u;              // byte offset of the current record
+  // ---- S4: gradient and Hessian of F^ at tau.  Pass A: constant + one-factor records c * slot (one load, one FMA) at fixed
+  // positions; pass B: two-factor records c * slot * slot, ONE software-pipelined stream over all polynomials: the slot operands
+  // of the next record are requested before the current one is accumulated (operands one record ahead, table words two).
   double dv[NDERIV];
-  {
-    if (NDIM >= QMC5_PAIR_MIN_DIM) {
-      // Two records per iteration (the table builder pads every derivative polynomial to an even count): operands one
-      // PAIR ahead, offsets two pairs ahead (the stream ends with FOUR sentinel records).  With two warps per scheduler
-      // one record of lead did not cover the LDS latency: the DMUL of the single-record loop took half of the loop's
-      // samples waiting for its operands (profiles/r01p_final.md).
-      uint2 roA = *reinterpret_cast<const uint2 *>(tb + rwb + 8), roB = *reinterpret_cast<const uint2 *>(tb + rwb + 24);
-      double a0 = slot_at(slr, roA.x), b0 = slot_at(slr, roA.y), a1 = slot_at(slr, roB.x), b1 = slot_at(slr, roB.y);
-      roA = *reinterpret_cast<const uint2 *>(tb + rwb + 40);
-      roB = *reinterpret_cast<const uint2 *>(tb + rwb + 56);
-  #pragma unroll
-      for (int q = 0; q < NDERIV; ++q) {
-        const uint32_t n = (cnt[q >> 2] >> (8 * (q & 3))) & 255u;
-        double acc0 = 0.0, acc1 = 0.0;
-  #pragma unroll 1
-        for (uint32_t i = 0; i < n; i += 2) {
-          const uint2 rc0 = *reinterpret_cast<const uint2 *>(tb + rwb), rc1 = *reinterpret_cast<const uint2 *>(tb + rwb + 16);
-          const double v0 = a0 * b0, v1 = a1 * b1;
-          rwb += 32u;
-          a0 = slot_at(slr, roA.x);
-          b0 = slot_at(slr, roA.y);
-          a1 = slot_at(slr, roB.x);
-          b1 = slot_at(slr, roB.y);
-          roA = *reinterpret_cast<const uint2 *>(tb + rwb + 40);
-          roB = *reinterpret_cast<const uint2 *>(tb + rwb + 56);
-          acc0 = fma(u2d(rc0.x, rc0.y), v0, acc0);
-          acc1 = fma(u2d(rc1.x, rc1.y), v1, acc1);
-        }
-        dv[q] = acc0 + acc1;
+  {  // pass A: fixed positions per polynomial (qmc_tables.h: qmc5_capA), straight-line code with compile-time record offsets
+    const unsigned char *ra = tb + rwb;
+#pragma unroll
+    for (int q = 0; q < NDERIV; ++q) {
+      double acc = *reinterpret_cast<const double *>(c0p + q * 8);
+#pragma unroll
+      for (int k = 0; k < qmc5_capA(NDIM, L, q); ++k) {
+        const uint4 r = *reinterpret_cast<const uint4 *>(ra + (qmc5_posA(NDIM, L, q) + k) * 16);
+        acc = fma(u2d(r.x, r.y), slot_at(slr, r.z), acc);
       }
-      rwb += 64u;  // the four real sentinels
-    } else {
-      // offsets two records ahead (uniform registers), operands one record ahead: neither the uniform load nor the LDS
-      // sits on the critical path of an iteration (the block ends with TWO sentinel records)
-      uint2 ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);
-      double ra = slot_at(slr, ro.x), rb = slot_at(slr, ro.y);
-      ro = *reinterpret_cast<const uint2 *>(tb + rwb + 24);
-  #pragma unroll
-      for (int q = 0; q < NDERIV; ++q) {
-        const uint32_t n = (cnt[q >> 2] >> (8 * (q & 3))) & 255u;
-        double acc = 0.0;
-  #pragma unroll 1
-        for (uint32_t i = 0; i < n; ++i) {
-          const uint2 rc = *reinterpret_cast<const uint2 *>(tb + rwb);
-          const double v = ra * rb;
-          rwb += 16u;
-          ra = slot_at(slr, ro.x);
-          rb = slot_at(slr, ro.y);
-          ro = *reinterpret_cast<const uint2 *>(tb + rwb + 24);
-          acc = fma(u2d(rc.x, rc.y), v, acc);
-        }
-        dv[q] = acc;
-      }
-      rwb += 32u;  // the two real sentinels
+      dv[q] = acc;
     }
+    rwb += (uint32_t)qmc5_posA(NDIM, L, NDERIV) * 16u;
+  }
+  {
+    uint2 ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);
+    double ra = slot_at(slr, ro.x), rb = slot_at(slr, ro.y);
+    ro = *reinterpret_cast<const uint2 *>(tb + rwb + 24);
+#pragma unroll
+    for (int q = 0; q < NDERIV; ++q) {
+      const uint32_t n = (cntB[q >> 2] >> (8 * (q & 3))) & 255u;
+      double acc = dv[q];
+#pragma unroll 1
+      for (uint32_t i = 0; i < n; ++i) {
+        const uint2 rc = *reinterpret_cast<const uint2 *>(tb + rwb);
+        const double v = ra * rb;
+        rwb += 16u;
+        ra = slot_at(slr, ro.x);
+        rb = slot_at(slr, ro.y);
+        ro = *reinterpret_cast<const uint2 *>(tb + rwb + 24);
+        acc = fma(u2d(rc.x, rc.y), v, acc);
+      }
+      dv[q] = acc;
+    }
+    rwb += 32u;  // the two sentinels of stream B
   }
   // rho_i, z_i, J = 1 + i B
   cd rho[NDIM], J[NDIM][NDIM];
@@ -224,14 +211,37 @@ __device__ __forceinline__ void corner5(const Qmc5Launch &p, const uint32_t cw, 
     }
   }
   cd UF[2];
-  {
+  {  // pass A: constant + one-factor complex records c * slot
+    uint32_t ro = *reinterpret_cast<const uint32_t *>(tb + rwb + 8);
+    double2 ra = cslot_at(slc, ro);
+    ro = *reinterpret_cast<const uint32_t *>(tb + rwb + 24);
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+      const uint32_t n = (cntA[(NDERIV + q) >> 2] >> (8 * ((NDERIV + q) & 3))) & 255u;
+      cd acc = cd{*reinterpret_cast<const double *>(c0p + (NDERIV + q) * 8), 0.0};
+#pragma unroll 1
+      for (uint32_t i = 0; i < n; ++i) {
+        const uint2 rc = *reinterpret_cast<const uint2 *>(tb + rwb);
+        const double2 v = ra;
+        rwb += 16u;
+        ra = cslot_at(slc, ro);
+        ro = *reinterpret_cast<const uint32_t *>(tb + rwb + 24);
+        const double c = u2d(rc.x, rc.y);
+        acc.re = fma(c, v.x, acc.re);
+        acc.im = fma(c, v.y, acc.im);
+      }
+      UF[q] = acc;
+    }
+    rwb += 32u;
+  }
+  {  // pass B: two-factor complex records c * slot * slot
     uint2 ro = *reinterpret_cast<const uint2 *>(tb + rwb + 8);
     double2 ra = cslot_at(slc, ro.x), rb = cslot_at(slc, ro.y);
     ro = *reinterpret_cast<const uint2 *>(tb + rwb + 24);
 #pragma unroll
     for (int q = 0; q < 2; ++q) {
-      const uint32_t n = (cnt[(NDERIV + q) >> 2] >> (8 * ((NDERIV + q) & 3))) & 255u;
-      cd acc = cd{0.0, 0.0};
+      const uint32_t n = (cntB[(NDERIV + q) >> 2] >> (8 * ((NDERIV + q) & 3))) & 255u;
+      cd acc = UF[q];
 #pragma unroll 1
       for (uint32_t i = 0; i < n; ++i) {
         const uint2 rc = *reinterpret_cast<const uint2 *>(tb + rwb);

@@ -104,11 +104,13 @@ bool qmc4_kernel_available(int ndim, int loops, int kmax);
 //   w2 = {beta[0..3] (i8 x 4), beta[4..7], 0, 0}      w3,w4 = 1/beta of the singular positions (f64 x 4)      w5,w6 = beta (f64 x 4)
 //   w7 = word offsets of the corner blocks Z = 0..3
 //   w8.. = local real program, local complex program (each padded to a word), then records [G0][L0 x nL0]
-//   corner block Z: u8 counts[npoly] (npoly = n + n(n+1)/2 + 2: F_i, F_ik (i <= k), U, F; padded to a word) of the
-//     records that survive at the corner (monomials free of the variables of Z), then the real records of the
-//     derivative polynomials (each padded to an even count with a zero-coefficient record), four real sentinels, the
-//     complex records of U^ and F^, two complex sentinels.
-//   A record is duplicated into every corner block that needs it: each corner is one flat stream without skips.
+//   corner block Z (npoly = n + n(n+1)/2 + 2 polynomials: F_i, F_ik (i <= k), U, F; only the monomials free of the variables of Z
+//     survive): u8 countsA[npoly] (one-factor records per polynomial; padded to a word), u8 countsB[npoly] (two-factor records),
+//     f64 c0[npoly] (the constant monomials, summed on the host; padded to a word), then real A: qmc5_capA FIXED positions per
+//     derivative polynomial {f64 c, u32 off, 0}: c * slot (unused: c = 0; a surplus travels in B as c * slot * 1), then three
+//     record streams, each closed by two sentinels:  real B {f64 c, u32 off0, u32 off1}: c * slot * slot;  complex A, complex B
+//     the same over the complex slots (U^ and F^).
+//   A record is duplicated into every corner block that needs it: each corner is flat streams without skips.
 struct Qmc5Launch {
   const double *logtab;          // device: 64 x {1/c, -ln(1/c)}
   const double *shifts;

@@ -91,11 +91,22 @@ struct Qmc2Chunk {      // host description of one chunk
 // refilled at every corner, that serves U^(z) and F^(z).  Records are sorted per polynomial by group; a corner Z keeps
 // the groups disjoint from Z.
 #define QMC3_THREADS 128
-// complex path, n >= QMC5_PAIR_MIN_DIM: the derivative-polynomial record stream is walked two records at a time (every
-// polynomial padded to an even count, four sentinels); below, one at a time (two sentinels).  Measured on B200: the pair
-// walk gains on the long polynomials of n = 5 (cfg5 229.4 -> 223.4 ms) and loses to its padding on the short ones of
-// n = 3 (cfg3 25.3 -> 26.4 ms).
-#define QMC5_PAIR_MIN_DIM 5
+// Complex path, stream A of a corner (one-factor records c * slot of the derivative polynomials): FIXED positions per polynomial,
+// evaluated in straight-line code (a polynomial with fewer records fills up with c = 0, a surplus goes to stream B as
+// c * slot * 1).  Gradient polynomials d_i F^ get QMC5_CAPG positions, Hessian polynomials d_i d_k F^ QMC5_CAPH: for L loops F^ has
+// degree L + 1, so at one loop the Hessian is constant (no positions) and the gradient linear (up to n terms); at two loops the
+// Hessian is linear (measured on cfg5: 3.5 one-factor records per Hessian polynomial, 4.4 per gradient polynomial).
+#if defined(__CUDACC__)
+#define QMC5_HD __host__ __device__
+#else
+#define QMC5_HD
+#endif
+QMC5_HD constexpr int qmc5_capA(int ndim, int loops, int q) { return q < ndim ? (loops == 1 ? ndim : 6) : (loops == 1 ? 0 : 4); }
+QMC5_HD constexpr int qmc5_posA(int ndim, int loops, int q) {  // first position of polynomial q; q = number of derivative polynomials: the total
+  int p = 0;
+  for (int i = 0; i < q; ++i) p += qmc5_capA(ndim, loops, i);
+  return p;
+}
 #define QMC3_MAXSLOTS_R 56
 #define QMC3_MAXSLOTS_C 40
 #define QMC3_MAXLOCAL 8
@@ -164,6 +175,7 @@ struct qmc_tables {
   std::vector<uint32_t> secoff3, secend3;
   std::vector<Qmc2Chunk> chunks3;    // nslots = real slots; prog_off/prog_bytes cover the chunk header + both programs
   std::vector<int> chunk3_nslots_c, chunk3_max_local_c;
+  std::vector<double> rec_flops5;    // per sector: FP64 operations of the record streams of all its corners (flop model)
   // launcher state (host-side caches; not thread-safe by design: one tables object per stream)
   const void *resident_ws = nullptr;  // workspace the image was last uploaded to
   int resident_kind = 0;              // 4: logarithm table (versions 4, 5), 1: version-1 image
