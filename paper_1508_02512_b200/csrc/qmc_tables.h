@@ -101,7 +101,13 @@ struct Qmc2Chunk {      // host description of one chunk
 #else
 #define QMC5_HD
 #endif
-QMC5_HD constexpr int qmc5_capA(int ndim, int loops, int q) { return q < ndim ? (loops == 1 ? ndim : 6) : (loops == 1 ? 0 : 4); }
+#ifndef QMC5_CAPG2
+#define QMC5_CAPG2 6  // two loops: positions per gradient polynomial
+#define QMC5_CAPH2 3  // ... per Hessian polynomial.  Measured on B200 (cfg5 / paper I_C / I_D, ms per step): (4,3) 138.1 / 267.4 /
+                      // 288.2; (5,4) 140.4 / 267.6 / 284.6; (6,3) 136.9 / 263.7 / 282.5; (6,4) 139.8 / 268.8 / 284.1; (8,5) 143.6 / 273.1 /
+                      // 293.1; (10,6) 151.1 / 285.3 / 295.9; (12,8) 162.0 / 304.0 / 315.4 (larger tables: more launches)
+#endif
+QMC5_HD constexpr int qmc5_capA(int ndim, int loops, int q) { return q < ndim ? (loops == 1 ? ndim : QMC5_CAPG2) : (loops == 1 ? 0 : QMC5_CAPH2); }
 QMC5_HD constexpr int qmc5_posA(int ndim, int loops, int q) {  // first position of polynomial q; q = number of derivative polynomials: the total
   int p = 0;
   for (int i = 0; i < q; ++i) p += qmc5_capA(ndim, loops, i);
