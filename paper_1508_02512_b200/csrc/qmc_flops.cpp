@@ -138,10 +138,9 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
       int nprod_c = 0;  // complex product slots of the sector's chunk
       for (size_t ci = 0; ci < t->chunks3.size(); ++ci)
         if (si >= t->chunks3[ci].sec_begin && si < t->chunks3[ci].sec_end) nprod_c = t->chunk3_nslots_c[ci] - (n + 1);
-      int nL0 = 0, nbeta = 0;
+      int nL0 = 0;
       for (int j = 0; j < n; ++j) {
         if (s.alpha[j] != -1 && s.beta[j]) ++nL0;
-        if (s.beta[j]) ++nbeta;
       }
       f = 3.0 * (1 + nL0);
       if (ns > 0) f += (ns - 1) + 6.0 + 1.0;   // 1 / prod t_k of the singular variables, onto G0
@@ -169,7 +168,13 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
         for (int j = 0; j < n; ++j)
           if (!in_Z(j)) f += std::abs(s.alpha[j]) * F_CMUL;
         f += (pow_muls(eU) + (eU ? 1 : 0) + pow_muls(eF) + (eF ? 1 : 0)) * F_CMUL + F_CINV + F_CMUL;
-        if (t->kmax + __builtin_popcount(Z) > 0) f += (2 + nbeta) * (F_CLOG3 + 4.0) + 1.0;   // Lambda: only where the series window is longer than one term
+        if (t->kmax + __builtin_popcount(Z) > 0) {   // Lambda: only where the series window is longer than one term
+          // ONE complex logarithm: Q = U^aU1 F^aF1 prod_j rho_j^beta_j by complex products (numerator over denominator), ln Q,
+          // the winding number from single-precision phase estimates (no FP64) added by one FMA, + L0
+          double qmuls = pow_muls(std::max(t->aU1, 0)) + pow_muls(std::max(-t->aF1, 0));
+          for (int j = 0; j < n; ++j) qmuls += std::abs(s.beta[j]);
+          f += qmuls * F_CMUL + F_CINV + F_CMUL + F_CLOG3 + 2.0;
+        }
         f += (t->kmax + __builtin_popcount(Z)) * 8.0;               // series
       }
       for (int l = 0; l < ns; ++l)
