@@ -57,7 +57,10 @@ typedef struct {
   int32_t n_vertices, n_edges, n_legs;
   const int32_t *edge_u, *edge_v; /* [n_edges] end points; multi-edges allowed (bubble) */
   const double *edge_m2;          /* [n_edges] squared internal masses */
-  const int32_t *edge_nu;         /* [n_edges] propagator powers; NULL = all 1 (anything else: QMC_EUNSUPPORTED) */
+  const int32_t *edge_nu;         /* [n_edges] propagator powers nu_j in 1..8 (Eq. 1); NULL = all 1.  Powers other than 1
+                                     change the exponents of U and F (Eq. 6 with N_nu = sum nu_j) and put x_j^(nu_j-1) into the
+                                     integrand; such tables run on the generic kernel.  A sector that ends with an exponent
+                                     alpha_j <= -2 (it needs the p >= 1 Taylor terms of Eq. 11) is QMC_EUNSUPPORTED as before */
   const int32_t *leg_vertex;      /* [n_legs] vertex each external leg (all incoming) attaches to */
 } qmc_graph;
 

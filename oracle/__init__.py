@@ -87,17 +87,45 @@ class Oracle:
 
     @classmethod
     def from_workload(cls, wl, lam: Optional[float] = None, eps_order: Optional[int] = None, max_depth: int = 64,
-                      order: int = 0):
-        """order = 0: decomposition rule A.3 (U^ first); 1: F^ first (only to pin strategy independence of the totals)."""
+                      order: int = 0, taylor: bool = False):
+        """order = 0: decomposition rule A.3 (U^ first); 1: F^ first (only to pin strategy independence of the totals).
+        wl.nu: propagator powers (None = all 1).  taylor: accept alpha_j <= -2 on the real path (the p >= 1 Taylor terms of
+        Eq. 11) instead of status -3."""
         eu, ev, m2, lv, gram = wl.arrays()
+        nu = getattr(wl, "nu", None)
+        nu_arr = None if nu is None else np.ascontiguousarray(nu, dtype=np.int32)
+        if nu_arr is not None and nu_arr.size != wl.n_edges:
+            raise ValueError("oracle: one propagator power per edge")
         L = _load()
-        L.orc_build_order.restype = C.c_void_p
-        h = L.orc_build_order(C.c_int(wl.n_vertices), C.c_int(wl.n_edges), C.c_int(len(lv)), _p(eu, C.c_int),
-                              _p(ev, C.c_int), _p(m2, C.c_double), _p(lv, C.c_int), _p(gram, C.c_double),
-                              C.c_double(wl.lam if lam is None else lam),
-                              C.c_int(wl.eps_order if eps_order is None else eps_order), C.c_int(max_depth), C.c_int(order))
+        L.orc_build_nu.restype = C.c_void_p
+        h = L.orc_build_nu(C.c_int(wl.n_vertices), C.c_int(wl.n_edges), C.c_int(len(lv)), _p(eu, C.c_int),
+                           _p(ev, C.c_int), _p(m2, C.c_double), _p(lv, C.c_int), _p(gram, C.c_double),
+                           C.c_double(wl.lam if lam is None else lam),
+                           C.c_int(wl.eps_order if eps_order is None else eps_order), C.c_int(max_depth), C.c_int(order),
+                           None if nu_arr is None else _p(nu_arr, C.c_int), C.c_int(1 if taylor else 0))
         o = cls(h)
         o.n_edges = wl.n_edges
+        return o
+
+    @classmethod
+    def from_sector(cls, alpha, beta, U, F, aU, aF, eps_order: int = 0):
+        """ONE explicit real sector prod_j t_j^(alpha_j + beta_j eps) U(t)^(aU[0] + aU[1] eps) F(t)^(aF[0] + aF[1] eps) on the
+        unit cube (the form of Eq. 9), Taylor terms enabled.  U, F: lists of (coefficient, exponent tuple),
+        each with a constant term."""
+        alpha = np.ascontiguousarray(alpha, dtype=np.int32); beta = np.ascontiguousarray(beta, dtype=np.int32)
+        n = alpha.size
+        def flat(Q):
+            c = np.ascontiguousarray([q[0] for q in Q], dtype=np.float64)
+            e = np.ascontiguousarray([q[1] for q in Q], dtype=np.int32).reshape(len(Q), n)
+            return c, e
+        cU, eU = flat(U); cF, eF = flat(F)
+        L = _load()
+        L.orc_from_sector.restype = C.c_void_p
+        h = L.orc_from_sector(C.c_int(n), _p(alpha, C.c_int), _p(beta, C.c_int), C.c_int(len(U)), _p(cU, C.c_double),
+                              _p(eU, C.c_int), C.c_int(len(F)), _p(cF, C.c_double), _p(eF, C.c_int), C.c_int(aU[0]),
+                              C.c_int(aU[1]), C.c_int(aF[0]), C.c_int(aF[1]), C.c_int(eps_order))
+        o = cls(h)
+        o.n_edges = n + 1
         return o
 
     @classmethod
@@ -148,6 +176,17 @@ class Oracle:
         _load().orc_sector_integrand(self._h, C.c_int(s), _p(t, C.c_double), _p(out.view(np.float64), C.c_double))
         ns = self.sector(s)["n_sing"]
         return out[: self.k_max + ns + 1]
+
+    def sector_integrand_taylor(self, s: int, t: Sequence[float]):
+        """The same c_k(t) through the Taylor-term formula (sector_point_taylor), whatever the sector; real path only.
+        Returns (c, sum of |terms|)."""
+        t = np.ascontiguousarray(t, dtype=np.float64)
+        out = np.zeros(self.K + 8); ab = np.zeros(self.K + 8)
+        rc = _load().orc_sector_integrand_taylor(self._h, C.c_int(s), _p(t, C.c_double), _p(out, C.c_double), _p(ab, C.c_double))
+        if rc != 0:
+            raise RuntimeError(f"oracle: Taylor-term formula is real-path only ({rc})")
+        ns = self.sector(s)["n_sing"]
+        return out[: self.k_max + ns + 1], ab[: self.k_max + ns + 1]
 
     # ---- the path ---------------------------------------------------------------------
     def integrate(self, N: int, z, shifts, transform: int = 0, index_range=None, sectors=None, threads: int = 0):

@@ -31,6 +31,12 @@
 // counts, lattice exactness, tiling identity, invariants.
 // No function here is "parity unpinned" except the final VALUE of config 5 (no closed form
 // in the container; pinned by invariants only -- see DESIGN.md).
+//
+// Beyond the five configs (readings C28, C29): propagator powers nu_j in O2, and, on the real path only and
+// only when asked for (orc_build_nu(..., taylor = 1)), the p >= 1 Taylor terms of Eq. 11 for alpha_j <= -2 in
+// sector_point_taylor.  Pins (tests/test_oracle_taylor_terms.py): reduction to the double sum of O7 where no alpha_j <= -2,
+// monomial integrals, Dirichlet eta values, Euler's hypergeometric integral, the Beta function of the massless propagator
+// with powers, Dirichlet's integral of the triangle with a squared propagator, simplex quadrature of a massive bubble.
 // =====================================================================================
 #include <algorithm>
 #include <cmath>
@@ -65,6 +71,7 @@ struct Graph {
   int V = 0, P = 0, nlegs = 0;
   std::vector<int> eu, ev, legv;
   std::vector<double> m2, gram;  // gram[i*nlegs+j] = p_i . p_j, all legs incoming
+  std::vector<int> nu;           // propagator powers nu_j (Eq. 1); empty = all 1 (every config of BASELINE.json)
 };
 
 int uf_find(std::vector<int>& par, int a) {
@@ -165,6 +172,7 @@ struct Sector {
   std::vector<int> alpha, beta;  // t_j^{alpha_j + beta_j eps}
   Poly U, F;                     // both with a non-zero constant term (Eqs. 7-8, constants kept inside; R:C6)
   std::vector<int> sing, reg;    // sing: alpha == -1 ; reg: alpha >= 0
+  std::vector<int> deep;         // alpha <= -2: needs the p >= 1 Taylor terms of Eq. 11; only with Problem::taylor
   std::vector<int> jac;          // exponents of the accumulated Jacobian monomial alone (tiling pin)
 };
 
@@ -177,6 +185,7 @@ struct Problem {
   int kmax = 0, kmin = 0;
   int max_depth = 64;
   int order = 0;  // 0: rule A.3 (target U^ first); 1: F^ first (strategy-independence pin)
+  bool taylor = false;  // accept alpha_j <= -2 on the real path (sector_point_taylor); off = R:C9 (unsupported)
   std::vector<Sector> sectors;
   int status = 0;  // 0 ok, -2 depth, -3 unsupported
 };
@@ -266,6 +275,8 @@ void decompose(Problem& pb, int primary, Poly U, Poly F, std::vector<int> alpha,
         s.sing.push_back(j);
       } else if (alpha[j] >= 0)
         s.reg.push_back(j);
+      else if (pb.taylor && pb.lambda == 0.0 && beta[j] != 0)
+        s.deep.push_back(j);  // p >= 1 Taylor terms of Eq. 11 (f3; real path only)
       else
         pb.status = -3;  // alpha <= -2 needs the p>=1 Taylor terms of Eq. 11 (R:C9)
     }
@@ -309,10 +320,13 @@ void decompose(Problem& pb, int primary, Poly U, Poly F, std::vector<int> alpha,
 void build_sectors(Problem& pb) {
   int P = pb.g.P;
   pb.n = P - 1;
-  // exponents for nu_j = 1: a_U = P-(L+1)D/2, a_F = -(P-LD/2), D = 4-2eps
-  pb.aU0 = P - 2 * (pb.L + 1);
+  // exponents (Eq. 6; restored Eq. 2, R:C1): a_U = N_nu-(L+1)D/2, a_F = -(N_nu-LD/2), D = 4-2eps, N_nu = sum_j nu_j
+  // (= P when every nu_j = 1, the case of all configs); the integrand carries prod_j x_j^{nu_j-1}
+  int Nnu = 0;
+  for (int j = 0; j < P; ++j) Nnu += pb.g.nu.empty() ? 1 : pb.g.nu[j];
+  pb.aU0 = Nnu - 2 * (pb.L + 1);
   pb.aU1 = pb.L + 1;
-  pb.aF0 = -(P - 2 * pb.L);
+  pb.aF0 = -(Nnu - 2 * pb.L);
   pb.aF1 = -pb.L;
   pb.sectors.clear();
   for (int l = 0; l < P; ++l) {
@@ -328,11 +342,13 @@ void build_sectors(Problem& pb) {
         poly_add(R, e, t.second);
       }
     }
-    std::vector<int> zero(pb.n, 0);
-    decompose(pb, l, Ul, Fl, zero, zero, zero, 0);
+    std::vector<int> zero(pb.n, 0), alpha0;
+    for (int j = 0; j < P; ++j)
+      if (j != l) alpha0.push_back(pb.g.nu.empty() ? 0 : pb.g.nu[j] - 1);  // x_j^{nu_j-1}; x_l = 1
+    decompose(pb, l, Ul, Fl, alpha0, zero, zero, 0);
   }
   int smax = 0;
-  for (auto& s : pb.sectors) smax = std::max(smax, (int)s.sing.size());
+  for (auto& s : pb.sectors) smax = std::max(smax, (int)(s.sing.size() + s.deep.size()));
   pb.kmin = -smax;
 }
 
@@ -575,6 +591,192 @@ void sector_point(const Problem& pb, const Sector& s, const double* t, const dou
   }
 }
 
+// ------------------------------------------------------------------------------------
+// f3: the p >= 1 Taylor terms of Eq. 11 for alpha_j <= -2.  REAL PATH ONLY (lambda = 0).
+//
+// For ONE variable with exponent -a + beta eps, a >= 1 (Eqs. 10-12, with p = 0 .. a-1):
+//   int_0^1 dt t^{-a+beta eps} g(t) = sum_{p<a} g_p / (p+1-a + beta eps)
+//                                    + int_0^1 dt t^{-a+beta eps} [ g(t) - sum_{p<a} g_p t^p ],     g_p = g^(p)(0) / p!
+// (the first sum is the integral of the Taylor polynomial; p = a-1 is the pole 1/(beta eps), the others are regular at eps = 0:
+// 1/(-q + beta eps) = -(1/q) sum_m (beta eps / q)^m, q = a-1-p > 0).  Applied to every variable of V = {j : alpha_j <= -1}
+// this is (A.4a) of SURVEY App. A with a Taylor order p_j on every variable of S (integrated analytically) and of R
+// (subtraction term taken):
+//   c(eps) = sum_{S, R disjoint subsets of V} sum_{p_j <= a_j - 1, j in S u R}
+//              prod_{j notin S u R} t_j^{-a_j}  prod_{j in R} ( - t_j^{p_j - a_j} )  prod_{j in S} 1/(p_j+1-a_j + beta_j eps)
+//              e^{eps sum_{j notin S} beta_j ln t_j}  [ prod_{j in S u R} t_j^{p_j} ] ( G e^{eps Lambda} )
+// where [.] takes the Taylor coefficient in the variables of Z = S u R at t_Z = 0 and G, Lambda are those of `corner` (Eq. 9
+// integrand).  With a_j = 1 everywhere (p_j = 0) this IS (A.4a); tests pin that the two functions then agree.
+// The Taylor coefficients come from truncated power-series arithmetic ("jets") in the variables of Z: U^ and F^ are
+// polynomials, so their jets are read off the monomial table; powers, reciprocal and logarithm of a jet a = a0 + x follow
+// from the series of f(a0 + x) in the nilpotent part x.
+// ------------------------------------------------------------------------------------
+struct JetShape {
+  std::vector<int> ord, stride;        // per jet variable: highest power kept; stride of its power in the dense index
+  int size = 1, total = 0;             // number of coefficients; sum of ord (x^{total+1} = 0 for a jet x without constant term)
+  std::vector<std::vector<int>> midx;  // dense index -> multi-index
+  explicit JetShape(const std::vector<int>& o) : ord(o) {
+    for (int v : ord) {
+      stride.push_back(size);
+      size *= v + 1;
+      total += v;
+    }
+    midx.assign(size, std::vector<int>(ord.size(), 0));
+    for (int i = 0; i < size; ++i)
+      for (size_t v = 0; v < ord.size(); ++v) midx[i][v] = (i / stride[v]) % (ord[v] + 1);
+  }
+};
+typedef std::vector<double> Jet;  // coefficient of prod_v d_v^{p_v} at index sum_v p_v stride_v
+
+Jet jet_mul(const JetShape& sh, const Jet& a, const Jet& b) {  // truncated product
+  Jet r(sh.size, 0.0);
+  for (int i = 0; i < sh.size; ++i)
+    for (int k = 0; k < sh.size; ++k) {
+      int idx = 0;
+      bool keep = true;
+      for (size_t v = 0; v < sh.ord.size(); ++v) {
+        int p = sh.midx[i][v] + sh.midx[k][v];
+        if (p > sh.ord[v]) keep = false;
+        idx += p * sh.stride[v];
+      }
+      if (keep) r[idx] += a[i] * b[k];
+    }
+  return r;
+}
+
+// f(a) for a jet a = a0 + x:  sum_{m=0}^{total} c[m] x^m  with c[m] = f^(m)(a0) / m!
+Jet jet_series(const JetShape& sh, const Jet& a, const std::vector<double>& c) {
+  Jet x = a, xm(sh.size, 0.0), r(sh.size, 0.0);
+  x[0] = 0.0;
+  xm[0] = 1.0;
+  for (int m = 0; m <= sh.total; ++m) {
+    for (int i = 0; i < sh.size; ++i) r[i] += c[m] * xm[i];
+    xm = jet_mul(sh, xm, x);
+  }
+  return r;
+}
+Jet jet_recip(const JetShape& sh, const Jet& a) {  // 1/(a0+x) = sum_m (-1)^m x^m / a0^{m+1}
+  std::vector<double> c(sh.total + 1);
+  for (int m = 0; m <= sh.total; ++m) c[m] = ((m & 1) ? -1.0 : 1.0) / ipow(a[0], m + 1);
+  return jet_series(sh, a, c);
+}
+Jet jet_log(const JetShape& sh, const Jet& a) {  // ln(a0+x) = ln a0 + sum_{m>=1} (-1)^{m+1} x^m / (m a0^m)
+  std::vector<double> c(sh.total + 1);
+  c[0] = std::log(a[0]);
+  for (int m = 1; m <= sh.total; ++m) c[m] = ((m & 1) ? 1.0 : -1.0) / (m * ipow(a[0], m));
+  return jet_series(sh, a, c);
+}
+Jet jet_ipow(const JetShape& sh, const Jet& a, int e) {  // integer power, e of either sign
+  Jet base = e >= 0 ? a : jet_recip(sh, a), r(sh.size, 0.0);
+  r[0] = 1.0;
+  for (int k = 0; k < std::abs(e); ++k) r = jet_mul(sh, r, base);
+  return r;
+}
+
+// c_k(t), k = -|V| .. kmax, of a real sector by the formula above.  out[k + |V|]; absout = sum of |terms| (R:C19).
+void sector_point_taylor(const Problem& pb, const Sector& s, const double* t, const double* lnt, std::vector<double>& out,
+                         std::vector<double>& absout) {
+  std::vector<int> V, a;  // variables with alpha <= -1 in index order, a_b = -alpha
+  for (int j = 0; j < pb.n; ++j)
+    if (s.alpha[j] <= -1) {
+      V.push_back(j);
+      a.push_back(-s.alpha[j]);
+    }
+  const int nv = (int)V.size(), M = pb.kmax + nv;  // the series of G e^{eps Lambda} is needed through eps^M
+  out.assign(M + 1, 0.0);
+  absout.assign(M + 1, 0.0);
+  double Greg = 1.0, Lreg = 0.0;  // regular variables (alpha >= 0): prod t^alpha and sum beta ln t, as in `corner`
+  for (int j = 0; j < pb.n; ++j)
+    if (s.alpha[j] >= 0) {
+      Greg *= ipow(t[j], s.alpha[j]);
+      Lreg += s.beta[j] * lnt[j];
+    }
+  for (int Z = 0; Z < (1 << nv); ++Z) {
+    std::vector<int> zb, ord, pos_of(pb.n, -1);  // jet variables: the members of Z, each kept through power a_b - 1
+    for (int b = 0; b < nv; ++b)
+      if (Z >> b & 1) {
+        pos_of[V[b]] = (int)zb.size();
+        zb.push_back(b);
+        ord.push_back(a[b] - 1);
+      }
+    JetShape sh(ord);
+    // a monomial c prod_j t_j^{e_j} puts c prod_{j notin Z} t_j^{e_j} on the coefficient of prod_{j in Z} t_j^{e_j}
+    auto poly_jet = [&](const Poly& Q) {
+      Jet r(sh.size, 0.0);
+      for (auto& term : Q) {
+        double c = term.second;
+        int idx = 0;
+        bool keep = true;
+        for (int j = 0; j < pb.n; ++j) {
+          int e = term.first[j];
+          if (pos_of[j] < 0)
+            c *= ipow(t[j], e);
+          else if (e > ord[pos_of[j]])
+            keep = false;
+          else
+            idx += e * sh.stride[pos_of[j]];
+        }
+        if (keep) r[idx] += c;
+      }
+      return r;
+    };
+    Jet Uj = poly_jet(s.U), Fj = poly_jet(s.F);
+    Jet G = jet_mul(sh, jet_ipow(sh, Uj, pb.aU0), jet_ipow(sh, Fj, pb.aF0));  // U^aU0 F^aF0 prod_reg t^alpha
+    for (double& v : G) v *= Greg;
+    Jet lU = jet_log(sh, Uj), lF = jet_log(sh, Fj), Lam(sh.size);              // aU1 ln U + aF1 ln F + sum_reg beta ln t
+    for (int i = 0; i < sh.size; ++i) Lam[i] = pb.aU1 * lU[i] + pb.aF1 * lF[i];
+    Lam[0] += Lreg;
+    for (int S = Z;; S = (S - 1) & Z) {  // all splits Z = S u R
+      const int R = Z & ~S;
+      Jet Lt = Lam;  // + sum_{j notin S} beta_j ln t_j (the regulators of the variables of R are kept)
+      for (int b = 0; b < nv; ++b)
+        if (!(S >> b & 1)) Lt[0] += s.beta[V[b]] * lnt[V[b]];
+      std::vector<Jet> T(M + 1);  // T[k] = G Lt^k / k!: the coefficient of eps^k of G e^{eps Lt}
+      T[0] = G;
+      for (int k = 1; k <= M; ++k) {
+        T[k] = jet_mul(sh, T[k - 1], Lt);
+        for (double& v : T[k]) v /= k;
+      }
+      for (int idx = 0; idx < sh.size; ++idx) {  // every assignment of Taylor orders p to the variables of Z
+        double scalar = 1.0;
+        int npole = 0;
+        std::vector<double> ser(M + 1);
+        for (int k = 0; k <= M; ++k) ser[k] = T[k][idx];
+        for (int b = 0; b < nv; ++b) {
+          const int j = V[b];
+          if (!(Z >> b & 1)) {
+            scalar *= 1.0 / ipow(t[j], a[b]);  // untouched: t^{-a}
+            continue;
+          }
+          const int p = sh.midx[idx][pos_of[j]], q = a[b] - 1 - p;
+          if (R >> b & 1) {
+            scalar *= -1.0 / ipow(t[j], a[b] - p);  // subtraction term: - t^{p-a}
+          } else if (q == 0) {
+            scalar *= 1.0 / s.beta[j];  // 1/(beta eps)
+            ++npole;
+          } else {  // 1/(-q + beta eps) = -(1/q) sum_m (beta eps / q)^m
+            std::vector<double> r(M + 1, 0.0);
+            for (int k = 0; k <= M; ++k) {
+              double gm = -1.0 / q;
+              for (int m = 0; k + m <= M; ++m) {
+                r[k + m] += ser[k] * gm;
+                gm *= (double)s.beta[j] / q;
+              }
+            }
+            ser = r;
+          }
+        }
+        for (int k = -nv; k <= pb.kmax; ++k) {
+          if (k + npole < 0) continue;
+          double term = scalar * ser[k + npole];
+          out[k + nv] += term;
+          absout[k + nv] += std::fabs(term);
+        }
+      }
+      if (S == 0) break;
+    }
+  }
+}
+
 }  // namespace
 
 // =====================================================================================
@@ -594,10 +796,24 @@ orc_problem* orc_build(int V, int P, int nlegs, const int* eu, const int* ev, co
   return orc_build_order(V, P, nlegs, eu, ev, m2, legv, gram, lambda, kmax, max_depth, 0);
 }
 // order = 0: rule A.3 (U^ first); 1: F^ first (strategy-independence pin only)
+orc_problem* orc_build_nu(int V, int P, int nlegs, const int* eu, const int* ev, const double* m2, const int* legv,
+                          const double* gram, double lambda, int kmax, int max_depth, int order, const int* nu, int taylor);
 orc_problem* orc_build_order(int V, int P, int nlegs, const int* eu, const int* ev, const double* m2, const int* legv,
                              const double* gram, double lambda, int kmax, int max_depth, int order) {
+  return orc_build_nu(V, P, nlegs, eu, ev, m2, legv, gram, lambda, kmax, max_depth, order, nullptr, 0);
+}
+// nu: propagator powers [P] (NULL = all 1); taylor != 0: accept alpha_j <= -2 on the real path (f3, sector_point_taylor)
+orc_problem* orc_build_nu(int V, int P, int nlegs, const int* eu, const int* ev, const double* m2, const int* legv,
+                          const double* gram, double lambda, int kmax, int max_depth, int order, const int* nu, int taylor) {
   orc_problem* h = new orc_problem;
   h->pb.order = order;
+  h->pb.taylor = taylor != 0;
+  if (nu) h->pb.g.nu.assign(nu, nu + P);
+  for (int v : h->pb.g.nu)
+    if (v < 1) {
+      delete h;
+      return nullptr;
+    }
   Graph& g = h->pb.g;
   g.V = V;
   g.P = P;
@@ -692,7 +908,7 @@ void orc_sector_meta(const orc_problem* h, int s, int* meta, int* alpha, int* be
   meta[0] = sc.primary;
   meta[1] = (int)sc.U.size();
   meta[2] = (int)sc.F.size();
-  meta[3] = (int)sc.sing.size();
+  meta[3] = (int)(sc.sing.size() + sc.deep.size());  // variables with alpha <= -1 = highest pole order of the sector
   for (int j = 0; j < h->pb.n; ++j) {
     alpha[j] = sc.alpha[j];
     beta[j] = sc.beta[j];
@@ -758,12 +974,66 @@ void orc_sector_integrand(const orc_problem* h, int s, const double* tpt, double
     }
   } else {
     std::vector<double> o;
-    sector_point<double>(pb, sc, tpt, lnt.data(), o, absout, cnt);
+    if (!sc.deep.empty())
+      sector_point_taylor(pb, sc, tpt, lnt.data(), o, absout);
+    else
+      sector_point<double>(pb, sc, tpt, lnt.data(), o, absout, cnt);
     for (size_t k = 0; k < o.size(); ++k) {
       out[2 * k] = o[k];
       out[2 * k + 1] = 0.0;
     }
   }
+}
+
+// the same through sector_point_taylor whatever the sector (real path only): pins that the Taylor formula reduces to
+// (A.4a) when every alpha_j >= -1.  out[kmax + n_sing + 1] values, absout likewise
+int orc_sector_integrand_taylor(const orc_problem* h, int s, const double* tpt, double* out, double* absout_) {
+  const Problem& pb = h->pb;
+  if (pb.lambda > 0.0) return -3;
+  const Sector& sc = pb.sectors[s];
+  std::vector<double> lnt(pb.n), o, ab;
+  for (int j = 0; j < pb.n; ++j) lnt[j] = std::log(tpt[j]);
+  sector_point_taylor(pb, sc, tpt, lnt.data(), o, ab);
+  for (size_t k = 0; k < o.size(); ++k) {
+    out[k] = o[k];
+    absout_[k] = ab[k];
+  }
+  return 0;
+}
+
+// ONE explicit real sector  prod_j t_j^{alpha_j + beta_j eps} U(t)^{aU0 + aU1 eps} F(t)^{aF0 + aF1 eps}  on (0,1)^n (the form of
+// Eq. 9), Taylor terms enabled: for pins whose closed form is elementary.  Polynomials as coeff[nterms], expo[nterms*n].
+orc_problem* orc_from_sector(int n, const int* alpha, const int* beta, int nU, const double* cU, const int* eU, int nF,
+                             const double* cF, const int* eF, int aU0, int aU1, int aF0, int aF1, int kmax) {
+  orc_problem* h = new orc_problem;
+  Problem& pb = h->pb;
+  pb.n = n;
+  pb.taylor = true;
+  pb.kmax = kmax;
+  pb.aU0 = aU0;
+  pb.aU1 = aU1;
+  pb.aF0 = aF0;
+  pb.aF1 = aF1;
+  Sector sc;
+  sc.alpha.assign(alpha, alpha + n);
+  sc.beta.assign(beta, beta + n);
+  sc.jac.assign(n, 0);
+  for (int m = 0; m < nU; ++m) poly_add(sc.U, Expo(eU + (size_t)m * n, eU + (size_t)(m + 1) * n), cU[m]);
+  for (int m = 0; m < nF; ++m) poly_add(sc.F, Expo(eF + (size_t)m * n, eF + (size_t)(m + 1) * n), cF[m]);
+  for (int j = 0; j < n; ++j) {
+    if (alpha[j] >= 0)
+      sc.reg.push_back(j);
+    else if (beta[j] == 0)
+      pb.status = -3;
+    else if (alpha[j] == -1)
+      sc.sing.push_back(j);
+    else
+      sc.deep.push_back(j);
+  }
+  if (!has_const(sc.U) || !has_const(sc.F)) pb.status = -3;
+  pb.kmin = -(int)(sc.sing.size() + sc.deep.size());
+  pb.sectors.push_back(sc);
+  return h;
 }
 
 // O8: S[sector][k-kmin][shift][2] and A[sector][k-kmin][shift] over the lattice indices
@@ -799,7 +1069,7 @@ int orc_integrate(const orc_problem* h, uint64_t N, const uint64_t* z, int m, co
     for (int si = 0; si < nsec; ++si)
       for (int kap = 0; kap < m; ++kap) {
         const Sector& sc = pb.sectors[sec_begin + si];
-        int ns = (int)sc.sing.size(), off = -ns - pb.kmin;  // order k sits at index k - kmin
+        int ns = (int)(sc.sing.size() + sc.deep.size()), off = -ns - pb.kmin;  // order k sits at index k - kmin
         std::vector<Neumaier> accRe(K), accIm(K), accA(K);
         for (uint64_t c = 0; c < i_count; ++c) {
           uint64_t i = i_begin + c * i_step;
@@ -820,7 +1090,10 @@ int orc_integrate(const orc_problem* h, uint64_t N, const uint64_t* z, int m, co
                 accA[off + k].add(w * absout[k]);
               }
           } else {
-            sector_point<double>(pb, sc, t.data(), lnt.data(), od, absout, cnt);
+            if (!sc.deep.empty())
+              sector_point_taylor(pb, sc, t.data(), lnt.data(), od, absout);  // f3: alpha_j <= -2 (Eq. 11 with p >= 1)
+            else
+              sector_point<double>(pb, sc, t.data(), lnt.data(), od, absout, cnt);
             for (auto& v : od) finite = finite && std::isfinite(v);
             if (finite)
               for (size_t k = 0; k < od.size(); ++k) {

@@ -193,19 +193,24 @@ class Tables:
 def qmc_prepare(wl=None, *, n_vertices=None, edges=None, leg_vertex=None, gram=None, eps_order: int = 0,
                 lam: float = 0.0, transform: int = 0, max_depth: int = 0, lattice: int = 0, slot_budget: int = 0,
                 chunk_bytes: int = 0, threads: int = 0, slot_budget_cplx_real: int = 0, slot_budget_cplx: int = 0,
-                dense_template: int = 0) -> Tables:
+                dense_template: int = 0, nu=None) -> Tables:
     """qmc_prepare(graph, kinematics, eps_order) -> sector tables.  `wl` is a qmc_inputs.Workload, or pass the
     graph explicitly (edges = [(u, v, m^2), ...]).  slot_budget .. slot_budget_cplx are the table-layout fields of
-    qmc_options (0 = the library's defaults)."""
+    qmc_options (0 = the library's defaults).  nu: propagator powers, one per edge (qmc_graph.edge_nu; None = all 1)."""
     if wl is not None:
         n_vertices, edges, leg_vertex, gram = wl.n_vertices, wl.edges, wl.leg_vertex, wl.gram
+        if nu is None:
+            nu = getattr(wl, "nu", None)
     eu = np.ascontiguousarray([e[0] for e in edges], dtype=np.int32)
     ev = np.ascontiguousarray([e[1] for e in edges], dtype=np.int32)
     m2 = np.ascontiguousarray([e[2] for e in edges], dtype=np.float64)
     lv = np.ascontiguousarray(leg_vertex, dtype=np.int32)
     gr = np.ascontiguousarray(gram, dtype=np.float64)
-    g = qmc_graph(n_vertices, len(edges), len(lv), _ptr(eu, C.c_int32), _ptr(ev, C.c_int32), _ptr(m2, C.c_double), None,
-                  _ptr(lv, C.c_int32))
+    nu_arr = None if nu is None else np.ascontiguousarray(nu, dtype=np.int32)
+    if nu_arr is not None and nu_arr.size != len(edges):
+        raise ValueError("qmc_prepare: one propagator power per edge")
+    g = qmc_graph(n_vertices, len(edges), len(lv), _ptr(eu, C.c_int32), _ptr(ev, C.c_int32), _ptr(m2, C.c_double),
+                  None if nu_arr is None else _ptr(nu_arr, C.c_int32), _ptr(lv, C.c_int32))
     k = qmc_kinematics(_ptr(gr, C.c_double))
     o = qmc_options(lam, transform, max_depth, lattice, slot_budget, chunk_bytes, threads, slot_budget_cplx_real,
                     slot_budget_cplx, dense_template)

@@ -137,7 +137,7 @@ static int qmc_build_sectors(const qmc_graph *g, const qmc_kinematics *kin, int 
   if (eps_order > QMC_KMAX_MAX) return QMC_EUNSUPPORTED;
   for (int e = 0; e < P; ++e) {
     if (g->edge_u[e] < 0 || g->edge_u[e] >= V || g->edge_v[e] < 0 || g->edge_v[e] >= V) return QMC_EINVAL;
-    if (g->edge_nu && g->edge_nu[e] != 1) return QMC_EUNSUPPORTED;
+    if (g->edge_nu && (g->edge_nu[e] < 1 || g->edge_nu[e] > 8)) return QMC_EINVAL;  // propagator powers: positive integers
   }
   for (int a = 0; a < NL; ++a)
     if (g->leg_vertex[a] < 0 || g->leg_vertex[a] >= V) return QMC_EINVAL;
@@ -185,13 +185,21 @@ static int qmc_build_sectors(const qmc_graph *g, const qmc_kinematics *kin, int 
   canonical(F);
   if (F.empty()) return QMC_EINVAL;  // scaleless integral
 
-  // ---- exponents (Eq. 6, D = 4 - 2 eps, nu_j = 1) -----------------------------------------
+  // ---- exponents (Eq. 6, D = 4 - 2 eps): a_U = N_nu - (L+1) D/2, a_F = -(N_nu - L D/2), N_nu = sum_j nu_j; the integrand
+  //      carries prod_j x_j^(nu_j - 1) (restored Eq. 2, R:C1).  nu_j = 1 everywhere: N_nu = P, the case the table-driven kernels
+  //      are compiled for (their exponents are functions of n and L); any other powers run on the generic kernel --------------
+  int Nnu = 0;
+  for (int e = 0; e < P; ++e) Nnu += g->edge_nu ? g->edge_nu[e] : 1;
+  if (T->sectors.empty())
+    T->generic_only = (Nnu != P);
+  else if (T->generic_only != (Nnu != P))
+    return QMC_EINVAL;
   T->n = P - 1;
   T->P = P;
   T->L = L;
-  T->aU0 = P - 2 * (L + 1);
+  T->aU0 = Nnu - 2 * (L + 1);
   T->aU1 = L + 1;
-  T->aF0 = -(P - 2 * L);
+  T->aF0 = -(Nnu - 2 * L);
   T->aF1 = -L;
   T->lambda = opt ? opt->lambda : 0.0;
   T->transform = opt ? opt->transform : 0;
@@ -209,6 +217,9 @@ static int qmc_build_sectors(const qmc_graph *g, const qmc_kinematics *kin, int 
     nd.depth = 0;
     std::memset(nd.alpha, 0, sizeof nd.alpha);
     std::memset(nd.beta, 0, sizeof nd.beta);
+    if (g->edge_nu)  // x_j^(nu_j - 1) of the variables that stay (x_l = 1)
+      for (int e = 0, j = 0; e < P; ++e)
+        if (e != l) nd.alpha[j++] = g->edge_nu[e] - 1;
     for (int which = 0; which < 2; ++which) {
       const Poly &Q = which ? F : U;
       Poly &R = which ? nd.F : nd.U;
@@ -354,6 +365,10 @@ static int qmc_finish_tables(qmc_tables *T, const qmc_options *opt) {
   // table-driven kernels: real path (version 4) and complex path (version 5).  What a builder cannot represent falls back
   // to the generic kernel: on failure EVERYTHING the builder left behind is dropped, so that qmc_integrate sees no
   // half-built tables
+  if (T->generic_only) {  // propagator powers other than 1: exponents the table-driven kernels are not compiled for
+    T->sec_cost.assign(T->sectors.size(), 1.0);
+    return QMC_OK;
+  }
   if (qmc_build_tables4(T, opt ? opt->slot_budget : 0, opt ? opt->chunk_bytes : 0, opt ? opt->threads : 0, opt ? opt->dense_template : 0) != QMC_OK) {
     T->tab4.clear();
     T->secoff4.clear();

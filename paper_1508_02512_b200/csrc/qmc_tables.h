@@ -187,6 +187,7 @@ struct qmc_tables {
   int resident_kind = 0;              // 4: logarithm table (versions 4, 5), 1: version-1 image
   int resident_m = 0;                 // number of shift vectors resident in that workspace (0 = none)
   uint64_t resident_seed = 0;         // seed that produced them ...
+  bool generic_only = false;          // propagator powers other than 1: only the generic kernel has run-time exponents
   bool resident_explicit = false;     // ... or: they were passed explicitly (qmc_run.shifts)
   uint64_t cached_N = 0;              // generating vector cache
   uint64_t cached_z[QMC_MAXDIM] = {0};

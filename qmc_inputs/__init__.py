@@ -12,7 +12,7 @@ Eqs. 22-27); the paper measures on no dataset.  Edge lists fol
 from __future__ import annotations
 
 from dataclasses import dataclass, field
-from typing import List, Sequence, Tuple
+from typing import List, Optional, Sequence, Tuple
 
 import numpy as np
 
@@ -36,6 +36,7 @@ class Workload:
     m: int = 16                                  # number of random shifts
     seed: int = 0
     meta: dict = field(default_factory=dict)
+    nu: Optional[Sequence[int]] = None           # propagator powers nu_k; None = all 1, as in every config
 
     @property
     def n_edges(self) -> int:

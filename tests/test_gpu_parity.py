@@ -510,3 +510,37 @@ def test_two_ranks_on_two_gpus():
              for r in range(2)]
     tot = parts[0].shift_totals + parts[1].shift_totals
     assert np.allclose(tot, full.shift_totals, rtol=1e-11, atol=1e-13)
+
+
+def test_propagator_powers_run_on_the_generic_kernel():
+    """qmc_graph.edge_nu (Eq. 1): N_nu = sum nu_j in the exponents of Eq. 6, x_j^(nu_j - 1) in the integrand.  The
+    table-driven kernels have their exponents compiled in for nu_j = 1; other powers run on the generic kernel by themselves.
+    Parity against the oracle on the product's tables (that these are the sectors of the oracle's own decomposition is a CPU
+    test: tests/test_product_host.py), and two closed forms on the GPU numbers."""
+    import dataclasses
+    import mpmath as mp
+    # real path, no singular variable: massive bubble with a squared propagator against the simplex form of the parameter integral
+    p2, m1, m2 = -1.3, 1.0, 2.5
+    wl = dataclasses.replace(qi.bubble(p2, m1, m2), nu=(2, 1), eps_order=2)
+    r, f, S, A, _ = parity(wl, 10007, 6)
+    assert "real-path tables 0 B" in q.qmc_prepare(wl, eps_order=2).describe()
+    F = lambda x: -p2 * x * (1 - x) + m1 * x + m2 * (1 - x)
+    want = [float(mp.quad(lambda x: x * F(x) ** (2 - 3) * (-mp.log(F(x))) ** k / mp.factorial(k), [0, 1])) for k in range(3)]
+    assert np.all(np.abs(f.coeff.real - want) <= 4 * f.err.real + 1e-12), (f.coeff.real, f.err.real, want)
+    # real path, one pole: massless propagator with powers (2, 1): J = (-p^2)^(-1-eps) B(-eps, 1-eps)
+    wl = dataclasses.replace(qi.bubble(-1.7, 0.0, 0.0), nu=(2, 1), eps_order=1)
+    r, f, S, A, _ = parity(wl, 32749, 6)
+    g = lambda x: mp.mpf(1.7) ** (-1 - x) * mp.beta(-x, 1 - x)
+    rad, npts = 0.25, 64
+    vals = [g(rad * mp.e ** (2j * mp.pi * i / npts)) for i in range(npts)]
+    want = [float((sum(v * mp.e ** (-2j * mp.pi * i * k / npts) for i, v in enumerate(vals)) / npts / rad ** k).real) for k in (-1, 0, 1)]
+    assert np.all(np.abs(f.coeff.real - want) <= 4 * f.err.real + 1e-12), (f.coeff.real, f.err.real, want)
+    # complex path (physical region): the massive box of config 3 with squared and cubed propagators
+    parity(dataclasses.replace(qi.massive_box(), nu=(2, 1, 1, 1)), 32749, 3)
+    parity(dataclasses.replace(qi.massive_box(), nu=(1, 3, 1, 2)), 16381, 2)
+    # two loops, complex path with a pole: the non-planar vertex of config 5 with a squared propagator, a third of its sectors
+    parity(dataclasses.replace(qi.nonplanar_vertex(), nu=(1, 2, 1, 1, 1, 1)), 16381, 2, sectors=(0, 12))
+    # alpha <= -2 stays QMC_EUNSUPPORTED
+    with pytest.raises(q.QmcError) as e:
+        q.qmc_prepare(dataclasses.replace(qi.bubble(-1.0, 0.0, 0.0), nu=(3, 1)))
+    assert e.value.status == -3

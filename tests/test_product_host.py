@@ -194,3 +194,42 @@ def test_every_workload_gets_table_driven_tables():
     # a budget that is too small on purpose still falls back (and says so: no chunks)
     t = q.qmc_prepare(qi.double_box(), slot_budget=15, chunk_bytes=1000)
     assert len(t.describe().splitlines()) == 1
+
+
+def test_propagator_powers_give_the_oracles_sectors_and_run_on_the_generic_kernel():
+    """qmc_graph.edge_nu (Eq. 1): exponents of Eq. 6 with N_nu = sum nu_j, x_j^(nu_j - 1) in the integrand.  The
+    product's sectors must be the ones of the oracle's own decomposition; the table-driven kernels are compiled for
+    nu_j = 1 (exponents functions of n and L), so such tables carry no table images and run on the generic kernel."""
+    import dataclasses
+    from oracle import Oracle
+    for wl in (dataclasses.replace(qi.bubble(-1.0, 1.0, 2.0), nu=(2, 1)),
+               dataclasses.replace(qi.massive_box(), nu=(2, 1, 1, 1)),
+               dataclasses.replace(qi.massive_box(), nu=(1, 3, 1, 2)),
+               dataclasses.replace(qi.bubble(-1.0, 0.0, 0.0), nu=(2, 1)),
+               dataclasses.replace(qi.nonplanar_vertex(), nu=(1, 2, 1, 1, 1, 1))):
+        t = q.qmc_prepare(wl, eps_order=wl.eps_order, lam=wl.lam)
+        a, b = Oracle.from_tables(t.export()), Oracle.from_workload(wl)
+        Nn, L = sum(wl.nu), b.L                      # (the exported tables do not carry the loop number)
+        assert (a.aU0, a.aU1, a.aF0, a.aF1) == (Nn - 2 * (L + 1), L + 1, -(Nn - 2 * L), -L) == (b.aU0, b.aU1, b.aF0, b.aF1)
+        assert (a.n_sectors, a.k_min, a.k_max) == (b.n_sectors, b.k_min, b.k_max)
+        for s in range(a.n_sectors):
+            x, y = a.sector(s), b.sector(s)
+            assert np.array_equal(x["alpha"], y["alpha"]) and np.array_equal(x["beta"], y["beta"])
+            for w in "UF":
+                assert np.array_equal(x[w][1], y[w][1]) and np.allclose(x[w][0], y[w][0], rtol=1e-15, atol=0.0)
+        d = t.describe()
+        assert "real-path tables 0 B" in d and "chunks 0" in d, d
+    # the same call with the powers as an argument instead of a workload field
+    t = q.qmc_prepare(qi.bubble(-1.0, 1.0, 2.0), eps_order=1, nu=(2, 1))
+    assert Oracle.from_tables(t.export()).aF0 == -1
+    # a sector that ends with alpha <= -2 is still refused (the p >= 1 Taylor terms of Eq. 11 exist in the oracle only)
+    for wl in (dataclasses.replace(qi.bubble(-1.0, 0.0, 0.0), nu=(3, 1)), dataclasses.replace(qi.triangle(), nu=(1, 1, 2))):
+        with pytest.raises(q.QmcError) as e:
+            q.qmc_prepare(wl)
+        assert e.value.status == -3
+    for bad in ((0, 1), (9, 1), (-1, 1)):
+        with pytest.raises(q.QmcError) as e:
+            q.qmc_prepare(qi.bubble(), nu=bad)
+        assert e.value.status == -1
+    with pytest.raises(ValueError):
+        q.qmc_prepare(qi.bubble(), nu=(1, 1, 1))
