@@ -45,8 +45,9 @@ typedef enum {
   QMC_OK = 0,
   QMC_EINVAL = -1,       /* bad graph (disconnected, leg on a missing vertex, L < 1, P > 9), bad N/z/m */
   QMC_EDEPTH = -2,       /* iterated decomposition did not terminate within max_depth (R:C7) */
-  QMC_EUNSUPPORTED = -3, /* alpha_j <= -2 (needs the p >= 1 Taylor terms of Eq. 11; R:C9), beta_j = 0 on a
-                            singular variable, more than 4 singular variables in one sector, nu_j != 1 */
+  QMC_EUNSUPPORTED = -3, /* alpha_j <= -4, or alpha_j <= -2 with lambda > 0 or on more than two variables of a sector (the p >= 1
+                            Taylor terms of Eq. 11, exist on the real path for alpha_j = -2, -3 only; R:C9, R:C28),
+                            beta_j = 0 on a variable with alpha_j <= -1, more than 4 such variables in one sector */
   QMC_ECUDA = -4,        /* CUDA runtime error or no device */
   QMC_ENOMEM = -5,       /* workspace / export buffer too small */
   QMC_ECONTOUR = -6      /* reserved: contour problems are REPORTED through counters, never fatal */
@@ -60,7 +61,9 @@ typedef struct {
   const int32_t *edge_nu;         /* [n_edges] propagator powers nu_j in 1..8 (Eq. 1); NULL = all 1.  Powers other than 1
                                      change the exponents of U and F (Eq. 6 with N_nu = sum nu_j) and put x_j^(nu_j-1) into the
                                      integrand; such tables run on the generic kernel.  A sector that ends with an exponent
-                                     alpha_j <= -2 (it needs the p >= 1 Taylor terms of Eq. 11) is QMC_EUNSUPPORTED as before */
+                                     alpha_j = -2 or -3 needs the p >= 1 Taylor terms of Eq. 11: served by the
+                                     generic kernel on the real path (lambda = 0), at most two such variables per sector;
+                                     alpha_j <= -4, a third such variable, or any of them with lambda > 0: QMC_EUNSUPPORTED */
   const int32_t *leg_vertex;      /* [n_legs] vertex each external leg (all incoming) attaches to */
 } qmc_graph;
 

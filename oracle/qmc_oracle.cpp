@@ -869,8 +869,13 @@ orc_problem* orc_from_tables(const int64_t* w, size_t nwords) {
     for (int j = 0; j < pb.n; ++j) {
       if (sc.alpha[j] == -1)
         sc.sing.push_back(j);
-      else
+      else if (sc.alpha[j] >= 0)
         sc.reg.push_back(j);
+      else if (pb.lambda == 0.0 && sc.beta[j] != 0) {
+        sc.deep.push_back(j);  // tables with alpha_j <= -2: the Taylor terms of Eq. 11 (f3), real path only
+        pb.taylor = true;
+      } else
+        pb.status = -3;
     }
     pb.sectors.push_back(sc);
     if (p > nwords) {

@@ -1261,7 +1261,7 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
   nchunks = (se - sb + spc - 1) / spc;
   const size_t smem = tab_bytes + (((size_t)(spc + 1) * 4 + 15) & ~(size_t)15) + fixed_smem + per_sector_acc * spc;
   int bps = 0;
-  const int flavor = !cplx ? 0 : (-t->kmin <= 1 ? 2 : 1);  // kmin = -(largest number of singular variables)
+  const int flavor = !cplx ? (t->has_taylor ? 3 : 0) : (-t->kmin <= 1 ? 2 : 1);  // kmin = -(largest number of singular variables)
   CUDA_OK(qmc_kernel_prepare(n, t->kmax, flavor, smem, &bps));
   if (bps < 1) return QMC_ECUDA;
   gx = std::min<long long>({(long long)sms * bps, (long long)QMC_MAX_BLOCKS, (long long)((icount + QMC_THREADS - 1) / QMC_THREADS)});

@@ -50,7 +50,7 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
     double f = 0.0;
     // per-sector set-up: series (beta_j ln t_j)^p / p! of the singular variables, regular-variable factor and log
     for (int j = 0; j < n; ++j) {
-      if (s.alpha[j] == -1) {
+      if (s.alpha[j] <= -1) {
         f += 1.0 + 2.0 * (K - 1);
       } else {
         if (s.alpha[j]) f += s.alpha[j];
@@ -77,7 +77,7 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
       if (ns > 0) f += (ns - 1) + F_RCP2 + 1.0;  // 1 / prod t_k of the singular variables, times G0
       {
         int pos[QMC_MAXDIM], k = 0;
-        for (int j = 0; j < n; ++j) pos[j] = s.alpha[j] == -1 ? k++ : -1;
+        for (int j = 0; j < n; ++j) pos[j] = s.alpha[j] <= -1 ? k++ : -1;
         for (int which = 0; which < 2; ++which) {
           unsigned seen = 0;
           for (const QmcMono &m : (which ? s.F : s.U)) {
@@ -91,7 +91,7 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
       }
       f += (double)ns * nc;                            // subset sums: ns * 2^(ns-1) additions per polynomial
       for (int j = 0; j < n; ++j)
-        if (s.alpha[j] == -1) f += 2.0 + 2.0 * std::max(0, K - 3);   // t_j / beta_j, beta_j ln t_j, then (.)^p / p! for p = 2 .. K-2
+        if (s.alpha[j] <= -1) f += 2.0 + 2.0 * std::max(0, K - 3);   // t_j / beta_j, beta_j ln t_j, then (.)^p / p! for p = 2 .. K-2
       // W = U^aU0 F^aF0 and the argument U^aU1 F^aF1 of the logarithm from U, 1/F (1/U), a = U/F (corner_powers)
       const int P = std::min(t->aU1, -t->aF1), Q = (t->aU0 > 0 && t->aF0 < 0) ? std::min(t->aU0, -t->aF0) : 0;
       auto factors_w = [&]() {
@@ -134,7 +134,7 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
       };
       const double F_LOG2 = 18.0, F_CLOG3 = 3.0 + F_LOG2 + 1.0 + F_ATAN2;  // 64-entry table logarithm of |a|^2, atan2
       int pos_of[QMC_MAXDIM], kk = 0;
-      for (int j = 0; j < n; ++j) pos_of[j] = (s.alpha[j] == -1) ? kk++ : -1;
+      for (int j = 0; j < n; ++j) pos_of[j] = (s.alpha[j] <= -1) ? kk++ : -1;
       int nprod_c = 0;  // complex product slots of the sector's chunk
       for (size_t ci = 0; ci < t->chunks3.size(); ++ci)
         if (si >= t->chunks3[ci].sec_begin && si < t->chunks3[ci].sec_end) nprod_c = t->chunk3_nslots_c[ci] - (n + 1);
@@ -145,7 +145,7 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
       f = 3.0 * (1 + nL0);
       if (ns > 0) f += (ns - 1) + 6.0 + 1.0;   // 1 / prod t_k of the singular variables, onto G0
       for (int j = 0; j < n; ++j)
-        if (s.alpha[j] == -1) f += 2.0 + 2.0 * std::max(0, K - 3);   // t_k / beta_k, beta_k ln t_k, (.)^p / p!
+        if (s.alpha[j] <= -1) f += 2.0 + 2.0 * std::max(0, K - 3);   // t_k / beta_k, beta_k ln t_k, (.)^p / p!
       // record streams of all corners (derivative polynomials, U^(z), F^(z)): constants 0, real one-factor record 2 (an FMA),
       // real two-factor 3, complex one-factor 4, complex two-factor 10 -- counted by the table builder (qmc_image3.cpp)
       if ((size_t)si < t->rec_flops5.size()) f += t->rec_flops5[si];

@@ -2,9 +2,9 @@
 #pragma once
 #include "qmc_kernels.cuh"
 
-template <int NDIM, int KMAX, bool CPLX, int NSCAP>
+template <int NDIM, int KMAX, bool CPLX, int NSCAP, bool TAYLOR = false>
 static cudaError_t qmc_op(int op, dim3 grid, size_t smem, cudaStream_t st, const QmcLaunch *p, int *bps) {
-  auto kern = qmc_eval_kernel<NDIM, KMAX, CPLX, NSCAP>;
+  auto kern = qmc_eval_kernel<NDIM, KMAX, CPLX, NSCAP, TAYLOR>;
   if (op == 0) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -15,7 +15,13 @@ static cudaError_t qmc_op(int op, dim3 grid, size_t smem, cudaStream_t st, const
 }
 
 template <int NDIM>
-static cudaError_t qmc_dim_ops(int kmax, int flavor /* 0 real, 1 complex, 2 complex with <= 1 singular variable */, int op, dim3 grid, size_t smem, cudaStream_t st, const QmcLaunch *p, int *bps) {
+static cudaError_t qmc_dim_ops(int kmax, int flavor /* 0 real, 1 complex, 2 complex with <= 1 singular variable, 3 real with Taylor sectors */, int op, dim3 grid, size_t smem, cudaStream_t st, const QmcLaunch *p, int *bps) {
+  if (flavor == 3) switch (kmax) {
+    case 0: return qmc_op<NDIM, 0, false, 4, true>(op, grid, smem, st, p, bps);
+    case 1: return qmc_op<NDIM, 1, false, 4, true>(op, grid, smem, st, p, bps);
+    case 2: return qmc_op<NDIM, 2, false, 4, true>(op, grid, smem, st, p, bps);
+    default: return cudaErrorInvalidValue;
+  }
   switch (kmax * 3 + flavor) {
     case 0: return qmc_op<NDIM, 0, false, 4>(op, grid, smem, st, p, bps);
     case 1: return qmc_op<NDIM, 0, true, 4>(op, grid, smem, st, p, bps);

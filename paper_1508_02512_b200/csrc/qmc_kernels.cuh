@@ -368,6 +368,207 @@ __device__ __forceinline__ void sector_eval(const QmcLaunch &p, const QmcSectorH
   cntReU += c.cntReU;
 }
 
+// ---- sectors with a variable of exponent alpha <= -2: the p >= 1 Taylor terms of Eq. 11, real path ----
+// Product form over the variables V with alpha_b = -a_b <= -1 (the oracle evaluates the expanded double sum instead):
+//   sum_k c_k eps^k = sum_{Z subset V}  sum_{p_b < a_b, b in Z}   [prod_{b in Z} t_b^{p_b}] g(t; eps)|_{t_Z = 0}
+//                        prod_{b notin Z} t_b^{-a_b} e^{eps beta_b ln t_b}    prod_{b in Z} C_{b,p_b}(eps),
+//   C_{b,p}(eps) = 1/(p + 1 - a_b + beta_b eps)  -  t_b^{p - a_b} e^{eps beta_b ln t_b}
+// ([.] = Taylor coefficient; for a_b = 1 the factor C_{b,0} is B_b - A_b of the fold above).  g = G e^{eps Lambda} with
+// G = G0 U^aU0 F^aF0, Lambda = aU1 ln U + aF1 ln F + L0.  Its Taylor coefficients in the variables of Z that have a_b > 1
+// (at most two per sector, a_b <= QMC_MAXTAYLOR) come from truncated power-series arithmetic: U^ and F^ are polynomials, a
+// power, reciprocal or logarithm of a series a0 + x is the series of the function in the nilpotent part x.
+// A slow path by design (run-time loops, local arrays): such sectors come with propagator powers, not with the configs.
+struct JetDims {
+  int d0, d1;  // 1 + highest power kept of the first / second series variable (1 = no such variable)
+};
+struct Jet {
+  double c[QMC_MAXTAYLOR * QMC_MAXTAYLOR];  // coefficient of x0^p0 x1^p1 at p0 + d0 * p1
+};
+__device__ __forceinline__ Jet jet_const(double v) {
+  Jet r;
+#pragma unroll
+  for (int i = 0; i < QMC_MAXTAYLOR * QMC_MAXTAYLOR; ++i) r.c[i] = 0.0;
+  r.c[0] = v;
+  return r;
+}
+static __device__ __noinline__ Jet jet_mul(const JetDims d, const Jet &a, const Jet &b) {  // truncated product
+  Jet r = jet_const(0.0);
+  for (int p1 = 0; p1 < d.d1; ++p1)
+    for (int p0 = 0; p0 < d.d0; ++p0) {
+      const double av = a.c[p0 + d.d0 * p1];
+      for (int q1 = 0; p1 + q1 < d.d1; ++q1)
+        for (int q0 = 0; p0 + q0 < d.d0; ++q0) r.c[(p0 + q0) + d.d0 * (p1 + q1)] += av * b.c[q0 + d.d0 * q1];
+    }
+  return r;
+}
+// f(a0 + x) = sum_m co[m] x^m, co[m] = f^(m)(a0) / m!; x^m = 0 beyond m = (d0 - 1) + (d1 - 1)
+static __device__ __noinline__ Jet jet_fn(const JetDims d, const Jet &a, const double (&co)[2 * QMC_MAXTAYLOR - 1]) {
+  Jet x = a, xm = jet_const(1.0), r = jet_const(0.0);
+  x.c[0] = 0.0;
+  const int M = d.d0 + d.d1 - 2, n = d.d0 * d.d1;
+  for (int m = 0; m <= M; ++m) {
+    for (int i = 0; i < n; ++i) r.c[i] += co[m] * xm.c[i];
+    if (m < M) xm = jet_mul(d, xm, x);
+  }
+  return r;
+}
+__device__ __forceinline__ Jet jet_recip(const JetDims d, const Jet &a) {  // sum_m (-1)^m x^m / a0^(m+1)
+  double co[2 * QMC_MAXTAYLOR - 1];
+  const double r0 = 1.0 / a.c[0];
+  double v = r0;
+#pragma unroll
+  for (int m = 0; m < 2 * QMC_MAXTAYLOR - 1; ++m) {
+    co[m] = v;
+    v *= -r0;
+  }
+  return jet_fn(d, a, co);
+}
+__device__ __forceinline__ Jet jet_log(const JetDims d, const Jet &a) {  // ln a0 + sum_{m>=1} (-1)^(m+1) x^m / (m a0^m)
+  double co[2 * QMC_MAXTAYLOR - 1];
+  const double r0 = 1.0 / a.c[0];
+  double v = r0;
+  co[0] = log(a.c[0]);
+#pragma unroll
+  for (int m = 1; m < 2 * QMC_MAXTAYLOR - 1; ++m) {
+    co[m] = v / (double)m;
+    v *= -r0;
+  }
+  return jet_fn(d, a, co);
+}
+__device__ __forceinline__ Jet jet_ipow(const JetDims d, const Jet &a, int e) {  // integer power of either sign
+  const Jet base = e >= 0 ? a : jet_recip(d, a);
+  Jet r = jet_const(1.0);
+  for (int q = 0; q < (e < 0 ? -e : e); ++q) r = jet_mul(d, r, base);
+  return r;
+}
+
+// out[a], a = k + QMC_MAXSING: the coefficient of eps^k of the sector at this point (zero where the sector has none)
+template <int NDIM, int KMAX>
+__device__ __noinline__ void sector_eval_taylor(const QmcLaunch &p, const QmcSectorHdr *h, const double *pt,
+                                                double (&out)[QMC_MAXSING + KMAX + 1]) {
+  constexpr int KS = QMC_MAXSING + KMAX + 1;
+  const double *coef = reinterpret_cast<const double *>(h + 1);
+  const uint32_t *exps = reinterpret_cast<const uint32_t *>(coef + (h->nU + h->nF));
+  const int nv = h->nsing, nU = h->nU, nT = h->nU + h->nF;
+  double t[NDIM], lt[NDIM];
+#pragma unroll
+  for (int k = 0; k < NDIM; ++k) {
+    const int j = h->perm[k];
+    t[k] = pt[(0 * NDIM + j) * QMC_THREADS];
+    lt[k] = pt[(1 * NDIM + j) * QMC_THREADS];
+  }
+  double G0 = 1.0, L0 = 0.0;  // regular variables
+  for (int k = nv; k < NDIM; ++k) {
+    G0 *= ipow_pos(t[k], h->alpha[k]);
+    L0 += (double)h->beta[k] * lt[k];
+  }
+#pragma unroll
+  for (int i = 0; i < KS; ++i) out[i] = 0.0;
+  for (int Z = 0; Z < (1 << nv); ++Z) {
+    int j0 = -1, j1 = -1, nz = 0;  // series variables: the members of Z with a_b > 1
+    JetDims d{1, 1};
+    double pref = 1.0, Lfree = L0;
+    for (int b = 0; b < nv; ++b) {
+      const int a = -h->alpha[b];
+      if (Z >> b & 1) {
+        ++nz;
+        if (a > 1) {
+          if (j0 < 0) {
+            j0 = b;
+            d.d0 = a;
+          } else {
+            j1 = b;
+            d.d1 = a;
+          }
+        }
+      } else {
+        pref *= 1.0 / ipow_pos(t[b], a);  // untouched variable: t^-a e^{eps beta ln t}
+        Lfree += (double)h->beta[b] * lt[b];
+      }
+    }
+    // U^, F^ as series: a monomial puts  c prod_{k notin Z} t_k^{e_k}  on the coefficient of  prod_{b in Z} t_b^{e_b}
+    Jet U = jet_const(0.0), F = jet_const(0.0);
+    for (int mi = 0; mi < nT; ++mi) {
+      const uint32_t w = exps[mi];
+      double c = coef[mi];
+      int idx = 0;
+      bool keep = true;
+#pragma unroll
+      for (int k = 0; k < NDIM; ++k) {
+        const int e = (w >> (4 * k)) & 15;
+        if (k < nv && (Z >> k & 1)) {
+          if (k == j0) {
+            if (e >= d.d0) keep = false;
+            idx += e;
+          } else if (k == j1) {
+            if (e >= d.d1) keep = false;
+            idx += d.d0 * e;
+          } else if (e) {
+            keep = false;
+          }
+        } else {
+          c *= ipow_pos(t[k], e);
+        }
+      }
+      if (keep) (mi < nU ? U : F).c[idx] += c;
+    }
+    Jet W = jet_mul(d, jet_ipow(d, U, p.aU0), jet_ipow(d, F, p.aF0));
+    const Jet lU = jet_log(d, U), lF = jet_log(d, F);
+    Jet Lam;
+    const int nj = d.d0 * d.d1;
+    for (int i = 0; i < QMC_MAXTAYLOR * QMC_MAXTAYLOR; ++i) {
+      W.c[i] *= G0;
+      Lam.c[i] = i < nj ? (double)p.aU1 * lU.c[i] + (double)p.aF1 * lF.c[i] : 0.0;
+    }
+    Lam.c[0] += Lfree;
+    // E[k] = W Lam^k / k!: the coefficient of eps^k of g times the regulators of the untouched variables
+    Jet E[KS];
+    E[0] = W;
+    for (int k = 1; k < KS; ++k) {
+      E[k] = jet_mul(d, E[k - 1], Lam);
+      const double rk = 1.0 / (double)k;
+      for (int i = 0; i < nj; ++i) E[k].c[i] *= rk;
+    }
+    for (int p1 = 0; p1 < d.d1; ++p1)
+      for (int p0 = 0; p0 < d.d0; ++p0) {
+        double ser[KS];  // eps^nz times the term: coefficients of eps^0 .. eps^(KS-1)
+        for (int k = 0; k < KS; ++k) ser[k] = E[k].c[p0 + d.d0 * p1];
+        for (int b = 0; b < nv; ++b) {
+          if (!(Z >> b & 1)) continue;
+          const int a = -h->alpha[b], pb = b == j0 ? p0 : (b == j1 ? p1 : 0), q = a - 1 - pb;
+          const double beta = (double)h->beta[b];
+          double cc[KS];  // eps C_{b,p}(eps)
+          if (q == 0) {  // the pole 1/(beta eps)
+            cc[0] = 1.0 / beta;
+            for (int m = 1; m < KS; ++m) cc[m] = 0.0;
+          } else {  // 1/(-q + beta eps) = -(1/q) sum_m (beta eps / q)^m
+            cc[0] = 0.0;
+            double gq = -1.0 / (double)q;
+            for (int m = 1; m < KS; ++m) {
+              cc[m] = gq;
+              gq *= beta / (double)q;
+            }
+          }
+          double term = 1.0 / ipow_pos(t[b], a - pb);  // - t^(p-a) e^{eps beta ln t}
+          const double Lb = beta * lt[b];
+          for (int m = 0; m + 1 < KS; ++m) {
+            cc[m + 1] -= term;
+            term *= Lb / (double)(m + 1);
+          }
+          double r[KS];
+          for (int i = 0; i < KS; ++i) r[i] = 0.0;
+          for (int i = 0; i < KS; ++i)
+            for (int jx = 0; i + jx < KS; ++jx) r[i + jx] += ser[i] * cc[jx];
+          for (int i = 0; i < KS; ++i) ser[i] = r[i];
+        }
+        for (int i = 0; i < KS; ++i) {
+          const int k = i - nz;  // order of eps
+          if (k <= KMAX) out[k + QMC_MAXSING] += pref * ser[i];
+        }
+      }
+  }
+}
+
 __device__ __forceinline__ bool finite_all(double v) { return fabs(v) <= 1.79769313486231570e308; }
 __device__ __forceinline__ bool finite_all(cd v) { return finite_all(v.re) && finite_all(v.im); }
 
@@ -426,7 +627,8 @@ __device__ __forceinline__ double block_sum(double v, double *scratch /*[QMC_THR
 #endif
 // NSCAP: largest number of singular variables of any sector of the tables this instantiation serves (the code of the
 // larger cases is not generated: the complex instantiation with NSCAP = 1 is a fraction of the size of NSCAP = 4)
-template <int NDIM, int KMAX, bool CPLX, int NSCAP>
+// TAYLOR: the instantiation that also serves sectors with alpha_j <= -2 (header flag 2; real path only)
+template <int NDIM, int KMAX, bool CPLX, int NSCAP, bool TAYLOR = false>
 __global__ void __launch_bounds__(QMC_THREADS, QMC_V1_MIN_BLOCKS) qmc_eval_kernel(const QmcLaunch p) {
   using namespace qmcdev;
   typedef typename std::conditional<CPLX, cd, double>::type T;
@@ -542,6 +744,17 @@ __global__ void __launch_bounds__(QMC_THREADS, QMC_V1_MIN_BLOCKS) qmc_eval_kerne
       }                                                                                 \
     }                                                                                   \
   } break;
+        if (TAYLOR && !CPLX && (h->flags & 2)) {
+          if constexpr (TAYLOR && !CPLX) {
+            double res[NACC];
+            sector_eval_taylor<NDIM, KMAX>(p, h, pt, res);
+#pragma unroll
+            for (int i = 0; i < NACC; ++i) {
+              fin = fin && finite_all(res[i]);
+              contrib[i] = res[i];
+            }
+          }
+        } else
         switch (ns) {
           QMC_CASE(0)
           QMC_CASE(1)

@@ -190,10 +190,7 @@ static int qmc_build_sectors(const qmc_graph *g, const qmc_kinematics *kin, int 
   //      are compiled for (their exponents are functions of n and L); any other powers run on the generic kernel --------------
   int Nnu = 0;
   for (int e = 0; e < P; ++e) Nnu += g->edge_nu ? g->edge_nu[e] : 1;
-  if (T->sectors.empty())
-    T->generic_only = (Nnu != P);
-  else if (T->generic_only != (Nnu != P))
-    return QMC_EINVAL;
+  if (Nnu != P) T->generic_only = true;  // (the points of a batch share the graph and its powers)
   T->n = P - 1;
   T->P = P;
   T->L = L;
@@ -243,12 +240,16 @@ static int qmc_build_sectors(const qmc_graph *g, const qmc_kinematics *kin, int 
       QmcSector s;
       s.primary = nd.primary;
       s.nsing = 0;
+      s.ndeep = 0;
       std::memset(s.alpha, 0, sizeof s.alpha);
       std::memset(s.beta, 0, sizeof s.beta);
       for (int j = 0; j < n; ++j) {
         s.alpha[j] = nd.alpha[j];
         s.beta[j] = nd.beta[j];
-        if (nd.alpha[j] <= -2) return QMC_EUNSUPPORTED;  // R:C9
+        if (nd.alpha[j] <= -2) {  // needs the p >= 1 Taylor terms of Eq. 11 (R:C9, R:C28): real path, alpha >= -3, two per sector
+          if (T->lambda > 0.0 || nd.alpha[j] < -QMC_MAXTAYLOR || nd.beta[j] == 0 || ++s.ndeep > 2) return QMC_EUNSUPPORTED;
+          ++s.nsing;  // (a variable that can give a pole: counted with the singular ones)
+        }
         if (nd.alpha[j] == -1) {
           if (nd.beta[j] == 0) return QMC_EUNSUPPORTED;
           ++s.nsing;
@@ -256,6 +257,7 @@ static int qmc_build_sectors(const qmc_graph *g, const qmc_kinematics *kin, int 
         if (nd.alpha[j] > 127 || nd.beta[j] > 127 || nd.beta[j] < -127) return QMC_EUNSUPPORTED;
       }
       if (s.nsing > QMC_MAXSING) return QMC_EUNSUPPORTED;
+      if (s.ndeep) T->has_taylor = T->generic_only = true;  // only the generic kernel has Taylor-coefficient corners
       smax = std::max(smax, s.nsing);
       for (int which = 0; which < 2; ++which)
         for (const Term &t : (which ? nd.F : nd.U)) {
@@ -318,7 +320,7 @@ static int qmc_finish_tables(qmc_tables *T, const qmc_options *opt) {
     int pos = 0, inv[QMC_MAXDIM];
     for (int pass = 0; pass < 2; ++pass)
       for (int j = 0; j < n; ++j)
-        if ((s.alpha[j] == -1) == (pass == 0)) {
+        if ((s.alpha[j] <= -1) == (pass == 0)) {  // the variables that can give a pole first
           h.perm[pos] = (uint8_t)j;
           inv[j] = pos;
           h.alpha[pos] = (int8_t)s.alpha[j];
@@ -326,6 +328,7 @@ static int qmc_finish_tables(qmc_tables *T, const qmc_options *opt) {
           ++pos;
         }
     h.nsing = (uint8_t)s.nsing;
+    if (s.ndeep) h.flags |= 2;  // a Taylor sector (sector_eval_taylor)
     auto group_of = [&](const QmcMono &m) {
       int gmask = 0;
       for (int b = 0; b < s.nsing; ++b)

@@ -8,6 +8,7 @@
 #include "../../include/qmc_feynman.h"
 
 #define QMC_MAXDIM 8    // integration variables per sector (P - 1)
+#define QMC_MAXTAYLOR 3   // most negative exponent -alpha of a variable the generic kernel's Taylor corners handle
 #define QMC_MAXSING 4   // singular variables (alpha = -1) per sector handled by the kernels
 #define QMC_MAXK 8      // eps orders kept: k_max - k_min + 1
 #define QMC_KMAX_MAX 2  // highest eps_order the kernels are instantiated for
@@ -143,7 +144,8 @@ struct QmcMono {
 struct QmcSector {
   int primary;
   int alpha[QMC_MAXDIM], beta[QMC_MAXDIM];  // original variable order
-  int nsing;
+  int nsing;  // variables with alpha <= -1 (each can give a pole)
+  int ndeep = 0;  // ... of which alpha <= -2 (Taylor terms p >= 1 of Eq. 11; generic kernel, real path only)
   std::vector<QmcMono> U, F;  // evaluation order (group-sorted)
 };
 
@@ -187,6 +189,7 @@ struct qmc_tables {
   int resident_kind = 0;              // 4: logarithm table (versions 4, 5), 1: version-1 image
   int resident_m = 0;                 // number of shift vectors resident in that workspace (0 = none)
   uint64_t resident_seed = 0;         // seed that produced them ...
+  bool has_taylor = false;            // some sector has a variable with alpha <= -2
   bool generic_only = false;          // propagator powers other than 1: only the generic kernel has run-time exponents
   bool resident_explicit = false;     // ... or: they were passed explicitly (qmc_run.shifts)
   uint64_t cached_N = 0;              // generating vector cache

@@ -45,7 +45,8 @@ def parity(wl, N, m, z=None, index_range=None, sectors=None, transform=0, shifts
     assert r.mode_used == 2 and r.shift_sums.shape == S.shape
     nfloor = check(r.shift_sums, S, A, wl.name + " per-sector")
     nz = np.abs(S) > 0
-    report_floor(f"{wl.name} N={N} m={m} sectors={sectors} idx={index_range} tr={transform} eps={eo} kernel={kernel} {sorted(layout.items())}",
+    nu = getattr(wl, "nu", None)
+    report_floor(f"{wl.name}{'' if nu is None else ' nu=' + str(tuple(nu))} N={N} m={m} sectors={sectors} idx={index_range} tr={transform} eps={eo} kernel={kernel} {sorted(layout.items())}",
                  nfloor, S.size, float((A[nz] / np.abs(S[nz])).max()) if nz.any() else 0.0)
     assert np.array_equal(r.counters, cnt), (r.counters, cnt)
     # fused mode (the throughput mode): per-shift totals over sectors
@@ -540,7 +541,50 @@ def test_propagator_powers_run_on_the_generic_kernel():
     parity(dataclasses.replace(qi.massive_box(), nu=(1, 3, 1, 2)), 16381, 2)
     # two loops, complex path with a pole: the non-planar vertex of config 5 with a squared propagator, a third of its sectors
     parity(dataclasses.replace(qi.nonplanar_vertex(), nu=(1, 2, 1, 1, 1, 1)), 16381, 2, sectors=(0, 12))
-    # alpha <= -2 stays QMC_EUNSUPPORTED
-    with pytest.raises(q.QmcError) as e:
-        q.qmc_prepare(dataclasses.replace(qi.bubble(-1.0, 0.0, 0.0), nu=(3, 1)))
-    assert e.value.status == -3
+
+
+def _laurent(f, kmin, kmax, radius=0.25, npts=64):
+    """Laurent coefficients of f around eps = 0 by the trapezoidal rule on a circle (mpmath)."""
+    import mpmath as mp
+    vals = [f(radius * mp.e ** (2j * mp.pi * i / npts)) for i in range(npts)]
+    return np.array([float((sum(v * mp.e ** (-2j * mp.pi * i * k / npts) for i, v in enumerate(vals)) / npts / radius ** k).real)
+                     for k in range(kmin, kmax + 1)])
+
+
+def test_taylor_terms_for_alpha_below_minus_one_on_the_generic_kernel():
+    """SURVEY 8(f) f3, reading C28: sectors with a variable of exponent alpha_j = -2 or -3 (they come with propagator powers)
+    need the p >= 1 Taylor terms of Eq. 11.  The generic kernel evaluates them in product form with
+    truncated power series in the variables set to zero (sector_eval_taylor); the oracle evaluates the expanded double sum.
+    Parity per sector, order and shift at the C19 tolerance; closed forms on the GPU numbers with the tent transform (under
+    Eq. 21's transform the subtraction at alpha = -2 is numerically unstable on BOTH sides, DESIGN.md section 10 f3)."""
+    import dataclasses
+    import mpmath as mp
+    # massless propagator with powers (3, 1): J = (-p^2)^(D/2-4) B(D/2-3, D/2-1)
+    wl = dataclasses.replace(qi.bubble(-1.7, 0.0, 0.0), nu=(3, 1), eps_order=1)
+    assert "real-path tables 0 B" in q.qmc_prepare(wl, eps_order=1).describe()
+    r, f, S, A, _ = parity(wl, 65521, 8, transform=1)
+    want = _laurent(lambda x: mp.mpf(1.7) ** (-2 - x) * mp.beta(-1 - x, 1 - x), -1, 1)
+    assert np.all(np.abs(f.coeff.real - want) <= 4 * f.err.real + 1e-11), (f.coeff.real, f.err.real, want)
+    parity(wl, 16381, 3)                                   # Eq. 21's transform: the two sides still agree
+    parity(wl, 16381, 3, transform=2)
+    # triangle with a squared propagator: sectors with exponents (-2, -2) and (-2, -1); Dirichlet's integral
+    s = -2.0
+    for nu in ((2, 1, 1), (1, 1, 2)):
+        wl = dataclasses.replace(qi.triangle(s), nu=nu, eps_order=0)
+        r, f, S, A, _ = parity(wl, 99991, 8, transform=1)
+        Nn = sum(nu)
+        want = _laurent(lambda x: (-s) ** (2 - x - Nn) * mp.gamma(nu[0]) * mp.gamma(nu[1] + 2 - x - Nn) * mp.gamma(nu[2] + 2 - x - Nn)
+                        / mp.gamma(4 - 2 * x - Nn), -2, 0)
+        assert np.all(np.abs(f.coeff.real - want) <= 4 * f.err.real + 1e-11), (nu, f.coeff.real, f.err.real, want)
+    parity(dataclasses.replace(qi.triangle(s), nu=(1, 1, 2), eps_order=1), 16381, 3)
+    # alpha = -3 (two regular Taylor terms and the pole)
+    parity(dataclasses.replace(qi.triangle(s), nu=(1, 1, 3)), 16381, 3, transform=1)
+    # three variables: the massless box of config 2 with squared propagators, sectors with two such variables
+    parity(dataclasses.replace(qi.massless_box(), nu=(2, 1, 1, 1)), 16381, 3, transform=1)
+    parity(dataclasses.replace(qi.massless_box(), nu=(1, 2, 1, 2), eps_order=1), 16381, 2, transform=1)
+    # refused: alpha = -4; the complex path
+    for wl in (dataclasses.replace(qi.bubble(-1.0, 0.0, 0.0), nu=(5, 1)),
+               dataclasses.replace(qi.bubble(-1.0, 0.0, 0.0), nu=(3, 1), lam=0.5)):
+        with pytest.raises(q.QmcError) as e:
+            q.qmc_prepare(wl, lam=wl.lam)
+        assert e.value.status == -3

@@ -222,10 +222,23 @@ def test_propagator_powers_give_the_oracles_sectors_and_run_on_the_generic_kerne
     # the same call with the powers as an argument instead of a workload field
     t = q.qmc_prepare(qi.bubble(-1.0, 1.0, 2.0), eps_order=1, nu=(2, 1))
     assert Oracle.from_tables(t.export()).aF0 == -1
-    # a sector that ends with alpha <= -2 is still refused (the p >= 1 Taylor terms of Eq. 11 exist in the oracle only)
-    for wl in (dataclasses.replace(qi.bubble(-1.0, 0.0, 0.0), nu=(3, 1)), dataclasses.replace(qi.triangle(), nu=(1, 1, 2))):
+    # sectors that end with alpha = -2, -3 (the p >= 1 Taylor terms of Eq. 11): accepted on the real path, same sectors as the oracle's
+    for wl in (dataclasses.replace(qi.bubble(-1.0, 0.0, 0.0), nu=(3, 1)), dataclasses.replace(qi.triangle(), nu=(1, 1, 2)),
+               dataclasses.replace(qi.triangle(), nu=(1, 1, 3)), dataclasses.replace(qi.massless_box(), nu=(2, 1, 1, 1))):
+        t = q.qmc_prepare(wl, eps_order=wl.eps_order)
+        a, b = Oracle.from_tables(t.export()), Oracle.from_workload(wl, taylor=True)
+        assert a.status == 0 and b.status == 0 and (a.n_sectors, a.k_min, a.k_max) == (b.n_sectors, b.k_min, b.k_max)
+        lowest = 0
+        for s in range(a.n_sectors):
+            x, y = a.sector(s), b.sector(s)
+            assert np.array_equal(x["alpha"], y["alpha"]) and np.array_equal(x["beta"], y["beta"]) and x["n_sing"] == y["n_sing"]
+            lowest = min(lowest, int(x["alpha"].min()))
+        assert lowest <= -2 and "real-path tables 0 B" in t.describe()
+    # refused: alpha = -4, and any alpha <= -2 on the complex path
+    for wl, lam in ((dataclasses.replace(qi.bubble(-1.0, 0.0, 0.0), nu=(5, 1)), 0.0),
+                    (dataclasses.replace(qi.bubble(-1.0, 0.0, 0.0), nu=(3, 1)), 0.5)):
         with pytest.raises(q.QmcError) as e:
-            q.qmc_prepare(wl)
+            q.qmc_prepare(wl, lam=lam)
         assert e.value.status == -3
     for bad in ((0, 1), (9, 1), (-1, 1)):
         with pytest.raises(q.QmcError) as e:
