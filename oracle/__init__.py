@@ -87,10 +87,11 @@ class Oracle:
 
     @classmethod
     def from_workload(cls, wl, lam: Optional[float] = None, eps_order: Optional[int] = None, max_depth: int = 64,
-                      order: int = 0, taylor: bool = False):
+                      order: int = 0, taylor: bool = False, ibp: bool = False):
         """order = 0: decomposition rule A.3 (U^ first); 1: F^ first (only to pin strategy independence of the totals).
         wl.nu: propagator powers (None = all 1).  taylor: accept alpha_j <= -2 on the real path (the p >= 1 Taylor terms of
-        Eq. 11) instead of status -3."""
+        Eq. 11) instead of status -3.  ibp: pole extraction by integration by parts
+        (Eq. 13) instead of the subtraction; real path only."""
         eu, ev, m2, lv, gram = wl.arrays()
         nu = getattr(wl, "nu", None)
         nu_arr = None if nu is None else np.ascontiguousarray(nu, dtype=np.int32)
@@ -102,13 +103,13 @@ class Oracle:
                            _p(ev, C.c_int), _p(m2, C.c_double), _p(lv, C.c_int), _p(gram, C.c_double),
                            C.c_double(wl.lam if lam is None else lam),
                            C.c_int(wl.eps_order if eps_order is None else eps_order), C.c_int(max_depth), C.c_int(order),
-                           None if nu_arr is None else _p(nu_arr, C.c_int), C.c_int(1 if taylor else 0))
+                           None if nu_arr is None else _p(nu_arr, C.c_int), C.c_int((1 if taylor else 0) | (2 if ibp else 0)))
         o = cls(h)
         o.n_edges = wl.n_edges
         return o
 
     @classmethod
-    def from_sector(cls, alpha, beta, U, F, aU, aF, eps_order: int = 0):
+    def from_sector(cls, alpha, beta, U, F, aU, aF, eps_order: int = 0, ibp: bool = False):
         """ONE explicit real sector prod_j t_j^(alpha_j + beta_j eps) U(t)^(aU[0] + aU[1] eps) F(t)^(aF[0] + aF[1] eps) on the
         unit cube (the form of Eq. 9), Taylor terms enabled.  U, F: lists of (coefficient, exponent tuple),
         each with a constant term."""
@@ -123,7 +124,7 @@ class Oracle:
         L.orc_from_sector.restype = C.c_void_p
         h = L.orc_from_sector(C.c_int(n), _p(alpha, C.c_int), _p(beta, C.c_int), C.c_int(len(U)), _p(cU, C.c_double),
                               _p(eU, C.c_int), C.c_int(len(F)), _p(cF, C.c_double), _p(eF, C.c_int), C.c_int(aU[0]),
-                              C.c_int(aU[1]), C.c_int(aF[0]), C.c_int(aF[1]), C.c_int(eps_order))
+                              C.c_int(aU[1]), C.c_int(aF[0]), C.c_int(aF[1]), C.c_int(eps_order), C.c_int(1 if ibp else 0))
         o = cls(h)
         o.n_edges = n + 1
         return o

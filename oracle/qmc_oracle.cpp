@@ -185,6 +185,7 @@ struct Problem {
   int kmax = 0, kmin = 0;
   int max_depth = 64;
   int order = 0;  // 0: rule A.3 (target U^ first); 1: F^ first (strategy-independence pin)
+  bool ibp = false;     // pole extraction by Eq. 13 (sector_point_ibp) instead of the subtraction; real path only
   bool taylor = false;  // accept alpha_j <= -2 on the real path (sector_point_taylor); off = R:C9 (unsupported)
   std::vector<Sector> sectors;
   int status = 0;  // 0 ok, -2 depth, -3 unsupported
@@ -777,6 +778,135 @@ void sector_point_taylor(const Problem& pb, const Sector& s, const double* t, co
   }
 }
 
+// ------------------------------------------------------------------------------------
+// f3: pole extraction by integration by parts, Eq. 13, instead of the subtraction.  REAL PATH ONLY.
+//
+// Eq. 13 repeated a = -alpha times on ONE variable with exponent -a + beta eps ("by repeating the above IBP formula enough
+// times, the power of t will not generate singularity"):
+//   int_0^1 dt t^{-a+beta eps} f(t) = sum_{r=0}^{a-1} (-1)^r f^(r)(1) / prod_{s=0}^{r} (s+1-a + beta eps)
+//                                    + (-1)^a / prod_{s=0}^{a-1} (s+1-a + beta eps)  int_0^1 dt t^{beta eps} f^(a)(t)
+// (the factor with s = a-1 is the pole 1/(beta eps); the others are regular: 1/(c + beta eps) = (1/c) sum_m (-beta eps/c)^m).
+// Over the variables V = {j : alpha_j <= -1} the operators multiply: every variable is either taken at the boundary
+// t_j = 1 with a derivative order r_j < a_j, or keeps its integral with the a_j-th derivative and the factor t_j^{beta_j eps}.
+// No subtraction and no 1/t_j: what is evaluated is a mixed partial derivative of g = G e^{eps Lambda} (Eq. 9 integrand) at a
+// point with some coordinates set to 1.  The derivatives are Taylor coefficients (times factorials) of g around that point,
+// from the same truncated power-series arithmetic as sector_point_taylor, centred at the point instead of at 0.  Every term
+// is summed on the full n-dimensional lattice (unused directions integrate to 1), as in O7.
+// ------------------------------------------------------------------------------------
+double binomial(int n, int k) {
+  double r = 1.0;
+  for (int i = 0; i < k; ++i) r = r * (n - i) / (i + 1);
+  return r;
+}
+
+void sector_point_ibp(const Problem& pb, const Sector& s, const double* t, const double* lnt, std::vector<double>& out,
+                      std::vector<double>& absout) {
+  std::vector<int> V, a;
+  for (int j = 0; j < pb.n; ++j)
+    if (s.alpha[j] <= -1) {
+      V.push_back(j);
+      a.push_back(-s.alpha[j]);
+    }
+  const int nv = (int)V.size(), M = pb.kmax + nv;
+  out.assign(M + 1, 0.0);
+  absout.assign(M + 1, 0.0);
+  double Greg = 1.0, Lreg = 0.0;
+  std::vector<int> pos_of(pb.n, -1);
+  for (int b = 0; b < nv; ++b) pos_of[V[b]] = b;
+  for (int j = 0; j < pb.n; ++j)
+    if (s.alpha[j] >= 0) {
+      Greg *= ipow(t[j], s.alpha[j]);
+      Lreg += s.beta[j] * lnt[j];
+    }
+  for (int B = 0; B < (1 << nv); ++B) {  // B: the variables taken at the boundary t_b = 1
+    std::vector<int> ord(nv);
+    std::vector<double> tau(nv);
+    double Lint = Lreg;  // + sum over the variables that keep their integral of beta_b ln t_b (the factor t_b^{beta_b eps})
+    for (int b = 0; b < nv; ++b) {
+      const bool atone = B >> b & 1;
+      ord[b] = atone ? a[b] - 1 : a[b];
+      tau[b] = atone ? 1.0 : t[V[b]];
+      if (!atone) Lint += s.beta[V[b]] * lnt[V[b]];
+    }
+    JetShape sh(ord);
+    // U^, F^ around the point: (tau + d)^e = sum_p C(e, p) tau^(e-p) d^p
+    auto poly_jet = [&](const Poly& Q) {
+      Jet r(sh.size, 0.0);
+      for (auto& term : Q) {
+        double c0 = term.second;
+        for (int j = 0; j < pb.n; ++j)
+          if (pos_of[j] < 0) c0 *= ipow(t[j], term.first[j]);
+        for (int idx = 0; idx < sh.size; ++idx) {
+          double c = c0;
+          bool keep = true;
+          for (int b = 0; b < nv; ++b) {
+            const int e = term.first[V[b]], p = sh.midx[idx][b];
+            if (p > e) {
+              keep = false;
+              break;
+            }
+            c *= binomial(e, p) * ipow(tau[b], e - p);
+          }
+          if (keep) r[idx] += c;
+        }
+      }
+      return r;
+    };
+    Jet Uj = poly_jet(s.U), Fj = poly_jet(s.F);
+    Jet G = jet_mul(sh, jet_ipow(sh, Uj, pb.aU0), jet_ipow(sh, Fj, pb.aF0));
+    for (double& v : G) v *= Greg;
+    Jet lU = jet_log(sh, Uj), lF = jet_log(sh, Fj), Lam(sh.size);
+    for (int i = 0; i < sh.size; ++i) Lam[i] = pb.aU1 * lU[i] + pb.aF1 * lF[i];
+    Lam[0] += Lint;
+    std::vector<Jet> T(M + 1);  // T[k] = G Lam^k / k!
+    T[0] = G;
+    for (int k = 1; k <= M; ++k) {
+      T[k] = jet_mul(sh, T[k - 1], Lam);
+      for (double& v : T[k]) v /= k;
+    }
+    for (int idx = 0; idx < sh.size; ++idx) {  // derivative orders: r_b < a_b at the boundary, exactly a_b under the integral
+      bool use = true;
+      for (int b = 0; b < nv; ++b)
+        if (!(B >> b & 1) && sh.midx[idx][b] != a[b]) use = false;
+      if (!use) continue;
+      double scalar = 1.0;
+      int npole = 0;
+      std::vector<double> ser(M + 1);
+      for (int k = 0; k <= M; ++k) ser[k] = T[k][idx];
+      for (int b = 0; b < nv; ++b) {
+        const int p = sh.midx[idx][b];
+        for (int q = 2; q <= p; ++q) scalar *= q;  // derivative = Taylor coefficient times p!
+        if (p & 1) scalar = -scalar;               // (-1)^r, (-1)^a
+        const int smax = std::min(p, a[b] - 1);
+        for (int sft = 0; sft <= smax; ++sft) {  // 1 / (s+1-a + beta eps)
+          const int c = sft + 1 - a[b];
+          const double beta = s.beta[V[b]];
+          if (c == 0) {
+            scalar *= 1.0 / beta;
+            ++npole;
+          } else {
+            std::vector<double> r(M + 1, 0.0);
+            for (int k = 0; k <= M; ++k) {
+              double gm = 1.0 / c;
+              for (int m = 0; k + m <= M; ++m) {
+                r[k + m] += ser[k] * gm;
+                gm *= -beta / c;
+              }
+            }
+            ser = r;
+          }
+        }
+      }
+      for (int k = -nv; k <= pb.kmax; ++k) {
+        if (k + npole < 0) continue;
+        double term = scalar * ser[k + npole];
+        out[k + nv] += term;
+        absout[k + nv] += std::fabs(term);
+      }
+    }
+  }
+}
+
 }  // namespace
 
 // =====================================================================================
@@ -807,7 +937,13 @@ orc_problem* orc_build_nu(int V, int P, int nlegs, const int* eu, const int* ev,
                           const double* gram, double lambda, int kmax, int max_depth, int order, const int* nu, int taylor) {
   orc_problem* h = new orc_problem;
   h->pb.order = order;
-  h->pb.taylor = taylor != 0;
+  h->pb.taylor = (taylor & 1) != 0;  // bit 0: Taylor terms / alpha <= -2 accepted; bit 1: IBP (Eq. 13) instead of the subtraction
+  h->pb.ibp = (taylor & 2) != 0 && lambda == 0.0;
+  if ((taylor & 2) && lambda > 0.0) {
+    delete h;
+    return nullptr;
+  }
+  if (h->pb.ibp) h->pb.taylor = true;
   if (nu) h->pb.g.nu.assign(nu, nu + P);
   for (int v : h->pb.g.nu)
     if (v < 1) {
@@ -979,7 +1115,9 @@ void orc_sector_integrand(const orc_problem* h, int s, const double* tpt, double
     }
   } else {
     std::vector<double> o;
-    if (!sc.deep.empty())
+    if (pb.ibp)
+      sector_point_ibp(pb, sc, tpt, lnt.data(), o, absout);
+    else if (!sc.deep.empty())
       sector_point_taylor(pb, sc, tpt, lnt.data(), o, absout);
     else
       sector_point<double>(pb, sc, tpt, lnt.data(), o, absout, cnt);
@@ -1009,11 +1147,12 @@ int orc_sector_integrand_taylor(const orc_problem* h, int s, const double* tpt, 
 // ONE explicit real sector  prod_j t_j^{alpha_j + beta_j eps} U(t)^{aU0 + aU1 eps} F(t)^{aF0 + aF1 eps}  on (0,1)^n (the form of
 // Eq. 9), Taylor terms enabled: for pins whose closed form is elementary.  Polynomials as coeff[nterms], expo[nterms*n].
 orc_problem* orc_from_sector(int n, const int* alpha, const int* beta, int nU, const double* cU, const int* eU, int nF,
-                             const double* cF, const int* eF, int aU0, int aU1, int aF0, int aF1, int kmax) {
+                             const double* cF, const int* eF, int aU0, int aU1, int aF0, int aF1, int kmax, int ibp) {
   orc_problem* h = new orc_problem;
   Problem& pb = h->pb;
   pb.n = n;
   pb.taylor = true;
+  pb.ibp = ibp != 0;  // pole extraction by Eq. 13 instead of the subtraction
   pb.kmax = kmax;
   pb.aU0 = aU0;
   pb.aU1 = aU1;
@@ -1095,7 +1234,9 @@ int orc_integrate(const orc_problem* h, uint64_t N, const uint64_t* z, int m, co
                 accA[off + k].add(w * absout[k]);
               }
           } else {
-            if (!sc.deep.empty())
+            if (pb.ibp)
+              sector_point_ibp(pb, sc, t.data(), lnt.data(), od, absout);     // f3: Eq. 13 instead of Eqs. 11-12
+            else if (!sc.deep.empty())
               sector_point_taylor(pb, sc, t.data(), lnt.data(), od, absout);  // f3: alpha_j <= -2 (Eq. 11 with p >= 1)
             else
               sector_point<double>(pb, sc, t.data(), lnt.data(), od, absout, cnt);
