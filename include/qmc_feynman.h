@@ -88,6 +88,10 @@ typedef struct {
   int32_t slot_budget_cplx_real, slot_budget_cplx; /* complex path: real / complex slots per chunk */
   int32_t dense_template;    /* real path: dense-position template of the sector tables, 1 = lean, 2 = two-loop sized
                                 (default: the one with the lower modelled cost) */
+  int32_t pole_extraction;   /* 0: subtraction (Eqs. 11-12; the default and the timed path).  1: integration by parts
+                                (Eq. 13, repeated -alpha_j times per variable; reading C30): same Laurent series, no
+                                large-number cancellation; real path only (lambda > 0: QMC_EUNSUPPORTED), generic kernel only,
+                                prod_j (1 - alpha_j) over the variables with alpha_j <= -1 of a sector at most 16 */
 } qmc_options;
 
 typedef struct qmc_tables qmc_tables; /* opaque sector tables (Eqs. 7-9) */
@@ -117,7 +121,8 @@ int qmc_tables_info(const qmc_tables *t, int32_t *n_sectors, int32_t *dim, int32
 
 /* Flat export of the tables so that an independent program can evaluate the SAME sectors (data, not code).
  * Layout: 8-byte words w[] (int64 unless noted):
- *   w[0]=0x514D4346 ('QMCF'), w[1]=version 1, w[2]=n_sectors, w[3]=dim n, w[4]=k_min, w[5]=k_max, w[6]=is_complex,
+ *   w[0]=0x514D4346 ('QMCF'), w[1]=version 1, w[2]=n_sectors, w[3]=dim n, w[4]=k_min, w[5]=k_max,
+ *   w[6]=is_complex + 2 * pole_extraction,
  *   w[7..10]=a_U0,a_U1,a_F0,a_F1 with U^{a_U0+a_U1 eps} F^{a_F0+a_F1 eps}, w[11]=lambda (double);
  *   then per sector: primary index, alpha[n], beta[n], nU, nF, nU x {coeff (double), e[n]}, nF x {coeff (double), e[n]}
  *   (variables in the ORIGINAL order t_1..t_n of Eq. 4, monomials in the library's evaluation order).

@@ -987,6 +987,8 @@ orc_problem* orc_from_tables(const int64_t* w, size_t nwords) {
   pb.aF0 = (int)w[9];
   pb.aF1 = (int)w[10];
   pb.lambda = d[11];
+  pb.ibp = (w[6] & 2) != 0 && pb.lambda == 0.0;  // tables prepared with pole_extraction = 1 (Eq. 13)
+  if (pb.ibp) pb.taylor = true;
   size_t p = 12;
   for (int s = 0; s < nsec; ++s) {
     Sector sc;

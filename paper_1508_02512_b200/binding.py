@@ -38,7 +38,8 @@ class qmc_kinematics(C.Structure):
 class qmc_options(C.Structure):
     _fields_ = [("lambda_", C.c_double), ("transform", C.c_int32), ("max_depth", C.c_int32), ("lattice", C.c_int32),
                 ("slot_budget", C.c_int32), ("chunk_bytes", C.c_int32), ("threads", C.c_int32),
-                ("slot_budget_cplx_real", C.c_int32), ("slot_budget_cplx", C.c_int32), ("dense_template", C.c_int32)]
+                ("slot_budget_cplx_real", C.c_int32), ("slot_budget_cplx", C.c_int32), ("dense_template", C.c_int32),
+                ("pole_extraction", C.c_int32)]
 
 
 class qmc_result(C.Structure):
@@ -193,10 +194,11 @@ class Tables:
 def qmc_prepare(wl=None, *, n_vertices=None, edges=None, leg_vertex=None, gram=None, eps_order: int = 0,
                 lam: float = 0.0, transform: int = 0, max_depth: int = 0, lattice: int = 0, slot_budget: int = 0,
                 chunk_bytes: int = 0, threads: int = 0, slot_budget_cplx_real: int = 0, slot_budget_cplx: int = 0,
-                dense_template: int = 0, nu=None) -> Tables:
+                dense_template: int = 0, nu=None, pole_extraction: int = 0) -> Tables:
     """qmc_prepare(graph, kinematics, eps_order) -> sector tables.  `wl` is a qmc_inputs.Workload, or pass the
     graph explicitly (edges = [(u, v, m^2), ...]).  slot_budget .. slot_budget_cplx are the table-layout fields of
-    qmc_options (0 = the library's defaults).  nu: propagator powers, one per edge (qmc_graph.edge_nu; None = all 1)."""
+    qmc_options (0 = the library's defaults).  nu: propagator powers, one per edge (qmc_graph.edge_nu; None = all 1).
+    pole_extraction = 1: integration by parts (Eq. 13) instead of the subtraction (real path, generic kernel)."""
     if wl is not None:
         n_vertices, edges, leg_vertex, gram = wl.n_vertices, wl.edges, wl.leg_vertex, wl.gram
         if nu is None:
@@ -213,7 +215,7 @@ def qmc_prepare(wl=None, *, n_vertices=None, edges=None, leg_vertex=None, gram=N
                   None if nu_arr is None else _ptr(nu_arr, C.c_int32), _ptr(lv, C.c_int32))
     k = qmc_kinematics(_ptr(gr, C.c_double))
     o = qmc_options(lam, transform, max_depth, lattice, slot_budget, chunk_bytes, threads, slot_budget_cplx_real,
-                    slot_budget_cplx, dense_template)
+                    slot_budget_cplx, dense_template, pole_extraction)
     h = C.c_void_p()
     rc = lib().qmc_prepare(C.byref(g), C.byref(k), eps_order, C.byref(o), C.byref(h))
     if rc:

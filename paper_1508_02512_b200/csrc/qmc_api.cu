@@ -684,7 +684,7 @@ int qmc_tables_export(const qmc_tables *t, void *buf, size_t *len) {
   w[p++] = t->n;
   w[p++] = t->kmin;
   w[p++] = t->kmax;
-  w[p++] = t->lambda > 0.0 ? 1 : 0;
+  w[p++] = (t->lambda > 0.0 ? 1 : 0) + (t->ibp ? 2 : 0);
   w[p++] = t->aU0;
   w[p++] = t->aU1;
   w[p++] = t->aF0;
@@ -1285,6 +1285,7 @@ int qmc_integrate_async(const qmc_tables *tc, uint64_t N, int32_t m, uint64_t se
   p.aU0 = t->aU0; p.aU1 = t->aU1; p.aF0 = t->aF0; p.aF1 = t->aF1;
   p.lambda = t->lambda;
   p.transform = t->transform;
+  p.ibp = t->ibp ? 1 : 0;
   qmc_transform_poly(t->transform, p.tc, p.wc);
   p.sec_begin = sb; p.sec_end = se; p.sec_per_chunk = spc;
   p.persec = persec ? 1 : 0;

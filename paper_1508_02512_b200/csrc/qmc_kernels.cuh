@@ -569,6 +569,205 @@ __device__ __noinline__ void sector_eval_taylor(const QmcLaunch &p, const QmcSec
   }
 }
 
+// ---- pole extraction by integration by parts (Eq. 13; qmc_options.pole_extraction = 1), real path -----
+// Eq. 13 applied a_b = -alpha_b times to every variable with alpha_b <= -1:
+//   int_0^1 dt t^(-a + beta eps) f = sum_{r<a} (-1)^r f^(r)(1) / prod_{s<=r} (s+1-a + beta eps)
+//                                  + (-1)^a / prod_{s<a} (s+1-a + beta eps)  int_0^1 dt t^(beta eps) f^(a)(t),
+// the operators of several variables multiplied out: a variable is taken at t_b = 1 with an order r_b < a_b, or keeps its
+// integral with order a_b.  f = G e^{eps Lambda}; its mixed derivatives are p! times the Taylor coefficients around the
+// point, from truncated power series in ALL variables with alpha_b <= -1 (at most QMC_IBP_JET coefficients).
+struct JetN {
+  double c[QMC_IBP_JET];
+};
+struct JetNShape {
+  int n, total;                                  // coefficients; sum of the orders kept
+  unsigned char dig[QMC_IBP_JET][QMC_MAXSING];   // index -> power of each variable
+  unsigned char dim[QMC_MAXSING], stride[QMC_MAXSING];
+};
+__device__ __forceinline__ JetN jetn_const(double v) {
+  JetN r;
+#pragma unroll
+  for (int i = 0; i < QMC_IBP_JET; ++i) r.c[i] = 0.0;
+  r.c[0] = v;
+  return r;
+}
+static __device__ __noinline__ JetN jetn_mul(const JetNShape &sh, const JetN &a, const JetN &b) {
+  JetN r = jetn_const(0.0);
+  for (int i = 0; i < sh.n; ++i)
+    for (int k = 0; k < sh.n; ++k) {
+      int idx = 0;
+      bool keep = true;
+#pragma unroll
+      for (int v = 0; v < QMC_MAXSING; ++v) {
+        const int pw = sh.dig[i][v] + sh.dig[k][v];
+        if (pw >= sh.dim[v]) keep = false;
+        idx += pw * sh.stride[v];
+      }
+      if (keep) r.c[idx] += a.c[i] * b.c[k];
+    }
+  return r;
+}
+// f(a0 + x) = sum_m co[m] x^m, x^m = 0 beyond m = total (<= QMC_IBP_JET - 1 orders)
+static __device__ __noinline__ JetN jetn_fn(const JetNShape &sh, const JetN &a, const double *co) {
+  JetN x = a, xm = jetn_const(1.0), r = jetn_const(0.0);
+  x.c[0] = 0.0;
+  for (int m = 0; m <= sh.total; ++m) {
+    for (int i = 0; i < sh.n; ++i) r.c[i] += co[m] * xm.c[i];
+    if (m < sh.total) xm = jetn_mul(sh, xm, x);
+  }
+  return r;
+}
+__device__ __forceinline__ JetN jetn_recip(const JetNShape &sh, const JetN &a) {
+  double co[QMC_IBP_JET];
+  const double r0 = 1.0 / a.c[0];
+  double v = r0;
+  for (int m = 0; m <= sh.total; ++m) {
+    co[m] = v;
+    v *= -r0;
+  }
+  return jetn_fn(sh, a, co);
+}
+__device__ __forceinline__ JetN jetn_log(const JetNShape &sh, const JetN &a) {
+  double co[QMC_IBP_JET];
+  const double r0 = 1.0 / a.c[0];
+  double v = r0;
+  co[0] = log(a.c[0]);
+  for (int m = 1; m <= sh.total; ++m) {
+    co[m] = v / (double)m;
+    v *= -r0;
+  }
+  return jetn_fn(sh, a, co);
+}
+__device__ __forceinline__ JetN jetn_ipow(const JetNShape &sh, const JetN &a, int e) {
+  const JetN base = e >= 0 ? a : jetn_recip(sh, a);
+  JetN r = jetn_const(1.0);
+  for (int q = 0; q < (e < 0 ? -e : e); ++q) r = jetn_mul(sh, r, base);
+  return r;
+}
+
+template <int NDIM, int KMAX>
+__device__ __noinline__ void sector_eval_ibp(const QmcLaunch &p, const QmcSectorHdr *h, const double *pt,
+                                             double (&out)[QMC_MAXSING + KMAX + 1]) {
+  constexpr int KS = QMC_MAXSING + KMAX + 1;
+  const double *coef = reinterpret_cast<const double *>(h + 1);
+  const uint32_t *exps = reinterpret_cast<const uint32_t *>(coef + (h->nU + h->nF));
+  const int nv = h->nsing, nU = h->nU, nT = h->nU + h->nF;
+  double t[NDIM], lt[NDIM];
+#pragma unroll
+  for (int k = 0; k < NDIM; ++k) {
+    const int j = h->perm[k];
+    t[k] = pt[(0 * NDIM + j) * QMC_THREADS];
+    lt[k] = pt[(1 * NDIM + j) * QMC_THREADS];
+  }
+  double G0 = 1.0, L0 = 0.0;
+  for (int k = nv; k < NDIM; ++k) {
+    G0 *= ipow_pos(t[k], h->alpha[k]);
+    L0 += (double)h->beta[k] * lt[k];
+  }
+#pragma unroll
+  for (int i = 0; i < KS; ++i) out[i] = 0.0;
+  for (int B = 0; B < (1 << nv); ++B) {  // B: the variables taken at the boundary t_b = 1
+    JetNShape sh;
+    double tau[QMC_MAXSING], Lint = L0;
+    sh.n = 1;
+    sh.total = 0;
+    for (int b = 0; b < QMC_MAXSING; ++b) {
+      int ord = 0;
+      tau[b] = 1.0;
+      if (b < nv) {
+        const int a = -h->alpha[b];
+        const bool atone = B >> b & 1;
+        ord = atone ? a - 1 : a;
+        if (!atone) {
+          tau[b] = t[b];
+          Lint += (double)h->beta[b] * lt[b];  // the factor t_b^(beta_b eps) under the integral
+        }
+      }
+      sh.dim[b] = (unsigned char)(ord + 1);
+      sh.stride[b] = (unsigned char)sh.n;
+      sh.n *= ord + 1;
+      sh.total += ord;
+    }
+    for (int i = 0; i < sh.n; ++i)
+      for (int b = 0; b < QMC_MAXSING; ++b) sh.dig[i][b] = (unsigned char)((i / sh.stride[b]) % sh.dim[b]);
+    // U^, F^ around the point: (tau + d)^e = sum_p C(e, p) tau^(e-p) d^p
+    JetN U = jetn_const(0.0), F = jetn_const(0.0);
+    for (int mi = 0; mi < nT; ++mi) {
+      const uint32_t w = exps[mi];
+      double c0 = coef[mi];
+      for (int k = nv; k < NDIM; ++k) c0 *= ipow_pos(t[k], (w >> (4 * k)) & 15);
+      for (int i = 0; i < sh.n; ++i) {
+        double c = c0;
+        bool keep = true;
+        for (int b = 0; b < nv; ++b) {
+          const int e = (w >> (4 * b)) & 15, pw = sh.dig[i][b];
+          if (pw > e) {
+            keep = false;
+            break;
+          }
+          double bin = 1.0;
+          for (int q = 0; q < pw; ++q) bin = bin * (double)(e - q) / (double)(q + 1);
+          c *= bin * ipow_pos(tau[b], e - pw);
+        }
+        if (keep) (mi < nU ? U : F).c[i] += c;
+      }
+    }
+    JetN W = jetn_mul(sh, jetn_ipow(sh, U, p.aU0), jetn_ipow(sh, F, p.aF0));
+    const JetN lU = jetn_log(sh, U), lF = jetn_log(sh, F);
+    JetN Lam = jetn_const(0.0);
+    for (int i = 0; i < sh.n; ++i) {
+      W.c[i] *= G0;
+      Lam.c[i] = (double)p.aU1 * lU.c[i] + (double)p.aF1 * lF.c[i];
+    }
+    Lam.c[0] += Lint;
+    JetN E[KS];  // E[k] = W Lam^k / k!
+    E[0] = W;
+    for (int k = 1; k < KS; ++k) {
+      E[k] = jetn_mul(sh, E[k - 1], Lam);
+      const double rk = 1.0 / (double)k;
+      for (int i = 0; i < sh.n; ++i) E[k].c[i] *= rk;
+    }
+    for (int i = 0; i < sh.n; ++i) {  // derivative orders: r_b < a_b at the boundary, exactly a_b under the integral
+      bool use = true;
+      for (int b = 0; b < nv; ++b)
+        if (!(B >> b & 1) && sh.dig[i][b] != -h->alpha[b]) use = false;
+      if (!use) continue;
+      double scalar = 1.0, ser[KS];
+      int npole = 0;
+      for (int k = 0; k < KS; ++k) ser[k] = E[k].c[i];
+      for (int b = 0; b < nv; ++b) {
+        const int a = -h->alpha[b], pw = sh.dig[i][b];
+        const double beta = (double)h->beta[b];
+        for (int q = 2; q <= pw; ++q) scalar *= (double)q;  // derivative = Taylor coefficient times p!
+        if (pw & 1) scalar = -scalar;
+        const int smax = pw < a - 1 ? pw : a - 1;
+        for (int sf = 0; sf <= smax; ++sf) {  // 1 / (s+1-a + beta eps)
+          const int c = sf + 1 - a;
+          if (c == 0) {
+            scalar *= 1.0 / beta;
+            ++npole;
+          } else {  // (1/c) sum_m (-beta eps / c)^m
+            double r[KS];
+            for (int k = 0; k < KS; ++k) r[k] = 0.0;
+            for (int k = 0; k < KS; ++k) {
+              double gm = 1.0 / (double)c;
+              for (int m = 0; k + m < KS; ++m) {
+                r[k + m] += ser[k] * gm;
+                gm *= -beta / (double)c;
+              }
+            }
+            for (int k = 0; k < KS; ++k) ser[k] = r[k];
+          }
+        }
+      }
+      for (int k = 0; k < KS; ++k) {
+        const int order = k - npole;
+        if (order <= KMAX) out[order + QMC_MAXSING] += scalar * ser[k];
+      }
+    }
+  }
+}
+
 __device__ __forceinline__ bool finite_all(double v) { return fabs(v) <= 1.79769313486231570e308; }
 __device__ __forceinline__ bool finite_all(cd v) { return finite_all(v.re) && finite_all(v.im); }
 
@@ -744,10 +943,13 @@ __global__ void __launch_bounds__(QMC_THREADS, QMC_V1_MIN_BLOCKS) qmc_eval_kerne
       }                                                                                 \
     }                                                                                   \
   } break;
-        if (TAYLOR && !CPLX && (h->flags & 2)) {
+        if (TAYLOR && !CPLX && (p.ibp ? ns > 0 : (h->flags & 2) != 0)) {
           if constexpr (TAYLOR && !CPLX) {
             double res[NACC];
-            sector_eval_taylor<NDIM, KMAX>(p, h, pt, res);
+            if (p.ibp)
+              sector_eval_ibp<NDIM, KMAX>(p, h, pt, res);
+            else
+              sector_eval_taylor<NDIM, KMAX>(p, h, pt, res);
 #pragma unroll
             for (int i = 0; i < NACC; ++i) {
               fin = fin && finite_all(res[i]);

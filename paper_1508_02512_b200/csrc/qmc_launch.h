@@ -37,6 +37,7 @@ struct QmcLaunch {
   int32_t transform;
   int32_t sec_begin, sec_end, sec_per_chunk;
   int32_t persec;                // 0: fused (all sectors of the chunk summed), 1: per-sector sums
+  int32_t ibp;                   // 1: pole extraction by integration by parts (Eq. 13) instead of the subtraction (Taylor flavour only)
   uint32_t tab_smem_bytes;       // shared-memory bytes reserved for the table chunk
 };
 

@@ -202,6 +202,12 @@ static int qmc_build_sectors(const qmc_graph *g, const qmc_kinematics *kin, int 
   T->transform = opt ? opt->transform : 0;
   T->lattice = opt ? opt->lattice : 0;
   if (T->lambda < 0.0 || (T->transform < 0 || T->transform > 2) || (T->lattice != 0 && T->lattice != 1)) return QMC_EINVAL;
+  const int pole = opt ? opt->pole_extraction : 0;
+  if (pole != 0 && pole != 1) return QMC_EINVAL;
+  if (pole == 1) {  // integration by parts (Eq. 13; R:C30): real path, generic kernel (its Taylor flavour)
+    if (T->lambda > 0.0) return QMC_EUNSUPPORTED;
+    T->ibp = T->has_taylor = T->generic_only = true;
+  }
   const int max_depth = (opt && opt->max_depth > 0) ? opt->max_depth : 64;
   const int n = T->n;
   T->kmax = eps_order;
@@ -257,6 +263,12 @@ static int qmc_build_sectors(const qmc_graph *g, const qmc_kinematics *kin, int 
         if (nd.alpha[j] > 127 || nd.beta[j] > 127 || nd.beta[j] < -127) return QMC_EUNSUPPORTED;
       }
       if (s.nsing > QMC_MAXSING) return QMC_EUNSUPPORTED;
+      if (T->ibp) {  // Taylor coefficients around the point: orders 0 .. -alpha_b in every variable with alpha_b <= -1
+        int njet = 1;
+        for (int j = 0; j < n; ++j)
+          if (nd.alpha[j] <= -1) njet *= 1 - nd.alpha[j];
+        if (njet > QMC_IBP_JET) return QMC_EUNSUPPORTED;
+      }
       if (s.ndeep) T->has_taylor = T->generic_only = true;  // only the generic kernel has Taylor-coefficient corners
       smax = std::max(smax, s.nsing);
       for (int which = 0; which < 2; ++which)

@@ -8,6 +8,7 @@
 #include "../../include/qmc_feynman.h"
 
 #define QMC_MAXDIM 8    // integration variables per sector (P - 1)
+#define QMC_IBP_JET 16    // integration by parts: largest number of Taylor coefficients prod_b (1 - alpha_b) of a sector
 #define QMC_MAXTAYLOR 3   // most negative exponent -alpha of a variable the generic kernel's Taylor corners handle
 #define QMC_MAXSING 4   // singular variables (alpha = -1) per sector handled by the kernels
 #define QMC_MAXK 8      // eps orders kept: k_max - k_min + 1
@@ -189,6 +190,7 @@ struct qmc_tables {
   int resident_kind = 0;              // 4: logarithm table (versions 4, 5), 1: version-1 image
   int resident_m = 0;                 // number of shift vectors resident in that workspace (0 = none)
   uint64_t resident_seed = 0;         // seed that produced them ...
+  bool ibp = false;                   // qmc_options.pole_extraction = 1: Eq. 13 instead of Eqs. 11-12 (generic kernel, real path)
   bool has_taylor = false;            // some sector has a variable with alpha <= -2
   bool generic_only = false;          // propagator powers other than 1: only the generic kernel has run-time exponents
   bool resident_explicit = false;     // ... or: they were passed explicitly (qmc_run.shifts)

@@ -588,3 +588,49 @@ def test_taylor_terms_for_alpha_below_minus_one_on_the_generic_kernel():
         with pytest.raises(q.QmcError) as e:
             q.qmc_prepare(wl, lam=wl.lam)
         assert e.value.status == -3
+
+
+def test_pole_extraction_by_integration_by_parts():
+    """SURVEY 8(f) f3, reading C30: qmc_options.pole_extraction = 1 extracts the poles by Eq. 13 instead of the
+    subtraction.  Parity per sector, order and shift against the oracle's own IBP (sector_point_ibp) on the product's tables;
+    the closed forms on the GPU numbers; the cancellation factor the paper introduces IBP for."""
+    import dataclasses
+    import mpmath as mp
+    # one-loop massless box: three variables, up to two singular ones; closed form
+    r, f, S, A, _ = parity(qi.massless_box(), 32749, 6, pole_extraction=1)
+    ex = [0.666666666666667, -1.2639198230760183, -1.2238036181980894]
+    assert np.all(np.abs(f.coeff.real - ex) <= 4 * f.err.real + 1e-12), (f.coeff.real, f.err.real)
+    T, AT = S.sum(axis=0), A.sum(axis=0)
+    assert (AT / np.abs(T)).max() < 100.0
+    parity(qi.massless_box(), 16381, 3, pole_extraction=1, eps_order=1, transform=1)
+    parity(qi.triangle(), 32749, 4, pole_extraction=1)
+    parity(qi.bubble(), 10007, 4, pole_extraction=1)                      # no singular variable: nothing to extract
+    # variables with alpha = -2, -3: Eq. 13 two and three times; Eq. 21's transform throughout
+    wl = dataclasses.replace(qi.bubble(-1.7, 0.0, 0.0), nu=(3, 1), eps_order=1)
+    r, f, S, A, _ = parity(wl, 65521, 8, pole_extraction=1)
+    want = _laurent(lambda x: mp.mpf(1.7) ** (-2 - x) * mp.beta(-1 - x, 1 - x), -1, 1)
+    assert np.all(np.abs(f.coeff.real - want) <= 4 * f.err.real + 1e-9), (f.coeff.real, f.err.real, want)
+    s = -2.0
+    for nu in ((2, 1, 1), (1, 1, 2)):
+        wl = dataclasses.replace(qi.triangle(s), nu=nu, eps_order=0)
+        r, f, S, A, _ = parity(wl, 99991, 8, pole_extraction=1)
+        Nn = sum(nu)
+        want = _laurent(lambda x: (-s) ** (2 - x - Nn) * mp.gamma(nu[0]) * mp.gamma(nu[1] + 2 - x - Nn) * mp.gamma(nu[2] + 2 - x - Nn)
+                        / mp.gamma(4 - 2 * x - Nn), -2, 0)
+        assert np.all(np.abs(f.coeff.real - want) <= 4 * f.err.real + 1e-9), (nu, f.coeff.real, f.err.real, want)
+        T, AT = S.sum(axis=0), A.sum(axis=0)
+        assert (AT / np.maximum(np.abs(T), 1e-300)).max() < 100.0      # the subtraction: 1e14 on the same graph (profiles/r02e_parity_floor.json)
+    parity(dataclasses.replace(qi.triangle(s), nu=(1, 1, 3)), 16381, 3, pole_extraction=1)
+    parity(dataclasses.replace(qi.massless_box(), nu=(2, 1, 1, 1)), 16381, 2, pole_extraction=1)
+    # two loops: sectors of the double box with two, three and four singular variables (16 Taylor coefficients)
+    parity(qi.double_box(), 16381, 2, sectors=(118, 126), pole_extraction=1)
+    # refused: the complex path; a sector whose series would need more than 16 coefficients
+    with pytest.raises(q.QmcError) as e:
+        q.qmc_prepare(qi.massive_box(), lam=0.5, pole_extraction=1)
+    assert e.value.status == -3
+    with pytest.raises(q.QmcError) as e:
+        q.qmc_prepare(dataclasses.replace(qi.massless_box(), nu=(3, 3, 1, 1)), pole_extraction=1)
+    assert e.value.status == -3
+    with pytest.raises(q.QmcError) as e:
+        q.qmc_prepare(qi.massless_box(), pole_extraction=2)
+    assert e.value.status == -1
