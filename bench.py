@@ -279,6 +279,30 @@ def closed_form_check(q, dev):
     return out
 
 
+def pole_extraction_comparison(q, dev):
+    """SURVEY 8(f) f3 (not part of the timed path): subtraction (Eqs. 11-12) against integration by parts (Eq. 13,
+    qmc_options.pole_extraction = 1), both on the generic kernel, same lattice and shifts, Eq. 21's transform: the massless box
+    of config 2 (every alpha_j >= -1) and the triangle with a squared propagator (a variable with alpha_j = -2, which needs the
+    p = 1 Taylor term of Eq. 11), with the ACTUAL deviation from the closed forms (massless box: tests/test_oracle_closed_forms.py;
+    triangle: Dirichlet's integral 2^(-2-eps) Gamma(-1-eps) Gamma(-eps) / Gamma(-2 eps), tests/test_oracle_taylor_terms.py)."""
+    import dataclasses
+    tri = dataclasses.replace(qi.triangle(-2.0), nu=(1, 1, 2), eps_order=0)
+    out = []
+    for wl, N, exact in ((qi.massless_box(), 99991, [0.666666666666667, -1.2639198230760183, -1.2238036181980894]),
+                         (tri, 99991, [0.0, 0.5, -0.8465735902799727])):
+        for pe in (0, 1):
+            t = q.qmc_prepare(wl, eps_order=wl.eps_order, pole_extraction=pe, nu=getattr(wl, "nu", None))
+            z = q.qmc_generating_vector(N, t.dim, device=dev)
+            sh = qi.splitmix64_shifts(wl.seed, 16, t.dim)
+            q.qmc_integrate(t, N, 16, z=z, shifts=sh, device=dev, kernel=1)
+            r = q.qmc_integrate(t, N, 16, z=z, shifts=sh, device=dev, kernel=1)
+            out.append({"workload": wl.name, "nu": list(getattr(wl, "nu", None) or []), "pole_extraction": pe, "N": N, "m": 16,
+                        "exact": exact, "value": [float(x) for x in r.coeff.real], "estimated_err": [float(x) for x in r.err.real],
+                        "deviation_in_sigma": [float(abs(v - e) / max(s, 1e-300)) for v, e, s in zip(r.coeff.real, exact, r.err.real)],
+                        "eval_kernel_ms": float(r.eval_kernel_ms)})
+    return out
+
+
 def per_sector_mode(q, t, N, m, z, shifts, dev, torch):
     """the per-sector (parity) mode of the kernel next to the fused (throughput) mode the headline times."""
     q.qmc_integrate(t, N, m, z=z, shifts=shifts, per_sector=True, device=dev)
@@ -497,6 +521,7 @@ def run_product(args):
         line["per_sector_mode"] = extra(per_sector_mode, q, t, min(N, 999983), m, q.qmc_generating_vector(min(N, 999983), t.dim, device=dev), shifts, dev, torch)
         line["other_workloads"] = extra(other_workloads, q, torch, dev, args.config)
         line["kinematic_scan"] = extra(kinematic_scan, q, torch)
+        line["pole_extraction"] = extra(pole_extraction_comparison, q, dev)
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

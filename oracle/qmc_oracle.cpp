@@ -37,6 +37,9 @@
 // sector_point_taylor.  Pins (tests/test_oracle_taylor_terms.py): reduction to the double sum of O7 where no alpha_j <= -2,
 // monomial integrals, Dirichlet eta values, Euler's hypergeometric integral, the Beta function of the massless propagator
 // with powers, Dirichlet's integral of the triangle with a squared propagator, simplex quadrature of a massive bubble.
+// Pole extraction by integration by parts (Eq. 13; reading C30) instead of the subtraction: sector_point_ibp, real
+// path only, when asked for (orc_build_nu(..., flags & 2), or tables exported with pole_extraction = 1).  Pins
+// (tests/test_oracle_ibp.py): the same closed forms and the massless box reached through IBP; cancellation factors.
 // =====================================================================================
 #include <algorithm>
 #include <cmath>

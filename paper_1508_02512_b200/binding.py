@@ -225,10 +225,16 @@ def qmc_prepare(wl=None, *, n_vertices=None, edges=None, leg_vertex=None, gram=N
 
 def qmc_prepare_batch(wls, *, eps_order: int = 0, lam: float = 0.0, transform: int = 0, max_depth: int = 0, lattice: int = 0,
                       slot_budget: int = 0, chunk_bytes: int = 0, threads: int = 0, slot_budget_cplx_real: int = 0,
-                      slot_budget_cplx: int = 0, dense_template: int = 0) -> Tables:
+                      slot_budget_cplx: int = 0, dense_template: int = 0, nu=None, pole_extraction: int = 0) -> Tables:
     """qmc_prepare_batch: ONE graph (taken from wls[0]) at the kinematic points of the workloads `wls` (their Gram matrices).
-    Integrate with qmc_integrate(..., mode=3): results per kinematic point."""
+    Integrate with qmc_integrate(..., mode=3): results per kinematic point.  nu, pole_extraction: as in qmc_prepare (such
+    tables run on the generic kernel, which has no mode 3: integrate them per point)."""
     w0 = wls[0]
+    if nu is None:
+        nu = getattr(w0, "nu", None)
+    nu_arr = None if nu is None else np.ascontiguousarray(nu, dtype=np.int32)
+    if nu_arr is not None and nu_arr.size != len(w0.edges):
+        raise ValueError("qmc_prepare_batch: one propagator power per edge")
     eu = np.ascontiguousarray([e[0] for e in w0.edges], dtype=np.int32)
     ev = np.ascontiguousarray([e[1] for e in w0.edges], dtype=np.int32)
     m2 = np.ascontiguousarray([e[2] for e in w0.edges], dtype=np.float64)
@@ -236,11 +242,11 @@ def qmc_prepare_batch(wls, *, eps_order: int = 0, lam: float = 0.0, transform: i
     grams = [np.ascontiguousarray(w.gram, dtype=np.float64) for w in wls]
     for w in wls:
         assert w.edges == w0.edges and list(w.leg_vertex) == list(w0.leg_vertex), "a batch is one graph at several kinematic points"
-    g = qmc_graph(w0.n_vertices, len(w0.edges), len(lv), _ptr(eu, C.c_int32), _ptr(ev, C.c_int32), _ptr(m2, C.c_double), None,
-                  _ptr(lv, C.c_int32))
+    g = qmc_graph(w0.n_vertices, len(w0.edges), len(lv), _ptr(eu, C.c_int32), _ptr(ev, C.c_int32), _ptr(m2, C.c_double),
+                  None if nu_arr is None else _ptr(nu_arr, C.c_int32), _ptr(lv, C.c_int32))
     kins = (qmc_kinematics * len(wls))(*[qmc_kinematics(_ptr(gr, C.c_double)) for gr in grams])
     o = qmc_options(lam, transform, max_depth, lattice, slot_budget, chunk_bytes, threads, slot_budget_cplx_real,
-                    slot_budget_cplx, dense_template)
+                    slot_budget_cplx, dense_template, pole_extraction)
     h = C.c_void_p()
     rc = lib().qmc_prepare_batch(C.byref(g), kins, len(wls), eps_order, C.byref(o), C.byref(h))
     if rc:
