@@ -15,7 +15,7 @@
 #include "qmc_tables.h"
 
 namespace {
-const double F_LOG = 44.0, F_RCP = 10.0, F_DIV = 16.0, F_ATAN2 = 60.0;
+const double F_LOG = 44.0, F_RCP = 10.0, F_ATAN2 = 60.0;
 const double F_CMUL = 6.0, F_CADD = 2.0;                  // complex multiply (4 mul + 2 add), complex add
 const double F_CINV = 3.0 + F_RCP + 2.0;                  // |a|^2, reciprocal, two scalings
 const double F_CLOG = 3.0 + F_LOG + 1.0 + F_ATAN2;        // 0.5 log(|a|^2), atan2
@@ -36,8 +36,8 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
   const bool cplx = t->lambda > 0.0;
   // S1-S3, once per (point, shift): u = r/N (IEEE division), y = u + Delta (wrap), t = y^2 (3 - 2y), w *= 6 y (1 - y),
   // ln t (table logarithm)
-  // (real path: r / N as r * RN(1/N) with one FMA correction, 5 flops; complex path: the division routine)
-  double per_point = n * ((cplx ? F_DIV : 5.0) + 2.0 + 4.0 + 4.0 + 18.0);
+  // (r / N as r * RN(1/N) with one FMA correction, 5 flops, on both paths)
+  double per_point = n * (5.0 + 2.0 + 4.0 + 4.0 + 18.0);
   if (!cplx)  // the chunks' product slots, once per point and chunk touched
     for (const Qmc2Chunk &c : t->chunks)
       if (c.sec_end > sb && c.sec_begin < se) per_point += (double)(c.nslots - (2 * n + 2 + c.nconst));

@@ -428,7 +428,7 @@ __global__ void __launch_bounds__(QMC3_THREADS, QMC5_MINB(NDIM)) qmc5_eval_kerne
   __syncthreads();
 
   const uint32_t N = p.N;
-  const double dN = (double)N;
+  const double dN = (double)N, invN = 1.0 / dN;
   const uint32_t stride = (uint32_t)p.nslices * T;
   uint32_t dz[NDIM];
 #pragma unroll
@@ -454,7 +454,10 @@ __global__ void __launch_bounds__(QMC3_THREADS, QMC5_MINB(NDIM)) qmc5_eval_kerne
       bool inside = true;
 #pragma unroll
       for (int j = 0; j < NDIM; ++j) {
-        double u = (double)r[j] / dN;
+        // u = r / N correctly rounded (the oracle's IEEE division) as on the real path: q = r * RN(1/N), exact remainder by
+        // FMA, one correction (Markstein; r, N integers below 2^31)
+        const double rd = (double)r[j], q0 = rd * invN;
+        const double u = fma(fma(-q0, dN, rd), invN, q0);
         double y = u + shf[kap * NDIM + j];
         if (y >= 1.0) y -= 1.0;
         double tj;
