@@ -86,7 +86,7 @@ __device__ __forceinline__ void corner5(const Qmc5Launch &p, const uint32_t cw, 
                                         const uint32_t lcw, const uint32_t nlocal_c,
                                         const double G0, const double L0, unsigned char *__restrict__ slr,
                                         unsigned char *__restrict__ slc, const double2 *__restrict__ tabq, cd &Wout, cd &Lout,
-                                        unsigned &cntImF, unsigned &cntReU) {
+                                        unsigned &cntImF, unsigned &cntReU, const bool need_lambda) {
   constexpr int T = QMC3_THREADS, NDERIV = NDIM + NDIM * (NDIM + 1) / 2, NPOLY = NDERIV + 2, CW = (NPOLY + 15) / 16;
   typedef Expo<NDIM, L> E;
   uint32_t zv = 0;  // variables set to zero
@@ -264,26 +264,35 @@ __device__ __forceinline__ void corner5(const Qmc5Launch &p, const uint32_t cw, 
   // The 2 + n principal logarithms are taken as ONE: Lambda_Z - L0 = ln Q + 2 pi i k with Q = U^aU1 F^aF1 prod_j rho_j^beta_j
   // (complex products) and the winding number k fixed by single-precision estimates of the same phases: the sum of the
   // principal phases, known to 1e-3, differs from the principal phase of Q by an exact multiple of 2 pi.
+  // Lambda_Z is needed only where the corner's eps-series has more than one term (need_lambda, warp-uniform: k_max > 0 or Z
+  // not empty); a corner with a one-term window -- every corner of a sector without singular variables at k_max = 0 -- skips it.
   cd num = cd{G0 * det.re, G0 * det.im}, den = cd{1.0, 0.0};
-  cd qn = cpow_c<(E::aU1 > 0 ? E::aU1 : 0)>(Uv), qd = cpow_c<(E::aF1 < 0 ? -E::aF1 : 0)>(Fv);
-  float th = (float)E::aU1 * arg_estimate(Uv) + (float)E::aF1 * arg_estimate(Fv);
 #pragma unroll
   for (int j = 0; j < NDIM; ++j) {
     const bool inZ = (zv >> j & 1u) != 0;
-    const int a = sext8(j < 4 ? alo : ahi, j & 3), b = sext8(j < 4 ? blo : bhi, j & 3);
+    const int a = sext8(j < 4 ? alo : ahi, j & 3);
     if (!inZ) {
       if (a < 0) den = den * rho[j];
       for (int q = 0; q < a; ++q) num = num * rho[j];
     }
-    if (b) {
-      th += (float)b * arg_estimate(rho[j]);
-      for (int q = 0; q < b; ++q) qn = qn * rho[j];
-      for (int q = 0; q < -b; ++q) qd = qd * rho[j];
-    }
   }
-  cd Lam = clog5(qn * cinv5(qd), tabq);
-  Lam.im = fma((double)rintf((th - (float)Lam.im) * 0.15915494f), 6.28318530717958647692, Lam.im);
-  Lam.re += L0;
+  cd Lam = cd{0.0, 0.0};
+  if (need_lambda) {
+    cd qn = cpow_c<(E::aU1 > 0 ? E::aU1 : 0)>(Uv), qd = cpow_c<(E::aF1 < 0 ? -E::aF1 : 0)>(Fv);
+    float th = (float)E::aU1 * arg_estimate(Uv) + (float)E::aF1 * arg_estimate(Fv);
+#pragma unroll
+    for (int j = 0; j < NDIM; ++j) {
+      const int b = sext8(j < 4 ? blo : bhi, j & 3);
+      if (b) {
+        th += (float)b * arg_estimate(rho[j]);
+        for (int q = 0; q < b; ++q) qn = qn * rho[j];
+        for (int q = 0; q < -b; ++q) qd = qd * rho[j];
+      }
+    }
+    Lam = clog5(qn * cinv5(qd), tabq);
+    Lam.im = fma((double)rintf((th - (float)Lam.im) * 0.15915494f), 6.28318530717958647692, Lam.im);
+    Lam.re += L0;
+  }
   if (E::aU0 > 0) num = num * cpow_c<(E::aU0 > 0 ? E::aU0 : 0)>(Uv);
   if (E::aU0 < 0) den = den * cpow_c<(E::aU0 < 0 ? -E::aU0 : 0)>(Uv);
   if (E::aF0 > 0) num = num * cpow_c<(E::aF0 > 0 ? E::aF0 : 0)>(Fv);
@@ -364,7 +373,8 @@ __device__ __forceinline__ void sector5(const Qmc5Launch &p, const uint32_t o, u
   for (int Z = 0; Z < NG; ++Z) {
     cd W, Lam;
     const uint32_t cw = o + (Z == 0 ? cws[0] : Z == 1 ? cws[1] : Z == 2 ? cws[2] : cws[3]);
-    corner5<NDIM, L, NS>(p, cw, Z, h1.x, h1.z, h1.w, h2.x, h2.y, lcw, nlocal_c, G0, L0, slr, slc, tabq, W, Lam, cntImF, cntReU);
+    corner5<NDIM, L, NS>(p, cw, Z, h1.x, h1.z, h1.w, h2.x, h2.y, lcw, nlocal_c, G0, L0, slr, slc, tabq, W, Lam, cntImF, cntReU,
+                         KMAX > 0 || Z != 0);
 #pragma unroll
     for (int q = 0; q < NG; ++q)
       if (Z == q) {  // warp-uniform: the results land in compile-time registers
