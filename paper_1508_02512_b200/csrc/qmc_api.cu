@@ -1470,10 +1470,18 @@ int qmc_tables_describe(const qmc_tables *t, char *buf, size_t len) {
   if (!t || !buf || len < 1) return QMC_EINVAL;
   std::string o;
   char line[256];
-  std::snprintf(line, sizeof line, "sectors %d dim %d loops %d orders %d..%d lambda %g generic image %zu B real-path tables %zu B chunks %zu threads %d template %d\n",
+  int ntaylor = 0;
+  for (const QmcSector &s : t->sectors) ntaylor += s.ndeep > 0;
+  std::snprintf(line, sizeof line, "sectors %d dim %d loops %d orders %d..%d lambda %g generic image %zu B real-path tables %zu B chunks %zu threads %d template %d",
                 (int)t->sectors.size(), t->n, t->L, t->kmin, t->kmax, t->lambda, t->image.size(), t->tab4.size() * 4, t->chunks.size(),
                 t->threads_real, t->tpl_real);
   o += line;
+  if (t->generic_only) {  // propagator powers, sectors with alpha <= -2, integration by parts: the generic kernel only
+    std::snprintf(line, sizeof line, " generic kernel only (exponents U^%d%+deps F^%d%+deps, sectors with Taylor terms %d, pole extraction %s)",
+                  t->aU0, t->aU1, t->aF0, t->aF1, ntaylor, t->ibp ? "by parts" : "subtraction");
+    o += line;
+  }
+  o += "\n";
   for (size_t c = 0; c < t->chunks.size(); ++c) {
     const Qmc2Chunk &ch = t->chunks[c];
     std::snprintf(line, sizeof line, "chunk %zu: sectors [%d,%d) slots %d (constants %d, products %d) tables %u B records %d (one-factor %d, beyond the dense positions %d) local products %d (max local slots %d) cost %.0f\n", c,
