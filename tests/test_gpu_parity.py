@@ -173,6 +173,35 @@ def test_paper_table1_kinematics():
     parity(qi.double_box(-2 / 3, -2 / 3, p2=(0, 0, -1, -1)), 16381, 2, sectors=(0, 60))
 
 
+def test_paper_table1_values_from_the_gpu_numbers():
+    """Level 2 on the paper's worked example: its Table 1 (fixture tests/golden/paper_table1.txt, the loader
+    and the prefactor convention of tests/test_oracle_paper_table1.py) from the library's own run -- qmc_prepare, the library's
+    generating vector and seeded shifts, the fused kernels -- at N = 999983: all printed entries of the three mass assignments
+    within 4 sigma of the printed values (both columns), with our error at most a tenth of a percent of the value."""
+    import mpmath as mp
+    from test_oracle_paper_table1 import load_table
+    s = t = -2.0 / 3.0
+    pref = np.array([float(x) for x in mp.taylor(lambda e: mp.exp(2 * e * mp.euler) * mp.mpf(-s) ** (3 + 2 * e) * mp.gamma(3 + 2 * e), 0, 4)])
+    checked = 0
+    for legs, table in sorted(load_table().items()):
+        tb = q.qmc_prepare(qi.double_box(s, t, p2=legs), eps_order=0)
+        m = 8
+        r = q.qmc_integrate(tb, 999983, m, seed=101)
+        assert not r.counters.any()
+        T = r.shift_totals.real                      # [K, m], orders k_min .. 0
+        full = np.zeros((5, m))
+        full[5 - T.shape[0]:] = T
+        for i in range(5):                           # P_i: coefficient of eps^-i, per shift (errors include the correlations)
+            k = 4 - i
+            Pi = sum(pref[qq] * full[k - qq] for qq in range(k + 1))
+            mean, err = Pi.mean(), Pi.std(ddof=1) / np.sqrt(m)
+            assert err <= max(1e-3 * abs(table[i][1][0]), 1e-6), (legs, i, err)
+            for val, perr in table[i]:
+                assert abs(mean - val) <= 4.0 * np.hypot(err, perr) + 1e-5 * max(1.0, abs(val)), (legs, i, mean, err, val, perr)
+                checked += 1
+    assert checked == 30
+
+
 def test_edge_cases_boundary_points_and_tiny_lattices():
     wl = qi.massless_box()
     # a zero shift component puts lattice index 0 on the boundary: contributes exactly 0, counted
