@@ -92,6 +92,11 @@ typedef struct {
                                 (Eq. 13, repeated -alpha_j times per variable; reading C30): same Laurent series, no
                                 large-number cancellation; real path only (lambda > 0: QMC_EUNSUPPORTED), generic kernel only,
                                 prod_j (1 - alpha_j) over the variables with alpha_j <= -1 of a sector at most 16 */
+  int32_t strategy;          /* decomposition strategy.  0: iterated, the deterministic rule of DESIGN.md reading C7 (all configs, the
+                                default).  1: geometric (Kaneko-Ueda; the strategy the paper says it uses): one monomial
+                                substitution per simplicial cone of the normal fan of the Newton polyhedron of U_l F_l, guaranteed to
+                                terminate (reading C31; a cone with |det V| > 1: QMC_EUNSUPPORTED -- none was met).  The totals do not
+                                depend on the strategy, the sectors do */
 } qmc_options;
 
 typedef struct qmc_tables qmc_tables; /* opaque sector tables (Eqs. 7-9) */

@@ -39,7 +39,7 @@ class qmc_options(C.Structure):
     _fields_ = [("lambda_", C.c_double), ("transform", C.c_int32), ("max_depth", C.c_int32), ("lattice", C.c_int32),
                 ("slot_budget", C.c_int32), ("chunk_bytes", C.c_int32), ("threads", C.c_int32),
                 ("slot_budget_cplx_real", C.c_int32), ("slot_budget_cplx", C.c_int32), ("dense_template", C.c_int32),
-                ("pole_extraction", C.c_int32)]
+                ("pole_extraction", C.c_int32), ("strategy", C.c_int32)]
 
 
 class qmc_result(C.Structure):
@@ -194,7 +194,7 @@ class Tables:
 def qmc_prepare(wl=None, *, n_vertices=None, edges=None, leg_vertex=None, gram=None, eps_order: int = 0,
                 lam: float = 0.0, transform: int = 0, max_depth: int = 0, lattice: int = 0, slot_budget: int = 0,
                 chunk_bytes: int = 0, threads: int = 0, slot_budget_cplx_real: int = 0, slot_budget_cplx: int = 0,
-                dense_template: int = 0, nu=None, pole_extraction: int = 0) -> Tables:
+                dense_template: int = 0, nu=None, pole_extraction: int = 0, strategy: int = 0) -> Tables:
     """qmc_prepare(graph, kinematics, eps_order) -> sector tables.  `wl` is a qmc_inputs.Workload, or pass the
     graph explicitly (edges = [(u, v, m^2), ...]).  slot_budget .. slot_budget_cplx are the table-layout fields of
     qmc_options (0 = the library's defaults).  nu: propagator powers, one per edge (qmc_graph.edge_nu; None = all 1).
@@ -215,7 +215,7 @@ def qmc_prepare(wl=None, *, n_vertices=None, edges=None, leg_vertex=None, gram=N
                   None if nu_arr is None else _ptr(nu_arr, C.c_int32), _ptr(lv, C.c_int32))
     k = qmc_kinematics(_ptr(gr, C.c_double))
     o = qmc_options(lam, transform, max_depth, lattice, slot_budget, chunk_bytes, threads, slot_budget_cplx_real,
-                    slot_budget_cplx, dense_template, pole_extraction)
+                    slot_budget_cplx, dense_template, pole_extraction, strategy)
     h = C.c_void_p()
     rc = lib().qmc_prepare(C.byref(g), C.byref(k), eps_order, C.byref(o), C.byref(h))
     if rc:
@@ -225,7 +225,7 @@ def qmc_prepare(wl=None, *, n_vertices=None, edges=None, leg_vertex=None, gram=N
 
 def qmc_prepare_batch(wls, *, eps_order: int = 0, lam: float = 0.0, transform: int = 0, max_depth: int = 0, lattice: int = 0,
                       slot_budget: int = 0, chunk_bytes: int = 0, threads: int = 0, slot_budget_cplx_real: int = 0,
-                      slot_budget_cplx: int = 0, dense_template: int = 0, nu=None, pole_extraction: int = 0) -> Tables:
+                      slot_budget_cplx: int = 0, dense_template: int = 0, nu=None, pole_extraction: int = 0, strategy: int = 0) -> Tables:
     """qmc_prepare_batch: ONE graph (taken from wls[0]) at the kinematic points of the workloads `wls` (their Gram matrices).
     Integrate with qmc_integrate(..., mode=3): results per kinematic point.  nu, pole_extraction: as in qmc_prepare (such
     tables run on the generic kernel, which has no mode 3: integrate them per point)."""
@@ -246,7 +246,7 @@ def qmc_prepare_batch(wls, *, eps_order: int = 0, lam: float = 0.0, transform: i
                   None if nu_arr is None else _ptr(nu_arr, C.c_int32), _ptr(lv, C.c_int32))
     kins = (qmc_kinematics * len(wls))(*[qmc_kinematics(_ptr(gr, C.c_double)) for gr in grams])
     o = qmc_options(lam, transform, max_depth, lattice, slot_budget, chunk_bytes, threads, slot_budget_cplx_real,
-                    slot_budget_cplx, dense_template, pole_extraction)
+                    slot_budget_cplx, dense_template, pole_extraction, strategy)
     h = C.c_void_p()
     rc = lib().qmc_prepare_batch(C.byref(g), kins, len(wls), eps_order, C.byref(o), C.byref(h))
     if rc:

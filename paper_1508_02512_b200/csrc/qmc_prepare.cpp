@@ -5,6 +5,7 @@
 // 4 bits per variable; U comes from a deletion-contraction recursion, F from U of the graphs with two leg
 // vertices identified; the decomposition runs on an explicit stack.
 #include <algorithm>
+#include <array>
 #include <cmath>
 #include <cstring>
 
@@ -73,6 +74,8 @@ struct Node {  // one (sub-)sector under construction
   Poly U, F;
   int alpha[QMC_MAXDIM], beta[QMC_MAXDIM];
   int depth;
+  long long weight = 1;  // geometric strategy: |det V| of the cone's substitution (must be 1)
+  bool final = false;    // geometric strategy: the substitution is complete, nothing left to split
 };
 
 bool constant_term(const Poly &p) { return !p.empty() && p.front().k == 0; }  // sorted: key 0 first
@@ -123,6 +126,234 @@ unsigned smallest_hitting_set(const Poly &target, int n) {
     }
   }
   return best;
+}
+
+// ---- geometric decomposition strategy (the strategy the paper says it uses, refs [25, 26]) ------
+// Kaneko-Ueda: for a primary sector with polynomials U_l, F_l in t_1..t_n, the Newton polyhedron of P = U_l F_l,
+//   Delta = conv{exponent vectors of P} + R^n_{>=0},
+// has facets with inward primitive integer normals v >= 0.  The normal cones of its vertices tile the orthant x = -ln t >= 0.
+// Every cone is cut into simplicial cones with generators v_1..v_n (rows of V); on such a cone the monomial substitution
+//   t_j = prod_k y_k^(v_kj),  y in (0,1]^n,   d^n t prod_j t_j^(a_j) = |det V| prod_k y_k^(<v_k, a+1> - 1) d^n y
+// turns every monomial t^e into y^(V e), and both polynomials into a monomial times a polynomial with a constant term
+// (the minimum of <v_k, e> over a polynomial's monomials is attained at ONE monomial for all k: the vertex).  One step, no
+// iteration, termination guaranteed.  A cone with |det V| > 1 would put a constant factor on its sector, which the tables
+// do not carry: QMC_EUNSUPPORTED (none was met: on every graph tried all cones are unimodular, reading C31).
+// Facets are found by testing the primitive vectors with entries 0..B: v is a facet normal iff the points where <v, e> is
+// minimal, together with the free directions e_j (v_j = 0), span an affine set of dimension n-1.  Completeness is CHECKED, not
+// assumed: the simplicial cones must tile the orthant, sum |det V| / prod_k <v_k, 1> = 1 (the integral of the Jacobian alone);
+// if they do not, B is raised, and beyond B = 5 the call fails (QMC_EDEPTH) rather than return a partial decomposition.
+typedef std::array<int, QMC_MAXDIM> IVec;
+
+long long det_exact(int n, std::vector<std::array<long long, QMC_MAXDIM>> M) {  // fraction-free (Bareiss) elimination
+  long long prev = 1, sign = 1;
+  for (int k = 0; k < n; ++k) {
+    int piv = -1;
+    for (int i = k; i < n; ++i)
+      if (M[i][k] != 0) {
+        piv = i;
+        break;
+      }
+    if (piv < 0) return 0;
+    if (piv != k) {
+      std::swap(M[piv], M[k]);
+      sign = -sign;
+    }
+    for (int i = k + 1; i < n; ++i)
+      for (int j = k + 1; j < n; ++j) M[i][j] = (M[i][j] * M[k][k] - M[i][k] * M[k][j]) / prev;
+    prev = M[k][k];
+  }
+  return sign * M[n - 1][n - 1];
+}
+
+int rank_exact(int n, std::vector<std::array<long long, QMC_MAXDIM>> M) {  // integer row reduction, rows kept primitive
+  int rank = 0;
+  for (int col = 0; col < n && rank < (int)M.size(); ++col) {
+    int piv = -1;
+    for (size_t i = rank; i < M.size(); ++i)
+      if (M[i][col] != 0) {
+        piv = (int)i;
+        break;
+      }
+    if (piv < 0) continue;
+    std::swap(M[piv], M[rank]);
+    for (size_t i = rank + 1; i < M.size(); ++i) {
+      if (M[i][col] == 0) continue;
+      const long long a = M[rank][col], b = M[i][col];
+      long long g = 0;
+      for (int j = 0; j < n; ++j) {
+        M[i][j] = M[i][j] * a - M[rank][j] * b;
+        g = std::__gcd(g, M[i][j] < 0 ? -M[i][j] : M[i][j]);
+      }
+      if (g > 1)
+        for (int j = 0; j < n; ++j) M[i][j] /= g;
+    }
+    ++rank;
+  }
+  return rank;
+}
+
+struct GeoCone {
+  IVec v[QMC_MAXDIM];  // generators (rows)
+  long long weight;    // |det V|
+};
+
+// simplicial cones of the normal fan of the Newton polyhedron of U * F (n variables); QMC_EDEPTH if they do not tile the orthant
+int geometric_cones(const Poly &U, const Poly &F, int n, std::vector<GeoCone> &out) {
+  std::vector<IVec> supp;  // exponent vectors of the product (Minkowski sum of the supports)
+  {
+    std::vector<Key> keys;
+    for (const Term &a : U)
+      for (const Term &b : F) keys.push_back(a.k + b.k);  // (4-bit fields: exponents of a product of two graph polynomials stay below 16)
+    std::sort(keys.begin(), keys.end());
+    keys.erase(std::unique(keys.begin(), keys.end()), keys.end());
+    for (Key k : keys) {
+      IVec e{};
+      for (int j = 0; j < n; ++j) e[j] = expo(k, j);
+      supp.push_back(e);
+    }
+  }
+  if (supp.empty()) return QMC_EINVAL;
+  for (int B = 2; B <= 5; ++B) {
+    // facets
+    std::vector<IVec> normal;
+    std::vector<int> level;
+    IVec v{};
+    long long ncand = 1;
+    for (int j = 0; j < n; ++j) ncand *= B + 1;
+    for (long long code = 1; code < ncand; ++code) {
+      long long c = code;
+      int g = 0;
+      for (int j = 0; j < n; ++j) {
+        v[j] = (int)(c % (B + 1));
+        c /= B + 1;
+        g = std::__gcd(g, v[j]);
+      }
+      if (g != 1) continue;
+      int m = 1 << 30;
+      for (const IVec &e : supp) {
+        int d = 0;
+        for (int j = 0; j < n; ++j) d += v[j] * e[j];
+        m = std::min(m, d);
+      }
+      std::vector<std::array<long long, QMC_MAXDIM>> rows;
+      const IVec *first = nullptr;
+      for (const IVec &e : supp) {
+        int d = 0;
+        for (int j = 0; j < n; ++j) d += v[j] * e[j];
+        if (d != m) continue;
+        if (!first) {
+          first = &e;
+          continue;
+        }
+        std::array<long long, QMC_MAXDIM> r{};
+        for (int j = 0; j < n; ++j) r[j] = e[j] - (*first)[j];
+        rows.push_back(r);
+      }
+      for (int j = 0; j < n; ++j)
+        if (v[j] == 0) {
+          std::array<long long, QMC_MAXDIM> r{};
+          r[j] = 1;
+          rows.push_back(r);
+        }
+      if ((int)rows.size() < n - 1 || rank_exact(n, rows) != n - 1) continue;
+      normal.push_back(v);
+      level.push_back(m);
+    }
+    // vertices and their normal cones
+    std::vector<GeoCone> cones;
+    bool ok = true;
+    for (const IVec &e : supp) {
+      std::vector<int> gens;
+      for (size_t f = 0; f < normal.size(); ++f) {
+        int d = 0;
+        for (int j = 0; j < n; ++j) d += normal[f][j] * e[j];
+        if (d == level[f]) gens.push_back((int)f);
+      }
+      if ((int)gens.size() < n) continue;
+      std::vector<std::array<long long, QMC_MAXDIM>> rows;
+      for (int f : gens) {
+        std::array<long long, QMC_MAXDIM> r{};
+        for (int j = 0; j < n; ++j) r[j] = normal[f][j];
+        rows.push_back(r);
+      }
+      if (rank_exact(n, rows) != n) continue;  // not a vertex
+      // placing triangulation of cone{normal[g] : g in gens}: start from n independent generators, then add the others; a
+      // new generator is joined to every boundary facet of the cone built so far that it sees from outside
+      auto detof = [&](const std::vector<int> &idx) {
+        std::vector<std::array<long long, QMC_MAXDIM>> M;
+        for (int f : idx) {
+          std::array<long long, QMC_MAXDIM> r{};
+          for (int j = 0; j < n; ++j) r[j] = normal[f][j];
+          M.push_back(r);
+        }
+        return det_exact(n, M);
+      };
+      std::vector<int> start, rest;
+      {
+        std::vector<std::array<long long, QMC_MAXDIM>> acc;
+        for (int f : gens) {
+          std::array<long long, QMC_MAXDIM> r{};
+          for (int j = 0; j < n; ++j) r[j] = normal[f][j];
+          acc.push_back(r);
+          if ((int)start.size() < n && rank_exact(n, acc) == (int)acc.size())
+            start.push_back(f);
+          else {
+            acc.pop_back();
+            rest.push_back(f);
+          }
+        }
+      }
+      std::vector<std::vector<int>> simp{start};
+      for (int g : rest) {
+        std::vector<std::vector<int>> add;
+        for (size_t si = 0; si < simp.size(); ++si)
+          for (int k = 0; k < n; ++k) {
+            std::vector<int> face;
+            for (int q = 0; q < n; ++q)
+              if (q != k) face.push_back(simp[si][q]);
+            std::vector<int> key = face;
+            std::sort(key.begin(), key.end());
+            int shared = 0;  // a boundary facet belongs to exactly one simplex
+            for (size_t sj = 0; sj < simp.size(); ++sj) {
+              std::vector<int> o = simp[sj];
+              std::sort(o.begin(), o.end());
+              if (std::includes(o.begin(), o.end(), key.begin(), key.end())) ++shared;
+            }
+            if (shared != 1) continue;
+            std::vector<int> with_u = face, with_g = face;
+            with_u.push_back(simp[si][k]);
+            with_g.push_back(g);
+            const long long du = detof(with_u), dg = detof(with_g);
+            if ((du > 0 && dg < 0) || (du < 0 && dg > 0)) add.push_back(with_g);
+          }
+        for (auto &s : add) simp.push_back(s);
+      }
+      for (auto &s : simp) {
+        GeoCone c;
+        for (int k = 0; k < n; ++k) c.v[k] = normal[s[k]];
+        const long long d = detof(s);
+        c.weight = d < 0 ? -d : d;
+        if (c.weight == 0) ok = false;
+        cones.push_back(c);
+      }
+    }
+    // the cones must tile the orthant: sum |det V| / prod_k <v_k, 1> = 1
+    double tile = 0.0;
+    for (const GeoCone &c : cones) {
+      double den = 1.0;
+      for (int k = 0; k < n; ++k) {
+        int sum = 0;
+        for (int j = 0; j < n; ++j) sum += c.v[k][j];
+        den *= sum;
+      }
+      tile += (double)c.weight / den;
+    }
+    if (ok && std::fabs(tile - 1.0) < 1e-9) {
+      out = cones;
+      return QMC_OK;
+    }
+  }
+  return QMC_EDEPTH;
 }
 
 }  // namespace
@@ -209,6 +440,8 @@ static int qmc_build_sectors(const qmc_graph *g, const qmc_kinematics *kin, int 
     T->ibp = T->has_taylor = T->generic_only = true;
   }
   const int max_depth = (opt && opt->max_depth > 0) ? opt->max_depth : 64;
+  const int strategy = opt ? opt->strategy : 0;  // 0: iterated (rule R:C7), 1: geometric (Kaneko-Ueda)
+  if (strategy != 0 && strategy != 1) return QMC_EINVAL;
   const int n = T->n;
   T->kmax = eps_order;
 
@@ -233,7 +466,63 @@ static int qmc_build_sectors(const qmc_graph *g, const qmc_kinematics *kin, int 
       }
       canonical(R);
     }
-    stack.push_back(nd);
+    if (strategy == 0) {
+      stack.push_back(nd);
+      continue;
+    }
+    // geometric strategy: one monomial substitution per simplicial cone of the normal fan, pushed in reverse so that the
+    // cones of a primary sector come out in the order geometric_cones found them
+    std::vector<GeoCone> cones;
+    const int rcg = geometric_cones(nd.U, nd.F, n, cones);
+    if (rcg != QMC_OK) return rcg;
+    for (size_t ci = cones.size(); ci-- > 0;) {
+      const GeoCone &cn = cones[ci];
+      Node ch;
+      ch.primary = l;
+      ch.depth = 1;
+      ch.final = true;
+      ch.weight = cn.weight;
+      std::memset(ch.alpha, 0, sizeof ch.alpha);
+      std::memset(ch.beta, 0, sizeof ch.beta);
+      for (int k = 0; k < n; ++k) {  // y_k^(<v_k, alpha + 1> - 1 + eps <v_k, beta>)
+        int a = -1, b = 0;
+        for (int j = 0; j < n; ++j) {
+          a += cn.v[k][j] * (nd.alpha[j] + 1);
+          b += cn.v[k][j] * nd.beta[j];
+        }
+        ch.alpha[k] = a;
+        ch.beta[k] = b;
+      }
+      for (int which = 0; which < 2; ++which) {
+        const Poly &Q = which ? nd.F : nd.U;
+        Poly &R = which ? ch.F : ch.U;
+        std::vector<IVec> ex(Q.size());
+        IVec lo;
+        lo.fill(1 << 30);
+        for (size_t q = 0; q < Q.size(); ++q)
+          for (int k = 0; k < n; ++k) {
+            int d = 0;
+            for (int j = 0; j < n; ++j) d += cn.v[k][j] * expo(Q[q].k, j);
+            ex[q][k] = d;
+            lo[k] = std::min(lo[k], d);
+          }
+        const int a0 = which ? T->aF0 : T->aU0, a1 = which ? T->aF1 : T->aU1;
+        for (int k = 0; k < n; ++k) {  // the common monomial y^lo goes to the exponents at once (the keys hold 4 bits per variable)
+          ch.alpha[k] += lo[k] * a0;
+          ch.beta[k] += lo[k] * a1;
+        }
+        for (size_t q = 0; q < Q.size(); ++q) {
+          Key key = 0;
+          for (int k = 0; k < n; ++k) {
+            if (ex[q][k] - lo[k] > 15) return QMC_EUNSUPPORTED;
+            key += (Key)(ex[q][k] - lo[k]) << (4 * k);
+          }
+          R.push_back(Term{key, Q[q].c});
+        }
+        canonical(R);
+      }
+      stack.push_back(ch);
+    }
   }
   int smax = -T->kmin;  // (a batch appends the sectors of several kinematic points: kmin = the most negative of all)
   while (!stack.empty()) {
@@ -242,9 +531,11 @@ static int qmc_build_sectors(const qmc_graph *g, const qmc_kinematics *kin, int 
     pull_common(nd.U, n, T->aU0, T->aU1, nd.alpha, nd.beta);
     pull_common(nd.F, n, T->aF0, T->aF1, nd.alpha, nd.beta);
     const Poly *target = !constant_term(nd.U) ? &nd.U : (!constant_term(nd.F) ? &nd.F : nullptr);
+    if (target && nd.final) return QMC_EDEPTH;  // (cannot happen when the cones tile the orthant: checked in geometric_cones)
     if (!target) {  // emit
       QmcSector s;
       s.primary = nd.primary;
+      if (nd.weight != 1) return QMC_EUNSUPPORTED;  // a non-unimodular cone (|det V| > 1) would need a constant factor per sector: R:C31
       s.nsing = 0;
       s.ndeep = 0;
       std::memset(s.alpha, 0, sizeof s.alpha);
