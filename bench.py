@@ -303,6 +303,27 @@ def pole_extraction_comparison(q, dev):
     return out
 
 
+def strategy_comparison(q, dev):
+    """SURVEY 8(f) f3 (not part of the timed path, whose config says "iterated"): the geometric decomposition strategy
+    (qmc_options.strategy = 1, reading C31) against the iterated rule on the same lattice and shifts: sectors, kernel
+    time of a step, error estimate of the finite part, and the difference of the two totals in units of their combined error."""
+    out = []
+    for wl, N in ((qi.double_box(), 999983), (qi.nonplanar_vertex(), 1048573)):
+        res = []
+        for st in (0, 1):
+            t = q.qmc_prepare(wl, eps_order=wl.eps_order, lam=wl.lam, strategy=st)
+            q.qmc_integrate(t, N, wl.m, seed=wl.seed, device=dev)
+            r = q.qmc_integrate(t, N, wl.m, seed=wl.seed, device=dev)
+            res.append((t.n_sectors, r))
+        (n0, r0), (n1, r1) = res
+        comb = np.maximum(np.hypot(np.abs(r0.err.real), np.abs(r1.err.real)), 1e-300)
+        out.append({"workload": wl.name, "N": N, "m": wl.m, "sectors": [n0, n1],
+                    "eval_kernel_ms": [float(r0.eval_kernel_ms), float(r1.eval_kernel_ms)],
+                    "err_finite_part": [float(abs(r0.err[-1].real)), float(abs(r1.err[-1].real))],
+                    "difference_in_sigma": [float(x) for x in np.abs(r0.coeff.real - r1.coeff.real) / comb]})
+    return out
+
+
 def per_sector_mode(q, t, N, m, z, shifts, dev, torch):
     """the per-sector (parity) mode of the kernel next to the fused (throughput) mode the headline times."""
     q.qmc_integrate(t, N, m, z=z, shifts=shifts, per_sector=True, device=dev)
@@ -522,6 +543,7 @@ def run_product(args):
         line["other_workloads"] = extra(other_workloads, q, torch, dev, args.config)
         line["kinematic_scan"] = extra(kinematic_scan, q, torch)
         line["pole_extraction"] = extra(pole_extraction_comparison, q, dev)
+        line["strategy_comparison"] = extra(strategy_comparison, q, dev)
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -143,6 +143,9 @@ unsigned smallest_hitting_set(const Poly &target, int n) {
 // assumed: the simplicial cones must tile the orthant, sum |det V| / prod_k <v_k, 1> = 1 (the integral of the Jacobian alone);
 // if they do not, B is raised, and beyond B = 5 the call fails (QMC_EDEPTH) rather than return a partial decomposition.
 typedef std::array<int, QMC_MAXDIM> IVec;
+#ifndef QMC_GEO_ORDERS
+#define QMC_GEO_ORDERS 24  // generator orders tried per non-simplicial cone
+#endif
 
 long long det_exact(int n, std::vector<std::array<long long, QMC_MAXDIM>> M) {  // fraction-free (Bareiss) elimination
   long long prev = 1, sign = 1;
@@ -288,6 +291,23 @@ int geometric_cones(const Poly &U, const Poly &F, int n, std::vector<GeoCone> &o
         }
         return det_exact(n, M);
       };
+      // The triangulation depends on the order of the generators; a few deterministic orders are tried (as found, reversed,
+      // rotations, a fixed multiplicative shuffle) and the one with the fewest simplices is kept: fewer sectors, same integral.
+      std::vector<std::vector<int>> best;
+      const std::vector<int> gens0 = gens;
+      const int ntry = (int)gens0.size() > n ? QMC_GEO_ORDERS : 1;
+      for (int attempt = 0; attempt < ntry; ++attempt) {
+      gens = gens0;
+      const int m = (int)gens0.size();
+      if (attempt == 1) std::reverse(gens.begin(), gens.end());
+      if (attempt >= 2 && attempt < 2 + m) std::rotate(gens.begin(), gens.begin() + (attempt - 2) % m, gens.end());
+      if (attempt >= 2 + m) {
+        unsigned long long st = 0x9E3779B97F4A7C15ull * (unsigned long long)(attempt + 1);
+        for (int i = m - 1; i > 0; --i) {
+          st = st * 6364136223846793005ull + 1442695040888963407ull;
+          std::swap(gens[i], gens[(int)((st >> 33) % (unsigned long long)(i + 1))]);
+        }
+      }
       std::vector<int> start, rest;
       {
         std::vector<std::array<long long, QMC_MAXDIM>> acc;
@@ -328,7 +348,9 @@ int geometric_cones(const Poly &U, const Poly &F, int n, std::vector<GeoCone> &o
           }
         for (auto &s : add) simp.push_back(s);
       }
-      for (auto &s : simp) {
+      if (best.empty() || simp.size() < best.size()) best = simp;
+      }  // attempts
+      for (auto &s : best) {
         GeoCone c;
         for (int k = 0; k < n; ++k) c.v[k] = normal[s[k]];
         const long long d = detof(s);
