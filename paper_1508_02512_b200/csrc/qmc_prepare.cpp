@@ -146,8 +146,15 @@ typedef std::array<int, QMC_MAXDIM> IVec;
 #ifndef QMC_GEO_ORDERS
 #define QMC_GEO_ORDERS 24  // generator orders tried per non-simplicial cone
 #endif
+#define QMC_GEO_MAX_SIMPLICES 200u  // per vertex cone; beyond: QMC_EUNSUPPORTED (the double box needs at most a few per cone)
+
+// work done by one geometric_cones call (exact determinants and ranks): beyond QMC_GEO_MAX_WORK the call gives up (QMC_EUNSUPPORTED)
+// instead of running for minutes on polytopes with hundreds of vertices (a six-loop banana); the double box needs about 4e5
+thread_local long long geo_work = 0;
+#define QMC_GEO_MAX_WORK 20000000ll
 
 long long det_exact(int n, std::vector<std::array<long long, QMC_MAXDIM>> M) {  // fraction-free (Bareiss) elimination
+  geo_work += n * n;
   long long prev = 1, sign = 1;
   for (int k = 0; k < n; ++k) {
     int piv = -1;
@@ -169,6 +176,7 @@ long long det_exact(int n, std::vector<std::array<long long, QMC_MAXDIM>> M) {  
 }
 
 int rank_exact(int n, std::vector<std::array<long long, QMC_MAXDIM>> M) {  // integer row reduction, rows kept primitive
+  geo_work += (long long)n * (long long)M.size();
   int rank = 0;
   for (int col = 0; col < n && rank < (int)M.size(); ++col) {
     int piv = -1;
@@ -216,6 +224,7 @@ int geometric_cones(const Poly &U, const Poly &F, int n, std::vector<GeoCone> &o
     }
   }
   if (supp.empty()) return QMC_EINVAL;
+  geo_work = 0;
   for (int B = 2; B <= 5; ++B) {
     // facets
     std::vector<IVec> normal;
@@ -224,6 +233,7 @@ int geometric_cones(const Poly &U, const Poly &F, int n, std::vector<GeoCone> &o
     long long ncand = 1;
     for (int j = 0; j < n; ++j) ncand *= B + 1;
     for (long long code = 1; code < ncand; ++code) {
+      if (geo_work > QMC_GEO_MAX_WORK) return QMC_EUNSUPPORTED;
       long long c = code;
       int g = 0;
       for (int j = 0; j < n; ++j) {
@@ -266,6 +276,7 @@ int geometric_cones(const Poly &U, const Poly &F, int n, std::vector<GeoCone> &o
     std::vector<GeoCone> cones;
     bool ok = true;
     for (const IVec &e : supp) {
+      if (geo_work > QMC_GEO_MAX_WORK) return QMC_EUNSUPPORTED;
       std::vector<int> gens;
       for (size_t f = 0; f < normal.size(); ++f) {
         int d = 0;
@@ -294,9 +305,10 @@ int geometric_cones(const Poly &U, const Poly &F, int n, std::vector<GeoCone> &o
       // The triangulation depends on the order of the generators; a few deterministic orders are tried (as found, reversed,
       // rotations, a fixed multiplicative shuffle) and the one with the fewest simplices is kept: fewer sectors, same integral.
       std::vector<std::vector<int>> best;
+      bool too_big = false;
       const std::vector<int> gens0 = gens;
       const int ntry = (int)gens0.size() > n ? QMC_GEO_ORDERS : 1;
-      for (int attempt = 0; attempt < ntry; ++attempt) {
+      for (int attempt = 0; attempt < ntry && !too_big; ++attempt) {
       gens = gens0;
       const int m = (int)gens0.size();
       if (attempt == 1) std::reverse(gens.begin(), gens.end());
@@ -325,6 +337,7 @@ int geometric_cones(const Poly &U, const Poly &F, int n, std::vector<GeoCone> &o
       }
       std::vector<std::vector<int>> simp{start};
       for (int g : rest) {
+        if (geo_work > QMC_GEO_MAX_WORK) return QMC_EUNSUPPORTED;
         std::vector<std::vector<int>> add;
         for (size_t si = 0; si < simp.size(); ++si)
           for (int k = 0; k < n; ++k) {
@@ -333,6 +346,7 @@ int geometric_cones(const Poly &U, const Poly &F, int n, std::vector<GeoCone> &o
               if (q != k) face.push_back(simp[si][q]);
             std::vector<int> key = face;
             std::sort(key.begin(), key.end());
+            geo_work += (long long)simp.size() * n;
             int shared = 0;  // a boundary facet belongs to exactly one simplex
             for (size_t sj = 0; sj < simp.size(); ++sj) {
               std::vector<int> o = simp[sj];
@@ -347,9 +361,16 @@ int geometric_cones(const Poly &U, const Poly &F, int n, std::vector<GeoCone> &o
             if ((du > 0 && dg < 0) || (du < 0 && dg > 0)) add.push_back(with_g);
           }
         for (auto &s : add) simp.push_back(s);
+        if (simp.size() > QMC_GEO_MAX_SIMPLICES) break;  // (the boundary test above is cubic in the number of simplices)
+      }
+      if (simp.size() > QMC_GEO_MAX_SIMPLICES) {
+        if (attempt == 0) too_big = true;  // the first order already blows up: do not try 23 more
+        continue;
       }
       if (best.empty() || simp.size() < best.size()) best = simp;
+      if (too_big) break;
       }  // attempts
+      if (best.empty()) return QMC_EUNSUPPORTED;  // a cone that needs more than QMC_GEO_MAX_SIMPLICES simplices
       for (auto &s : best) {
         GeoCone c;
         for (int k = 0; k < n; ++k) c.v[k] = normal[s[k]];

@@ -87,3 +87,54 @@ def test_geometric_strategy_with_propagator_powers_and_other_options():
     with pytest.raises(q.QmcError) as err:
         q.qmc_prepare(qi.massless_box(), strategy=2)
     assert err.value.status == -1
+
+
+def test_random_graphs_either_decompose_into_the_form_of_eqs_7_to_9_or_fail_with_a_status():
+    """Robustness of the host code on inputs nobody chose: random connected multigraphs (2-5 vertices, up to 7 edges, up to six
+    loops), random masses, Euclidean momenta with some light-like legs, random propagator powers, both strategies and both pole
+    extractions.  Every call either returns tables whose sectors have the form of Eqs. 7-9 or a status (unsupported, depth cap);
+    the geometric strategy never runs into the depth cap (it does not iterate), and its work budget keeps a call short."""
+    import collections
+    import time
+    from qmc_inputs import Workload
+    rng = np.random.default_rng(7)
+    stat = collections.Counter()
+    t_begin = time.time()
+    for it in range(60):
+        V = int(rng.integers(2, 6)); P = int(rng.integers(max(V, 2), 8))
+        edges = [(int(rng.integers(0, v)), v) for v in range(1, V)]
+        while len(edges) < P:
+            a, b = int(rng.integers(0, V)), int(rng.integers(0, V))
+            if a != b or rng.random() < 0.05:
+                edges.append((a, b))
+        masses = [float(rng.choice([0.0, 0.0, 1.0, 2.5])) for _ in edges]
+        nl = int(rng.integers(2, min(V, 4) + 1))
+        legs = [int(x) for x in rng.choice(V, size=nl, replace=False)]
+        p = rng.normal(size=(nl, 4)); p[-1] = -p[:-1].sum(axis=0)
+        gram = -(p @ p.T)
+        if rng.random() < 0.3:
+            for i in range(nl):
+                if rng.random() < 0.5:
+                    gram[i, i] = 0.0
+        nu = None if rng.random() < 0.5 else [int(rng.choice([1, 1, 2, 3])) for _ in edges]
+        wl = Workload("random", V, [(a, b, m) for (a, b), m in zip(edges, masses)], legs, gram)
+        for strategy in (0, 1):
+            for pole in (0, 1):
+                t0 = time.time()
+                try:
+                    t = q.qmc_prepare(wl, eps_order=int(rng.integers(0, 3)), strategy=strategy, pole_extraction=pole, nu=nu, max_depth=12)
+                except q.QmcError as e:
+                    assert e.status in (-2, -3) and not (strategy == 1 and e.status == -2), (it, strategy, e.status)
+                    stat[("status", strategy, e.status)] += 1
+                    continue
+                finally:
+                    assert time.time() - t0 < 20.0, (it, strategy, "qmc_prepare took too long")
+                o = Oracle.from_tables(t.export())
+                for s in range(min(o.n_sectors, 30)):
+                    sec = o.sector(s)
+                    for which in "UF":
+                        coeff, expo = sec[which]
+                        assert (expo.sum(axis=1) == 0).sum() == 1 and np.all(expo.min(axis=0) == 0), (it, strategy, s, which)
+                stat[("tables", strategy)] += 1
+    assert stat[("tables", 0)] > 40 and stat[("tables", 1)] > 40, dict(stat)
+    assert time.time() - t_begin < 240.0
