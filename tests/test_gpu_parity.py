@@ -686,3 +686,56 @@ def test_geometric_decomposition_strategy():
     assert np.all(np.abs(rg.coeff.real[:3] - ex4) <= 4 * rg.err.real[:3]), (rg.coeff.real, rg.err.real)
     assert np.all(np.abs(rg.coeff.real - ri.coeff.real) <= 4 * np.hypot(rg.err.real, ri.err.real)), (rg.coeff.real, ri.coeff.real)
     assert np.all(rg.err.real <= 1e-4 * np.maximum(np.abs(rg.coeff.real), 1e-2))
+
+
+@pytest.mark.parametrize("physical", [False, True], ids=["euclidean", "physical"])
+def test_random_graphs_parity(physical):
+    """Inputs nobody chose: random connected multigraphs (2-5 vertices, up to 6 edges, up to five loops), random masses and
+    momenta, random propagator powers, both decomposition strategies, both pole extractions, random eps order, a random window
+    of eight sectors, a random Korobov vector: whatever qmc_prepare accepts must agree with the oracle per sector, order and
+    shift at the C19 tolerance, counters included -- on the table-driven kernels and on the generic one, as the tables decide.
+    (A case whose contour counters are non-zero is skipped: the deformation crossed the cut, the values sit on branch cuts.)"""
+    import collections
+    from qmc_inputs import Workload
+    rng = np.random.default_rng(11 if physical else 1)
+    stat = collections.Counter()
+    for it in range(40):
+        V = int(rng.integers(2, 6)); P = int(rng.integers(max(V, 2), 7))
+        edges = [(int(rng.integers(0, v)), v) for v in range(1, V)]
+        while len(edges) < P:
+            a, b = int(rng.integers(0, V)), int(rng.integers(0, V))
+            if a != b:
+                edges.append((a, b))
+        masses = [float(rng.choice([1.0, 2.5, 0.6] if physical else [0.0, 0.0, 1.0, 2.5])) for _ in edges]
+        nl = int(rng.integers(2, min(V, 4) + 1))
+        legs = [int(x) for x in rng.choice(V, size=nl, replace=False)]
+        p = rng.normal(size=(nl, 4)); p[-1] = -p[:-1].sum(axis=0)
+        gram = 6.0 * (p @ p.T) if physical else -(p @ p.T)
+        nu = None if rng.random() < 0.6 else [int(rng.choice([1, 1, 2])) for _ in edges]
+        lam = float(rng.choice([0.2, 0.5])) if physical else 0.0
+        wl = Workload("random", V, [(a, b, m) for (a, b), m in zip(edges, masses)], legs, gram, lam)
+        for strategy in (0, 1):
+            pole = int(rng.random() < 0.3) if lam == 0.0 else 0
+            eo = int(rng.integers(0, 2))
+            try:
+                t = q.qmc_prepare(wl, eps_order=eo, lam=lam, strategy=strategy, pole_extraction=pole, nu=nu, max_depth=10)
+            except q.QmcError as e:
+                assert e.status in (-2, -3)
+                stat["refused"] += 1
+                continue
+            o = Oracle.from_tables(t.export())
+            assert o.status == 0
+            N = 4093 if t.dim > 1 else 1021
+            z = qi.korobov_vector(N, t.dim, int(rng.integers(2, N - 1)))
+            sh = qi.splitmix64_shifts(int(rng.integers(1, 1000)), 2, t.dim)
+            s0 = int(rng.integers(0, max(1, t.n_sectors - 8))); s1 = min(t.n_sectors, s0 + 8)
+            r = q.qmc_integrate(t, N, 2, z=z, shifts=sh, sectors=(s0, s1), per_sector=True)
+            S, A, cnt = o.integrate(N, z, sh, sectors=(s0, s1))
+            assert np.array_equal(r.counters, cnt), (it, strategy, r.counters, cnt)
+            if cnt[0] or cnt[1]:
+                stat["contour counters"] += 1
+                continue
+            check(r.shift_sums, S, A, f"random graph {it} strategy {strategy} pole {pole} nu {nu} edges {edges}")
+            lines = t.describe().splitlines()
+            stat[lines[1].split()[0] if len(lines) > 1 else "generic"] += 1
+    assert stat["generic"] >= 10 and stat["complex" if physical else "chunk"] >= 10, dict(stat)
