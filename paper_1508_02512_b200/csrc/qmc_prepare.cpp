@@ -302,74 +302,75 @@ int geometric_cones(const Poly &U, const Poly &F, int n, std::vector<GeoCone> &o
         }
         return det_exact(n, M);
       };
-      // The triangulation depends on the order of the generators; a few deterministic orders are tried (as found, reversed,
-      // rotations, a fixed multiplicative shuffle) and the one with the fewest simplices is kept: fewer sectors, same integral.
-      std::vector<std::vector<int>> best;
-      bool too_big = false;
-      const std::vector<int> gens0 = gens;
-      const int ntry = (int)gens0.size() > n ? QMC_GEO_ORDERS : 1;
-      for (int attempt = 0; attempt < ntry && !too_big; ++attempt) {
-      gens = gens0;
-      const int m = (int)gens0.size();
-      if (attempt == 1) std::reverse(gens.begin(), gens.end());
-      if (attempt >= 2 && attempt < 2 + m) std::rotate(gens.begin(), gens.begin() + (attempt - 2) % m, gens.end());
-      if (attempt >= 2 + m) {
-        unsigned long long st = 0x9E3779B97F4A7C15ull * (unsigned long long)(attempt + 1);
-        for (int i = m - 1; i > 0; --i) {
-          st = st * 6364136223846793005ull + 1442695040888963407ull;
-          std::swap(gens[i], gens[(int)((st >> 33) % (unsigned long long)(i + 1))]);
-        }
-      }
-      std::vector<int> start, rest;
-      {
+      // Placing triangulation for one order of the generators: start from the first n independent ones, then join every further
+      // generator to the boundary facets of the cone built so far that it sees from outside.  Empty result: too many simplices.
+      auto triangulate = [&](const std::vector<int> &order) {
+        std::vector<int> start, rest;
         std::vector<std::array<long long, QMC_MAXDIM>> acc;
-        for (int f : gens) {
+        for (int f : order) {
           std::array<long long, QMC_MAXDIM> r{};
           for (int j = 0; j < n; ++j) r[j] = normal[f][j];
           acc.push_back(r);
-          if ((int)start.size() < n && rank_exact(n, acc) == (int)acc.size())
+          if ((int)start.size() < n && rank_exact(n, acc) == (int)acc.size()) {
             start.push_back(f);
-          else {
+          } else {
             acc.pop_back();
             rest.push_back(f);
           }
         }
-      }
-      std::vector<std::vector<int>> simp{start};
-      for (int g : rest) {
-        if (geo_work > QMC_GEO_MAX_WORK) return QMC_EUNSUPPORTED;
-        std::vector<std::vector<int>> add;
-        for (size_t si = 0; si < simp.size(); ++si)
-          for (int k = 0; k < n; ++k) {
-            std::vector<int> face;
-            for (int q = 0; q < n; ++q)
-              if (q != k) face.push_back(simp[si][q]);
-            std::vector<int> key = face;
-            std::sort(key.begin(), key.end());
-            geo_work += (long long)simp.size() * n;
-            int shared = 0;  // a boundary facet belongs to exactly one simplex
-            for (size_t sj = 0; sj < simp.size(); ++sj) {
-              std::vector<int> o = simp[sj];
-              std::sort(o.begin(), o.end());
-              if (std::includes(o.begin(), o.end(), key.begin(), key.end())) ++shared;
+        std::vector<std::vector<int>> simp{start};
+        for (int g : rest) {
+          if (geo_work > QMC_GEO_MAX_WORK) return std::vector<std::vector<int>>();
+          std::vector<std::vector<int>> add;
+          for (size_t si = 0; si < simp.size(); ++si)
+            for (int k = 0; k < n; ++k) {
+              std::vector<int> face;
+              for (int q = 0; q < n; ++q)
+                if (q != k) face.push_back(simp[si][q]);
+              std::vector<int> key = face;
+              std::sort(key.begin(), key.end());
+              geo_work += (long long)simp.size() * n;
+              int shared = 0;  // a boundary facet belongs to exactly one simplex
+              for (size_t sj = 0; sj < simp.size(); ++sj) {
+                std::vector<int> o = simp[sj];
+                std::sort(o.begin(), o.end());
+                if (std::includes(o.begin(), o.end(), key.begin(), key.end())) ++shared;
+              }
+              if (shared != 1) continue;
+              std::vector<int> with_u = face, with_g = face;
+              with_u.push_back(simp[si][k]);
+              with_g.push_back(g);
+              const long long du = detof(with_u), dg = detof(with_g);
+              if ((du > 0 && dg < 0) || (du < 0 && dg > 0)) add.push_back(with_g);
             }
-            if (shared != 1) continue;
-            std::vector<int> with_u = face, with_g = face;
-            with_u.push_back(simp[si][k]);
-            with_g.push_back(g);
-            const long long du = detof(with_u), dg = detof(with_g);
-            if ((du > 0 && dg < 0) || (du < 0 && dg > 0)) add.push_back(with_g);
+          for (auto &sx : add) simp.push_back(sx);
+          if (simp.size() > QMC_GEO_MAX_SIMPLICES) return std::vector<std::vector<int>>();  // (the boundary test is cubic in their number)
+        }
+        return simp;
+      };
+      // The triangulation depends on the order of the generators: a few deterministic orders are tried (as found, reversed,
+      // rotations, fixed shuffles) and the one with the fewest simplices is kept -- fewer sectors, same integral.  If the first
+      // order already needs too many simplices the others are not tried.
+      std::vector<std::vector<int>> best;
+      const int m = (int)gens.size(), ntry = m > n ? QMC_GEO_ORDERS : 1;
+      for (int attempt = 0; attempt < ntry; ++attempt) {
+        std::vector<int> order = gens;
+        if (attempt == 1) std::reverse(order.begin(), order.end());
+        if (attempt >= 2 && attempt < 2 + m) std::rotate(order.begin(), order.begin() + (attempt - 2) % m, order.end());
+        if (attempt >= 2 + m) {
+          unsigned long long st = 0x9E3779B97F4A7C15ull * (unsigned long long)(attempt + 1);
+          for (int i = m - 1; i > 0; --i) {
+            st = st * 6364136223846793005ull + 1442695040888963407ull;
+            std::swap(order[i], order[(int)((st >> 33) % (unsigned long long)(i + 1))]);
           }
-        for (auto &s : add) simp.push_back(s);
-        if (simp.size() > QMC_GEO_MAX_SIMPLICES) break;  // (the boundary test above is cubic in the number of simplices)
+        }
+        const std::vector<std::vector<int>> simp = triangulate(order);
+        if (simp.empty()) {
+          if (attempt == 0) break;
+          continue;
+        }
+        if (best.empty() || simp.size() < best.size()) best = simp;
       }
-      if (simp.size() > QMC_GEO_MAX_SIMPLICES) {
-        if (attempt == 0) too_big = true;  // the first order already blows up: do not try 23 more
-        continue;
-      }
-      if (best.empty() || simp.size() < best.size()) best = simp;
-      if (too_big) break;
-      }  // attempts
       if (best.empty()) return QMC_EUNSUPPORTED;  // a cone that needs more than QMC_GEO_MAX_SIMPLICES simplices
       for (auto &s : best) {
         GeoCone c;
