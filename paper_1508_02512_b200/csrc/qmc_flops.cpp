@@ -34,6 +34,9 @@ extern "C" int qmc_flop_model(const qmc_tables *t, int32_t sector_begin, int32_t
   const int sb = sector_begin, se = sector_end > 0 ? sector_end : nsec;
   if (sb < 0 || se > nsec || sb >= se) return QMC_EINVAL;
   const bool cplx = t->lambda > 0.0;
+  // Tables that only the generic kernel runs (propagator powers, sectors with alpha <= -2, integration by parts: t->generic_only)
+  // are counted with the scheme of the table-driven kernels and every variable with alpha <= -1 as a singular one: a lower bound
+  // of what their slow paths (power-series arithmetic) execute.  No reported number uses the model on such tables.
   // S1-S3, once per (point, shift): u = r/N (IEEE division), y = u + Delta (wrap), t = y^2 (3 - 2y), w *= 6 y (1 - y),
   // ln t (table logarithm)
   // (r / N as r * RN(1/N) with one FMA correction, 5 flops, on both paths)
